@@ -1,0 +1,132 @@
+"""Physics-level pins for the oracle: Sod shock tube against the exact Riemann solution (PAPER.md
+§5.1.2) and second-order convergence on the stationary isentropic vortex (§5.2.1).
+The exact Riemann solver below is the textbook construction (two-shock/rarefaction pressure
+function, Newton iteration), independent of the oracle."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+GAMMA = 1.4
+
+
+def exact_riemann(rl, ul, pl, rr, ur, pr, xi, g=GAMMA):
+    """Exact solution of the 1D Riemann problem sampled at xi = (x - x0)/t."""
+    cl, cr = np.sqrt(g * pl / rl), np.sqrt(g * pr / rr)
+
+    def f(p, r, pk, c):
+        if p > pk:   # shock
+            A, B = 2 / ((g + 1) * r), (g - 1) / (g + 1) * pk
+            return (p - pk) * np.sqrt(A / (p + B)), np.sqrt(A / (p + B)) * (1 - 0.5 * (p - pk) / (p + B))
+        return 2 * c / (g - 1) * ((p / pk) ** ((g - 1) / (2 * g)) - 1), 1 / (r * c) * (p / pk) ** (-(g + 1) / (2 * g))
+
+    p = 0.5 * (pl + pr)
+    for _ in range(100):
+        fl, dfl = f(p, rl, pl, cl)
+        fr, dfr = f(p, rr, pr, cr)
+        dp = (fl + fr + ur - ul) / (dfl + dfr)
+        p = max(p - dp, 1e-12)
+        if abs(dp) < 1e-15 * p:
+            break
+    us = 0.5 * (ul + ur) + 0.5 * (f(p, rr, pr, cr)[0] - f(p, rl, pl, cl)[0])
+    rho = np.empty_like(xi)
+    # left of the contact
+    if p > pl:
+        rsl = rl * ((p / pl + (g - 1) / (g + 1)) / ((g - 1) / (g + 1) * p / pl + 1))
+        sl = ul - cl * np.sqrt((g + 1) / (2 * g) * p / pl + (g - 1) / (2 * g))
+        left = np.where(xi < sl, rl, rsl)
+    else:
+        rsl = rl * (p / pl) ** (1 / g)
+        csl = cl * (p / pl) ** ((g - 1) / (2 * g))
+        head, tail = ul - cl, us - csl
+        fan = rl * (2 / (g + 1) + (g - 1) / ((g + 1) * cl) * (ul - xi)) ** (2 / (g - 1))
+        left = np.where(xi < head, rl, np.where(xi < tail, fan, rsl))
+    if p > pr:
+        rsr = rr * ((p / pr + (g - 1) / (g + 1)) / ((g - 1) / (g + 1) * p / pr + 1))
+        sr = ur + cr * np.sqrt((g + 1) / (2 * g) * p / pr + (g - 1) / (2 * g))
+        right = np.where(xi > sr, rr, rsr)
+    else:
+        rsr = rr * (p / pr) ** (1 / g)
+        csr = cr * (p / pr) ** ((g - 1) / (2 * g))
+        head, tail = ur + cr, us + csr
+        fan = rr * (2 / (g + 1) - (g - 1) / ((g + 1) * cr) * (ur - xi)) ** (2 / (g - 1))
+        right = np.where(xi > head, rr, np.where(xi > tail, fan, rsr))
+    rho = np.where(xi < us, left, right)
+    return rho, p, us
+
+
+def test_exact_solver_reproduces_the_standard_sod_star_state():
+    # standard values for Sod's problem, gamma = 1.4 (also listed in SURVEY.md §8c)
+    xi = np.array([-2.0, 0.0, 1.2, 3.0])
+    rho, ps, us = exact_riemann(1.0, 0.0, 1.0, 0.125, 0.0, 0.1, xi)
+    assert abs(ps - 0.303130) < 2e-6 and abs(us - 0.927453) < 2e-6
+    assert abs(rho[1] - 0.426319) < 2e-6 and abs(rho[2] - 0.265574) < 2e-6
+    assert rho[0] == 1.0 and rho[3] == 0.125
+
+
+def run_sod(n, scheme, order):
+    cfg = wl.make_config("sod", n=n)
+    m = cfg.mesh
+    om = oracle.OracleMesh(m.xy, m.tri, vertex_flag=cfg.vertex_flag, wall_edge=cfg.wall_edge,
+                           scheme=scheme, time_order=order, threads=4)
+    om.set_state(cfg.W0)
+    om.step(100000, t_end=0.2)
+    W = om.get_state().reshape(4, m.shape[1], m.shape[0])
+    x = m.xy[:, 0].reshape(m.shape[1], m.shape[0])[0]
+    return x, W
+
+
+@pytest.mark.slow
+def test_sod_against_exact_riemann_solution():
+    errs = {}
+    for n in (64, 128, 256):
+        x, W = run_sod(n, oracle.SCHEME_B, 2)
+        exact, _, _ = exact_riemann(1.0, 0.0, 1.0, 0.125, 0.0, 0.1, (x - 0.5) / 0.2)
+        errs[n] = np.mean(np.abs(W[0] - exact))             # eq. 72 on a uniform mesh, all rows
+        # The tube is only approximately y-independent: the diagonal split is not mirror-symmetric in y
+        # and wall vertices have half cells, so a transverse velocity appears at the shock. The rows
+        # must still agree with each other much better than with the exact solution.
+        assert np.mean(np.abs(W[0] - W[0, W.shape[1] // 2])) < 0.25 * errs[n]
+    # sub-linear but steady convergence (L800: between sqrt(h) and h), and a small error at 256
+    assert errs[128] < 0.8 * errs[64] and errs[256] < 0.8 * errs[128]
+    assert errs[256] < 6e-3
+    # first-order N scheme: monotone, no new extrema (L792)
+    x, W = run_sod(128, oracle.SCHEME_N, 1)
+    rho = W[0, W.shape[1] // 2]
+    assert W[0].max() <= 1.0 + 1e-12 and W[0].min() >= 0.125 - 1e-12
+    assert np.all(np.diff(rho) <= 1e-3)
+    exact, _, _ = exact_riemann(1.0, 0.0, 1.0, 0.125, 0.0, 0.1, (x - 0.5) / 0.2)
+    assert np.mean(np.abs(rho - exact)) < 2.5e-2
+    # shock position at t = 0.2: x = 0.5 + 1.752156 * 0.2 = 0.85043; find the steepest descent right of the contact
+    xB, WB = run_sod(256, oracle.SCHEME_B, 2)
+    sel = xB > 0.75
+    k = np.argmin(np.diff(WB[0, WB.shape[1] // 2][sel]))
+    assert abs(xB[sel][k] - 0.85043) < 3.0 / 256
+
+
+@pytest.mark.slow
+def test_stationary_vortex_converges_at_second_order():
+    # L885: "All second order schemes show second order convergence"; stationary vortex, B scheme, L1(rho) eq. 72
+    errs = []
+    for n in (32, 64, 128):
+        cfg = wl.make_config("vortex", n=n)
+        m = cfg.mesh
+        om = oracle.OracleMesh(m.xy, m.tri, period=m.period, threads=8)
+        om.set_state(cfg.W0)
+        om.step(100000, t_end=1.0)
+        rho = om.get_state()[0]
+        errs.append(np.mean(np.abs(rho - wl.vortex_exact_density(m))))
+    o1 = np.log2(errs[0] / errs[1])
+    o2 = np.log2(errs[1] / errs[2])
+    assert 1.6 < o2 < 2.6 and o1 > 1.3, (errs, o1, o2)
+
+
+def test_vortex_centre_values():
+    # closed-form values of eq. 78-80 at r = 0 for beta = 5: T = 0.754090, rho = 0.493807, p = 0.372375
+    m = wl.uniform_mesh(4, 4, 10.0, 10.0, periodic=True)
+    m.xy[0] = (5.0, 5.0)
+    W = wl.vortex_state(m)
+    rho, u, v, p = wl.conserved_to_primitive(W)
+    assert abs(rho[0] - 0.493807) < 1e-6 and abs(p[0] - 0.372375) < 1e-6 and abs(p[0] / rho[0] - 0.754090) < 1e-6
+    assert u[0] == 0 and v[0] == 0
