@@ -1,0 +1,253 @@
+"""ctypes binding of include/mrd.h.  Marshalling only; no arithmetic of the method lives here."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import re
+
+import numpy as np
+
+from . import build as _build
+
+MRD_OK, MRD_EINVAL, MRD_ENOMEM, MRD_ECUDA, MRD_ENONPHYSICAL = 0, -1, -2, -3, -4
+SCHEME_N, SCHEME_LDA, SCHEME_B = 0, 1, 2
+FP64, FP32 = 0, 1
+
+
+class Params(C.Structure):
+    """mrd_params of include/mrd.h."""
+    _fields_ = [("gamma", C.c_double), ("cfl", C.c_double), ("scheme", C.c_int32), ("time_order", C.c_int32),
+                ("precision", C.c_int32), ("reorder", C.c_int32), ("period_x", C.c_double), ("period_y", C.c_double),
+                ("tile", C.c_int32), ("reserved", C.c_int32)]
+
+
+class MrdError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"mrd error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+_dp, _ip, _lp, _bp = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int64), C.POINTER(C.c_uint8)
+
+
+def lib():
+    """Load (building it first when missing or stale) paper_1705_02028_b200/libmrd.so. Fails loudly."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        vp, pp = C.c_void_p, C.POINTER(Params)
+        mesh_args = [pp, C.c_int64, _dp, C.c_int64, _ip, _bp, C.c_int64, _ip]
+        L.mrd_layout_create.argtypes = [C.POINTER(vp)] + mesh_args
+        L.mrd_layout_destroy.argtypes = [vp]
+        L.mrd_layout_destroy.restype = None
+        L.mrd_layout_sizes.argtypes = [vp, _lp]
+        L.mrd_layout_get.argtypes = [vp, _ip, _ip, _ip, _ip, _ip, _dp, _dp]
+        L.mrd_mesh_create.argtypes = [C.POINTER(vp)] + mesh_args
+        L.mrd_mesh_destroy.argtypes = [vp]
+        L.mrd_mesh_destroy.restype = None
+        L.mrd_mesh_device_bytes.argtypes = [vp, _lp]
+        L.mrd_set_state.argtypes = [vp, vp, vp]
+        L.mrd_set_state_host.argtypes = [vp, vp, vp]
+        L.mrd_get_state.argtypes = [vp, vp, vp]
+        L.mrd_get_state_host.argtypes = [vp, vp, vp]
+        L.mrd_step.argtypes = [vp, C.c_int64, C.c_double, vp, _lp, _dp, _dp]
+        L.mrd_step_async.argtypes = [vp, C.c_int64, vp]
+        L.mrd_sync.argtypes = [vp, vp, _lp, _dp, _dp]
+        L.mrd_get_diagnostics.argtypes = [vp, _dp, _dp, _dp, vp]
+        L.mrd_dump_stage1.argtypes = [vp, _dp, _dp, _dp, _dp, _dp, vp]
+        L.mrd_measure_peaks.argtypes = [_dp, _dp, _dp, vp]
+        L.mrd_launch_count.argtypes = [vp, _lp]
+        L.mrd_step_profile.argtypes = [vp, vp, C.POINTER(C.c_float)]
+        L.mrd_last_error.restype = C.c_char_p
+        L.mrd_version.restype = C.c_char_p
+        L._path = path
+        _lib = L
+    return _lib
+
+
+def exported_symbols():
+    """Names declared in include/mrd.h (functions `mrd_*(`), for the symbol-export test."""
+    hdr = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "mrd.h")
+    text = open(hdr).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(mrd_[a-z0-9_]+)\s*\(", text)))
+
+
+def version() -> str:
+    return lib().mrd_version().decode()
+
+
+def _check(rc):
+    if rc != 0:
+        raise MrdError(rc, lib().mrd_last_error().decode())
+
+
+def _np_ptr(a, ctype):
+    return None if a is None else a.ctypes.data_as(C.POINTER(ctype))
+
+
+def _mesh_args(xy, tri, vertex_flag, wall_edge):
+    xy = np.ascontiguousarray(xy, dtype=np.float64)
+    tri = np.ascontiguousarray(tri, dtype=np.int32)
+    assert xy.ndim == 2 and xy.shape[1] == 2 and tri.ndim == 2 and tri.shape[1] == 3
+    flag = None if vertex_flag is None else np.ascontiguousarray(vertex_flag, dtype=np.uint8)
+    wedge = None if wall_edge is None else np.ascontiguousarray(wall_edge, dtype=np.int32)
+    ne = 0 if wedge is None else int(wedge.shape[0])
+    keep = (xy, tri, flag, wedge)
+    args = (xy.shape[0], _np_ptr(xy, C.c_double), tri.shape[0], _np_ptr(tri, C.c_int32), _np_ptr(flag, C.c_uint8), ne,
+            _np_ptr(wedge, C.c_int32))
+    return keep, args
+
+
+def make_params(gamma=1.4, cfl=0.5, scheme=SCHEME_B, time_order=2, precision=FP64, reorder=True,
+                period=(0.0, 0.0), tile=0) -> Params:
+    return Params(float(gamma), float(cfl), int(scheme), int(time_order), int(precision), int(bool(reorder)),
+                  float(period[0]), float(period[1]), int(tile), 0)
+
+
+class Layout:
+    """mrd_layout_*: the host-only mesh-layout stage (no CUDA needed)."""
+
+    def __init__(self, xy, tri, vertex_flag=None, wall_edge=None, **params):
+        self.params = make_params(**params)
+        keep, args = _mesh_args(xy, tri, vertex_flag, wall_edge)
+        h = C.c_void_p()
+        _check(lib().mrd_layout_create(C.byref(h), C.byref(self.params), *args))
+        self._h = h
+        n = (C.c_int64 * 6)()
+        _check(lib().mrd_layout_sizes(h, n))
+        self.nv, self.nt, self.ne, self.nf, self.ntile, self.nslot = [int(x) for x in n]
+
+    def __del__(self):
+        h, self._h = getattr(self, "_h", None), None
+        if h:
+            lib().mrd_layout_destroy(h)
+
+    def get(self):
+        nv, nt = self.nv, self.nt
+        o = dict(vperm=np.empty(nv, np.int32), tperm=np.empty(nt, np.int32), tri=np.empty((nt, 3), np.int32),
+                 csr_off=np.empty(nv + 1, np.int32), csr_ent=np.empty(3 * nt, np.int32), area=np.empty(nt),
+                 vol=np.empty(nv))
+        _check(lib().mrd_layout_get(self._h, _np_ptr(o["vperm"], C.c_int32), _np_ptr(o["tperm"], C.c_int32),
+                                    _np_ptr(o["tri"], C.c_int32), _np_ptr(o["csr_off"], C.c_int32),
+                                    _np_ptr(o["csr_ent"], C.c_int32), _np_ptr(o["area"], C.c_double),
+                                    _np_ptr(o["vol"], C.c_double)))
+        return o
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(int(stream.cuda_stream))
+
+
+class Mesh:
+    """mrd_mesh_*: mesh + device state + stepper.  State tensors are torch CUDA tensors [4][nv]
+    (float64 or float32 per `precision`) in USER numbering, or numpy arrays for the *_host calls."""
+
+    def __init__(self, xy, tri, vertex_flag=None, wall_edge=None, **params):
+        import torch
+        if not torch.cuda.is_available():
+            raise MrdError(MRD_ECUDA, "no CUDA device: the mrd path has no CPU fallback")
+        self._torch = torch
+        self.params = make_params(**params)
+        self.dtype = torch.float64 if self.params.precision == FP64 else torch.float32
+        self.np_dtype = np.float64 if self.params.precision == FP64 else np.float32
+        keep, args = _mesh_args(xy, tri, vertex_flag, wall_edge)
+        self.nv, self.nt = int(args[0]), int(args[2])
+        h = C.c_void_p()
+        _check(lib().mrd_mesh_create(C.byref(h), C.byref(self.params), *args))
+        self._h = h
+
+    def __del__(self):
+        h, self._h = getattr(self, "_h", None), None
+        if h:
+            lib().mrd_mesh_destroy(h)
+
+    close = __del__
+
+    def device_bytes(self) -> int:
+        n = C.c_int64()
+        _check(lib().mrd_mesh_device_bytes(self._h, C.byref(n)))
+        return n.value
+
+    def _check_tensor(self, W):
+        t = self._torch
+        assert isinstance(W, t.Tensor) and W.is_cuda and W.dtype == self.dtype and W.is_contiguous()
+        assert tuple(W.shape) == (4, self.nv), (tuple(W.shape), self.nv)
+
+    def set_state(self, W, stream=None):
+        self._check_tensor(W)
+        _check(lib().mrd_set_state(self._h, C.c_void_p(W.data_ptr()), _stream_ptr(stream)))
+
+    def set_state_host(self, W, stream=None):
+        W = np.ascontiguousarray(W, dtype=self.np_dtype)
+        assert W.shape == (4, self.nv)
+        _check(lib().mrd_set_state_host(self._h, C.c_void_p(W.ctypes.data), _stream_ptr(stream)))
+
+    def get_state(self, out=None, stream=None):
+        if out is None:
+            out = self._torch.empty((4, self.nv), dtype=self.dtype, device="cuda")
+        self._check_tensor(out)
+        _check(lib().mrd_get_state(self._h, C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+        return out
+
+    def get_state_host(self, out=None, stream=None):
+        if out is None:
+            out = np.empty((4, self.nv), dtype=self.np_dtype)
+        assert out.dtype == self.np_dtype and out.shape == (4, self.nv) and out.flags.c_contiguous
+        _check(lib().mrd_get_state_host(self._h, C.c_void_p(out.ctypes.data), _stream_ptr(stream)))
+        return out
+
+    def step(self, max_steps=1, t_end=0.0, stream=None):
+        n, t, dt = C.c_int64(0), C.c_double(0.0), C.c_double(0.0)
+        _check(lib().mrd_step(self._h, int(max_steps), float(t_end), _stream_ptr(stream), C.byref(n), C.byref(t),
+                              C.byref(dt)))
+        return n.value, t.value, dt.value
+
+    def step_async(self, n_steps, stream=None):
+        _check(lib().mrd_step_async(self._h, int(n_steps), _stream_ptr(stream)))
+
+    def sync(self, stream=None):
+        n, t, dt = C.c_int64(0), C.c_double(0.0), C.c_double(0.0)
+        _check(lib().mrd_sync(self._h, _stream_ptr(stream), C.byref(n), C.byref(t), C.byref(dt)))
+        return n.value, t.value, dt.value
+
+    def diagnostics(self, stream=None):
+        tot = np.empty(4)
+        mr, mp = C.c_double(), C.c_double()
+        _check(lib().mrd_get_diagnostics(self._h, _np_ptr(tot, C.c_double), C.byref(mr), C.byref(mp),
+                                         _stream_ptr(stream)))
+        return tot, mr.value, mp.value
+
+    def dump_stage1(self, stream=None):
+        nt = self.nt
+        o = dict(phiT=np.empty((nt, 4)), phiN=np.empty((nt, 3, 4)), phiLDA=np.empty((nt, 3, 4)),
+                 phiB=np.empty((nt, 3, 4)), sT=np.empty(nt))
+        _check(lib().mrd_dump_stage1(self._h, _np_ptr(o["phiT"], C.c_double), _np_ptr(o["phiN"], C.c_double),
+                                     _np_ptr(o["phiLDA"], C.c_double), _np_ptr(o["phiB"], C.c_double),
+                                     _np_ptr(o["sT"], C.c_double), _stream_ptr(stream)))
+        return o
+
+    PROFILE_SLOTS = ("tri_stage1", "gather_dt", "wall1", "update", "tri_stage2", "wall2", "gather_update", "ctl")
+
+    def step_profile(self, stream=None):
+        """One step with per-kernel CUDA-event timing: dict slot name -> ms."""
+        ms = (C.c_float * 8)()
+        _check(lib().mrd_step_profile(self._h, _stream_ptr(stream), ms))
+        return dict(zip(self.PROFILE_SLOTS, [float(x) for x in ms]))
+
+    def launch_count(self) -> int:
+        n = C.c_int64()
+        _check(lib().mrd_launch_count(self._h, C.byref(n)))
+        return n.value
+
+
+def measure_peaks(stream=None):
+    """(fp64 TFLOP/s, fp32 TFLOP/s, copy GB/s) micro-benchmarks of the current device."""
+    a, b, c = C.c_double(), C.c_double(), C.c_double()
+    _check(lib().mrd_measure_peaks(C.byref(a), C.byref(b), C.byref(c), _stream_ptr(stream)))
+    return a.value, b.value, c.value

@@ -1,0 +1,699 @@
+// mrd_api.cu -- the C-ABI of include/mrd.h: host orchestration of the sm_100a kernels.
+// No torch types, no CPU fallback: every step of the path runs in the kernels of mrd_kernels.cuh.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/mrd.h"
+#include "mrd_kernels.cuh"
+#include "mrd_layout.h"
+
+namespace {
+
+thread_local std::string g_err;
+int fail(int code, const std::string &msg) {
+  g_err = msg;
+  return code;
+}
+#define CUDA_TRY(expr)                                                                          \
+  do {                                                                                          \
+    cudaError_t e_ = (expr);                                                                    \
+    if (e_ != cudaSuccess)                                                                      \
+      return fail(e_ == cudaErrorMemoryAllocation ? MRD_ENOMEM : MRD_ECUDA,                     \
+                  std::string(#expr) + ": " + cudaGetErrorString(e_));                          \
+  } while (0)
+
+inline unsigned blocks_for(int64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+}  // namespace
+
+struct mrd_mesh {
+  mrd_layout L;
+  int device = 0;
+  std::vector<void *> allocs;
+  int64_t dev_bytes = 0;
+  int64_t launches = 0;
+  // device arrays (element type per L.p.precision where it says R)
+  int32_t *d_vperm = nullptr, *d_vrank = nullptr, *d_tperm = nullptr;
+  int32_t *d_tv[3] = {nullptr, nullptr, nullptr};
+  void *d_gnx[3], *d_gny[3], *d_ghl[3], *d_area3 = nullptr, *d_lmax = nullptr;  // R
+  int32_t *d_csr_off = nullptr, *d_csr_ent = nullptr;
+  void *d_vol = nullptr;          // R
+  uint8_t *d_frozen = nullptr;    // or null
+  uint8_t *d_tswap = nullptr;
+  // walls
+  int64_t nwv = 0;
+  int32_t *d_wv_vertex = nullptr, *d_wv_off = nullptr, *d_wv_ent = nullptr, *d_wall_a = nullptr, *d_wall_b = nullptr;
+  void *d_wall_nx = nullptr, *d_wall_ny = nullptr, *d_wall_len = nullptr;  // R
+  // state: pairs (W, Z, spd) x 2; `cur` holds W^n
+  void *d_W[2] = {nullptr, nullptr}, *d_Z[2] = {nullptr, nullptr}, *d_spd[2] = {nullptr, nullptr};
+  int cur = 0;
+  void *d_acc = nullptr, *d_dWdt = nullptr, *d_wall_acc = nullptr;       // Vec4<R> [nv]
+  void *d_phi = nullptr, *d_phiN = nullptr, *d_phiT = nullptr, *d_sT = nullptr;  // per triangle
+  void *d_user = nullptr;         // R [4][nv] staging for the host variants and dumps
+  mrd::Ctl *d_ctl = nullptr;
+  int *d_flag = nullptr;          // non-physical flag raised by kernels
+  double *d_diag = nullptr;       // [DIAG_BLOCKS][6]
+  void *h_pinned = nullptr;       // pinned host staging, R [4][nv]
+  bool has_state = false;
+  int64_t steps_base = 0;         // completed steps at the last sync (for buffer parity)
+};
+
+namespace {
+
+constexpr int DIAG_BLOCKS = 1024;
+
+template <class T> int dev_alloc(mrd_mesh *m, T **out, int64_t count) {
+  size_t bytes = (size_t)(count > 0 ? count : 1) * sizeof(T);
+  void *p = nullptr;
+  CUDA_TRY(cudaMalloc(&p, bytes));
+  m->allocs.push_back(p);
+  m->dev_bytes += (int64_t)bytes;
+  *out = static_cast<T *>(p);
+  return MRD_OK;
+}
+template <class T> int dev_upload(mrd_mesh *m, T **out, const T *src, int64_t count) {
+  int rc = dev_alloc(m, out, count);
+  if (rc) return rc;
+  if (count > 0) CUDA_TRY(cudaMemcpy(*out, src, (size_t)count * sizeof(T), cudaMemcpyHostToDevice));
+  return MRD_OK;
+}
+// upload a double array converted to the sweep precision
+template <class R> int dev_upload_real(mrd_mesh *m, void **out, const double *src, int64_t count, double scale = 1.0) {
+  std::vector<R> tmp((size_t)count);
+  for (int64_t i = 0; i < count; ++i) tmp[i] = (R)(src[i] * scale);
+  R *p = nullptr;
+  int rc = dev_upload<R>(m, &p, tmp.data(), count);
+  *out = p;
+  return rc;
+}
+
+template <class R> mrd::MeshDev<R> mesh_dev(const mrd_mesh *m) {
+  mrd::MeshDev<R> d;
+  d.nv = m->L.nv;
+  d.nt = m->L.nt;
+  for (int i = 0; i < 3; ++i) {
+    d.tv[i] = m->d_tv[i];
+    d.gnx[i] = (const R *)m->d_gnx[i];
+    d.gny[i] = (const R *)m->d_gny[i];
+    d.ghl[i] = (const R *)m->d_ghl[i];
+  }
+  d.area3 = (const R *)m->d_area3;
+  d.lmax = (const R *)m->d_lmax;
+  d.csr_off = m->d_csr_off;
+  d.csr_ent = m->d_csr_ent;
+  d.vol = (const R *)m->d_vol;
+  d.frozen = m->d_frozen;
+  return d;
+}
+template <class R> mrd::WallDev<R> wall_dev(const mrd_mesh *m) {
+  mrd::WallDev<R> w;
+  w.nwv = m->nwv;
+  w.wv_vertex = m->d_wv_vertex;
+  w.wv_off = m->d_wv_off;
+  w.wv_ent = m->d_wv_ent;
+  w.wall_a = m->d_wall_a;
+  w.wall_b = m->d_wall_b;
+  w.nx = (const R *)m->d_wall_nx;
+  w.ny = (const R *)m->d_wall_ny;
+  w.len = (const R *)m->d_wall_len;
+  return w;
+}
+
+template <class R> int upload_impl(mrd_mesh *m) {
+  using V4 = mrd::Vec4<R>;
+  mrd_layout &L = m->L;
+  const int64_t nv = L.nv, nt = L.nt;
+  int rc;
+  if ((rc = dev_upload(m, &m->d_vperm, L.vperm.data(), nv))) return rc;
+  if ((rc = dev_upload(m, &m->d_vrank, L.vrank.data(), nv))) return rc;
+  if ((rc = dev_upload(m, &m->d_tperm, L.tperm.data(), nt))) return rc;
+  if ((rc = dev_upload(m, &m->d_tswap, L.tswap.data(), nt))) return rc;
+  {
+    std::vector<int32_t> col(nt);
+    for (int j = 0; j < 3; ++j) {
+      for (int64_t t = 0; t < nt; ++t) col[t] = L.tri[3 * t + j];
+      if ((rc = dev_upload(m, &m->d_tv[j], col.data(), nt))) return rc;
+    }
+  }
+  for (int i = 0; i < 3; ++i) {
+    if ((rc = dev_upload_real<R>(m, &m->d_gnx[i], L.nx[i].data(), nt))) return rc;
+    if ((rc = dev_upload_real<R>(m, &m->d_gny[i], L.ny[i].data(), nt))) return rc;
+    if ((rc = dev_upload_real<R>(m, &m->d_ghl[i], L.hl[i].data(), nt))) return rc;
+  }
+  if ((rc = dev_upload_real<R>(m, &m->d_area3, L.area.data(), nt, 1.0 / 3.0))) return rc;
+  if ((rc = dev_upload_real<R>(m, &m->d_lmax, L.lmax.data(), nt))) return rc;
+  if ((rc = dev_upload(m, &m->d_csr_off, L.csr_off.data(), nv + 1))) return rc;
+  if ((rc = dev_upload(m, &m->d_csr_ent, L.csr_ent.data(), 3 * nt))) return rc;
+  if ((rc = dev_upload_real<R>(m, &m->d_vol, L.vol.data(), nv))) return rc;
+  if (L.nf > 0 && (rc = dev_upload(m, &m->d_frozen, L.frozen.data(), nv))) return rc;
+  m->nwv = (int64_t)L.wv_vertex.size();
+  if (L.ne > 0) {
+    if ((rc = dev_upload(m, &m->d_wv_vertex, L.wv_vertex.data(), m->nwv))) return rc;
+    if ((rc = dev_upload(m, &m->d_wv_off, L.wv_off.data(), m->nwv + 1))) return rc;
+    if ((rc = dev_upload(m, &m->d_wv_ent, L.wv_ent.data(), (int64_t)L.wv_ent.size()))) return rc;
+    if ((rc = dev_upload(m, &m->d_wall_a, L.wall_a.data(), L.ne))) return rc;
+    if ((rc = dev_upload(m, &m->d_wall_b, L.wall_b.data(), L.ne))) return rc;
+    if ((rc = dev_upload_real<R>(m, &m->d_wall_nx, L.wall_nx.data(), L.ne))) return rc;
+    if ((rc = dev_upload_real<R>(m, &m->d_wall_ny, L.wall_ny.data(), L.ne))) return rc;
+    if ((rc = dev_upload_real<R>(m, &m->d_wall_len, L.wall_len.data(), L.ne))) return rc;
+    V4 *wa = nullptr;
+    if ((rc = dev_alloc(m, &wa, nv))) return rc;
+    CUDA_TRY(cudaMemset(wa, 0, (size_t)nv * sizeof(V4)));
+    m->d_wall_acc = wa;
+  }
+  for (int b = 0; b < 2; ++b) {
+    V4 *w = nullptr, *z = nullptr;
+    R *s = nullptr;
+    if ((rc = dev_alloc(m, &w, nv)) || (rc = dev_alloc(m, &z, nv)) || (rc = dev_alloc(m, &s, nv))) return rc;
+    m->d_W[b] = w; m->d_Z[b] = z; m->d_spd[b] = s;
+  }
+  {
+    V4 *a = nullptr, *d = nullptr, *p = nullptr, *pn = nullptr, *pt = nullptr;
+    R *st = nullptr, *us = nullptr;
+    if ((rc = dev_alloc(m, &a, nv)) || (rc = dev_alloc(m, &d, nv))) return rc;
+    if ((rc = dev_alloc(m, &p, 3 * nt)) || (rc = dev_alloc(m, &pn, 3 * nt)) || (rc = dev_alloc(m, &pt, nt))) return rc;
+    if ((rc = dev_alloc(m, &st, nt)) || (rc = dev_alloc(m, &us, 4 * nv))) return rc;
+    m->d_acc = a; m->d_dWdt = d; m->d_phi = p; m->d_phiN = pn; m->d_phiT = pt; m->d_sT = st; m->d_user = us;
+  }
+  if ((rc = dev_alloc(m, &m->d_ctl, 1)) || (rc = dev_alloc(m, &m->d_flag, 1)) || (rc = dev_alloc(m, &m->d_diag, DIAG_BLOCKS * 6))) return rc;
+  CUDA_TRY(cudaMemset(m->d_ctl, 0, sizeof(mrd::Ctl)));
+  CUDA_TRY(cudaMemset(m->d_flag, 0, sizeof(int)));
+  CUDA_TRY(cudaDeviceSynchronize());
+  return MRD_OK;
+}
+
+template <class R> int set_state_impl(mrd_mesh *m, const R *W_dev, cudaStream_t s) {
+  using V4 = mrd::Vec4<R>;
+  const int64_t nv = m->L.nv;
+  m->cur = 0;
+  m->has_state = false;
+  mrd::Ctl c{};
+  c.t = 0.0; c.dt = 0.0; c.t_end = 0.0; c.cfl = m->L.p.cfl;
+  c.dmin_bits = 0x7FF0000000000000ull; c.steps = 0; c.status = 0; c.active = 0;
+  CUDA_TRY(cudaMemcpyAsync(m->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
+  mrd::set_state_kernel<R><<<blocks_for(nv, 256), 256, 0, s>>>(nv, m->d_vperm, W_dev, (R)m->L.p.gamma, (V4 *)m->d_W[0],
+                                                               (V4 *)m->d_Z[0], (R *)m->d_spd[0], m->d_flag);
+  m->launches++;
+  int flag = 0;
+  CUDA_TRY(cudaMemcpyAsync(&flag, m->d_flag, sizeof(int), cudaMemcpyDeviceToHost, s));
+  CUDA_TRY(cudaStreamSynchronize(s));
+  CUDA_TRY(cudaGetLastError());
+  m->steps_base = 0;
+  if (flag) {
+    CUDA_TRY(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
+    return fail(MRD_ENONPHYSICAL, "state has rho <= 0 or p <= 0");
+  }
+  m->has_state = true;
+  return MRD_OK;
+}
+
+template <class R> int get_state_impl(mrd_mesh *m, R *W_dev, cudaStream_t s) {
+  using V4 = mrd::Vec4<R>;
+  const int64_t nv = m->L.nv;
+  mrd::get_state_kernel<R><<<blocks_for(nv, 256), 256, 0, s>>>(nv, m->d_vrank, (const V4 *)m->d_W[m->cur], W_dev);
+  m->launches++;
+  CUDA_TRY(cudaGetLastError());
+  return MRD_OK;
+}
+
+template <class R, int SCHEME> void launch_stage1(mrd_mesh *m, bool store, int a, cudaStream_t s) {
+  using V4 = mrd::Vec4<R>;
+  auto md = mesh_dev<R>(m);
+  const unsigned nb = blocks_for(md.nt, 128);
+  if (store)
+    mrd::tri_stage1_kernel<R, SCHEME, true><<<nb, 128, 0, s>>>(md, (R)m->L.p.gamma, m->d_ctl, (const V4 *)m->d_Z[a], (const R *)m->d_spd[a],
+                                                            (V4 *)m->d_phi, (V4 *)m->d_phiN, (V4 *)m->d_phiT, (R *)m->d_sT, m->d_flag);
+  else
+    mrd::tri_stage1_kernel<R, SCHEME, false><<<nb, 128, 0, s>>>(md, (R)m->L.p.gamma, m->d_ctl, (const V4 *)m->d_Z[a], (const R *)m->d_spd[a],
+                                                             (V4 *)m->d_phi, (V4 *)m->d_phiN, (V4 *)m->d_phiT, (R *)m->d_sT, m->d_flag);
+  m->launches++;
+}
+template <class R, int SCHEME> void launch_stage2(mrd_mesh *m, int b, cudaStream_t s) {
+  using V4 = mrd::Vec4<R>;
+  auto md = mesh_dev<R>(m);
+  mrd::tri_stage2_kernel<R, SCHEME><<<blocks_for(md.nt, 128), 128, 0, s>>>(md, (R)m->L.p.gamma, m->d_ctl, (const V4 *)m->d_Z[b],
+                                                                        (const V4 *)m->d_dWdt, (const V4 *)m->d_phiN, (const V4 *)m->d_phiT,
+                                                                        (V4 *)m->d_phi, m->d_flag);
+  m->launches++;
+}
+
+// optional per-kernel timing of one step (mrd_step_profile): an event after every launch
+struct Prof {
+  cudaEvent_t ev[MRD_PROFILE_SLOTS + 2];
+  int slot[MRD_PROFILE_SLOTS + 2];
+  int n = 0;
+  void mark(int k, cudaStream_t s) {
+    slot[n] = k;
+    cudaEventRecord(ev[n], s);
+    ++n;
+  }
+};
+#define PROF_MARK(k) \
+  if (prof) prof->mark((k), s);
+
+// one time step enqueued on s; `a` = buffer pair holding W^n
+template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_t s, Prof *prof = nullptr) {
+  using V4 = mrd::Vec4<R>;
+  const int b = a ^ 1;
+  const bool rk2 = m->L.p.time_order == 2;
+  auto md = mesh_dev<R>(m);
+  const R gamma = (R)m->L.p.gamma;
+  switch (scheme) {
+    case MRD_SCHEME_N: launch_stage1<R, MRD_SCHEME_N>(m, rk2, a, s); break;
+    case MRD_SCHEME_LDA: launch_stage1<R, MRD_SCHEME_LDA>(m, rk2, a, s); break;
+    default: launch_stage1<R, MRD_SCHEME_B>(m, rk2, a, s); break;
+  }
+  PROF_MARK(MRD_PROF_TRI1)
+  mrd::gather_dt_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, m->d_ctl, (const V4 *)m->d_phi, (const R *)m->d_sT, (V4 *)m->d_acc);
+  m->launches++;
+  PROF_MARK(MRD_PROF_GATHER_DT)
+  if (m->nwv > 0) {
+    mrd::wall_kernel<R, 1><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[a], (V4 *)m->d_acc);
+    m->launches++;
+    PROF_MARK(MRD_PROF_WALL1)
+  }
+  if (!rk2) {
+    mrd::update_kernel<R, true><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_acc, (V4 *)m->d_W[b],
+                                                                    (V4 *)m->d_Z[b], (R *)m->d_spd[b], (V4 *)m->d_dWdt, m->d_flag);
+    m->launches++;
+    PROF_MARK(MRD_PROF_UPDATE)
+  } else {
+    mrd::update_kernel<R, false><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_acc, (V4 *)m->d_W[b],
+                                                                     (V4 *)m->d_Z[b], (R *)m->d_spd[b], (V4 *)m->d_dWdt, m->d_flag);
+    m->launches++;
+    PROF_MARK(MRD_PROF_UPDATE)
+    switch (scheme) {
+      case MRD_SCHEME_N: launch_stage2<R, MRD_SCHEME_N>(m, b, s); break;
+      case MRD_SCHEME_LDA: launch_stage2<R, MRD_SCHEME_LDA>(m, b, s); break;
+      default: launch_stage2<R, MRD_SCHEME_B>(m, b, s); break;
+    }
+    PROF_MARK(MRD_PROF_TRI2)
+    if (m->nwv > 0) {
+      mrd::wall_kernel<R, 2><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[b], (V4 *)m->d_wall_acc);
+      m->launches++;
+      PROF_MARK(MRD_PROF_WALL2)
+    }
+    mrd::gather_update_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_phi, (const V4 *)m->d_wall_acc, (V4 *)m->d_W[b],
+                                                                     (V4 *)m->d_Z[b], (R *)m->d_spd[b], m->d_flag);
+    m->launches++;
+    PROF_MARK(MRD_PROF_GATHER_UPDATE)
+  }
+  mrd::ctl_kernel<<<1, 1, 0, s>>>(m->d_ctl, 1, 0.0, m->d_flag);
+  m->launches++;
+  PROF_MARK(MRD_PROF_CTL)
+}
+
+// fetch the control block (after a stream sync) and bring the host bookkeeping up to date
+int fetch_ctl(mrd_mesh *m, cudaStream_t s, mrd::Ctl *out) {
+  CUDA_TRY(cudaMemcpyAsync(out, m->d_ctl, sizeof(mrd::Ctl), cudaMemcpyDeviceToHost, s));
+  CUDA_TRY(cudaStreamSynchronize(s));
+  CUDA_TRY(cudaGetLastError());
+  // every completed step swapped the buffer pairs once
+  int64_t done = out->steps - m->steps_base;
+  if (done & 1) m->cur ^= 1;
+  m->steps_base = out->steps;
+  return MRD_OK;
+}
+
+template <class R> int step_impl(mrd_mesh *m, int64_t max_steps, double t_end, cudaStream_t s, bool sync,
+                                 int64_t *steps_done, double *t, double *dt_last) {
+  if (!m->has_state) return fail(MRD_EINVAL, "no state set");
+  if (max_steps < 0) return fail(MRD_EINVAL, "max_steps < 0");
+  mrd::Ctl c{};
+  int rc;
+  // steps enqueued by earlier async calls change the parity: settle it first
+  if ((rc = fetch_ctl(m, s, &c))) return rc;
+  if (c.status) return fail(MRD_ENONPHYSICAL, "state is non-physical (an earlier step failed)");
+  const int64_t steps0 = c.steps;
+  mrd::ctl_kernel<<<1, 1, 0, s>>>(m->d_ctl, 0, t_end > 0.0 ? t_end : 0.0, m->d_flag);
+  m->launches++;
+  const int scheme = m->L.p.scheme;
+  int64_t enq = 0;
+  int a = m->cur;
+  if (!(t_end > 0.0)) {
+    for (; enq < max_steps; ++enq, a ^= 1) enqueue_step<R>(m, scheme, a, s);
+    if (!sync) { CUDA_TRY(cudaGetLastError()); return MRD_OK; }
+    if ((rc = fetch_ctl(m, s, &c))) return rc;
+  } else {
+    // t_end mode: the device decides when to stop; the host enqueues in chunks and looks at the clock
+    const int64_t chunk = 32;
+    while (enq < max_steps) {
+      int64_t n = std::min<int64_t>(chunk, max_steps - enq);
+      for (int64_t k = 0; k < n; ++k, a ^= 1) enqueue_step<R>(m, scheme, a, s);
+      enq += n;
+      if ((rc = fetch_ctl(m, s, &c))) return rc;
+      a = m->cur;
+      if (c.status || c.t >= t_end) break;
+      if (c.steps - steps0 < enq) break;  // defensive: device stopped for another reason
+    }
+  }
+  if (steps_done) *steps_done = c.steps - steps0;
+  if (t) *t = c.t;
+  if (dt_last) *dt_last = c.dt;
+  if (c.status) {
+    // the failed step is discarded: clear the flag so that the state (last good step) stays usable
+    mrd::Ctl fix = c;
+    fix.status = 0;
+    fix.active = 0;
+    CUDA_TRY(cudaMemcpyAsync(m->d_ctl, &fix, sizeof fix, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    return fail(MRD_ENONPHYSICAL, "non-physical state (rho <= 0, p <= 0 or c^2 <= 0) met; state left at the last good step");
+  }
+  return MRD_OK;
+}
+
+template <class R> int diag_impl(mrd_mesh *m, double totals[4], double *min_rho, double *min_p, cudaStream_t s) {
+  using V4 = mrd::Vec4<R>;
+  mrd::diag_kernel<R><<<DIAG_BLOCKS, 256, 0, s>>>(m->L.nv, (R)m->L.p.gamma, (const V4 *)m->d_W[m->cur], (const R *)m->d_vol, m->d_diag);
+  m->launches++;
+  std::vector<double> h(DIAG_BLOCKS * 6);
+  CUDA_TRY(cudaMemcpyAsync(h.data(), m->d_diag, h.size() * sizeof(double), cudaMemcpyDeviceToHost, s));
+  CUDA_TRY(cudaStreamSynchronize(s));
+  CUDA_TRY(cudaGetLastError());
+  double tot[4] = {0, 0, 0, 0}, mr = INFINITY, mp = INFINITY;
+  for (int b = 0; b < DIAG_BLOCKS; ++b) {
+    for (int k = 0; k < 4; ++k) tot[k] += h[6 * b + k];
+    mr = std::fmin(mr, h[6 * b + 4]);
+    mp = std::fmin(mp, h[6 * b + 5]);
+  }
+  if (totals) std::memcpy(totals, tot, sizeof tot);
+  if (min_rho) *min_rho = mr;
+  if (min_p) *min_p = mp;
+  return MRD_OK;
+}
+
+// per-triangle dump of stage 1 in USER numbering / node order
+template <class R> int dump_impl(mrd_mesh *m, double *phiT, double *phiN, double *phiLDA, double *phiB, double *sT, cudaStream_t s) {
+  using V4 = mrd::Vec4<R>;
+  const int64_t nt = m->L.nt;
+  mrd::Ctl c{};
+  int rc;
+  if ((rc = fetch_ctl(m, s, &c))) return rc;
+  // arm the guard without touching the clock
+  mrd::Ctl armed = c;
+  armed.active = 1;
+  CUDA_TRY(cudaMemcpyAsync(m->d_ctl, &armed, sizeof armed, cudaMemcpyHostToDevice, s));
+  std::vector<R> h3((size_t)12 * nt), h1((size_t)4 * nt), hs((size_t)nt);
+  auto put3 = [&](double *dst) {  // [nt][3][4] internal -> user triangle order, undo the node swap
+    for (int64_t k = 0; k < nt; ++k) {
+      int64_t u = m->L.tperm[k];
+      for (int i = 0; i < 3; ++i) {
+        int iu = (m->L.tswap[k] && i > 0) ? 3 - i : i;
+        for (int q = 0; q < 4; ++q) dst[12 * u + 4 * iu + q] = (double)h3[12 * k + 4 * i + q];
+      }
+    }
+  };
+  const int a = m->cur;
+  for (int pass = 0; pass < 2; ++pass) {
+    if (pass == 0) launch_stage1<R, MRD_SCHEME_LDA>(m, true, a, s);
+    else launch_stage1<R, MRD_SCHEME_B>(m, true, a, s);
+    CUDA_TRY(cudaMemcpyAsync(h3.data(), m->d_phi, h3.size() * sizeof(R), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    CUDA_TRY(cudaGetLastError());
+    if (pass == 0 && phiLDA) put3(phiLDA);
+    if (pass == 1 && phiB) put3(phiB);
+  }
+  if (phiN) {
+    CUDA_TRY(cudaMemcpy(h3.data(), m->d_phiN, h3.size() * sizeof(R), cudaMemcpyDeviceToHost));
+    put3(phiN);
+  }
+  if (phiT) {
+    CUDA_TRY(cudaMemcpy(h1.data(), m->d_phiT, h1.size() * sizeof(R), cudaMemcpyDeviceToHost));
+    for (int64_t k = 0; k < nt; ++k)
+      for (int q = 0; q < 4; ++q) phiT[4 * (int64_t)m->L.tperm[k] + q] = (double)h1[4 * k + q];
+  }
+  if (sT) {
+    CUDA_TRY(cudaMemcpy(hs.data(), m->d_sT, hs.size() * sizeof(R), cudaMemcpyDeviceToHost));
+    for (int64_t k = 0; k < nt; ++k) sT[m->L.tperm[k]] = (double)hs[k];
+  }
+  int flag = 0;
+  CUDA_TRY(cudaMemcpy(&flag, m->d_flag, sizeof(int), cudaMemcpyDeviceToHost));
+  CUDA_TRY(cudaMemcpy(m->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice));
+  CUDA_TRY(cudaMemset(m->d_flag, 0, sizeof(int)));
+  if (flag) return fail(MRD_ENONPHYSICAL, "non-physical linearised state");
+  return MRD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *mrd_last_error(void) { return g_err.c_str(); }
+const char *mrd_version(void) { return "mrd 0.1 (sm_100a)"; }
+
+int mrd_layout_create(mrd_layout **out, const mrd_params *p, int64_t nv, const double *xy, int64_t nt,
+                      const int32_t *tri, const uint8_t *vertex_flag, int64_t ne, const int32_t *wall_edge) {
+  if (!out) return fail(MRD_EINVAL, "null output pointer");
+  mrd_layout *L = new (std::nothrow) mrd_layout();
+  if (!L) return fail(MRD_ENOMEM, "out of memory");
+  std::string err;
+  int rc;
+  try {
+    rc = mrd_host::layout_build(*L, p, nv, xy, nt, tri, vertex_flag, ne, wall_edge, err);
+  } catch (const std::bad_alloc &) {
+    rc = MRD_ENOMEM;
+    err = "out of host memory in the layout stage";
+  }
+  if (rc) { delete L; return fail(rc, err); }
+  *out = L;
+  return MRD_OK;
+}
+void mrd_layout_destroy(mrd_layout *l) { delete l; }
+
+int mrd_layout_sizes(const mrd_layout *l, int64_t n[6]) {
+  if (!l || !n) return fail(MRD_EINVAL, "null argument");
+  n[0] = l->nv; n[1] = l->nt; n[2] = l->ne; n[3] = l->nf; n[4] = l->ntile; n[5] = l->nslot;
+  return MRD_OK;
+}
+int mrd_layout_get(const mrd_layout *l, int32_t *vperm, int32_t *tperm, int32_t *tri_int, int32_t *csr_off,
+                   int32_t *csr_ent, double *area, double *vol) {
+  if (!l) return fail(MRD_EINVAL, "null argument");
+  if (vperm) std::memcpy(vperm, l->vperm.data(), sizeof(int32_t) * l->nv);
+  if (tperm) std::memcpy(tperm, l->tperm.data(), sizeof(int32_t) * l->nt);
+  if (tri_int) std::memcpy(tri_int, l->tri.data(), sizeof(int32_t) * 3 * l->nt);
+  if (csr_off) std::memcpy(csr_off, l->csr_off.data(), sizeof(int32_t) * (l->nv + 1));
+  if (csr_ent) std::memcpy(csr_ent, l->csr_ent.data(), sizeof(int32_t) * 3 * l->nt);
+  if (area) std::memcpy(area, l->area.data(), sizeof(double) * l->nt);
+  if (vol) std::memcpy(vol, l->vol.data(), sizeof(double) * l->nv);
+  return MRD_OK;
+}
+
+int mrd_mesh_create(mrd_mesh **out, const mrd_params *p, int64_t nv, const double *xy, int64_t nt,
+                    const int32_t *tri, const uint8_t *vertex_flag, int64_t ne, const int32_t *wall_edge) {
+  if (!out) return fail(MRD_EINVAL, "null output pointer");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0)
+    return fail(MRD_ECUDA, std::string("no CUDA device (there is no CPU fallback): ") + cudaGetErrorString(e));
+  mrd_mesh *m = new (std::nothrow) mrd_mesh();
+  if (!m) return fail(MRD_ENOMEM, "out of memory");
+  std::string err;
+  int rc;
+  try {
+    rc = mrd_host::layout_build(m->L, p, nv, xy, nt, tri, vertex_flag, ne, wall_edge, err);
+    if (rc) { delete m; return fail(rc, err); }
+    cudaGetDevice(&m->device);
+    rc = m->L.p.precision == MRD_FP64 ? upload_impl<double>(m) : upload_impl<float>(m);
+  } catch (const std::bad_alloc &) {
+    rc = fail(MRD_ENOMEM, "out of host memory");
+  }
+  if (rc) { mrd_mesh_destroy(m); return rc; }
+  *out = m;
+  return MRD_OK;
+}
+
+void mrd_mesh_destroy(mrd_mesh *m) {
+  if (!m) return;
+  for (void *p : m->allocs) cudaFree(p);
+  if (m->h_pinned) cudaFreeHost(m->h_pinned);
+  delete m;
+}
+
+int mrd_mesh_device_bytes(const mrd_mesh *m, int64_t *bytes) {
+  if (!m || !bytes) return fail(MRD_EINVAL, "null argument");
+  *bytes = m->dev_bytes;
+  return MRD_OK;
+}
+
+int mrd_set_state(mrd_mesh *m, const void *W_dev, void *stream) {
+  if (!m || !W_dev) return fail(MRD_EINVAL, "null argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  return m->L.p.precision == MRD_FP64 ? set_state_impl<double>(m, (const double *)W_dev, s)
+                                      : set_state_impl<float>(m, (const float *)W_dev, s);
+}
+
+int mrd_set_state_host(mrd_mesh *m, const void *W_host, void *stream) {
+  if (!m || !W_host) return fail(MRD_EINVAL, "null argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  size_t bytes = (size_t)4 * m->L.nv * (m->L.p.precision == MRD_FP64 ? 8 : 4);
+  CUDA_TRY(cudaMemcpyAsync(m->d_user, W_host, bytes, cudaMemcpyHostToDevice, s));
+  return mrd_set_state(m, m->d_user, stream);
+}
+
+int mrd_get_state(mrd_mesh *m, void *W_out_dev, void *stream) {
+  if (!m || !W_out_dev) return fail(MRD_EINVAL, "null argument");
+  if (!m->has_state) return fail(MRD_EINVAL, "no state set");
+  cudaStream_t s = (cudaStream_t)stream;
+  mrd::Ctl c{};
+  int rc = fetch_ctl(m, s, &c);  // settles the buffer parity after async steps
+  if (rc) return rc;
+  return m->L.p.precision == MRD_FP64 ? get_state_impl<double>(m, (double *)W_out_dev, s)
+                                      : get_state_impl<float>(m, (float *)W_out_dev, s);
+}
+
+int mrd_get_state_host(mrd_mesh *m, void *W_out_host, void *stream) {
+  if (!m || !W_out_host) return fail(MRD_EINVAL, "null argument");
+  int rc = mrd_get_state(m, m->d_user, stream);
+  if (rc) return rc;
+  cudaStream_t s = (cudaStream_t)stream;
+  size_t bytes = (size_t)4 * m->L.nv * (m->L.p.precision == MRD_FP64 ? 8 : 4);
+  CUDA_TRY(cudaMemcpyAsync(W_out_host, m->d_user, bytes, cudaMemcpyDeviceToHost, s));
+  CUDA_TRY(cudaStreamSynchronize(s));
+  return MRD_OK;
+}
+
+int mrd_step(mrd_mesh *m, int64_t max_steps, double t_end, void *stream, int64_t *steps_done, double *t, double *dt_last) {
+  if (!m) return fail(MRD_EINVAL, "null argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  return m->L.p.precision == MRD_FP64 ? step_impl<double>(m, max_steps, t_end, s, true, steps_done, t, dt_last)
+                                      : step_impl<float>(m, max_steps, t_end, s, true, steps_done, t, dt_last);
+}
+
+int mrd_step_async(mrd_mesh *m, int64_t n_steps, void *stream) {
+  if (!m) return fail(MRD_EINVAL, "null argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  return m->L.p.precision == MRD_FP64 ? step_impl<double>(m, n_steps, 0.0, s, false, nullptr, nullptr, nullptr)
+                                      : step_impl<float>(m, n_steps, 0.0, s, false, nullptr, nullptr, nullptr);
+}
+
+int mrd_sync(mrd_mesh *m, void *stream, int64_t *steps_total, double *t, double *dt_last) {
+  if (!m) return fail(MRD_EINVAL, "null argument");
+  mrd::Ctl c{};
+  int rc = fetch_ctl(m, (cudaStream_t)stream, &c);
+  if (rc) return rc;
+  if (steps_total) *steps_total = c.steps;
+  if (t) *t = c.t;
+  if (dt_last) *dt_last = c.dt;
+  if (c.status) return fail(MRD_ENONPHYSICAL, "non-physical state met in an asynchronous step");
+  return MRD_OK;
+}
+
+int mrd_get_diagnostics(mrd_mesh *m, double totals[4], double *min_rho, double *min_p, void *stream) {
+  if (!m) return fail(MRD_EINVAL, "null argument");
+  if (!m->has_state) return fail(MRD_EINVAL, "no state set");
+  cudaStream_t s = (cudaStream_t)stream;
+  mrd::Ctl c{};
+  int rc = fetch_ctl(m, s, &c);
+  if (rc) return rc;
+  return m->L.p.precision == MRD_FP64 ? diag_impl<double>(m, totals, min_rho, min_p, s) : diag_impl<float>(m, totals, min_rho, min_p, s);
+}
+
+int mrd_dump_stage1(mrd_mesh *m, double *phiT, double *phiN, double *phiLDA, double *phiB, double *sT, void *stream) {
+  if (!m) return fail(MRD_EINVAL, "null argument");
+  if (!m->has_state) return fail(MRD_EINVAL, "no state set");
+  cudaStream_t s = (cudaStream_t)stream;
+  return m->L.p.precision == MRD_FP64 ? dump_impl<double>(m, phiT, phiN, phiLDA, phiB, sT, s)
+                                      : dump_impl<float>(m, phiT, phiN, phiLDA, phiB, sT, s);
+}
+
+int mrd_step_profile(mrd_mesh *m, void *stream, float ms[MRD_PROFILE_SLOTS]) {
+  if (!m || !ms) return fail(MRD_EINVAL, "null argument");
+  if (!m->has_state) return fail(MRD_EINVAL, "no state set");
+  cudaStream_t s = (cudaStream_t)stream;
+  mrd::Ctl c{};
+  int rc = fetch_ctl(m, s, &c);
+  if (rc) return rc;
+  if (c.status) return fail(MRD_ENONPHYSICAL, "state is non-physical (an earlier step failed)");
+  Prof prof;
+  const int nev = MRD_PROFILE_SLOTS + 2;
+  for (int k = 0; k < nev; ++k) CUDA_TRY(cudaEventCreate(&prof.ev[k]));
+  mrd::ctl_kernel<<<1, 1, 0, s>>>(m->d_ctl, 0, 0.0, m->d_flag);
+  m->launches++;
+  prof.mark(-1, s);
+  if (m->L.p.precision == MRD_FP64) enqueue_step<double>(m, m->L.p.scheme, m->cur, s, &prof);
+  else enqueue_step<float>(m, m->L.p.scheme, m->cur, s, &prof);
+  rc = fetch_ctl(m, s, &c);
+  for (int k = 0; k < MRD_PROFILE_SLOTS; ++k) ms[k] = 0.f;
+  if (!rc)
+    for (int k = 1; k < prof.n; ++k) {
+      float t = 0.f;
+      cudaEventElapsedTime(&t, prof.ev[k - 1], prof.ev[k]);
+      ms[prof.slot[k]] += t;
+    }
+  for (int k = 0; k < nev; ++k) cudaEventDestroy(prof.ev[k]);
+  if (rc) return rc;
+  if (c.status) return fail(MRD_ENONPHYSICAL, "non-physical state met in the profiled step");
+  return MRD_OK;
+}
+
+int mrd_launch_count(const mrd_mesh *m, int64_t *launches) {
+  if (!m || !launches) return fail(MRD_EINVAL, "null argument");
+  *launches = m->launches;
+  return MRD_OK;
+}
+
+int mrd_measure_peaks(double *fp64_tflops, double *fp32_tflops, double *copy_gbs, void *stream) {
+  cudaStream_t s = (cudaStream_t)stream;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(MRD_ECUDA, "no CUDA device");
+  cudaDeviceProp prop;
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+  cudaEvent_t e0, e1;
+  CUDA_TRY(cudaEventCreate(&e0));
+  CUDA_TRY(cudaEventCreate(&e1));
+  const int blocks = prop.multiProcessorCount * 8, threads = 256;
+  double *scratch = nullptr;
+  CUDA_TRY(cudaMalloc(&scratch, (size_t)blocks * threads * sizeof(double)));
+  float ms = 0.f;
+  auto best_of = [&](auto launch, int reps, float &best) -> cudaError_t {
+    best = 1e30f;
+    for (int r = 0; r < reps; ++r) {
+      cudaEventRecord(e0, s);
+      launch();
+      cudaEventRecord(e1, s);
+      cudaError_t e = cudaEventSynchronize(e1);
+      if (e != cudaSuccess) return e;
+      float t;
+      cudaEventElapsedTime(&t, e0, e1);
+      if (r > 0 && t < best) best = t;
+    }
+    return cudaGetLastError();
+  };
+  if (fp64_tflops) {
+    const int iters = 4096;
+    CUDA_TRY(best_of([&] { mrd::fma_peak_kernel<double><<<blocks, threads, 0, s>>>(scratch, iters, 0.999999, 1e-7); }, 4, ms));
+    *fp64_tflops = 2.0 * 64.0 * iters * (double)blocks * threads / (ms * 1e-3) * 1e-12;
+  }
+  if (fp32_tflops) {
+    const int iters = 8192;
+    CUDA_TRY(best_of([&] { mrd::fma_peak_kernel<float><<<blocks, threads, 0, s>>>((float *)scratch, iters, 0.999999f, 1e-7f); }, 4, ms));
+    *fp32_tflops = 2.0 * 64.0 * iters * (double)blocks * threads / (ms * 1e-3) * 1e-12;
+  }
+  cudaFree(scratch);
+  if (copy_gbs) {
+    const int64_t n = (int64_t)1 << 26;  // 2 x 1 GiB
+    double2 *a = nullptr, *b = nullptr;
+    CUDA_TRY(cudaMalloc(&a, n * sizeof(double2)));
+    CUDA_TRY(cudaMalloc(&b, n * sizeof(double2)));
+    CUDA_TRY(cudaMemsetAsync(a, 0, n * sizeof(double2), s));
+    CUDA_TRY(best_of([&] { mrd::copy_kernel<<<prop.multiProcessorCount * 16, 256, 0, s>>>(a, b, n); }, 5, ms));
+    *copy_gbs = 2.0 * n * sizeof(double2) / (ms * 1e-3) * 1e-9;
+    cudaFree(a);
+    cudaFree(b);
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  return MRD_OK;
+}
+
+}  // extern "C"

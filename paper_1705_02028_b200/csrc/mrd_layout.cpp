@@ -1,0 +1,359 @@
+// mrd_layout.cpp -- host-side mesh-layout stage. See mrd_layout.h. No CUDA, no oracle code.
+#include "mrd_layout.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <numeric>
+
+namespace {
+
+inline double min_image(double d, double period) {
+  // PAPER.md L584 ("periodic boundaries are handled by the mesh"), reading C19
+  if (period > 0.0) {
+    if (d > 0.5 * period) d -= period;
+    else if (d < -0.5 * period) d += period;
+  }
+  return d;
+}
+inline int image_shift(double d, double period) {
+  if (period > 0.0) {
+    if (d > 0.5 * period) return -1;
+    if (d < -0.5 * period) return 1;
+  }
+  return 0;
+}
+
+// spread the low 21 bits of v so that there is one zero bit between consecutive bits
+inline uint64_t spread21(uint64_t v) {
+  v &= 0x1FFFFFull;
+  v = (v | (v << 16)) & 0x0000FFFF0000FFFFull;
+  v = (v | (v << 8)) & 0x00FF00FF00FF00FFull;
+  v = (v | (v << 4)) & 0x0F0F0F0F0F0F0F0Full;
+  v = (v | (v << 2)) & 0x3333333333333333ull;
+  v = (v | (v << 1)) & 0x5555555555555555ull;
+  return v;
+}
+// Morton (Z-order) key of a point, 21 bits per axis (L669-L675)
+inline uint64_t morton_key(double x, double y, const double lo[2], const double inv[2]) {
+  const double q = 2097151.0;  // 2^21 - 1
+  double fx = (x - lo[0]) * inv[0], fy = (y - lo[1]) * inv[1];
+  fx = std::min(std::max(fx, 0.0), 1.0);
+  fy = std::min(std::max(fy, 0.0), 1.0);
+  return spread21((uint64_t)(fx * q)) | (spread21((uint64_t)(fy * q)) << 1);
+}
+
+// stable LSD radix sort of `idx` by 48-bit `key`
+void radix_sort(std::vector<uint64_t> &key, std::vector<int32_t> &idx) {
+  const size_t n = key.size();
+  std::vector<uint64_t> key2(n);
+  std::vector<int32_t> idx2(n);
+  for (int pass = 0; pass < 6; ++pass) {
+    const int sh = 8 * pass;
+    size_t cnt[257] = {0};
+    for (size_t i = 0; i < n; ++i) cnt[((key[i] >> sh) & 0xFF) + 1]++;
+    if (cnt[((key[0] >> sh) & 0xFF) + 1] == n) continue;  // all digits equal: nothing to do
+    for (int b = 0; b < 256; ++b) cnt[b + 1] += cnt[b];
+    for (size_t i = 0; i < n; ++i) {
+      size_t d = cnt[(key[i] >> sh) & 0xFF]++;
+      key2[d] = key[i];
+      idx2[d] = idx[i];
+    }
+    key.swap(key2);
+    idx.swap(idx2);
+  }
+}
+
+}  // namespace
+
+namespace mrd_host {
+
+static void build_tile_plan(mrd_layout &L, const std::vector<double> &xyi);
+
+int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *xy, int64_t nt,
+                 const int32_t *tri, const uint8_t *vertex_flag, int64_t ne, const int32_t *wall_edge,
+                 std::string &err) {
+  if (!p || !xy || !tri || nv < 3 || nt < 1) { err = "null or empty mesh"; return MRD_EINVAL; }
+  if (nv > 0x7FFFFFF0ll || 3 * nt > 0x7FFFFFF0ll) { err = "mesh too large for 32-bit indices"; return MRD_EINVAL; }
+  if (!(p->gamma > 1.0) || !(p->cfl > 0.0)) { err = "gamma must be > 1 and cfl > 0"; return MRD_EINVAL; }
+  if (p->scheme < 0 || p->scheme > 2 || (p->time_order != 1 && p->time_order != 2)) { err = "bad scheme/time_order"; return MRD_EINVAL; }
+  if (p->precision != MRD_FP64 && p->precision != MRD_FP32) { err = "bad precision"; return MRD_EINVAL; }
+  if (p->period_x < 0.0 || p->period_y < 0.0) { err = "negative period"; return MRD_EINVAL; }
+  if (ne < 0 || (ne > 0 && !wall_edge)) { err = "bad wall edge list"; return MRD_EINVAL; }
+  if (p->tile < 0 || p->tile > 256 || (p->tile % 32) != 0) { err = "tile must be a multiple of 32, <= 256"; return MRD_EINVAL; }
+  L.p = *p;
+  L.nv = nv; L.nt = nt; L.ne = ne;
+  const double period[2] = {p->period_x, p->period_y};
+
+  // ---- validation + orientation fix in USER numbering ------------------------------------------
+  std::vector<int32_t> utri(tri, tri + 3 * nt);
+  std::vector<uint8_t> uswap(nt, 0);
+  std::vector<int32_t> deg(nv, 0);
+  for (int64_t t = 0; t < nt; ++t) {
+    int32_t *v = &utri[3 * t];
+    for (int j = 0; j < 3; ++j)
+      if (v[j] < 0 || v[j] >= nv) { err = "triangle index out of range"; return MRD_EINVAL; }
+    if (v[0] == v[1] || v[1] == v[2] || v[0] == v[2]) { err = "degenerate triangle"; return MRD_EINVAL; }
+    double x0 = xy[2 * v[0]], y0 = xy[2 * v[0] + 1];
+    double ax = min_image(xy[2 * v[1]] - x0, period[0]), ay = min_image(xy[2 * v[1] + 1] - y0, period[1]);
+    double bx = min_image(xy[2 * v[2]] - x0, period[0]), by = min_image(xy[2 * v[2] + 1] - y0, period[1]);
+    double cross = ax * by - ay * bx;
+    if (cross == 0.0 || !(cross == cross)) { err = "zero-area triangle"; return MRD_EINVAL; }
+    if (cross < 0.0) { std::swap(v[1], v[2]); uswap[t] = 1; }
+    for (int j = 0; j < 3; ++j) deg[v[j]]++;
+  }
+  for (int64_t i = 0; i < nv; ++i)
+    if (deg[i] == 0) { err = "vertex without triangle"; return MRD_EINVAL; }
+
+  // ---- Morton renumbering (L669-L675) ------------------------------------------------------------
+  L.vperm.resize(nv); L.vrank.resize(nv); L.tperm.resize(nt); L.trank.resize(nt);
+  std::iota(L.vperm.begin(), L.vperm.end(), 0);
+  std::iota(L.tperm.begin(), L.tperm.end(), 0);
+  if (p->reorder) {
+    double lo[2] = {xy[0], xy[1]}, hi[2] = {xy[0], xy[1]};
+    for (int64_t i = 0; i < nv; ++i)
+      for (int d = 0; d < 2; ++d) {
+        lo[d] = std::min(lo[d], xy[2 * i + d]);
+        hi[d] = std::max(hi[d], xy[2 * i + d]);
+      }
+    for (int d = 0; d < 2; ++d)
+      if (period[d] > 0.0) { lo[d] = 0.0; hi[d] = period[d]; }
+    // one common scale for both axes keeps the curve's cells square
+    double ext = std::max(hi[0] - lo[0], hi[1] - lo[1]);
+    double inv[2] = {ext > 0 ? 1.0 / ext : 0.0, ext > 0 ? 1.0 / ext : 0.0};
+    std::vector<uint64_t> key(nv);
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < nv; ++i) key[i] = morton_key(xy[2 * i], xy[2 * i + 1], lo, inv);
+    radix_sort(key, L.vperm);
+    key.assign(nt, 0);
+#pragma omp parallel for schedule(static)
+    for (int64_t t = 0; t < nt; ++t) {
+      const int32_t *v = &utri[3 * t];
+      double x0 = xy[2 * v[0]], y0 = xy[2 * v[0] + 1];
+      double cx = x0 + (min_image(xy[2 * v[1]] - x0, period[0]) + min_image(xy[2 * v[2]] - x0, period[0])) / 3.0;
+      double cy = y0 + (min_image(xy[2 * v[1] + 1] - y0, period[1]) + min_image(xy[2 * v[2] + 1] - y0, period[1])) / 3.0;
+      if (period[0] > 0.0) cx -= period[0] * std::floor(cx / period[0]);
+      if (period[1] > 0.0) cy -= period[1] * std::floor(cy / period[1]);
+      key[t] = morton_key(cx, cy, lo, inv);
+    }
+    radix_sort(key, L.tperm);
+  }
+  for (int64_t k = 0; k < nv; ++k) L.vrank[L.vperm[k]] = (int32_t)k;
+  for (int64_t k = 0; k < nt; ++k) L.trank[L.tperm[k]] = (int32_t)k;
+
+  // ---- internal connectivity, geometry (eq. 35), volumes (L441, C5) -------------------
+  L.tri.resize(3 * nt); L.tswap.resize(nt);
+  for (int i = 0; i < 3; ++i) { L.nx[i].resize(nt); L.ny[i].resize(nt); L.hl[i].resize(nt); }
+  L.area.resize(nt); L.lmax.resize(nt);
+  std::vector<double> xyi(2 * nv);
+#pragma omp parallel for schedule(static)
+  for (int64_t k = 0; k < nv; ++k) {
+    xyi[2 * k] = xy[2 * (int64_t)L.vperm[k]];
+    xyi[2 * k + 1] = xy[2 * (int64_t)L.vperm[k] + 1];
+  }
+#pragma omp parallel for schedule(static)
+  for (int64_t k = 0; k < nt; ++k) {
+    const int32_t *uv = &utri[3 * (int64_t)L.tperm[k]];
+    int32_t *v = &L.tri[3 * k];
+    for (int j = 0; j < 3; ++j) v[j] = L.vrank[uv[j]];
+    L.tswap[k] = uswap[L.tperm[k]];
+    double x[3][2];
+    x[0][0] = xyi[2 * v[0]]; x[0][1] = xyi[2 * v[0] + 1];
+    for (int j = 1; j < 3; ++j)
+      for (int d = 0; d < 2; ++d) x[j][d] = x[0][d] + min_image(xyi[2 * v[j] + d] - x[0][d], period[d]);
+    double lm = 0.0;
+    for (int i = 0; i < 3; ++i) {
+      // edge opposite node i runs from node i+1 to node i+2 (CCW); inward normal = (-e_y, e_x)
+      int a = (i + 1) % 3, b = (i + 2) % 3;
+      double ex = x[b][0] - x[a][0], ey = x[b][1] - x[a][1];
+      double l = std::sqrt(ex * ex + ey * ey);
+      L.nx[i][k] = -ey / l;
+      L.ny[i][k] = ex / l;
+      L.hl[i][k] = 0.5 * l;
+      lm = std::max(lm, l);
+    }
+    L.lmax[k] = lm;
+    L.area[k] = 0.5 * ((x[1][0] - x[0][0]) * (x[2][1] - x[0][1]) - (x[1][1] - x[0][1]) * (x[2][0] - x[0][0]));
+  }
+  L.vol.assign(nv, 0.0);
+  for (int64_t k = 0; k < nt; ++k)
+    for (int j = 0; j < 3; ++j) L.vol[L.tri[3 * k + j]] += L.area[k] / 3.0;
+
+  // ---- vertex -> (triangle, node) incidence, ascending (replaces the paper's atomics, L734) -------
+  L.csr_off.assign(nv + 1, 0);
+  for (int64_t e = 0; e < 3 * nt; ++e) L.csr_off[L.tri[e] + 1]++;
+  for (int64_t i = 0; i < nv; ++i) L.csr_off[i + 1] += L.csr_off[i];
+  L.csr_ent.resize(3 * nt);
+  {
+    std::vector<int32_t> cur(L.csr_off.begin(), L.csr_off.end() - 1);
+    for (int64_t e = 0; e < 3 * nt; ++e) L.csr_ent[cur[L.tri[e]]++] = (int32_t)e;
+  }
+
+  // ---- frozen vertices (L582) ---------------------------------------------------------------------
+  L.frozen.assign(nv, 0);
+  L.nf = 0;
+  if (vertex_flag)
+    for (int64_t k = 0; k < nv; ++k) {
+      L.frozen[k] = vertex_flag[L.vperm[k]] ? 1 : 0;
+      L.nf += L.frozen[k];
+    }
+
+  // ---- reflecting-wall edges (L586-L602; outward normal, reading C15) ------------------------------
+  L.wall_a.resize(ne); L.wall_b.resize(ne); L.wall_nx.resize(ne); L.wall_ny.resize(ne); L.wall_len.resize(ne);
+  for (int64_t e = 0; e < ne; ++e) {
+    int32_t ua = wall_edge[2 * e], ub = wall_edge[2 * e + 1];
+    if (ua < 0 || ua >= nv || ub < 0 || ub >= nv || ua == ub) { err = "bad wall edge"; return MRD_EINVAL; }
+    int32_t a = L.vrank[ua], b = L.vrank[ub];
+    int found = 0;
+    int64_t ft = -1;
+    int fa = 0, fb = 0;
+    for (int32_t q = L.csr_off[a]; q < L.csr_off[a + 1]; ++q) {
+      int64_t t = L.csr_ent[q] / 3;
+      for (int j = 0; j < 3; ++j)
+        if (L.tri[3 * t + j] == b) { ++found; ft = t; fa = L.csr_ent[q] % 3; fb = j; }
+    }
+    if (found != 1) { err = "wall edge must belong to exactly one triangle"; return MRD_EINVAL; }
+    int fc = 3 - fa - fb;
+    const int32_t *v = &L.tri[3 * ft];
+    double x[3][2];
+    x[0][0] = xyi[2 * v[0]]; x[0][1] = xyi[2 * v[0] + 1];
+    for (int j = 1; j < 3; ++j)
+      for (int d = 0; d < 2; ++d) x[j][d] = x[0][d] + min_image(xyi[2 * v[j] + d] - x[0][d], period[d]);
+    double ex = x[fb][0] - x[fa][0], ey = x[fb][1] - x[fa][1];
+    double len = std::sqrt(ex * ex + ey * ey);
+    double nx = ey / len, ny = -ex / len;
+    double mx = 0.5 * (x[fa][0] + x[fb][0]), my = 0.5 * (x[fa][1] + x[fb][1]);
+    if (nx * (x[fc][0] - mx) + ny * (x[fc][1] - my) > 0.0) { nx = -nx; ny = -ny; }  // point away from the third vertex
+    L.wall_a[e] = a; L.wall_b[e] = b; L.wall_nx[e] = nx; L.wall_ny[e] = ny; L.wall_len[e] = len;
+  }
+  {
+    // wall vertex -> (edge, side) lists, ascending
+    std::vector<std::pair<int32_t, int32_t>> inc;
+    inc.reserve(2 * ne);
+    for (int64_t e = 0; e < ne; ++e) {
+      inc.emplace_back(L.wall_a[e], (int32_t)(2 * e));
+      inc.emplace_back(L.wall_b[e], (int32_t)(2 * e + 1));
+    }
+    std::sort(inc.begin(), inc.end());
+    {  // the same edge given twice, in either orientation
+      std::vector<std::pair<int32_t, int32_t>> keys(ne);
+      for (int64_t e = 0; e < ne; ++e) keys[e] = {std::min(L.wall_a[e], L.wall_b[e]), std::max(L.wall_a[e], L.wall_b[e])};
+      std::sort(keys.begin(), keys.end());
+      for (int64_t e = 1; e < ne; ++e)
+        if (keys[e] == keys[e - 1]) { err = "duplicate wall edge"; return MRD_EINVAL; }
+    }
+    L.wv_vertex.clear(); L.wv_off.assign(1, 0); L.wv_ent.clear();
+    for (size_t q = 0; q < inc.size(); ++q) {
+      if (q == 0 || inc[q].first != inc[q - 1].first) {
+        if (q) L.wv_off.push_back((int32_t)L.wv_ent.size());
+        L.wv_vertex.push_back(inc[q].first);
+      }
+      L.wv_ent.push_back(inc[q].second);
+    }
+    if (!inc.empty()) L.wv_off.push_back((int32_t)L.wv_ent.size());
+  }
+
+  L.tile = p->tile;
+  if (L.tile > 0) build_tile_plan(L, xyi);
+  return MRD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Tile plan: tile b = internal triangles [b*tile, (b+1)*tile).  A "slot" is one (vertex, periodic image)
+// pair used by the tile; every slot carries the vertex coordinates unwrapped into the tile's frame, so the
+// fused kernel needs no minimum-image arithmetic, and receives one partial sum per stage.
+// ---------------------------------------------------------------------------------------------------
+static void build_tile_plan(mrd_layout &L, const std::vector<double> &xyi) {
+  const int64_t nt = L.nt, nv = L.nv;
+  const int T = L.tile;
+  const double period[2] = {L.p.period_x, L.p.period_y};
+  const int64_t ntile = (nt + T - 1) / T;
+  L.ntile = ntile;
+  L.tile_tri.assign((size_t)ntile * T * 4, 0);
+  std::vector<int32_t> nslot_of(ntile + 1, 0);
+  // pass 1 (parallel): per tile the sorted unique keys, local ids of every node
+  std::vector<std::vector<int64_t>> keys(ntile);
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t b = 0; b < ntile; ++b) {
+    const int64_t t0 = b * T, t1 = std::min(nt, t0 + T);
+    const int32_t anchor = L.tri[3 * t0];
+    const double ax = xyi[2 * anchor], ay = xyi[2 * anchor + 1];
+    int64_t nodekey[256 * 3];
+    std::vector<int64_t> &uk = keys[b];
+    uk.reserve(3 * (t1 - t0));
+    for (int64_t t = t0; t < t1; ++t) {
+      const int32_t *v = &L.tri[3 * t];
+      const double x0 = xyi[2 * v[0]], y0 = xyi[2 * v[0] + 1];
+      const int tsx = image_shift(x0 - ax, period[0]), tsy = image_shift(y0 - ay, period[1]);
+      for (int j = 0; j < 3; ++j) {
+        int sx = tsx, sy = tsy;
+        if (j) {
+          sx += image_shift(xyi[2 * v[j]] - x0, period[0]);
+          sy += image_shift(xyi[2 * v[j] + 1] - y0, period[1]);
+        }
+        int64_t key = (int64_t)v[j] * 25 + (sx + 2) * 5 + (sy + 2);
+        nodekey[3 * (t - t0) + j] = key;
+        uk.push_back(key);
+      }
+    }
+    std::sort(uk.begin(), uk.end());
+    uk.erase(std::unique(uk.begin(), uk.end()), uk.end());
+    nslot_of[b + 1] = (int32_t)uk.size();
+    for (int64_t t = t0; t < t1; ++t)
+      for (int j = 0; j < 3; ++j) {
+        int64_t key = nodekey[3 * (t - t0) + j];
+        int loc = (int)(std::lower_bound(uk.begin(), uk.end(), key) - uk.begin());
+        L.tile_tri[((size_t)b * T + (t - t0)) * 4 + j] = (uint16_t)loc;
+      }
+  }
+  L.tile_slot_off.assign(ntile + 1, 0);
+  for (int64_t b = 0; b < ntile; ++b) L.tile_slot_off[b + 1] = L.tile_slot_off[b] + nslot_of[b + 1];
+  const int64_t nslot = L.tile_slot_off[ntile];
+  L.nslot = nslot;
+  L.slot_vertex.resize(nslot);
+  L.slot_xy.resize(2 * nslot);
+  L.slot_ent_off.assign(nslot + 1, 0);
+  L.slot_ent.resize(3 * nt);
+  // pass 2: slot records and per-slot incidence counts
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t b = 0; b < ntile; ++b) {
+    const int64_t t0 = b * T, t1 = std::min(nt, t0 + T);
+    const int32_t s0 = L.tile_slot_off[b];
+    const std::vector<int64_t> &uk = keys[b];
+    for (size_t q = 0; q < uk.size(); ++q) {
+      int32_t v = (int32_t)(uk[q] / 25);
+      int r = (int)(uk[q] % 25);
+      int sx = r / 5 - 2, sy = r % 5 - 2;
+      L.slot_vertex[s0 + q] = v;
+      L.slot_xy[2 * (s0 + q)] = xyi[2 * v] + sx * period[0];
+      L.slot_xy[2 * (s0 + q) + 1] = xyi[2 * v + 1] + sy * period[1];
+    }
+    for (int64_t t = t0; t < t1; ++t)
+      for (int j = 0; j < 3; ++j) L.slot_ent_off[s0 + L.tile_tri[((size_t)b * T + (t - t0)) * 4 + j] + 1]++;
+  }
+  for (int64_t s = 0; s < nslot; ++s) L.slot_ent_off[s + 1] += L.slot_ent_off[s];
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t b = 0; b < ntile; ++b) {
+    const int64_t t0 = b * T, t1 = std::min(nt, t0 + T);
+    const int32_t s0 = L.tile_slot_off[b];
+    const int ns = L.tile_slot_off[b + 1] - s0;
+    std::vector<int32_t> cur(ns);
+    for (int q = 0; q < ns; ++q) cur[q] = L.slot_ent_off[s0 + q];
+    for (int64_t t = t0; t < t1; ++t)
+      for (int j = 0; j < 3; ++j) {
+        int loc = L.tile_tri[((size_t)b * T + (t - t0)) * 4 + j];
+        L.slot_ent[cur[loc]++] = (uint16_t)((t - t0) * 4 + j);
+      }
+  }
+  // vertex -> slots, ascending (slots are tile-major, so this is ascending triangle order)
+  L.vslot_off.assign(nv + 1, 0);
+  for (int64_t s = 0; s < nslot; ++s) L.vslot_off[L.slot_vertex[s] + 1]++;
+  for (int64_t i = 0; i < nv; ++i) L.vslot_off[i + 1] += L.vslot_off[i];
+  L.vslot_ent.resize(nslot);
+  {
+    std::vector<int32_t> cur(L.vslot_off.begin(), L.vslot_off.end() - 1);
+    for (int64_t s = 0; s < nslot; ++s) L.vslot_ent[cur[L.slot_vertex[s]]++] = (int32_t)s;
+  }
+}
+
+}  // namespace mrd_host

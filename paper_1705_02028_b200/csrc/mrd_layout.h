@@ -1,0 +1,48 @@
+// mrd_layout.h -- host-side mesh-layout stage: orientation fix, minimum-image
+// unwrap, Morton renumbering, vertex -> incident-triangle CSR (new: the paper
+// had no such map and used atomics, L734), triangle geometry (eq. 35-37), dual volumes
+// V_i (L441, reading C5), wall-edge and frozen-vertex lists (L580-L602), and the tile plan of the
+// fused kernels.  Plain C++17, no CUDA.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/mrd.h"
+
+struct mrd_layout {
+  mrd_params p{};
+  int64_t nv = 0, nt = 0, ne = 0, nf = 0;
+  // renumbering: internal k <-> user index
+  std::vector<int32_t> vperm, vrank;  // vperm[k] = user vertex of internal k; vrank = inverse
+  std::vector<int32_t> tperm, trank;
+  std::vector<uint8_t> tswap;         // [nt] internal: 1 = user nodes 2 and 3 were swapped (CCW fix)
+  std::vector<int32_t> tri;           // [nt][3] internal vertex ids, CCW
+  std::vector<int32_t> csr_off, csr_ent;  // [nv+1], [3 nt]: entries tri*3+node ascending
+  // geometry, internal triangle order (double; cast to the sweep precision at upload)
+  std::vector<double> nx[3], ny[3], hl[3];  // unit inward normals, half edge lengths
+  std::vector<double> area, lmax;           // |T|, longest edge
+  std::vector<double> vol;                  // [nv] V_i
+  std::vector<uint8_t> frozen;              // [nv] internal
+  // reflecting-wall edges (internal vertex ids) with OUTWARD unit normal and length (reading C15)
+  std::vector<int32_t> wall_a, wall_b;
+  std::vector<double> wall_nx, wall_ny, wall_len;
+  // wall vertex -> (edge*2 + side) incidence, ascending; side 0 = vertex is `a`, 1 = `b`
+  std::vector<int32_t> wv_vertex, wv_off, wv_ent;
+  // ---- tile plan of the fused kernels ----
+  int32_t tile = 0;                    // triangles per tile (0: no plan built)
+  int64_t ntile = 0, nslot = 0;
+  std::vector<int32_t> tile_slot_off;  // [ntile+1]: first slot of each tile
+  std::vector<int32_t> slot_vertex;    // [nslot]: internal vertex of each (tile-local vertex) slot
+  std::vector<double> slot_xy;         // [nslot][2]: coordinates unwrapped into the tile's frame
+  std::vector<uint16_t> tile_tri;      // [ntile*tile][4]: tile-local vertex of nodes 0..2 (+ pad)
+  std::vector<int32_t> slot_ent_off;   // [nslot+1]: tile-local incidence of each slot ...
+  std::vector<uint16_t> slot_ent;      // ... entries (local triangle)*4 + node, ascending
+  std::vector<int32_t> vslot_off, vslot_ent;  // vertex -> its slots, ascending: [nv+1], [nslot]
+};
+
+namespace mrd_host {
+int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *xy, int64_t nt,
+                 const int32_t *tri, const uint8_t *vertex_flag, int64_t ne, const int32_t *wall_edge,
+                 std::string &err);
+}

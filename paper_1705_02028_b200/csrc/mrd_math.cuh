@@ -1,0 +1,319 @@
+// mrd_math.cuh -- per-triangle and per-vertex arithmetic of the residual-distribution sweep (device).
+//
+// Written from PAPER.md (arXiv:1705.02028); shares nothing with oracle/.  Templated on the scalar
+// R = double | float.  The formulation is the exact similarity transform of the paper's matrices
+// into the symmetrising variables dQ = (dp/c, du, dv, dp - c^2 drho) (unit reference density), in
+// which K_i = (l_i/2) [[w, c n^T, 0], [c n, w I, 0], [0, 0, w]]:
+//   - K_i^(+/-) (eq. 40-42; App. A eq. A10-A25) are applied as characteristic
+//     projections with a = (l1+l2)/2, b = (l1-l2)/2 (the paper's l_12) and a - l3 (its l_123);
+//   - sum_j K_j^- becomes a symmetric 3x3 block plus the entropy scalar, so N-hat (eq. 49)
+//     is a 3x3 cofactor inverse and a reciprocal; the stagnation rule C8 is the scalar's 0/0 -> 0;
+//   - residuals are mapped back to conserved variables before the blend of eq. 52-53 (L493-L503),
+//     which is defined per conserved component.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace mrd {
+
+// ---------------------------------------------------------------------------------------------
+// scalar helpers: reciprocal / reciprocal square root by hardware seed + Newton steps (the fp64
+// division and sqrt of CUDA are IEEE-rounded subroutine calls; 1-2 ulp is enough here, see
+// DESIGN.md "Tolerance").  Arguments are positive and normal wherever these are used.
+// ---------------------------------------------------------------------------------------------
+template <class R> struct Fast;
+
+template <> struct Fast<double> {
+  static __device__ __forceinline__ double rcp(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    return r;
+  }
+  static __device__ __forceinline__ double rsqrt(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double hx = 0.5 * x;
+    double e = fma(-hx * y, y, 0.5);
+    y = fma(y, e, y);
+    e = fma(-hx * y, y, 0.5);
+    y = fma(y, e, y);
+    return y;
+  }
+  // sqrt(x) for x >= 0 (exactly 0 for x = 0), given nothing else
+  static __device__ __forceinline__ double sqrt0(double x) {
+    if (!(x > 0.0)) return 0.0;
+    double y = rsqrt(x);
+    double s = x * y;
+    double r = fma(-s, s, x);
+    return fma(r, 0.5 * y, s);
+  }
+  static __device__ __forceinline__ double abs(double x) { return fabs(x); }
+  static __device__ __forceinline__ double max(double a, double b) { return fmax(a, b); }
+  static __device__ __forceinline__ double min(double a, double b) { return fmin(a, b); }
+  static __device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
+};
+
+template <> struct Fast<float> {
+  static __device__ __forceinline__ float rcp(float x) { return __frcp_rn(x); }
+  static __device__ __forceinline__ float rsqrt(float x) { return rsqrtf(x); }
+  static __device__ __forceinline__ float sqrt0(float x) { return x > 0.0f ? __fsqrt_rn(x) : 0.0f; }
+  static __device__ __forceinline__ float abs(float x) { return fabsf(x); }
+  static __device__ __forceinline__ float max(float a, float b) { return fmaxf(a, b); }
+  static __device__ __forceinline__ float min(float a, float b) { return fminf(a, b); }
+  static __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+};
+
+template <class R> struct Vec4 { R x, y, z, w; };
+template <> struct __align__(32) Vec4<double> { double x, y, z, w; };
+template <> struct __align__(16) Vec4<float> { float x, y, z, w; };
+
+template <class R> __device__ __forceinline__ Vec4<R> ld4(const Vec4<R> *p) {
+  return *p;
+}
+template <> __device__ __forceinline__ Vec4<double> ld4<double>(const Vec4<double> *p) {
+  const double2 *q = reinterpret_cast<const double2 *>(p);
+  double2 a = __ldg(q), b = __ldg(q + 1);
+  return Vec4<double>{a.x, a.y, b.x, b.y};
+}
+template <> __device__ __forceinline__ Vec4<float> ld4<float>(const Vec4<float> *p) {
+  float4 a = __ldg(reinterpret_cast<const float4 *>(p));
+  return Vec4<float>{a.x, a.y, a.z, a.w};
+}
+template <class R> __device__ __forceinline__ void st4(Vec4<R> *p, const Vec4<R> &v);
+template <> __device__ __forceinline__ void st4<double>(Vec4<double> *p, const Vec4<double> &v) {
+  double2 *q = reinterpret_cast<double2 *>(p);
+  q[0] = make_double2(v.x, v.y);
+  q[1] = make_double2(v.z, v.w);
+}
+template <> __device__ __forceinline__ void st4<float>(Vec4<float> *p, const Vec4<float> &v) {
+  *reinterpret_cast<float4 *>(p) = make_float4(v.x, v.y, v.z, v.w);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Per-vertex quantities: parameter vector Z = sqrt(rho) (1, u, v, h) (eq. 20
+// L290-L294 and its 2D analogue L419, reading C1) with p from eq. 10 (L224), and the signal speed
+// |v| + c, c^2 = gamma p / rho, of eq. 45 (L447-L449, reading C14).  Returns false when rho <= 0
+// or p <= 0.
+// ---------------------------------------------------------------------------------------------
+template <class R>
+__device__ __forceinline__ bool vertex_prepare(R gamma, const Vec4<R> &W, Vec4<R> &Z, R &speed, R &p_out) {
+  using F = Fast<R>;
+  const R g1 = gamma - R(1);
+  R rho = W.x;
+  bool ok = rho > R(0);
+  R rs = ok ? rho : R(1);
+  R ir = F::rcp(rs);
+  R u = W.y * ir, v = W.z * ir;
+  R ke2 = W.y * u + W.z * v;  // rho (u^2 + v^2)
+  R p = g1 * (W.w - R(0.5) * ke2);
+  p_out = p;
+  ok = ok && (p > R(0));
+  R ps = ok ? p : R(1);
+  R h = (W.w + ps) * ir;
+  R isr = F::rsqrt(rs);
+  R s = rs * isr;  // sqrt(rho)
+  s = F::fma_(F::fma_(-s, s, rs), R(0.5) * isr, s);
+  Z.x = s;
+  Z.y = s * u;
+  Z.z = s * v;
+  Z.w = s * h;
+  speed = F::sqrt0(u * u + v * v) + F::sqrt0(gamma * ps * ir);
+  return ok;
+}
+
+// ---------------------------------------------------------------------------------------------
+// One triangle at one state: everything the distribution needs.
+// ---------------------------------------------------------------------------------------------
+template <class R> struct TriGeom {
+  R nx[3], ny[3];  // unit inward normal of the edge opposite node i (eq. 35; reading C4)
+  R hl[3];         // l_i / 2 (eq. 37 with d = 2)
+};
+
+template <class R> struct TriCore {
+  // linearised state (eq. 39)
+  R u, v, hq2 /* (u^2+v^2)/2 */, c, c2, ic /* 1/c */, ic2, cg /* c/(gamma-1) */;
+  // positive parts per edge: a+ = (l1+ + l2+)/2, b+ = (l1+ - l2+)/2, l3+
+  R ap[3], bp[3], l3p[3];
+  // N-hat (eq. 49): symmetric 3x3 inverse (00,01,02,11,12,22) and the entropy reciprocal
+  R n00, n01, n02, n11, n12, n22, ns;
+  bool ok;
+};
+
+// y = K x in the rotated frame of edge (nx, ny) with coefficients (a, b, l3):
+//   y0 = a x0 + b xn,  yn = b x0 + a xn,  yt = l3 xt,  y3 = l3 x3  -> accumulated into acc (sign s)
+template <class R>
+__device__ __forceinline__ void apply_split(R a, R b, R l3, R nx, R ny, const R x[4], R acc[4]) {
+  R xn = nx * x[1] + ny * x[2];
+  R xt = nx * x[2] - ny * x[1];
+  R y0 = a * x[0] + b * xn;
+  R yn = b * x[0] + a * xn;
+  R yt = l3 * xt;
+  acc[0] += y0;
+  acc[1] += nx * yn - ny * yt;
+  acc[2] += ny * yn + nx * yt;
+  acc[3] += l3 * x[3];
+}
+
+// symmetrising variables -> conserved variables (unit reference density)
+template <class R> __device__ __forceinline__ void to_conserved(const TriCore<R> &k, const R q[4], R w[4]) {
+  R drho = (k.c * q[0] - q[3]) * k.ic2;
+  w[0] = drho;
+  w[1] = k.u * drho + q[1];
+  w[2] = k.v * drho + q[2];
+  w[3] = k.cg * q[0] + k.hq2 * drho + k.u * q[1] + k.v * q[2];
+}
+// conserved -> symmetrising
+template <class R> __device__ __forceinline__ void to_symmetrising(R g1, const TriCore<R> &k, const R w[4], R q[4]) {
+  R dp = g1 * (w[3] - k.u * w[1] - k.v * w[2] + k.hq2 * w[0]);
+  q[0] = dp * k.ic;
+  q[1] = w[1] - k.u * w[0];
+  q[2] = w[2] - k.v * w[0];
+  q[3] = dp - k.c2 * w[0];
+}
+
+// S2-S5: from the three parameter vectors and the geometry to phi^T (eq. 36) and phi_i^N (eq. 48),
+// both in conserved variables; `k` keeps what beta_i = -K_i^+ N-hat (eq. 51) needs.
+template <class R>
+__device__ __forceinline__ void triangle_core(R gamma, const Vec4<R> Z[3], const TriGeom<R> &g, TriCore<R> &k,
+                                              R phiT[4], R phiN[3][4]) {
+  using F = Fast<R>;
+  const R g1 = gamma - R(1);
+  const R third = R(1) / R(3);
+  // eq. 39: Zbar, and u, v, h, c of the linearised state
+  R zb0 = (Z[0].x + Z[1].x + Z[2].x) * third;
+  R zb1 = (Z[0].y + Z[1].y + Z[2].y) * third;
+  R zb2 = (Z[0].z + Z[1].z + Z[2].z) * third;
+  R zb3 = (Z[0].w + Z[1].w + Z[2].w) * third;
+  R iz = F::rcp(zb0);
+  k.u = zb1 * iz;
+  k.v = zb2 * iz;
+  R h = zb3 * iz;
+  k.hq2 = R(0.5) * (k.u * k.u + k.v * k.v);
+  R c2 = g1 * (h - k.hq2);
+  k.ok = c2 > R(0);
+  c2 = k.ok ? c2 : R(1);
+  k.c2 = c2;
+  k.ic = F::rsqrt(c2);
+  k.c = c2 * k.ic;
+  k.ic2 = k.ic * k.ic;
+  k.cg = k.c / g1;
+
+  // O3 (reading C3): delta_j = D(Zbar)(Z_j - Z_0) mapped to symmetrising variables; the composition is
+  //   drho = 2 zb0 d0, du = zb0 d1 - zb1 d0, dv = zb0 d2 - zb2 d0,
+  //   dp = (g1/gamma) (zb3 d0 + zb0 d3 - zb1 d1 - zb2 d2)
+  // (exactly zero when Z_j == Z_0, so uniform flow has zero residual, L237)
+  const R gg = g1 / gamma;
+  R dq[3][4];
+  dq[0][0] = dq[0][1] = dq[0][2] = dq[0][3] = R(0);
+#pragma unroll
+  for (int j = 1; j < 3; ++j) {
+    R d0 = Z[j].x - Z[0].x, d1 = Z[j].y - Z[0].y, d2 = Z[j].z - Z[0].z, d3 = Z[j].w - Z[0].w;
+    R dp = gg * (zb3 * d0 + zb0 * d3 - zb1 * d1 - zb2 * d2);
+    R drho = R(2) * zb0 * d0;
+    dq[j][0] = dp * k.ic;
+    dq[j][1] = zb0 * d1 - zb1 * d0;
+    dq[j][2] = zb0 * d2 - zb2 * d0;
+    dq[j][3] = dp - c2 * drho;
+  }
+
+  // O4: per edge the split eigenvalues (eq. 41-42) and the sums over edges
+  R s00 = 0, s01 = 0, s02 = 0, s11 = 0, s12 = 0, s22 = 0, s33 = 0;
+  R accm[4] = {0, 0, 0, 0};   // sum_j K_j^- dq_j
+  R phiq[4] = {0, 0, 0, 0};   // sum_j K_j dq_j = phi^T (eq. 36)
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    R nx = g.nx[i], ny = g.ny[i], hl = g.hl[i];
+    R wl = hl * (k.u * nx + k.v * ny);
+    R cl = hl * k.c;
+    R l1 = wl + cl, l2 = wl - cl, l3 = wl;
+    R l1p = R(0.5) * (l1 + F::abs(l1)), l2p = R(0.5) * (l2 + F::abs(l2)), l3p = R(0.5) * (l3 + F::abs(l3));
+    R l1m = l1 - l1p, l2m = l2 - l2p, l3m = l3 - l3p;
+    R ap = R(0.5) * (l1p + l2p), bp = R(0.5) * (l1p - l2p);
+    R am = R(0.5) * (l1m + l2m), bm = R(0.5) * (l1m - l2m);
+    k.ap[i] = ap;
+    k.bp[i] = bp;
+    k.l3p[i] = l3p;
+    R nxx = nx * nx, nyy = ny * ny, nxy = nx * ny;
+    s00 += am;
+    s01 += bm * nx;
+    s02 += bm * ny;
+    s11 += am * nxx + l3m * nyy;
+    s12 += (am - l3m) * nxy;
+    s22 += am * nyy + l3m * nxx;
+    s33 += l3m;
+    if (i > 0) {
+      apply_split(am, bm, l3m, nx, ny, dq[i], accm);
+      apply_split(wl, cl, wl, nx, ny, dq[i], phiq);
+    }
+  }
+
+  // O5: N-hat = (sum K^-)^-1: cofactor inverse of the symmetric 3x3 block, reciprocal of the entropy
+  // scalar; stagnation rule (reading C8): u^2 + v^2 <= (1e-14 c)^2 -> entropy part of N-hat = 0
+  R c00 = s11 * s22 - s12 * s12;
+  R c01 = s02 * s12 - s01 * s22;
+  R c02 = s01 * s12 - s02 * s11;
+  R c11 = s00 * s22 - s02 * s02;
+  R c12 = s01 * s02 - s00 * s12;
+  R c22 = s00 * s11 - s01 * s01;
+  R det = s00 * c00 + s01 * c01 + s02 * c02;
+  R idet = F::rcp(det);  // det < 0 (negative definite block); rcp seeds handle the sign
+  k.n00 = c00 * idet; k.n01 = c01 * idet; k.n02 = c02 * idet;
+  k.n11 = c11 * idet; k.n12 = c12 * idet; k.n22 = c22 * idet;
+  const R eps = R(1e-14);
+  bool stagnant = (R(2) * k.hq2 <= (eps * eps) * c2) || !(s33 < R(0));
+  k.ns = stagnant ? R(0) : F::rcp(stagnant ? R(-1) : s33);
+
+  // eq. 48: phi_i^N = K_i^+ (dq_i - N-hat sum_j K_j^- dq_j)
+  R win[4];
+  win[0] = k.n00 * accm[0] + k.n01 * accm[1] + k.n02 * accm[2];
+  win[1] = k.n01 * accm[0] + k.n11 * accm[1] + k.n12 * accm[2];
+  win[2] = k.n02 * accm[0] + k.n12 * accm[1] + k.n22 * accm[2];
+  win[3] = k.ns * accm[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    R d[4] = {dq[i][0] - win[0], dq[i][1] - win[1], dq[i][2] - win[2], dq[i][3] - win[3]};
+    R y[4] = {0, 0, 0, 0};
+    apply_split(k.ap[i], k.bp[i], k.l3p[i], g.nx[i], g.ny[i], d, y);
+    to_conserved(k, y, phiN[i]);
+  }
+  to_conserved(k, phiq, phiT);
+}
+
+// eq. 50-51: out_i = beta_i X = -K_i^+ N-hat X for a conserved-variable vector X (phi^T in stage 1,
+// Phi^T in stage 2: eq. 63 with eq. 65, reading C12)
+template <class R>
+__device__ __forceinline__ void apply_beta(R gamma, const TriCore<R> &k, const TriGeom<R> &g, const R X[4], R out[3][4]) {
+  R q[4];
+  to_symmetrising(gamma - R(1), k, X, q);
+  R y[4];
+  y[0] = -(k.n00 * q[0] + k.n01 * q[1] + k.n02 * q[2]);
+  y[1] = -(k.n01 * q[0] + k.n11 * q[1] + k.n12 * q[2]);
+  y[2] = -(k.n02 * q[0] + k.n12 * q[1] + k.n22 * q[2]);
+  y[3] = -(k.ns * q[3]);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    R z[4] = {0, 0, 0, 0};
+    apply_split(k.ap[i], k.bp[i], k.l3p[i], g.nx[i], g.ny[i], y, z);
+    to_conserved(k, z, out[i]);
+  }
+}
+
+// eq. 52-53 (+ reading C10): Theta_kk = min(1, |X_k| / sum_j |N_j,k|), 0 when the denominator is 0;
+// B_i = Theta N_i + (1 - Theta) LDA_i, written over N.
+template <class R> __device__ __forceinline__ void blend(const R X[4], R N[3][4], const R L[3][4]) {
+  using F = Fast<R>;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    R den = F::abs(N[0][c]) + F::abs(N[1][c]) + F::abs(N[2][c]);
+    bool pos = den > R(0);
+    R th = F::min(R(1), F::abs(X[c]) * F::rcp(pos ? den : R(1)));
+    th = pos ? th : R(0);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) N[i][c] = L[i][c] + th * (N[i][c] - L[i][c]);
+  }
+}
+
+}  // namespace mrd

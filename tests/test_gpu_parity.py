@@ -1,0 +1,248 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by element on
+the same seeded inputs.  Tolerances (BASELINE.json north_star, reading C17):
+fp64 max relative field error <= 1e-12 after 1 step and <= 1e-9 after 100 steps; fp32 <= 1e-5 after
+10 steps against the fp64 oracle."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+from helpers import field_errors
+
+pytestmark = pytest.mark.gpu
+
+TOL_1 = 1e-12
+TOL_100 = 1e-9
+TOL_F32 = 1e-5
+
+
+@pytest.fixture(scope="module")
+def mrd():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_1705_02028_b200 as m
+    return m
+
+
+def gpu_mesh(mrd, cfg_or_mesh, W, **kw):
+    import torch
+    mesh = cfg_or_mesh
+    gm = mrd.Mesh(mesh.xy, mesh.tri, period=mesh.period, **kw)
+    dt = torch.float64 if kw.get("precision", 0) == 0 else torch.float32
+    gm.set_state(torch.tensor(W, dtype=dt, device="cuda"))
+    return gm
+
+
+def orc_mesh(mesh, W, **kw):
+    om = oracle.OracleMesh(mesh.xy, mesh.tri, period=mesh.period, **kw)
+    om.set_state(W)
+    return om
+
+
+def rel(a, b):
+    s = np.abs(b).max()
+    return np.abs(a - b).max() / (s if s > 0 else 1.0)
+
+
+# ------------------------------------------------------------------------------------------------
+# per-triangle quantities
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("case", ["smooth_jitter", "vortex", "kh_permuted", "supersonic"])
+@pytest.mark.parametrize("tile", [0, 128])
+def test_stage1_per_triangle_matches_oracle(mrd, case, tile):
+    if case == "smooth_jitter":
+        mesh = wl.jitter_mesh(wl.uniform_mesh(37, 29, 2.0, 1.5, periodic=True), 0.22, seed=3)
+        W = wl.random_smooth_state(mesh, mach=0.7, seed=1)
+    elif case == "vortex":
+        mesh = wl.uniform_mesh(48, 48, 10.0, 10.0, periodic=True)
+        W = wl.vortex_state(mesh)
+    elif case == "kh_permuted":
+        mesh = wl.permute_mesh(wl.uniform_mesh(40, 40, 1.0, 1.0, periodic=True), 12345)[0]
+        W = wl.kelvin_helmholtz_state(mesh)
+    else:
+        mesh = wl.jitter_mesh(wl.uniform_mesh(30, 31, 1.0, 1.0, periodic=True), 0.15, seed=8)
+        W = wl.random_smooth_state(mesh, mach=2.5, seed=5)
+    g = gpu_mesh(mrd, mesh, W, tile=tile).dump_stage1()
+    o = orc_mesh(mesh, W).dump_stage1()
+    scale = np.abs(o["phiN"]).max()
+    for key in ("phiT", "phiN", "phiLDA", "phiB"):
+        assert np.abs(g[key] - o[key]).max() <= 2e-13 * scale, key
+    assert np.allclose(g["sT"], o["sT"], rtol=1e-14, atol=0)
+
+
+def test_uniform_flow_has_exactly_zero_residual_and_state_is_bitwise_kept(mrd):
+    mesh = wl.jitter_mesh(wl.uniform_mesh(24, 20, 3.0, 2.0, periodic=True), 0.25, seed=5)
+    for prim in [(1.3, 0.4, -0.7, 2.1), (1.0, 0.0, 0.0, 1.0), (0.2, 2.5, 1.0, 0.1)]:
+        W = wl.uniform_state(mesh, *prim)
+        for scheme, order in [(2, 2), (0, 1), (1, 2)]:
+            gm = gpu_mesh(mrd, mesh, W, scheme=scheme, time_order=order)
+            d = gm.dump_stage1()
+            assert np.all(d["phiB"] == 0.0) and np.all(d["phiN"] == 0.0) and np.all(d["phiT"] == 0.0)
+            gm.step(5)
+            assert np.array_equal(gm.get_state().cpu().numpy(), W)
+
+
+# ------------------------------------------------------------------------------------------------
+# whole steps
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("scheme,order", [(2, 2), (0, 1), (1, 2), (0, 2), (2, 1)])
+@pytest.mark.parametrize("reorder", [True, False])
+@pytest.mark.parametrize("tile", [0, 128])
+def test_one_step_and_many_steps_match_oracle(mrd, scheme, order, reorder, tile):
+    mesh = wl.jitter_mesh(wl.uniform_mesh(33, 27, 1.0, 1.0, periodic=True), 0.2, seed=11)
+    W = wl.random_smooth_state(mesh, mach=1.2, seed=4)
+    gm = gpu_mesh(mrd, mesh, W, scheme=scheme, time_order=order, reorder=reorder, tile=tile)
+    om = orc_mesh(mesh, W, scheme=scheme, time_order=order)
+    n, t, dt = gm.step(1)
+    no, to, dto = om.step(1)
+    assert n == 1 and abs(dt - dto) <= 1e-14 * dto
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_1
+    gm.step(99)
+    om.step(99)
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_100
+    assert abs(gm.sync()[1] - om.step(0)[1]) <= 1e-11
+
+
+def test_config1_vortex_10_steps(mrd):
+    cfg = wl.make_config("vortex")
+    gm = gpu_mesh(mrd, cfg.mesh, cfg.W0)
+    om = orc_mesh(cfg.mesh, cfg.W0)
+    for _ in range(10):
+        gm.step(1)
+        om.step(1)
+        assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= 10 * TOL_1
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= 1e-11
+
+
+def test_config2_sod_walls_frozen_and_t_end(mrd):
+    cfg = wl.make_config("sod", n=256)
+    kw = dict(vertex_flag=cfg.vertex_flag, wall_edge=cfg.wall_edge)
+    gm = gpu_mesh(mrd, cfg.mesh, cfg.W0, **kw)
+    om = orc_mesh(cfg.mesh, cfg.W0, **kw)
+    gm.step(1)
+    om.step(1)
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_1
+    n, t, _ = gm.step(100000, t_end=0.05)
+    no, to, _ = om.step(100000, t_end=0.05)
+    assert abs(n - no) <= 1 and t == 0.05 and abs(to - 0.05) < 1e-15
+    Wg, Wo = gm.get_state().cpu().numpy(), om.get_state()
+    assert field_errors(Wg, Wo) <= TOL_100
+    frozen = cfg.vertex_flag.astype(bool)
+    assert np.array_equal(Wg[:, frozen], cfg.W0[:, frozen])
+
+
+def test_oblique_wall_terms_match_oracle(mrd):
+    # flow not aligned with the walls: the correction of eq. 68-71 is non-zero
+    mesh = wl.uniform_mesh(24, 12, 2.0, 1.0, periodic=False)
+    W = wl.random_smooth_state(mesh, mach=0.6, seed=9)
+    kw = dict(vertex_flag=wl.boundary_vertices(mesh, True, False), wall_edge=wl.wall_edges_y(mesh))
+    for reorder in (True, False):
+        gm = gpu_mesh(mrd, mesh, W, reorder=reorder, **kw)
+        om = orc_mesh(mesh, W, **kw)
+        gm.step(1)
+        om.step(1)
+        assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_1
+        gm.step(30)
+        om.step(30)
+        assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_100
+
+
+def test_config3_kh_permuted_fp64_and_fp32(mrd):
+    cfg = wl.make_config("kh", n=128)
+    om = orc_mesh(cfg.mesh, cfg.W0)
+    for reorder in (True, False):
+        gm = gpu_mesh(mrd, cfg.mesh, cfg.W0, reorder=reorder)
+        om.set_state(cfg.W0)
+        gm.step(1)
+        om.step(1)
+        assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_1
+        gm.step(99)
+        om.step(99)
+        assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_100
+    om.set_state(cfg.W0)
+    g32 = gpu_mesh(mrd, cfg.mesh, cfg.W0, precision=1)
+    g32.step(10)
+    om.step(10)
+    assert field_errors(g32.get_state().cpu().numpy().astype(np.float64), om.get_state()) <= TOL_F32
+
+
+def test_config4_riemann_frozen_boundary_and_stagnation(mrd):
+    cfg = wl.make_config("riemann4", n=127)
+    kw = dict(vertex_flag=cfg.vertex_flag)
+    gm = gpu_mesh(mrd, cfg.mesh, cfg.W0, **kw)
+    om = orc_mesh(cfg.mesh, cfg.W0, **kw)
+    gm.step(1)
+    om.step(1)
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_1
+    gm.step(19)
+    om.step(19)
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_100
+    _, mr, mp = gm.diagnostics()
+    assert mr > 0 and mp > 0
+
+
+def test_conservation_determinism_and_permutation_invariance(mrd):
+    base = wl.uniform_mesh(48, 48, 1.0, 1.0, periodic=True)
+    W = wl.kelvin_helmholtz_state(base)
+    gm = gpu_mesh(mrd, base, W)
+    tot0, _, _ = gm.diagnostics()
+    gm.step(25)
+    tot1, mr, mp = gm.diagnostics()
+    scale = np.array([tot0[0], 1.0, 1.0, tot0[3]])
+    assert np.all(np.abs(tot1 - tot0) <= 5e-13 * scale) and mr > 0 and mp > 0
+    W1 = gm.get_state().cpu().numpy()
+    gm2 = gpu_mesh(mrd, base, W)
+    gm2.step(25)
+    assert np.array_equal(gm2.get_state().cpu().numpy(), W1)          # run-to-run bitwise determinism (C20)
+    perm, vorder, _ = wl.permute_mesh(base, 77)
+    gp = gpu_mesh(mrd, perm, W[:, vorder])
+    gp.step(25)
+    assert field_errors(gp.get_state().cpu().numpy(), W1[:, vorder]) <= 1e-10
+
+
+def test_host_buffer_calls_and_async_stepping(mrd):
+    mesh = wl.uniform_mesh(32, 32, 10.0, 10.0, periodic=True)
+    W = wl.vortex_state(mesh)
+    gm = gpu_mesh(mrd, mesh, W)
+    g2 = mrd.Mesh(mesh.xy, mesh.tri, period=mesh.period)
+    g2.set_state_host(W)
+    assert np.array_equal(g2.get_state_host(), W)
+    gm.step(7)
+    g2.step_async(3)
+    g2.step_async(4)
+    n, t, dt = g2.sync()
+    assert n == 7
+    assert np.array_equal(g2.get_state_host(), gm.get_state().cpu().numpy())
+    assert g2.launch_count() > 7 * 5
+
+
+def test_nonphysical_state_is_reported_and_state_kept(mrd):
+    import torch
+    mesh = wl.uniform_mesh(16, 16, 1.0, 1.0, periodic=True)
+    W = wl.uniform_state(mesh)
+    bad = W.copy()
+    bad[0, 5] = -1.0
+    gm = mrd.Mesh(mesh.xy, mesh.tri, period=mesh.period)
+    with pytest.raises(mrd.MrdError) as e:
+        gm.set_state(torch.tensor(bad, device="cuda"))
+    assert e.value.code == mrd.MRD_ENONPHYSICAL
+    # a state that turns non-physical during a step: huge momentum spike next to near-vacuum
+    W2 = wl.primitive_to_conserved(np.where(np.arange(mesh.nv) % 7 == 0, 1e-6, 1.0), 0.0, 0.0,
+                                   np.where(np.arange(mesh.nv) % 5 == 0, 1e3, 1e-6))
+    gm.set_state(torch.tensor(W2, device="cuda"))
+    om = orc_mesh(mesh, W2)
+    try:
+        om.step(50)
+        oracle_failed = False
+    except oracle.OracleError:
+        oracle_failed = True
+    try:
+        gm.step(50)
+        gpu_failed = False
+    except mrd.MrdError as err:
+        gpu_failed = err.code == mrd.MRD_ENONPHYSICAL
+    assert gpu_failed == oracle_failed
+    if gpu_failed:                                          # state left at the last good step, still usable
+        Wg = gm.get_state().cpu().numpy()
+        assert np.isfinite(Wg).all() and (Wg[0] > 0).all()
+        assert field_errors(Wg, om.get_state()) <= 1e-6
