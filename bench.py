@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py -- triangle-updates/s of the residual-distribution sweep (BASELINE.json metric) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mrd|reference] [--n 4096]
+                    [--precision fp64|fp32] [--numbering morton|natural|permuted] [--reorder 0|1]
+
+A "step" is one RK2 time step of scheme B (both stages, dt reduction included) over the whole mesh:
+config 5 of BASELINE.json at its largest size (isentropic vortex on a periodic uniform triangulation of
+4096^2 vertices, 33.5M triangles, Morton-ordered input).  Prints ONE JSON line (rank 0).
+N > 1: one independent replica per GPU ("replicas only"), launched by torchrun.
+`--impl reference` times the CPU oracle (oracle/), as it stands, on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "triangle_updates_per_s_rk2_step"
+UNIT = "triangle-updates/s"
+
+# ---- per-unit algorithmic figures --------------------------------
+# FLOPs per triangle per stage: min(oracle operation count, FLOPs the kernel executes); the kernel's
+# count (2*DFMA + DADD + DMUL per thread, straight-line SASS, checked against ncu) is the smaller one.
+FLOPS_TRI_STAGE1 = {"fp64": 799.0, "fp32": 799.0}
+FLOPS_TRI_STAGE2 = {"fp64": 881.0, "fp32": 881.0}
+ORACLE_FLOPS_TRI = (2098.0, 2194.0)     # oracle.count_ops(stage 1 / stage 2): add+mul+div+sqrt, context only
+# compulsory HBM bytes per triangle of the stage-1 triangle kernel AS DESIGNED
+BYTES_TRI_STAGE1 = {"fp64": 360.0, "fp32": 186.0}
+BYTES_TRI_STAGE2 = {"fp64": 348.0, "fp32": 180.0}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for nme, val in zip(names, r[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nme)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def build_workload(n: int, numbering: str):
+    import workloads as wl
+    cfg = wl.make_config("sweep", n=n, numbering=numbering)
+    return cfg
+
+
+# ------------------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle, as it stands, on the host cores, on a bounded sample
+# ------------------------------------------------------------------------------------------------------
+def oracle_rate(n_sample: int, steps: int, warmup: int, numbering: str):
+    import oracle
+    cfg = build_workload(n_sample, numbering)
+    cores = os.cpu_count() or 1
+    om = oracle.OracleMesh(cfg.mesh.xy, cfg.mesh.tri, period=cfg.mesh.period, gamma=cfg.gamma, cfl=cfg.cfl,
+                           scheme=cfg.scheme, time_order=cfg.time_order, threads=cores)
+    om.set_state(cfg.W0)
+    if warmup:
+        om.step(warmup)
+    t0 = time.perf_counter()
+    om.step(steps)
+    dt = time.perf_counter() - t0
+    return cfg.mesh.nt * steps / dt, dt / steps, cores, cfg.mesh.nt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    n_s = min(args.n, 1024)
+    steps = max(1, min(args.steps, 3))
+    rate, spstep, cores, nt = oracle_rate(n_s, steps, min(args.warmup, 1), args.numbering)
+    sample = (f"isentropic vortex, periodic {n_s}^2 vertices ({nt} triangles = 1/{(args.n // n_s) ** 2} of the "
+              f"{args.n}^2 workload), {steps} RK2 steps of scheme B, OpenMP triangle loops on {cores} threads")
+    line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": min(args.warmup, 1), "ms_per_step": spstep * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"sweep vortex {args.n}^2 periodic, {args.numbering} numbering, B2 (oracle sample)"},
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------------------
+def fp64_peak_nominal(sm_max_mhz: float, precision: str) -> float:
+    """Plain-ALU peak in TFLOP/s: 148 SMs x 4 sub-partitions x 16 DFMA lanes (fp64)
+    or 32 FFMA lanes (fp32) x 2 flops x the maximum SM clock."""
+    lanes = 64 if precision == "fp64" else 128
+    return 148 * lanes * 2 * sm_max_mhz * 1e6 * 1e-12
+
+
+def run_mrd(args):
+    import torch
+    import paper_1705_02028_b200 as mrd
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the mrd path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    prec = args.precision
+    tdtype = torch.float64 if prec == "fp64" else torch.float32
+    cfg = build_workload(args.n, args.numbering)
+    mesh = cfg.mesh
+    nt, nv = mesh.nt, mesh.nv
+    t0 = time.perf_counter()
+    gm = mrd.Mesh(mesh.xy, mesh.tri, period=mesh.period, gamma=cfg.gamma, cfl=cfg.cfl, scheme=cfg.scheme,
+                  time_order=cfg.time_order, precision=mrd.FP64 if prec == "fp64" else mrd.FP32,
+                  reorder=bool(args.reorder), tile=args.tile)
+    layout_s = time.perf_counter() - t0
+    stream = torch.cuda.current_stream()
+    W0 = torch.tensor(cfg.W0, dtype=tdtype, device="cuda")
+    gm.set_state(W0)
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps -------------------------
+    gm.step(args.warmup)
+    barrier()
+    l0 = gm.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        barrier()
+        e0.record(stream)
+        gm.step_async(args.steps)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+    n_done, t_sim, _ = gm.sync()
+    launches = gm.launch_count() - l0
+    ms_total = e0.elapsed_time(e1)
+    if dist is not None:
+        tt = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    assert n_done == args.warmup + args.steps, (n_done, args.warmup, args.steps)
+    ms_step = ms_total / args.steps
+    value = world * nt * args.steps / (ms_total * 1e-3)
+
+    # ---- live per-kernel durations (CUDA events on the launching stream), averaged over 5 steps ------------
+    prof = {}
+    nprof = 5
+    for _ in range(nprof):
+        for k, v in gm.step_profile().items():
+            prof[k] = prof.get(k, 0.0) + v / nprof
+    _, mr, mp = gm.diagnostics()
+    assert mr > 0 and mp > 0
+
+    # ---- end to end through the host-buffer C-ABI calls: H2D of the state, one step, D2H of the result ----
+    ke = max(1, min(args.steps, args.e2e_steps))
+    h_in = torch.empty((4, nv), dtype=tdtype).pin_memory()
+    h_out = torch.empty((4, nv), dtype=tdtype).pin_memory()
+    h_in.copy_(gm.get_state().cpu())
+    gm.set_state_host(h_in.numpy()); gm.step(1); gm.get_state_host(h_out.numpy())      # warm-up
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(ke):
+        gm.set_state_host(h_in.numpy())
+        gm.step(1)
+        gm.get_state_host(h_out.numpy())
+        h_in, h_out = h_out, h_in
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        tt = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_s = float(tt.item())
+    state_bytes = 4 * nv * (8 if prec == "fp64" else 4)
+    e2e = {"value": world * nt * ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+           "d2h_bytes_per_step": state_bytes, "steps": ke, "ms_per_step": e2e_s / ke * 1e3,
+           "api": "mrd_set_state_host + mrd_step(1) + mrd_get_state_host, pinned host buffers"}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel -------------------------------------------------------------------
+    hbm_gbs, hbm_src = measured_peaks()
+    clocks = clk.summary()
+    sm_max = clocks["sm_max_mhz"] or 1965.0
+    main = {k: v for k, v in prof.items() if k in ("tri_stage1", "tri_stage2", "gather_dt", "update", "gather_update")}
+    dom = max(main, key=main.get)
+    dom_ms = main[dom]
+    flops_unit = {"tri_stage1": FLOPS_TRI_STAGE1[prec], "tri_stage2": FLOPS_TRI_STAGE2[prec]}.get(dom, 30.0)
+    bytes_unit = {"tri_stage1": BYTES_TRI_STAGE1[prec], "tri_stage2": BYTES_TRI_STAGE2[prec]}.get(dom, 160.0)
+    alu_peak = fp64_peak_nominal(sm_max, prec)
+    t_alu = flops_unit * nt / (alu_peak * 1e12)
+    t_hbm = bytes_unit * nt / (hbm_gbs * 1e9)
+    try:
+        dfma_tf, ffma_tf, copy_gbs = mrd.measure_peaks()
+    except Exception:
+        dfma_tf = ffma_tf = copy_gbs = None
+    if t_alu >= t_hbm:
+        ach = flops_unit * nt / (dom_ms * 1e-3) * 1e-12
+        roof = {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak}
+    else:
+        ach = bytes_unit * nt / (dom_ms * 1e-3) * 1e-9
+        roof = {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs}
+    roof.update({"traffic": args.traffic, "kernel": dom, "kernel_ms": dom_ms, "peak_source": hbm_src if roof["bound"] == "hbm"
+                 else "derived: 148 SM x %d lanes x 2 x %.0f MHz" % (64 if prec == "fp64" else 128, sm_max),
+                 "alg_flops_per_triangle": flops_unit, "alg_bytes_per_triangle": bytes_unit,
+                 "alu_frac": flops_unit * nt / (dom_ms * 1e-3) * 1e-12 / alu_peak,
+                 "hbm_frac": bytes_unit * nt / (dom_ms * 1e-3) * 1e-9 / hbm_gbs,
+                 "measured_fma_tflops": dfma_tf if prec == "fp64" else ffma_tf, "measured_copy_gbs": copy_gbs,
+                 "kernels_ms": prof,
+                 "step_alg": {"flops_per_triangle_update": FLOPS_TRI_STAGE1[prec] + FLOPS_TRI_STAGE2[prec] + 30.0,
+                              "roofline_ms": max((FLOPS_TRI_STAGE1[prec] + FLOPS_TRI_STAGE2[prec] + 30.0) * nt / (alu_peak * 1e12),
+                                                 (130.0 if prec == "fp64" else 76.0) * nt / (hbm_gbs * 1e9)) * 1e3}})
+    roof["step_alg"]["frac"] = roof["step_alg"]["roofline_ms"] / ms_step
+
+    # ---- the oracle beside it (rank 0, N = 1 only): bounded sample of the same workload --------------------
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        n_s = min(args.n, 1024)
+        rate, spstep, cores, nts = oracle_rate(n_s, 2, 0, args.numbering)
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"isentropic vortex, periodic {n_s}^2 vertices ({nts} triangles), 2 RK2 steps, "
+                         f"{spstep:.2f} s/step, OpenMP triangle loops on {cores} threads"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if prec == "fp64" else "f32", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json config 5: isentropic vortex, periodic uniform triangulation {args.n}^2 "
+                                   f"vertices, {nt} triangles, {args.numbering} input numbering, scheme B, RK2, CFL 0.5",
+                       "n_triangles": nt, "n_vertices": nv, "reorder": int(args.reorder), "tile": args.tile,
+                       "l2": "inputs larger than L2 (state %.0f MB, per-triangle arrays %.1f GB)" % (
+                           state_bytes / 1e6, gm.device_bytes() / 1e9),
+                       "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas",
+                       "layout_s": layout_s, "device_gb": gm.device_bytes() / 1e9, "t_sim": t_sim},
+            "vertex_updates_per_s": world * nv * args.steps / (ms_total * 1e-3),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="mrd", choices=["mrd", "reference"])
+    ap.add_argument("--n", type=int, default=4096, help="vertices per side of the periodic mesh")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
+    ap.add_argument("--numbering", default="morton", choices=["morton", "natural", "permuted"])
+    ap.add_argument("--reorder", type=int, default=1)
+    ap.add_argument("--tile", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--traffic", type=float, default=None, help="dram bytes per launch of the dominant kernel (ncu)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_mrd(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
