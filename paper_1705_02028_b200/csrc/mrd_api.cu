@@ -11,6 +11,7 @@
 
 #include "../../include/mrd.h"
 #include "mrd_kernels.cuh"
+#include "mrd_tile.cuh"
 #include "mrd_layout.h"
 
 namespace {
@@ -60,6 +61,15 @@ struct mrd_mesh {
   int *d_flag = nullptr;          // non-physical flag raised by kernels
   double *d_diag = nullptr;       // [DIAG_BLOCKS][6]
   void *h_pinned = nullptr;       // pinned host staging, R [4][nv]
+  // fused tile path (mrd_tile.cuh): tile plan + one partial per slot
+  bool fused = false;
+  bool dbg = false;               // dump: tile kernels also write per-triangle residuals to d_phi / d_sT
+  int32_t *d_tile_slot_off = nullptr, *d_slot_vertex = nullptr, *d_slot_ent_off = nullptr, *d_vslot_off = nullptr,
+          *d_vslot_ent = nullptr;
+  ushort4 *d_tile_tri = nullptr;
+  uint16_t *d_slot_ent = nullptr;
+  void *d_slot_xy = nullptr;      // R [nslot][2]
+  void *d_part = nullptr, *d_partS = nullptr;  // Vec4<R> [nslot], R [nslot]
   bool has_state = false;
   int64_t steps_base = 0;         // completed steps at the last sync (for buffer parity)
 };
@@ -111,6 +121,22 @@ template <class R> mrd::MeshDev<R> mesh_dev(const mrd_mesh *m) {
   d.frozen = m->d_frozen;
   return d;
 }
+template <class R> mrd::TileDev<R> tile_dev(const mrd_mesh *m) {
+  mrd::TileDev<R> t;
+  t.tile = m->L.tile;
+  t.ntile = m->L.ntile;
+  t.nslot = m->L.nslot;
+  t.nt = m->L.nt;
+  t.tile_slot_off = m->d_tile_slot_off;
+  t.slot_vertex = m->d_slot_vertex;
+  t.slot_xy = (const R *)m->d_slot_xy;
+  t.tile_tri = m->d_tile_tri;
+  t.slot_ent_off = m->d_slot_ent_off;
+  t.slot_ent = m->d_slot_ent;
+  t.vslot_off = m->d_vslot_off;
+  t.vslot_ent = m->d_vslot_ent;
+  return t;
+}
 template <class R> mrd::WallDev<R> wall_dev(const mrd_mesh *m) {
   mrd::WallDev<R> w;
   w.nwv = m->nwv;
@@ -134,22 +160,37 @@ template <class R> int upload_impl(mrd_mesh *m) {
   if ((rc = dev_upload(m, &m->d_vrank, L.vrank.data(), nv))) return rc;
   if ((rc = dev_upload(m, &m->d_tperm, L.tperm.data(), nt))) return rc;
   if ((rc = dev_upload(m, &m->d_tswap, L.tswap.data(), nt))) return rc;
-  {
+  m->fused = L.tile > 0;
+  if (!m->fused) {
     std::vector<int32_t> col(nt);
     for (int j = 0; j < 3; ++j) {
       for (int64_t t = 0; t < nt; ++t) col[t] = L.tri[3 * t + j];
       if ((rc = dev_upload(m, &m->d_tv[j], col.data(), nt))) return rc;
     }
+    for (int i = 0; i < 3; ++i) {
+      if ((rc = dev_upload_real<R>(m, &m->d_gnx[i], L.nx[i].data(), nt))) return rc;
+      if ((rc = dev_upload_real<R>(m, &m->d_gny[i], L.ny[i].data(), nt))) return rc;
+      if ((rc = dev_upload_real<R>(m, &m->d_ghl[i], L.hl[i].data(), nt))) return rc;
+    }
+    if ((rc = dev_upload_real<R>(m, &m->d_area3, L.area.data(), nt, 1.0 / 3.0))) return rc;
+    if ((rc = dev_upload_real<R>(m, &m->d_lmax, L.lmax.data(), nt))) return rc;
+    if ((rc = dev_upload(m, &m->d_csr_off, L.csr_off.data(), nv + 1))) return rc;
+    if ((rc = dev_upload(m, &m->d_csr_ent, L.csr_ent.data(), 3 * nt))) return rc;
+  } else {
+    static_assert(sizeof(ushort4) == 8, "tile_tri packing");
+    if ((rc = dev_upload(m, &m->d_tile_slot_off, L.tile_slot_off.data(), L.ntile + 1))) return rc;
+    if ((rc = dev_upload(m, &m->d_slot_vertex, L.slot_vertex.data(), L.nslot))) return rc;
+    if ((rc = dev_upload_real<R>(m, &m->d_slot_xy, L.slot_xy.data(), 2 * L.nslot))) return rc;
+    if ((rc = dev_upload(m, &m->d_tile_tri, reinterpret_cast<const ushort4 *>(L.tile_tri.data()), L.ntile * L.tile))) return rc;
+    if ((rc = dev_upload(m, &m->d_slot_ent_off, L.slot_ent_off.data(), L.nslot + 1))) return rc;
+    if ((rc = dev_upload(m, &m->d_slot_ent, L.slot_ent.data(), 3 * nt))) return rc;
+    if ((rc = dev_upload(m, &m->d_vslot_off, L.vslot_off.data(), nv + 1))) return rc;
+    if ((rc = dev_upload(m, &m->d_vslot_ent, L.vslot_ent.data(), L.nslot))) return rc;
+    V4 *pp = nullptr;
+    R *ps = nullptr;
+    if ((rc = dev_alloc(m, &pp, L.nslot)) || (rc = dev_alloc(m, &ps, L.nslot))) return rc;
+    m->d_part = pp; m->d_partS = ps;
   }
-  for (int i = 0; i < 3; ++i) {
-    if ((rc = dev_upload_real<R>(m, &m->d_gnx[i], L.nx[i].data(), nt))) return rc;
-    if ((rc = dev_upload_real<R>(m, &m->d_gny[i], L.ny[i].data(), nt))) return rc;
-    if ((rc = dev_upload_real<R>(m, &m->d_ghl[i], L.hl[i].data(), nt))) return rc;
-  }
-  if ((rc = dev_upload_real<R>(m, &m->d_area3, L.area.data(), nt, 1.0 / 3.0))) return rc;
-  if ((rc = dev_upload_real<R>(m, &m->d_lmax, L.lmax.data(), nt))) return rc;
-  if ((rc = dev_upload(m, &m->d_csr_off, L.csr_off.data(), nv + 1))) return rc;
-  if ((rc = dev_upload(m, &m->d_csr_ent, L.csr_ent.data(), 3 * nt))) return rc;
   if ((rc = dev_upload_real<R>(m, &m->d_vol, L.vol.data(), nv))) return rc;
   if (L.nf > 0 && (rc = dev_upload(m, &m->d_frozen, L.frozen.data(), nv))) return rc;
   m->nwv = (int64_t)L.wv_vertex.size();
@@ -177,8 +218,9 @@ template <class R> int upload_impl(mrd_mesh *m) {
     V4 *a = nullptr, *d = nullptr, *p = nullptr, *pn = nullptr, *pt = nullptr;
     R *st = nullptr, *us = nullptr;
     if ((rc = dev_alloc(m, &a, nv)) || (rc = dev_alloc(m, &d, nv))) return rc;
-    if ((rc = dev_alloc(m, &p, 3 * nt)) || (rc = dev_alloc(m, &pn, 3 * nt)) || (rc = dev_alloc(m, &pt, nt))) return rc;
-    if ((rc = dev_alloc(m, &st, nt)) || (rc = dev_alloc(m, &us, 4 * nv))) return rc;
+    if (!m->fused && ((rc = dev_alloc(m, &p, 3 * nt)) || (rc = dev_alloc(m, &st, nt)))) return rc;
+    if ((rc = dev_alloc(m, &pn, 3 * nt)) || (rc = dev_alloc(m, &pt, nt))) return rc;
+    if ((rc = dev_alloc(m, &us, 4 * nv))) return rc;
     m->d_acc = a; m->d_dWdt = d; m->d_phi = p; m->d_phiN = pn; m->d_phiT = pt; m->d_sT = st; m->d_user = us;
   }
   if ((rc = dev_alloc(m, &m->d_ctl, 1)) || (rc = dev_alloc(m, &m->d_flag, 1)) || (rc = dev_alloc(m, &m->d_diag, DIAG_BLOCKS * 6))) return rc;
@@ -223,22 +265,55 @@ template <class R> int get_state_impl(mrd_mesh *m, R *W_dev, cudaStream_t s) {
   return MRD_OK;
 }
 
+template <class R> void set_tile_smem(const void *fn, size_t bytes) {
+  if (bytes > 48 * 1024) cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
 template <class R, int SCHEME> void launch_stage1(mrd_mesh *m, bool store, int a, cudaStream_t s) {
   using V4 = mrd::Vec4<R>;
+  const R gamma = (R)m->L.p.gamma;
+  if (m->fused) {
+    auto td = tile_dev<R>(m);
+    const int T = td.tile;
+    const size_t sh = mrd::TileSmem<R>::bytes(T, false);
+    V4 *dbg = m->dbg ? (V4 *)m->d_phi : nullptr;
+    R *dbgs = m->dbg ? (R *)m->d_sT : nullptr;
+    if (store) {
+      set_tile_smem<R>((const void *)mrd::tile_stage1_kernel<R, SCHEME, true>, sh);
+      mrd::tile_stage1_kernel<R, SCHEME, true><<<(unsigned)td.ntile, T, sh, s>>>(td, gamma, m->d_ctl, (const V4 *)m->d_Z[a], (const R *)m->d_spd[a], (V4 *)m->d_part,
+                                                                          (R *)m->d_partS, (V4 *)m->d_phiN, (V4 *)m->d_phiT, dbg, dbgs, m->d_flag);
+    } else {
+      set_tile_smem<R>((const void *)mrd::tile_stage1_kernel<R, SCHEME, false>, sh);
+      mrd::tile_stage1_kernel<R, SCHEME, false><<<(unsigned)td.ntile, T, sh, s>>>(td, gamma, m->d_ctl, (const V4 *)m->d_Z[a], (const R *)m->d_spd[a], (V4 *)m->d_part,
+                                                                           (R *)m->d_partS, (V4 *)m->d_phiN, (V4 *)m->d_phiT, dbg, dbgs, m->d_flag);
+    }
+    m->launches++;
+    return;
+  }
   auto md = mesh_dev<R>(m);
   const unsigned nb = blocks_for(md.nt, 128);
   if (store)
-    mrd::tri_stage1_kernel<R, SCHEME, true><<<nb, 128, 0, s>>>(md, (R)m->L.p.gamma, m->d_ctl, (const V4 *)m->d_Z[a], (const R *)m->d_spd[a],
+    mrd::tri_stage1_kernel<R, SCHEME, true><<<nb, 128, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_Z[a], (const R *)m->d_spd[a],
                                                             (V4 *)m->d_phi, (V4 *)m->d_phiN, (V4 *)m->d_phiT, (R *)m->d_sT, m->d_flag);
   else
-    mrd::tri_stage1_kernel<R, SCHEME, false><<<nb, 128, 0, s>>>(md, (R)m->L.p.gamma, m->d_ctl, (const V4 *)m->d_Z[a], (const R *)m->d_spd[a],
+    mrd::tri_stage1_kernel<R, SCHEME, false><<<nb, 128, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_Z[a], (const R *)m->d_spd[a],
                                                              (V4 *)m->d_phi, (V4 *)m->d_phiN, (V4 *)m->d_phiT, (R *)m->d_sT, m->d_flag);
   m->launches++;
 }
 template <class R, int SCHEME> void launch_stage2(mrd_mesh *m, int b, cudaStream_t s) {
   using V4 = mrd::Vec4<R>;
+  const R gamma = (R)m->L.p.gamma;
+  if (m->fused) {
+    auto td = tile_dev<R>(m);
+    const int T = td.tile;
+    const size_t sh = mrd::TileSmem<R>::bytes(T, true);
+    set_tile_smem<R>((const void *)mrd::tile_stage2_kernel<R, SCHEME>, sh);
+    mrd::tile_stage2_kernel<R, SCHEME><<<(unsigned)td.ntile, T, sh, s>>>(td, gamma, m->d_ctl, (const V4 *)m->d_Z[b], (const V4 *)m->d_dWdt, (const V4 *)m->d_phiN,
+                                                                  (const V4 *)m->d_phiT, (V4 *)m->d_part, m->d_flag);
+    m->launches++;
+    return;
+  }
   auto md = mesh_dev<R>(m);
-  mrd::tri_stage2_kernel<R, SCHEME><<<blocks_for(md.nt, 128), 128, 0, s>>>(md, (R)m->L.p.gamma, m->d_ctl, (const V4 *)m->d_Z[b],
+  mrd::tri_stage2_kernel<R, SCHEME><<<blocks_for(md.nt, 128), 128, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_Z[b],
                                                                         (const V4 *)m->d_dWdt, (const V4 *)m->d_phiN, (const V4 *)m->d_phiT,
                                                                         (V4 *)m->d_phi, m->d_flag);
   m->launches++;
@@ -271,7 +346,10 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
     default: launch_stage1<R, MRD_SCHEME_B>(m, rk2, a, s); break;
   }
   PROF_MARK(MRD_PROF_TRI1)
-  mrd::gather_dt_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, m->d_ctl, (const V4 *)m->d_phi, (const R *)m->d_sT, (V4 *)m->d_acc);
+  if (m->fused)
+    mrd::slot_gather_dt_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, tile_dev<R>(m), m->d_ctl, (const V4 *)m->d_part, (const R *)m->d_partS, (V4 *)m->d_acc);
+  else
+    mrd::gather_dt_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, m->d_ctl, (const V4 *)m->d_phi, (const R *)m->d_sT, (V4 *)m->d_acc);
   m->launches++;
   PROF_MARK(MRD_PROF_GATHER_DT)
   if (m->nwv > 0) {
@@ -300,8 +378,12 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
       m->launches++;
       PROF_MARK(MRD_PROF_WALL2)
     }
-    mrd::gather_update_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_phi, (const V4 *)m->d_wall_acc, (V4 *)m->d_W[b],
-                                                                     (V4 *)m->d_Z[b], (R *)m->d_spd[b], m->d_flag);
+    if (m->fused)
+      mrd::slot_gather_update_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, tile_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
+                                                                            (V4 *)m->d_W[b], (V4 *)m->d_Z[b], (R *)m->d_spd[b], m->d_flag);
+    else
+      mrd::gather_update_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_phi, (const V4 *)m->d_wall_acc, (V4 *)m->d_W[b],
+                                                                       (V4 *)m->d_Z[b], (R *)m->d_spd[b], m->d_flag);
     m->launches++;
     PROF_MARK(MRD_PROF_GATHER_UPDATE)
   }
@@ -412,6 +494,14 @@ template <class R> int dump_impl(mrd_mesh *m, double *phiT, double *phiN, double
     }
   };
   const int a = m->cur;
+  if (m->fused && !m->d_phi) {
+    V4 *p = nullptr;
+    R *st = nullptr;
+    if ((rc = dev_alloc(m, &p, 3 * nt)) || (rc = dev_alloc(m, &st, nt))) return rc;
+    m->d_phi = p;
+    m->d_sT = st;
+  }
+  m->dbg = m->fused;
   for (int pass = 0; pass < 2; ++pass) {
     if (pass == 0) launch_stage1<R, MRD_SCHEME_LDA>(m, true, a, s);
     else launch_stage1<R, MRD_SCHEME_B>(m, true, a, s);
@@ -434,6 +524,7 @@ template <class R> int dump_impl(mrd_mesh *m, double *phiT, double *phiN, double
     CUDA_TRY(cudaMemcpy(hs.data(), m->d_sT, hs.size() * sizeof(R), cudaMemcpyDeviceToHost));
     for (int64_t k = 0; k < nt; ++k) sT[m->L.tperm[k]] = (double)hs[k];
   }
+  m->dbg = false;
   int flag = 0;
   CUDA_TRY(cudaMemcpy(&flag, m->d_flag, sizeof(int), cudaMemcpyDeviceToHost));
   CUDA_TRY(cudaMemcpy(m->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice));

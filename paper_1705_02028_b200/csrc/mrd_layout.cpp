@@ -80,7 +80,7 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
   if (p->precision != MRD_FP64 && p->precision != MRD_FP32) { err = "bad precision"; return MRD_EINVAL; }
   if (p->period_x < 0.0 || p->period_y < 0.0) { err = "negative period"; return MRD_EINVAL; }
   if (ne < 0 || (ne > 0 && !wall_edge)) { err = "bad wall edge list"; return MRD_EINVAL; }
-  if (p->tile < 0 || p->tile > 256 || (p->tile % 32) != 0) { err = "tile must be a multiple of 32, <= 256"; return MRD_EINVAL; }
+  if (p->tile < -1 || p->tile > 256 || (p->tile > 0 && (p->tile % 32) != 0)) { err = "tile must be -1, 0 or a multiple of 32 <= 256"; return MRD_EINVAL; }
   L.p = *p;
   L.nv = nv; L.nt = nt; L.ne = ne;
   const double period[2] = {p->period_x, p->period_y};
@@ -253,7 +253,7 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
     if (!inc.empty()) L.wv_off.push_back((int32_t)L.wv_ent.size());
   }
 
-  L.tile = p->tile;
+  L.tile = p->tile == 0 ? 128 : (p->tile < 0 ? 0 : p->tile);  // 0 = default tile, -1 = unfused kernels
   if (L.tile > 0) build_tile_plan(L, xyi);
   return MRD_OK;
 }
@@ -319,14 +319,17 @@ static void build_tile_plan(mrd_layout &L, const std::vector<double> &xyi) {
   for (int64_t b = 0; b < ntile; ++b) {
     const int64_t t0 = b * T, t1 = std::min(nt, t0 + T);
     const int32_t s0 = L.tile_slot_off[b];
+    const int32_t anchor = L.tri[3 * t0];
+    const double ax = xyi[2 * anchor], ay = xyi[2 * anchor + 1];
     const std::vector<int64_t> &uk = keys[b];
     for (size_t q = 0; q < uk.size(); ++q) {
       int32_t v = (int32_t)(uk[q] / 25);
       int r = (int)(uk[q] % 25);
       int sx = r / 5 - 2, sy = r % 5 - 2;
       L.slot_vertex[s0 + q] = v;
-      L.slot_xy[2 * (s0 + q)] = xyi[2 * v] + sx * period[0];
-      L.slot_xy[2 * (s0 + q) + 1] = xyi[2 * v + 1] + sy * period[1];
+      // relative to the tile's anchor vertex: keeps fp32 coordinates accurate to ulp(tile size), not ulp(domain)
+      L.slot_xy[2 * (s0 + q)] = (xyi[2 * v] + sx * period[0]) - ax;
+      L.slot_xy[2 * (s0 + q) + 1] = (xyi[2 * v + 1] + sy * period[1]) - ay;
     }
     for (int64_t t = t0; t < t1; ++t)
       for (int j = 0; j < 3; ++j) L.slot_ent_off[s0 + L.tile_tri[((size_t)b * T + (t - t0)) * 4 + j] + 1]++;
