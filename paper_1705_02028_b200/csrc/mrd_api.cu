@@ -64,12 +64,13 @@ struct mrd_mesh {
   // fused tile path (mrd_tile.cuh): tile plan + one partial per slot
   bool fused = false;
   bool dbg = false;               // dump: tile kernels also write per-triangle residuals to d_phi / d_sT
-  int32_t *d_tile_slot_off = nullptr, *d_slot_vertex = nullptr, *d_slot_ent_off = nullptr, *d_vslot_off = nullptr,
-          *d_vslot_ent = nullptr;
-  ushort4 *d_tile_tri = nullptr;
-  uint16_t *d_slot_ent = nullptr;
+  int32_t *d_tile_slot_off = nullptr, *d_vslot_off = nullptr, *d_vslot_ent = nullptr;
+  uint16_t *d_plan = nullptr;     // [ntile][plan_stride]
   void *d_slot_xy = nullptr;      // R [nslot][2]
   void *d_part = nullptr, *d_partS = nullptr;  // Vec4<R> [nslot], R [nslot]
+  void *d_slotZ[2] = {nullptr, nullptr}, *d_slotS[2] = {nullptr, nullptr}, *d_slotD = nullptr;  // slot-major Z, |v|+c, dW/dt
+  void *d_phi16 = nullptr;        // R [ntile][16][T]: phi^N(W^n) (12) and phi^T(W^n) (4), component-major per tile
+  int nsm = 0;
   bool has_state = false;
   int64_t steps_base = 0;         // completed steps at the last sync (for buffer parity)
 };
@@ -124,18 +125,36 @@ template <class R> mrd::MeshDev<R> mesh_dev(const mrd_mesh *m) {
 template <class R> mrd::TileDev<R> tile_dev(const mrd_mesh *m) {
   mrd::TileDev<R> t;
   t.tile = m->L.tile;
+  t.maxslots = m->L.maxslots;
+  t.offn = m->L.offn;
+  t.plan_stride = m->L.plan_stride;
   t.ntile = m->L.ntile;
   t.nslot = m->L.nslot;
   t.nt = m->L.nt;
   t.tile_slot_off = m->d_tile_slot_off;
-  t.slot_vertex = m->d_slot_vertex;
+  t.plan = m->d_plan;
   t.slot_xy = (const R *)m->d_slot_xy;
-  t.tile_tri = m->d_tile_tri;
-  t.slot_ent_off = m->d_slot_ent_off;
-  t.slot_ent = m->d_slot_ent;
   t.vslot_off = m->d_vslot_off;
   t.vslot_ent = m->d_vslot_ent;
   return t;
+}
+// where the vertex kernels put Z / |v|+c / dW/dt of buffer pair `pair`
+template <class R> mrd::VertexSink<R> sink_for(const mrd_mesh *m, int pair, bool want_spd, bool want_d) {
+  mrd::VertexSink<R> k;
+  if (m->fused) {
+    k.Z = (mrd::Vec4<R> *)m->d_slotZ[pair];
+    k.spd = want_spd ? (R *)m->d_slotS[pair] : nullptr;
+    k.D = want_d ? (mrd::Vec4<R> *)m->d_slotD : nullptr;
+    k.vslot_off = m->d_vslot_off;
+    k.vslot_ent = m->d_vslot_ent;
+  } else {
+    k.Z = (mrd::Vec4<R> *)m->d_Z[pair];
+    k.spd = want_spd ? (R *)m->d_spd[pair] : nullptr;
+    k.D = want_d ? (mrd::Vec4<R> *)m->d_dWdt : nullptr;
+    k.vslot_off = nullptr;
+    k.vslot_ent = nullptr;
+  }
+  return k;
 }
 template <class R> mrd::WallDev<R> wall_dev(const mrd_mesh *m) {
   mrd::WallDev<R> w;
@@ -177,18 +196,28 @@ template <class R> int upload_impl(mrd_mesh *m) {
     if ((rc = dev_upload(m, &m->d_csr_off, L.csr_off.data(), nv + 1))) return rc;
     if ((rc = dev_upload(m, &m->d_csr_ent, L.csr_ent.data(), 3 * nt))) return rc;
   } else {
-    static_assert(sizeof(ushort4) == 8, "tile_tri packing");
     if ((rc = dev_upload(m, &m->d_tile_slot_off, L.tile_slot_off.data(), L.ntile + 1))) return rc;
-    if ((rc = dev_upload(m, &m->d_slot_vertex, L.slot_vertex.data(), L.nslot))) return rc;
+    if ((rc = dev_upload(m, &m->d_plan, L.tile_plan.data(), (int64_t)L.tile_plan.size()))) return rc;
     if ((rc = dev_upload_real<R>(m, &m->d_slot_xy, L.slot_xy.data(), 2 * L.nslot))) return rc;
-    if ((rc = dev_upload(m, &m->d_tile_tri, reinterpret_cast<const ushort4 *>(L.tile_tri.data()), L.ntile * L.tile))) return rc;
-    if ((rc = dev_upload(m, &m->d_slot_ent_off, L.slot_ent_off.data(), L.nslot + 1))) return rc;
-    if ((rc = dev_upload(m, &m->d_slot_ent, L.slot_ent.data(), 3 * nt))) return rc;
     if ((rc = dev_upload(m, &m->d_vslot_off, L.vslot_off.data(), nv + 1))) return rc;
-    if ((rc = dev_upload(m, &m->d_vslot_ent, L.vslot_ent.data(), L.nslot))) return rc;
-    V4 *pp = nullptr;
-    R *ps = nullptr;
-    if ((rc = dev_alloc(m, &pp, L.nslot)) || (rc = dev_alloc(m, &ps, L.nslot))) return rc;
+    if ((rc = dev_upload(m, &m->d_vslot_ent, L.vslot_ent.data(), (int64_t)L.vslot_ent.size()))) return rc;
+    V4 *pp = nullptr, *sd = nullptr;
+    R *ps = nullptr, *p16 = nullptr;
+    if ((rc = dev_alloc(m, &pp, L.nslot)) || (rc = dev_alloc(m, &ps, L.nslot)) || (rc = dev_alloc(m, &sd, L.nslot))) return rc;
+    if ((rc = dev_alloc(m, &p16, L.ntile * 16 * L.tile))) return rc;
+    CUDA_TRY(cudaMemset(sd, 0, sizeof(V4) * L.nslot));
+    m->d_slotD = sd; m->d_phi16 = p16;
+    for (int b = 0; b < 2; ++b) {
+      V4 *z = nullptr;
+      R *sp = nullptr;
+      if ((rc = dev_alloc(m, &z, L.nslot)) || (rc = dev_alloc(m, &sp, L.nslot))) return rc;
+      CUDA_TRY(cudaMemset(z, 0, sizeof(V4) * L.nslot));   // padding slots are copied (never used): keep them defined
+      CUDA_TRY(cudaMemset(sp, 0, sizeof(R) * L.nslot));
+      m->d_slotZ[b] = z; m->d_slotS[b] = sp;
+    }
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, m->device));
+    m->nsm = prop.multiProcessorCount;
     m->d_part = pp; m->d_partS = ps;
   }
   if ((rc = dev_upload_real<R>(m, &m->d_vol, L.vol.data(), nv))) return rc;
@@ -211,15 +240,17 @@ template <class R> int upload_impl(mrd_mesh *m) {
   for (int b = 0; b < 2; ++b) {
     V4 *w = nullptr, *z = nullptr;
     R *s = nullptr;
-    if ((rc = dev_alloc(m, &w, nv)) || (rc = dev_alloc(m, &z, nv)) || (rc = dev_alloc(m, &s, nv))) return rc;
+    if ((rc = dev_alloc(m, &w, nv))) return rc;
+    if (!m->fused && ((rc = dev_alloc(m, &z, nv)) || (rc = dev_alloc(m, &s, nv)))) return rc;
     m->d_W[b] = w; m->d_Z[b] = z; m->d_spd[b] = s;
   }
   {
     V4 *a = nullptr, *d = nullptr, *p = nullptr, *pn = nullptr, *pt = nullptr;
     R *st = nullptr, *us = nullptr;
-    if ((rc = dev_alloc(m, &a, nv)) || (rc = dev_alloc(m, &d, nv))) return rc;
-    if (!m->fused && ((rc = dev_alloc(m, &p, 3 * nt)) || (rc = dev_alloc(m, &st, nt)))) return rc;
-    if ((rc = dev_alloc(m, &pn, 3 * nt)) || (rc = dev_alloc(m, &pt, nt))) return rc;
+    if ((rc = dev_alloc(m, &a, nv))) return rc;
+    if (!m->fused && ((rc = dev_alloc(m, &d, nv)) || (rc = dev_alloc(m, &p, 3 * nt)) || (rc = dev_alloc(m, &st, nt)) ||
+                      (rc = dev_alloc(m, &pn, 3 * nt)) || (rc = dev_alloc(m, &pt, nt))))
+      return rc;
     if ((rc = dev_alloc(m, &us, 4 * nv))) return rc;
     m->d_acc = a; m->d_dWdt = d; m->d_phi = p; m->d_phiN = pn; m->d_phiT = pt; m->d_sT = st; m->d_user = us;
   }
@@ -241,7 +272,7 @@ template <class R> int set_state_impl(mrd_mesh *m, const R *W_dev, cudaStream_t 
   CUDA_TRY(cudaMemcpyAsync(m->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s));
   CUDA_TRY(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
   mrd::set_state_kernel<R><<<blocks_for(nv, 256), 256, 0, s>>>(nv, m->d_vperm, W_dev, (R)m->L.p.gamma, (V4 *)m->d_W[0],
-                                                               (V4 *)m->d_Z[0], (R *)m->d_spd[0], m->d_flag);
+                                                               sink_for<R>(m, 0, true, false), m->d_flag);
   m->launches++;
   int flag = 0;
   CUDA_TRY(cudaMemcpyAsync(&flag, m->d_flag, sizeof(int), cudaMemcpyDeviceToHost, s));
@@ -265,28 +296,31 @@ template <class R> int get_state_impl(mrd_mesh *m, R *W_dev, cudaStream_t s) {
   return MRD_OK;
 }
 
-template <class R> void set_tile_smem(const void *fn, size_t bytes) {
-  if (bytes > 48 * 1024) cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+// persistent launch of a tile kernel: dynamic shared memory opt-in, grid = SMs x resident blocks (<= ntile)
+template <class K, class... Args> void launch_tile(mrd_mesh *m, K kernel, size_t sh, cudaStream_t s, Args... args) {
+  const int T = m->L.tile;
+  cudaFuncSetAttribute((const void *)kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh);
+  int occ = 1;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, T, sh);
+  if (occ < 1) occ = 1;
+  int64_t grid = std::min<int64_t>(m->L.ntile, (int64_t)m->nsm * occ);
+  kernel<<<(unsigned)grid, T, sh, s>>>(args...);
+  m->launches++;
 }
 template <class R, int SCHEME> void launch_stage1(mrd_mesh *m, bool store, int a, cudaStream_t s) {
   using V4 = mrd::Vec4<R>;
   const R gamma = (R)m->L.p.gamma;
   if (m->fused) {
     auto td = tile_dev<R>(m);
-    const int T = td.tile;
-    const size_t sh = mrd::TileSmem<R>::bytes(T, false);
+    const size_t sh = mrd::TileSmem<R, 1>(td.tile, td.maxslots, td.plan_stride).total;
     V4 *dbg = m->dbg ? (V4 *)m->d_phi : nullptr;
     R *dbgs = m->dbg ? (R *)m->d_sT : nullptr;
-    if (store) {
-      set_tile_smem<R>((const void *)mrd::tile_stage1_kernel<R, SCHEME, true>, sh);
-      mrd::tile_stage1_kernel<R, SCHEME, true><<<(unsigned)td.ntile, T, sh, s>>>(td, gamma, m->d_ctl, (const V4 *)m->d_Z[a], (const R *)m->d_spd[a], (V4 *)m->d_part,
-                                                                          (R *)m->d_partS, (V4 *)m->d_phiN, (V4 *)m->d_phiT, dbg, dbgs, m->d_flag);
-    } else {
-      set_tile_smem<R>((const void *)mrd::tile_stage1_kernel<R, SCHEME, false>, sh);
-      mrd::tile_stage1_kernel<R, SCHEME, false><<<(unsigned)td.ntile, T, sh, s>>>(td, gamma, m->d_ctl, (const V4 *)m->d_Z[a], (const R *)m->d_spd[a], (V4 *)m->d_part,
-                                                                           (R *)m->d_partS, (V4 *)m->d_phiN, (V4 *)m->d_phiT, dbg, dbgs, m->d_flag);
-    }
-    m->launches++;
+    if (store)
+      launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, true>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl, (const V4 *)m->d_slotZ[a],
+                  (const R *)m->d_slotS[a], (const V4 *)m->d_slotD, (R *)m->d_phi16, (V4 *)m->d_part, (R *)m->d_partS, dbg, dbgs, m->d_flag);
+    else
+      launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, false>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl, (const V4 *)m->d_slotZ[a],
+                  (const R *)m->d_slotS[a], (const V4 *)m->d_slotD, (R *)m->d_phi16, (V4 *)m->d_part, (R *)m->d_partS, dbg, dbgs, m->d_flag);
     return;
   }
   auto md = mesh_dev<R>(m);
@@ -304,12 +338,10 @@ template <class R, int SCHEME> void launch_stage2(mrd_mesh *m, int b, cudaStream
   const R gamma = (R)m->L.p.gamma;
   if (m->fused) {
     auto td = tile_dev<R>(m);
-    const int T = td.tile;
-    const size_t sh = mrd::TileSmem<R>::bytes(T, true);
-    set_tile_smem<R>((const void *)mrd::tile_stage2_kernel<R, SCHEME>, sh);
-    mrd::tile_stage2_kernel<R, SCHEME><<<(unsigned)td.ntile, T, sh, s>>>(td, gamma, m->d_ctl, (const V4 *)m->d_Z[b], (const V4 *)m->d_dWdt, (const V4 *)m->d_phiN,
-                                                                  (const V4 *)m->d_phiT, (V4 *)m->d_part, m->d_flag);
-    m->launches++;
+    const size_t sh = mrd::TileSmem<R, 2>(td.tile, td.maxslots, td.plan_stride).total;
+    launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, false>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl, (const V4 *)m->d_slotZ[b],
+                (const R *)nullptr, (const V4 *)m->d_slotD, (R *)m->d_phi16, (V4 *)m->d_part, (R *)nullptr, (V4 *)nullptr, (R *)nullptr,
+                m->d_flag);
     return;
   }
   auto md = mesh_dev<R>(m);
@@ -359,12 +391,12 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
   }
   if (!rk2) {
     mrd::update_kernel<R, true><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_acc, (V4 *)m->d_W[b],
-                                                                    (V4 *)m->d_Z[b], (R *)m->d_spd[b], (V4 *)m->d_dWdt, m->d_flag);
+                                                                    sink_for<R>(m, b, true, false), m->d_flag);
     m->launches++;
     PROF_MARK(MRD_PROF_UPDATE)
   } else {
     mrd::update_kernel<R, false><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_acc, (V4 *)m->d_W[b],
-                                                                     (V4 *)m->d_Z[b], (R *)m->d_spd[b], (V4 *)m->d_dWdt, m->d_flag);
+                                                                     sink_for<R>(m, b, false, true), m->d_flag);
     m->launches++;
     PROF_MARK(MRD_PROF_UPDATE)
     switch (scheme) {
@@ -380,10 +412,10 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
     }
     if (m->fused)
       mrd::slot_gather_update_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, tile_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
-                                                                            (V4 *)m->d_W[b], (V4 *)m->d_Z[b], (R *)m->d_spd[b], m->d_flag);
+                                                                            (V4 *)m->d_W[b], sink_for<R>(m, b, true, false), m->d_flag);
     else
       mrd::gather_update_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_phi, (const V4 *)m->d_wall_acc, (V4 *)m->d_W[b],
-                                                                       (V4 *)m->d_Z[b], (R *)m->d_spd[b], m->d_flag);
+                                                                       sink_for<R>(m, b, true, false), m->d_flag);
     m->launches++;
     PROF_MARK(MRD_PROF_GATHER_UPDATE)
   }
@@ -511,12 +543,23 @@ template <class R> int dump_impl(mrd_mesh *m, double *phiT, double *phiN, double
     if (pass == 0 && phiLDA) put3(phiLDA);
     if (pass == 1 && phiB) put3(phiB);
   }
+  if (m->fused && (phiN || phiT)) {
+    // stored stage-1 values of the fused path: phi16[tile][16][T] -> the unfused [nt][3][4] / [nt][4] shapes
+    const int T = m->L.tile;
+    std::vector<R> h16((size_t)m->L.ntile * 16 * T);
+    CUDA_TRY(cudaMemcpy(h16.data(), m->d_phi16, h16.size() * sizeof(R), cudaMemcpyDeviceToHost));
+    for (int64_t k = 0; k < nt; ++k) {
+      const R *o = &h16[(size_t)(k / T) * 16 * T + (k % T)];
+      for (int c = 0; c < 12; ++c) h3[12 * k + c] = o[(size_t)c * T];
+      for (int c = 0; c < 4; ++c) h1[4 * k + c] = o[(size_t)(12 + c) * T];
+    }
+  }
   if (phiN) {
-    CUDA_TRY(cudaMemcpy(h3.data(), m->d_phiN, h3.size() * sizeof(R), cudaMemcpyDeviceToHost));
+    if (!m->fused) CUDA_TRY(cudaMemcpy(h3.data(), m->d_phiN, h3.size() * sizeof(R), cudaMemcpyDeviceToHost));
     put3(phiN);
   }
   if (phiT) {
-    CUDA_TRY(cudaMemcpy(h1.data(), m->d_phiT, h1.size() * sizeof(R), cudaMemcpyDeviceToHost));
+    if (!m->fused) CUDA_TRY(cudaMemcpy(h1.data(), m->d_phiT, h1.size() * sizeof(R), cudaMemcpyDeviceToHost));
     for (int64_t k = 0; k < nt; ++k)
       for (int q = 0; q < 4; ++q) phiT[4 * (int64_t)m->L.tperm[k] + q] = (double)h1[4 * k + q];
   }

@@ -29,6 +29,32 @@ template <class R> struct MeshDev {
   const uint8_t *frozen;        // or nullptr
 };
 
+// Where a vertex kernel puts the per-vertex quantities the triangle kernels read: per-vertex arrays (unfused
+// path) or one copy per tile slot of the vertex (fused path: the tile kernels then stream contiguous slot
+// ranges with bulk copies and never gather by vertex index).
+template <class R> struct VertexSink {
+  Vec4<R> *Z;                 // parameter vector (S1)
+  R *spd;                     // |v| + c (S6), may be null
+  Vec4<R> *D;                 // dW/dt of stage 1 (eq. 57), may be null
+  const int32_t *vslot_off;   // null: index by vertex; else Z/spd/D are indexed by slot
+  const int32_t *vslot_ent;
+  __device__ __forceinline__ void put(int64_t i, const Vec4<R> &z, R s, bool has_d, const Vec4<R> &d) const {
+    if (vslot_off) {
+      const int32_t q0 = __ldg(vslot_off + i), q1 = __ldg(vslot_off + i + 1);
+      for (int32_t q = q0; q < q1; ++q) {
+        const int32_t sl = __ldg(vslot_ent + q);
+        st4(&Z[sl], z);
+        if (spd) spd[sl] = s;
+        if (has_d) st4(&D[sl], d);
+      }
+    } else {
+      st4(&Z[i], z);
+      if (spd) spd[i] = s;
+      if (has_d) st4(&D[i], d);
+    }
+  }
+};
+
 #define MRD_CTL_GUARD(ctl) \
   if ((ctl)->status != 0 || (ctl)->active == 0) return;
 
@@ -63,8 +89,7 @@ __global__ void ctl_kernel(Ctl *c, int mode, double t_end, const int *flag) {
 // ---------------------------------------------------------------------------------------------
 template <class R>
 __global__ void set_state_kernel(int64_t nv, const int32_t *__restrict__ vperm, const R *__restrict__ Wuser,
-                                 R gamma, Vec4<R> *__restrict__ W, Vec4<R> *__restrict__ Z, R *__restrict__ spd,
-                                 int *bad) {
+                                 R gamma, Vec4<R> *__restrict__ W, VertexSink<R> sink, int *bad) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= nv) return;
   int64_t u = vperm[i];
@@ -73,8 +98,7 @@ __global__ void set_state_kernel(int64_t nv, const int32_t *__restrict__ vperm, 
   R s, p;
   bool ok = vertex_prepare(gamma, w, z, s, p);
   st4(&W[i], w);
-  st4(&Z[i], z);
-  spd[i] = s;
+  sink.put(i, z, s, false, z);
   if (!ok) atomicOr(bad, 1);
 }
 
@@ -241,29 +265,27 @@ gather_dt_kernel(MeshDev<R> m, Ctl *__restrict__ ctl, const Vec4<R> *__restrict_
 // initial state, L582); then Z and the signal speed of the new state (S1, S6), positivity check.
 template <class R, bool WANT_DWDT>
 __device__ __forceinline__ void vertex_finish(R gamma, R dt, R vol, bool frozen, const Vec4<R> &Wold, const R a[4],
-                                              const Vec4<R> &Wn, Vec4<R> *Wout, Vec4<R> *Zout, R *spd_out,
-                                              Vec4<R> *dWdt_out, int *status) {
+                                              int64_t i, Vec4<R> *Wout, const VertexSink<R> &sink, int *status) {
   R f = frozen ? R(0) : dt * Fast<R>::rcp(vol);
   Vec4<R> w{Wold.x - f * a[0], Wold.y - f * a[1], Wold.z - f * a[2], Wold.w - f * a[3]};
   Vec4<R> z;
   R s, p;
   bool ok = vertex_prepare(gamma, w, z, s, p);
   if (!ok) atomicOr(status, 1);
-  st4(Wout, w);
-  st4(Zout, z);
-  if (spd_out) *spd_out = s;
+  st4(&Wout[i], w);
+  Vec4<R> d{0, 0, 0, 0};
   if (WANT_DWDT) {
     R idt = Fast<R>::rcp(dt);
-    st4(dWdt_out, Vec4<R>{(w.x - Wn.x) * idt, (w.y - Wn.y) * idt, (w.z - Wn.z) * idt, (w.w - Wn.w) * idt});
+    d = Vec4<R>{(w.x - Wold.x) * idt, (w.y - Wold.y) * idt, (w.z - Wold.z) * idt, (w.w - Wold.w) * idt};
   }
+  sink.put(i, z, s, WANT_DWDT, d);
 }
 
 // after gather_dt (+ wall terms): FINAL = false: stage 1 of RK2 -> W*, Z*, dW/dt; true: eq. 43 -> W^{n+1}
 template <class R, bool FINAL>
 __global__ void __launch_bounds__(256)
 update_kernel(MeshDev<R> m, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ Wn,
-              const Vec4<R> *__restrict__ acc, Vec4<R> *__restrict__ Wout, Vec4<R> *__restrict__ Zout,
-              R *__restrict__ spd_out, Vec4<R> *__restrict__ dWdt, int *status) {
+              const Vec4<R> *__restrict__ acc, Vec4<R> *__restrict__ Wout, VertexSink<R> sink, int *status) {
   MRD_CTL_GUARD(ctl)
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= m.nv) return;
@@ -272,16 +294,14 @@ update_kernel(MeshDev<R> m, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> 
   Vec4<R> a = ld4(&acc[i]);
   R av[4] = {a.x, a.y, a.z, a.w};
   bool fr = m.frozen ? (m.frozen[i] != 0) : false;
-  vertex_finish<R, !FINAL>(gamma, dt, __ldg(m.vol + i), fr, w, av, w, &Wout[i], &Zout[i],
-                           FINAL ? &spd_out[i] : nullptr, FINAL ? nullptr : &dWdt[i], status);
+  vertex_finish<R, !FINAL>(gamma, dt, __ldg(m.vol + i), fr, w, av, i, Wout, sink, status);
 }
 
 // stage 2: gather the total residuals and finish W^{n+1} = W* - dt/V sum Phi_i (eq. 61), in place over W*
 template <class R>
 __global__ void __launch_bounds__(256)
 gather_update_kernel(MeshDev<R> m, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ phi,
-                     const Vec4<R> *__restrict__ wall_acc, Vec4<R> *__restrict__ Ws, Vec4<R> *__restrict__ Zs,
-                     R *__restrict__ spd, int *status) {
+                     const Vec4<R> *__restrict__ wall_acc, Vec4<R> *__restrict__ Ws, VertexSink<R> sink, int *status) {
   MRD_CTL_GUARD(ctl)
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= m.nv) return;
@@ -298,7 +318,7 @@ gather_update_kernel(MeshDev<R> m, R gamma, const Ctl *__restrict__ ctl, const V
   R dt = (R)ctl_dt(ctl);
   Vec4<R> w = Ws[i];
   bool fr = m.frozen ? (m.frozen[i] != 0) : false;
-  vertex_finish<R, false>(gamma, dt, __ldg(m.vol + i), fr, w, a, w, &Ws[i], &Zs[i], &spd[i], nullptr, status);
+  vertex_finish<R, false>(gamma, dt, __ldg(m.vol + i), fr, w, a, i, Ws, sink, status);
 }
 
 // ---------------------------------------------------------------------------------------------

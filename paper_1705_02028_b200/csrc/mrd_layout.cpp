@@ -298,7 +298,7 @@ static void build_tile_plan(mrd_layout &L, const std::vector<double> &xyi) {
     }
     std::sort(uk.begin(), uk.end());
     uk.erase(std::unique(uk.begin(), uk.end()), uk.end());
-    nslot_of[b + 1] = (int32_t)uk.size();
+    nslot_of[b + 1] = (int32_t)((uk.size() + 3) / 4 * 4);  // padded: 16-byte granularity of the bulk copies
     for (int64_t t = t0; t < t1; ++t)
       for (int j = 0; j < 3; ++j) {
         int64_t key = nodekey[3 * (t - t0) + j];
@@ -310,8 +310,8 @@ static void build_tile_plan(mrd_layout &L, const std::vector<double> &xyi) {
   for (int64_t b = 0; b < ntile; ++b) L.tile_slot_off[b + 1] = L.tile_slot_off[b] + nslot_of[b + 1];
   const int64_t nslot = L.tile_slot_off[ntile];
   L.nslot = nslot;
-  L.slot_vertex.resize(nslot);
-  L.slot_xy.resize(2 * nslot);
+  L.slot_vertex.assign(nslot, -1);  // -1 = padding slot
+  L.slot_xy.assign(2 * nslot, 0.0);
   L.slot_ent_off.assign(nslot + 1, 0);
   L.slot_ent.resize(3 * nt);
   // pass 2: slot records and per-slot incidence counts
@@ -350,12 +350,32 @@ static void build_tile_plan(mrd_layout &L, const std::vector<double> &xyi) {
   }
   // vertex -> slots, ascending (slots are tile-major, so this is ascending triangle order)
   L.vslot_off.assign(nv + 1, 0);
-  for (int64_t s = 0; s < nslot; ++s) L.vslot_off[L.slot_vertex[s] + 1]++;
+  for (int64_t s = 0; s < nslot; ++s)
+    if (L.slot_vertex[s] >= 0) L.vslot_off[L.slot_vertex[s] + 1]++;
   for (int64_t i = 0; i < nv; ++i) L.vslot_off[i + 1] += L.vslot_off[i];
   L.vslot_ent.resize(nslot);
   {
     std::vector<int32_t> cur(L.vslot_off.begin(), L.vslot_off.end() - 1);
-    for (int64_t s = 0; s < nslot; ++s) L.vslot_ent[cur[L.slot_vertex[s]]++] = (int32_t)s;
+    for (int64_t s = 0; s < nslot; ++s)
+      if (L.slot_vertex[s] >= 0) L.vslot_ent[cur[L.slot_vertex[s]]++] = (int32_t)s;
+  }
+  L.vslot_ent.resize(L.vslot_off[nv]);
+  // per-tile plan record, one bulk copy: [T x 4] local slots of the triangle nodes, [3T] incidence entries grouped
+  // by slot, [offn] first entry of each slot (tile-local; padded with the end value)
+  int32_t maxs = 0;
+  for (int64_t b = 0; b < ntile; ++b) maxs = std::max(maxs, L.tile_slot_off[b + 1] - L.tile_slot_off[b]);
+  L.maxslots = maxs;
+  L.offn = (maxs + 1 + 7) / 8 * 8;
+  L.plan_stride = 7 * T + L.offn;
+  L.tile_plan.assign((size_t)ntile * L.plan_stride, 0);
+#pragma omp parallel for schedule(static)
+  for (int64_t b = 0; b < ntile; ++b) {
+    uint16_t *rec = &L.tile_plan[(size_t)b * L.plan_stride];
+    std::memcpy(rec, &L.tile_tri[(size_t)b * T * 4], sizeof(uint16_t) * 4 * T);
+    const int64_t e0 = 3 * b * T, e1 = std::min<int64_t>(3 * nt, e0 + 3 * T);
+    std::memcpy(rec + 4 * T, &L.slot_ent[e0], sizeof(uint16_t) * (e1 - e0));
+    const int32_t s0 = L.tile_slot_off[b], ns = L.tile_slot_off[b + 1] - s0;
+    for (int j = 0; j < L.offn; ++j) rec[7 * T + j] = (uint16_t)(L.slot_ent_off[s0 + std::min(j, ns)] - e0);
   }
 }
 

@@ -38,7 +38,9 @@ struct mrd_layout {
   std::vector<uint16_t> tile_tri;      // [ntile*tile][4]: tile-local vertex of nodes 0..2 (+ pad)
   std::vector<int32_t> slot_ent_off;   // [nslot+1]: tile-local incidence of each slot ...
   std::vector<uint16_t> slot_ent;      // ... entries (local triangle)*4 + node, ascending
-  std::vector<int32_t> vslot_off, vslot_ent;  // vertex -> its slots, ascending: [nv+1], [nslot]
+  std::vector<int32_t> vslot_off, vslot_ent;  // vertex -> its slots, ascending: [nv+1], [#real slots]
+  int32_t maxslots = 0, offn = 0, plan_stride = 0;  // largest (padded) slot count of a tile; plan record sizes
+  std::vector<uint16_t> tile_plan;     // [ntile][plan_stride]: tile_tri | slot_ent | tile-local slot offsets
 };
 
 namespace mrd_host {

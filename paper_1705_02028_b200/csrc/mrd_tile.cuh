@@ -1,31 +1,62 @@
-// mrd_tile.cuh -- the fused tile kernels (the production path): one thread block owns a run of
-// `tile` consecutive (Morton-ordered) triangles.
+// mrd_tile.cuh -- the fused tile kernels (the production path).  A tile is a run of `tile` consecutive
+// (Morton-ordered) triangles; a "slot" is one tile-local vertex (mrd_layout.h).  Persistent thread blocks
+// walk over tiles with a two-deep software pipeline:
 //
-//   prologue : the block's tile-local vertices ("slots", mrd_layout.h) are staged in shared memory ONCE:
-//              parameter vector Z, signal speed, tile-frame coordinates (stage 2 also dW/dt)
-//   body     : one thread per triangle; geometry of eq. 35 (L397-L399) from the staged coordinates,
-//              then S2-S5 / S9 of SURVEY 8a exactly as the unfused kernels (same device functions)
-//   epilogue : the distributed residuals go to shared memory and every slot sums its incident
-//              (triangle, node) entries in ascending order -> ONE partial per slot leaves the SM, instead
-//              of three 4-vectors per triangle (no float atomics, deterministic; replaces L734)
-// The vertex kernels then add a vertex's few partials (ascending slot = ascending triangle order).
+//   stage-in : everything a tile needs lives in CONTIGUOUS global ranges (slot-major copies of Z, |v|+c,
+//              dW/dt written by the vertex kernels; tile-frame coordinates; the tile's plan record; for
+//              stage 2 the stored phi^N(W^n), phi^T(W^n)), so one elected thread brings the NEXT tile in
+//              with a handful of TMA bulk copies (cp.async.bulk + mbarrier complete_tx) while the block
+//              computes the current one -- no gather by vertex index, no dependent global latency;
+//   body     : one thread per triangle; geometry of eq. 35 (L397-L399) from the staged coordinates, then
+//              S2-S5 / S9 of SURVEY 8a with the same device functions as the unfused kernels;
+//   epilogue : distributed residuals -> shared memory; every slot sums its incident (triangle, node) entries
+//              in ascending order; ONE partial per slot leaves the SM (deterministic; replaces the float
+//              atomics of L734 and the 3 x 4 values per triangle of the unfused design).
+// The vertex kernels add a vertex's few partials (ascending slot = ascending triangle order) and scatter
+// the new per-vertex quantities back to the vertex's slots.
 #pragma once
 #include "mrd_kernels.cuh"
 
 namespace mrd {
 
 template <class R> struct TileDev {
-  int32_t tile;
+  int32_t tile, maxslots, offn, plan_stride;
   int64_t ntile, nslot, nt;
-  const int32_t *tile_slot_off;  // [ntile+1]
-  const int32_t *slot_vertex;    // [nslot]
-  const R *slot_xy;              // [nslot][2], relative to the tile's first slot
-  const ushort4 *tile_tri;       // [ntile*tile]: tile-local slot of nodes 0..2
-  const int32_t *slot_ent_off;   // [nslot+1]
-  const uint16_t *slot_ent;      // [3 nt]: (local triangle)*4 + node, ascending
+  const int32_t *tile_slot_off;  // [ntile+1] (padded slot counts: multiples of 4)
+  const uint16_t *plan;          // [ntile][plan_stride]: tile_tri[T][4] | ent[3T] | off[offn]
+  const R *slot_xy;              // [nslot][2], relative to the tile's anchor vertex
   const int32_t *vslot_off;      // [nv+1]
-  const int32_t *vslot_ent;      // [nslot]
+  const int32_t *vslot_ent;      // [#real slots]
 };
+
+// ---- PTX wrappers: mbarrier + TMA bulk copy (SASS: UBLKCP) ----------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "MRD_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra MRD_DONE;\n"
+      "bra MRD_WAIT;\n"
+      "MRD_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
 // geometry of one CCW triangle from its vertex coordinates (eq. 35; reading C4):
 // the edge opposite node i runs from node i+1 to node i+2, inward normal (-e_y, e_x)
@@ -48,198 +79,192 @@ __device__ __forceinline__ void tile_geometry(const R x[3], const R y[3], TriGeo
   area3 = ((x[1] - x[0]) * (y[2] - y[0]) - (y[1] - y[0]) * (x[2] - x[0])) * (R(1) / R(6));
 }
 
-// shared-memory carve-up (dynamic): all arrays sized for the worst case of 3*tile slots
-template <class R> struct TileSmem {
-  Vec4<R> *Z;   // [3T]
-  Vec4<R> *D;   // [3T]  (stage 2: dW/dt)
-  R *X, *Y;     // [3T]
-  R *spd;       // [3T]  (stage 1)
-  R *res;       // [12][T]  component-major distributed residuals
-  R *sT;        // [T]
-  __device__ TileSmem(unsigned char *base, int T, bool stage2) {
-    Z = reinterpret_cast<Vec4<R> *>(base);
-    unsigned char *p = base + sizeof(Vec4<R>) * 3 * T;
-    if (stage2) { D = reinterpret_cast<Vec4<R> *>(p); p += sizeof(Vec4<R>) * 3 * T; } else { D = nullptr; }
-    X = reinterpret_cast<R *>(p); p += sizeof(R) * 3 * T;
-    Y = reinterpret_cast<R *>(p); p += sizeof(R) * 3 * T;
-    spd = reinterpret_cast<R *>(p); p += sizeof(R) * 3 * T;
-    res = reinterpret_cast<R *>(p); p += sizeof(R) * 12 * T;
-    sT = reinterpret_cast<R *>(p);
-  }
-  static size_t bytes(int T, bool stage2) {
-    return sizeof(Vec4<R>) * 3 * T * (stage2 ? 2 : 1) + sizeof(R) * (9 * T + 12 * T + T);
+// ---- shared-memory carve-up (dynamic).  Two stage-in buffers + the residual exchange area ----------------
+template <class R, int STAGE> struct TileSmem {
+  size_t oZ, oD, oS, oXY, oPlan, oPhi, buf_bytes;  // per buffer
+  size_t oRes, oST, oBar, total;                   // shared
+  __host__ __device__ static size_t up16(size_t x) { return (x + 15) & ~size_t(15); }
+  __host__ __device__ TileSmem(int T, int maxslots, int plan_stride) {
+    size_t o = 0;
+    oZ = o; o += up16(sizeof(Vec4<R>) * maxslots);
+    oD = o; if (STAGE == 2) o += up16(sizeof(Vec4<R>) * maxslots);
+    oS = o; if (STAGE == 1) o += up16(sizeof(R) * maxslots);
+    oXY = o; o += up16(sizeof(R) * 2 * maxslots);
+    oPlan = o; o += up16(sizeof(uint16_t) * plan_stride);
+    oPhi = o; if (STAGE == 2) o += up16(sizeof(R) * 16 * T);
+    buf_bytes = (o + 31) & ~size_t(31);
+    size_t s = 2 * buf_bytes;
+    oRes = s; s += sizeof(R) * 12 * T;
+    oST = s; s += up16(sizeof(R) * T);
+    oBar = s; s += 16;
+    total = s;
   }
 };
 
-// epilogue shared by both stages: per slot, ascending sum of its tile-local incidences
+// bring tile b into buffer `buf` (one thread): expect_tx, then the bulk copies
+template <class R, int STAGE>
+__device__ __forceinline__ void tile_stage_in(const TileDev<R> &td, const TileSmem<R, STAGE> &L, unsigned char *buf,
+                                              uint64_t *bar, int64_t b, int s0, int ns, const Vec4<R> *slotZ,
+                                              const R *slotS, const Vec4<R> *slotD, const R *phi16) {
+  const int T = td.tile;
+  const unsigned bZ = sizeof(Vec4<R>) * ns, bS = sizeof(R) * ns, bXY = sizeof(R) * 2 * ns;
+  const unsigned bPlan = sizeof(uint16_t) * td.plan_stride, bPhi = sizeof(R) * 16 * T;
+  unsigned total = bZ + bXY + bPlan + (STAGE == 1 ? bS : bZ + bPhi);
+  mbar_expect_tx(bar, total);
+  bulk_g2s(buf + L.oZ, slotZ + s0, bZ, bar);
+  bulk_g2s(buf + L.oXY, td.slot_xy + 2 * (int64_t)s0, bXY, bar);
+  bulk_g2s(buf + L.oPlan, td.plan + b * td.plan_stride, bPlan, bar);
+  if (STAGE == 1) {
+    bulk_g2s(buf + L.oS, slotS + s0, bS, bar);
+  } else {
+    bulk_g2s(buf + L.oD, slotD + s0, bZ, bar);
+    bulk_g2s(buf + L.oPhi, phi16 + b * 16 * T, bPhi, bar);
+  }
+}
+
+// epilogue shared by both stages: per slot, ascending sum of its tile-local incidences (all from shared memory)
 template <class R, bool WITH_ST>
-__device__ __forceinline__ void tile_epilogue(const TileDev<R> &td, const TileSmem<R> &sm, int s0, int ns,
-                                              Vec4<R> *__restrict__ part, R *__restrict__ partS) {
-  const int T = blockDim.x;
+__device__ __forceinline__ void tile_epilogue(int T, const R *res, const R *sT, const uint16_t *ent, const uint16_t *off,
+                                              int s0, int ns, Vec4<R> *__restrict__ part, R *__restrict__ partS) {
   for (int j = threadIdx.x; j < ns; j += T) {
-    const int32_t q0 = __ldg(td.slot_ent_off + s0 + j), q1 = __ldg(td.slot_ent_off + s0 + j + 1);
+    const int q0 = off[j], q1 = off[j + 1];
     R a0 = 0, a1 = 0, a2 = 0, a3 = 0, S = 0;
-    for (int32_t q = q0; q < q1; ++q) {
-      const int e = __ldg(td.slot_ent + q);
+    for (int q = q0; q < q1; ++q) {
+      const int e = ent[q];
       const int lt = e >> 2, nd = e & 3;
-      const R *r = sm.res + (nd * 4) * T + lt;
+      const R *r = res + (nd * 4) * T + lt;
       a0 += r[0];
       a1 += r[T];
       a2 += r[2 * T];
       a3 += r[3 * T];
-      if (WITH_ST) S += sm.sT[lt];
+      if (WITH_ST) S += sT[lt];
     }
     st4(&part[s0 + j], Vec4<R>{a0, a1, a2, a3});
     if (WITH_ST) partS[s0 + j] = S;
   }
 }
 
-template <class R, int SCHEME, bool STORE>
+// STAGE 1: SCHEME residuals of W^n -> partials, s_T sums, and (STORE) phi^N(W^n), phi^T(W^n) as phi16[tile][16][T]
+// STAGE 2: total residuals (eq. 57, 61-65; reading C12) -> partials
+template <class R, int SCHEME, int STAGE, bool STORE>
 __global__ void __launch_bounds__(256)
-tile_stage1_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ Z,
-                   const R *__restrict__ spd, Vec4<R> *__restrict__ part, R *__restrict__ partS,
-                   Vec4<R> *__restrict__ phiN_n, Vec4<R> *__restrict__ phiT_n, Vec4<R> *__restrict__ phi_dbg,
-                   R *__restrict__ sT_dbg, int *status) {
+tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ slotZ,
+            const R *__restrict__ slotS, const Vec4<R> *__restrict__ slotD, R *__restrict__ phi16,
+            Vec4<R> *__restrict__ part, R *__restrict__ partS, Vec4<R> *__restrict__ phi_dbg, R *__restrict__ sT_dbg,
+            int *status) {
   MRD_CTL_GUARD(ctl)
-  extern __shared__ __align__(32) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   const int T = blockDim.x, tid = threadIdx.x;
-  TileSmem<R> sm(smem_raw, T, false);
-  const int64_t b = blockIdx.x;
-  const int s0 = __ldg(td.tile_slot_off + b), ns = __ldg(td.tile_slot_off + b + 1) - s0;
-  for (int j = tid; j < ns; j += T) {
-    const int32_t v = __ldg(td.slot_vertex + s0 + j);
-    sm.Z[j] = ld4(&Z[v]);
-    sm.spd[j] = __ldg(spd + v);
-    sm.X[j] = __ldg(td.slot_xy + 2 * (int64_t)(s0 + j));
-    sm.Y[j] = __ldg(td.slot_xy + 2 * (int64_t)(s0 + j) + 1);
+  const TileSmem<R, STAGE> L(T, td.maxslots, td.plan_stride);
+  R *res = reinterpret_cast<R *>(smem_raw + L.oRes);
+  R *sST = reinterpret_cast<R *>(smem_raw + L.oST);
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + L.oBar);
+  if (tid == 0) {
+    mbar_init(&bar[0], 1);
+    mbar_init(&bar[1], 1);
+    fence_mbar_init();
   }
   __syncthreads();
-  const int64_t t = b * T + tid;
-  R pN[3][4];
-  R st = R(0);
-#pragma unroll
-  for (int i = 0; i < 3; ++i)
-#pragma unroll
-    for (int c = 0; c < 4; ++c) pN[i][c] = R(0);
-  if (t < td.nt) {
-    const ushort4 lv = __ldg(td.tile_tri + t);
-    const int l[3] = {lv.x, lv.y, lv.z};
-    Vec4<R> z[3] = {sm.Z[l[0]], sm.Z[l[1]], sm.Z[l[2]]};
-    R x[3] = {sm.X[l[0]], sm.X[l[1]], sm.X[l[2]]}, y[3] = {sm.Y[l[0]], sm.Y[l[1]], sm.Y[l[2]]};
-    TriGeom<R> g;
-    R area3, lmax;
-    tile_geometry(x, y, g, area3, lmax);
-    st = lmax * Fast<R>::max(sm.spd[l[0]], Fast<R>::max(sm.spd[l[1]], sm.spd[l[2]]));  // eq. 44-45
-    TriCore<R> k;
-    R pT[4];
-    triangle_core(gamma, z, g, k, pT, pN);
-    if (!k.ok) atomicOr(status, 1);
-    if (STORE) {
-      st4(&phiT_n[t], Vec4<R>{pT[0], pT[1], pT[2], pT[3]});
-#pragma unroll
-      for (int i = 0; i < 3; ++i) st4(&phiN_n[3 * t + i], Vec4<R>{pN[i][0], pN[i][1], pN[i][2], pN[i][3]});
-    }
-    if (SCHEME != MRD_SCHEME_N) {
-      R pL[3][4];
-      apply_beta(gamma, k, g, pT, pL);
-      if (SCHEME == MRD_SCHEME_B) {
-        blend(pT, pN, pL);
-      } else {
-#pragma unroll
-        for (int i = 0; i < 3; ++i)
-#pragma unroll
-          for (int c = 0; c < 4; ++c) pN[i][c] = pL[i][c];
+  int64_t b = blockIdx.x;
+  // slot range of the tile in flight; the next tile's range is fetched one iteration ahead
+  int s0 = __ldg(td.tile_slot_off + b), ns = __ldg(td.tile_slot_off + b + 1) - s0;
+  if (tid == 0) tile_stage_in<R, STAGE>(td, L, smem_raw, &bar[0], b, s0, ns, slotZ, slotS, slotD, phi16);
+  for (int k = 0; b < td.ntile; b += gridDim.x, ++k) {
+    const int cur = k & 1;
+    unsigned char *buf = smem_raw + cur * L.buf_bytes;
+    const int64_t nb = b + gridDim.x;
+    int s0n = 0, nsn = 0;
+    if (nb < td.ntile) {
+      s0n = __ldg(td.tile_slot_off + nb);
+      nsn = __ldg(td.tile_slot_off + nb + 1) - s0n;
+      if (tid == 0) {
+        fence_proxy_async();  // buffer cur^1 was read through the generic proxy in iteration k-1
+        tile_stage_in<R, STAGE>(td, L, smem_raw + (cur ^ 1) * L.buf_bytes, &bar[cur ^ 1], nb, s0n, nsn, slotZ, slotS, slotD,
+                                phi16);
       }
     }
-    if (phi_dbg) {
+    mbar_wait(&bar[cur], (k >> 1) & 1);
+    const Vec4<R> *sZ = reinterpret_cast<const Vec4<R> *>(buf + L.oZ);
+    const R *sXY = reinterpret_cast<const R *>(buf + L.oXY);
+    const uint16_t *plan = reinterpret_cast<const uint16_t *>(buf + L.oPlan);
+    const int64_t t = b * T + tid;
+    R pN[3][4];
+    R st = R(0);
 #pragma unroll
-      for (int i = 0; i < 3; ++i) st4(&phi_dbg[3 * t + i], Vec4<R>{pN[i][0], pN[i][1], pN[i][2], pN[i][3]});
-      sT_dbg[t] = st;
-    }
-  }
+    for (int i = 0; i < 3; ++i)
 #pragma unroll
-  for (int i = 0; i < 3; ++i)
+      for (int c = 0; c < 4; ++c) pN[i][c] = R(0);
+    if (t < td.nt) {
+      const ushort4 lv = reinterpret_cast<const ushort4 *>(plan)[tid];
+      const int l[3] = {lv.x, lv.y, lv.z};
+      Vec4<R> z[3] = {sZ[l[0]], sZ[l[1]], sZ[l[2]]};
+      R x[3] = {sXY[2 * l[0]], sXY[2 * l[1]], sXY[2 * l[2]]}, y[3] = {sXY[2 * l[0] + 1], sXY[2 * l[1] + 1], sXY[2 * l[2] + 1]};
+      TriGeom<R> g;
+      R a3, lmax;
+      tile_geometry(x, y, g, a3, lmax);
+      TriCore<R> kk;
+      R pT[4];
+      triangle_core(gamma, z, g, kk, pT, pN);  // stage 2: all matrices re-evaluated at W* (reading C12)
+      if (!kk.ok) atomicOr(status, 1);
+      R X[4] = {pT[0], pT[1], pT[2], pT[3]};
+      if (STAGE == 1) {
+        const R *sS = reinterpret_cast<const R *>(buf + L.oS);
+        st = lmax * Fast<R>::max(sS[l[0]], Fast<R>::max(sS[l[1]], sS[l[2]]));  // eq. 44-45
+        if (STORE) {
+          R *o = phi16 + b * 16 * T + tid;
 #pragma unroll
-    for (int c = 0; c < 4; ++c) sm.res[(i * 4 + c) * T + tid] = pN[i][c];
-  sm.sT[tid] = st;
-  __syncthreads();
-  tile_epilogue<R, true>(td, sm, s0, ns, part, partS);
-}
-
-template <class R, int SCHEME>
-__global__ void __launch_bounds__(256)
-tile_stage2_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ Zs,
-                   const Vec4<R> *__restrict__ dWdt, const Vec4<R> *__restrict__ phiN_n,
-                   const Vec4<R> *__restrict__ phiT_n, Vec4<R> *__restrict__ part, int *status) {
-  MRD_CTL_GUARD(ctl)
-  extern __shared__ __align__(32) unsigned char smem_raw[];
-  const int T = blockDim.x, tid = threadIdx.x;
-  TileSmem<R> sm(smem_raw, T, true);
-  const int64_t b = blockIdx.x;
-  const int s0 = __ldg(td.tile_slot_off + b), ns = __ldg(td.tile_slot_off + b + 1) - s0;
-  for (int j = tid; j < ns; j += T) {
-    const int32_t v = __ldg(td.slot_vertex + s0 + j);
-    sm.Z[j] = ld4(&Zs[v]);
-    sm.D[j] = ld4(&dWdt[v]);
-    sm.X[j] = __ldg(td.slot_xy + 2 * (int64_t)(s0 + j));
-    sm.Y[j] = __ldg(td.slot_xy + 2 * (int64_t)(s0 + j) + 1);
-  }
-  __syncthreads();
-  const int64_t t = b * T + tid;
-  R pN[3][4];
+          for (int i = 0; i < 3; ++i)
 #pragma unroll
-  for (int i = 0; i < 3; ++i)
+            for (int c = 0; c < 4; ++c) o[(i * 4 + c) * T] = pN[i][c];
 #pragma unroll
-    for (int c = 0; c < 4; ++c) pN[i][c] = R(0);
-  if (t < td.nt) {
-    const ushort4 lv = __ldg(td.tile_tri + t);
-    const int l[3] = {lv.x, lv.y, lv.z};
-    Vec4<R> z[3] = {sm.Z[l[0]], sm.Z[l[1]], sm.Z[l[2]]};
-    R x[3] = {sm.X[l[0]], sm.X[l[1]], sm.X[l[2]]}, y[3] = {sm.Y[l[0]], sm.Y[l[1]], sm.Y[l[2]]};
-    TriGeom<R> g;
-    R a3, lmax;
-    tile_geometry(x, y, g, a3, lmax);
-    TriCore<R> k;
-    R pT[4];
-    triangle_core(gamma, z, g, k, pT, pN);  // all matrices re-evaluated at W* (reading C12)
-    if (!k.ok) atomicOr(status, 1);
-    // eq. 57 / 61: Phi^T = |T|/3 sum_j dW_j/dt + (phi^T(W^n) + phi^T(W*))/2;  eq. 62 per node
-    R PT[4];
-    {
-      Vec4<R> o = ld4(&phiT_n[t]);
-      PT[0] = R(0.5) * (o.x + pT[0]); PT[1] = R(0.5) * (o.y + pT[1]);
-      PT[2] = R(0.5) * (o.z + pT[2]); PT[3] = R(0.5) * (o.w + pT[3]);
-    }
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      Vec4<R> d = sm.D[l[i]];
-      Vec4<R> o = ld4(&phiN_n[3 * t + i]);
-      R m0 = a3 * d.x, m1 = a3 * d.y, m2 = a3 * d.z, m3 = a3 * d.w;
-      PT[0] += m0; PT[1] += m1; PT[2] += m2; PT[3] += m3;
-      pN[i][0] = m0 + R(0.5) * (pN[i][0] + o.x);
-      pN[i][1] = m1 + R(0.5) * (pN[i][1] + o.y);
-      pN[i][2] = m2 + R(0.5) * (pN[i][2] + o.z);
-      pN[i][3] = m3 + R(0.5) * (pN[i][3] + o.w);
-    }
-    if (SCHEME != MRD_SCHEME_N) {
-      R pL[3][4];
-      apply_beta(gamma, k, g, PT, pL);  // eq. 63 with eq. 65
-      if (SCHEME == MRD_SCHEME_B) {
-        blend(PT, pN, pL);
+          for (int c = 0; c < 4; ++c) o[(12 + c) * T] = pT[c];
+        }
       } else {
+        // eq. 57 / 61: Phi^T = |T|/3 sum_j dW_j/dt + (phi^T(W^n) + phi^T(W*))/2;  eq. 62 per node
+        const Vec4<R> *sD = reinterpret_cast<const Vec4<R> *>(buf + L.oD);
+        const R *sP = reinterpret_cast<const R *>(buf + L.oPhi) + tid;
 #pragma unroll
-        for (int i = 0; i < 3; ++i)
+        for (int c = 0; c < 4; ++c) X[c] = R(0.5) * (sP[(12 + c) * T] + pT[c]);
 #pragma unroll
-          for (int c = 0; c < 4; ++c) pN[i][c] = pL[i][c];
+        for (int i = 0; i < 3; ++i) {
+          Vec4<R> d = sD[l[i]];
+          R m[4] = {a3 * d.x, a3 * d.y, a3 * d.z, a3 * d.w};
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            X[c] += m[c];
+            pN[i][c] = m[c] + R(0.5) * (pN[i][c] + sP[(i * 4 + c) * T]);
+          }
+        }
+      }
+      if (SCHEME != MRD_SCHEME_N) {
+        R pL[3][4];
+        apply_beta(gamma, kk, g, X, pL);  // eq. 50-51; stage 2: eq. 63 with eq. 65
+        if (SCHEME == MRD_SCHEME_B) {
+          blend(X, pN, pL);
+        } else {
+#pragma unroll
+          for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) pN[i][c] = pL[i][c];
+        }
+      }
+      if (STAGE == 1 && phi_dbg) {
+#pragma unroll
+        for (int i = 0; i < 3; ++i) st4(&phi_dbg[3 * t + i], Vec4<R>{pN[i][0], pN[i][1], pN[i][2], pN[i][3]});
+        sT_dbg[t] = st;
       }
     }
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) res[(i * 4 + c) * T + tid] = pN[i][c];
+    if (STAGE == 1) sST[tid] = st;
+    __syncthreads();
+    tile_epilogue<R, STAGE == 1>(T, res, sST, plan + 4 * T, plan + 7 * T, s0, ns, part, partS);
+    __syncthreads();  // res and buffer `cur` are free again
+    s0 = s0n;
+    ns = nsn;
   }
-#pragma unroll
-  for (int i = 0; i < 3; ++i)
-#pragma unroll
-    for (int c = 0; c < 4; ++c) sm.res[(i * 4 + c) * T + tid] = pN[i][c];
-  __syncthreads();
-  tile_epilogue<R, false>(td, sm, s0, ns, part, nullptr);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -271,7 +296,7 @@ template <class R>
 __global__ void __launch_bounds__(256)
 slot_gather_update_kernel(MeshDev<R> m, TileDev<R> td, R gamma, const Ctl *__restrict__ ctl,
                           const Vec4<R> *__restrict__ part, const Vec4<R> *__restrict__ wall_acc,
-                          Vec4<R> *__restrict__ Ws, Vec4<R> *__restrict__ Zs, R *__restrict__ spd, int *status) {
+                          Vec4<R> *__restrict__ Ws, VertexSink<R> sink, int *status) {
   MRD_CTL_GUARD(ctl)
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= m.nv) return;
@@ -288,7 +313,7 @@ slot_gather_update_kernel(MeshDev<R> m, TileDev<R> td, R gamma, const Ctl *__res
   R dt = (R)ctl_dt(ctl);
   Vec4<R> w = Ws[i];
   bool fr = m.frozen ? (m.frozen[i] != 0) : false;
-  vertex_finish<R, false>(gamma, dt, __ldg(m.vol + i), fr, w, a, w, &Ws[i], &Zs[i], &spd[i], nullptr, status);
+  vertex_finish<R, false>(gamma, dt, __ldg(m.vol + i), fr, w, a, i, Ws, sink, status);
 }
 
 }  // namespace mrd
