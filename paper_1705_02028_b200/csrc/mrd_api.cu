@@ -307,6 +307,13 @@ template <class K, class... Args> void launch_tile(mrd_mesh *m, K kernel, size_t
   kernel<<<(unsigned)grid, T, sh, s>>>(args...);
   m->launches++;
 }
+// tile sizes the fused kernels are compiled for
+#define MRD_TILE_DISPATCH(T, CALL) \
+  switch (T) {                     \
+    case 32: { constexpr int TILE = 32; CALL; } break;   \
+    case 64: { constexpr int TILE = 64; CALL; } break;   \
+    default: { constexpr int TILE = 128; CALL; } break;  \
+  }
 template <class R, int SCHEME> void launch_stage1(mrd_mesh *m, bool store, int a, cudaStream_t s) {
   using V4 = mrd::Vec4<R>;
   const R gamma = (R)m->L.p.gamma;
@@ -315,12 +322,15 @@ template <class R, int SCHEME> void launch_stage1(mrd_mesh *m, bool store, int a
     const size_t sh = mrd::TileSmem<R, 1>(td.tile, td.maxslots, td.plan_stride).total;
     V4 *dbg = m->dbg ? (V4 *)m->d_phi : nullptr;
     R *dbgs = m->dbg ? (R *)m->d_sT : nullptr;
-    if (store)
-      launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, true>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl, (const V4 *)m->d_slotZ[a],
-                  (const R *)m->d_slotS[a], (const V4 *)m->d_slotD, (R *)m->d_phi16, (V4 *)m->d_part, (R *)m->d_partS, dbg, dbgs, m->d_flag);
-    else
-      launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, false>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl, (const V4 *)m->d_slotZ[a],
-                  (const R *)m->d_slotS[a], (const V4 *)m->d_slotD, (R *)m->d_phi16, (V4 *)m->d_part, (R *)m->d_partS, dbg, dbgs, m->d_flag);
+    if (store) {
+      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, true, TILE>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
+                                              (const V4 *)m->d_slotZ[a], (const R *)m->d_slotS[a], (const V4 *)m->d_slotD, (R *)m->d_phi16,
+                                              (V4 *)m->d_part, (R *)m->d_partS, dbg, dbgs, m->d_flag)))
+    } else {
+      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, false, TILE>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
+                                              (const V4 *)m->d_slotZ[a], (const R *)m->d_slotS[a], (const V4 *)m->d_slotD, (R *)m->d_phi16,
+                                              (V4 *)m->d_part, (R *)m->d_partS, dbg, dbgs, m->d_flag)))
+    }
     return;
   }
   auto md = mesh_dev<R>(m);
@@ -339,9 +349,9 @@ template <class R, int SCHEME> void launch_stage2(mrd_mesh *m, int b, cudaStream
   if (m->fused) {
     auto td = tile_dev<R>(m);
     const size_t sh = mrd::TileSmem<R, 2>(td.tile, td.maxslots, td.plan_stride).total;
-    launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, false>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl, (const V4 *)m->d_slotZ[b],
-                (const R *)nullptr, (const V4 *)m->d_slotD, (R *)m->d_phi16, (V4 *)m->d_part, (R *)nullptr, (V4 *)nullptr, (R *)nullptr,
-                m->d_flag);
+    MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, false, TILE>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
+                                            (const V4 *)m->d_slotZ[b], (const R *)nullptr, (const V4 *)m->d_slotD, (R *)m->d_phi16,
+                                            (V4 *)m->d_part, (R *)nullptr, (V4 *)nullptr, (R *)nullptr, m->d_flag)))
     return;
   }
   auto md = mesh_dev<R>(m);

@@ -143,18 +143,46 @@ template <class R> struct TriCore {
 };
 
 // y = K x in the rotated frame of edge (nx, ny) with coefficients (a, b, l3):
-//   y0 = a x0 + b xn,  yn = b x0 + a xn,  yt = l3 xt,  y3 = l3 x3  -> accumulated into acc (sign s)
-template <class R>
-__device__ __forceinline__ void apply_split(R a, R b, R l3, R nx, R ny, const R x[4], R acc[4]) {
-  R xn = nx * x[1] + ny * x[2];
-  R xt = nx * x[2] - ny * x[1];
-  R y0 = a * x[0] + b * xn;
-  R yn = b * x[0] + a * xn;
+//   y0 = a x0 + b xn,  yn = b x0 + a xn,  yt = l3 xt,  y3 = l3 x3,  (y1, y2) = rotation back of (yn, yt).
+// ACC = false: y is overwritten; ACC = true: added to y.  Written as explicit FMA chains (the fp64 pipe is the
+// binding unit of the sweep: every DADD saved counts).
+template <bool ACC, class R>
+__device__ __forceinline__ void apply_split(R a, R b, R l3, R nx, R ny, const R x[4], R y[4]) {
+  using F = Fast<R>;
+  R xn = F::fma_(nx, x[1], ny * x[2]);
+  R xt = F::fma_(nx, x[2], -(ny * x[1]));
+  R yn = F::fma_(b, x[0], a * xn);
   R yt = l3 * xt;
-  acc[0] += y0;
-  acc[1] += nx * yn - ny * yt;
-  acc[2] += ny * yn + nx * yt;
-  acc[3] += l3 * x[3];
+  if (ACC) {
+    y[0] = F::fma_(a, x[0], F::fma_(b, xn, y[0]));
+    y[1] = F::fma_(nx, yn, F::fma_(-ny, yt, y[1]));
+    y[2] = F::fma_(ny, yn, F::fma_(nx, yt, y[2]));
+    y[3] = F::fma_(l3, x[3], y[3]);
+  } else {
+    y[0] = F::fma_(a, x[0], b * xn);
+    y[1] = F::fma_(nx, yn, -(ny * yt));
+    y[2] = F::fma_(ny, yn, nx * yt);
+    y[3] = l3 * x[3];
+  }
+}
+// the unsplit K_i = (l_i/2)(A nx + B ny) applied to x: in symmetrising variables
+//   y0 = wl x0 + cl (n.x),  (y1, y2) = wl (x1, x2) + cl x0 (nx, ny),  y3 = wl x3      (wl = l/2 w, cl = l/2 c)
+template <bool ACC, class R>
+__device__ __forceinline__ void apply_full(R wl, R cl, R nx, R ny, const R x[4], R y[4]) {
+  using F = Fast<R>;
+  R xn = F::fma_(nx, x[1], ny * x[2]);
+  R t = cl * x[0];
+  if (ACC) {
+    y[0] = F::fma_(wl, x[0], F::fma_(cl, xn, y[0]));
+    y[1] = F::fma_(wl, x[1], F::fma_(t, nx, y[1]));
+    y[2] = F::fma_(wl, x[2], F::fma_(t, ny, y[2]));
+    y[3] = F::fma_(wl, x[3], y[3]);
+  } else {
+    y[0] = F::fma_(wl, x[0], cl * xn);
+    y[1] = F::fma_(wl, x[1], t * nx);
+    y[2] = F::fma_(wl, x[2], t * ny);
+    y[3] = wl * x[3];
+  }
 }
 
 // symmetrising variables -> conserved variables (unit reference density)
@@ -219,34 +247,50 @@ __device__ __forceinline__ void triangle_core(R gamma, const Vec4<R> Z[3], const
     dq[j][3] = dp - c2 * drho;
   }
 
-  // O4: per edge the split eigenvalues (eq. 41-42) and the sums over edges
+  // O4: per edge the split eigenvalues (eq. 41-42) and the sums over edges.  With q = l_i/8 the halves
+  // lambda^(+/-)/2 = q lambda +/- |q lambda| come out of one addition each (scaling by powers of two is exact).
   R s00 = 0, s01 = 0, s02 = 0, s11 = 0, s12 = 0, s22 = 0, s33 = 0;
   R accm[4] = {0, 0, 0, 0};   // sum_j K_j^- dq_j
   R phiq[4] = {0, 0, 0, 0};   // sum_j K_j dq_j = phi^T (eq. 36)
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
     R nx = g.nx[i], ny = g.ny[i], hl = g.hl[i];
-    R wl = hl * (k.u * nx + k.v * ny);
-    R cl = hl * k.c;
-    R l1 = wl + cl, l2 = wl - cl, l3 = wl;
-    R l1p = R(0.5) * (l1 + F::abs(l1)), l2p = R(0.5) * (l2 + F::abs(l2)), l3p = R(0.5) * (l3 + F::abs(l3));
-    R l1m = l1 - l1p, l2m = l2 - l2p, l3m = l3 - l3p;
-    R ap = R(0.5) * (l1p + l2p), bp = R(0.5) * (l1p - l2p);
-    R am = R(0.5) * (l1m + l2m), bm = R(0.5) * (l1m - l2m);
+    R wn = F::fma_(k.u, nx, k.v * ny);
+    R hq = R(0.25) * hl;
+    R wq = hq * wn, cq = hq * k.c;            // (l_i/8) w, (l_i/8) c
+    R l1q = wq + cq, l2q = wq - cq;
+    R p1 = l1q + F::abs(l1q), p2 = l2q + F::abs(l2q);  // l1+/2, l2+/2
+    R m1 = l1q - F::abs(l1q), m2 = l2q - F::abs(l2q);  // l1-/2, l2-/2
+    R ap = p1 + p2, bp = p1 - p2, am = m1 + m2, bm = m1 - m2;
+    R l3h = wq + wq;                          // l3/2
+    R l3p = l3h + F::abs(l3h), l3m = l3h - F::abs(l3h);
     k.ap[i] = ap;
     k.bp[i] = bp;
     k.l3p[i] = l3p;
     R nxx = nx * nx, nyy = ny * ny, nxy = nx * ny;
-    s00 += am;
-    s01 += bm * nx;
-    s02 += bm * ny;
-    s11 += am * nxx + l3m * nyy;
-    s12 += (am - l3m) * nxy;
-    s22 += am * nyy + l3m * nxx;
-    s33 += l3m;
-    if (i > 0) {
-      apply_split(am, bm, l3m, nx, ny, dq[i], accm);
-      apply_split(wl, cl, wl, nx, ny, dq[i], phiq);
+    if (i == 0) {  // (0 + x is not x for x = -0, so the compiler keeps additions to a zero accumulator)
+      s00 = am;
+      s01 = bm * nx;
+      s02 = bm * ny;
+      s11 = F::fma_(am, nxx, l3m * nyy);
+      s12 = (am - l3m) * nxy;
+      s22 = F::fma_(am, nyy, l3m * nxx);
+      s33 = l3m;
+    } else {
+      s00 += am;
+      s01 = F::fma_(bm, nx, s01);
+      s02 = F::fma_(bm, ny, s02);
+      s11 = F::fma_(am, nxx, F::fma_(l3m, nyy, s11));
+      s12 = F::fma_(am - l3m, nxy, s12);
+      s22 = F::fma_(am, nyy, F::fma_(l3m, nxx, s22));
+      s33 += l3m;
+    }
+    if (i == 1) {
+      apply_split<false>(am, bm, l3m, nx, ny, dq[i], accm);
+      apply_full<false>(hl * wn, hl * k.c, nx, ny, dq[i], phiq);
+    } else if (i == 2) {
+      apply_split<true>(am, bm, l3m, nx, ny, dq[i], accm);
+      apply_full<true>(hl * wn, hl * k.c, nx, ny, dq[i], phiq);
     }
   }
 
@@ -272,14 +316,20 @@ __device__ __forceinline__ void triangle_core(R gamma, const Vec4<R> Z[3], const
   win[1] = k.n01 * accm[0] + k.n11 * accm[1] + k.n12 * accm[2];
   win[2] = k.n02 * accm[0] + k.n12 * accm[1] + k.n22 * accm[2];
   win[3] = k.ns * accm[3];
+  // nodes 0 and 1 directly; node 2 from sum_i phi_i^N = phi^T, which holds identically because sum_i K_i = 0 and
+  // N-hat sum_j K_j^- = I (in the stagnation case both entropy parts vanish): 8 additions instead of ~26 operations
 #pragma unroll
-  for (int i = 0; i < 3; ++i) {
-    R d[4] = {dq[i][0] - win[0], dq[i][1] - win[1], dq[i][2] - win[2], dq[i][3] - win[3]};
-    R y[4] = {0, 0, 0, 0};
-    apply_split(k.ap[i], k.bp[i], k.l3p[i], g.nx[i], g.ny[i], d, y);
+  for (int i = 0; i < 2; ++i) {
+    R d[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) d[c] = i == 0 ? -win[c] : dq[i][c] - win[c];  // dq_0 = 0
+    R y[4];
+    apply_split<false>(k.ap[i], k.bp[i], k.l3p[i], g.nx[i], g.ny[i], d, y);
     to_conserved(k, y, phiN[i]);
   }
   to_conserved(k, phiq, phiT);
+#pragma unroll
+  for (int c = 0; c < 4; ++c) phiN[2][c] = (phiT[c] - phiN[0][c]) - phiN[1][c];
 }
 
 // eq. 50-51: out_i = beta_i X = -K_i^+ N-hat X for a conserved-variable vector X (phi^T in stage 1,
@@ -295,8 +345,8 @@ __device__ __forceinline__ void apply_beta(R gamma, const TriCore<R> &k, const T
   y[3] = -(k.ns * q[3]);
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    R z[4] = {0, 0, 0, 0};
-    apply_split(k.ap[i], k.bp[i], k.l3p[i], g.nx[i], g.ny[i], y, z);
+    R z[4];
+    apply_split<false>(k.ap[i], k.bp[i], k.l3p[i], g.nx[i], g.ny[i], y, z);
     to_conserved(k, z, out[i]);
   }
 }

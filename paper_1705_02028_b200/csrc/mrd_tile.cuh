@@ -122,7 +122,8 @@ __device__ __forceinline__ void tile_stage_in(const TileDev<R> &td, const TileSm
   }
 }
 
-// epilogue shared by both stages: per slot, ascending sum of its tile-local incidences (all from shared memory)
+// epilogue shared by both stages: per slot, ascending sum of its tile-local incidences (all from shared memory).
+// (A (slot, component)-parallel variant was measured: 15 % slower -- the kernel is issue-bound, not barrier-bound.)
 template <class R, bool WITH_ST>
 __device__ __forceinline__ void tile_epilogue(int T, const R *res, const R *sT, const uint16_t *ent, const uint16_t *off,
                                               int s0, int ns, Vec4<R> *__restrict__ part, R *__restrict__ partS) {
@@ -146,15 +147,19 @@ __device__ __forceinline__ void tile_epilogue(int T, const R *res, const R *sT, 
 
 // STAGE 1: SCHEME residuals of W^n -> partials, s_T sums, and (STORE) phi^N(W^n), phi^T(W^n) as phi16[tile][16][T]
 // STAGE 2: total residuals (eq. 57, 61-65; reading C12) -> partials
-template <class R, int SCHEME, int STAGE, bool STORE>
-__global__ void __launch_bounds__(256)
+#ifndef MRD_TILE_MINB
+#define MRD_TILE_MINB 4
+#endif
+template <class R, int SCHEME, int STAGE, bool STORE, int TILE>
+__global__ void __launch_bounds__(TILE, (MRD_TILE_MINB * 128) / TILE)
 tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ slotZ,
             const R *__restrict__ slotS, const Vec4<R> *__restrict__ slotD, R *__restrict__ phi16,
             Vec4<R> *__restrict__ part, R *__restrict__ partS, Vec4<R> *__restrict__ phi_dbg, R *__restrict__ sT_dbg,
             int *status) {
   MRD_CTL_GUARD(ctl)
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  const int T = blockDim.x, tid = threadIdx.x;
+  constexpr int T = TILE;  // compile-time tile size: shared-memory and phi16 strides become immediates
+  const int tid = threadIdx.x;
   const TileSmem<R, STAGE> L(T, td.maxslots, td.plan_stride);
   R *res = reinterpret_cast<R *>(smem_raw + L.oRes);
   R *sST = reinterpret_cast<R *>(smem_raw + L.oST);
@@ -169,17 +174,25 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
   // slot range of the tile in flight; the next tile's range is fetched one iteration ahead
   int s0 = __ldg(td.tile_slot_off + b), ns = __ldg(td.tile_slot_off + b + 1) - s0;
   if (tid == 0) tile_stage_in<R, STAGE>(td, L, smem_raw, &bar[0], b, s0, ns, slotZ, slotS, slotD, phi16);
+  int s0n = 0, s1n = 0;  // slot range of the next tile: loaded one iteration before it is needed
+  if (b + gridDim.x < td.ntile) {
+    s0n = __ldg(td.tile_slot_off + b + gridDim.x);
+    s1n = __ldg(td.tile_slot_off + b + gridDim.x + 1);
+  }
+  bool bad = false;  // linearised c^2 <= 0 met by this thread (raised once, after the loop)
   for (int k = 0; b < td.ntile; b += gridDim.x, ++k) {
     const int cur = k & 1;
     unsigned char *buf = smem_raw + cur * L.buf_bytes;
     const int64_t nb = b + gridDim.x;
-    int s0n = 0, nsn = 0;
+    const int s0x = s0n, nsx = s1n - s0n;
     if (nb < td.ntile) {
-      s0n = __ldg(td.tile_slot_off + nb);
-      nsn = __ldg(td.tile_slot_off + nb + 1) - s0n;
+      if (nb + gridDim.x < td.ntile) {  // in flight during this iteration, consumed at the top of the next one
+        s0n = __ldg(td.tile_slot_off + nb + gridDim.x);
+        s1n = __ldg(td.tile_slot_off + nb + gridDim.x + 1);
+      }
       if (tid == 0) {
         fence_proxy_async();  // buffer cur^1 was read through the generic proxy in iteration k-1
-        tile_stage_in<R, STAGE>(td, L, smem_raw + (cur ^ 1) * L.buf_bytes, &bar[cur ^ 1], nb, s0n, nsn, slotZ, slotS, slotD,
+        tile_stage_in<R, STAGE>(td, L, smem_raw + (cur ^ 1) * L.buf_bytes, &bar[cur ^ 1], nb, s0x, nsx, slotZ, slotS, slotD,
                                 phi16);
       }
     }
@@ -190,10 +203,6 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
     const int64_t t = b * T + tid;
     R pN[3][4];
     R st = R(0);
-#pragma unroll
-    for (int i = 0; i < 3; ++i)
-#pragma unroll
-      for (int c = 0; c < 4; ++c) pN[i][c] = R(0);
     if (t < td.nt) {
       const ushort4 lv = reinterpret_cast<const ushort4 *>(plan)[tid];
       const int l[3] = {lv.x, lv.y, lv.z};
@@ -205,7 +214,7 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
       TriCore<R> kk;
       R pT[4];
       triangle_core(gamma, z, g, kk, pT, pN);  // stage 2: all matrices re-evaluated at W* (reading C12)
-      if (!kk.ok) atomicOr(status, 1);
+      bad |= !kk.ok;
       R X[4] = {pT[0], pT[1], pT[2], pT[3]};
       if (STAGE == 1) {
         const R *sS = reinterpret_cast<const R *>(buf + L.oS);
@@ -253,6 +262,11 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
         for (int i = 0; i < 3; ++i) st4(&phi_dbg[3 * t + i], Vec4<R>{pN[i][0], pN[i][1], pN[i][2], pN[i][3]});
         sT_dbg[t] = st;
       }
+    } else {  // padding thread of the last tile: contributes nothing
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) pN[i][c] = R(0);
     }
 #pragma unroll
     for (int i = 0; i < 3; ++i)
@@ -262,9 +276,10 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
     __syncthreads();
     tile_epilogue<R, STAGE == 1>(T, res, sST, plan + 4 * T, plan + 7 * T, s0, ns, part, partS);
     __syncthreads();  // res and buffer `cur` are free again
-    s0 = s0n;
-    ns = nsn;
+    s0 = s0x;
+    ns = nsx;
   }
+  if (bad) atomicOr(status, 1);
 }
 
 // ---------------------------------------------------------------------------------------------
