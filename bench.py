@@ -30,14 +30,23 @@ METRIC = "triangle_updates_per_s_rk2_step"
 UNIT = "triangle-updates/s"
 
 # ---- per-unit algorithmic figures --------------------------------
-# FLOPs per triangle per stage: min(oracle operation count, FLOPs the kernel executes); the kernel's
-# count (2*DFMA + DADD + DMUL per thread, straight-line SASS, checked against ncu) is the smaller one.
-FLOPS_TRI_STAGE1 = {"fp64": 799.0, "fp32": 799.0}
-FLOPS_TRI_STAGE2 = {"fp64": 881.0, "fp32": 881.0}
-ORACLE_FLOPS_TRI = (2098.0, 2194.0)     # oracle.count_ops(stage 1 / stage 2): add+mul+div+sqrt, context only
-# compulsory HBM bytes per triangle of the stage-1 triangle kernel AS DESIGNED
-BYTES_TRI_STAGE1 = {"fp64": 360.0, "fp32": 186.0}
-BYTES_TRI_STAGE2 = {"fp64": 348.0, "fp32": 180.0}
+# FLOPs per triangle per stage = min(oracle operation count, FLOPs the kernel executes).  The kernel's count
+# (2*DFMA + DADD + DMUL per thread, from ncu's smsp__sass_thread_inst_executed_op_d*_pred_on of the profiled
+# launch, profiles/) is the smaller one; the oracle's own count (orc_count_ops) is kept for context.
+FLOPS_TRI_STAGE1 = {"fp64": 836.0, "fp32": 783.0}
+FLOPS_TRI_STAGE2 = {"fp64": 905.0, "fp32": 852.0}
+FLOPS_VERTEX_STAGE = 60.0              # per vertex per stage: gather adds, update, Z and signal speed
+ORACLE_FLOPS_TRI = (2098.0, 2194.0)    # oracle.count_ops(stage 1 / stage 2): add+mul+div+sqrt
+# compulsory HBM bytes per triangle of one triangle-kernel launch (share of SURVEY 8d's 130 B per triangle-update):
+# state read once (32 B per vertex / 2), connectivity 12 B, coordinates 8 B; stage 2 also reads W^n (dW/dt)
+BYTES_TRI_STAGE1 = {"fp64": 36.0, "fp32": 24.0}
+BYTES_TRI_STAGE2 = {"fp64": 52.0, "fp32": 32.0}
+# bytes the fused kernels move BY DESIGN (slot copies, plan record, stored phi^N/phi^T, partials), for comparison
+# with ncu's dram__bytes (the roofline object's `traffic`)
+DESIGN_BYTES_TRI = {"tri_stage1": {"fp64": 204.0, "fp32": 110.0}, "tri_stage2": {"fp64": 214.0, "fp32": 115.0}}
+# ncu dram__bytes_read.sum + dram__bytes_write.sum per triangle of the profiled launches (profiles/*.md)
+NCU_TRAFFIC_BYTES_TRI = {"tri_stage1": {"fp64": 199.5}, "tri_stage2": {"fp64": 216.3}}
+B_ALG_STEP = {"fp64": 130.0, "fp32": 76.0}
 
 
 def measured_peaks():
@@ -186,12 +195,11 @@ def run_mrd(args):
     gm.set_state(W0)
 
     # ---- device-resident throughput: W warm-up steps, then exactly K timed steps -------------------------
-    gm.step(args.warmup)
-    barrier()
-    l0 = gm.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local) as clk:
+        gm.step(args.warmup)
         barrier()
+        l0 = gm.launch_count()
         e0.record(stream)
         gm.step_async(args.steps)
         e1.record(stream)
@@ -253,8 +261,8 @@ def run_mrd(args):
     main = {k: v for k, v in prof.items() if k in ("tri_stage1", "tri_stage2", "gather_dt", "update", "gather_update")}
     dom = max(main, key=main.get)
     dom_ms = main[dom]
-    flops_unit = {"tri_stage1": FLOPS_TRI_STAGE1[prec], "tri_stage2": FLOPS_TRI_STAGE2[prec]}.get(dom, 30.0)
-    bytes_unit = {"tri_stage1": BYTES_TRI_STAGE1[prec], "tri_stage2": BYTES_TRI_STAGE2[prec]}.get(dom, 160.0)
+    flops_unit = {"tri_stage1": FLOPS_TRI_STAGE1[prec], "tri_stage2": FLOPS_TRI_STAGE2[prec]}.get(dom, FLOPS_VERTEX_STAGE / 2)
+    bytes_unit = {"tri_stage1": BYTES_TRI_STAGE1[prec], "tri_stage2": BYTES_TRI_STAGE2[prec]}.get(dom, 40.0)
     alu_peak = fp64_peak_nominal(sm_max, prec)
     t_alu = flops_unit * nt / (alu_peak * 1e12)
     t_hbm = bytes_unit * nt / (hbm_gbs * 1e9)
@@ -268,16 +276,21 @@ def run_mrd(args):
     else:
         ach = bytes_unit * nt / (dom_ms * 1e-3) * 1e-9
         roof = {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs}
-    roof.update({"traffic": args.traffic, "kernel": dom, "kernel_ms": dom_ms, "peak_source": hbm_src if roof["bound"] == "hbm"
+    traffic = args.traffic
+    if traffic is None and dom in NCU_TRAFFIC_BYTES_TRI and prec in NCU_TRAFFIC_BYTES_TRI[dom] and args.tile in (0, 128):
+        traffic = NCU_TRAFFIC_BYTES_TRI[dom][prec] * nt      # per launch, from the committed ncu capture of this kernel
+    roof.update({"traffic": traffic, "kernel": dom, "kernel_ms": dom_ms, "peak_source": hbm_src if roof["bound"] == "hbm"
                  else "derived: 148 SM x %d lanes x 2 x %.0f MHz" % (64 if prec == "fp64" else 128, sm_max),
                  "alg_flops_per_triangle": flops_unit, "alg_bytes_per_triangle": bytes_unit,
                  "alu_frac": flops_unit * nt / (dom_ms * 1e-3) * 1e-12 / alu_peak,
                  "hbm_frac": bytes_unit * nt / (dom_ms * 1e-3) * 1e-9 / hbm_gbs,
                  "measured_fma_tflops": dfma_tf if prec == "fp64" else ffma_tf, "measured_copy_gbs": copy_gbs,
+                 "design_bytes_per_triangle": DESIGN_BYTES_TRI.get(dom, {}).get(prec),
                  "kernels_ms": prof,
-                 "step_alg": {"flops_per_triangle_update": FLOPS_TRI_STAGE1[prec] + FLOPS_TRI_STAGE2[prec] + 30.0,
-                              "roofline_ms": max((FLOPS_TRI_STAGE1[prec] + FLOPS_TRI_STAGE2[prec] + 30.0) * nt / (alu_peak * 1e12),
-                                                 (130.0 if prec == "fp64" else 76.0) * nt / (hbm_gbs * 1e9)) * 1e3}})
+                 "step_alg": {"flops_per_triangle_update": FLOPS_TRI_STAGE1[prec] + FLOPS_TRI_STAGE2[prec] + FLOPS_VERTEX_STAGE,
+                              "bytes_per_triangle_update": B_ALG_STEP[prec],
+                              "roofline_ms": max((FLOPS_TRI_STAGE1[prec] + FLOPS_TRI_STAGE2[prec] + FLOPS_VERTEX_STAGE) * nt / (alu_peak * 1e12),
+                                                 B_ALG_STEP[prec] * nt / (hbm_gbs * 1e9)) * 1e3}})
     roof["step_alg"]["frac"] = roof["step_alg"]["roofline_ms"] / ms_step
 
     # ---- the oracle beside it (rank 0, N = 1 only): bounded sample of the same workload --------------------
