@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- triangle-updates/s of the residual-distribution sweep (BASELINE.json metric) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mrd|reference] [--n 4096]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mrd|reference] [--size 4096]
                     [--precision fp64|fp32] [--numbering morton|natural|permuted] [--reorder 0|1]
 
 A "step" is one RK2 time step of scheme B (both stages, dt reduction included) over the whole mesh:
@@ -15,7 +15,6 @@ from __future__ import annotations
 import argparse
 import json
 import os
-import subprocess
 import sys
 import threading
 import time
@@ -33,8 +32,8 @@ UNIT = "triangle-updates/s"
 # FLOPs per triangle per stage = min(oracle operation count, FLOPs the kernel executes).  The kernel's count
 # (2*DFMA + DADD + DMUL per thread, from ncu's smsp__sass_thread_inst_executed_op_d*_pred_on of the profiled
 # launch, profiles/) is the smaller one; the oracle's own count (orc_count_ops) is kept for context.
-FLOPS_TRI_STAGE1 = {"fp64": 836.0, "fp32": 783.0}
-FLOPS_TRI_STAGE2 = {"fp64": 905.0, "fp32": 852.0}
+FLOPS_TRI_STAGE1 = {"fp64": 736.0, "fp32": 690.0}
+FLOPS_TRI_STAGE2 = {"fp64": 817.0, "fp32": 770.0}
 FLOPS_VERTEX_STAGE = 60.0              # per vertex per stage: gather adds, update, Z and signal speed
 ORACLE_FLOPS_TRI = (2098.0, 2194.0)    # oracle.count_ops(stage 1 / stage 2): add+mul+div+sqrt
 # compulsory HBM bytes per triangle of one triangle-kernel launch (share of SURVEY 8d's 130 B per triangle-update):
@@ -45,7 +44,7 @@ BYTES_TRI_STAGE2 = {"fp64": 52.0, "fp32": 32.0}
 # with ncu's dram__bytes (the roofline object's `traffic`)
 DESIGN_BYTES_TRI = {"tri_stage1": {"fp64": 204.0, "fp32": 110.0}, "tri_stage2": {"fp64": 214.0, "fp32": 115.0}}
 # ncu dram__bytes_read.sum + dram__bytes_write.sum per triangle of the profiled launches (profiles/*.md)
-NCU_TRAFFIC_BYTES_TRI = {"tri_stage1": {"fp64": 199.5}, "tri_stage2": {"fp64": 216.3}}
+NCU_TRAFFIC_BYTES_TRI = {"tri_stage1": {"fp64": 204.8}, "tri_stage2": {"fp64": 216.9}}
 B_ALG_STEP = {"fp64": 130.0, "fp32": 76.0}
 
 
@@ -60,51 +59,72 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md)."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons sampled DURING the timed region (B200_PROFILING.md), through NVML
+    (nvidia_ml_py; the same counters nvidia-smi prints) every 20 ms from a background thread."""
+    REASONS = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
 
     def __init__(self, index: int):
-        self.rows, self.proc, self.index = [], None, index
+        self.index, self.sm, self.mask, self.max_mhz, self.power = index, [], 0, None, []
+        self._stop = threading.Event()
+        self._thread = None
 
     def __enter__(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.thread = threading.Thread(target=self._read, daemon=True)
-            self.thread.start()
+            import pynvml
+            pynvml.nvmlInit()
+            visible = os.environ.get("CUDA_VISIBLE_DEVICES")
+            idx = self.index
+            if visible:
+                try:
+                    idx = int(visible.split(",")[self.index])
+                except Exception:
+                    pass
+            self._nvml = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(idx)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
         except Exception:
-            self.proc = None
+            self._thread = None
         return self
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
+    def _run(self):
+        n = self._nvml
+        while not self._stop.is_set():
+            try:
+                self.sm.append(float(n.nvmlDeviceGetClockInfo(self._h, n.NVML_CLOCK_SM)))
+                self.mask |= int(n.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                self.power.append(n.nvmlDeviceGetPowerUsage(self._h) / 1000.0)
+            except Exception:
+                pass
+            self._stop.wait(0.02)
 
     def __exit__(self, *a):
-        if self.proc:
-            self.proc.terminate()
-            try:
-                self.proc.wait(timeout=2)
-            except Exception:
-                self.proc.kill()
+        self._stop.set()
+        if self._thread:
+            self._thread.join(timeout=2)
 
     def summary(self):
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
-            try:
-                sm.append(float(r[0])); mx.append(float(r[1]))
-            except Exception:
-                continue
-            for nme, val in zip(names, r[3:7]):
-                if val.lower().startswith("active"):
-                    reasons.add(nme)
-        if not sm:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
-                "samples": len(sm)}
+        if not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(self.sm)), "sm_min_mhz": float(min(self.sm)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(k for k, bit in self.REASONS.items() if self.mask & bit), "samples": len(self.sm),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+def max_over_ranks(value: float, dist, device) -> float:
+    """Multi-rank timings are the MAX over ranks (one process per GPU); identity for a single process."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(world: int, units_per_rank: int, steps: int, seconds: float) -> float:
+    """Weak scaling: every rank steps its own replica; value = all units processed / max-over-ranks time."""
+    return world * units_per_rank * steps / seconds
 
 
 def build_workload(n: int, numbering: str):
@@ -207,14 +227,10 @@ def run_mrd(args):
         barrier()
     n_done, t_sim, _ = gm.sync()
     launches = gm.launch_count() - l0
-    ms_total = e0.elapsed_time(e1)
-    if dist is not None:
-        tt = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
+    ms_total = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
     assert n_done == args.warmup + args.steps, (n_done, args.warmup, args.steps)
     ms_step = ms_total / args.steps
-    value = world * nt * args.steps / (ms_total * 1e-3)
+    value = whole_job_rate(world, nt, args.steps, ms_total * 1e-3)
 
     # ---- live per-kernel durations (CUDA events on the launching stream), averaged over 5 steps ------------
     prof = {}
@@ -239,13 +255,9 @@ def run_mrd(args):
         gm.get_state_host(h_out.numpy())
         h_in, h_out = h_out, h_in
     torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        tt = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_s = float(tt.item())
+    e2e_s = max_over_ranks(time.perf_counter() - t0, dist, "cuda")
     state_bytes = 4 * nv * (8 if prec == "fp64" else 4)
-    e2e = {"value": world * nt * ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+    e2e = {"value": whole_job_rate(world, nt, ke, e2e_s), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
            "d2h_bytes_per_step": state_bytes, "steps": ke, "ms_per_step": e2e_s / ke * 1e3,
            "api": "mrd_set_state_host + mrd_step(1) + mrd_get_state_host, pinned host buffers"}
 
@@ -326,7 +338,7 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="mrd", choices=["mrd", "reference"])
-    ap.add_argument("--n", type=int, default=4096, help="vertices per side of the periodic mesh")
+    ap.add_argument("--size", dest="n", type=int, default=4096, help="vertices per side of the periodic mesh")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
     ap.add_argument("--numbering", default="morton", choices=["morton", "natural", "permuted"])
     ap.add_argument("--reorder", type=int, default=1)
