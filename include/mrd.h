@@ -135,6 +135,11 @@ int mrd_get_diagnostics(mrd_mesh *m, double totals[4], double *min_rho, double *
 int mrd_dump_stage1(mrd_mesh *m, double *phiT, double *phiN, double *phiLDA, double *phiB, double *sT,
                     void *stream);
 
+/* As mrd_dump_stage1 for a SAMPLE of triangles (full-size meshes): tri_user[n_sample] HOST user triangle ids;
+ * outputs are HOST arrays indexed by sample: phiT[n][4], phiN/phiLDA/phiB[n][3][4], sT[n]; any may be NULL. */
+int mrd_dump_stage1_sample(mrd_mesh *m, int64_t n_sample, const int64_t *tri_user, double *phiT, double *phiN,
+                           double *phiLDA, double *phiB, double *sT, void *stream);
+
 /* Micro-benchmarks of the device the roofline is quoted against (host out, any may be NULL):
  * dependent-chain-free DFMA and FFMA loops (TFLOP/s, 2 flops per FMA) and a device-to-device copy
  * (GB/s, read + write bytes). Synchronises. */

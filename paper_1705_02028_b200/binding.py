@@ -57,6 +57,7 @@ def lib():
         L.mrd_sync.argtypes = [vp, vp, _lp, _dp, _dp]
         L.mrd_get_diagnostics.argtypes = [vp, _dp, _dp, _dp, vp]
         L.mrd_dump_stage1.argtypes = [vp, _dp, _dp, _dp, _dp, _dp, vp]
+        L.mrd_dump_stage1_sample.argtypes = [vp, C.c_int64, _lp, _dp, _dp, _dp, _dp, _dp, vp]
         L.mrd_measure_peaks.argtypes = [_dp, _dp, _dp, vp]
         L.mrd_launch_count.argtypes = [vp, _lp]
         L.mrd_step_profile.argtypes = [vp, vp, C.POINTER(C.c_float)]
@@ -230,6 +231,17 @@ class Mesh:
         _check(lib().mrd_dump_stage1(self._h, _np_ptr(o["phiT"], C.c_double), _np_ptr(o["phiN"], C.c_double),
                                      _np_ptr(o["phiLDA"], C.c_double), _np_ptr(o["phiB"], C.c_double),
                                      _np_ptr(o["sT"], C.c_double), _stream_ptr(stream)))
+        return o
+
+    def dump_stage1_sample(self, tri_ids, stream=None):
+        ids = np.ascontiguousarray(tri_ids, dtype=np.int64)
+        n = len(ids)
+        o = dict(phiT=np.empty((n, 4)), phiN=np.empty((n, 3, 4)), phiLDA=np.empty((n, 3, 4)), phiB=np.empty((n, 3, 4)),
+                 sT=np.empty(n))
+        _check(lib().mrd_dump_stage1_sample(self._h, n, _np_ptr(ids, C.c_int64), _np_ptr(o["phiT"], C.c_double),
+                                            _np_ptr(o["phiN"], C.c_double), _np_ptr(o["phiLDA"], C.c_double),
+                                            _np_ptr(o["phiB"], C.c_double), _np_ptr(o["sT"], C.c_double),
+                                            _stream_ptr(stream)))
         return o
 
     PROFILE_SLOTS = ("tri_stage1", "gather_dt", "wall1", "update", "tri_stage2", "wall2", "gather_update", "ctl")

@@ -586,6 +586,79 @@ template <class R> int dump_impl(mrd_mesh *m, double *phiT, double *phiN, double
   return MRD_OK;
 }
 
+// sampled variant of dump_impl: only the listed USER triangles are copied back (full-size meshes)
+template <class R> int dump_sample_impl(mrd_mesh *m, int64_t ns, const int64_t *ids, double *phiT, double *phiN, double *phiLDA,
+                                        double *phiB, double *sT, cudaStream_t s) {
+  using V4 = mrd::Vec4<R>;
+  const int64_t nt = m->L.nt;
+  for (int64_t q = 0; q < ns; ++q)
+    if (ids[q] < 0 || ids[q] >= nt) return fail(MRD_EINVAL, "sample triangle id out of range");
+  mrd::Ctl c{};
+  int rc;
+  if ((rc = fetch_ctl(m, s, &c))) return rc;
+  mrd::Ctl armed = c;
+  armed.active = 1;
+  CUDA_TRY(cudaMemcpyAsync(m->d_ctl, &armed, sizeof armed, cudaMemcpyHostToDevice, s));
+  if (m->fused && !m->d_phi) {
+    V4 *p = nullptr;
+    R *st = nullptr;
+    if ((rc = dev_alloc(m, &p, 3 * nt)) || (rc = dev_alloc(m, &st, nt))) return rc;
+    m->d_phi = p;
+    m->d_sT = st;
+  }
+  m->dbg = m->fused;
+  const int a = m->cur;
+  R buf[12];
+  auto fetch3 = [&](const void *base, int64_t k, int64_t q, double *dst) -> cudaError_t {  // [nt][3][4] layout
+    cudaError_t e = cudaMemcpy(buf, (const R *)base + 12 * k, sizeof(R) * 12, cudaMemcpyDeviceToHost);
+    for (int i = 0; i < 3; ++i) {
+      int iu = (m->L.tswap[k] && i > 0) ? 3 - i : i;
+      for (int x = 0; x < 4; ++x) dst[12 * q + 4 * iu + x] = (double)buf[4 * i + x];
+    }
+    return e;
+  };
+  for (int pass = 0; pass < 2; ++pass) {
+    if (pass == 0) launch_stage1<R, MRD_SCHEME_LDA>(m, true, a, s);
+    else launch_stage1<R, MRD_SCHEME_B>(m, true, a, s);
+    CUDA_TRY(cudaStreamSynchronize(s));
+    CUDA_TRY(cudaGetLastError());
+    double *dst = pass == 0 ? phiLDA : phiB;
+    if (dst)
+      for (int64_t q = 0; q < ns; ++q) CUDA_TRY(fetch3(m->d_phi, m->L.trank[ids[q]], q, dst));
+  }
+  m->dbg = false;
+  for (int64_t q = 0; q < ns; ++q) {
+    const int64_t k = m->L.trank[ids[q]];
+    R v16[16];
+    if (m->fused) {
+      const int T = m->L.tile;
+      const R *o = (const R *)m->d_phi16 + (size_t)(k / T) * 16 * T + (k % T);
+      CUDA_TRY(cudaMemcpy2D(v16, sizeof(R), o, sizeof(R) * T, sizeof(R), 16, cudaMemcpyDeviceToHost));
+    } else {
+      CUDA_TRY(cudaMemcpy(v16, (const R *)m->d_phiN + 12 * k, sizeof(R) * 12, cudaMemcpyDeviceToHost));
+      CUDA_TRY(cudaMemcpy(v16 + 12, (const R *)m->d_phiT + 4 * k, sizeof(R) * 4, cudaMemcpyDeviceToHost));
+    }
+    if (phiN)
+      for (int i = 0; i < 3; ++i) {
+        int iu = (m->L.tswap[k] && i > 0) ? 3 - i : i;
+        for (int x = 0; x < 4; ++x) phiN[12 * q + 4 * iu + x] = (double)v16[4 * i + x];
+      }
+    if (phiT)
+      for (int x = 0; x < 4; ++x) phiT[4 * q + x] = (double)v16[12 + x];
+    if (sT) {
+      R v;
+      CUDA_TRY(cudaMemcpy(&v, (const R *)m->d_sT + k, sizeof(R), cudaMemcpyDeviceToHost));
+      sT[q] = (double)v;
+    }
+  }
+  int flag = 0;
+  CUDA_TRY(cudaMemcpy(&flag, m->d_flag, sizeof(int), cudaMemcpyDeviceToHost));
+  CUDA_TRY(cudaMemcpy(m->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice));
+  CUDA_TRY(cudaMemset(m->d_flag, 0, sizeof(int)));
+  if (flag) return fail(MRD_ENONPHYSICAL, "non-physical linearised state");
+  return MRD_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -746,6 +819,15 @@ int mrd_dump_stage1(mrd_mesh *m, double *phiT, double *phiN, double *phiLDA, dou
   cudaStream_t s = (cudaStream_t)stream;
   return m->L.p.precision == MRD_FP64 ? dump_impl<double>(m, phiT, phiN, phiLDA, phiB, sT, s)
                                       : dump_impl<float>(m, phiT, phiN, phiLDA, phiB, sT, s);
+}
+
+int mrd_dump_stage1_sample(mrd_mesh *m, int64_t n_sample, const int64_t *tri_user, double *phiT, double *phiN, double *phiLDA,
+                           double *phiB, double *sT, void *stream) {
+  if (!m || (n_sample > 0 && !tri_user) || n_sample < 0) return fail(MRD_EINVAL, "bad argument");
+  if (!m->has_state) return fail(MRD_EINVAL, "no state set");
+  cudaStream_t s = (cudaStream_t)stream;
+  return m->L.p.precision == MRD_FP64 ? dump_sample_impl<double>(m, n_sample, tri_user, phiT, phiN, phiLDA, phiB, sT, s)
+                                      : dump_sample_impl<float>(m, n_sample, tri_user, phiT, phiN, phiLDA, phiB, sT, s);
 }
 
 int mrd_step_profile(mrd_mesh *m, void *stream, float ms[MRD_PROFILE_SLOTS]) {

@@ -124,6 +124,33 @@ __device__ __forceinline__ bool vertex_prepare(R gamma, const Vec4<R> &W, Vec4<R
   return ok;
 }
 
+// fp64: the per-vertex kernels are bound by HBM, not by arithmetic, so Z and the signal speed are evaluated with
+// IEEE-rounded division / square root and without FMA contraction, operation by operation as eq. 10, 20, 45 are
+// written.  This matters on fine meshes: the triangle kernels difference Z between neighbouring vertices
+// (delta = Z_j - Z_1 ~ h), so an ulp of error in Z is 1/h ulps in every residual.
+template <>
+__device__ __forceinline__ bool vertex_prepare<double>(double gamma, const Vec4<double> &W, Vec4<double> &Z, double &speed,
+                                                       double &p_out) {
+  const double g1 = gamma - 1.0;
+  double rho = W.x;
+  bool ok = rho > 0.0;
+  double rs = ok ? rho : 1.0;
+  double u = __ddiv_rn(W.y, rs), v = __ddiv_rn(W.z, rs);
+  double m2 = __dadd_rn(__dmul_rn(W.y, W.y), __dmul_rn(W.z, W.z));
+  double p = __dmul_rn(g1, __dadd_rn(W.w, -__ddiv_rn(__dmul_rn(0.5, m2), rs)));
+  p_out = p;
+  ok = ok && (p > 0.0);
+  double ps = ok ? p : 1.0;
+  double h = __ddiv_rn(__dadd_rn(W.w, ps), rs);
+  double s = __dsqrt_rn(rs);
+  Z.x = s;
+  Z.y = __dmul_rn(s, u);
+  Z.z = __dmul_rn(s, v);
+  Z.w = __dmul_rn(s, h);
+  speed = __dadd_rn(__dsqrt_rn(__dadd_rn(__dmul_rn(u, u), __dmul_rn(v, v))), __dsqrt_rn(__ddiv_rn(__dmul_rn(gamma, ps), rs)));
+  return ok;
+}
+
 // ---------------------------------------------------------------------------------------------
 // One triangle at one state: everything the distribution needs.
 // ---------------------------------------------------------------------------------------------

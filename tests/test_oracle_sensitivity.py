@@ -31,3 +31,12 @@ def test_round_off_is_amplified_on_grid_aligned_shocks_but_not_on_smooth_flow():
     assert drift(wl.make_config("sod", n=256), 200) > 1e-7
     assert drift(wl.make_config("vortex", n=32), 100) < 1e-12
     assert drift(wl.make_config("kh", n=48), 100) < 1e-9
+
+
+@pytest.mark.slow
+def test_round_off_amplification_grows_with_resolution_on_the_smooth_vortex():
+    # the blend coefficient Theta = |phi| / sum |phi^N| divides an O(h^2) residual by O(h) ones: a 1-ulp
+    # perturbation of a smooth state is amplified the more the finer the mesh (transiently, then it saturates)
+    coarse = drift(wl.make_config("sweep", n=128), 4, amp=1e-16)
+    fine = drift(wl.make_config("sweep", n=512), 4, amp=1e-16)
+    assert coarse < 1e-14 and fine > 20 * coarse
