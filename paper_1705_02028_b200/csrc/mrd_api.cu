@@ -247,8 +247,7 @@ template <class R> int upload_impl(mrd_mesh *m) {
   {
     V4 *a = nullptr, *d = nullptr, *p = nullptr, *pn = nullptr, *pt = nullptr;
     R *st = nullptr, *us = nullptr;
-    if ((rc = dev_alloc(m, &a, nv))) return rc;
-    if (!m->fused && ((rc = dev_alloc(m, &d, nv)) || (rc = dev_alloc(m, &p, 3 * nt)) || (rc = dev_alloc(m, &st, nt)) ||
+    if (!m->fused && ((rc = dev_alloc(m, &a, nv)) || (rc = dev_alloc(m, &d, nv)) || (rc = dev_alloc(m, &p, 3 * nt)) || (rc = dev_alloc(m, &st, nt)) ||
                       (rc = dev_alloc(m, &pn, 3 * nt)) || (rc = dev_alloc(m, &pt, nt))))
       return rc;
     if ((rc = dev_alloc(m, &us, 4 * nv))) return rc;
@@ -388,46 +387,84 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
     default: launch_stage1<R, MRD_SCHEME_B>(m, rk2, a, s); break;
   }
   PROF_MARK(MRD_PROF_TRI1)
-  if (m->fused)
-    mrd::slot_gather_dt_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, tile_dev<R>(m), m->d_ctl, (const V4 *)m->d_part, (const R *)m->d_partS, (V4 *)m->d_acc);
-  else
-    mrd::gather_dt_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, m->d_ctl, (const V4 *)m->d_phi, (const R *)m->d_sT, (V4 *)m->d_acc);
-  m->launches++;
-  PROF_MARK(MRD_PROF_GATHER_DT)
-  if (m->nwv > 0) {
-    mrd::wall_kernel<R, 1><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[a], (V4 *)m->d_acc);
+  const unsigned vb = blocks_for(md.nv, 256);
+  if (m->fused) {
+    // fused path: dt from the partial s_T sums alone; the update kernels gather the residual partials themselves
+    auto td = tile_dev<R>(m);
+    mrd::slot_dt_kernel<R><<<vb, 256, 0, s>>>(md, td, m->d_ctl, (const R *)m->d_partS);
     m->launches++;
-    PROF_MARK(MRD_PROF_WALL1)
-  }
-  if (!rk2) {
-    mrd::update_kernel<R, true><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_acc, (V4 *)m->d_W[b],
-                                                                    sink_for<R>(m, b, true, false), m->d_flag);
-    m->launches++;
-    PROF_MARK(MRD_PROF_UPDATE)
-  } else {
-    mrd::update_kernel<R, false><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_acc, (V4 *)m->d_W[b],
-                                                                     sink_for<R>(m, b, false, true), m->d_flag);
-    m->launches++;
-    PROF_MARK(MRD_PROF_UPDATE)
-    switch (scheme) {
-      case MRD_SCHEME_N: launch_stage2<R, MRD_SCHEME_N>(m, b, s); break;
-      case MRD_SCHEME_LDA: launch_stage2<R, MRD_SCHEME_LDA>(m, b, s); break;
-      default: launch_stage2<R, MRD_SCHEME_B>(m, b, s); break;
-    }
-    PROF_MARK(MRD_PROF_TRI2)
+    PROF_MARK(MRD_PROF_GATHER_DT)
     if (m->nwv > 0) {
-      mrd::wall_kernel<R, 2><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[b], (V4 *)m->d_wall_acc);
+      mrd::wall_kernel<R, 1, true><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[a],
+                                                                        (V4 *)m->d_wall_acc);
       m->launches++;
-      PROF_MARK(MRD_PROF_WALL2)
+      PROF_MARK(MRD_PROF_WALL1)
     }
-    if (m->fused)
-      mrd::slot_gather_update_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, tile_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
-                                                                            (V4 *)m->d_W[b], sink_for<R>(m, b, true, false), m->d_flag);
-    else
-      mrd::gather_update_kernel<R><<<blocks_for(md.nv, 256), 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_phi, (const V4 *)m->d_wall_acc, (V4 *)m->d_W[b],
-                                                                       sink_for<R>(m, b, true, false), m->d_flag);
+    if (!rk2) {
+      mrd::slot_gather_update_kernel<R, 1><<<vb, 256, 0, s>>>(md, td, gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
+                                                           (const V4 *)m->d_W[a], (V4 *)m->d_W[b], sink_for<R>(m, b, true, false), m->d_flag);
+      m->launches++;
+      PROF_MARK(MRD_PROF_UPDATE)
+    } else {
+      mrd::slot_gather_update_kernel<R, 0><<<vb, 256, 0, s>>>(md, td, gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
+                                                           (const V4 *)m->d_W[a], (V4 *)m->d_W[b], sink_for<R>(m, b, false, true), m->d_flag);
+      m->launches++;
+      PROF_MARK(MRD_PROF_UPDATE)
+      switch (scheme) {
+        case MRD_SCHEME_N: launch_stage2<R, MRD_SCHEME_N>(m, b, s); break;
+        case MRD_SCHEME_LDA: launch_stage2<R, MRD_SCHEME_LDA>(m, b, s); break;
+        default: launch_stage2<R, MRD_SCHEME_B>(m, b, s); break;
+      }
+      PROF_MARK(MRD_PROF_TRI2)
+      if (m->nwv > 0) {
+        mrd::wall_kernel<R, 2><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[b],
+                                                                    (V4 *)m->d_wall_acc);
+        m->launches++;
+        PROF_MARK(MRD_PROF_WALL2)
+      }
+      mrd::slot_gather_update_kernel<R, 2><<<vb, 256, 0, s>>>(md, td, gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
+                                                           (const V4 *)m->d_W[b], (V4 *)m->d_W[b], sink_for<R>(m, b, true, false), m->d_flag);
+      m->launches++;
+      PROF_MARK(MRD_PROF_GATHER_UPDATE)
+    }
+  } else {
+    // unfused comparison path: per-triangle residuals through HBM, CSR gathers, acc round trip
+    mrd::gather_dt_kernel<R><<<vb, 256, 0, s>>>(md, m->d_ctl, (const V4 *)m->d_phi, (const R *)m->d_sT, (V4 *)m->d_acc);
     m->launches++;
-    PROF_MARK(MRD_PROF_GATHER_UPDATE)
+    PROF_MARK(MRD_PROF_GATHER_DT)
+    if (m->nwv > 0) {
+      mrd::wall_kernel<R, 1, false><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[a],
+                                                                         (V4 *)m->d_acc);
+      m->launches++;
+      PROF_MARK(MRD_PROF_WALL1)
+    }
+    if (!rk2) {
+      mrd::update_kernel<R, true><<<vb, 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_acc, (V4 *)m->d_W[b],
+                                                  sink_for<R>(m, b, true, false), m->d_flag);
+      m->launches++;
+      PROF_MARK(MRD_PROF_UPDATE)
+    } else {
+      mrd::update_kernel<R, false><<<vb, 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_acc, (V4 *)m->d_W[b],
+                                                   sink_for<R>(m, b, false, true), m->d_flag);
+      m->launches++;
+      PROF_MARK(MRD_PROF_UPDATE)
+      switch (scheme) {
+        case MRD_SCHEME_N: launch_stage2<R, MRD_SCHEME_N>(m, b, s); break;
+        case MRD_SCHEME_LDA: launch_stage2<R, MRD_SCHEME_LDA>(m, b, s); break;
+        default: launch_stage2<R, MRD_SCHEME_B>(m, b, s); break;
+      }
+      PROF_MARK(MRD_PROF_TRI2)
+      if (m->nwv > 0) {
+        mrd::wall_kernel<R, 2><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[b],
+                                                                    (V4 *)m->d_wall_acc);
+        m->launches++;
+        PROF_MARK(MRD_PROF_WALL2)
+      }
+      mrd::gather_update_kernel<R><<<vb, 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_phi, (const V4 *)m->d_wall_acc, (V4 *)m->d_W[b],
+                                                   sink_for<R>(m, b, true, false), m->d_flag);
+      m->launches++;
+      PROF_MARK(MRD_PROF_GATHER_UPDATE)
+    }
   }
   mrd::ctl_kernel<<<1, 1, 0, s>>>(m->d_ctl, 1, 0.0, m->d_flag);
   m->launches++;

@@ -324,7 +324,7 @@ gather_update_kernel(MeshDev<R> m, R gamma, const Ctl *__restrict__ ctl, const V
 // ---------------------------------------------------------------------------------------------
 // Reflecting walls (eq. 68-71; alpha = 0.75; outward normal, reading C15): one thread per
 // wall VERTEX adds, in ascending edge order, the correction of every wall edge it belongs to.
-//   stage 1: dst[v] += Phi^c(W^n)            (dst = acc of gather_dt)
+//   stage 1: dst[v] += Phi^c(W^n)            (dst = acc of gather_dt; SET: dst[v] = ..., dst = wall_acc, fused path)
 //   stage 2: dst[v]  = sum (Phi^c(W^n) + Phi^c(W*))/2   (dst = wall_acc, zero elsewhere)
 // ---------------------------------------------------------------------------------------------
 template <class R> struct WallDev {
@@ -344,7 +344,7 @@ template <class R> __device__ __forceinline__ void wall_flux(R gamma, const Vec4
   F[3] = -((W.w + p) * vn);
 }
 
-template <class R, int STAGE>
+template <class R, int STAGE, bool SET = (STAGE == 2)>
 __global__ void wall_kernel(WallDev<R> wd, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ Wn,
                             const Vec4<R> *__restrict__ Ws, Vec4<R> *__restrict__ dst) {
   MRD_CTL_GUARD(ctl)
@@ -373,11 +373,12 @@ __global__ void wall_kernel(WallDev<R> wd, R gamma, const Ctl *__restrict__ ctl,
       for (int c = 0; c < 4; ++c) s[c] += R(0.5) * (hl * (ca * Fa[c] + cb * Fb[c]) + hl * (ca * Ga[c] + cb * Gb[c]));
     }
   }
-  Vec4<R> d = dst[vtx];
-  if (STAGE == 1) {
-    d.x += s[0]; d.y += s[1]; d.z += s[2]; d.w += s[3];
-  } else {
+  Vec4<R> d;
+  if (SET) {
     d = Vec4<R>{s[0], s[1], s[2], s[3]};
+  } else {
+    d = dst[vtx];
+    d.x += s[0]; d.y += s[1]; d.z += s[2]; d.w += s[3];
   }
   dst[vtx] = d;
 }

@@ -124,10 +124,23 @@ __device__ __forceinline__ bool vertex_prepare(R gamma, const Vec4<R> &W, Vec4<R
   return ok;
 }
 
-// fp64: the per-vertex kernels are bound by HBM, not by arithmetic, so Z and the signal speed are evaluated with
-// IEEE-rounded division / square root and without FMA contraction, operation by operation as eq. 10, 20, 45 are
-// written.  This matters on fine meshes: the triangle kernels difference Z between neighbouring vertices
-// (delta = Z_j - Z_1 ~ h), so an ulp of error in Z is 1/h ulps in every residual.
+// fp64 per-vertex quantities, operation by operation as eq. 10, 20, 45 are written and without FMA contraction of
+// the formulas themselves.  Quotients by rho use ONE reciprocal plus a residual correction each
+// (q = a r; q += fma(-q, rho, a) r: correctly rounded except in rare half-ulp cases), square roots the analogous
+// correction of x rsqrt(x).  This matters on fine meshes: the triangle kernels difference Z between neighbouring
+// vertices (delta = Z_j - Z_1 ~ h), so an ulp of error in Z is 1/h ulps in every residual; with these forms Z and the
+// signal speed equal the oracle's IEEE results bit for bit in all but rare cases, at a quarter of the instructions
+// of CUDA's IEEE division/sqrt subroutines (the update kernels became fp64-bound with those).
+__device__ __forceinline__ double div_by(double a, double rho, double r) {
+  double q = a * r;
+  return fma(fma(-q, rho, a), r, q);
+}
+__device__ __forceinline__ double sqrt_near(double x) {
+  if (!(x > 0.0)) return 0.0;
+  double y = Fast<double>::rsqrt(x);
+  double sq = x * y;
+  return fma(fma(-sq, sq, x), 0.5 * y, sq);
+}
 template <>
 __device__ __forceinline__ bool vertex_prepare<double>(double gamma, const Vec4<double> &W, Vec4<double> &Z, double &speed,
                                                        double &p_out) {
@@ -135,19 +148,21 @@ __device__ __forceinline__ bool vertex_prepare<double>(double gamma, const Vec4<
   double rho = W.x;
   bool ok = rho > 0.0;
   double rs = ok ? rho : 1.0;
-  double u = __ddiv_rn(W.y, rs), v = __ddiv_rn(W.z, rs);
+  double r = Fast<double>::rcp(rs);
+  r = fma(fma(-rs, r, 1.0), r, r);
+  double u = div_by(W.y, rs, r), v = div_by(W.z, rs, r);
   double m2 = __dadd_rn(__dmul_rn(W.y, W.y), __dmul_rn(W.z, W.z));
-  double p = __dmul_rn(g1, __dadd_rn(W.w, -__ddiv_rn(__dmul_rn(0.5, m2), rs)));
+  double p = __dmul_rn(g1, __dadd_rn(W.w, -div_by(__dmul_rn(0.5, m2), rs, r)));
   p_out = p;
   ok = ok && (p > 0.0);
   double ps = ok ? p : 1.0;
-  double h = __ddiv_rn(__dadd_rn(W.w, ps), rs);
-  double s = __dsqrt_rn(rs);
-  Z.x = s;
-  Z.y = __dmul_rn(s, u);
-  Z.z = __dmul_rn(s, v);
-  Z.w = __dmul_rn(s, h);
-  speed = __dadd_rn(__dsqrt_rn(__dadd_rn(__dmul_rn(u, u), __dmul_rn(v, v))), __dsqrt_rn(__ddiv_rn(__dmul_rn(gamma, ps), rs)));
+  double h = div_by(__dadd_rn(W.w, ps), rs, r);
+  double sr = sqrt_near(rs);
+  Z.x = sr;
+  Z.y = __dmul_rn(sr, u);
+  Z.z = __dmul_rn(sr, v);
+  Z.w = __dmul_rn(sr, h);
+  speed = __dadd_rn(sqrt_near(__dadd_rn(__dmul_rn(u, u), __dmul_rn(v, v))), sqrt_near(div_by(__dmul_rn(gamma, ps), rs, r)));
   return ok;
 }
 

@@ -285,33 +285,31 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
 // ---------------------------------------------------------------------------------------------
 // vertex side of the fused path: add the vertex's partials (ascending slot order)
 // ---------------------------------------------------------------------------------------------
+// S7 on the fused path: d_i = 2 V_i / sum of the vertex's partial s_T sums (eq. 44), block minimum -> atomicMin
 template <class R>
 __global__ void __launch_bounds__(256)
-slot_gather_dt_kernel(MeshDev<R> m, TileDev<R> td, Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ part,
-                      const R *__restrict__ partS, Vec4<R> *__restrict__ acc) {
+slot_dt_kernel(MeshDev<R> m, TileDev<R> td, Ctl *__restrict__ ctl, const R *__restrict__ partS) {
   MRD_CTL_GUARD(ctl)
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   double d = __longlong_as_double(0x7FF0000000000000ll);
   if (i < m.nv) {
-    R a0 = 0, a1 = 0, a2 = 0, a3 = 0, S = 0;
+    R S = 0;
     const int32_t q0 = __ldg(td.vslot_off + i), q1 = __ldg(td.vslot_off + i + 1);
-    for (int32_t q = q0; q < q1; ++q) {
-      const int32_t s = __ldg(td.vslot_ent + q);
-      Vec4<R> f = ld4(&part[s]);
-      a0 += f.x; a1 += f.y; a2 += f.z; a3 += f.w;
-      S += __ldg(partS + s);
-    }
-    st4(&acc[i], Vec4<R>{a0, a1, a2, a3});
-    d = 2.0 * (double)__ldg(m.vol + i) / (double)S;  // eq. 44
+    for (int32_t q = q0; q < q1; ++q) S += __ldg(partS + __ldg(td.vslot_ent + q));
+    d = 2.0 * (double)__ldg(m.vol + i) / (double)S;
   }
   block_min_to_global(d, &ctl->dmin_bits);
 }
 
-template <class R>
+// S8 / S10 / S12 on the fused path: gather the vertex's partials (ascending slot order), add the wall terms, update.
+//   MODE 0: stage 1 of RK2   W* = W^n - dt/V sum        (Win -> Wout; Z*, dW/dt to the slots)
+//   MODE 1: single stage     W^{n+1} = W^n - dt/V sum   (Win -> Wout; Z, |v|+c to the slots)        eq. 43
+//   MODE 2: stage 2 of RK2   W^{n+1} = W* - dt/V sum    (in place: Win == Wout; Z, |v|+c to the slots) eq. 61
+template <class R, int MODE>
 __global__ void __launch_bounds__(256)
 slot_gather_update_kernel(MeshDev<R> m, TileDev<R> td, R gamma, const Ctl *__restrict__ ctl,
-                          const Vec4<R> *__restrict__ part, const Vec4<R> *__restrict__ wall_acc,
-                          Vec4<R> *__restrict__ Ws, VertexSink<R> sink, int *status) {
+                          const Vec4<R> *__restrict__ part, const Vec4<R> *__restrict__ wall_acc, const Vec4<R> *Win,
+                          Vec4<R> *Wout, VertexSink<R> sink, int *status) {
   MRD_CTL_GUARD(ctl)
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= m.nv) return;
@@ -326,9 +324,9 @@ slot_gather_update_kernel(MeshDev<R> m, TileDev<R> td, R gamma, const Ctl *__res
     a[0] += f.x; a[1] += f.y; a[2] += f.z; a[3] += f.w;
   }
   R dt = (R)ctl_dt(ctl);
-  Vec4<R> w = Ws[i];
+  Vec4<R> w = Win[i];
   bool fr = m.frozen ? (m.frozen[i] != 0) : false;
-  vertex_finish<R, false>(gamma, dt, __ldg(m.vol + i), fr, w, a, i, Ws, sink, status);
+  vertex_finish<R, MODE == 0>(gamma, dt, __ldg(m.vol + i), fr, w, a, i, Wout, sink, status);
 }
 
 }  // namespace mrd
