@@ -4,6 +4,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -64,7 +65,9 @@ struct mrd_mesh {
   // fused tile path (mrd_tile.cuh): tile plan + one partial per slot
   bool fused = false;
   bool dbg = false;               // dump: tile kernels also write per-triangle residuals to d_phi / d_sT
-  int32_t *d_tile_slot_off = nullptr, *d_vslot_off = nullptr, *d_vslot_ent = nullptr;
+  int2 *d_tile_info = nullptr;    // [ntile+1]: first slot, first geometry record
+  void *d_shape_geom = nullptr;   // R [nshape][12] (geometry-table kernels)
+  int32_t *d_vslot_off = nullptr, *d_vslot_ent = nullptr;
   uint16_t *d_plan = nullptr;     // [ntile][plan_stride]
   void *d_slot_xy = nullptr;      // R [nslot][2]
   void *d_part = nullptr, *d_partS = nullptr;  // Vec4<R> [nslot], R [nslot]
@@ -131,7 +134,9 @@ template <class R> mrd::TileDev<R> tile_dev(const mrd_mesh *m) {
   t.ntile = m->L.ntile;
   t.nslot = m->L.nslot;
   t.nt = m->L.nt;
-  t.tile_slot_off = m->d_tile_slot_off;
+  t.maxshapes = m->L.geom_table ? m->L.maxshapes : 0;
+  t.tile_info = m->d_tile_info;
+  t.shape_geom = (const R *)m->d_shape_geom;
   t.plan = m->d_plan;
   t.slot_xy = (const R *)m->d_slot_xy;
   t.vslot_off = m->d_vslot_off;
@@ -196,9 +201,14 @@ template <class R> int upload_impl(mrd_mesh *m) {
     if ((rc = dev_upload(m, &m->d_csr_off, L.csr_off.data(), nv + 1))) return rc;
     if ((rc = dev_upload(m, &m->d_csr_ent, L.csr_ent.data(), 3 * nt))) return rc;
   } else {
-    if ((rc = dev_upload(m, &m->d_tile_slot_off, L.tile_slot_off.data(), L.ntile + 1))) return rc;
+    {
+      std::vector<int2> info(L.ntile + 1);
+      for (int64_t b = 0; b <= L.ntile; ++b) info[b] = make_int2(L.tile_slot_off[b], L.geom_table ? L.tile_shape_off[b] : 0);
+      if ((rc = dev_upload(m, &m->d_tile_info, info.data(), L.ntile + 1))) return rc;
+    }
+    if (L.geom_table && (rc = dev_upload_real<R>(m, &m->d_shape_geom, L.shape_geom.data(), (int64_t)L.shape_geom.size()))) return rc;
     if ((rc = dev_upload(m, &m->d_plan, L.tile_plan.data(), (int64_t)L.tile_plan.size()))) return rc;
-    if ((rc = dev_upload_real<R>(m, &m->d_slot_xy, L.slot_xy.data(), 2 * L.nslot))) return rc;
+    if (!L.geom_table && (rc = dev_upload_real<R>(m, &m->d_slot_xy, L.slot_xy.data(), 2 * L.nslot))) return rc;
     if ((rc = dev_upload(m, &m->d_vslot_off, L.vslot_off.data(), nv + 1))) return rc;
     if ((rc = dev_upload(m, &m->d_vslot_ent, L.vslot_ent.data(), (int64_t)L.vslot_ent.size()))) return rc;
     V4 *pp = nullptr, *sd = nullptr;
@@ -302,31 +312,39 @@ template <class K, class... Args> void launch_tile(mrd_mesh *m, K kernel, size_t
   int occ = 1;
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, T, sh);
   if (occ < 1) occ = 1;
+  if (const char *cap = std::getenv("MRD_TILE_OCC")) {  // tuning knob: cap the resident blocks per SM of the tile kernels
+    int c = std::atoi(cap);
+    if (c >= 1 && c < occ) occ = c;
+  }
   int64_t grid = std::min<int64_t>(m->L.ntile, (int64_t)m->nsm * occ);
   kernel<<<(unsigned)grid, T, sh, s>>>(args...);
   m->launches++;
 }
 // tile sizes the fused kernels are compiled for
-#define MRD_TILE_DISPATCH(T, CALL) \
-  switch (T) {                     \
+#define MRD_TILE_DISPATCH_G(T, CALL)                      \
+  switch (T) {                                           \
     case 32: { constexpr int TILE = 32; CALL; } break;   \
     case 64: { constexpr int TILE = 64; CALL; } break;   \
     default: { constexpr int TILE = 128; CALL; } break;  \
   }
+#define MRD_TILE_DISPATCH(T, CALL)                                      \
+  if (m->L.geom_table) { constexpr bool GTAB = true; MRD_TILE_DISPATCH_G(T, CALL) } \
+  else { constexpr bool GTAB = false; MRD_TILE_DISPATCH_G(T, CALL) }
 template <class R, int SCHEME> void launch_stage1(mrd_mesh *m, bool store, int a, cudaStream_t s) {
   using V4 = mrd::Vec4<R>;
   const R gamma = (R)m->L.p.gamma;
   if (m->fused) {
     auto td = tile_dev<R>(m);
-    const size_t sh = mrd::TileSmem<R, 1>(td.tile, td.maxslots, td.plan_stride).total;
+    const size_t sh = m->L.geom_table ? mrd::TileSmem<R, 1, true>(td.tile, td.maxslots, td.plan_stride, td.maxshapes).total
+                                      : mrd::TileSmem<R, 1, false>(td.tile, td.maxslots, td.plan_stride, 0).total;
     V4 *dbg = m->dbg ? (V4 *)m->d_phi : nullptr;
     R *dbgs = m->dbg ? (R *)m->d_sT : nullptr;
     if (store) {
-      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, true, TILE>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
+      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, true, TILE, GTAB>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
                                               (const V4 *)m->d_slotZ[a], (const R *)m->d_slotS[a], (const V4 *)m->d_slotD, (R *)m->d_phi16,
                                               (V4 *)m->d_part, (R *)m->d_partS, dbg, dbgs, m->d_flag)))
     } else {
-      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, false, TILE>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
+      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, false, TILE, GTAB>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
                                               (const V4 *)m->d_slotZ[a], (const R *)m->d_slotS[a], (const V4 *)m->d_slotD, (R *)m->d_phi16,
                                               (V4 *)m->d_part, (R *)m->d_partS, dbg, dbgs, m->d_flag)))
     }
@@ -347,8 +365,9 @@ template <class R, int SCHEME> void launch_stage2(mrd_mesh *m, int b, cudaStream
   const R gamma = (R)m->L.p.gamma;
   if (m->fused) {
     auto td = tile_dev<R>(m);
-    const size_t sh = mrd::TileSmem<R, 2>(td.tile, td.maxslots, td.plan_stride).total;
-    MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, false, TILE>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
+    const size_t sh = m->L.geom_table ? mrd::TileSmem<R, 2, true>(td.tile, td.maxslots, td.plan_stride, td.maxshapes).total
+                                      : mrd::TileSmem<R, 2, false>(td.tile, td.maxslots, td.plan_stride, 0).total;
+    MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, false, TILE, GTAB>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
                                             (const V4 *)m->d_slotZ[b], (const R *)nullptr, (const V4 *)m->d_slotD, (R *)m->d_phi16,
                                             (V4 *)m->d_part, (R *)nullptr, (V4 *)nullptr, (R *)nullptr, m->d_flag)))
     return;

@@ -377,6 +377,54 @@ static void build_tile_plan(mrd_layout &L, const std::vector<double> &xyi) {
     const int32_t s0 = L.tile_slot_off[b], ns = L.tile_slot_off[b + 1] - s0;
     for (int j = 0; j < L.offn; ++j) rec[7 * T + j] = (uint16_t)(L.slot_ent_off[s0 + std::min(j, ns)] - e0);
   }
+  // geometry table: distinct (bitwise) geometry records per tile; the record index goes into the 4th entry of tile_tri
+  {
+    std::vector<std::vector<double>> recs(ntile);
+    std::vector<int32_t> nshape_of(ntile + 1, 0);
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t b = 0; b < ntile; ++b) {
+      const int64_t t0 = b * T, t1 = std::min(nt, t0 + T);
+      const int n = (int)(t1 - t0);
+      double g[128][12];
+      int order[128];
+      for (int q = 0; q < n; ++q) {
+        const int64_t t = t0 + q;
+        for (int i = 0; i < 3; ++i) { g[q][i] = L.nx[i][t]; g[q][3 + i] = L.ny[i][t]; g[q][6 + i] = L.hl[i][t]; }
+        g[q][9] = L.area[t] / 3.0;
+        g[q][10] = L.lmax[t];
+        g[q][11] = 0.0;
+        order[q] = q;
+      }
+      std::sort(order, order + n, [&](int a, int c) { return std::memcmp(g[a], g[c], sizeof g[0]) < 0; });
+      std::vector<double> &out = recs[b];
+      int ns = 0;
+      for (int q = 0; q < n; ++q) {
+        if (q == 0 || std::memcmp(g[order[q]], g[order[q - 1]], sizeof g[0]) != 0) {
+          out.insert(out.end(), g[order[q]], g[order[q]] + 12);
+          ++ns;
+        }
+        L.tile_plan[(size_t)b * L.plan_stride + 4 * order[q] + 3] = (uint16_t)(ns - 1);
+      }
+      nshape_of[b + 1] = ns;
+    }
+    L.tile_shape_off.assign(ntile + 1, 0);
+    int32_t maxsh = 0;
+    for (int64_t b = 0; b < ntile; ++b) {
+      L.tile_shape_off[b + 1] = L.tile_shape_off[b] + nshape_of[b + 1];
+      maxsh = std::max(maxsh, nshape_of[b + 1]);
+    }
+    const int64_t nshape = L.tile_shape_off[ntile];
+    // it pays when the table is much smaller than per-triangle geometry: 96 B per record against ~60 fp64
+    // instructions per triangle and stage
+    L.geom_table = nshape * 8 <= nt;
+    L.maxshapes = maxsh;
+    if (L.geom_table) {
+      L.shape_geom.resize((size_t)nshape * 12);
+#pragma omp parallel for schedule(static)
+      for (int64_t b = 0; b < ntile; ++b)
+        std::memcpy(&L.shape_geom[(size_t)L.tile_shape_off[b] * 12], recs[b].data(), sizeof(double) * recs[b].size());
+    }
+  }
 }
 
 }  // namespace mrd_host

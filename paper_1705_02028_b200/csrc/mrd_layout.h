@@ -41,6 +41,12 @@ struct mrd_layout {
   std::vector<int32_t> vslot_off, vslot_ent;  // vertex -> its slots, ascending: [nv+1], [#real slots]
   int32_t maxslots = 0, offn = 0, plan_stride = 0;  // largest (padded) slot count of a tile; plan record sizes
   std::vector<uint16_t> tile_plan;     // [ntile][plan_stride]: tile_tri | slot_ent | tile-local slot offsets
+  // geometry table: per tile the DISTINCT geometry records of its triangles (bitwise; uniform meshes have 2 per tile).
+  // Record = nx[3], ny[3], hl[3], |T|/3, l_max, pad (12 values). Used by the tile kernels when it pays (geom_table).
+  bool geom_table = false;
+  int32_t maxshapes = 0;
+  std::vector<int32_t> tile_shape_off;  // [ntile+1]
+  std::vector<double> shape_geom;       // [nshape][12]
 };
 
 namespace mrd_host {

@@ -20,9 +20,10 @@
 namespace mrd {
 
 template <class R> struct TileDev {
-  int32_t tile, maxslots, offn, plan_stride;
+  int32_t tile, maxslots, offn, plan_stride, maxshapes;
   int64_t ntile, nslot, nt;
-  const int32_t *tile_slot_off;  // [ntile+1] (padded slot counts: multiples of 4)
+  const int2 *tile_info;         // [ntile+1]: .x first slot (padded slot counts: multiples of 4), .y first geometry record
+  const R *shape_geom;           // [nshape][12] geometry records (GTAB kernels), else null
   const uint16_t *plan;          // [ntile][plan_stride]: tile_tri[T][4] | ent[3T] | off[offn]
   const R *slot_xy;              // [nslot][2], relative to the tile's anchor vertex
   const int32_t *vslot_off;      // [nv+1]
@@ -55,6 +56,19 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned by
                "l"(src), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
 }
+// tile_info prefetch: a plain (per-thread register) global load whose result is handed over through an opaque
+// move at the point of use.  Without this the compiler turns the block-uniform value into a uniform register
+// right after the load (R2UR), stalling every warp on the global latency once per tile (10 % of all stall samples).
+__device__ __forceinline__ int2 ld_info(const int2 *p) {
+  int2 v;
+  asm volatile("ld.global.nc.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ int2 use_info(int2 v) {
+  int2 o;
+  asm volatile("mov.b32 %0, %2;\n\tmov.b32 %1, %3;" : "=r"(o.x), "=r"(o.y) : "r"(v.x), "r"(v.y));
+  return o;
+}
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
@@ -80,39 +94,44 @@ __device__ __forceinline__ void tile_geometry(const R x[3], const R y[3], TriGeo
 }
 
 // ---- shared-memory carve-up (dynamic).  Two stage-in buffers + the residual exchange area ----------------
-template <class R, int STAGE> struct TileSmem {
-  size_t oZ, oD, oS, oXY, oPlan, oPhi, buf_bytes;  // per buffer
+template <class R, int STAGE, bool GTAB> struct TileSmem {
+  size_t oZ, oD, oS, oXY, oPlan, oPhi, buf_bytes;  // per buffer (oXY holds the geometry records when GTAB)
   size_t oRes, oST, oBar, total;                   // shared
   __host__ __device__ static size_t up16(size_t x) { return (x + 15) & ~size_t(15); }
-  __host__ __device__ TileSmem(int T, int maxslots, int plan_stride) {
+  __host__ __device__ TileSmem(int T, int maxslots, int plan_stride, int maxshapes) {
     size_t o = 0;
     oZ = o; o += up16(sizeof(Vec4<R>) * maxslots);
     oD = o; if (STAGE == 2) o += up16(sizeof(Vec4<R>) * maxslots);
     oS = o; if (STAGE == 1) o += up16(sizeof(R) * maxslots);
-    oXY = o; o += up16(sizeof(R) * 2 * maxslots);
+    oXY = o; o += GTAB ? up16(sizeof(R) * 12 * maxshapes) : up16(sizeof(R) * 2 * maxslots);
     oPlan = o; o += up16(sizeof(uint16_t) * plan_stride);
     oPhi = o; if (STAGE == 2) o += up16(sizeof(R) * 16 * T);
     buf_bytes = (o + 31) & ~size_t(31);
     size_t s = 2 * buf_bytes;
-    oRes = s; s += sizeof(R) * 12 * T;
-    oST = s; s += up16(sizeof(R) * T);
+    // stage 2: the residual exchange area aliases the current buffer's phi16 block -- thread `tid` only overwrites the
+    // 12 entries [c][tid] it has consumed itself, so no other thread's data is touched (saves 12 KB: 4 blocks per SM)
+    oRes = s; if (STAGE == 1) s += sizeof(R) * 12 * T;
+    oST = s; if (STAGE == 1) s += up16(sizeof(R) * T);
     oBar = s; s += 16;
     total = s;
   }
 };
 
 // bring tile b into buffer `buf` (one thread): expect_tx, then the bulk copies
-template <class R, int STAGE>
-__device__ __forceinline__ void tile_stage_in(const TileDev<R> &td, const TileSmem<R, STAGE> &L, unsigned char *buf,
-                                              uint64_t *bar, int64_t b, int s0, int ns, const Vec4<R> *slotZ,
+template <class R, int STAGE, bool GTAB>
+__device__ __forceinline__ void tile_stage_in(const TileDev<R> &td, const TileSmem<R, STAGE, GTAB> &L, unsigned char *buf,
+                                              uint64_t *bar, int64_t b, int2 i0, int2 i1, const Vec4<R> *slotZ,
                                               const R *slotS, const Vec4<R> *slotD, const R *phi16) {
   const int T = td.tile;
-  const unsigned bZ = sizeof(Vec4<R>) * ns, bS = sizeof(R) * ns, bXY = sizeof(R) * 2 * ns;
+  const int s0 = i0.x, ns = i1.x - i0.x;
+  const unsigned bZ = sizeof(Vec4<R>) * ns, bS = sizeof(R) * ns;
+  const unsigned bXY = GTAB ? sizeof(R) * 12 * (i1.y - i0.y) : sizeof(R) * 2 * ns;
   const unsigned bPlan = sizeof(uint16_t) * td.plan_stride, bPhi = sizeof(R) * 16 * T;
   unsigned total = bZ + bXY + bPlan + (STAGE == 1 ? bS : bZ + bPhi);
   mbar_expect_tx(bar, total);
   bulk_g2s(buf + L.oZ, slotZ + s0, bZ, bar);
-  bulk_g2s(buf + L.oXY, td.slot_xy + 2 * (int64_t)s0, bXY, bar);
+  if (GTAB) bulk_g2s(buf + L.oXY, td.shape_geom + 12 * (int64_t)i0.y, bXY, bar);
+  else bulk_g2s(buf + L.oXY, td.slot_xy + 2 * (int64_t)s0, bXY, bar);
   bulk_g2s(buf + L.oPlan, td.plan + b * td.plan_stride, bPlan, bar);
   if (STAGE == 1) {
     bulk_g2s(buf + L.oS, slotS + s0, bS, bar);
@@ -150,7 +169,7 @@ __device__ __forceinline__ void tile_epilogue(int T, const R *res, const R *sT, 
 #ifndef MRD_TILE_MINB
 #define MRD_TILE_MINB 4
 #endif
-template <class R, int SCHEME, int STAGE, bool STORE, int TILE>
+template <class R, int SCHEME, int STAGE, bool STORE, int TILE, bool GTAB>
 __global__ void __launch_bounds__(TILE, (MRD_TILE_MINB * 128) / TILE)
 tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ slotZ,
             const R *__restrict__ slotS, const Vec4<R> *__restrict__ slotD, R *__restrict__ phi16,
@@ -160,8 +179,8 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int T = TILE;  // compile-time tile size: shared-memory and phi16 strides become immediates
   const int tid = threadIdx.x;
-  const TileSmem<R, STAGE> L(T, td.maxslots, td.plan_stride);
-  R *res = reinterpret_cast<R *>(smem_raw + L.oRes);
+  const TileSmem<R, STAGE, GTAB> L(T, td.maxslots, td.plan_stride, td.maxshapes);
+  R *res1 = reinterpret_cast<R *>(smem_raw + L.oRes);
   R *sST = reinterpret_cast<R *>(smem_raw + L.oST);
   uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + L.oBar);
   if (tid == 0) {
@@ -171,35 +190,37 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
   }
   __syncthreads();
   int64_t b = blockIdx.x;
-  // slot range of the tile in flight; the next tile's range is fetched one iteration ahead
-  int s0 = __ldg(td.tile_slot_off + b), ns = __ldg(td.tile_slot_off + b + 1) - s0;
-  if (tid == 0) tile_stage_in<R, STAGE>(td, L, smem_raw, &bar[0], b, s0, ns, slotZ, slotS, slotD, phi16);
-  int s0n = 0, s1n = 0;  // slot range of the next tile: loaded one iteration before it is needed
+  // slot / geometry-record range of the tile in flight (i0, i1); the next tile's range is fetched one iteration ahead
+  int2 i0 = __ldg(td.tile_info + b), i1 = __ldg(td.tile_info + b + 1);
+  if (tid == 0) tile_stage_in<R, STAGE, GTAB>(td, L, smem_raw, &bar[0], b, i0, i1, slotZ, slotS, slotD, phi16);
+  int2 n0 = make_int2(0, 0), n1 = make_int2(0, 0);
   if (b + gridDim.x < td.ntile) {
-    s0n = __ldg(td.tile_slot_off + b + gridDim.x);
-    s1n = __ldg(td.tile_slot_off + b + gridDim.x + 1);
+    n0 = ld_info(td.tile_info + b + gridDim.x);
+    n1 = ld_info(td.tile_info + b + gridDim.x + 1);
   }
   bool bad = false;  // linearised c^2 <= 0 met by this thread (raised once, after the loop)
   for (int k = 0; b < td.ntile; b += gridDim.x, ++k) {
     const int cur = k & 1;
     unsigned char *buf = smem_raw + cur * L.buf_bytes;
     const int64_t nb = b + gridDim.x;
-    const int s0x = s0n, nsx = s1n - s0n;
+    const int2 x0 = use_info(n0), x1 = use_info(n1);
     if (nb < td.ntile) {
       if (nb + gridDim.x < td.ntile) {  // in flight during this iteration, consumed at the top of the next one
-        s0n = __ldg(td.tile_slot_off + nb + gridDim.x);
-        s1n = __ldg(td.tile_slot_off + nb + gridDim.x + 1);
+        n0 = ld_info(td.tile_info + nb + gridDim.x);
+        n1 = ld_info(td.tile_info + nb + gridDim.x + 1);
       }
       if (tid == 0) {
         fence_proxy_async();  // buffer cur^1 was read through the generic proxy in iteration k-1
-        tile_stage_in<R, STAGE>(td, L, smem_raw + (cur ^ 1) * L.buf_bytes, &bar[cur ^ 1], nb, s0x, nsx, slotZ, slotS, slotD,
-                                phi16);
+        tile_stage_in<R, STAGE, GTAB>(td, L, smem_raw + (cur ^ 1) * L.buf_bytes, &bar[cur ^ 1], nb, x0, x1, slotZ, slotS, slotD,
+                                      phi16);
       }
     }
+    const int s0 = i0.x, ns = i1.x - i0.x;
     mbar_wait(&bar[cur], (k >> 1) & 1);
     const Vec4<R> *sZ = reinterpret_cast<const Vec4<R> *>(buf + L.oZ);
     const R *sXY = reinterpret_cast<const R *>(buf + L.oXY);
     const uint16_t *plan = reinterpret_cast<const uint16_t *>(buf + L.oPlan);
+    R *res = STAGE == 1 ? res1 : reinterpret_cast<R *>(buf + L.oPhi);
     const int64_t t = b * T + tid;
     R pN[3][4];
     R st = R(0);
@@ -207,10 +228,18 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
       const ushort4 lv = reinterpret_cast<const ushort4 *>(plan)[tid];
       const int l[3] = {lv.x, lv.y, lv.z};
       Vec4<R> z[3] = {sZ[l[0]], sZ[l[1]], sZ[l[2]]};
-      R x[3] = {sXY[2 * l[0]], sXY[2 * l[1]], sXY[2 * l[2]]}, y[3] = {sXY[2 * l[0] + 1], sXY[2 * l[1] + 1], sXY[2 * l[2] + 1]};
       TriGeom<R> g;
       R a3, lmax;
-      tile_geometry(x, y, g, a3, lmax);
+      if (GTAB) {  // geometry record of this triangle's shape (layout stage; bitwise the oracle's geometry)
+        const R *G = sXY + 12 * lv.w;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { g.nx[i] = G[i]; g.ny[i] = G[3 + i]; g.hl[i] = G[6 + i]; }
+        a3 = G[9];
+        lmax = G[10];
+      } else {
+        R x[3] = {sXY[2 * l[0]], sXY[2 * l[1]], sXY[2 * l[2]]}, y[3] = {sXY[2 * l[0] + 1], sXY[2 * l[1] + 1], sXY[2 * l[2] + 1]};
+        tile_geometry(x, y, g, a3, lmax);
+      }
       TriCore<R> kk;
       R pT[4];
       triangle_core(gamma, z, g, kk, pT, pN);  // stage 2: all matrices re-evaluated at W* (reading C12)
@@ -276,8 +305,8 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
     __syncthreads();
     tile_epilogue<R, STAGE == 1>(T, res, sST, plan + 4 * T, plan + 7 * T, s0, ns, part, partS);
     __syncthreads();  // res and buffer `cur` are free again
-    s0 = s0x;
-    ns = nsx;
+    i0 = x0;
+    i1 = x1;
   }
   if (bad) atomicOr(status, 1);
 }
