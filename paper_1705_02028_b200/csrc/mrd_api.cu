@@ -410,7 +410,7 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
   if (m->fused) {
     // fused path: dt from the partial s_T sums alone; the update kernels gather the residual partials themselves
     auto td = tile_dev<R>(m);
-    mrd::slot_dt_kernel<R><<<vb, 256, 0, s>>>(md, td, m->d_ctl, (const R *)m->d_partS);
+    mrd::slot_dt_kernel<R><<<std::min<unsigned>(vb, (unsigned)m->nsm * 8), 256, 0, s>>>(md, td, m->d_ctl, (const R *)m->d_partS);
     m->launches++;
     PROF_MARK(MRD_PROF_GATHER_DT)
     if (m->nwv > 0) {

@@ -274,33 +274,54 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
           }
         }
       }
-      if (SCHEME != MRD_SCHEME_N) {
-        R pL[3][4];
-        apply_beta(gamma, kk, g, X, pL);  // eq. 50-51; stage 2: eq. 63 with eq. 65
-        if (SCHEME == MRD_SCHEME_B) {
-          blend(X, pN, pL);
+      // The nodal N residuals go to shared memory now (their final place for scheme N); the LDA residuals are then
+      // produced node by node and blended in place -- 24 fewer values live at once than blending from registers.
+      R th[4];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        if (SCHEME == MRD_SCHEME_B) {  // eq. 53 (+ C10): Theta = min(1, |X| / sum_i |N_i|), 0 on a zero denominator
+          R den = Fast<R>::abs(pN[0][c]) + Fast<R>::abs(pN[1][c]) + Fast<R>::abs(pN[2][c]);
+          bool pos = den > R(0);
+          R t = Fast<R>::min(R(1), Fast<R>::abs(X[c]) * Fast<R>::rcp(pos ? den : R(1)));
+          th[c] = pos ? t : R(0);
         } else {
+          th[c] = R(0);
+        }
 #pragma unroll
-          for (int i = 0; i < 3; ++i)
+        for (int i = 0; i < 3; ++i) res[(i * 4 + c) * T + tid] = pN[i][c];
+      }
+      if (SCHEME != MRD_SCHEME_N) {
+        // eq. 50-51 (stage 2: eq. 63 with eq. 65): L_i = -K_i^+ N-hat X;  eq. 52: B_i = L_i + Theta (N_i - L_i)
+        R q[4], y[4];
+        to_symmetrising(gamma - R(1), kk, X, q);
+        y[0] = -(kk.n00 * q[0] + kk.n01 * q[1] + kk.n02 * q[2]);
+        y[1] = -(kk.n01 * q[0] + kk.n11 * q[1] + kk.n12 * q[2]);
+        y[2] = -(kk.n02 * q[0] + kk.n12 * q[1] + kk.n22 * q[2]);
+        y[3] = -(kk.ns * q[3]);
 #pragma unroll
-            for (int c = 0; c < 4; ++c) pN[i][c] = pL[i][c];
+        for (int i = 0; i < 3; ++i) {
+          R z[4], Lw[4];
+          apply_split<false>(kk.ap[i], kk.bp[i], kk.l3p[i], g.nx[i], g.ny[i], y, z);
+          to_conserved(kk, z, Lw);
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            R *r = res + (i * 4 + c) * T + tid;
+            *r = SCHEME == MRD_SCHEME_B ? Lw[c] + th[c] * (*r - Lw[c]) : Lw[c];
+          }
         }
       }
       if (STAGE == 1 && phi_dbg) {
 #pragma unroll
-        for (int i = 0; i < 3; ++i) st4(&phi_dbg[3 * t + i], Vec4<R>{pN[i][0], pN[i][1], pN[i][2], pN[i][3]});
+        for (int i = 0; i < 3; ++i) {
+          const R *r = res + (i * 4) * T + tid;
+          st4(&phi_dbg[3 * t + i], Vec4<R>{r[0], r[T], r[2 * T], r[3 * T]});
+        }
         sT_dbg[t] = st;
       }
     } else {  // padding thread of the last tile: contributes nothing
 #pragma unroll
-      for (int i = 0; i < 3; ++i)
-#pragma unroll
-        for (int c = 0; c < 4; ++c) pN[i][c] = R(0);
+      for (int i = 0; i < 12; ++i) res[i * T + tid] = R(0);
     }
-#pragma unroll
-    for (int i = 0; i < 3; ++i)
-#pragma unroll
-      for (int c = 0; c < 4; ++c) res[(i * 4 + c) * T + tid] = pN[i][c];
     if (STAGE == 1) sST[tid] = st;
     __syncthreads();
     tile_epilogue<R, STAGE == 1>(T, res, sST, plan + 4 * T, plan + 7 * T, s0, ns, part, partS);
@@ -319,13 +340,14 @@ template <class R>
 __global__ void __launch_bounds__(256)
 slot_dt_kernel(MeshDev<R> m, TileDev<R> td, Ctl *__restrict__ ctl, const R *__restrict__ partS) {
   MRD_CTL_GUARD(ctl)
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  // grid-stride: a few blocks per SM, so that only ~10^3 atomicMin hit the one address (65 536 one-per-block atomics
+  // serialise in L2 and took longer than the gather itself)
   double d = __longlong_as_double(0x7FF0000000000000ll);
-  if (i < m.nv) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m.nv; i += (int64_t)gridDim.x * blockDim.x) {
     R S = 0;
     const int32_t q0 = __ldg(td.vslot_off + i), q1 = __ldg(td.vslot_off + i + 1);
     for (int32_t q = q0; q < q1; ++q) S += __ldg(partS + __ldg(td.vslot_ent + q));
-    d = 2.0 * (double)__ldg(m.vol + i) / (double)S;
+    d = fmin(d, 2.0 * (double)__ldg(m.vol + i) / (double)S);
   }
   block_min_to_global(d, &ctl->dmin_bits);
 }
