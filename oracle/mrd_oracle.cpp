@@ -304,6 +304,8 @@ template <class R> void apply_beta(const Core<R> &o, const R x[4], R out[3][4]) 
 }
 
 // eq. 52-53 (+ reading C10): Theta_kk = min(1, |phi_k| / sum_j |phi^N_{j,k}|), 0 when the denominator is 0
+// Bmax / Bmin (L503): "setting all diagonal values of Theta to theta, [where] theta can be taken to be either the
+// maximum (Bmax) or the minimum (Bmin) over all Theta_kk".
 template <class R>
 void blend(int scheme, const R phiT[4], const R phiN[3][4], const R phiLDA[3][4], R theta[4], R phiB[3][4]) {
   for (int k = 0; k < 4; ++k) {
@@ -313,8 +315,14 @@ void blend(int scheme, const R phiT[4], const R phiN[3][4], const R phiLDA[3][4]
     if (scheme == ORC_SCHEME_N) th = R(1.0);
     if (scheme == ORC_SCHEME_LDA) th = R(0.0);
     theta[k] = th;
-    for (int i = 0; i < 3; ++i) phiB[i][k] = th * phiN[i][k] + (R(1.0) - th) * phiLDA[i][k];
   }
+  if (scheme == ORC_SCHEME_BMAX || scheme == ORC_SCHEME_BMIN) {
+    R t = theta[0];
+    for (int k = 1; k < 4; ++k) t = scheme == ORC_SCHEME_BMAX ? Max(t, theta[k]) : Min(t, theta[k]);
+    for (int k = 0; k < 4; ++k) theta[k] = t;
+  }
+  for (int k = 0; k < 4; ++k)
+    for (int i = 0; i < 3; ++i) phiB[i][k] = theta[k] * phiN[i][k] + (R(1.0) - theta[k]) * phiLDA[i][k];
 }
 
 template <class R> struct Stage1Out {
@@ -450,7 +458,7 @@ int orc_mesh_create(orc_mesh **out, double gamma, double cfl, int scheme, int ti
                     const uint8_t *vertex_flag, int64_t ne, const int32_t *wall_edge) {
   if (!out || !xy || !tri || nv < 3 || nt < 1) return fail(ORC_EINVAL, "null or empty mesh");
   if (!(gamma > 1.0) || !(cfl > 0.0)) return fail(ORC_EINVAL, "gamma must be > 1 and cfl > 0");
-  if (scheme < 0 || scheme > 2 || (time_order != 1 && time_order != 2)) return fail(ORC_EINVAL, "bad scheme/time_order");
+  if (scheme < 0 || scheme > 4 || (time_order != 1 && time_order != 2)) return fail(ORC_EINVAL, "bad scheme/time_order");
   if (ne < 0 || (ne > 0 && !wall_edge)) return fail(ORC_EINVAL, "bad wall edge list");
   orc_mesh *m = new (std::nothrow) orc_mesh();
   if (!m) return fail(ORC_ENOMEM, "out of memory");
