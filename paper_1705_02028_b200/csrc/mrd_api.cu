@@ -278,6 +278,7 @@ template <class R> int set_state_impl(mrd_mesh *m, const R *W_dev, cudaStream_t 
   mrd::Ctl c{};
   c.t = 0.0; c.dt = 0.0; c.t_end = 0.0; c.cfl = m->L.p.cfl;
   c.dmin_bits = 0x7FF0000000000000ull; c.steps = 0; c.status = 0; c.active = 0;
+  c.bvar = m->L.p.scheme == MRD_SCHEME_BMAX ? 1 : (m->L.p.scheme == MRD_SCHEME_BMIN ? 2 : 0);
   CUDA_TRY(cudaMemcpyAsync(m->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s));
   CUDA_TRY(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
   mrd::set_state_kernel<R><<<blocks_for(nv, 256), 256, 0, s>>>(nv, m->d_vperm, W_dev, (R)m->L.p.gamma, (V4 *)m->d_W[0],

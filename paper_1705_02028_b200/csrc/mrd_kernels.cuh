@@ -17,6 +17,8 @@ struct Ctl {
   long long steps;               // completed steps since set_state
   int status;                    // 0, or MRD_ENONPHYSICAL (as positive flag 1)
   int active;                    // 1 while the step in flight has to be done
+  int bvar;                      // blend variant of scheme B (L503): 0 = diagonal Theta, 1 = Bmax, 2 = Bmin
+  int pad;
 };
 
 template <class R> struct MeshDev {
@@ -155,7 +157,7 @@ tri_stage1_kernel(MeshDev<R> m, R gamma, const Ctl *__restrict__ ctl, const Vec4
     R pL[3][4];
     apply_beta(gamma, k, g, pT, pL);
     if (SCHEME == MRD_SCHEME_B) {
-      blend(pT, pN, pL);
+      blend(pT, pN, pL, ctl->bvar);
     } else {
 #pragma unroll
       for (int i = 0; i < 3; ++i)
@@ -206,7 +208,7 @@ tri_stage2_kernel(MeshDev<R> m, R gamma, const Ctl *__restrict__ ctl, const Vec4
     R pL[3][4];
     apply_beta(gamma, k, g, PT, pL);  // eq. 63 with eq. 65: Phi_i^LDA = beta_i(W*) Phi^T
     if (SCHEME == MRD_SCHEME_B) {
-      blend(PT, pN, pL);
+      blend(PT, pN, pL, ctl->bvar);
     } else {
 #pragma unroll
       for (int i = 0; i < 3; ++i)

@@ -76,7 +76,7 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
   if (!p || !xy || !tri || nv < 3 || nt < 1) { err = "null or empty mesh"; return MRD_EINVAL; }
   if (nv > 0x7FFFFFF0ll || 3 * nt > 0x7FFFFFF0ll) { err = "mesh too large for 32-bit indices"; return MRD_EINVAL; }
   if (!(p->gamma > 1.0) || !(p->cfl > 0.0)) { err = "gamma must be > 1 and cfl > 0"; return MRD_EINVAL; }
-  if (p->scheme < 0 || p->scheme > 2 || (p->time_order != 1 && p->time_order != 2)) { err = "bad scheme/time_order"; return MRD_EINVAL; }
+  if (p->scheme < 0 || p->scheme > 4 || (p->time_order != 1 && p->time_order != 2)) { err = "bad scheme/time_order"; return MRD_EINVAL; }
   if (p->precision != MRD_FP64 && p->precision != MRD_FP32) { err = "bad precision"; return MRD_EINVAL; }
   if (p->period_x < 0.0 || p->period_y < 0.0) { err = "negative period"; return MRD_EINVAL; }
   if (ne < 0 || (ne > 0 && !wall_edge)) { err = "bad wall edge list"; return MRD_EINVAL; }

@@ -395,17 +395,31 @@ __device__ __forceinline__ void apply_beta(R gamma, const TriCore<R> &k, const T
 
 // eq. 52-53 (+ reading C10): Theta_kk = min(1, |X_k| / sum_j |N_j,k|), 0 when the denominator is 0;
 // B_i = Theta N_i + (1 - Theta) LDA_i, written over N.
-template <class R> __device__ __forceinline__ void blend(const R X[4], R N[3][4], const R L[3][4]) {
+// Theta_kk of eq. 53 for all four components; bvar 1 / 2: all entries replaced by their maximum / minimum (Bmax / Bmin,
+// L503)
+template <class R> __device__ __forceinline__ void blend_theta(const R X[4], const R N[3][4], int bvar, R th[4]) {
   using F = Fast<R>;
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     R den = F::abs(N[0][c]) + F::abs(N[1][c]) + F::abs(N[2][c]);
     bool pos = den > R(0);
-    R th = F::min(R(1), F::abs(X[c]) * F::rcp(pos ? den : R(1)));
-    th = pos ? th : R(0);
-#pragma unroll
-    for (int i = 0; i < 3; ++i) N[i][c] = L[i][c] + th * (N[i][c] - L[i][c]);
+    R t = F::min(R(1), F::abs(X[c]) * F::rcp(pos ? den : R(1)));
+    th[c] = pos ? t : R(0);
   }
+  if (bvar != 0) {
+    R hi = F::max(F::max(th[0], th[1]), F::max(th[2], th[3]));
+    R lo = F::min(F::min(th[0], th[1]), F::min(th[2], th[3]));
+    R t = bvar == 1 ? hi : lo;
+    th[0] = th[1] = th[2] = th[3] = t;
+  }
+}
+template <class R> __device__ __forceinline__ void blend(const R X[4], R N[3][4], const R L[3][4], int bvar) {
+  R th[4];
+  blend_theta(X, N, bvar, th);
+#pragma unroll
+  for (int c = 0; c < 4; ++c)
+#pragma unroll
+    for (int i = 0; i < 3; ++i) N[i][c] = L[i][c] + th[c] * (N[i][c] - L[i][c]);
 }
 
 }  // namespace mrd

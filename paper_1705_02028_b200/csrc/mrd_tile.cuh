@@ -198,6 +198,7 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
     n0 = ld_info(td.tile_info + b + gridDim.x);
     n1 = ld_info(td.tile_info + b + gridDim.x + 1);
   }
+  const int bvar = ctl->bvar;
   bool bad = false;  // linearised c^2 <= 0 met by this thread (raised once, after the loop)
   for (int k = 0; b < td.ntile; b += gridDim.x, ++k) {
     const int cur = k & 1;
@@ -276,20 +277,12 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
       }
       // The nodal N residuals go to shared memory now (their final place for scheme N); the LDA residuals are then
       // produced node by node and blended in place -- 24 fewer values live at once than blending from registers.
-      R th[4];
+      R th[4] = {0, 0, 0, 0};
+      if (SCHEME == MRD_SCHEME_B) blend_theta(X, pN, bvar, th);  // eq. 53 (+ C10); Bmax / Bmin: L503
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        if (SCHEME == MRD_SCHEME_B) {  // eq. 53 (+ C10): Theta = min(1, |X| / sum_i |N_i|), 0 on a zero denominator
-          R den = Fast<R>::abs(pN[0][c]) + Fast<R>::abs(pN[1][c]) + Fast<R>::abs(pN[2][c]);
-          bool pos = den > R(0);
-          R t = Fast<R>::min(R(1), Fast<R>::abs(X[c]) * Fast<R>::rcp(pos ? den : R(1)));
-          th[c] = pos ? t : R(0);
-        } else {
-          th[c] = R(0);
-        }
+      for (int c = 0; c < 4; ++c)
 #pragma unroll
         for (int i = 0; i < 3; ++i) res[(i * 4 + c) * T + tid] = pN[i][c];
-      }
       if (SCHEME != MRD_SCHEME_N) {
         // eq. 50-51 (stage 2: eq. 63 with eq. 65): L_i = -K_i^+ N-hat X;  eq. 52: B_i = L_i + Theta (N_i - L_i)
         R q[4], y[4];

@@ -259,3 +259,24 @@ def test_nonphysical_state_is_reported_and_state_kept(mrd):
         Wg = gm.get_state().cpu().numpy()
         assert np.isfinite(Wg).all() and (Wg[0] > 0).all()
         assert field_errors(Wg, om.get_state()) <= 1e-6
+
+
+@pytest.mark.parametrize("scheme", [3, 4])          # Bmax, Bmin
+@pytest.mark.parametrize("tile", [-1, 0])
+def test_bmax_bmin_variants_match_oracle(mrd, scheme, tile):
+    mesh = wl.jitter_mesh(wl.uniform_mesh(31, 26, 1.0, 1.0, periodic=True), 0.2, seed=21)
+    W = wl.random_smooth_state(mesh, mach=1.1, seed=6)
+    gm = gpu_mesh(mrd, mesh, W, scheme=scheme, tile=tile)
+    om = orc_mesh(mesh, W, scheme=scheme)
+    g, o = gm.dump_stage1(), om.dump_stage1()
+    assert np.abs(g["phiB"] - o["phiB"]).max() <= 2e-13 * np.abs(o["phiN"]).max()
+    gm.step(1)
+    om.step(1)
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_1
+    gm.step(49)
+    om.step(49)
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_100
+    # the variant is not the diagonal blend
+    gb = gpu_mesh(mrd, mesh, W, scheme=2, tile=tile)
+    gb.step(50)
+    assert field_errors(gb.get_state().cpu().numpy(), om.get_state()) > 1e-6
