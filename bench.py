@@ -32,9 +32,9 @@ UNIT = "triangle-updates/s"
 # FLOPs per triangle per stage = min(oracle operation count, FLOPs the kernel executes).  The kernel's count
 # (2*DFMA + DADD + DMUL per thread, from ncu's smsp__sass_thread_inst_executed_op_d*_pred_on of the profiled
 # launch, profiles/) is the smaller one; the oracle's own count (orc_count_ops) is kept for context.
-FLOPS_TRI_STAGE1 = {"fp64": 736.0, "fp32": 690.0}
-FLOPS_TRI_STAGE2 = {"fp64": 817.0, "fp32": 770.0}
-FLOPS_VERTEX_STAGE = 60.0              # per vertex per stage: gather adds, update, Z and signal speed
+FLOPS_TRI_STAGE1 = {"fp64": 677.0, "fp32": 640.0}
+FLOPS_TRI_STAGE2 = {"fp64": 751.0, "fp32": 710.0}
+FLOPS_VERTEX_STAGE = 144.0             # per triangle-update, all three vertex kernels together (ncu: 8.6 + 71.5 + 63.5)
 ORACLE_FLOPS_TRI = (2098.0, 2194.0)    # oracle.count_ops(stage 1 / stage 2): add+mul+div+sqrt
 # compulsory HBM bytes per triangle of one triangle-kernel launch (share of SURVEY 8d's 130 B per triangle-update):
 # state read once (32 B per vertex / 2), connectivity 12 B, coordinates 8 B; stage 2 also reads W^n (dW/dt)
@@ -42,9 +42,9 @@ BYTES_TRI_STAGE1 = {"fp64": 36.0, "fp32": 24.0}
 BYTES_TRI_STAGE2 = {"fp64": 52.0, "fp32": 32.0}
 # bytes the fused kernels move BY DESIGN (slot copies, plan record, stored phi^N/phi^T, partials), for comparison
 # with ncu's dram__bytes (the roofline object's `traffic`)
-DESIGN_BYTES_TRI = {"tri_stage1": {"fp64": 204.0, "fp32": 110.0}, "tri_stage2": {"fp64": 214.0, "fp32": 115.0}}
+DESIGN_BYTES_TRI = {"tri_stage1": {"fp64": 196.0, "fp32": 106.0}, "tri_stage2": {"fp64": 207.0, "fp32": 112.0}}
 # ncu dram__bytes_read.sum + dram__bytes_write.sum per triangle of the profiled launches (profiles/*.md)
-NCU_TRAFFIC_BYTES_TRI = {"tri_stage1": {"fp64": 204.8}, "tri_stage2": {"fp64": 216.9}}
+NCU_TRAFFIC_BYTES_TRI = {"tri_stage1": {"fp64": 195.8}, "tri_stage2": {"fp64": 207.8}}
 B_ALG_STEP = {"fp64": 130.0, "fp32": 76.0}
 
 
