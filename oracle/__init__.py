@@ -28,6 +28,9 @@ def lib():
         L.orc_mesh_destroy.argtypes = [C.c_void_p]
         L.orc_mesh_destroy.restype = None
         L.orc_set_num_threads.argtypes = [C.c_void_p, C.c_int]
+        L.orc_set_lumping.argtypes = [C.c_void_p, C.c_int]
+        L.orc_triangle_stage2_lumping.argtypes = [C.c_int]
+        L.orc_triangle_stage2_lumping.restype = None
         L.orc_set_state.argtypes = [C.c_void_p, dp]
         L.orc_get_state.argtypes = [C.c_void_p, dp]
         L.orc_step.argtypes = [C.c_void_p, C.c_int64, C.c_double, C.POINTER(C.c_int64), dp, dp]
@@ -76,7 +79,7 @@ class OracleMesh:
     """The oracle's mesh + stepper."""
 
     def __init__(self, xy, tri, gamma=1.4, cfl=0.5, scheme=SCHEME_B, time_order=2, period=(0.0, 0.0),
-                 vertex_flag=None, wall_edge=None, threads=1):
+                 vertex_flag=None, wall_edge=None, threads=1, lumping=0):
         L = lib()
         self._xy = _f64(xy)
         self._tri = np.ascontiguousarray(tri, dtype=np.int32)
@@ -93,6 +96,8 @@ class OracleMesh:
         self.gamma = gamma
         if threads != 1:
             self.set_threads(threads)
+        if lumping:
+            _check(L.orc_set_lumping(self._h, int(lumping)))
 
     def __del__(self):
         h, self._h = getattr(self, "_h", None), None
@@ -164,7 +169,8 @@ def triangle_stage1(gamma, W, xy):
     return o
 
 
-def triangle_stage2(gamma, Wn, Ws, xy, dt, phiT_n, phiN_n):
+def triangle_stage2(gamma, Wn, Ws, xy, dt, phiT_n, phiN_n, lumping=0):
+    lib().orc_triangle_stage2_lumping(int(lumping))
     Wn, Ws, xy = _f64(Wn, (3, 4)), _f64(Ws, (3, 4)), _f64(xy, (3, 2))
     pT, pN = _f64(phiT_n, (4,)), _f64(phiN_n, (3, 4))
     o = dict(PhiT=np.empty(4), PhiN=np.empty((3, 4)), PhiLDA=np.empty((3, 4)), PhiB=np.empty((3, 4)))

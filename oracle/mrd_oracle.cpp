@@ -348,9 +348,13 @@ template <class R> struct Stage2Out {
 };
 
 // O9: total residuals of the second Runge-Kutta stage (eq. 57, 61-65; reading C12)
+// `lumping` = 1: selective lumping (eq. 66-67): the anti-diffusive term
+//   sum_j (|T| delta_ij / 3 - m^G_ij) dW_j/dt,  m^G_ij = |T|/12 (delta_ij + 1)  (Galerkin mass matrix)
+// is added to BOTH Phi_i^N and Phi_i^LDA ("Phi_i can be either Phi_i^LDA or Phi_i^N", L567) before they are "mixed in
+// the usual way" (L572); it sums to zero over the nodes, so Phi^T and conservation are unchanged.
 template <class R>
 int triangle_stage2(R gamma, int scheme, const R Wn[3][4], const R Ws[3][4], const Geom<R> &g, R dt,
-                    const R phiT_n[4], const R phiN_n[3][4], Core<R> &core, Stage2Out<R> &o) {
+                    const R phiT_n[4], const R phiN_n[3][4], Core<R> &core, Stage2Out<R> &o, int lumping = 0) {
   int rc = triangle_core(gamma, Ws, g, core);  // all matrices re-evaluated at W*
   if (rc) return rc;
   R third = g.area / R(3.0);
@@ -364,6 +368,19 @@ int triangle_stage2(R gamma, int scheme, const R Wn[3][4], const R Ws[3][4], con
       o.PhiN[i][k] = third * dW[i][k] + R(0.5) * (core.phiN[i][k] + phiN_n[i][k]);
   }
   apply_beta(core, o.PhiT, o.PhiLDA);  // eq. 63 with eq. 65: Phi_i^LDA = beta_i(W*) Phi^T
+  if (lumping == 1) {
+    for (int i = 0; i < 3; ++i)
+      for (int k = 0; k < 4; ++k) {
+        R extra = R(0.0);
+        for (int j = 0; j < 3; ++j) {
+          R lumped = (i == j) ? g.area / R(3.0) : R(0.0);                       // |T| delta_ij / 3
+          R galerkin = g.area / R(12.0) * ((i == j) ? R(2.0) : R(1.0));         // eq. 67
+          extra = extra + (lumped - galerkin) * dW[j][k];                       // eq. 66
+        }
+        o.PhiN[i][k] = o.PhiN[i][k] + extra;
+        o.PhiLDA[i][k] = o.PhiLDA[i][k] + extra;
+      }
+  }
   blend(scheme, o.PhiT, o.PhiN, o.PhiLDA, o.theta, o.PhiB);
   return ORC_OK;
 }
@@ -403,6 +420,7 @@ bool wall_edge(R gamma, const R Wa[4], const R Wb[4], R nx, R ny, R len, R Pa[4]
 struct orc_mesh {
   double gamma, cfl;
   int scheme, time_order;
+  int lumping = 0;  // 0 = global lumping (all tests of the paper, L576); 1 = selective lumping (eq. 66-67)
   double period[2];
   int64_t nv, nt, ne;
   std::vector<double> xy;            // [nv][2]
@@ -545,6 +563,12 @@ int orc_mesh_create(orc_mesh **out, double gamma, double cfl, int scheme, int ti
 
 void orc_mesh_destroy(orc_mesh *m) { delete m; }
 
+int orc_set_lumping(orc_mesh *m, int lumping) {
+  if (!m || (lumping != 0 && lumping != 1)) return fail(ORC_EINVAL, "lumping must be 0 (global) or 1 (selective)");
+  m->lumping = lumping;
+  return ORC_OK;
+}
+
 int orc_set_num_threads(orc_mesh *m, int n) {
   if (!m || n < 1) return fail(ORC_EINVAL, "bad thread count");
   m->nthreads = n;
@@ -628,7 +652,7 @@ int stage2_triangles(orc_mesh *m, double dt) {
     for (int k = 0; k < 4; ++k) pT[k] = m->phiT_n[4 * t + k];
     Core<double> core;
     Stage2Out<double> o;
-    if (triangle_stage2(m->gamma, m->scheme, wn, ws, m->geo[t], dt, pT, pN, core, o)) { bad |= 1; continue; }
+    if (triangle_stage2(m->gamma, m->scheme, wn, ws, m->geo[t], dt, pT, pN, core, o, m->lumping)) { bad |= 1; continue; }
     for (int i = 0; i < 3; ++i)
       for (int k = 0; k < 4; ++k) m->phi[12 * t + 4 * i + k] = o.PhiB[i][k];
   }
@@ -801,6 +825,9 @@ int orc_triangle_stage1(double gamma, const double *W, const double *xy, double 
   return ORC_OK;
 }
 
+static thread_local int g_stage2_lumping = 0;
+void orc_triangle_stage2_lumping(int lumping) { g_stage2_lumping = lumping; }
+
 int orc_triangle_stage2(double gamma, const double *Wn, const double *Ws, const double *xy, double dt,
                         const double *phiT_n, const double *phiN_n, double *PhiT, double *PhiN, double *PhiLDA,
                         double *PhiB) {
@@ -815,7 +842,7 @@ int orc_triangle_stage2(double gamma, const double *Wn, const double *Ws, const 
   if (!(g.area > 0.0)) return fail(ORC_EINVAL, "triangle must be counter-clockwise");
   Core<double> core;
   Stage2Out<double> o;
-  int rc = triangle_stage2(gamma, ORC_SCHEME_B, wn, ws, g, dt, pT, pN, core, o);
+  int rc = triangle_stage2(gamma, ORC_SCHEME_B, wn, ws, g, dt, pT, pN, core, o, g_stage2_lumping);
   if (rc) return fail(rc, "non-physical state");
   if (PhiT) std::memcpy(PhiT, o.PhiT, sizeof o.PhiT);
   if (PhiN) std::memcpy(PhiN, o.PhiN, sizeof o.PhiN);

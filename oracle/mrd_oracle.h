@@ -28,6 +28,7 @@ int orc_mesh_create(orc_mesh **out, double gamma, double cfl, int scheme, int ti
                     const uint8_t *vertex_flag,                  /* [nv] or NULL; 1 = frozen (L582) */
                     int64_t n_wall_edge, const int32_t *wall_edge /* [ne][2] or NULL (L586) */);
 void orc_mesh_destroy(orc_mesh *m);
+int orc_set_lumping(orc_mesh *m, int lumping);   /* 0 = global (L576, default), 1 = selective lumping eq. 66-67 */
 int orc_set_num_threads(orc_mesh *m, int n);     /* OpenMP threads for the triangle loop (timing only) */
 int orc_set_state(orc_mesh *m, const double *W);  /* also records the frozen-vertex values */
 int orc_get_state(const orc_mesh *m, double *W);
@@ -61,6 +62,8 @@ int orc_triangle_stage1(double gamma, const double *W, const double *xy,
 int orc_triangle_stage2(double gamma, const double *Wn, const double *Ws, const double *xy, double dt,
                         const double *phiT_n, const double *phiN_n,
                         double *PhiT, double *PhiN, double *PhiLDA, double *PhiB);
+/* Lumping used by the NEXT calls of orc_triangle_stage2 on this thread (0 global, 1 selective). */
+void orc_triangle_stage2_lumping(int lumping);
 /* Wall correction of eq. 68-71 for one edge a->b with OUTWARD unit normal n: out Phi_a[4], Phi_b[4]. */
 void orc_wall_edge(double gamma, const double *Wa, const double *Wb, double nx, double ny, double len,
                    double *Phi_a, double *Phi_b);
