@@ -18,7 +18,7 @@ class Params(C.Structure):
     """mrd_params of include/mrd.h."""
     _fields_ = [("gamma", C.c_double), ("cfl", C.c_double), ("scheme", C.c_int32), ("time_order", C.c_int32),
                 ("precision", C.c_int32), ("reorder", C.c_int32), ("period_x", C.c_double), ("period_y", C.c_double),
-                ("tile", C.c_int32), ("reserved", C.c_int32)]
+                ("tile", C.c_int32), ("lumping", C.c_int32)]
 
 
 class MrdError(RuntimeError):
@@ -103,9 +103,9 @@ def _mesh_args(xy, tri, vertex_flag, wall_edge):
 
 
 def make_params(gamma=1.4, cfl=0.5, scheme=SCHEME_B, time_order=2, precision=FP64, reorder=True,
-                period=(0.0, 0.0), tile=0) -> Params:
+                period=(0.0, 0.0), tile=0, lumping=0) -> Params:
     return Params(float(gamma), float(cfl), int(scheme), int(time_order), int(precision), int(bool(reorder)),
-                  float(period[0]), float(period[1]), int(tile), 0)
+                  float(period[0]), float(period[1]), int(tile), int(lumping))
 
 
 class Layout:

@@ -279,6 +279,7 @@ template <class R> int set_state_impl(mrd_mesh *m, const R *W_dev, cudaStream_t 
   c.t = 0.0; c.dt = 0.0; c.t_end = 0.0; c.cfl = m->L.p.cfl;
   c.dmin_bits = 0x7FF0000000000000ull; c.steps = 0; c.status = 0; c.active = 0;
   c.bvar = m->L.p.scheme == MRD_SCHEME_BMAX ? 1 : (m->L.p.scheme == MRD_SCHEME_BMIN ? 2 : 0);
+  c.lumping = m->L.p.lumping;
   CUDA_TRY(cudaMemcpyAsync(m->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s));
   CUDA_TRY(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
   mrd::set_state_kernel<R><<<blocks_for(nv, 256), 256, 0, s>>>(nv, m->d_vperm, W_dev, (R)m->L.p.gamma, (V4 *)m->d_W[0],
@@ -324,7 +325,6 @@ template <class K, class... Args> void launch_tile(mrd_mesh *m, K kernel, size_t
 // tile sizes the fused kernels are compiled for
 #define MRD_TILE_DISPATCH_G(T, CALL)                      \
   switch (T) {                                           \
-    case 32: { constexpr int TILE = 32; CALL; } break;   \
     case 64: { constexpr int TILE = 64; CALL; } break;   \
     default: { constexpr int TILE = 128; CALL; } break;  \
   }
@@ -368,9 +368,17 @@ template <class R, int SCHEME> void launch_stage2(mrd_mesh *m, int b, cudaStream
     auto td = tile_dev<R>(m);
     const size_t sh = m->L.geom_table ? mrd::TileSmem<R, 2, true>(td.tile, td.maxslots, td.plan_stride, td.maxshapes).total
                                       : mrd::TileSmem<R, 2, false>(td.tile, td.maxslots, td.plan_stride, 0).total;
-    MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, false, TILE, GTAB>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
-                                            (const V4 *)m->d_slotZ[b], (const R *)nullptr, (const V4 *)m->d_slotD, (R *)m->d_phi16,
-                                            (V4 *)m->d_part, (R *)nullptr, (V4 *)nullptr, (R *)nullptr, m->d_flag)))
+    if (m->L.p.lumping) {
+      constexpr bool LUMP = true;
+      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, LUMP, TILE, GTAB>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
+                                              (const V4 *)m->d_slotZ[b], (const R *)nullptr, (const V4 *)m->d_slotD, (R *)m->d_phi16,
+                                              (V4 *)m->d_part, (R *)nullptr, (V4 *)nullptr, (R *)nullptr, m->d_flag)))
+    } else {
+      constexpr bool LUMP = false;
+      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, LUMP, TILE, GTAB>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
+                                              (const V4 *)m->d_slotZ[b], (const R *)nullptr, (const V4 *)m->d_slotD, (R *)m->d_phi16,
+                                              (V4 *)m->d_part, (R *)nullptr, (V4 *)nullptr, (R *)nullptr, m->d_flag)))
+    }
     return;
   }
   auto md = mesh_dev<R>(m);

@@ -18,7 +18,7 @@ struct Ctl {
   int status;                    // 0, or MRD_ENONPHYSICAL (as positive flag 1)
   int active;                    // 1 while the step in flight has to be done
   int bvar;                      // blend variant of scheme B (L503): 0 = diagonal Theta, 1 = Bmax, 2 = Bmin
-  int pad;
+  int lumping;                   // 0 = global lumping (L576), 1 = selective lumping (eq. 66-67)
 };
 
 template <class R> struct MeshDev {
@@ -204,9 +204,28 @@ tri_stage2_kernel(MeshDev<R> m, R gamma, const Ctl *__restrict__ ctl, const Vec4
     pN[i][2] = m2 + R(0.5) * (pN[i][2] + o.z);
     pN[i][3] = m3 + R(0.5) * (pN[i][3] + o.w);
   }
+  R E[3][4];
+  const bool lump = ctl->lumping != 0;
+  if (lump) {  // selective lumping (eq. 66-67): E_i = |T|/12 (3 dW_i/dt - sum_j dW_j/dt), on Phi^N and Phi^LDA alike
+    Vec4<R> d0 = ld4(&dWdt[v[0]]), d1 = ld4(&dWdt[v[1]]), d2 = ld4(&dWdt[v[2]]);
+    R dv[3][4] = {{d0.x, d0.y, d0.z, d0.w}, {d1.x, d1.y, d1.z, d1.w}, {d2.x, d2.y, d2.z, d2.w}};
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        E[i][c] = (R(0.25) * a3) * (R(3) * dv[i][c] - (dv[0][c] + dv[1][c] + dv[2][c]));
+        pN[i][c] += E[i][c];
+      }
+  }
   if (SCHEME != MRD_SCHEME_N) {
     R pL[3][4];
     apply_beta(gamma, k, g, PT, pL);  // eq. 63 with eq. 65: Phi_i^LDA = beta_i(W*) Phi^T
+    if (lump) {
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) pL[i][c] += E[i][c];
+    }
     if (SCHEME == MRD_SCHEME_B) {
       blend(PT, pN, pL, ctl->bvar);
     } else {

@@ -78,9 +78,10 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
   if (!(p->gamma > 1.0) || !(p->cfl > 0.0)) { err = "gamma must be > 1 and cfl > 0"; return MRD_EINVAL; }
   if (p->scheme < 0 || p->scheme > 4 || (p->time_order != 1 && p->time_order != 2)) { err = "bad scheme/time_order"; return MRD_EINVAL; }
   if (p->precision != MRD_FP64 && p->precision != MRD_FP32) { err = "bad precision"; return MRD_EINVAL; }
+  if (p->lumping != 0 && p->lumping != 1) { err = "lumping must be 0 (global) or 1 (selective)"; return MRD_EINVAL; }
   if (p->period_x < 0.0 || p->period_y < 0.0) { err = "negative period"; return MRD_EINVAL; }
   if (ne < 0 || (ne > 0 && !wall_edge)) { err = "bad wall edge list"; return MRD_EINVAL; }
-  if (p->tile != -1 && p->tile != 0 && p->tile != 32 && p->tile != 64 && p->tile != 128) { err = "tile must be -1, 0, 32, 64 or 128"; return MRD_EINVAL; }
+  if (p->tile != -1 && p->tile != 0 && p->tile != 64 && p->tile != 128) { err = "tile must be -1, 0, 64 or 128"; return MRD_EINVAL; }
   L.p = *p;
   L.nv = nv; L.nt = nt; L.ne = ne;
   const double period[2] = {p->period_x, p->period_y};

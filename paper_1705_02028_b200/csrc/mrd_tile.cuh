@@ -169,6 +169,8 @@ __device__ __forceinline__ void tile_epilogue(int T, const R *res, const R *sT, 
 #ifndef MRD_TILE_MINB
 #define MRD_TILE_MINB 4
 #endif
+// STORE: stage 1 keeps phi^N(W^n), phi^T(W^n) for stage 2; stage 2 reuses the flag for selective lumping (eq. 66-67), a
+// compile-time switch because the extra live ranges of a run-time branch cost the headline configuration 8 %.
 template <class R, int SCHEME, int STAGE, bool STORE, int TILE, bool GTAB>
 __global__ void __launch_bounds__(TILE, (MRD_TILE_MINB * 128) / TILE)
 tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ slotZ,
@@ -199,6 +201,7 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
     n1 = ld_info(td.tile_info + b + gridDim.x + 1);
   }
   const int bvar = ctl->bvar;
+  constexpr bool lump = STAGE == 2 && STORE;
   bool bad = false;  // linearised c^2 <= 0 met by this thread (raised once, after the loop)
   for (int k = 0; b < td.ntile; b += gridDim.x, ++k) {
     const int cur = k & 1;
@@ -274,6 +277,17 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
             pN[i][c] = m[c] + R(0.5) * (pN[i][c] + sP[(i * 4 + c) * T]);
           }
         }
+        if (lump) {  // selective lumping (eq. 66-67): E_i = sum_j (|T| d_ij/3 - m^G_ij) dW_j/dt = |T|/12 (3 dW_i - sum_j dW_j)
+          Vec4<R> d0 = sD[l[0]], d1 = sD[l[1]], d2 = sD[l[2]];
+          R sm[4] = {d0.x + d1.x + d2.x, d0.y + d1.y + d2.y, d0.z + d1.z + d2.z, d0.w + d1.w + d2.w};
+#pragma unroll
+          for (int i = 0; i < 3; ++i) {
+            Vec4<R> d = sD[l[i]];
+            R dv[4] = {d.x, d.y, d.z, d.w};
+#pragma unroll
+            for (int c = 0; c < 4; ++c) pN[i][c] += (R(0.25) * a3) * (R(3) * dv[c] - sm[c]);
+          }
+        }
       }
       // The nodal N residuals go to shared memory now (their final place for scheme N); the LDA residuals are then
       // produced node by node and blended in place -- 24 fewer values live at once than blending from registers.
@@ -296,6 +310,14 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
           R z[4], Lw[4];
           apply_split<false>(kk.ap[i], kk.bp[i], kk.l3p[i], g.nx[i], g.ny[i], y, z);
           to_conserved(kk, z, Lw);
+          if (STAGE == 2 && lump) {  // the same anti-diffusive term on the LDA residual (L567)
+            const Vec4<R> *sD = reinterpret_cast<const Vec4<R> *>(buf + L.oD);
+            Vec4<R> d0 = sD[l[0]], d1 = sD[l[1]], d2 = sD[l[2]], d = sD[l[i]];
+            Lw[0] += (R(0.25) * a3) * (R(3) * d.x - (d0.x + d1.x + d2.x));
+            Lw[1] += (R(0.25) * a3) * (R(3) * d.y - (d0.y + d1.y + d2.y));
+            Lw[2] += (R(0.25) * a3) * (R(3) * d.z - (d0.z + d1.z + d2.z));
+            Lw[3] += (R(0.25) * a3) * (R(3) * d.w - (d0.w + d1.w + d2.w));
+          }
 #pragma unroll
           for (int c = 0; c < 4; ++c) {
             R *r = res + (i * 4 + c) * T + tid;

@@ -280,3 +280,24 @@ def test_bmax_bmin_variants_match_oracle(mrd, scheme, tile):
     gb = gpu_mesh(mrd, mesh, W, scheme=2, tile=tile)
     gb.step(50)
     assert field_errors(gb.get_state().cpu().numpy(), om.get_state()) > 1e-6
+
+
+@pytest.mark.parametrize("scheme", [2, 1, 0])
+@pytest.mark.parametrize("tile", [-1, 0])
+def test_selective_lumping_matches_oracle(mrd, scheme, tile):
+    # eq. 66-67 (L563-L570): advected vortex, so that dW/dt and with it the anti-diffusive term is O(1)
+    mesh = wl.uniform_mesh(40, 36, 10.0, 10.0, periodic=True)
+    W = wl.vortex_state(mesh, advect=(1.0, 0.5))
+    gm = gpu_mesh(mrd, mesh, W, scheme=scheme, tile=tile, lumping=1)
+    om = oracle.OracleMesh(mesh.xy, mesh.tri, period=mesh.period, scheme=scheme, lumping=1)
+    om.set_state(W)
+    gm.step(1)
+    om.step(1)
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_1
+    gm.step(49)
+    om.step(49)
+    Wo = om.get_state()
+    assert field_errors(gm.get_state().cpu().numpy(), Wo) <= TOL_100
+    g0 = gpu_mesh(mrd, mesh, W, scheme=scheme, tile=tile)            # global lumping is a different scheme
+    g0.step(50)
+    assert field_errors(g0.get_state().cpu().numpy(), Wo) > 1e-6
