@@ -94,3 +94,70 @@ def test_fp32_at_2048_squared(mrd):
     g32.step(10)
     om.step(10)
     assert field_errors(g32.get_state().cpu().numpy().astype(np.float64), om.get_state()) <= 1e-5
+
+
+def _per_step_parity(mrd, cfg, steps, fp32_too=False, **kw):
+    """1e-12 per step from resynchronised states at a config's FULL size; returns the last GPU state."""
+    import torch
+    mesh = cfg.mesh
+    mk = dict(vertex_flag=cfg.vertex_flag, wall_edge=cfg.wall_edge)
+    gm = mrd.Mesh(mesh.xy, mesh.tri, period=mesh.period, **mk, **kw)
+    om = oracle.OracleMesh(mesh.xy, mesh.tri, period=mesh.period, threads=os.cpu_count() or 1, **mk)
+    om.set_state(cfg.W0)
+    Wg = None
+    for k in range(steps):
+        gm.set_state(torch.tensor(om.get_state(), device="cuda"))
+        n, t, dt = gm.step(1)
+        no, to, dto = om.step(1)
+        assert n == 1 and abs(dt - dto) <= 1e-14 * dto
+        Wg = gm.get_state().cpu().numpy()
+        assert field_errors(Wg, om.get_state()) <= 1e-12, k
+    if fp32_too:
+        g32 = mrd.Mesh(mesh.xy, mesh.tri, period=mesh.period, precision=mrd.FP32, **mk, **kw)
+        g32.set_state(torch.tensor(cfg.W0, device="cuda", dtype=torch.float32))
+        o2 = oracle.OracleMesh(mesh.xy, mesh.tri, period=mesh.period, threads=os.cpu_count() or 1, **mk)
+        o2.set_state(cfg.W0)
+        g32.step(10)
+        o2.step(10)
+        assert field_errors(g32.get_state().cpu().numpy().astype(np.float64), o2.get_state()) <= 1e-5
+    return gm, Wg
+
+
+def test_config2_sod_full_size(mrd):
+    cfg = wl.make_config("sod")                                   # 1025 x 129 vertices, 262 144 triangles
+    assert cfg.mesh.nt == 262144 and cfg.mesh.nv == 132225
+    gm, Wg = _per_step_parity(mrd, cfg, 4)
+    frozen = cfg.vertex_flag.astype(bool)
+    assert frozen.sum() == 258 and np.array_equal(Wg[:, frozen], cfg.W0[:, frozen])
+
+
+def test_config3_kh_full_size_permuted_fp64_and_fp32(mrd):
+    cfg = wl.make_config("kh")                                    # 1024^2 periodic, seeded random numbering
+    assert cfg.mesh.nt == 2097152
+    for reorder in (True, False):
+        gm, Wg = _per_step_parity(mrd, cfg, 2, fp32_too=reorder, reorder=reorder)
+    tot0 = None
+    import torch
+    g = mrd.Mesh(cfg.mesh.xy, cfg.mesh.tri, period=cfg.mesh.period)
+    g.set_state(torch.tensor(cfg.W0, device="cuda"))
+    tot0, _, _ = g.diagnostics()
+    g.step(20)
+    tot1, mr, mp = g.diagnostics()
+    assert np.all(np.abs(tot1 - tot0) <= 1e-12 * np.array([tot0[0], 1.0, 1.0, tot0[3]])) and mr > 0 and mp > 0
+
+
+def test_config4_riemann_full_size_and_diagonal_symmetry(mrd):
+    cfg = wl.make_config("riemann4")                              # 2048^2 vertices, 8 380 418 triangles
+    assert cfg.mesh.nv == 2048 * 2048 and cfg.mesh.nt == 8380418
+    gm, Wg = _per_step_parity(mrd, cfg, 3)
+    frozen = cfg.vertex_flag.astype(bool)
+    assert frozen.sum() == 8188 and np.array_equal(Wg[:, frozen], cfg.W0[:, frozen])
+    # the problem and the SW-NE split mesh are symmetric under (x, y, u, v) -> (y, x, v, u): so is one step of the
+    # solution (to round-off: mirrored triangles are summed in a different order)
+    n = 2048
+    F = Wg.reshape(4, n, n)                                       # [field][j (y)][i (x)], natural numbering
+    assert np.abs(F[0] - F[0].T).max() <= 1e-12 * np.abs(F[0]).max()
+    assert np.abs(F[3] - F[3].T).max() <= 1e-12 * np.abs(F[3]).max()
+    assert np.abs(F[1] - F[2].T).max() <= 1e-12 * np.abs(F[1]).max()
+    _, mr, mp = gm.diagnostics()
+    assert mr > 0 and mp > 0
