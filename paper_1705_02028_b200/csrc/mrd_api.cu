@@ -74,6 +74,12 @@ struct mrd_mesh {
   void *d_slotZ[2] = {nullptr, nullptr}, *d_slotS[2] = {nullptr, nullptr}, *d_slotD = nullptr;  // slot-major Z, |v|+c, dW/dt
   void *d_phi16 = nullptr;        // R [ntile][16][T]: phi^N(W^n) (12) and phi^T(W^n) (4), component-major per tile
   int nsm = 0;
+  // CUDA graphs for launch-bound (small) meshes: two consecutive steps (buffer parity a, then a^1) captured once per
+  // starting parity on an internal stream and replayed; forked from / joined to the caller's stream by events
+  cudaStream_t s_int = nullptr;
+  cudaEvent_t ev_in = nullptr, ev_out = nullptr;
+  cudaGraphExec_t gexec[2] = {nullptr, nullptr};
+  bool graph_ok = false;
   bool has_state = false;
   int64_t steps_base = 0;         // completed steps at the last sync (for buffer parity)
 };
@@ -499,6 +505,45 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
   PROF_MARK(MRD_PROF_CTL)
 }
 
+// n consecutive steps starting from buffer pair `a` (updated).  Small meshes replay a captured two-step graph.
+template <class R> int run_steps(mrd_mesh *m, int scheme, int64_t n, int &a, cudaStream_t s) {
+  if (!m->graph_ok || n < 4) {
+    for (int64_t k = 0; k < n; ++k, a ^= 1) enqueue_step<R>(m, scheme, a, s);
+    return MRD_OK;
+  }
+  CUDA_TRY(cudaEventRecord(m->ev_in, s));
+  CUDA_TRY(cudaStreamWaitEvent(m->s_int, m->ev_in, 0));
+  if (!m->gexec[a]) {
+    enqueue_step<R>(m, scheme, a, m->s_int);  // eager once: sets the kernels' shared-memory attributes before the capture
+    a ^= 1;
+    --n;
+    if (!m->gexec[a]) {
+      const int64_t lc = m->launches;
+      cudaGraph_t g = nullptr;
+      CUDA_TRY(cudaStreamBeginCapture(m->s_int, cudaStreamCaptureModeThreadLocal));
+      enqueue_step<R>(m, scheme, a, m->s_int);
+      enqueue_step<R>(m, scheme, a ^ 1, m->s_int);
+      CUDA_TRY(cudaStreamEndCapture(m->s_int, &g));
+      m->launches = lc;  // captured, not launched
+      cudaError_t e = cudaGraphInstantiate(&m->gexec[a], g, 0);
+      cudaGraphDestroy(g);
+      if (e != cudaSuccess) return fail(MRD_ECUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e));
+    }
+  }
+  const int64_t per_step = (m->L.p.time_order == 2 ? 6 : 4) + (m->nwv > 0 ? (m->L.p.time_order == 2 ? 2 : 1) : 0);
+  for (int64_t k = 0; k + 1 < n; k += 2) {
+    CUDA_TRY(cudaGraphLaunch(m->gexec[a], m->s_int));
+    m->launches += 2 * per_step;
+  }
+  if (n & 1) {
+    enqueue_step<R>(m, scheme, a, m->s_int);
+    a ^= 1;
+  }
+  CUDA_TRY(cudaEventRecord(m->ev_out, m->s_int));
+  CUDA_TRY(cudaStreamWaitEvent(s, m->ev_out, 0));
+  return MRD_OK;
+}
+
 // fetch the control block (after a stream sync) and bring the host bookkeeping up to date
 int fetch_ctl(mrd_mesh *m, cudaStream_t s, mrd::Ctl *out) {
   CUDA_TRY(cudaMemcpyAsync(out, m->d_ctl, sizeof(mrd::Ctl), cudaMemcpyDeviceToHost, s));
@@ -527,7 +572,8 @@ template <class R> int step_impl(mrd_mesh *m, int64_t max_steps, double t_end, c
   int64_t enq = 0;
   int a = m->cur;
   if (!(t_end > 0.0)) {
-    for (; enq < max_steps; ++enq, a ^= 1) enqueue_step<R>(m, scheme, a, s);
+    if ((rc = run_steps<R>(m, scheme, max_steps, a, s))) return rc;
+    enq = max_steps;
     if (!sync) { CUDA_TRY(cudaGetLastError()); return MRD_OK; }
     if ((rc = fetch_ctl(m, s, &c))) return rc;
   } else {
@@ -535,7 +581,7 @@ template <class R> int step_impl(mrd_mesh *m, int64_t max_steps, double t_end, c
     const int64_t chunk = 32;
     while (enq < max_steps) {
       int64_t n = std::min<int64_t>(chunk, max_steps - enq);
-      for (int64_t k = 0; k < n; ++k, a ^= 1) enqueue_step<R>(m, scheme, a, s);
+      if ((rc = run_steps<R>(m, scheme, n, a, s))) return rc;
       enq += n;
       if ((rc = fetch_ctl(m, s, &c))) return rc;
       a = m->cur;
@@ -788,12 +834,24 @@ int mrd_mesh_create(mrd_mesh **out, const mrd_params *p, int64_t nv, const doubl
     rc = fail(MRD_ENOMEM, "out of host memory");
   }
   if (rc) { mrd_mesh_destroy(m); return rc; }
+  // launch-bound regime: below ~4M triangles a step is tens of microseconds, comparable to 6 kernel launches
+  if (m->L.nt <= (int64_t(1) << 22) && !std::getenv("MRD_NO_GRAPH")) {
+    if (cudaStreamCreateWithFlags(&m->s_int, cudaStreamNonBlocking) == cudaSuccess &&
+        cudaEventCreateWithFlags(&m->ev_in, cudaEventDisableTiming) == cudaSuccess &&
+        cudaEventCreateWithFlags(&m->ev_out, cudaEventDisableTiming) == cudaSuccess)
+      m->graph_ok = true;
+  }
   *out = m;
   return MRD_OK;
 }
 
 void mrd_mesh_destroy(mrd_mesh *m) {
   if (!m) return;
+  for (int k = 0; k < 2; ++k)
+    if (m->gexec[k]) cudaGraphExecDestroy(m->gexec[k]);
+  if (m->ev_in) cudaEventDestroy(m->ev_in);
+  if (m->ev_out) cudaEventDestroy(m->ev_out);
+  if (m->s_int) cudaStreamDestroy(m->s_int);
   for (void *p : m->allocs) cudaFree(p);
   if (m->h_pinned) cudaFreeHost(m->h_pinned);
   delete m;
