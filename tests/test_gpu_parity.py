@@ -301,3 +301,52 @@ def test_selective_lumping_matches_oracle(mrd, scheme, tile):
     g0 = gpu_mesh(mrd, mesh, W, scheme=scheme, tile=tile)            # global lumping is a different scheme
     g0.step(50)
     assert field_errors(g0.get_state().cpu().numpy(), Wo) > 1e-6
+
+
+def test_api_edge_cases(mrd):
+    import torch
+    cfg = wl.make_config("sod", n=64)
+    kw = dict(vertex_flag=cfg.vertex_flag, wall_edge=cfg.wall_edge)
+    gm = mrd.Mesh(cfg.mesh.xy, cfg.mesh.tri, period=cfg.mesh.period, **kw)
+    with pytest.raises(mrd.MrdError) as e:                       # no state yet
+        gm.step(1)
+    assert e.value.code == mrd.MRD_EINVAL
+    with pytest.raises(mrd.MrdError):
+        gm.get_state()
+    W0 = torch.tensor(cfg.W0, device="cuda")
+    gm.set_state(W0)
+    assert gm.step(0) == (0, 0.0, 0.0)                           # nothing to do
+    n, t, dt = gm.step(5)
+    assert n == 5 and t > 0 and dt > 0
+    n2, t2, _ = gm.step(1000, t_end=t)                           # already there
+    assert n2 == 0 and t2 == t
+    n3, t3, _ = gm.step(3, t_end=1.0)                            # max_steps binds before t_end
+    assert n3 == 3 and t < t3 < 1.0
+    gm.set_state(W0)                                             # restart: clock and counters reset
+    assert gm.sync()[0] == 0 and gm.sync()[1] == 0.0
+    a = mrd.Mesh(cfg.mesh.xy, cfg.mesh.tri, period=cfg.mesh.period, **kw)   # two meshes alive at once, interleaved
+    a.set_state(W0)
+    a.step_async(4); gm.step_async(4); a.step_async(3); gm.step_async(3)
+    assert np.array_equal(a.get_state().cpu().numpy(), gm.get_state().cpu().numpy())
+    s = torch.cuda.Stream()                                      # a non-default stream
+    with torch.cuda.stream(s):
+        b = mrd.Mesh(cfg.mesh.xy, cfg.mesh.tri, period=cfg.mesh.period, **kw)
+        b.set_state(W0, stream=s)
+        b.step(7, stream=s)
+        Wb = b.get_state(stream=s)
+    s.synchronize()
+    assert np.array_equal(Wb.cpu().numpy(), gm.get_state().cpu().numpy())
+
+
+@pytest.mark.parametrize("scheme,order", [(2, 2), (0, 1)])
+def test_walls_and_frozen_vertices_in_fp32_and_first_order(mrd, scheme, order):
+    cfg = wl.make_config("sod", n=128)
+    kw = dict(vertex_flag=cfg.vertex_flag, wall_edge=cfg.wall_edge, scheme=scheme, time_order=order)
+    om = orc_mesh(cfg.mesh, cfg.W0, **kw)
+    gm = gpu_mesh(mrd, cfg.mesh, cfg.W0, **kw)
+    g32 = gpu_mesh(mrd, cfg.mesh, cfg.W0, precision=1, **kw)
+    gm.step(1); om.step(1)
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_1
+    gm.step(9); om.step(9); g32.step(10)
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_100
+    assert field_errors(g32.get_state().cpu().numpy().astype(np.float64), om.get_state()) <= TOL_F32
