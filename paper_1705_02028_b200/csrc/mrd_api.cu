@@ -342,16 +342,15 @@ template <class R, int SCHEME> void launch_stage1(mrd_mesh *m, bool store, int a
   const R gamma = (R)m->L.p.gamma;
   if (m->fused) {
     auto td = tile_dev<R>(m);
-    const size_t sh = m->L.geom_table ? mrd::TileSmem<R, 1, true>(td.tile, td.maxslots, td.plan_stride, td.maxshapes).total
-                                      : mrd::TileSmem<R, 1, false>(td.tile, td.maxslots, td.plan_stride, 0).total;
+#define MRD_SMEM(STAGE) mrd::TileSmem<R, STAGE, GTAB>(td.tile, td.maxslots, td.plan_stride, td.maxshapes)
     V4 *dbg = m->dbg ? (V4 *)m->d_phi : nullptr;
     R *dbgs = m->dbg ? (R *)m->d_sT : nullptr;
     if (store) {
-      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, true, TILE, GTAB>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
+      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, true, TILE, GTAB>, MRD_SMEM(1).total, s, td, MRD_SMEM(1), gamma, (const mrd::Ctl *)m->d_ctl,
                                               (const V4 *)m->d_slotZ[a], (const R *)m->d_slotS[a], (const V4 *)m->d_slotD, (R *)m->d_phi16,
                                               (V4 *)m->d_part, (R *)m->d_partS, dbg, dbgs, m->d_flag)))
     } else {
-      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, false, TILE, GTAB>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
+      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, false, TILE, GTAB>, MRD_SMEM(1).total, s, td, MRD_SMEM(1), gamma, (const mrd::Ctl *)m->d_ctl,
                                               (const V4 *)m->d_slotZ[a], (const R *)m->d_slotS[a], (const V4 *)m->d_slotD, (R *)m->d_phi16,
                                               (V4 *)m->d_part, (R *)m->d_partS, dbg, dbgs, m->d_flag)))
     }
@@ -372,16 +371,15 @@ template <class R, int SCHEME> void launch_stage2(mrd_mesh *m, int b, cudaStream
   const R gamma = (R)m->L.p.gamma;
   if (m->fused) {
     auto td = tile_dev<R>(m);
-    const size_t sh = m->L.geom_table ? mrd::TileSmem<R, 2, true>(td.tile, td.maxslots, td.plan_stride, td.maxshapes).total
-                                      : mrd::TileSmem<R, 2, false>(td.tile, td.maxslots, td.plan_stride, 0).total;
+
     if (m->L.p.lumping) {
       constexpr bool LUMP = true;
-      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, LUMP, TILE, GTAB>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
+      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, LUMP, TILE, GTAB>, MRD_SMEM(2).total, s, td, MRD_SMEM(2), gamma, (const mrd::Ctl *)m->d_ctl,
                                               (const V4 *)m->d_slotZ[b], (const R *)nullptr, (const V4 *)m->d_slotD, (R *)m->d_phi16,
                                               (V4 *)m->d_part, (R *)nullptr, (V4 *)nullptr, (R *)nullptr, m->d_flag)))
     } else {
       constexpr bool LUMP = false;
-      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, LUMP, TILE, GTAB>, sh, s, td, gamma, (const mrd::Ctl *)m->d_ctl,
+      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, LUMP, TILE, GTAB>, MRD_SMEM(2).total, s, td, MRD_SMEM(2), gamma, (const mrd::Ctl *)m->d_ctl,
                                               (const V4 *)m->d_slotZ[b], (const R *)nullptr, (const V4 *)m->d_slotD, (R *)m->d_phi16,
                                               (V4 *)m->d_part, (R *)nullptr, (V4 *)nullptr, (R *)nullptr, m->d_flag)))
     }

@@ -269,13 +269,13 @@ __device__ __forceinline__ void triangle_core(R gamma, const Vec4<R> Z[3], const
   k.ic = F::rsqrt(c2);
   k.c = c2 * k.ic;
   k.ic2 = k.ic * k.ic;
-  k.cg = k.c / g1;
+  k.cg = k.c * F::rcp(g1);  // (an IEEE division of two block-uniform values costs ~25 instructions and a branch per thread)
 
   // O3 (reading C3): delta_j = D(Zbar)(Z_j - Z_0) mapped to symmetrising variables; the composition is
   //   drho = 2 zb0 d0, du = zb0 d1 - zb1 d0, dv = zb0 d2 - zb2 d0,
   //   dp = (g1/gamma) (zb3 d0 + zb0 d3 - zb1 d1 - zb2 d2)
   // (exactly zero when Z_j == Z_0, so uniform flow has zero residual, L237)
-  const R gg = g1 / gamma;
+  const R gg = g1 * F::rcp(gamma);
   R dq[3][4];
   dq[0][0] = dq[0][1] = dq[0][2] = dq[0][3] = R(0);
 #pragma unroll

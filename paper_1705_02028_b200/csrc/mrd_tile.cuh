@@ -95,22 +95,23 @@ __device__ __forceinline__ void tile_geometry(const R x[3], const R y[3], TriGeo
 
 // ---- shared-memory carve-up (dynamic).  Two stage-in buffers + the residual exchange area ----------------
 template <class R, int STAGE, bool GTAB> struct TileSmem {
-  size_t oZ, oD, oS, oXY, oPlan, oPhi, buf_bytes;  // per buffer (oXY holds the geometry records when GTAB)
-  size_t oRes, oST, oBar, total;                   // shared
-  __host__ __device__ static size_t up16(size_t x) { return (x + 15) & ~size_t(15); }
+  // computed once on the host and passed to the kernel by value (the device code recomputed it every tile otherwise)
+  uint32_t oZ, oD, oS, oXY, oPlan, oPhi, buf_bytes;  // per buffer (oXY holds the geometry records when GTAB)
+  uint32_t oRes, oST, oBar, total;                   // shared
+  __host__ __device__ static uint32_t up16(size_t x) { return (uint32_t)((x + 15) & ~size_t(15)); }
   __host__ __device__ TileSmem(int T, int maxslots, int plan_stride, int maxshapes) {
-    size_t o = 0;
+    uint32_t o = 0;
     oZ = o; o += up16(sizeof(Vec4<R>) * maxslots);
     oD = o; if (STAGE == 2) o += up16(sizeof(Vec4<R>) * maxslots);
     oS = o; if (STAGE == 1) o += up16(sizeof(R) * maxslots);
     oXY = o; o += GTAB ? up16(sizeof(R) * 12 * maxshapes) : up16(sizeof(R) * 2 * maxslots);
     oPlan = o; o += up16(sizeof(uint16_t) * plan_stride);
     oPhi = o; if (STAGE == 2) o += up16(sizeof(R) * 16 * T);
-    buf_bytes = (o + 31) & ~size_t(31);
-    size_t s = 2 * buf_bytes;
+    buf_bytes = (o + 31u) & ~31u;
+    uint32_t s = 2 * buf_bytes;
     // stage 2: the residual exchange area aliases the current buffer's phi16 block -- thread `tid` only overwrites the
     // 12 entries [c][tid] it has consumed itself, so no other thread's data is touched (saves 12 KB: 4 blocks per SM)
-    oRes = s; if (STAGE == 1) s += sizeof(R) * 12 * T;
+    oRes = s; if (STAGE == 1) s += (uint32_t)(sizeof(R) * 12 * T);
     oST = s; if (STAGE == 1) s += up16(sizeof(R) * T);
     oBar = s; s += 16;
     total = s;
@@ -173,7 +174,7 @@ __device__ __forceinline__ void tile_epilogue(int T, const R *res, const R *sT, 
 // compile-time switch because the extra live ranges of a run-time branch cost the headline configuration 8 %.
 template <class R, int SCHEME, int STAGE, bool STORE, int TILE, bool GTAB>
 __global__ void __launch_bounds__(TILE, (MRD_TILE_MINB * 128) / TILE)
-tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ slotZ,
+tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ slotZ,
             const R *__restrict__ slotS, const Vec4<R> *__restrict__ slotD, R *__restrict__ phi16,
             Vec4<R> *__restrict__ part, R *__restrict__ partS, Vec4<R> *__restrict__ phi_dbg, R *__restrict__ sT_dbg,
             int *status) {
@@ -181,7 +182,6 @@ tile_kernel(TileDev<R> td, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int T = TILE;  // compile-time tile size: shared-memory and phi16 strides become immediates
   const int tid = threadIdx.x;
-  const TileSmem<R, STAGE, GTAB> L(T, td.maxslots, td.plan_stride, td.maxshapes);
   R *res1 = reinterpret_cast<R *>(smem_raw + L.oRes);
   R *sST = reinterpret_cast<R *>(smem_raw + L.oST);
   uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + L.oBar);
