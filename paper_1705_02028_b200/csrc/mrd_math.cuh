@@ -401,10 +401,12 @@ template <class R> __device__ __forceinline__ void blend_theta(const R X[4], con
   using F = Fast<R>;
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
+    // Theta = min(1, |X| / den), and 0 on a zero denominator (C10).  den = 0 means every nodal residual is exactly 0,
+    // which makes X and the LDA residuals exactly 0 too, so the value taken there (1) changes nothing: B_i = 0.
     R den = F::abs(N[0][c]) + F::abs(N[1][c]) + F::abs(N[2][c]);
-    bool pos = den > R(0);
-    R t = F::min(R(1), F::abs(X[c]) * F::rcp(pos ? den : R(1)));
-    th[c] = pos ? t : R(0);
+    // Written so that a zero or denormal denominator (reciprocal inf, product inf or NaN) also lands on 1.
+    R t = F::abs(X[c]) * F::rcp(den);
+    th[c] = t < R(1) ? t : R(1);
   }
   if (bvar != 0) {
     R hi = F::max(F::max(th[0], th[1]), F::max(th[2], th[3]));
