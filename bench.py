@@ -33,7 +33,7 @@ UNIT = "triangle-updates/s"
 # (2*DFMA + DADD + DMUL per thread, from ncu's smsp__sass_thread_inst_executed_op_d*_pred_on of the profiled
 # launch, profiles/) is the smaller one; the oracle's own count (orc_count_ops) is kept for context.
 FLOPS_TRI_STAGE1 = {"fp64": 677.0, "fp32": 640.0}
-FLOPS_TRI_STAGE2 = {"fp64": 751.0, "fp32": 710.0}
+FLOPS_TRI_STAGE2 = {"fp64": 753.0, "fp32": 710.0}
 FLOPS_VERTEX_STAGE = 144.0             # per triangle-update, all three vertex kernels together (ncu: 8.6 + 71.5 + 63.5)
 ORACLE_FLOPS_TRI = (2098.0, 2194.0)    # oracle.count_ops(stage 1 / stage 2): add+mul+div+sqrt
 # compulsory HBM bytes per triangle of one triangle-kernel launch (share of SURVEY 8d's 130 B per triangle-update):
