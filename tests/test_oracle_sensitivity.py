@@ -40,3 +40,24 @@ def test_round_off_amplification_grows_with_resolution_on_the_smooth_vortex():
     coarse = drift(wl.make_config("sweep", n=128), 4, amp=1e-16)
     fine = drift(wl.make_config("sweep", n=512), 4, amp=1e-16)
     assert coarse < 1e-14 and fine > 20 * coarse
+
+
+def test_blend_coefficient_is_decided_by_round_off_where_a_residual_component_vanishes():
+    # linear sound wave along x (L766): the exact y-momentum residual is zero while the nodal N residuals are not, so
+    # Theta_y = |phi_y| / sum |phi^N_y| (eq. 53) is round-off over O(1): the B scheme's result depends on the last bit,
+    # the LDA and N schemes' results do not
+    mesh = wl.uniform_mesh(64, 4, 1.0, 4.0 / 64, periodic=True)
+    W = wl.sound_wave_state(mesh)
+    rng = np.random.default_rng(0)
+    Wp = W * (1.0 + 2e-16 * rng.standard_normal(W.shape))
+    d = {}
+    for name, scheme, order in (("B", oracle.SCHEME_B, 2), ("LDA", oracle.SCHEME_LDA, 2), ("N", oracle.SCHEME_N, 1)):
+        a = oracle.OracleMesh(mesh.xy, mesh.tri, period=mesh.period, scheme=scheme, time_order=order)
+        b = oracle.OracleMesh(mesh.xy, mesh.tri, period=mesh.period, scheme=scheme, time_order=order)
+        a.set_state(W)
+        b.set_state(Wp)
+        a.step(10 ** 6, t_end=0.25)
+        b.step(10 ** 6, t_end=0.25)
+        d[name] = np.abs(a.get_state()[0] - b.get_state()[0]).max()
+    assert d["LDA"] < 1e-13 and d["N"] < 1e-13
+    assert 1e-10 < d["B"] < 1e-3 * 1e-4                   # ~2e-8: five orders above round-off, still << the amplitude

@@ -26,5 +26,7 @@ from .states import (  # noqa: F401
     riemann4_state,
     uniform_state,
     random_smooth_state,
+    sound_wave_state,
+    noh_state,
 )
 from .configs import make_config, CONFIG_NAMES  # noqa: F401

@@ -131,3 +131,24 @@ def random_smooth_state(mesh: UniformMesh, gamma: float = 1.4, seed: int = 3, ma
     u = mach * c * np.tanh(field())
     v = mach * c * np.tanh(field())
     return primitive_to_conserved(rho, u, v, p, gamma)
+
+
+def sound_wave_state(mesh: UniformMesh, gamma: float = 1.4, amplitude: float = 1e-4) -> np.ndarray:
+    """Linear right-moving sound wave, PAPER.md 5.1.1 (L766): rho = 1, v = 0, c = 1 background, wavelength = domain
+    length in x, amplitude 1e-4.  Eigenvector of the linearised equations: d rho = A s, d u = c A s / rho, d p = c^2 A s."""
+    s = np.sin(2.0 * np.pi * mesh.xy[:, 0] / mesh.lengths[0])
+    rho = 1.0 + amplitude * s
+    u = amplitude * s
+    p = 1.0 / gamma + amplitude * s
+    return primitive_to_conserved(rho, u, 0.0, p, gamma)
+
+
+def noh_state(mesh: UniformMesh, gamma: float = 5.0 / 3.0, p0: float = 1e-6) -> np.ndarray:
+    """Noh problem, PAPER.md 5.2.2 (L901-L913): rho = 1, unit velocity towards the centre of the domain, p = 1e-6."""
+    x = mesh.xy[:, 0] - 0.5 * mesh.lengths[0]
+    y = mesh.xy[:, 1] - 0.5 * mesh.lengths[1]
+    r = np.sqrt(x * x + y * y)
+    safe = np.where(r > 0, r, 1.0)
+    u = np.where(r > 0, -x / safe, 0.0)
+    v = np.where(r > 0, -y / safe, 0.0)
+    return primitive_to_conserved(np.ones(mesh.nv), u, v, p0, gamma)
