@@ -67,7 +67,8 @@ typedef struct {
  * (L397-L399) and the dual volumes V_i = sum |T|/3 (L441, reading C5).
  *   xy   host [nv][2] double   vertexCoordinates  (L656-L663)
  *   tri  host [nt][3] int32    triangleVertices, any orientation
- *   vertex_flag host [nv] uint8 or NULL: 1 = frozen ghost vertex that keeps its initial state (L582)
+ *   vertex_flag host [nv] uint8 or NULL: 1 = frozen ghost vertex that keeps its initial state (L582);
+ *               2 = halo vertex of a partition (see mrd_partition_create)
  *   wall_edge   host [ne][2] int32 or NULL: vertex pairs of edges on reflecting walls (L586-L602);
  *               each must belong to exactly one triangle
  * Errors: MRD_EINVAL (null/empty mesh, index out of range, repeated vertex in a triangle, zero-area
@@ -161,6 +162,76 @@ enum {
   MRD_PROFILE_SLOTS = 8
 };
 int mrd_step_profile(mrd_mesh *m, void *stream, float ms[MRD_PROFILE_SLOTS]);
+
+/* ------------------------------------------------------------------------------------------------
+ * Domain decomposition for several GPUs (the paper ran on one device and names no scheme, so
+ * this is this library's own: owner-computes over contiguous ranges of the vertices' Morton order,
+ * L669-L675).  Part `part` of `n_part` OWNS the vertices of its range, holds every triangle incident to
+ * an owned vertex (triangles cut by the partition are held and recomputed by each side: no residual is
+ * exchanged) and, as HALO vertices, the other vertices of those triangles.  One exchange of vertex states
+ * per stage (after eq. 60 and after eq. 61 / 43) and one min-reduction of a double per step (eq. 44)
+ * keep every part's copy equal to the single-device run up to summation order.
+ *
+ * mrd_partition_create (host only, no CUDA): arguments as mrd_layout_create plus the periods; the global
+ * mesh is given in full to every part.  Errors: MRD_EINVAL (as the layout stage; vertex_flag other than
+ * 0/1; n_part < 1; part out of range; a part without vertices), MRD_ENOMEM.
+ * mrd_partition_sizes: n[0] = local vertices (owned first, then halo; each group in ascending global id),
+ *   n[1] = owned vertices, n[2] = local triangles (ascending global id), n[3] = local wall edges,
+ *   n[4] = neighbour parts, n[5] = vertices sent per exchange, n[6] = vertices received per exchange,
+ *   n[7] = global vertices.
+ * mrd_partition_get(name, dst host, bytes = exact size of the array; MRD_EINVAL otherwise):
+ *   "vertex_global" int32[n0]    global id of each local vertex
+ *   "xy"            double[n0][2]
+ *   "tri"           int32[n2][3] local vertex ids, node order of the global triangle
+ *   "tri_global"    int32[n2]
+ *   "vertex_flag"   uint8[n0]    0 free, 1 frozen (L582), 2 halo  -> pass to mrd_mesh_create
+ *   "wall_edge"     int32[n3][2] local ids (wall edges with an owned end)
+ *   "neighbour"     int32[n4]    ascending part ids
+ *   "send_off"      int32[n4+1], "send_idx" int32[n5]: owned local vertices whose state neighbour k needs,
+ *   "recv_off"      int32[n4+1], "recv_idx" int32[n6]: halo local vertices owned by neighbour k; both lists
+ *                   ascending in global id per neighbour, so that send list of a for b == recv list of b from a
+ *   "owner"         int32[n7]    owning part of every global vertex
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct mrd_partition mrd_partition;
+int mrd_partition_create(mrd_partition **out, int64_t n_vertex, const double *xy, int64_t n_triangle,
+                         const int32_t *tri, const uint8_t *vertex_flag, int64_t n_wall_edge,
+                         const int32_t *wall_edge, double period_x, double period_y, int32_t n_part, int32_t part);
+void mrd_partition_destroy(mrd_partition *p);
+int mrd_partition_sizes(const mrd_partition *p, int64_t n[8]);
+int mrd_partition_get(const mrd_partition *p, const char *name, void *dst, int64_t bytes);
+
+/* Halo lists of a mesh created from a partition (vertex_flag 2 = halo: such a vertex keeps its value in
+ * the updates like a frozen one, is left out of the minimum of eq. 44 and of the totals of
+ * mrd_get_diagnostics, and gets its value from mrd_halo_unpack).  send_idx / recv_idx: HOST int32 lists
+ * of USER (= partition-local) vertex ids, copied; recv_idx must name halo vertices only (MRD_EINVAL). */
+int mrd_halo_set(mrd_mesh *m, int64_t n_send, const int32_t *send_idx, int64_t n_recv, const int32_t *recv_idx);
+
+/* One time step in phases, for a caller that exchanges between them (all enqueued on `stream`; none
+ * synchronises except begin/end).  Sequence per step, the same on every part:
+ *   mrd_phase(RESIDUAL1)   stage-1 triangle pass, wall terms, local min of 2 V_i / sum s_T (eq. 44-45)
+ *   mrd_dt_get -> min-reduce the two doubles over all parts -> mrd_dt_set
+ *   mrd_phase(UPDATE1)     eq. 60 (time_order 2) or eq. 43 (time_order 1) on the owned vertices
+ *   mrd_halo_pack -> exchange -> mrd_halo_unpack
+ *   time_order 2 only: mrd_phase(STAGE2) (stage-2 triangle pass, eq. 61 on the owned vertices), then
+ *   mrd_halo_pack -> exchange -> mrd_halo_unpack
+ *   mrd_phase(END)         advance t, count the step
+ * mrd_phase_begin settles earlier asynchronous work, arms the stepper and sets t_end (<= 0: none; every part
+ * must pass the same); mrd_phase_end synchronises and reports like mrd_step (steps_done counts the steps since
+ * mrd_phase_begin).  A non-physical state met by any part reaches all of them through the second double of
+ * mrd_dt_get/set one step later; the distributed state is then undefined until the next mrd_set_state. */
+enum { MRD_PHASE_RESIDUAL1 = 0, MRD_PHASE_UPDATE1 = 1, MRD_PHASE_STAGE2 = 2, MRD_PHASE_END = 3 };
+int mrd_phase_begin(mrd_mesh *m, double t_end, void *stream);
+int mrd_phase(mrd_mesh *m, int32_t phase, void *stream);
+int mrd_phase_end(mrd_mesh *m, void *stream, int64_t *steps_done, double *t, double *dt_last);
+/* d DEVICE double[2]: d[0] = local min_i 2 V_i / sum s_T over non-halo vertices, d[1] = -1 if this part met a
+ * non-physical state, else 0.  After the min-reduction, mrd_dt_set installs both. */
+int mrd_dt_get(mrd_mesh *m, double *d_dev, void *stream);
+int mrd_dt_set(mrd_mesh *m, const double *d_dev, void *stream);
+/* buf DEVICE [n_send][4] / [n_recv][4] (double or float per precision), rows in list order: the conserved
+ * state just written by the preceding UPDATE1 / STAGE2 phase.  Unpack also derives what the triangle kernels
+ * read (Z, and dW/dt of eq. 57 or |v| + c) exactly as the owner did, so halo copies are bitwise the owner's. */
+int mrd_halo_pack(mrd_mesh *m, void *buf_dev, void *stream);
+int mrd_halo_unpack(mrd_mesh *m, const void *buf_dev, void *stream);
 
 /* Kernel launch counter: number of the library's own kernel launches since the mesh was created. */
 int mrd_launch_count(const mrd_mesh *m, int64_t *launches);

@@ -61,6 +61,20 @@ def lib():
         L.mrd_measure_peaks.argtypes = [_dp, _dp, _dp, vp]
         L.mrd_launch_count.argtypes = [vp, _lp]
         L.mrd_step_profile.argtypes = [vp, vp, C.POINTER(C.c_float)]
+        L.mrd_partition_create.argtypes = [C.POINTER(vp), C.c_int64, _dp, C.c_int64, _ip, _bp, C.c_int64, _ip, C.c_double,
+                                           C.c_double, C.c_int32, C.c_int32]
+        L.mrd_partition_destroy.argtypes = [vp]
+        L.mrd_partition_destroy.restype = None
+        L.mrd_partition_sizes.argtypes = [vp, _lp]
+        L.mrd_partition_get.argtypes = [vp, C.c_char_p, vp, C.c_int64]
+        L.mrd_halo_set.argtypes = [vp, C.c_int64, _ip, C.c_int64, _ip]
+        L.mrd_phase_begin.argtypes = [vp, C.c_double, vp]
+        L.mrd_phase.argtypes = [vp, C.c_int32, vp]
+        L.mrd_phase_end.argtypes = [vp, vp, _lp, _dp, _dp]
+        L.mrd_dt_get.argtypes = [vp, vp, vp]
+        L.mrd_dt_set.argtypes = [vp, vp, vp]
+        L.mrd_halo_pack.argtypes = [vp, vp, vp]
+        L.mrd_halo_unpack.argtypes = [vp, vp, vp]
         L.mrd_last_error.restype = C.c_char_p
         L.mrd_version.restype = C.c_char_p
         L._path = path
@@ -143,6 +157,35 @@ def _stream_ptr(stream):
         import torch
         stream = torch.cuda.current_stream()
     return C.c_void_p(int(stream.cuda_stream))
+
+
+class Partition:
+    """mrd_partition_*: one part of the domain decomposition of a global mesh (host only, no CUDA needed)."""
+
+    _ARRAYS = (("vertex_global", np.int32, lambda n: (n[0],)), ("xy", np.float64, lambda n: (n[0], 2)),
+               ("tri", np.int32, lambda n: (n[2], 3)), ("tri_global", np.int32, lambda n: (n[2],)),
+               ("vertex_flag", np.uint8, lambda n: (n[0],)), ("wall_edge", np.int32, lambda n: (n[3], 2)),
+               ("neighbour", np.int32, lambda n: (n[4],)), ("send_off", np.int32, lambda n: (n[4] + 1,)),
+               ("send_idx", np.int32, lambda n: (n[5],)), ("recv_off", np.int32, lambda n: (n[4] + 1,)),
+               ("recv_idx", np.int32, lambda n: (n[6],)), ("owner", np.int32, lambda n: (n[7],)))
+
+    def __init__(self, xy, tri, n_part, part, vertex_flag=None, wall_edge=None, period=(0.0, 0.0)):
+        keep, args = _mesh_args(xy, tri, vertex_flag, wall_edge)
+        h = C.c_void_p()
+        _check(lib().mrd_partition_create(C.byref(h), *args, float(period[0]), float(period[1]), int(n_part), int(part)))
+        try:
+            n = (C.c_int64 * 8)()
+            _check(lib().mrd_partition_sizes(h, n))
+            n = [int(x) for x in n]
+            (self.n_local, self.n_owned, self.n_tri, self.n_wall, self.n_neighbour, self.n_send, self.n_recv,
+             self.n_global) = n
+            for name, dt, shape in self._ARRAYS:
+                a = np.empty(shape(n), dtype=dt)
+                _check(lib().mrd_partition_get(h, name.encode(), C.c_void_p(a.ctypes.data), a.nbytes))
+                setattr(self, name, a)
+        finally:
+            lib().mrd_partition_destroy(h)
+        self.n_part, self.part, self.period = int(n_part), int(part), (float(period[0]), float(period[1]))
 
 
 class Mesh:
@@ -243,6 +286,47 @@ class Mesh:
                                             _np_ptr(o["phiB"], C.c_double), _np_ptr(o["sT"], C.c_double),
                                             _stream_ptr(stream)))
         return o
+
+    # ---- domain decomposition: halo lists and the step in phases (include/mrd.h "Domain decomposition") ----
+    PHASE_RESIDUAL1, PHASE_UPDATE1, PHASE_STAGE2, PHASE_END = 0, 1, 2, 3
+
+    def halo_set(self, send_idx, recv_idx):
+        si = np.ascontiguousarray(send_idx, dtype=np.int32)
+        ri = np.ascontiguousarray(recv_idx, dtype=np.int32)
+        _check(lib().mrd_halo_set(self._h, len(si), _np_ptr(si, C.c_int32), len(ri), _np_ptr(ri, C.c_int32)))
+        self.n_send, self.n_recv = len(si), len(ri)
+
+    def phase_begin(self, t_end=0.0, stream=None):
+        _check(lib().mrd_phase_begin(self._h, float(t_end), _stream_ptr(stream)))
+
+    def phase(self, k, stream=None):
+        _check(lib().mrd_phase(self._h, int(k), _stream_ptr(stream)))
+
+    def phase_end(self, stream=None):
+        n, t, dt = C.c_int64(0), C.c_double(0.0), C.c_double(0.0)
+        _check(lib().mrd_phase_end(self._h, _stream_ptr(stream), C.byref(n), C.byref(t), C.byref(dt)))
+        return n.value, t.value, dt.value
+
+    def _check_buf(self, buf, rows, dtype):
+        t = self._torch
+        assert isinstance(buf, t.Tensor) and buf.is_cuda and buf.dtype == dtype and buf.is_contiguous()
+        assert buf.numel() == rows, (buf.numel(), rows)
+
+    def dt_get(self, d, stream=None):
+        self._check_buf(d, 2, self._torch.float64)
+        _check(lib().mrd_dt_get(self._h, C.c_void_p(d.data_ptr()), _stream_ptr(stream)))
+
+    def dt_set(self, d, stream=None):
+        self._check_buf(d, 2, self._torch.float64)
+        _check(lib().mrd_dt_set(self._h, C.c_void_p(d.data_ptr()), _stream_ptr(stream)))
+
+    def halo_pack(self, buf, stream=None):
+        self._check_buf(buf, 4 * self.n_send, self.dtype)
+        _check(lib().mrd_halo_pack(self._h, C.c_void_p(buf.data_ptr()), _stream_ptr(stream)))
+
+    def halo_unpack(self, buf, stream=None):
+        self._check_buf(buf, 4 * self.n_recv, self.dtype)
+        _check(lib().mrd_halo_unpack(self._h, C.c_void_p(buf.data_ptr()), _stream_ptr(stream)))
 
     PROFILE_SLOTS = ("tri_stage1", "gather_dt", "wall1", "update", "tri_stage2", "wall2", "gather_update", "ctl")
 

@@ -82,6 +82,13 @@ struct mrd_mesh {
   bool graph_ok = false;
   bool has_state = false;
   int64_t steps_base = 0;         // completed steps at the last sync (for buffer parity)
+  // domain decomposition (include/mrd.h "Domain decomposition"): halo lists in INTERNAL vertex ids, phase stepping
+  int64_t n_send = 0, n_recv = 0;
+  int32_t *d_send_idx = nullptr, *d_recv_idx = nullptr;
+  bool in_phases = false;
+  int phase_a = 0;                // buffer pair holding W^n of the step in flight
+  int phase_next = 0;             // the phase expected next
+  int64_t phase_steps0 = 0;       // device step counter at mrd_phase_begin
 };
 
 namespace {
@@ -406,101 +413,90 @@ struct Prof {
 #define PROF_MARK(k) \
   if (prof) prof->mark((k), s);
 
-// one time step enqueued on s; `a` = buffer pair holding W^n
-template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_t s, Prof *prof = nullptr) {
+// one time step enqueued on s; `a` = buffer pair holding W^n.  `mask` selects phases (bit k = MRD_PHASE_k): the
+// whole step by default; mrd_phase enqueues them one at a time so that a caller can exchange in between.
+template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_t s, Prof *prof = nullptr, int mask = 15) {
   using V4 = mrd::Vec4<R>;
   const int b = a ^ 1;
   const bool rk2 = m->L.p.time_order == 2;
   auto md = mesh_dev<R>(m);
   const R gamma = (R)m->L.p.gamma;
-  switch (scheme) {
-    case MRD_SCHEME_N: launch_stage1<R, MRD_SCHEME_N>(m, rk2, a, s); break;
-    case MRD_SCHEME_LDA: launch_stage1<R, MRD_SCHEME_LDA>(m, rk2, a, s); break;
-    default: launch_stage1<R, MRD_SCHEME_B>(m, rk2, a, s); break;
-  }
-  PROF_MARK(MRD_PROF_TRI1)
   const unsigned vb = blocks_for(md.nv, 256);
-  if (m->fused) {
-    // fused path: dt from the partial s_T sums alone; the update kernels gather the residual partials themselves
-    auto td = tile_dev<R>(m);
-    mrd::slot_dt_kernel<R><<<std::min<unsigned>(vb, (unsigned)m->nsm * 8), 256, 0, s>>>(md, td, m->d_ctl, (const R *)m->d_partS);
+  const bool fused = m->fused;
+  if (mask & (1 << MRD_PHASE_RESIDUAL1)) {
+    switch (scheme) {
+      case MRD_SCHEME_N: launch_stage1<R, MRD_SCHEME_N>(m, rk2, a, s); break;
+      case MRD_SCHEME_LDA: launch_stage1<R, MRD_SCHEME_LDA>(m, rk2, a, s); break;
+      default: launch_stage1<R, MRD_SCHEME_B>(m, rk2, a, s); break;
+    }
+    PROF_MARK(MRD_PROF_TRI1)
+    if (fused) {
+      // fused path: dt from the partial s_T sums alone; the update kernels gather the residual partials themselves
+      mrd::slot_dt_kernel<R><<<std::min<unsigned>(vb, (unsigned)m->nsm * 8), 256, 0, s>>>(md, tile_dev<R>(m), m->d_ctl, (const R *)m->d_partS);
+    } else {
+      // unfused comparison path: per-triangle residuals through HBM, CSR gathers, acc round trip
+      mrd::gather_dt_kernel<R><<<vb, 256, 0, s>>>(md, m->d_ctl, (const V4 *)m->d_phi, (const R *)m->d_sT, (V4 *)m->d_acc);
+    }
     m->launches++;
     PROF_MARK(MRD_PROF_GATHER_DT)
     if (m->nwv > 0) {
-      mrd::wall_kernel<R, 1, true><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[a],
-                                                                        (V4 *)m->d_wall_acc);
+      if (fused)
+        mrd::wall_kernel<R, 1, true><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[a],
+                                                                          (V4 *)m->d_wall_acc);
+      else
+        mrd::wall_kernel<R, 1, false><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[a],
+                                                                           (V4 *)m->d_acc);
       m->launches++;
       PROF_MARK(MRD_PROF_WALL1)
     }
-    if (!rk2) {
-      mrd::slot_gather_update_kernel<R, 1><<<vb, 256, 0, s>>>(md, td, gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
-                                                           (const V4 *)m->d_W[a], (V4 *)m->d_W[b], sink_for<R>(m, b, true, false), m->d_flag);
-      m->launches++;
-      PROF_MARK(MRD_PROF_UPDATE)
+  }
+  if (mask & (1 << MRD_PHASE_UPDATE1)) {
+    if (fused) {
+      auto td = tile_dev<R>(m);
+      if (!rk2)
+        mrd::slot_gather_update_kernel<R, 1><<<vb, 256, 0, s>>>(md, td, gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
+                                                             (const V4 *)m->d_W[a], (V4 *)m->d_W[b], sink_for<R>(m, b, true, false), m->d_flag);
+      else
+        mrd::slot_gather_update_kernel<R, 0><<<vb, 256, 0, s>>>(md, td, gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
+                                                             (const V4 *)m->d_W[a], (V4 *)m->d_W[b], sink_for<R>(m, b, false, true), m->d_flag);
     } else {
-      mrd::slot_gather_update_kernel<R, 0><<<vb, 256, 0, s>>>(md, td, gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
-                                                           (const V4 *)m->d_W[a], (V4 *)m->d_W[b], sink_for<R>(m, b, false, true), m->d_flag);
+      if (!rk2)
+        mrd::update_kernel<R, true><<<vb, 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_acc, (V4 *)m->d_W[b],
+                                                    sink_for<R>(m, b, true, false), m->d_flag);
+      else
+        mrd::update_kernel<R, false><<<vb, 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_acc, (V4 *)m->d_W[b],
+                                                     sink_for<R>(m, b, false, true), m->d_flag);
+    }
+    m->launches++;
+    PROF_MARK(MRD_PROF_UPDATE)
+  }
+  if (rk2 && (mask & (1 << MRD_PHASE_STAGE2))) {
+    switch (scheme) {
+      case MRD_SCHEME_N: launch_stage2<R, MRD_SCHEME_N>(m, b, s); break;
+      case MRD_SCHEME_LDA: launch_stage2<R, MRD_SCHEME_LDA>(m, b, s); break;
+      default: launch_stage2<R, MRD_SCHEME_B>(m, b, s); break;
+    }
+    PROF_MARK(MRD_PROF_TRI2)
+    if (m->nwv > 0) {
+      mrd::wall_kernel<R, 2><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[b],
+                                                                  (V4 *)m->d_wall_acc);
       m->launches++;
-      PROF_MARK(MRD_PROF_UPDATE)
-      switch (scheme) {
-        case MRD_SCHEME_N: launch_stage2<R, MRD_SCHEME_N>(m, b, s); break;
-        case MRD_SCHEME_LDA: launch_stage2<R, MRD_SCHEME_LDA>(m, b, s); break;
-        default: launch_stage2<R, MRD_SCHEME_B>(m, b, s); break;
-      }
-      PROF_MARK(MRD_PROF_TRI2)
-      if (m->nwv > 0) {
-        mrd::wall_kernel<R, 2><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[b],
-                                                                    (V4 *)m->d_wall_acc);
-        m->launches++;
-        PROF_MARK(MRD_PROF_WALL2)
-      }
-      mrd::slot_gather_update_kernel<R, 2><<<vb, 256, 0, s>>>(md, td, gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
+      PROF_MARK(MRD_PROF_WALL2)
+    }
+    if (fused)
+      mrd::slot_gather_update_kernel<R, 2><<<vb, 256, 0, s>>>(md, tile_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
                                                            (const V4 *)m->d_W[b], (V4 *)m->d_W[b], sink_for<R>(m, b, true, false), m->d_flag);
-      m->launches++;
-      PROF_MARK(MRD_PROF_GATHER_UPDATE)
-    }
-  } else {
-    // unfused comparison path: per-triangle residuals through HBM, CSR gathers, acc round trip
-    mrd::gather_dt_kernel<R><<<vb, 256, 0, s>>>(md, m->d_ctl, (const V4 *)m->d_phi, (const R *)m->d_sT, (V4 *)m->d_acc);
-    m->launches++;
-    PROF_MARK(MRD_PROF_GATHER_DT)
-    if (m->nwv > 0) {
-      mrd::wall_kernel<R, 1, false><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[a],
-                                                                         (V4 *)m->d_acc);
-      m->launches++;
-      PROF_MARK(MRD_PROF_WALL1)
-    }
-    if (!rk2) {
-      mrd::update_kernel<R, true><<<vb, 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_acc, (V4 *)m->d_W[b],
-                                                  sink_for<R>(m, b, true, false), m->d_flag);
-      m->launches++;
-      PROF_MARK(MRD_PROF_UPDATE)
-    } else {
-      mrd::update_kernel<R, false><<<vb, 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_acc, (V4 *)m->d_W[b],
-                                                   sink_for<R>(m, b, false, true), m->d_flag);
-      m->launches++;
-      PROF_MARK(MRD_PROF_UPDATE)
-      switch (scheme) {
-        case MRD_SCHEME_N: launch_stage2<R, MRD_SCHEME_N>(m, b, s); break;
-        case MRD_SCHEME_LDA: launch_stage2<R, MRD_SCHEME_LDA>(m, b, s); break;
-        default: launch_stage2<R, MRD_SCHEME_B>(m, b, s); break;
-      }
-      PROF_MARK(MRD_PROF_TRI2)
-      if (m->nwv > 0) {
-        mrd::wall_kernel<R, 2><<<blocks_for(m->nwv, 128), 128, 0, s>>>(wall_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_W[a], (const V4 *)m->d_W[b],
-                                                                    (V4 *)m->d_wall_acc);
-        m->launches++;
-        PROF_MARK(MRD_PROF_WALL2)
-      }
+    else
       mrd::gather_update_kernel<R><<<vb, 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_phi, (const V4 *)m->d_wall_acc, (V4 *)m->d_W[b],
                                                    sink_for<R>(m, b, true, false), m->d_flag);
-      m->launches++;
-      PROF_MARK(MRD_PROF_GATHER_UPDATE)
-    }
+    m->launches++;
+    PROF_MARK(MRD_PROF_GATHER_UPDATE)
   }
-  mrd::ctl_kernel<<<1, 1, 0, s>>>(m->d_ctl, 1, 0.0, m->d_flag);
-  m->launches++;
-  PROF_MARK(MRD_PROF_CTL)
+  if (mask & (1 << MRD_PHASE_END)) {
+    mrd::ctl_kernel<<<1, 1, 0, s>>>(m->d_ctl, 1, 0.0, m->d_flag);
+    m->launches++;
+    PROF_MARK(MRD_PROF_CTL)
+  }
 }
 
 // n consecutive steps starting from buffer pair `a` (updated).  Small meshes replay a captured two-step graph.
@@ -558,6 +554,7 @@ template <class R> int step_impl(mrd_mesh *m, int64_t max_steps, double t_end, c
                                  int64_t *steps_done, double *t, double *dt_last) {
   if (!m->has_state) return fail(MRD_EINVAL, "no state set");
   if (max_steps < 0) return fail(MRD_EINVAL, "max_steps < 0");
+  if (m->in_phases) return fail(MRD_EINVAL, "mrd_step inside mrd_phase_begin / mrd_phase_end");
   mrd::Ctl c{};
   int rc;
   // steps enqueued by earlier async calls change the parity: settle it first
@@ -603,9 +600,43 @@ template <class R> int step_impl(mrd_mesh *m, int64_t max_steps, double t_end, c
   return MRD_OK;
 }
 
+// ---- phase stepping and halo exchange (include/mrd.h "Domain decomposition") --------------------------------
+template <class R> int phase_impl(mrd_mesh *m, int phase, cudaStream_t s) {
+  enqueue_step<R>(m, m->L.p.scheme, m->phase_a, s, nullptr, 1 << phase);
+  CUDA_TRY(cudaGetLastError());
+  return MRD_OK;
+}
+template <class R> int halo_pack_impl(mrd_mesh *m, void *buf, cudaStream_t s) {
+  using V4 = mrd::Vec4<R>;
+  if (m->n_send > 0) {
+    mrd::halo_pack_kernel<R><<<blocks_for(m->n_send, 256), 256, 0, s>>>(m->n_send, m->d_send_idx, m->d_ctl, (const V4 *)m->d_W[m->phase_a ^ 1], (V4 *)buf);
+    m->launches++;
+    CUDA_TRY(cudaGetLastError());
+  }
+  return MRD_OK;
+}
+template <class R> int halo_unpack_impl(mrd_mesh *m, const void *buf, cudaStream_t s) {
+  using V4 = mrd::Vec4<R>;
+  if (m->n_recv == 0) return MRD_OK;
+  const int a = m->phase_a, b = a ^ 1;
+  const R gamma = (R)m->L.p.gamma;
+  const unsigned nb = blocks_for(m->n_recv, 256);
+  // after UPDATE1 of RK2 the buffer holds W*; otherwise W^{n+1}
+  const bool first = m->L.p.time_order == 2 && m->phase_next == MRD_PHASE_STAGE2;
+  if (first)
+    mrd::halo_unpack_kernel<R, true><<<nb, 256, 0, s>>>(m->n_recv, m->d_recv_idx, gamma, m->d_ctl, (const V4 *)buf, (const V4 *)m->d_W[a], (V4 *)m->d_W[b],
+                                                      sink_for<R>(m, b, false, true), m->d_flag);
+  else
+    mrd::halo_unpack_kernel<R, false><<<nb, 256, 0, s>>>(m->n_recv, m->d_recv_idx, gamma, m->d_ctl, (const V4 *)buf, (const V4 *)m->d_W[a], (V4 *)m->d_W[b],
+                                                       sink_for<R>(m, b, true, false), m->d_flag);
+  m->launches++;
+  CUDA_TRY(cudaGetLastError());
+  return MRD_OK;
+}
+
 template <class R> int diag_impl(mrd_mesh *m, double totals[4], double *min_rho, double *min_p, cudaStream_t s) {
   using V4 = mrd::Vec4<R>;
-  mrd::diag_kernel<R><<<DIAG_BLOCKS, 256, 0, s>>>(m->L.nv, (R)m->L.p.gamma, (const V4 *)m->d_W[m->cur], (const R *)m->d_vol, m->d_diag);
+  mrd::diag_kernel<R><<<DIAG_BLOCKS, 256, 0, s>>>(m->L.nv, (R)m->L.p.gamma, (const V4 *)m->d_W[m->cur], (const R *)m->d_vol, m->d_frozen, m->d_diag);
   m->launches++;
   std::vector<double> h(DIAG_BLOCKS * 6);
   CUDA_TRY(cudaMemcpyAsync(h.data(), m->d_diag, h.size() * sizeof(double), cudaMemcpyDeviceToHost, s));
@@ -979,6 +1010,144 @@ int mrd_step_profile(mrd_mesh *m, void *stream, float ms[MRD_PROFILE_SLOTS]) {
   if (rc) return rc;
   if (c.status) return fail(MRD_ENONPHYSICAL, "non-physical state met in the profiled step");
   return MRD_OK;
+}
+
+int mrd_partition_create(mrd_partition **out, int64_t nv, const double *xy, int64_t nt, const int32_t *tri,
+                         const uint8_t *vertex_flag, int64_t ne, const int32_t *wall_edge, double period_x, double period_y,
+                         int32_t n_part, int32_t part) {
+  if (!out) return fail(MRD_EINVAL, "null output pointer");
+  mrd_partition *P = new (std::nothrow) mrd_partition();
+  if (!P) return fail(MRD_ENOMEM, "out of memory");
+  std::string err;
+  int rc;
+  try {
+    rc = mrd_host::partition_build(*P, nv, xy, nt, tri, vertex_flag, ne, wall_edge, period_x, period_y, n_part, part, err);
+  } catch (const std::bad_alloc &) {
+    rc = MRD_ENOMEM;
+    err = "out of host memory in the partitioner";
+  }
+  if (rc) { delete P; return fail(rc, err); }
+  *out = P;
+  return MRD_OK;
+}
+void mrd_partition_destroy(mrd_partition *p) { delete p; }
+int mrd_partition_sizes(const mrd_partition *p, int64_t n[8]) {
+  if (!p || !n) return fail(MRD_EINVAL, "null argument");
+  return mrd_host::partition_sizes(*p, n);
+}
+int mrd_partition_get(const mrd_partition *p, const char *name, void *dst, int64_t bytes) {
+  if (!p) return fail(MRD_EINVAL, "null argument");
+  std::string err;
+  int rc = mrd_host::partition_get(*p, name, dst, bytes, err);
+  return rc ? fail(rc, err) : MRD_OK;
+}
+
+int mrd_halo_set(mrd_mesh *m, int64_t n_send, const int32_t *send_idx, int64_t n_recv, const int32_t *recv_idx) {
+  if (!m || n_send < 0 || n_recv < 0 || (n_send > 0 && !send_idx) || (n_recv > 0 && !recv_idx)) return fail(MRD_EINVAL, "bad halo lists");
+  if (m->in_phases) return fail(MRD_EINVAL, "mrd_halo_set inside mrd_phase_begin / mrd_phase_end");
+  const int64_t nv = m->L.nv;
+  std::vector<int32_t> si((size_t)n_send), ri((size_t)n_recv);
+  for (int64_t k = 0; k < n_send; ++k) {
+    if (send_idx[k] < 0 || send_idx[k] >= nv) return fail(MRD_EINVAL, "halo send index out of range");
+    si[k] = m->L.vrank[send_idx[k]];
+    if (m->L.frozen[si[k]] == 2) return fail(MRD_EINVAL, "halo send list names a halo vertex");
+  }
+  for (int64_t k = 0; k < n_recv; ++k) {
+    if (recv_idx[k] < 0 || recv_idx[k] >= nv) return fail(MRD_EINVAL, "halo receive index out of range");
+    ri[k] = m->L.vrank[recv_idx[k]];
+    if (m->L.frozen[ri[k]] != 2) return fail(MRD_EINVAL, "halo receive list names a vertex that is not flagged 2 (halo)");
+  }
+  int rc;
+  if ((rc = dev_upload(m, &m->d_send_idx, si.data(), n_send))) return rc;
+  if ((rc = dev_upload(m, &m->d_recv_idx, ri.data(), n_recv))) return rc;
+  m->n_send = n_send;
+  m->n_recv = n_recv;
+  return MRD_OK;
+}
+
+int mrd_phase_begin(mrd_mesh *m, double t_end, void *stream) {
+  if (!m) return fail(MRD_EINVAL, "null argument");
+  if (!m->has_state) return fail(MRD_EINVAL, "no state set");
+  if (m->in_phases) return fail(MRD_EINVAL, "mrd_phase_begin called twice");
+  cudaStream_t s = (cudaStream_t)stream;
+  mrd::Ctl c{};
+  int rc = fetch_ctl(m, s, &c);
+  if (rc) return rc;
+  if (c.status) return fail(MRD_ENONPHYSICAL, "state is non-physical (an earlier step failed)");
+  mrd::ctl_kernel<<<1, 1, 0, s>>>(m->d_ctl, 0, t_end > 0.0 ? t_end : 0.0, m->d_flag);
+  m->launches++;
+  CUDA_TRY(cudaGetLastError());
+  m->in_phases = true;
+  m->phase_a = m->cur;
+  m->phase_next = MRD_PHASE_RESIDUAL1;
+  m->phase_steps0 = c.steps;
+  return MRD_OK;
+}
+
+int mrd_phase(mrd_mesh *m, int32_t phase, void *stream) {
+  if (!m) return fail(MRD_EINVAL, "null argument");
+  if (!m->in_phases) return fail(MRD_EINVAL, "mrd_phase outside mrd_phase_begin / mrd_phase_end");
+  if (phase != m->phase_next) return fail(MRD_EINVAL, "phases out of order (RESIDUAL1, UPDATE1, [STAGE2], END)");
+  cudaStream_t s = (cudaStream_t)stream;
+  int rc = m->L.p.precision == MRD_FP64 ? phase_impl<double>(m, phase, s) : phase_impl<float>(m, phase, s);
+  if (rc) return rc;
+  if (phase == MRD_PHASE_END) {
+    m->phase_a ^= 1;
+    m->phase_next = MRD_PHASE_RESIDUAL1;
+  } else if (phase == MRD_PHASE_UPDATE1 && m->L.p.time_order == 1) {
+    m->phase_next = MRD_PHASE_END;
+  } else {
+    m->phase_next = phase + 1;
+  }
+  return MRD_OK;
+}
+
+int mrd_phase_end(mrd_mesh *m, void *stream, int64_t *steps_done, double *t, double *dt_last) {
+  if (!m) return fail(MRD_EINVAL, "null argument");
+  if (!m->in_phases) return fail(MRD_EINVAL, "mrd_phase_end without mrd_phase_begin");
+  if (m->phase_next != MRD_PHASE_RESIDUAL1) return fail(MRD_EINVAL, "mrd_phase_end in the middle of a step");
+  m->in_phases = false;
+  cudaStream_t s = (cudaStream_t)stream;
+  mrd::Ctl c{};
+  int rc = fetch_ctl(m, s, &c);
+  if (rc) return rc;
+  if (steps_done) *steps_done = c.steps - m->phase_steps0;
+  if (t) *t = c.t;
+  if (dt_last) *dt_last = c.dt;
+  if (c.status) return fail(MRD_ENONPHYSICAL, "non-physical state (rho <= 0, p <= 0 or c^2 <= 0) met by some part; set the state again");
+  return MRD_OK;
+}
+
+int mrd_dt_get(mrd_mesh *m, double *d_dev, void *stream) {
+  if (!m || !d_dev) return fail(MRD_EINVAL, "null argument");
+  if (!m->in_phases || m->phase_next != MRD_PHASE_UPDATE1) return fail(MRD_EINVAL, "mrd_dt_get must follow mrd_phase(RESIDUAL1)");
+  mrd::dt_get_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(m->d_ctl, m->d_flag, d_dev);
+  m->launches++;
+  CUDA_TRY(cudaGetLastError());
+  return MRD_OK;
+}
+int mrd_dt_set(mrd_mesh *m, const double *d_dev, void *stream) {
+  if (!m || !d_dev) return fail(MRD_EINVAL, "null argument");
+  if (!m->in_phases || m->phase_next != MRD_PHASE_UPDATE1) return fail(MRD_EINVAL, "mrd_dt_set must follow mrd_phase(RESIDUAL1)");
+  mrd::dt_set_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(m->d_ctl, m->d_flag, d_dev);
+  m->launches++;
+  CUDA_TRY(cudaGetLastError());
+  return MRD_OK;
+}
+
+int mrd_halo_pack(mrd_mesh *m, void *buf_dev, void *stream) {
+  if (!m || (m->n_send > 0 && !buf_dev)) return fail(MRD_EINVAL, "null argument");
+  if (!m->in_phases || (m->phase_next != MRD_PHASE_STAGE2 && m->phase_next != MRD_PHASE_END))
+    return fail(MRD_EINVAL, "mrd_halo_pack must follow mrd_phase(UPDATE1) or mrd_phase(STAGE2)");
+  cudaStream_t s = (cudaStream_t)stream;
+  return m->L.p.precision == MRD_FP64 ? halo_pack_impl<double>(m, buf_dev, s) : halo_pack_impl<float>(m, buf_dev, s);
+}
+int mrd_halo_unpack(mrd_mesh *m, const void *buf_dev, void *stream) {
+  if (!m || (m->n_recv > 0 && !buf_dev)) return fail(MRD_EINVAL, "null argument");
+  if (!m->in_phases || (m->phase_next != MRD_PHASE_STAGE2 && m->phase_next != MRD_PHASE_END))
+    return fail(MRD_EINVAL, "mrd_halo_unpack must follow mrd_phase(UPDATE1) or mrd_phase(STAGE2)");
+  cudaStream_t s = (cudaStream_t)stream;
+  return m->L.p.precision == MRD_FP64 ? halo_unpack_impl<double>(m, buf_dev, s) : halo_unpack_impl<float>(m, buf_dev, s);
 }
 
 int mrd_launch_count(const mrd_mesh *m, int64_t *launches) {

@@ -277,7 +277,7 @@ gather_dt_kernel(MeshDev<R> m, Ctl *__restrict__ ctl, const Vec4<R> *__restrict_
       S += __ldg(sT + e / 3);
     }
     st4(&acc[i], Vec4<R>{a0, a1, a2, a3});
-    d = 2.0 * (double)__ldg(m.vol + i) / (double)S;
+    if (!(m.frozen && m.frozen[i] == 2)) d = 2.0 * (double)__ldg(m.vol + i) / (double)S;  // halo: fan incomplete here
   }
   block_min_to_global(d, &ctl->dmin_bits);
 }
@@ -410,11 +410,12 @@ __global__ void wall_kernel(WallDev<R> wd, R gamma, const Ctl *__restrict__ ctl,
 // ---------------------------------------------------------------------------------------------
 template <class R>
 __global__ void __launch_bounds__(256)
-diag_kernel(int64_t nv, R gamma, const Vec4<R> *__restrict__ W, const R *__restrict__ vol, double *__restrict__ partial) {
+diag_kernel(int64_t nv, R gamma, const Vec4<R> *__restrict__ W, const R *__restrict__ vol, const uint8_t *__restrict__ flag,
+            double *__restrict__ partial) {
   double s[4] = {0, 0, 0, 0}, mr = __longlong_as_double(0x7FF0000000000000ll), mp = mr;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nv; i += (int64_t)gridDim.x * blockDim.x) {
     Vec4<R> w = ld4(&W[i]);
-    double V = (double)vol[i];
+    double V = (flag && flag[i] == 2) ? 0.0 : (double)vol[i];  // a halo vertex is counted by the part that owns it
     s[0] += V * (double)w.x; s[1] += V * (double)w.y; s[2] += V * (double)w.z; s[3] += V * (double)w.w;
     double p = ((double)gamma - 1.0) * ((double)w.w - 0.5 * ((double)w.y * (double)w.y + (double)w.z * (double)w.z) / (double)w.x);
     mr = fmin(mr, (double)w.x);
@@ -434,6 +435,52 @@ diag_kernel(int64_t nv, R gamma, const Vec4<R> *__restrict__ W, const R *__restr
     __syncthreads();
   }
   if (tid < 6) partial[blockIdx.x * 6 + tid] = sh[0][tid];
+}
+
+// ---------------------------------------------------------------------------------------------
+// Domain decomposition (include/mrd.h "Domain decomposition"): halo pack / unpack, dt exchange
+// ---------------------------------------------------------------------------------------------
+template <class R>
+__global__ void halo_pack_kernel(int64_t n, const int32_t *__restrict__ idx, const Ctl *__restrict__ ctl,
+                                 const Vec4<R> *__restrict__ W, Vec4<R> *__restrict__ buf) {
+  MRD_CTL_GUARD(ctl)
+  int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < n) st4(&buf[k], ld4(&W[idx[k]]));
+}
+
+// FIRST: after stage 1 of RK2 (the owner's W*; Z* and dW/dt = (W* - W^n)/dt to the slots, as vertex_finish<.., true>);
+// else the owner's W^{n+1} (Z and |v| + c to the slots)
+template <class R, bool FIRST>
+__global__ void halo_unpack_kernel(int64_t n, const int32_t *__restrict__ idx, R gamma, const Ctl *__restrict__ ctl,
+                                   const Vec4<R> *__restrict__ buf, const Vec4<R> *__restrict__ Wold,
+                                   Vec4<R> *__restrict__ Wout, VertexSink<R> sink, int *status) {
+  MRD_CTL_GUARD(ctl)
+  int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  const int64_t i = idx[k];
+  Vec4<R> w = ld4(&buf[k]);
+  Vec4<R> z;
+  R s, p;
+  bool ok = vertex_prepare(gamma, w, z, s, p);
+  if (!ok) atomicOr(status, 1);
+  Vec4<R> d{0, 0, 0, 0};
+  if (FIRST) {
+    Vec4<R> o = ld4(&Wold[i]);
+    R idt = Fast<R>::rcp((R)ctl_dt(ctl));
+    d = Vec4<R>{(w.x - o.x) * idt, (w.y - o.y) * idt, (w.z - o.z) * idt, (w.w - o.w) * idt};
+  }
+  st4(&Wout[i], w);
+  sink.put(i, z, s, FIRST, d);
+}
+
+// d[0] = local min of 2 V_i / sum s_T (eq. 44), d[1] = -1 if a kernel of this part met a non-physical state
+__global__ void dt_get_kernel(const Ctl *__restrict__ c, const int *__restrict__ flag, double *__restrict__ d) {
+  d[0] = __longlong_as_double((long long)c->dmin_bits);
+  d[1] = (*flag || c->status) ? -1.0 : 0.0;
+}
+__global__ void dt_set_kernel(Ctl *__restrict__ c, int *__restrict__ flag, const double *__restrict__ d) {
+  c->dmin_bits = (unsigned long long)__double_as_longlong(d[0]);
+  if (d[1] < 0.0) *flag = 1;
 }
 
 // ---------------------------------------------------------------------------------------------

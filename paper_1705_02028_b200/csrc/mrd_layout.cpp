@@ -70,6 +70,33 @@ namespace mrd_host {
 
 static void build_tile_plan(mrd_layout &L, const std::vector<double> &xyi);
 
+// frame of the Morton keys: the bounding box (the period where periodic), one common scale for both axes so that the
+// curve's cells stay square
+static void morton_frame(int64_t nv, const double *xy, const double period[2], double lo[2], double inv[2]) {
+  double hi[2] = {xy[0], xy[1]};
+  lo[0] = xy[0]; lo[1] = xy[1];
+  for (int64_t i = 0; i < nv; ++i)
+    for (int d = 0; d < 2; ++d) {
+      lo[d] = std::min(lo[d], xy[2 * i + d]);
+      hi[d] = std::max(hi[d], xy[2 * i + d]);
+    }
+  for (int d = 0; d < 2; ++d)
+    if (period[d] > 0.0) { lo[d] = 0.0; hi[d] = period[d]; }
+  double ext = std::max(hi[0] - lo[0], hi[1] - lo[1]);
+  inv[0] = inv[1] = ext > 0 ? 1.0 / ext : 0.0;
+}
+
+void morton_order_vertices(int64_t nv, const double *xy, const double period[2], std::vector<int32_t> &perm) {
+  double lo[2], inv[2];
+  morton_frame(nv, xy, period, lo, inv);
+  std::vector<uint64_t> key(nv);
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < nv; ++i) key[i] = morton_key(xy[2 * i], xy[2 * i + 1], lo, inv);
+  perm.resize(nv);
+  std::iota(perm.begin(), perm.end(), 0);
+  radix_sort(key, perm);
+}
+
 int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *xy, int64_t nt,
                  const int32_t *tri, const uint8_t *vertex_flag, int64_t ne, const int32_t *wall_edge,
                  std::string &err) {
@@ -111,17 +138,8 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
   std::iota(L.vperm.begin(), L.vperm.end(), 0);
   std::iota(L.tperm.begin(), L.tperm.end(), 0);
   if (p->reorder) {
-    double lo[2] = {xy[0], xy[1]}, hi[2] = {xy[0], xy[1]};
-    for (int64_t i = 0; i < nv; ++i)
-      for (int d = 0; d < 2; ++d) {
-        lo[d] = std::min(lo[d], xy[2 * i + d]);
-        hi[d] = std::max(hi[d], xy[2 * i + d]);
-      }
-    for (int d = 0; d < 2; ++d)
-      if (period[d] > 0.0) { lo[d] = 0.0; hi[d] = period[d]; }
-    // one common scale for both axes keeps the curve's cells square
-    double ext = std::max(hi[0] - lo[0], hi[1] - lo[1]);
-    double inv[2] = {ext > 0 ? 1.0 / ext : 0.0, ext > 0 ? 1.0 / ext : 0.0};
+    double lo[2], inv[2];
+    morton_frame(nv, xy, period, lo, inv);
     std::vector<uint64_t> key(nv);
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < nv; ++i) key[i] = morton_key(xy[2 * i], xy[2 * i + 1], lo, inv);
@@ -195,8 +213,9 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
   L.nf = 0;
   if (vertex_flag)
     for (int64_t k = 0; k < nv; ++k) {
-      L.frozen[k] = vertex_flag[L.vperm[k]] ? 1 : 0;
-      L.nf += L.frozen[k];
+      L.frozen[k] = vertex_flag[L.vperm[k]];  // 1 = frozen (L582), 2 = halo vertex of a partition
+      if (L.frozen[k] > 2) { err = "vertex_flag must be 0, 1 or 2"; return MRD_EINVAL; }
+      L.nf += L.frozen[k] != 0;
     }
 
   // ---- reflecting-wall edges (L586-L602; outward normal, reading C15) ------------------------------

@@ -49,8 +49,28 @@ struct mrd_layout {
   std::vector<double> shape_geom;       // [nshape][12]
 };
 
+// one part of a domain decomposition (mrd_partition.cpp; include/mrd.h "Domain decomposition")
+struct mrd_partition {
+  int64_t nv_g = 0, nt_g = 0, n_owned = 0;
+  int32_t n_part = 1, part = 0;
+  std::vector<int32_t> owner;          // [nv_g]
+  std::vector<int32_t> vertex_global;  // local -> global: owned (ascending), then halo (ascending)
+  std::vector<double> xy;
+  std::vector<int32_t> tri, tri_global;
+  std::vector<uint8_t> flag;
+  std::vector<int32_t> wall;
+  std::vector<int32_t> nbr, send_off, send_idx, recv_off, recv_idx;
+};
+
 namespace mrd_host {
 int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *xy, int64_t nt,
                  const int32_t *tri, const uint8_t *vertex_flag, int64_t ne, const int32_t *wall_edge,
                  std::string &err);
+// vertex ids in ascending Morton key (stable), the order the layout stage and the partitioner share
+void morton_order_vertices(int64_t nv, const double *xy, const double period[2], std::vector<int32_t> &perm);
+int partition_build(mrd_partition &P, int64_t nv, const double *xy, int64_t nt, const int32_t *tri,
+                    const uint8_t *vertex_flag, int64_t ne, const int32_t *wall_edge, double period_x, double period_y,
+                    int32_t n_part, int32_t part, std::string &err);
+int partition_sizes(const mrd_partition &P, int64_t n[8]);
+int partition_get(const mrd_partition &P, const char *name, void *dst, int64_t bytes, std::string &err);
 }

@@ -359,6 +359,7 @@ slot_dt_kernel(MeshDev<R> m, TileDev<R> td, Ctl *__restrict__ ctl, const R *__re
   // serialise in L2 and took longer than the gather itself)
   double d = __longlong_as_double(0x7FF0000000000000ll);
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m.nv; i += (int64_t)gridDim.x * blockDim.x) {
+    if (m.frozen && m.frozen[i] == 2) continue;  // halo vertex of a partition: its fan is incomplete here
     R S = 0;
     const int32_t q0 = __ldg(td.vslot_off + i), q1 = __ldg(td.vslot_off + i + 1);
     for (int32_t q = q0; q < q1; ++q) S += __ldg(partS + __ldg(td.vslot_ent + q));

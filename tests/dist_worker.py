@@ -1,0 +1,66 @@
+"""Worker of tests/test_gpu_distributed.py: one rank of a `DistributedMesh` run, launched by torch.distributed.run
+with the gloo backend.  All ranks share cuda:0 (the box has one GPU; the halo rows are staged through host memory,
+no kernel waits on another rank's kernel).  Rank 0 writes the gathered results to --out (npz)."""
+import argparse
+import os
+import sys
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+
+def cases():
+    """name -> (mesh, W0, vertex_flag, wall_edge, params, steps, t_end); the test rebuilds the same inputs."""
+    out = {}
+    m = wl.uniform_mesh(48, 48, 10.0, 10.0, periodic=True)
+    out["vortex_b2"] = (m, wl.vortex_state(m), None, None, dict(scheme=2, time_order=2), 20, 0.0)
+    out["vortex_b2_fp32"] = (m, wl.vortex_state(m), None, None, dict(scheme=2, time_order=2, precision=1), 10, 0.0)
+    out["vortex_b2_unfused"] = (m, wl.vortex_state(m), None, None, dict(scheme=2, time_order=2, tile=-1), 5, 0.0)
+    c = wl.make_config("sod", n=64)
+    out["sod_walls_tend"] = (c.mesh, c.W0, c.vertex_flag, c.wall_edge, dict(scheme=2, time_order=2), 200, 0.02)
+    k = wl.make_config("kh", n=40, numbering="permuted")
+    out["kh_permuted_n1"] = (k.mesh, k.W0, None, None, dict(scheme=0, time_order=1), 8, 0.0)
+    j = wl.jitter_mesh(wl.uniform_mesh(33, 27, 1.0, 1.0, periodic=True), 0.2, seed=11)
+    out["jitter_lda2"] = (j, wl.random_smooth_state(j, mach=0.5, seed=4), None, None,
+                          dict(scheme=1, time_order=2, reorder=False, tile=64), 10, 0.0)
+    r = wl.make_config("riemann4", n=40)
+    out["riemann4_frozen"] = (r.mesh, r.W0, r.vertex_flag, None, dict(scheme=2, time_order=2), 6, 0.0)
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--out", required=True)
+    args = ap.parse_args()
+    import torch
+    import torch.distributed as dist
+    from paper_1705_02028_b200.distributed import DistributedMesh
+    torch.cuda.set_device(0)
+    dist.init_process_group("gloo")
+    rank = dist.get_rank()
+    res = {}
+    for name, (mesh, W0, flag, wall, params, steps, t_end) in cases().items():
+        dm = DistributedMesh(mesh.xy, mesh.tri, vertex_flag=flag, wall_edge=wall, period=mesh.period, **params)
+        dm.set_state(W0)
+        n1, t1, dt1 = dm.step(1)
+        W1 = dm.get_state()
+        n, t, dt = dm.step(steps - 1, t_end)
+        W = dm.get_state()
+        tot, mr, mp = dm.diagnostics()
+        res[name + "/W1"] = W1
+        res[name + "/W"] = W
+        res[name + "/scalars"] = np.array([n1, t1, dt1, n, t, dt, mr, mp, dm.part.n_owned, dm.part.n_recv, dm.launch_count()], dtype=np.float64)
+        res[name + "/totals"] = tot
+        dm.close()
+    dist.barrier()
+    if rank == 0:
+        np.savez(args.out, **res)
+    dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,77 @@
+"""The N > 1 path on the GPU: a `DistributedMesh` over 2 and 3 ranks (separate processes, gloo backend, all
+on the one GPU of the box, halo rows staged through host memory) against the CPU oracle on the WHOLE mesh, element
+by element, and against the single-mesh run of the same library (they differ by summation order only).
+Tolerances as tests/test_gpu_parity.py."""
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+import oracle
+from dist_worker import cases
+from helpers import field_errors
+
+pytestmark = pytest.mark.gpu
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _run(world, tmp_path):
+    out = str(tmp_path / f"dist_{world}.npz")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world), "--master-addr", "127.0.0.1",
+           "--master-port", str(29700 + os.getpid() % 200 + world), os.path.join(ROOT, "tests", "dist_worker.py"), "--out", out]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=1500, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-3000:]
+    return np.load(out)
+
+
+@pytest.fixture(scope="module")
+def single():
+    """The same cases on one mesh: oracle and single-GPU library results."""
+    import torch
+    import paper_1705_02028_b200 as mrd
+    ref = {}
+    for name, (mesh, W0, flag, wall, params, steps, t_end) in cases().items():
+        fp32 = params.get("precision", 0) == 1
+        gm = mrd.Mesh(mesh.xy, mesh.tri, vertex_flag=flag, wall_edge=wall, period=mesh.period, **params)
+        gm.set_state(torch.tensor(np.ascontiguousarray(W0), dtype=torch.float32 if fp32 else torch.float64, device="cuda"))
+        g1 = gm.step(1)
+        G1 = gm.get_state().cpu().numpy()
+        g = gm.step(steps - 1, t_end)
+        G = gm.get_state().cpu().numpy()
+        gtot = gm.diagnostics()
+        om = oracle.OracleMesh(mesh.xy, mesh.tri, period=mesh.period, vertex_flag=flag, wall_edge=wall,
+                               scheme=params["scheme"], time_order=params["time_order"])
+        om.set_state(W0)
+        o1 = om.step(1)
+        O1 = om.get_state().copy()
+        o = om.step(steps - 1, t_end)
+        O = om.get_state().copy()
+        ref[name] = dict(g1=g1, G1=G1, g=g, G=G, gtot=gtot, o1=o1, O1=O1, o=o, O=O, fp32=fp32, nv=mesh.nv)
+    return ref
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_distributed_mesh_matches_oracle_and_single_mesh(world, single, tmp_path):
+    res = _run(world, tmp_path)
+    for name, ref in single.items():
+        W1, W, sc, tot = res[name + "/W1"], res[name + "/W"], res[name + "/scalars"], res[name + "/totals"]
+        n1, t1, dt1, n, t, dt, mr, mp, n_owned, n_recv, launches = sc
+        tol1, toln = (1e-5, 1e-5) if ref["fp32"] else (1e-12, 1e-9)
+        # the oracle on the whole mesh
+        assert n1 == 1 and n == ref["o"][0], name
+        assert abs(dt1 - ref["o1"][2]) <= (1e-6 if ref["fp32"] else 1e-14) * ref["o1"][2], name
+        assert field_errors(W1, ref["O1"]) <= tol1, name
+        assert field_errors(W, ref["O"]) <= toln, name
+        assert abs(t - ref["o"][1]) <= (1e-5 if ref["fp32"] else 1e-11) * max(1.0, abs(t)), name
+        # the single-mesh run of the library: same step count, time step and state up to summation order
+        assert n == ref["g"][0] and abs(dt - ref["g"][2]) <= (1e-5 if ref["fp32"] else 1e-12) * dt, name
+        assert field_errors(W1, ref["G1"]) <= (1e-6 if ref["fp32"] else 1e-13), name
+        gt, gmr, gmp = ref["gtot"]
+        scale = np.abs(gt).max()
+        assert np.abs(tot - gt).max() <= (1e-5 if ref["fp32"] else 1e-11) * scale, name   # halo vertices are not double counted
+        assert abs(mr - gmr) <= 1e-5 * abs(gmr) and abs(mp - gmp) <= 1e-4 * abs(gmp), name
+        # the work really was split and exchanged, and ran in this library's kernels
+        assert 0 < n_owned < ref["nv"] and n_recv > 0 and launches > 0, name
