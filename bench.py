@@ -7,7 +7,9 @@
 A "step" is one RK2 time step of scheme B (both stages, dt reduction included) over the whole mesh:
 config 5 of BASELINE.json at its largest size (isentropic vortex on a periodic uniform triangulation of
 4096^2 vertices, 33.5M triangles, Morton-ordered input).  Prints ONE JSON line (rank 0).
-N > 1: one independent replica per GPU ("replicas only"), launched by torchrun.
+N > 1 (launched by torchrun, one process per GPU): ONE mesh -- N copies of that workload stacked in y -- spread over
+the N GPUs by the domain decomposition of DESIGN.md section 9 (halo exchange per stage + one min-reduction per step over
+NCCL); `--decomposition replicas` runs N independent replicas instead.
 `--impl reference` times the CPU oracle (oracle/), as it stands, on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -123,7 +125,7 @@ def max_over_ranks(value: float, dist, device) -> float:
 
 
 def whole_job_rate(world: int, units_per_rank: int, steps: int, seconds: float) -> float:
-    """Weak scaling: every rank steps its own replica; value = all units processed / max-over-ranks time."""
+    """Weak scaling: value = the units all ranks processed / the max-over-ranks time."""
     return world * units_per_rank * steps / seconds
 
 
@@ -189,11 +191,17 @@ def run_mrd(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the mrd path has no CPU fallback")
+    local %= torch.cuda.device_count()    # (more ranks than GPUs only happens with --backend gloo, a functional test)
     torch.cuda.set_device(local)
     dist = None
+    rdev = "cuda"                          # where the max-over-ranks reduction lives
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")
+            rdev = "cpu"
 
     def barrier():
         if dist is not None:
@@ -202,64 +210,90 @@ def run_mrd(args):
 
     prec = args.precision
     tdtype = torch.float64 if prec == "fp64" else torch.float32
-    cfg = build_workload(args.n, args.numbering)
-    mesh = cfg.mesh
-    nt, nv = mesh.nt, mesh.nv
-    t0 = time.perf_counter()
-    gm = mrd.Mesh(mesh.xy, mesh.tri, period=mesh.period, gamma=cfg.gamma, cfl=cfg.cfl, scheme=cfg.scheme,
-                  time_order=cfg.time_order, precision=mrd.FP64 if prec == "fp64" else mrd.FP32,
+    halo = world > 1 and args.decomposition == "halo"
+    params = dict(gamma=1.4, cfl=0.5, scheme=mrd.SCHEME_B, time_order=2, precision=mrd.FP64 if prec == "fp64" else mrd.FP32,
                   reorder=bool(args.reorder), tile=args.tile)
-    layout_s = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    if not halo:
+        # one GPU, or N independent replicas of the single-GPU workload
+        cfg = build_workload(args.n, args.numbering)
+        mesh = cfg.mesh
+        nt, nv = mesh.nt, mesh.nv                 # units per rank
+        nt_job, nv_job = world * nt, world * nv
+        gm = sim = mrd.Mesh(mesh.xy, mesh.tri, period=mesh.period, **params)
+        layout_s = time.perf_counter() - t0
+        gm.set_state(torch.tensor(cfg.W0, dtype=tdtype, device="cuda"))
+        parallelism = "1 GPU" if world == 1 else f"{world} independent replicas"
+    else:
+        # ONE mesh over N GPUs (weak scaling): a periodic strip of N copies of the single-GPU workload stacked in y, cut into
+        # N Morton ranges (= the N squares); one halo exchange per stage and one min-reduction per step over NCCL
+        import workloads as wl
+        from paper_1705_02028_b200.distributed import DistributedMesh
+        n = args.n
+        cell = build_workload(n, "natural")
+        mesh = wl.uniform_mesh(n, n * world, 10.0, 10.0 * world, periodic=True)
+        W0 = np.ascontiguousarray(np.tile(cell.W0.reshape(4, n, n), (1, world, 1)).reshape(4, -1))
+        sim = DistributedMesh(mesh.xy, mesh.tri, period=mesh.period, **params)
+        gm = sim.mesh                             # this rank's part (owned + halo vertices, cut triangles on both sides)
+        nt_job, nv_job = mesh.nt, mesh.nv         # unique triangles / vertices of the whole mesh
+        nt, nv = gm.nt, gm.nv                     # this rank's share (kernel-level numbers)
+        layout_s = time.perf_counter() - t0
+        sim.set_state(W0)
+        parallelism = (f"one mesh over {world} GPUs: Morton-range domain decomposition, {sim.part.n_send} halo vertices sent per "
+                       f"rank per stage to {sim.part.n_neighbour} neighbours, 1 all-reduce(min) per step")
+        del W0, cell
     stream = torch.cuda.current_stream()
-    W0 = torch.tensor(cfg.W0, dtype=tdtype, device="cuda")
-    gm.set_state(W0)
 
     # ---- device-resident throughput: W warm-up steps, then exactly K timed steps -------------------------
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local) as clk:
-        gm.step(args.warmup)
+        sim.step(args.warmup)
         barrier()
-        l0 = gm.launch_count()
+        l0 = sim.launch_count()
         e0.record(stream)
-        gm.step_async(args.steps)
+        sim.step_async(args.steps)
         e1.record(stream)
         torch.cuda.synchronize()
         barrier()
-    n_done, t_sim, _ = gm.sync()
-    launches = gm.launch_count() - l0
-    ms_total = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
-    assert n_done == args.warmup + args.steps, (n_done, args.warmup, args.steps)
+    n_done, t_sim, _ = sim.sync()
+    launches = sim.launch_count() - l0
+    ms_total = max_over_ranks(e0.elapsed_time(e1), dist, rdev)
+    assert n_done == (args.steps if halo else args.warmup + args.steps), (n_done, args.warmup, args.steps)
     ms_step = ms_total / args.steps
-    value = whole_job_rate(world, nt, args.steps, ms_total * 1e-3)
+    value = whole_job_rate(1, nt_job, args.steps, ms_total * 1e-3)
+
+    _, mr, mp = sim.diagnostics()
+    assert mr > 0 and mp > 0
+
+    # ---- end to end through the host-buffer C-ABI calls: H2D of the state, one step, D2H of the result ----
+    # (N > 1, one mesh: every rank moves its own part, halo copies included, and the step runs with its exchanges)
+    ke = max(1, min(args.steps, args.e2e_steps))
+    h_in = torch.empty((4, nv), dtype=tdtype).pin_memory()
+    h_out = torch.empty((4, nv), dtype=tdtype).pin_memory()
+    h_in.copy_(gm.get_state().cpu())
+    gm.set_state_host(h_in.numpy()); sim.step(1); gm.get_state_host(h_out.numpy())      # warm-up
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(ke):
+        gm.set_state_host(h_in.numpy())
+        sim.step(1)
+        gm.get_state_host(h_out.numpy())
+        h_in, h_out = h_out, h_in
+    torch.cuda.synchronize()
+    e2e_s = max_over_ranks(time.perf_counter() - t0, dist, rdev)
+    state_bytes = 4 * nv * (8 if prec == "fp64" else 4)
+    e2e = {"value": whole_job_rate(1, nt_job, ke, e2e_s), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+           "d2h_bytes_per_step": state_bytes, "steps": ke, "ms_per_step": e2e_s / ke * 1e3,
+           "api": "mrd_set_state_host + mrd_step(1) + mrd_get_state_host, pinned host buffers"
+                  + (" (bytes per rank; the step is the phase sequence with its halo exchanges)" if halo else "")}
 
     # ---- live per-kernel durations (CUDA events on the launching stream), averaged over 5 steps ------------
+    # (last: on a partitioned mesh these local steps run without exchanges, which is all a kernel timing needs)
     prof = {}
     nprof = 5
     for _ in range(nprof):
         for k, v in gm.step_profile().items():
             prof[k] = prof.get(k, 0.0) + v / nprof
-    _, mr, mp = gm.diagnostics()
-    assert mr > 0 and mp > 0
-
-    # ---- end to end through the host-buffer C-ABI calls: H2D of the state, one step, D2H of the result ----
-    ke = max(1, min(args.steps, args.e2e_steps))
-    h_in = torch.empty((4, nv), dtype=tdtype).pin_memory()
-    h_out = torch.empty((4, nv), dtype=tdtype).pin_memory()
-    h_in.copy_(gm.get_state().cpu())
-    gm.set_state_host(h_in.numpy()); gm.step(1); gm.get_state_host(h_out.numpy())      # warm-up
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(ke):
-        gm.set_state_host(h_in.numpy())
-        gm.step(1)
-        gm.get_state_host(h_out.numpy())
-        h_in, h_out = h_out, h_in
-    torch.cuda.synchronize()
-    e2e_s = max_over_ranks(time.perf_counter() - t0, dist, "cuda")
-    state_bytes = 4 * nv * (8 if prec == "fp64" else 4)
-    e2e = {"value": whole_job_rate(world, nt, ke, e2e_s), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
-           "d2h_bytes_per_step": state_bytes, "steps": ke, "ms_per_step": e2e_s / ke * 1e3,
-           "api": "mrd_set_state_host + mrd_step(1) + mrd_get_state_host, pinned host buffers"}
 
     if rank != 0:
         if dist is not None:
@@ -317,14 +351,17 @@ def run_mrd(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64" if prec == "fp64" else "f32", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json config 5: isentropic vortex, periodic uniform triangulation {args.n}^2 "
-                                   f"vertices, {nt} triangles, {args.numbering} input numbering, scheme B, RK2, CFL 0.5",
-                       "n_triangles": nt, "n_vertices": nv, "reorder": int(args.reorder), "tile": args.tile,
+            "config": {"workload": (f"BASELINE.json config 5: isentropic vortex, periodic uniform triangulation {args.n}^2 "
+                                    f"vertices, {nt} triangles, {args.numbering} input numbering, scheme B, RK2, CFL 0.5") if not halo else
+                                   (f"BASELINE.json config 5 stacked {world} times in y: row of {world} isentropic vortices, periodic uniform "
+                                    f"triangulation {args.n} x {args.n * world} vertices, {nt_job} triangles, natural input numbering, "
+                                    f"scheme B, RK2, CFL 0.5"),
+                       "n_triangles": nt_job, "n_vertices": nv_job, "n_triangles_rank0": nt, "reorder": int(args.reorder), "tile": args.tile,
                        "l2": "inputs larger than L2 (state %.0f MB, per-triangle arrays %.1f GB)" % (
                            state_bytes / 1e6, gm.device_bytes() / 1e9),
-                       "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas",
+                       "parallelism": parallelism,
                        "layout_s": layout_s, "device_gb": gm.device_bytes() / 1e9, "t_sim": t_sim},
-            "vertex_updates_per_s": world * nv * args.steps / (ms_total * 1e-3),
+            "vertex_updates_per_s": nv_job * args.steps / (ms_total * 1e-3),
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if dist is not None:
@@ -346,6 +383,10 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--traffic", type=float, default=None, help="dram bytes per launch of the dominant kernel (ncu)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="N > 1: torch.distributed backend (gloo stages the halo rows through host memory; functional tests only)")
+    ap.add_argument("--decomposition", default="halo", choices=["halo", "replicas"],
+                    help="N > 1: one mesh over the N GPUs with halo exchanges (default), or N independent replicas")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

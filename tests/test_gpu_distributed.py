@@ -75,3 +75,20 @@ def test_distributed_mesh_matches_oracle_and_single_mesh(world, single, tmp_path
         assert abs(mr - gmr) <= 1e-5 * abs(gmr) and abs(mp - gmp) <= 1e-4 * abs(gmp), name
         # the work really was split and exchanged, and ran in this library's kernels
         assert 0 < n_owned < ref["nv"] and n_recv > 0 and launches > 0, name
+
+
+def test_bench_n2_runs_one_mesh_over_two_ranks():
+    """bench.py --gpus 2 as the driver launches it, except for the backend (two ranks on the one GPU need gloo)."""
+    import json
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(29950 + os.getpid() % 40), os.path.join(ROOT, "bench.py"), "--gpus", "2", "--size", "256", "--steps", "4",
+           "--warmup", "3", "--backend", "gloo"]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=900, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-3000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "weak" and d["value"] > 0 and d["gpu_launches"] > 0
+    assert d["config"]["n_triangles"] == 2 * 2 * 256 * 256 and "one mesh over 2 GPUs" in d["config"]["parallelism"]
+    assert d["config"]["n_triangles_rank0"] > 2 * 256 * 256          # its square plus the cut triangles of both cut lines
+    assert d["e2e"]["h2d_bytes_per_step"] > 0 and d["roofline"]["kernel"].startswith("tri_stage")
