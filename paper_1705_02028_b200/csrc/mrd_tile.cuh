@@ -111,9 +111,10 @@ template <class R, int STAGE, bool GTAB> struct TileSmem {
     uint32_t s = 2 * buf_bytes;
     // stage 2: the residual exchange area aliases the current buffer's phi16 block -- thread `tid` only overwrites the
     // 12 entries [c][tid] it has consumed itself, so no other thread's data is touched (saves 12 KB: 4 blocks per SM)
-    oRes = s; if (STAGE == 1) s += (uint32_t)(sizeof(R) * 12 * T);
-    oST = s; if (STAGE == 1) s += up16(sizeof(R) * T);
-    oBar = s; s += 16;
+    // stage 1: two residual areas (tile k's epilogue may still read one while a faster warp writes tile k+1's)
+    oRes = s; if (STAGE == 1) s += 2 * (uint32_t)(sizeof(R) * 12 * T);
+    oST = s; if (STAGE == 1) s += 2 * up16(sizeof(R) * T);
+    oBar = s; s += 32;  // two mbarriers, two "warps done with the buffer" counters
     total = s;
   }
 };
@@ -185,21 +186,25 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
   R *res1 = reinterpret_cast<R *>(smem_raw + L.oRes);
   R *sST = reinterpret_cast<R *>(smem_raw + L.oST);
   uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + L.oBar);
-  if (tid == 0) {
-    mbar_init(&bar[0], 1);
-    mbar_init(&bar[1], 1);
-    fence_mbar_init();
-  }
-  __syncthreads();
+  unsigned *done = reinterpret_cast<unsigned *>(smem_raw + L.oBar + 16);
+  constexpr unsigned NW = TILE / 32;
   int64_t b = blockIdx.x;
   // slot / geometry-record range of the tile in flight (i0, i1); the next tile's range is fetched one iteration ahead
   int2 i0 = __ldg(td.tile_info + b), i1 = __ldg(td.tile_info + b + 1);
-  if (tid == 0) tile_stage_in<R, STAGE, GTAB>(td, L, smem_raw, &bar[0], b, i0, i1, slotZ, slotS, slotD, phi16);
-  int2 n0 = make_int2(0, 0), n1 = make_int2(0, 0);
-  if (b + gridDim.x < td.ntile) {
-    n0 = ld_info(td.tile_info + b + gridDim.x);
-    n1 = ld_info(td.tile_info + b + gridDim.x + 1);
+  if (tid == 0) {
+    mbar_init(&bar[0], 1);
+    mbar_init(&bar[1], 1);
+    done[0] = done[1] = 0;
+    fence_mbar_init();
+    // the first two tiles of this block; every later copy is issued by the last warp to leave the buffer it refills
+    tile_stage_in<R, STAGE, GTAB>(td, L, smem_raw, &bar[0], b, i0, i1, slotZ, slotS, slotD, phi16);
+    const int64_t b1 = b + gridDim.x;
+    if (b1 < td.ntile)
+      tile_stage_in<R, STAGE, GTAB>(td, L, smem_raw + L.buf_bytes, &bar[1], b1, __ldg(td.tile_info + b1), __ldg(td.tile_info + b1 + 1),
+                                    slotZ, slotS, slotD, phi16);
   }
+  __syncthreads();
+  int2 n0 = make_int2(0, 0), n1 = make_int2(0, 0);
   const int bvar = ctl->bvar;
   constexpr bool lump = STAGE == 2 && STORE;
   bool bad = false;  // linearised c^2 <= 0 met by this thread (raised once, after the loop)
@@ -207,24 +212,17 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
     const int cur = k & 1;
     unsigned char *buf = smem_raw + cur * L.buf_bytes;
     const int64_t nb = b + gridDim.x;
-    const int2 x0 = use_info(n0), x1 = use_info(n1);
-    if (nb < td.ntile) {
-      if (nb + gridDim.x < td.ntile) {  // in flight during this iteration, consumed at the top of the next one
-        n0 = ld_info(td.tile_info + nb + gridDim.x);
-        n1 = ld_info(td.tile_info + nb + gridDim.x + 1);
-      }
-      if (tid == 0) {
-        fence_proxy_async();  // buffer cur^1 was read through the generic proxy in iteration k-1
-        tile_stage_in<R, STAGE, GTAB>(td, L, smem_raw + (cur ^ 1) * L.buf_bytes, &bar[cur ^ 1], nb, x0, x1, slotZ, slotS, slotD,
-                                      phi16);
-      }
+    if (nb < td.ntile) {  // in flight during this iteration, consumed at its end
+      n0 = ld_info(td.tile_info + nb);
+      n1 = ld_info(td.tile_info + nb + 1);
     }
     const int s0 = i0.x, ns = i1.x - i0.x;
     mbar_wait(&bar[cur], (k >> 1) & 1);
     const Vec4<R> *sZ = reinterpret_cast<const Vec4<R> *>(buf + L.oZ);
     const R *sXY = reinterpret_cast<const R *>(buf + L.oXY);
     const uint16_t *plan = reinterpret_cast<const uint16_t *>(buf + L.oPlan);
-    R *res = STAGE == 1 ? res1 : reinterpret_cast<R *>(buf + L.oPhi);
+    R *res = STAGE == 1 ? res1 + cur * (12 * T) : reinterpret_cast<R *>(buf + L.oPhi);
+    R *sSTc = sST + cur * T;
     const int64_t t = b * T + tid;
     R pN[3][4];
     R st = R(0);
@@ -337,12 +335,28 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
 #pragma unroll
       for (int i = 0; i < 12; ++i) res[i * T + tid] = R(0);
     }
-    if (STAGE == 1) sST[tid] = st;
+    if (STAGE == 1) sSTc[tid] = st;
     __syncthreads();
-    tile_epilogue<R, STAGE == 1>(T, res, sST, plan + 4 * T, plan + 7 * T, s0, ns, part, partS);
-    __syncthreads();  // res and buffer `cur` are free again
-    i0 = x0;
-    i1 = x1;
+    tile_epilogue<R, STAGE == 1>(T, res, sSTc, plan + 4 * T, plan + 7 * T, s0, ns, part, partS);
+    // No second block barrier: a warp that is done goes on to the next tile (the other buffer, the other residual
+    // area) while slower warps finish this epilogue; the LAST warp to leave refills buffer `cur` with tile k+2.
+    // (Nobody runs more than one tile ahead: the barrier above needs every warp.)
+    __syncwarp();
+    if ((tid & 31) == 0) {
+      __threadfence_block();
+      if (atomicAdd(&done[cur], 1u) == NW - 1) {
+        __threadfence_block();
+        done[cur] = 0;
+        const int64_t b2 = nb + gridDim.x;
+        if (b2 < td.ntile) {
+          fence_proxy_async();  // buffer `cur` was read through the generic proxy
+          tile_stage_in<R, STAGE, GTAB>(td, L, buf, &bar[cur], b2, __ldg(td.tile_info + b2), __ldg(td.tile_info + b2 + 1), slotZ, slotS,
+                                        slotD, phi16);
+        }
+      }
+    }
+    i0 = use_info(n0);
+    i1 = use_info(n1);
   }
   if (bad) atomicOr(status, 1);
 }
