@@ -148,18 +148,35 @@ __device__ __forceinline__ void tile_stage_in(const TileDev<R> &td, const TileSm
 template <class R, bool WITH_ST>
 __device__ __forceinline__ void tile_epilogue(int T, const R *res, const R *sT, const uint16_t *ent, const uint16_t *off,
                                               int s0, int ns, Vec4<R> *__restrict__ part, R *__restrict__ partS) {
+  // The incidences of a slot are fetched EPI at a time, all loads issued before the first add: the plain loop is a chain of
+  // dependent shared-memory loads (entry -> residual -> add) per incidence, ~70 cycles each, and every warp of the block
+  // waits for the slowest one at the barrier before this.  Missing incidences add +0.0, which changes nothing.
+  constexpr int EPI = 8;
   for (int j = threadIdx.x; j < ns; j += T) {
     const int q0 = off[j], q1 = off[j + 1];
     R a0 = 0, a1 = 0, a2 = 0, a3 = 0, S = 0;
-    for (int q = q0; q < q1; ++q) {
-      const int e = ent[q];
-      const int lt = e >> 2, nd = e & 3;
-      const R *r = res + (nd * 4) * T + lt;
-      a0 += r[0];
-      a1 += r[T];
-      a2 += r[2 * T];
-      a3 += r[3 * T];
-      if (WITH_ST) S += sT[lt];
+    for (int q = q0; q < q1; q += EPI) {
+      R v[EPI][4], sv[EPI];
+#pragma unroll
+      for (int u = 0; u < EPI; ++u) {
+        const bool on = q + u < q1;
+        const int e = on ? ent[q + u] : 0;
+        const int lt = e >> 2, nd = e & 3;
+        const R *r = res + (nd * 4) * T + lt;
+        v[u][0] = on ? r[0] : R(0);
+        v[u][1] = on ? r[T] : R(0);
+        v[u][2] = on ? r[2 * T] : R(0);
+        v[u][3] = on ? r[3 * T] : R(0);
+        if (WITH_ST) sv[u] = on ? sT[lt] : R(0);
+      }
+#pragma unroll
+      for (int u = 0; u < EPI; ++u) {
+        a0 += v[u][0];
+        a1 += v[u][1];
+        a2 += v[u][2];
+        a3 += v[u][3];
+        if (WITH_ST) S += sv[u];
+      }
     }
     st4(&part[s0 + j], Vec4<R>{a0, a1, a2, a3});
     if (WITH_ST) partS[s0 + j] = S;
