@@ -129,9 +129,17 @@ def whole_job_rate(world: int, units_per_rank: int, steps: int, seconds: float) 
     return world * units_per_rank * steps / seconds
 
 
-def build_workload(n: int, numbering: str):
+def build_workload(n: int, numbering: str, kind: str = "uniform"):
+    """config 5; kind 'jitter' moves every vertex by up to 0.2 cell widths (no two triangles alike), 'flip' also flips a seeded
+    third of the edges (valence 4...10): the second, genuinely unstructured workload of SURVEY 8f-2."""
     import workloads as wl
     cfg = wl.make_config("sweep", n=n, numbering=numbering)
+    if kind in ("jitter", "flip"):
+        cfg.mesh = wl.jitter_mesh(cfg.mesh, 0.2, seed=7)
+    if kind == "flip":
+        cfg.mesh = wl.flip_edges(cfg.mesh, seed=11)
+    if kind != "uniform":
+        cfg.W0 = wl.vortex_state(cfg.mesh)     # the same vortex, sampled at the moved vertices
     return cfg
 
 
@@ -216,7 +224,7 @@ def run_mrd(args):
     t0 = time.perf_counter()
     if not halo:
         # one GPU, or N independent replicas of the single-GPU workload
-        cfg = build_workload(args.n, args.numbering)
+        cfg = build_workload(args.n, args.numbering, args.mesh)
         mesh = cfg.mesh
         nt, nv = mesh.nt, mesh.nv                 # units per rank
         nt_job, nv_job = world * nt, world * nv
@@ -352,7 +360,8 @@ def run_mrd(args):
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64" if prec == "fp64" else "f32", "data": "synthetic",
             "config": {"workload": (f"BASELINE.json config 5: isentropic vortex, periodic uniform triangulation {args.n}^2 "
-                                    f"vertices, {nt} triangles, {args.numbering} input numbering, scheme B, RK2, CFL 0.5") if not halo else
+                                    f"vertices, {nt} triangles, {args.numbering} input numbering, scheme B, RK2, CFL 0.5"
+                                    + ("" if args.mesh == "uniform" else f", mesh variant '{args.mesh}'")) if not halo else
                                    (f"BASELINE.json config 5 stacked {world} times in y: row of {world} isentropic vortices, periodic uniform "
                                     f"triangulation {args.n} x {args.n * world} vertices, {nt_job} triangles, natural input numbering, "
                                     f"scheme B, RK2, CFL 0.5"),
@@ -383,6 +392,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--traffic", type=float, default=None, help="dram bytes per launch of the dominant kernel (ncu)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mesh", default="uniform", choices=["uniform", "jitter", "flip"],
+                    help="uniform triangulation (config 5), jittered vertices, or jittered + flipped edges (variable valence)")
     ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
                     help="N > 1: torch.distributed backend (gloo stages the halo rows through host memory; functional tests only)")
     ap.add_argument("--decomposition", default="halo", choices=["halo", "replicas"],

@@ -27,6 +27,8 @@ def cases():
     j = wl.jitter_mesh(wl.uniform_mesh(33, 27, 1.0, 1.0, periodic=True), 0.2, seed=11)
     out["jitter_lda2"] = (j, wl.random_smooth_state(j, mach=0.5, seed=4), None, None,
                           dict(scheme=1, time_order=2, reorder=False, tile=64), 10, 0.0)
+    f = wl.flip_edges(wl.jitter_mesh(wl.uniform_mesh(40, 36, 2.0, 1.8, periodic=True), 0.2, seed=3), seed=11)
+    out["variable_valence_b2"] = (f, wl.random_smooth_state(f, mach=0.8, seed=6), None, None, dict(scheme=2, time_order=2), 10, 0.0)
     r = wl.make_config("riemann4", n=40)
     out["riemann4_frozen"] = (r.mesh, r.W0, r.vertex_flag, None, dict(scheme=2, time_order=2), 6, 0.0)
     return out

@@ -390,3 +390,37 @@ def test_noh_infinite_mach_shock_first_order(mrd):
     assert field_errors(Wg, Wo) <= TOL_100
     _, mr, mp = gm.diagnostics()
     assert mr > 0 and mp > 0 and Wg[0].max() > 2.0               # the central compression has started
+
+
+# ------------------------------------------------------------------------------------------------
+# variable-valence triangulation (stand-in for the paper's Delaunay-refined meshes, L685)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("tile", [-1, 0, 64])
+@pytest.mark.parametrize("periodic", [True, False])
+def test_variable_valence_mesh_matches_oracle(mrd, tile, periodic):
+    mesh = wl.flip_edges(wl.jitter_mesh(wl.uniform_mesh(40, 36, 2.0, 1.8, periodic=periodic), 0.2, seed=3), seed=11)
+    val = np.bincount(mesh.tri.ravel(), minlength=mesh.nv)
+    assert val.max() >= 8 and val.min() <= 4
+    W = wl.random_smooth_state(mesh, mach=0.8, seed=6)
+    flag = None if periodic else wl.boundary_vertices(mesh)
+    import torch
+    gm = mrd.Mesh(mesh.xy, mesh.tri, vertex_flag=flag, period=mesh.period, tile=tile)
+    gm.set_state(torch.tensor(W, device="cuda"))
+    om = oracle.OracleMesh(mesh.xy, mesh.tri, period=mesh.period, vertex_flag=flag)
+    om.set_state(W)
+    g, o = gm.dump_stage1(), om.dump_stage1()
+    scale = np.abs(o["phiN"]).max()
+    for key in ("phiT", "phiN", "phiLDA", "phiB"):
+        assert np.abs(g[key] - o[key]).max() <= 2e-13 * scale, key
+    assert np.allclose(g["sT"], o["sT"], rtol=1e-14, atol=0)
+    n, t, dt = gm.step(1)
+    no, to, dto = om.step(1)
+    assert abs(dt - dto) <= 1e-14 * dto
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_1
+    gm.step(49)
+    om.step(49)
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= TOL_100
+    if periodic:
+        tot0 = (W * om.geometry()[1][None, :]).sum(axis=1)
+        tot = gm.diagnostics()[0]
+        assert np.abs(tot - tot0).max() <= 1e-12 * np.abs(tot0).max()        # conservation with variable V_i and valence

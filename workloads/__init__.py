@@ -12,6 +12,7 @@ from .meshes import (  # noqa: F401
     permute_mesh,
     morton_order_mesh,
     jitter_mesh,
+    flip_edges,
     boundary_vertices,
     wall_edges_y,
     UniformMesh,

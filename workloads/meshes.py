@@ -139,6 +139,57 @@ def jitter_mesh(mesh: UniformMesh, amplitude: float = 0.25, seed: int = 7) -> Un
     return replace(mesh, xy=np.ascontiguousarray(xy))
 
 
+def flip_edges(mesh: UniformMesh, fraction: float = 0.35, seed: int = 11, rounds: int = 2) -> UniformMesh:
+    """Variable-valence triangulation (stand-in for the paper's Delaunay-refined meshes, L685, which are not in
+    the container): flip a seeded random set of interior edges.  Edge ab shared by the CCW triangles (a,b,c) and
+    (b,a,d) becomes edge cd, giving (a,d,c) and (d,b,c); it is flipped only if both new triangles keep a
+    positive area of at least 15 % of the mean (strictly convex quadrilateral).  Per round every edge is a
+    candidate with probability `fraction`, and a candidate is taken when it has the highest random priority among
+    the candidates of both its triangles (so no triangle is flipped twice in a round).  Vertices a, b lose one
+    incident triangle, c, d gain one: valences spread from 6 to about 4...9.  Vertex numbering, coordinates and
+    boundary edges are unchanged (bounded meshes keep their wall edges and frozen vertices)."""
+    rng = np.random.default_rng(seed)
+    tri = mesh.tri.astype(np.int64).copy()
+    nt = tri.shape[0]
+    px, py = mesh.period
+
+    def unwrap(d, period):
+        return d - period * np.round(d / period) if period > 0.0 else d
+
+    def area2(a, b, c):
+        abx, aby = unwrap(mesh.xy[b, 0] - mesh.xy[a, 0], px), unwrap(mesh.xy[b, 1] - mesh.xy[a, 1], py)
+        acx, acy = unwrap(mesh.xy[c, 0] - mesh.xy[a, 0], px), unwrap(mesh.xy[c, 1] - mesh.xy[a, 1], py)
+        return abx * acy - aby * acx
+
+    amin = 0.15 * float(np.mean(area2(tri[:, 0], tri[:, 1], tri[:, 2])))
+    for _ in range(rounds):
+        # directed edges (a -> b) of every triangle with the opposite vertex; pair a->b with b->a
+        t_id = np.repeat(np.arange(nt), 3)
+        k = np.tile(np.arange(3), nt)
+        a, b, c = tri[t_id, k], tri[t_id, (k + 1) % 3], tri[t_id, (k + 2) % 3]
+        key = a * mesh.nv + b
+        rkey = b * mesh.nv + a
+        order = np.argsort(key)
+        pos = np.searchsorted(key[order], rkey)
+        pos = np.minimum(pos, len(key) - 1)
+        mate = order[pos]
+        has = (key[mate] == rkey) & (a < b)               # interior edge, counted once
+        e1 = np.nonzero(has)[0]
+        e2 = mate[e1]
+        A, B, Cc, D = a[e1], b[e1], c[e1], c[e2]
+        T1, T2 = t_id[e1], t_id[e2]
+        ok = (area2(A, D, Cc) > amin) & (area2(D, B, Cc) > amin) & (rng.random(len(e1)) < fraction)
+        prio = rng.random(len(e1)) + 1.0
+        prio[~ok] = 0.0
+        best = np.zeros(nt)
+        np.maximum.at(best, T1, prio)
+        np.maximum.at(best, T2, prio)
+        take = ok & (prio == best[T1]) & (prio == best[T2])
+        tri[T1[take]] = np.stack([A[take], D[take], Cc[take]], axis=1)
+        tri[T2[take]] = np.stack([D[take], B[take], Cc[take]], axis=1)
+    return replace(mesh, tri=np.ascontiguousarray(tri.astype(np.int32)))
+
+
 def boundary_vertices(mesh: UniformMesh, x_ends: bool = True, y_ends: bool = True) -> np.ndarray:
     """uint8 [nv] flag: 1 on the requested boundary rows/columns of a bounded mesh (PAPER.md L582:
     boundary vertices promoted to ghost vertices that keep the initial condition)."""
