@@ -13,7 +13,7 @@ import numpy as np
 from . import build as _build
 
 ORC_OK, ORC_EINVAL, ORC_ENOMEM, ORC_ENONPHYSICAL = 0, -1, -2, -4
-SCHEME_N, SCHEME_LDA, SCHEME_B, SCHEME_BMAX, SCHEME_BMIN = 0, 1, 2, 3, 4
+SCHEME_N, SCHEME_LDA, SCHEME_B, SCHEME_BMAX, SCHEME_BMIN, SCHEME_BX = 0, 1, 2, 3, 4, 5
 
 _lib = None
 

@@ -306,14 +306,17 @@ template <class R> void apply_beta(const Core<R> &o, const R x[4], R out[3][4]) 
 // eq. 52-53 (+ reading C10): Theta_kk = min(1, |phi_k| / sum_j |phi^N_{j,k}|), 0 when the denominator is 0
 // Bmax / Bmin (L503): "setting all diagonal values of Theta to theta, [where] theta can be taken to be either the
 // maximum (Bmax) or the minimum (Bmin) over all Theta_kk".
+// Bx (eq. 54): one scalar theta from the shock sensor (bx_theta below), passed in as theta_bx.
 template <class R>
-void blend(int scheme, const R phiT[4], const R phiN[3][4], const R phiLDA[3][4], R theta[4], R phiB[3][4]) {
+void blend(int scheme, const R phiT[4], const R phiN[3][4], const R phiLDA[3][4], R theta[4], R phiB[3][4],
+           R theta_bx = R(0.0)) {
   for (int k = 0; k < 4; ++k) {
     R den = Abs(phiN[0][k]) + Abs(phiN[1][k]) + Abs(phiN[2][k]);
     R th = R(0.0);
     if (den > R(0.0)) th = Min(R(1.0), Abs(phiT[k]) / den);
     if (scheme == ORC_SCHEME_N) th = R(1.0);
     if (scheme == ORC_SCHEME_LDA) th = R(0.0);
+    if (scheme == ORC_SCHEME_BX) th = theta_bx;
     theta[k] = th;
   }
   if (scheme == ORC_SCHEME_BMAX || scheme == ORC_SCHEME_BMIN) {
@@ -325,19 +328,45 @@ void blend(int scheme, const R phiT[4], const R phiN[3][4], const R phiLDA[3][4]
     for (int i = 0; i < 3; ++i) phiB[i][k] = theta[k] * phiN[i][k] + (R(1.0) - theta[k]) * phiLDA[i][k];
 }
 
+// Bx shock sensor, eq. 55-56 (L509-L517), readings C23-C26 of DESIGN.md:
+//   s = ( -L div v / (|v|_max - |v|_min) )^+ ,  theta = min(1, s^2 h)
+// * div v: divergence of the LINEAR interpolant of the vertex velocities u_j = m_j / rho_j on the triangle,
+//   sum_j (u_j . n_j) l_j / (2 |T|) with the inward normal n_j opposite vertex j (grad N_j = n_j l_j / (2|T|));
+// * |v|_max, |v|_min: extremes of the vertex speeds over the WHOLE mesh at the state the stage is evaluated at
+//   (only then is s = O(1) in smooth flow, as L517 says); equal extremes (e.g. fluid at rest): s = 0;
+// * L: the domain size = the larger side of the domain's bounding box (the period where periodic);
+// * h: "a measure of the size of the element" made dimensionless with L: l_max^T / L (l_max as in eq. 44);
+//   theta is clamped to 1 (a blend coefficient).
+template <class R> struct BxCtx {
+  R L;       // domain size
+  R vrange;  // |v|_max - |v|_min of the stage's state
+};
+template <class R> R bx_theta(const R W[3][4], const Geom<R> &g, const BxCtx<R> &bx) {
+  R div = R(0.0);
+  for (int j = 0; j < 3; ++j) {
+    R u = W[j][1] / W[j][0], v = W[j][2] / W[j][0];
+    div = div + (u * g.nx[j] + v * g.ny[j]) * g.len[j];
+  }
+  div = div / (R(2.0) * g.area);
+  if (!(bx.vrange > R(0.0))) return R(0.0);
+  R s = Max(R(0.0), -(bx.L * div) / bx.vrange);  // eq. 56
+  return Min(R(1.0), s * s * (g.lmax / bx.L));   // eq. 55
+}
+
 template <class R> struct Stage1Out {
   R phiT[4], phiN[3][4], phiLDA[3][4], phiB[3][4], theta[4], sT;
 };
 
 template <class R>
-int triangle_stage1(R gamma, int scheme, const R W[3][4], const Geom<R> &g, Core<R> &core, Stage1Out<R> &o) {
+int triangle_stage1(R gamma, int scheme, const R W[3][4], const Geom<R> &g, Core<R> &core, Stage1Out<R> &o,
+                    const BxCtx<R> *bx = nullptr) {
   int rc = triangle_core(gamma, W, g, core);
   if (rc) return rc;
   for (int k = 0; k < 4; ++k) o.phiT[k] = core.phiT[k];
   for (int i = 0; i < 3; ++i)
     for (int k = 0; k < 4; ++k) o.phiN[i][k] = core.phiN[i][k];
   apply_beta(core, core.phiT, o.phiLDA);  // eq. 50
-  blend(scheme, o.phiT, o.phiN, o.phiLDA, o.theta, o.phiB);
+  blend(scheme, o.phiT, o.phiN, o.phiLDA, o.theta, o.phiB, (scheme == ORC_SCHEME_BX && bx) ? bx_theta(W, g, *bx) : R(0.0));
   // O7 / eq. 44-45: s_T = l_max * max_j (|v_j| + c_j)
   o.sT = g.lmax * Max(core.speed[0], Max(core.speed[1], core.speed[2]));
   return ORC_OK;
@@ -354,7 +383,8 @@ template <class R> struct Stage2Out {
 // the usual way" (L572); it sums to zero over the nodes, so Phi^T and conservation are unchanged.
 template <class R>
 int triangle_stage2(R gamma, int scheme, const R Wn[3][4], const R Ws[3][4], const Geom<R> &g, R dt,
-                    const R phiT_n[4], const R phiN_n[3][4], Core<R> &core, Stage2Out<R> &o, int lumping = 0) {
+                    const R phiT_n[4], const R phiN_n[3][4], Core<R> &core, Stage2Out<R> &o, int lumping = 0,
+                    const BxCtx<R> *bx = nullptr) {
   int rc = triangle_core(gamma, Ws, g, core);  // all matrices re-evaluated at W*
   if (rc) return rc;
   R third = g.area / R(3.0);
@@ -381,7 +411,8 @@ int triangle_stage2(R gamma, int scheme, const R Wn[3][4], const R Ws[3][4], con
         o.PhiLDA[i][k] = o.PhiLDA[i][k] + extra;
       }
   }
-  blend(scheme, o.PhiT, o.PhiN, o.PhiLDA, o.theta, o.PhiB);
+  // Bx in stage 2: the sensor of the state the matrices are evaluated at, W* (as C12)
+  blend(scheme, o.PhiT, o.PhiN, o.PhiLDA, o.theta, o.PhiB, (scheme == ORC_SCHEME_BX && bx) ? bx_theta(Ws, g, *bx) : R(0.0));
   return ORC_OK;
 }
 
@@ -434,6 +465,7 @@ struct orc_mesh {
   std::vector<double> phi, phiN_n, phiT_n, sT;  // per-triangle scratch: [nt][3][4], [nt][3][4], [nt][4], [nt]
   std::vector<double> acc;           // [nv][4]
   std::vector<double> wallN;         // [ne][2][4] stage-1 wall terms
+  double Ldom = 1.0;                 // domain size L of eq. 56 (Bx)
   int nthreads = 1;
   double t = 0.0;
   bool has_state = false;
@@ -476,7 +508,7 @@ int orc_mesh_create(orc_mesh **out, double gamma, double cfl, int scheme, int ti
                     const uint8_t *vertex_flag, int64_t ne, const int32_t *wall_edge) {
   if (!out || !xy || !tri || nv < 3 || nt < 1) return fail(ORC_EINVAL, "null or empty mesh");
   if (!(gamma > 1.0) || !(cfl > 0.0)) return fail(ORC_EINVAL, "gamma must be > 1 and cfl > 0");
-  if (scheme < 0 || scheme > 4 || (time_order != 1 && time_order != 2)) return fail(ORC_EINVAL, "bad scheme/time_order");
+  if (scheme < 0 || scheme > 5 || (time_order != 1 && time_order != 2)) return fail(ORC_EINVAL, "bad scheme/time_order");
   if (ne < 0 || (ne > 0 && !wall_edge)) return fail(ORC_EINVAL, "bad wall edge list");
   orc_mesh *m = new (std::nothrow) orc_mesh();
   if (!m) return fail(ORC_ENOMEM, "out of memory");
@@ -511,6 +543,17 @@ int orc_mesh_create(orc_mesh **out, double gamma, double cfl, int scheme, int ti
   }
   for (int64_t i = 0; i < nv; ++i)
     if (deg[i] == 0) { delete m; return fail(ORC_EINVAL, "vertex without triangle"); }
+  {  // domain size L of eq. 56: larger side of the bounding box, the period where periodic (reading C25)
+    double lo[2] = {xy[0], xy[1]}, hi[2] = {xy[0], xy[1]};
+    for (int64_t i = 0; i < nv; ++i)
+      for (int d = 0; d < 2; ++d) {
+        lo[d] = std::min(lo[d], xy[2 * i + d]);
+        hi[d] = std::max(hi[d], xy[2 * i + d]);
+      }
+    double side[2];
+    for (int d = 0; d < 2; ++d) side[d] = m->period[d] > 0.0 ? m->period[d] : hi[d] - lo[d];
+    m->Ldom = std::max(side[0], side[1]);
+  }
   // wall edges: outward unit normal = away from the third vertex of the one triangle holding the edge
   if (ne > 0) {
     m->wedge.assign(wall_edge, wall_edge + 2 * ne);
@@ -617,16 +660,30 @@ int orc_get_diagnostics(const orc_mesh *m, double totals[4], double *min_rho, do
 
 namespace {
 
+// |v|_max - |v|_min over all vertices of the state W (Bx, eq. 56)
+BxCtx<double> bx_context(const orc_mesh *m, const std::vector<double> &W) {
+  double vmax = 0.0, vmin = INFINITY;
+  for (int64_t i = 0; i < m->nv; ++i) {
+    double u = W[m->nv + i] / W[i], v = W[2 * m->nv + i] / W[i];
+    double a = std::sqrt(u * u + v * v);
+    vmax = std::max(vmax, a);
+    vmin = std::min(vmin, a);
+  }
+  return BxCtx<double>{m->Ldom, vmax - vmin};
+}
+
 // Stage-1 triangle loop over the state `W`: fills m->phi (scheme residuals), m->phiN_n, m->phiT_n, m->sT.
 int stage1_triangles(orc_mesh *m, const std::vector<double> &W, double *dump_LDA, double *dump_B) {
   int bad = 0;
+  BxCtx<double> bx{m->Ldom, 0.0};
+  if (m->scheme == ORC_SCHEME_BX) bx = bx_context(m, W);
 #pragma omp parallel for schedule(static) num_threads(m->nthreads) reduction(| : bad)
   for (int64_t t = 0; t < m->nt; ++t) {
     double w[3][4];
     gather(m, W, t, w);
     Core<double> core;
     Stage1Out<double> o;
-    if (triangle_stage1(m->gamma, m->scheme, w, m->geo[t], core, o)) { bad |= 1; continue; }
+    if (triangle_stage1(m->gamma, m->scheme, w, m->geo[t], core, o, &bx)) { bad |= 1; continue; }
     for (int i = 0; i < 3; ++i)
       for (int k = 0; k < 4; ++k) {
         m->phi[12 * t + 4 * i + k] = o.phiB[i][k];
@@ -642,6 +699,8 @@ int stage1_triangles(orc_mesh *m, const std::vector<double> &W, double *dump_LDA
 
 int stage2_triangles(orc_mesh *m, double dt) {
   int bad = 0;
+  BxCtx<double> bx{m->Ldom, 0.0};
+  if (m->scheme == ORC_SCHEME_BX) bx = bx_context(m, m->Ws);
 #pragma omp parallel for schedule(static) num_threads(m->nthreads) reduction(| : bad)
   for (int64_t t = 0; t < m->nt; ++t) {
     double wn[3][4], ws[3][4], pN[3][4], pT[4];
@@ -652,7 +711,7 @@ int stage2_triangles(orc_mesh *m, double dt) {
     for (int k = 0; k < 4; ++k) pT[k] = m->phiT_n[4 * t + k];
     Core<double> core;
     Stage2Out<double> o;
-    if (triangle_stage2(m->gamma, m->scheme, wn, ws, m->geo[t], dt, pT, pN, core, o, m->lumping)) { bad |= 1; continue; }
+    if (triangle_stage2(m->gamma, m->scheme, wn, ws, m->geo[t], dt, pT, pN, core, o, m->lumping, &bx)) { bad |= 1; continue; }
     for (int i = 0; i < 3; ++i)
       for (int k = 0; k < 4; ++k) m->phi[12 * t + 4 * i + k] = o.PhiB[i][k];
   }

@@ -18,7 +18,8 @@ extern "C" {
 typedef struct orc_mesh orc_mesh;
 
 enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENOMEM = -2, ORC_ENONPHYSICAL = -4 };
-enum { ORC_SCHEME_N = 0, ORC_SCHEME_LDA = 1, ORC_SCHEME_B = 2, ORC_SCHEME_BMAX = 3, ORC_SCHEME_BMIN = 4 /* L503 */ };
+enum { ORC_SCHEME_N = 0, ORC_SCHEME_LDA = 1, ORC_SCHEME_B = 2, ORC_SCHEME_BMAX = 3, ORC_SCHEME_BMIN = 4 /* L503 */,
+       ORC_SCHEME_BX = 5 /* shock-sensor blend, eq. 54-56 L505-L517 */ };
 
 /* Mesh + parameters (PAPER.md L656-L663 mesh arrays; L576 scheme choices; eq. 44 CFL). */
 int orc_mesh_create(orc_mesh **out, double gamma, double cfl, int scheme, int time_order,
