@@ -37,7 +37,10 @@ enum {
   MRD_ENONPHYSICAL = -4  /* rho <= 0, p <= 0 or linearised c^2 <= 0 met; state = last good step  */
 };
 enum { MRD_SCHEME_N = 0, MRD_SCHEME_LDA = 1, MRD_SCHEME_B = 2,      /* eq. 48-49 / 50-51 / 52-53 */
-       MRD_SCHEME_BMAX = 3, MRD_SCHEME_BMIN = 4 };                   /* B with all Theta_kk = their max / min (L503) */
+       MRD_SCHEME_BMAX = 3, MRD_SCHEME_BMIN = 4,                     /* B with all Theta_kk = their max / min (L503) */
+       MRD_SCHEME_BX = 5 };  /* scalar blend from the shock sensor of eq. 54-56 (L505-L517; readings C23-C26 of DESIGN.md):
+                                one more pass over the vertices per stage for |v|_max - |v|_min; not available on a
+                                partitioned mesh (mrd_phase* returns MRD_EINVAL) */
 enum { MRD_FP64 = 0, MRD_FP32 = 1 };
 
 typedef struct mrd_mesh mrd_mesh;     /* opaque: mesh layout + device state + stepper */
@@ -46,7 +49,7 @@ typedef struct mrd_layout mrd_layout; /* opaque: host-only result of the mesh-la
 typedef struct {
   double gamma;       /* ratio of specific heats, > 1 (eq. 10)                                  */
   double cfl;         /* dt = cfl * (bound of eq. 44), > 0                                       */
-  int32_t scheme;     /* MRD_SCHEME_N | _LDA | _B | _BMAX | _BMIN                                      */
+  int32_t scheme;     /* MRD_SCHEME_N | _LDA | _B | _BMAX | _BMIN | _BX                                */
   int32_t time_order; /* 1 = single stage eq. 43 (L437); 2 = RK2 eq. 60-61 (L539-L553)                 */
   int32_t precision;  /* MRD_FP64 | MRD_FP32: arithmetic AND storage type of the sweep                 */
   int32_t reorder;    /* 1 = renumber vertices/triangles along a Morton curve (L669-L675); 0 = keep    */

@@ -7,6 +7,6 @@ calls raise.
 """
 from .binding import (  # noqa: F401
     MRD_OK, MRD_EINVAL, MRD_ENOMEM, MRD_ECUDA, MRD_ENONPHYSICAL,
-    SCHEME_N, SCHEME_LDA, SCHEME_B, SCHEME_BMAX, SCHEME_BMIN, FP64, FP32,
+    SCHEME_N, SCHEME_LDA, SCHEME_B, SCHEME_BMAX, SCHEME_BMIN, SCHEME_BX, FP64, FP32,
     MrdError, Params, Layout, Partition, Mesh, lib, measure_peaks, exported_symbols, version,
 )

@@ -10,7 +10,7 @@ import numpy as np
 from . import build as _build
 
 MRD_OK, MRD_EINVAL, MRD_ENOMEM, MRD_ECUDA, MRD_ENONPHYSICAL = 0, -1, -2, -3, -4
-SCHEME_N, SCHEME_LDA, SCHEME_B, SCHEME_BMAX, SCHEME_BMIN = 0, 1, 2, 3, 4
+SCHEME_N, SCHEME_LDA, SCHEME_B, SCHEME_BMAX, SCHEME_BMIN, SCHEME_BX = 0, 1, 2, 3, 4, 5
 FP64, FP32 = 0, 1
 
 

@@ -238,10 +238,12 @@ template <class R> int upload_impl(mrd_mesh *m) {
       CUDA_TRY(cudaMemset(sp, 0, sizeof(R) * L.nslot));
       m->d_slotZ[b] = z; m->d_slotS[b] = sp;
     }
+    m->d_part = pp; m->d_partS = ps;
+  }
+  {
     cudaDeviceProp prop;
     CUDA_TRY(cudaGetDeviceProperties(&prop, m->device));
     m->nsm = prop.multiProcessorCount;
-    m->d_part = pp; m->d_partS = ps;
   }
   if ((rc = dev_upload_real<R>(m, &m->d_vol, L.vol.data(), nv))) return rc;
   if (L.nf > 0 && (rc = dev_upload(m, &m->d_frozen, L.frozen.data(), nv))) return rc;
@@ -293,6 +295,9 @@ template <class R> int set_state_impl(mrd_mesh *m, const R *W_dev, cudaStream_t 
   c.dmin_bits = 0x7FF0000000000000ull; c.steps = 0; c.status = 0; c.active = 0;
   c.bvar = m->L.p.scheme == MRD_SCHEME_BMAX ? 1 : (m->L.p.scheme == MRD_SCHEME_BMIN ? 2 : 0);
   c.lumping = m->L.p.lumping;
+  c.bx_L = m->L.domain_size;
+  c.vmax_bits[0] = c.vmax_bits[1] = 0ull;
+  c.vmin_bits[0] = c.vmin_bits[1] = 0x7FF0000000000000ull;
   CUDA_TRY(cudaMemcpyAsync(m->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice, s));
   CUDA_TRY(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
   mrd::set_state_kernel<R><<<blocks_for(nv, 256), 256, 0, s>>>(nv, m->d_vperm, W_dev, (R)m->L.p.gamma, (V4 *)m->d_W[0],
@@ -424,9 +429,14 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
   const unsigned vb = blocks_for(md.nv, 256);
   const bool fused = m->fused;
   if (mask & (1 << MRD_PHASE_RESIDUAL1)) {
+    if (scheme == MRD_SCHEME_BX) {  // eq. 56: |v|_max - |v|_min of W^n
+      mrd::vrange_kernel<R><<<std::min<unsigned>(vb, (unsigned)m->nsm * 8), 256, 0, s>>>(md.nv, (const V4 *)m->d_W[a], m->d_ctl, 0);
+      m->launches++;
+    }
     switch (scheme) {
       case MRD_SCHEME_N: launch_stage1<R, MRD_SCHEME_N>(m, rk2, a, s); break;
       case MRD_SCHEME_LDA: launch_stage1<R, MRD_SCHEME_LDA>(m, rk2, a, s); break;
+      case MRD_SCHEME_BX: launch_stage1<R, MRD_SCHEME_BX>(m, rk2, a, s); break;
       default: launch_stage1<R, MRD_SCHEME_B>(m, rk2, a, s); break;
     }
     PROF_MARK(MRD_PROF_TRI1)
@@ -471,9 +481,14 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
     PROF_MARK(MRD_PROF_UPDATE)
   }
   if (rk2 && (mask & (1 << MRD_PHASE_STAGE2))) {
+    if (scheme == MRD_SCHEME_BX) {  // ... and of W*
+      mrd::vrange_kernel<R><<<std::min<unsigned>(vb, (unsigned)m->nsm * 8), 256, 0, s>>>(md.nv, (const V4 *)m->d_W[b], m->d_ctl, 1);
+      m->launches++;
+    }
     switch (scheme) {
       case MRD_SCHEME_N: launch_stage2<R, MRD_SCHEME_N>(m, b, s); break;
       case MRD_SCHEME_LDA: launch_stage2<R, MRD_SCHEME_LDA>(m, b, s); break;
+      case MRD_SCHEME_BX: launch_stage2<R, MRD_SCHEME_BX>(m, b, s); break;
       default: launch_stage2<R, MRD_SCHEME_B>(m, b, s); break;
     }
     PROF_MARK(MRD_PROF_TRI2)
@@ -524,7 +539,8 @@ template <class R> int run_steps(mrd_mesh *m, int scheme, int64_t n, int &a, cud
       if (e != cudaSuccess) return fail(MRD_ECUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e));
     }
   }
-  const int64_t per_step = (m->L.p.time_order == 2 ? 6 : 4) + (m->nwv > 0 ? (m->L.p.time_order == 2 ? 2 : 1) : 0);
+  const int64_t per_step = (m->L.p.time_order == 2 ? 6 : 4) + (m->nwv > 0 ? (m->L.p.time_order == 2 ? 2 : 1) : 0) +
+                           (scheme == MRD_SCHEME_BX ? m->L.p.time_order : 0);
   for (int64_t k = 0; k + 1 < n; k += 2) {
     CUDA_TRY(cudaGraphLaunch(m->gexec[a], m->s_int));
     m->launches += 2 * per_step;
@@ -654,6 +670,15 @@ template <class R> int diag_impl(mrd_mesh *m, double totals[4], double *min_rho,
   return MRD_OK;
 }
 
+// stage 1 of the Bx blend for the dumps: the speed range of the current state (eq. 56), then the Bx kernels
+template <class R> void launch_bx_stage1(mrd_mesh *m, int a, cudaStream_t s) {
+  using V4 = mrd::Vec4<R>;
+  const unsigned vb = blocks_for(m->L.nv, 256);
+  mrd::vrange_kernel<R><<<std::min<unsigned>(vb, (unsigned)m->nsm * 8), 256, 0, s>>>(m->L.nv, (const V4 *)m->d_W[a], m->d_ctl, 0);
+  m->launches++;
+  launch_stage1<R, MRD_SCHEME_BX>(m, true, a, s);
+}
+
 // per-triangle dump of stage 1 in USER numbering / node order
 template <class R> int dump_impl(mrd_mesh *m, double *phiT, double *phiN, double *phiLDA, double *phiB, double *sT, cudaStream_t s) {
   using V4 = mrd::Vec4<R>;
@@ -686,6 +711,7 @@ template <class R> int dump_impl(mrd_mesh *m, double *phiT, double *phiN, double
   m->dbg = m->fused;
   for (int pass = 0; pass < 2; ++pass) {
     if (pass == 0) launch_stage1<R, MRD_SCHEME_LDA>(m, true, a, s);
+    else if (m->L.p.scheme == MRD_SCHEME_BX) launch_bx_stage1<R>(m, a, s);
     else launch_stage1<R, MRD_SCHEME_B>(m, true, a, s);
     CUDA_TRY(cudaMemcpyAsync(h3.data(), m->d_phi, h3.size() * sizeof(R), cudaMemcpyDeviceToHost, s));
     CUDA_TRY(cudaStreamSynchronize(s));
@@ -759,6 +785,7 @@ template <class R> int dump_sample_impl(mrd_mesh *m, int64_t ns, const int64_t *
   };
   for (int pass = 0; pass < 2; ++pass) {
     if (pass == 0) launch_stage1<R, MRD_SCHEME_LDA>(m, true, a, s);
+    else if (m->L.p.scheme == MRD_SCHEME_BX) launch_bx_stage1<R>(m, a, s);
     else launch_stage1<R, MRD_SCHEME_B>(m, true, a, s);
     CUDA_TRY(cudaStreamSynchronize(s));
     CUDA_TRY(cudaGetLastError());
@@ -1069,6 +1096,7 @@ int mrd_phase_begin(mrd_mesh *m, double t_end, void *stream) {
   if (!m) return fail(MRD_EINVAL, "null argument");
   if (!m->has_state) return fail(MRD_EINVAL, "no state set");
   if (m->in_phases) return fail(MRD_EINVAL, "mrd_phase_begin called twice");
+  if (m->L.p.scheme == MRD_SCHEME_BX) return fail(MRD_EINVAL, "the Bx blend needs the speed range of the whole mesh: not available in phases");
   cudaStream_t s = (cudaStream_t)stream;
   mrd::Ctl c{};
   int rc = fetch_ctl(m, s, &c);

@@ -19,7 +19,15 @@ struct Ctl {
   int active;                    // 1 while the step in flight has to be done
   int bvar;                      // blend variant of scheme B (L503): 0 = diagonal Theta, 1 = Bmax, 2 = Bmin
   int lumping;                   // 0 = global lumping (L576), 1 = selective lumping (eq. 66-67)
+  // Bx (eq. 56): domain size and the bit patterns of max / min vertex speed of the state of stage 1 ([0]) and 2 ([1])
+  double bx_L;
+  unsigned long long vmax_bits[2], vmin_bits[2];
 };
+// 1 / (|v|_max - |v|_min) of stage `k`, 0 when the speeds are all equal (reading C24)
+__device__ __forceinline__ double bx_inv_range(const Ctl *c, int k) {
+  double r = __longlong_as_double((long long)c->vmax_bits[k]) - __longlong_as_double((long long)c->vmin_bits[k]);
+  return r > 0.0 ? 1.0 / r : 0.0;
+}
 
 template <class R> struct MeshDev {
   int64_t nv, nt;
@@ -83,6 +91,8 @@ __global__ void ctl_kernel(Ctl *c, int mode, double t_end, const int *flag) {
     }
   }
   c->dmin_bits = 0x7FF0000000000000ull;  // +inf
+  c->vmax_bits[0] = c->vmax_bits[1] = 0ull;
+  c->vmin_bits[0] = c->vmin_bits[1] = 0x7FF0000000000000ull;
   c->active = (c->status == 0 && !(c->t_end > 0.0 && c->t >= c->t_end)) ? 1 : 0;
 }
 
@@ -158,6 +168,12 @@ tri_stage1_kernel(MeshDev<R> m, R gamma, const Ctl *__restrict__ ctl, const Vec4
     apply_beta(gamma, k, g, pT, pL);
     if (SCHEME == MRD_SCHEME_B) {
       blend(pT, pN, pL, ctl->bvar);
+    } else if (SCHEME == MRD_SCHEME_BX) {
+      const R th = bx_theta(z, g, __ldg(m.area3 + t), __ldg(m.lmax + t), (R)ctl->bx_L, (R)bx_inv_range(ctl, 0));
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) pN[i][c] = pL[i][c] + th * (pN[i][c] - pL[i][c]);
     } else {
 #pragma unroll
       for (int i = 0; i < 3; ++i)
@@ -228,6 +244,12 @@ tri_stage2_kernel(MeshDev<R> m, R gamma, const Ctl *__restrict__ ctl, const Vec4
     }
     if (SCHEME == MRD_SCHEME_B) {
       blend(PT, pN, pL, ctl->bvar);
+    } else if (SCHEME == MRD_SCHEME_BX) {  // the sensor of W*, the state the matrices are evaluated at (as C12)
+      const R th = bx_theta(z, g, a3, __ldg(m.lmax + t), (R)ctl->bx_L, (R)bx_inv_range(ctl, 1));
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) pN[i][c] = pL[i][c] + th * (pN[i][c] - pL[i][c]);
     } else {
 #pragma unroll
       for (int i = 0; i < 3; ++i)
@@ -280,6 +302,34 @@ gather_dt_kernel(MeshDev<R> m, Ctl *__restrict__ ctl, const Vec4<R> *__restrict_
     if (!(m.frozen && m.frozen[i] == 2)) d = 2.0 * (double)__ldg(m.vol + i) / (double)S;  // halo: fan incomplete here
   }
   block_min_to_global(d, &ctl->dmin_bits);
+}
+
+// Bx (eq. 56, reading C24): max and min of the vertex speeds |v_i| of the state W, into slot `k` of the control block
+template <class R>
+__global__ void __launch_bounds__(256) vrange_kernel(int64_t nv, const Vec4<R> *__restrict__ W, Ctl *__restrict__ ctl, int k) {
+  MRD_CTL_GUARD(ctl)
+  double hi = 0.0, lo = __longlong_as_double(0x7FF0000000000000ll);
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nv; i += (int64_t)gridDim.x * blockDim.x) {
+    Vec4<R> w = ld4(&W[i]);
+    double u = (double)w.y / (double)w.x, v = (double)w.z / (double)w.x;
+    double a = sqrt(u * u + v * v);
+    hi = fmax(hi, a);
+    lo = fmin(lo, a);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    hi = fmax(hi, __shfl_xor_sync(0xFFFFFFFFu, hi, o));
+    lo = fmin(lo, __shfl_xor_sync(0xFFFFFFFFu, lo, o));
+  }
+  __shared__ double shi[8], slo[8];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (lane == 0) { shi[w] = hi; slo[w] = lo; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int q = 1; q < 8; ++q) { hi = fmax(hi, shi[q]); lo = fmin(lo, slo[q]); }
+    atomicMax(&ctl->vmax_bits[k], (unsigned long long)__double_as_longlong(hi));  // non-negative doubles order like their bits
+    atomicMin(&ctl->vmin_bits[k], (unsigned long long)__double_as_longlong(lo));
+  }
 }
 
 // finish a vertex: W_new = W_old - dt/V * acc (eq. 43 / 60 / 61); frozen vertices keep W_old (their

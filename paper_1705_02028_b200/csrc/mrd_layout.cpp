@@ -103,7 +103,7 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
   if (!p || !xy || !tri || nv < 3 || nt < 1) { err = "null or empty mesh"; return MRD_EINVAL; }
   if (nv > 0x7FFFFFF0ll || 3 * nt > 0x7FFFFFF0ll) { err = "mesh too large for 32-bit indices"; return MRD_EINVAL; }
   if (!(p->gamma > 1.0) || !(p->cfl > 0.0)) { err = "gamma must be > 1 and cfl > 0"; return MRD_EINVAL; }
-  if (p->scheme < 0 || p->scheme > 4 || (p->time_order != 1 && p->time_order != 2)) { err = "bad scheme/time_order"; return MRD_EINVAL; }
+  if (p->scheme < 0 || p->scheme > 5 || (p->time_order != 1 && p->time_order != 2)) { err = "bad scheme/time_order"; return MRD_EINVAL; }
   if (p->precision != MRD_FP64 && p->precision != MRD_FP32) { err = "bad precision"; return MRD_EINVAL; }
   if (p->lumping != 0 && p->lumping != 1) { err = "lumping must be 0 (global) or 1 (selective)"; return MRD_EINVAL; }
   if (p->period_x < 0.0 || p->period_y < 0.0) { err = "negative period"; return MRD_EINVAL; }
@@ -113,6 +113,16 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
   L.nv = nv; L.nt = nt; L.ne = ne;
   const double period[2] = {p->period_x, p->period_y};
 
+  {  // domain size L of the Bx sensor (eq. 56, reading C25): larger side of the bounding box, the period where periodic
+    double lo[2] = {xy[0], xy[1]}, hi[2] = {xy[0], xy[1]};
+    for (int64_t i = 0; i < nv; ++i)
+      for (int d = 0; d < 2; ++d) {
+        lo[d] = std::min(lo[d], xy[2 * i + d]);
+        hi[d] = std::max(hi[d], xy[2 * i + d]);
+      }
+    const double sx = period[0] > 0.0 ? period[0] : hi[0] - lo[0], sy = period[1] > 0.0 ? period[1] : hi[1] - lo[1];
+    L.domain_size = std::max(sx, sy);
+  }
   // ---- validation + orientation fix in USER numbering ------------------------------------------
   std::vector<int32_t> utri(tri, tri + 3 * nt);
   std::vector<uint8_t> uswap(nt, 0);

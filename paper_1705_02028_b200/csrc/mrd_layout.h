@@ -13,6 +13,7 @@
 struct mrd_layout {
   mrd_params p{};
   int64_t nv = 0, nt = 0, ne = 0, nf = 0;
+  double domain_size = 1.0;           // L of eq. 56 (Bx)
   // renumbering: internal k <-> user index
   std::vector<int32_t> vperm, vrank;  // vperm[k] = user vertex of internal k; vrank = inverse
   std::vector<int32_t> tperm, trank;

@@ -415,6 +415,24 @@ template <class R> __device__ __forceinline__ void blend_theta(const R X[4], con
     th[0] = th[1] = th[2] = th[3] = t;
   }
 }
+// Bx (eq. 54-56; readings C23-C26): theta = min(1, s^2 l_max / L), s = (-L div v / (|v|_max - |v|_min))^+,
+// div v of the linear interpolant of the vertex velocities = sum_j (u_j . n_j) l_j / (2|T|) (inward normals).
+// Z = sqrt(rho) (1, u, v, h), so u_j = Z_j.y / Z_j.x.  area3 = |T|/3, hl = l/2; inv_range = 1 / (|v|_max - |v|_min) or 0.
+template <class R>
+__device__ __forceinline__ R bx_theta(const Vec4<R> z[3], const TriGeom<R> &g, R area3, R lmax, R Ldom, R inv_range) {
+  using F = Fast<R>;
+  R acc = R(0);
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    R iz = F::rcp(z[j].x);
+    acc = F::fma_(F::fma_(z[j].y * iz, g.nx[j], (z[j].z * iz) * g.ny[j]), g.hl[j], acc);
+  }
+  R div = acc * F::rcp(R(3) * area3);
+  R s = F::max(R(0), -(Ldom * div) * inv_range);
+  R t = s * s * (lmax * F::rcp(Ldom));
+  return t < R(1) ? t : R(1);
+}
+
 template <class R> __device__ __forceinline__ void blend(const R X[4], R N[3][4], const R L[3][4], int bvar) {
   R th[4];
   blend_theta(X, N, bvar, th);

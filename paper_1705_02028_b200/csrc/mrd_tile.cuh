@@ -223,6 +223,7 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
   __syncthreads();
   int2 n0 = make_int2(0, 0), n1 = make_int2(0, 0);
   const int bvar = ctl->bvar;
+  const R bxL = (R)ctl->bx_L, bxInv = SCHEME == MRD_SCHEME_BX ? (R)bx_inv_range(ctl, STAGE - 1) : R(0);
   constexpr bool lump = STAGE == 2 && STORE;
   bool bad = false;  // linearised c^2 <= 0 met by this thread (raised once, after the loop)
   for (int k = 0; b < td.ntile; b += gridDim.x, ++k) {
@@ -308,6 +309,8 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
       // produced node by node and blended in place -- 24 fewer values live at once than blending from registers.
       R th[4] = {0, 0, 0, 0};
       if (SCHEME == MRD_SCHEME_B) blend_theta(X, pN, bvar, th);  // eq. 53 (+ C10); Bmax / Bmin: L503
+      if (SCHEME == MRD_SCHEME_BX)                               // eq. 54-56: one theta from the shock sensor of this stage's state
+        th[0] = th[1] = th[2] = th[3] = bx_theta(z, g, a3, lmax, bxL, bxInv);
 #pragma unroll
       for (int c = 0; c < 4; ++c)
 #pragma unroll
@@ -336,7 +339,7 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
 #pragma unroll
           for (int c = 0; c < 4; ++c) {
             R *r = res + (i * 4 + c) * T + tid;
-            *r = SCHEME == MRD_SCHEME_B ? Lw[c] + th[c] * (*r - Lw[c]) : Lw[c];
+            *r = (SCHEME == MRD_SCHEME_B || SCHEME == MRD_SCHEME_BX) ? Lw[c] + th[c] * (*r - Lw[c]) : Lw[c];
           }
         }
       }
