@@ -101,7 +101,7 @@ class OracleMesh:
 
     def __del__(self):
         h, self._h = getattr(self, "_h", None), None
-        if h:
+        if h and lib is not None:      # (module globals are already gone at interpreter shutdown)
             lib().orc_mesh_destroy(h)
 
     def set_threads(self, n):
