@@ -1,4 +1,4 @@
-"""The N > 1 path on the GPU: a `DistributedMesh` over 2 and 3 ranks (separate processes, gloo backend, all
+"""The N > 1 path on the GPU: a `DistributedMesh` over 2, 3 and 4 ranks (separate processes, gloo backend, all
 on the one GPU of the box, halo rows staged through host memory) against the CPU oracle on the WHOLE mesh, element
 by element, and against the single-mesh run of the same library (they differ by summation order only).
 Tolerances as tests/test_gpu_parity.py."""
@@ -53,7 +53,7 @@ def single():
     return ref
 
 
-@pytest.mark.parametrize("world", [2, 3])
+@pytest.mark.parametrize("world", [2, 3, 4])
 def test_distributed_mesh_matches_oracle_and_single_mesh(world, single, tmp_path):
     res = _run(world, tmp_path)
     for name, ref in single.items():
