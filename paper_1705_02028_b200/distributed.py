@@ -76,6 +76,8 @@ class DistributedMesh:
         import torch.distributed as dist
         self._torch, self._dist, self.group = torch, dist, group
         self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        if params.get("scheme") == 5:
+            raise ValueError("the Bx blend (scheme 5) needs the speed range of the whole mesh and is not available on a partitioned mesh")
         period = params.get("period", (0.0, 0.0))
         P = self.part = Partition(xy, tri, self.world, self.rank, vertex_flag=vertex_flag, wall_edge=wall_edge, period=period)
         self.mesh = Mesh(P.xy, P.tri, vertex_flag=P.vertex_flag, wall_edge=P.wall_edge if P.n_wall else None, **params)
