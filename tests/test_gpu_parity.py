@@ -475,3 +475,14 @@ def test_bx_on_the_sod_tube_with_walls_and_frozen_ends(mrd):
         gm.set_state(torch.tensor(om.get_state(), device="cuda"))
     with pytest.raises(mrd.MrdError):      # a partitioned mesh has no global speed range
         gm.phase_begin()
+
+
+@pytest.mark.parametrize("scheme", [2, 5])
+def test_fp32_on_the_variable_valence_mesh(mrd, scheme):
+    mesh = wl.flip_edges(wl.jitter_mesh(wl.uniform_mesh(40, 36, 2.0, 1.8, periodic=True), 0.2, seed=3), seed=11)
+    W = wl.random_smooth_state(mesh, mach=0.8, seed=6)
+    gm = gpu_mesh(mrd, mesh, W, scheme=scheme, precision=1)
+    om = orc_mesh(mesh, W, scheme=scheme)
+    gm.step(10)
+    om.step(10)
+    assert field_errors(gm.get_state().cpu().numpy().astype(np.float64), om.get_state()) <= TOL_F32

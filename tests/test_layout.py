@@ -127,3 +127,20 @@ def test_mesh_create_fails_loudly_without_gpu():
     rc = mrd.lib().mrd_mesh_create(C.byref(h), C.byref(p), mesh.nv, xy.ctypes.data_as(C.POINTER(C.c_double)), mesh.nt,
                                    tri.ctypes.data_as(C.POINTER(C.c_int32)), None, 0, None)
     assert rc == mrd.MRD_ECUDA and b"no CPU fallback" in mrd.lib().mrd_last_error()
+
+
+def test_maximum_size_is_checked_before_anything_is_read():
+    """Indices are 32-bit (int32 suffices up to 3 nt < 2^31): larger counts are refused up front, for the layout
+    stage and for the partitioner alike (the arrays passed here are tiny: nothing may be read before the check)."""
+    import ctypes as C
+    L = mrd.lib()
+    xy = np.zeros((3, 2))
+    tri = np.zeros((1, 3), np.int32)
+    p = mrd.binding.make_params()
+    dp, ip = C.POINTER(C.c_double), C.POINTER(C.c_int32)
+    for nv, nt in ((2 ** 31, 1), (3, 2 ** 30)):            # nv too large; 3 nt too large
+        h = C.c_void_p()
+        rc = L.mrd_layout_create(C.byref(h), C.byref(p), nv, xy.ctypes.data_as(dp), nt, tri.ctypes.data_as(ip), None, 0, None)
+        assert rc == mrd.MRD_EINVAL and b"32-bit" in L.mrd_last_error()
+        rc = L.mrd_partition_create(C.byref(h), nv, xy.ctypes.data_as(dp), nt, tri.ctypes.data_as(ip), None, 0, None, 0.0, 0.0, 2, 0)
+        assert rc == mrd.MRD_EINVAL and b"32-bit" in L.mrd_last_error()
