@@ -4,14 +4,15 @@
 //
 //   stage-in : everything a tile needs lives in CONTIGUOUS global ranges (slot-major copies of Z, |v|+c,
 //              dW/dt written by the vertex kernels; tile-frame coordinates; the tile's plan record; for
-//              stage 2 the stored phi^N(W^n), phi^T(W^n)), so one elected thread brings the NEXT tile in
-//              with a handful of TMA bulk copies (cp.async.bulk + mbarrier complete_tx) while the block
-//              computes the current one -- no gather by vertex index, no dependent global latency;
+//              stage 2 the stored phi^N(W^n), phi^T(W^n)), so one thread brings the tile AFTER NEXT in with a
+//              handful of TMA bulk copies (cp.async.bulk + mbarrier complete_tx) as soon as the last warp has
+//              left the buffer it goes into -- no gather by vertex index, no dependent global latency;
 //   body     : one thread per triangle; geometry of eq. 35 (L397-L399) from the staged coordinates, then
 //              S2-S5 / S9 of SURVEY 8a with the same device functions as the unfused kernels;
 //   epilogue : distributed residuals -> shared memory; every slot sums its incident (triangle, node) entries
 //              in ascending order; ONE partial per slot leaves the SM (deterministic; replaces the float
-//              atomics of L734 and the 3 x 4 values per triangle of the unfused design).
+//              atomics of L734 and the 3 x 4 values per triangle of the unfused design).  One block barrier
+//              per tile (between the residuals and their sums); warps that are done move on to the next tile.
 // The vertex kernels add a vertex's few partials (ascending slot = ascending triangle order) and scatter
 // the new per-vertex quantities back to the vertex's slots.
 #pragma once
