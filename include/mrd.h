@@ -39,8 +39,8 @@ enum {
 enum { MRD_SCHEME_N = 0, MRD_SCHEME_LDA = 1, MRD_SCHEME_B = 2,      /* eq. 48-49 / 50-51 / 52-53 */
        MRD_SCHEME_BMAX = 3, MRD_SCHEME_BMIN = 4,                     /* B with all Theta_kk = their max / min (L503) */
        MRD_SCHEME_BX = 5 };  /* scalar blend from the shock sensor of eq. 54-56 (L505-L517; readings C23-C26 of DESIGN.md):
-                                one more pass over the vertices per stage for |v|_max - |v|_min; not available on a
-                                partitioned mesh (mrd_phase* returns MRD_EINVAL) */
+                                one more pass over the vertices per stage for |v|_max - |v|_min; on a partitioned mesh
+                                the caller reduces that range over all parts (mrd_range_get / mrd_range_set) */
 enum { MRD_FP64 = 0, MRD_FP32 = 1 };
 
 typedef struct mrd_mesh mrd_mesh;     /* opaque: mesh layout + device state + stepper */
@@ -234,6 +234,13 @@ int mrd_dt_set(mrd_mesh *m, const double *d_dev, void *stream);
  * state just written by the preceding UPDATE1 / STAGE2 phase.  Unpack also derives what the triangle kernels
  * read (Z, and dW/dt of eq. 57 or |v| + c) exactly as the owner did, so halo copies are bitwise the owner's. */
 int mrd_halo_pack(mrd_mesh *m, void *buf_dev, void *stream);
+/* MRD_SCHEME_BX in phases: the sensor of eq. 56 needs |v|_max - |v|_min over the WHOLE mesh (reading C24).
+ * mrd_range_get: d DEVICE double[2] = (|v|_max, -|v|_min) over this part's vertices (halo copies included: they are
+ * some part's vertices) of the state that stage `stage` reads -- stage 1: W^n, call after mrd_phase_begin and after
+ * every mrd_phase(END); stage 2: W*, call after the halo unpack that follows mrd_phase(UPDATE1).  After a
+ * max-reduction of both doubles over all parts, mrd_range_set installs the result for that stage. */
+int mrd_range_get(mrd_mesh *m, int32_t stage, double *d_dev, void *stream);
+int mrd_range_set(mrd_mesh *m, int32_t stage, const double *d_dev, void *stream);
 int mrd_halo_unpack(mrd_mesh *m, const void *buf_dev, void *stream);
 
 /* Kernel launch counter: number of the library's own kernel launches since the mesh was created. */

@@ -74,6 +74,8 @@ def lib():
         L.mrd_dt_get.argtypes = [vp, vp, vp]
         L.mrd_dt_set.argtypes = [vp, vp, vp]
         L.mrd_halo_pack.argtypes = [vp, vp, vp]
+        L.mrd_range_get.argtypes = [vp, C.c_int32, vp, vp]
+        L.mrd_range_set.argtypes = [vp, C.c_int32, vp, vp]
         L.mrd_halo_unpack.argtypes = [vp, vp, vp]
         L.mrd_last_error.restype = C.c_char_p
         L.mrd_version.restype = C.c_char_p
@@ -319,6 +321,14 @@ class Mesh:
     def dt_set(self, d, stream=None):
         self._check_buf(d, 2, self._torch.float64)
         _check(lib().mrd_dt_set(self._h, C.c_void_p(d.data_ptr()), _stream_ptr(stream)))
+
+    def range_get(self, stage, d, stream=None):
+        self._check_buf(d, 2, self._torch.float64)
+        _check(lib().mrd_range_get(self._h, int(stage), C.c_void_p(d.data_ptr()), _stream_ptr(stream)))
+
+    def range_set(self, stage, d, stream=None):
+        self._check_buf(d, 2, self._torch.float64)
+        _check(lib().mrd_range_set(self._h, int(stage), C.c_void_p(d.data_ptr()), _stream_ptr(stream)))
 
     def halo_pack(self, buf, stream=None):
         self._check_buf(buf, 4 * self.n_send, self.dtype)

@@ -429,7 +429,7 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
   const unsigned vb = blocks_for(md.nv, 256);
   const bool fused = m->fused;
   if (mask & (1 << MRD_PHASE_RESIDUAL1)) {
-    if (scheme == MRD_SCHEME_BX) {  // eq. 56: |v|_max - |v|_min of W^n
+    if (scheme == MRD_SCHEME_BX && !m->in_phases) {  // eq. 56: |v|_max - |v|_min of W^n (in phases: mrd_range_get / _set)
       mrd::vrange_kernel<R><<<std::min<unsigned>(vb, (unsigned)m->nsm * 8), 256, 0, s>>>(md.nv, (const V4 *)m->d_W[a], m->d_ctl, 0);
       m->launches++;
     }
@@ -481,7 +481,7 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
     PROF_MARK(MRD_PROF_UPDATE)
   }
   if (rk2 && (mask & (1 << MRD_PHASE_STAGE2))) {
-    if (scheme == MRD_SCHEME_BX) {  // ... and of W*
+    if (scheme == MRD_SCHEME_BX && !m->in_phases) {  // ... and of W*
       mrd::vrange_kernel<R><<<std::min<unsigned>(vb, (unsigned)m->nsm * 8), 256, 0, s>>>(md.nv, (const V4 *)m->d_W[b], m->d_ctl, 1);
       m->launches++;
     }
@@ -1096,7 +1096,6 @@ int mrd_phase_begin(mrd_mesh *m, double t_end, void *stream) {
   if (!m) return fail(MRD_EINVAL, "null argument");
   if (!m->has_state) return fail(MRD_EINVAL, "no state set");
   if (m->in_phases) return fail(MRD_EINVAL, "mrd_phase_begin called twice");
-  if (m->L.p.scheme == MRD_SCHEME_BX) return fail(MRD_EINVAL, "the Bx blend needs the speed range of the whole mesh: not available in phases");
   cudaStream_t s = (cudaStream_t)stream;
   mrd::Ctl c{};
   int rc = fetch_ctl(m, s, &c);
@@ -1158,6 +1157,32 @@ int mrd_dt_set(mrd_mesh *m, const double *d_dev, void *stream) {
   if (!m || !d_dev) return fail(MRD_EINVAL, "null argument");
   if (!m->in_phases || m->phase_next != MRD_PHASE_UPDATE1) return fail(MRD_EINVAL, "mrd_dt_set must follow mrd_phase(RESIDUAL1)");
   mrd::dt_set_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(m->d_ctl, m->d_flag, d_dev);
+  m->launches++;
+  CUDA_TRY(cudaGetLastError());
+  return MRD_OK;
+}
+
+int mrd_range_get(mrd_mesh *m, int32_t stage, double *d_dev, void *stream) {
+  if (!m || !d_dev || (stage != 1 && stage != 2)) return fail(MRD_EINVAL, "bad argument");
+  if (!m->in_phases) return fail(MRD_EINVAL, "mrd_range_get outside mrd_phase_begin / mrd_phase_end");
+  cudaStream_t s = (cudaStream_t)stream;
+  // stage 1: the state the next RESIDUAL1 reads (W^n); stage 2: W* written by UPDATE1 (and the halo unpack after it)
+  const int pair = stage == 1 ? m->phase_a : (m->phase_a ^ 1);
+  const unsigned vb = blocks_for(m->L.nv, 256), nb = std::min<unsigned>(vb, (unsigned)m->nsm * 8);
+  mrd::range_reset_kernel<<<1, 1, 0, s>>>(m->d_ctl, stage - 1);
+  if (m->L.p.precision == MRD_FP64)
+    mrd::vrange_kernel<double><<<nb, 256, 0, s>>>(m->L.nv, (const mrd::Vec4<double> *)m->d_W[pair], m->d_ctl, stage - 1);
+  else
+    mrd::vrange_kernel<float><<<nb, 256, 0, s>>>(m->L.nv, (const mrd::Vec4<float> *)m->d_W[pair], m->d_ctl, stage - 1);
+  mrd::range_get_kernel<<<1, 1, 0, s>>>(m->d_ctl, stage - 1, d_dev);
+  m->launches += 3;
+  CUDA_TRY(cudaGetLastError());
+  return MRD_OK;
+}
+int mrd_range_set(mrd_mesh *m, int32_t stage, const double *d_dev, void *stream) {
+  if (!m || !d_dev || (stage != 1 && stage != 2)) return fail(MRD_EINVAL, "bad argument");
+  if (!m->in_phases) return fail(MRD_EINVAL, "mrd_range_set outside mrd_phase_begin / mrd_phase_end");
+  mrd::range_set_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(m->d_ctl, stage - 1, d_dev);
   m->launches++;
   CUDA_TRY(cudaGetLastError());
   return MRD_OK;

@@ -332,6 +332,21 @@ __global__ void __launch_bounds__(256) vrange_kernel(int64_t nv, const Vec4<R> *
   }
 }
 
+// Bx on a partitioned mesh: the local range of stage k as d = (|v|_max, -|v|_min) -- a max-reduction over all parts of both
+// numbers gives the global range -- and back
+__global__ void range_reset_kernel(Ctl *c, int k) {
+  c->vmax_bits[k] = 0ull;
+  c->vmin_bits[k] = 0x7FF0000000000000ull;
+}
+__global__ void range_get_kernel(const Ctl *__restrict__ c, int k, double *__restrict__ d) {
+  d[0] = __longlong_as_double((long long)c->vmax_bits[k]);
+  d[1] = -__longlong_as_double((long long)c->vmin_bits[k]);
+}
+__global__ void range_set_kernel(Ctl *__restrict__ c, int k, const double *__restrict__ d) {
+  c->vmax_bits[k] = (unsigned long long)__double_as_longlong(d[0]);
+  c->vmin_bits[k] = (unsigned long long)__double_as_longlong(-d[1]);
+}
+
 // finish a vertex: W_new = W_old - dt/V * acc (eq. 43 / 60 / 61); frozen vertices keep W_old (their
 // initial state, L582); then Z and the signal speed of the new state (S1, S6), positivity check.
 template <class R, bool WANT_DWDT>

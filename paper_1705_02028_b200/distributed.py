@@ -56,13 +56,19 @@ class HaloExchange:
             recv.copy_(dst)
 
     def allreduce_min(self, d):
+        self._allreduce(d, self._dist.ReduceOp.MIN)
+
+    def allreduce_max(self, d):
+        self._allreduce(d, self._dist.ReduceOp.MAX)
+
+    def _allreduce(self, d, op):
         dist = self._dist
         if self.staged:
             h = d.cpu()
-            dist.all_reduce(h, op=dist.ReduceOp.MIN, group=self.group)
+            dist.all_reduce(h, op=op, group=self.group)
             d.copy_(h)
         else:
-            dist.all_reduce(d, op=dist.ReduceOp.MIN, group=self.group)
+            dist.all_reduce(d, op=op, group=self.group)
 
 
 class DistributedMesh:
@@ -76,8 +82,6 @@ class DistributedMesh:
         import torch.distributed as dist
         self._torch, self._dist, self.group = torch, dist, group
         self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
-        if params.get("scheme") == 5:
-            raise ValueError("the Bx blend (scheme 5) needs the speed range of the whole mesh and is not available on a partitioned mesh")
         period = params.get("period", (0.0, 0.0))
         P = self.part = Partition(xy, tri, self.world, self.rank, vertex_flag=vertex_flag, wall_edge=wall_edge, period=period)
         self.mesh = Mesh(P.xy, P.tri, vertex_flag=P.vertex_flag, wall_edge=P.wall_edge if P.n_wall else None, **params)
@@ -89,6 +93,8 @@ class DistributedMesh:
         self._recv = torch.empty(4 * P.n_recv, dtype=self.dtype, device="cuda")
         self._d = torch.empty(2, dtype=torch.float64, device="cuda")
         self._rk2 = self.mesh.params.time_order == 2
+        self._bx = self.mesh.params.scheme == 5   # Bx: the speed range of eq. 56 is reduced over all parts
+        self._r = torch.empty(2, dtype=torch.float64, device="cuda")
         self._open = False
 
     def close(self):
@@ -136,6 +142,12 @@ class DistributedMesh:
         self.comm.exchange(self._send, self._recv)
         m.halo_unpack(self._recv)
 
+    def _range(self, stage):
+        m = self.mesh
+        m.range_get(stage, self._r)
+        self.comm.allreduce_max(self._r)
+        m.range_set(stage, self._r)
+
     def _one_step(self):
         m = self.mesh
         m.phase(m.PHASE_RESIDUAL1)
@@ -145,14 +157,20 @@ class DistributedMesh:
         m.phase(m.PHASE_UPDATE1)
         self._exchange()
         if self._rk2:
+            if self._bx:
+                self._range(2)
             m.phase(m.PHASE_STAGE2)
             self._exchange()
         m.phase(m.PHASE_END)
+        if self._bx:
+            self._range(1)
 
     def step_async(self, n_steps):
         """Enqueue n steps without the final synchronisation (timing loops); follow with sync()."""
         if not self._open:
             self.mesh.phase_begin(0.0)
+            if self._bx:
+                self._range(1)
             self._open = True
         for _ in range(int(n_steps)):
             self._one_step()
@@ -171,6 +189,8 @@ class DistributedMesh:
         while left > 0:
             chunk = min(left, 32) if t_end > 0.0 else left
             self.mesh.phase_begin(t_end)
+            if self._bx:
+                self._range(1)
             for _ in range(chunk):
                 self._one_step()
             n, t, dt = self.mesh.phase_end()

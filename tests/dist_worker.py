@@ -29,6 +29,8 @@ def cases():
                           dict(scheme=1, time_order=2, reorder=False, tile=64), 10, 0.0)
     f = wl.flip_edges(wl.jitter_mesh(wl.uniform_mesh(40, 36, 2.0, 1.8, periodic=True), 0.2, seed=3), seed=11)
     out["variable_valence_b2"] = (f, wl.random_smooth_state(f, mach=0.8, seed=6), None, None, dict(scheme=2, time_order=2), 10, 0.0)
+    out["variable_valence_bx"] = (f, wl.random_smooth_state(f, mach=1.1, seed=6), None, None, dict(scheme=5, time_order=2), 10, 0.0)
+    out["vortex_bx_n1"] = (m, wl.vortex_state(m, advect=(0.3, 0.1)), None, None, dict(scheme=5, time_order=1), 6, 0.0)
     r = wl.make_config("riemann4", n=40)
     out["riemann4_frozen"] = (r.mesh, r.W0, r.vertex_flag, None, dict(scheme=2, time_order=2), 6, 0.0)
     return out
