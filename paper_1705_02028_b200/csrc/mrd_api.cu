@@ -516,25 +516,28 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
 
 // n consecutive steps starting from buffer pair `a` (updated).  Small meshes replay a captured two-step graph.
 template <class R> int run_steps(mrd_mesh *m, int scheme, int64_t n, int &a, cudaStream_t s) {
-  if (!m->graph_ok || n < 4) {
+  if (!m->graph_ok || n < 2) {
     for (int64_t k = 0; k < n; ++k, a ^= 1) enqueue_step<R>(m, scheme, a, s);
     return MRD_OK;
   }
   CUDA_TRY(cudaEventRecord(m->ev_in, s));
   CUDA_TRY(cudaStreamWaitEvent(m->s_int, m->ev_in, 0));
-  if (!m->gexec[a]) {
-    enqueue_step<R>(m, scheme, a, m->s_int);  // eager once: sets the kernels' shared-memory attributes before the capture
+  if (!m->gexec[0] || !m->gexec[1]) {
+    // first multi-step call: one eager step (sets the kernels' shared-memory attributes before any capture), then the
+    // graphs of BOTH starting parities, so that no later call -- a timed one, say -- pays for an instantiation
+    enqueue_step<R>(m, scheme, a, m->s_int);
     a ^= 1;
     --n;
-    if (!m->gexec[a]) {
+    for (int p = 0; p < 2; ++p) {
+      if (m->gexec[p]) continue;
       const int64_t lc = m->launches;
       cudaGraph_t g = nullptr;
       CUDA_TRY(cudaStreamBeginCapture(m->s_int, cudaStreamCaptureModeThreadLocal));
-      enqueue_step<R>(m, scheme, a, m->s_int);
-      enqueue_step<R>(m, scheme, a ^ 1, m->s_int);
+      enqueue_step<R>(m, scheme, p, m->s_int);
+      enqueue_step<R>(m, scheme, p ^ 1, m->s_int);
       CUDA_TRY(cudaStreamEndCapture(m->s_int, &g));
       m->launches = lc;  // captured, not launched
-      cudaError_t e = cudaGraphInstantiate(&m->gexec[a], g, 0);
+      cudaError_t e = cudaGraphInstantiate(&m->gexec[p], g, 0);
       cudaGraphDestroy(g);
       if (e != cudaSuccess) return fail(MRD_ECUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e));
     }

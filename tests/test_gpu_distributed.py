@@ -92,3 +92,31 @@ def test_bench_n2_runs_one_mesh_over_two_ranks():
     assert d["config"]["n_triangles"] == 2 * 2 * 256 * 256 and "one mesh over 2 GPUs" in d["config"]["parallelism"]
     assert d["config"]["n_triangles_rank0"] > 2 * 256 * 256          # its square plus the cut triangles of both cut lines
     assert d["e2e"]["h2d_bytes_per_step"] > 0 and d["roofline"]["kernel"].startswith("tri_stage")
+
+
+def test_bench_line_carries_every_key_of_the_contract():
+    """python bench.py (N = 1) at a small size: one JSON line with the contract's keys, the roofline and the CPU baseline."""
+    import json
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--size", "256", "--steps", "4", "--warmup", "3"],
+                       capture_output=True, text=True, timeout=900, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-3000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline",
+                "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+        assert key in d, key
+    assert d["metric"] == "triangle_updates_per_s_rk2_step" and d["n_gpus"] == 1 and d["steps"] == 4 and d["warmup"] == 3
+    assert d["dtype"] == "f64" and d["data"] == "synthetic" and d["higher_is_better"] is True and d["vs_baseline"] is None
+    assert "workload" in d["config"] and d["value"] == pytest.approx(d["config"]["n_triangles"] * 1e3 / d["ms_per_step"], rel=1e-6)
+    assert d["gpu_launches"] >= 6 * 4                                   # six kernels per RK2 step
+    for key in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step"):
+        assert key in d["e2e"], key
+    assert d["e2e"]["h2d_bytes_per_step"] == 4 * 256 * 256 * 8 and 0 < d["e2e"]["value"] < d["value"]
+    for key in ("bound", "achieved", "peak", "unit", "frac", "traffic"):
+        assert key in d["roofline"], key
+    assert d["roofline"]["bound"] in ("alu", "hbm") and d["roofline"]["frac"] == pytest.approx(d["roofline"]["achieved"] / d["roofline"]["peak"])
+    for key in ("sm_mhz", "sm_max_mhz", "reasons"):
+        assert key in d["clocks"], key
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["unit"] == d["unit"] and c["sample"]
