@@ -245,8 +245,10 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
     const int64_t t = b * T + tid;
     R pN[3][4];
     R st = R(0);
-    if (t < td.nt) {
-      const ushort4 lv = reinterpret_cast<const ushort4 *>(plan)[tid];
+    // (no branch around the body: a padding triangle of the last tile computes on triangle 0 and its results are zeroed)
+    const bool valid = t < td.nt;
+    {
+      const ushort4 lv = reinterpret_cast<const ushort4 *>(plan)[valid ? tid : 0];
       const int l[3] = {lv.x, lv.y, lv.z};
       Vec4<R> z[3] = {sZ[l[0]], sZ[l[1]], sZ[l[2]]};
       TriGeom<R> g;
@@ -344,7 +346,7 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
           }
         }
       }
-      if (STAGE == 1 && phi_dbg) {
+      if (STAGE == 1 && phi_dbg && valid) {
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
           const R *r = res + (i * 4) * T + tid;
@@ -352,9 +354,11 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
         }
         sT_dbg[t] = st;
       }
-    } else {  // padding thread of the last tile: contributes nothing
+    }
+    if (!valid) {  // padding thread of the last tile: contributes nothing
 #pragma unroll
       for (int i = 0; i < 12; ++i) res[i * T + tid] = R(0);
+      st = R(0);
     }
     if (STAGE == 1) sSTc[tid] = st;
     __syncthreads();
