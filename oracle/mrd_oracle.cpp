@@ -10,8 +10,9 @@
 // R R^-1 = I, A10-A25 == R diag(l) R^-1, Simpson contour integral of the flux, sum(beta_i) = I,
 // sum(phi_i^N) = phi^T, symmetrising-variable block form, stagnation limit, uniform flow == 0 exactly,
 // conservation, permutation invariance, Heun reduction, Sod vs exact Riemann solution, vortex order ~ 2.
-// Wall boundary term (eq. 68-71): pinned by v_n = 0 -> 0, by the mass balance and by the oblique-wall
-// uniform-flow test; its stage-2 averaging is reading C15 ("parity unpinned" beyond those).
+// Wall boundary term (eq. 68-71): pinned by v_n = 0 -> 0, by the mass balance, by the oblique-wall
+// uniform-flow test, and its stage-2 averaging (reading C15) by the Heun reduction of RK2 with scheme N on
+// a mesh with walls and oblique flow (tests/test_oracle_step.py).  No function here is "parity unpinned".
 #include "mrd_oracle.h"
 
 #include <algorithm>

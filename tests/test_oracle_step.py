@@ -123,6 +123,68 @@ def test_rk2_with_scheme_N_is_heun():
     assert np.allclose(om2.get_state(), heun, rtol=0, atol=5e-14)
 
 
+def _wall_sums(mesh, walls, W, gamma=GAMMA, alpha=0.75):
+    """Per-vertex sum of the wall corrections of eq. 68-71 (L586-L602), retyped in numpy from the paper and independent of
+    the oracle's code: F^c = (desired no-through-flow flux) - (computed flux) = -(rho, rho u, rho v, e + p) v_n with the
+    OUTWARD unit normal n; Phi_a = l/2 (alpha F^c_a + (1 - alpha) F^c_b), Phi_b likewise with the weights swapped."""
+    nvx, nvy = mesh.shape
+    acc = np.zeros((mesh.nv, 4))
+    for a, b in walls:
+        ya = mesh.xy[a, 1]
+        n = np.array([0.0, -1.0]) if ya < 0.5 * mesh.lengths[1] else np.array([0.0, 1.0])
+        ln = np.hypot(*(mesh.xy[b] - mesh.xy[a]))
+        Fc = []
+        for i in (a, b):
+            rho, m, nn, e = W[:, i]
+            u, v = m / rho, nn / rho
+            p = (gamma - 1.0) * (e - 0.5 * rho * (u * u + v * v))
+            vn = u * n[0] + v * n[1]
+            Fc.append(-np.array([rho, m, nn, e + p]) * vn)
+        acc[a] += 0.5 * ln * (alpha * Fc[0] + (1.0 - alpha) * Fc[1])
+        acc[b] += 0.5 * ln * ((1.0 - alpha) * Fc[0] + alpha * Fc[1])
+    return acc
+
+
+def test_rk2_with_scheme_N_and_walls_is_heun_with_the_wall_term_averaged():
+    # Pin of reading C15 (stage 2 uses (Phi^c(W^n) + Phi^c(W*)) / 2).  Mathematics, not the oracle's formula: with scheme N
+    # and V_i = sum |T|/3 the two stages of eq. 60-62 are Heun's method for dW_i/dt = -(1/V_i)(sum_T phi_i^N + Phi_i^c), i.e.
+    #   W^{n+1} = W^n - dt/(2 V_i) [sum phi^N(W^n) + sum phi^N(W*) + Phi^c(W^n) + Phi^c(W*)],
+    # which holds only if the stage-2 wall term is the plain average of the two evaluations.  Oblique flow (v_n != 0 on
+    # both walls), no frozen vertices anywhere, so every wall vertex is updated with the term under test.
+    mesh = wl.jitter_mesh(wl.uniform_mesh(12, 7, 2.0, 1.0, periodic=False), 0.15, seed=5)
+    walls = wl.wall_edges_y(mesh)
+    W = wl.random_smooth_state(mesh, mach=0.6, seed=12)
+    on_wall = np.unique(walls.ravel())
+    assert np.abs(W[2, on_wall] / W[0, on_wall]).min() > 1e-3          # v_n != 0 at every wall vertex
+    om1 = oracle.OracleMesh(mesh.xy, mesh.tri, wall_edge=walls, scheme=oracle.SCHEME_N, time_order=1)
+    om1.set_state(W)
+    d0 = om1.dump_stage1()
+    _, vol = om1.geometry()
+    _, _, dt = om1.step(1)
+    Wstar = om1.get_state()
+    c0 = _wall_sums(mesh, walls, W)
+    acc0 = np.zeros((mesh.nv, 4))
+    np.add.at(acc0, mesh.tri.ravel(), d0["phiN"].reshape(-1, 4))
+    assert np.allclose(Wstar, W - dt / vol * (acc0 + c0).T, rtol=0, atol=5e-14)     # eq. 60 with the wall term
+    om1.set_state(Wstar)
+    d1 = om1.dump_stage1()
+    c1 = _wall_sums(mesh, walls, Wstar)
+    acc1 = np.zeros((mesh.nv, 4))
+    np.add.at(acc1, mesh.tri.ravel(), d1["phiN"].reshape(-1, 4))
+    heun = W - 0.5 * dt / vol * (acc0 + acc1 + c0 + c1).T
+    om2 = oracle.OracleMesh(mesh.xy, mesh.tri, wall_edge=walls, scheme=oracle.SCHEME_N, time_order=2)
+    om2.set_state(W)
+    _, _, dt2 = om2.step(1)
+    assert dt2 == dt
+    W2 = om2.get_state()
+    assert np.abs(W2 - heun).max() <= 5e-14
+    # the test has teeth: each plausible mistake (term of W^n dropped, term of W* dropped, no factor 1/2, wrong sign)
+    # moves the wall vertices by far more than the tolerance
+    for wrong in (c1, c0, 2.0 * (c0 + c1), -(c0 + c1), 0.5 * c0 + c1):
+        bad = W - 0.5 * dt / vol * (acc0 + acc1 + wrong).T
+        assert np.abs(W2 - bad)[:, on_wall].max() > 1e-6
+
+
 def test_renumbering_invariance():
     # permuting vertex / triangle numbering and rotating local node order permutes the result
     base = wl.jitter_mesh(wl.uniform_mesh(16, 16, 1.0, 1.0, periodic=True), 0.2, seed=13)
