@@ -60,6 +60,9 @@ typedef struct {
                          only                                                                          */
   int32_t lumping;    /* 0 = global lumping (all tests of the paper, L576); 1 = selective lumping with the Galerkin
                          mass matrix (eq. 66-67), stage 2 of time_order 2 only                        */
+  double domain_size; /* MRD_SCHEME_BX: "L, the domain size" of eq. 56 (L515; reading C25).  0 = take it from this mesh
+                         (larger side of its bounding box, the period where periodic); > 0 = use this value -- a part of
+                         a domain decomposition passes the WHOLE mesh's L (mrd_partition_domain_size)            */
 } mrd_params;
 
 /* ------------------------------------------------------------------------------------------------
@@ -201,6 +204,9 @@ int mrd_partition_create(mrd_partition **out, int64_t n_vertex, const double *xy
                          const int32_t *wall_edge, double period_x, double period_y, int32_t n_part, int32_t part);
 void mrd_partition_destroy(mrd_partition *p);
 int mrd_partition_sizes(const mrd_partition *p, int64_t n[8]);
+/* L of eq. 56 (reading C25) of the WHOLE mesh the partition was made from (host out): goes into the
+ * mrd_params.domain_size of every part's mesh, so that the Bx sensor is the same on all parts and on one device. */
+int mrd_partition_domain_size(const mrd_partition *p, double *L);
 int mrd_partition_get(const mrd_partition *p, const char *name, void *dst, int64_t bytes);
 
 /* Halo lists of a mesh created from a partition (vertex_flag 2 = halo: such a vertex keeps its value in
@@ -217,11 +223,13 @@ int mrd_halo_set(mrd_mesh *m, int64_t n_send, const int32_t *send_idx, int64_t n
  *   mrd_halo_pack -> exchange -> mrd_halo_unpack
  *   time_order 2 only: mrd_phase(STAGE2) (stage-2 triangle pass, eq. 61 on the owned vertices), then
  *   mrd_halo_pack -> exchange -> mrd_halo_unpack
- *   mrd_phase(END)         advance t, count the step
+ *   mrd_status_get -> max-reduce the double over all parts -> mrd_status_set
+ *   mrd_phase(END)         advance t, count the step -- or discard it on EVERY part if any part met rho <= 0, p <= 0 or
+ *                          c^2 <= 0 anywhere in it
  * mrd_phase_begin settles earlier asynchronous work, arms the stepper and sets t_end (<= 0: none; every part
  * must pass the same); mrd_phase_end synchronises and reports like mrd_step (steps_done counts the steps since
- * mrd_phase_begin).  A non-physical state met by any part reaches all of them through the second double of
- * mrd_dt_get/set one step later; the distributed state is then undefined until the next mrd_set_state. */
+ * mrd_phase_begin).  With the status reduction every part commits or discards the same steps, so (steps, t, error code)
+ * are identical on all parts and the state is left at the last good step everywhere (MRD_ENONPHYSICAL), as in mrd_step. */
 enum { MRD_PHASE_RESIDUAL1 = 0, MRD_PHASE_UPDATE1 = 1, MRD_PHASE_STAGE2 = 2, MRD_PHASE_END = 3 };
 int mrd_phase_begin(mrd_mesh *m, double t_end, void *stream);
 int mrd_phase(mrd_mesh *m, int32_t phase, void *stream);
@@ -230,6 +238,10 @@ int mrd_phase_end(mrd_mesh *m, void *stream, int64_t *steps_done, double *t, dou
  * non-physical state, else 0.  After the min-reduction, mrd_dt_set installs both. */
 int mrd_dt_get(mrd_mesh *m, double *d_dev, void *stream);
 int mrd_dt_set(mrd_mesh *m, const double *d_dev, void *stream);
+/* d DEVICE double[1]: 1 if this part met a non-physical state in the step in flight, else 0.  Call both after the last
+ * exchange of the step and before mrd_phase(END); between them, max-reduce the double over all parts. */
+int mrd_status_get(mrd_mesh *m, double *d_dev, void *stream);
+int mrd_status_set(mrd_mesh *m, const double *d_dev, void *stream);
 /* buf DEVICE [n_send][4] / [n_recv][4] (double or float per precision), rows in list order: the conserved
  * state just written by the preceding UPDATE1 / STAGE2 phase.  Unpack also derives what the triangle kernels
  * read (Z, and dW/dt of eq. 57 or |v| + c) exactly as the owner did, so halo copies are bitwise the owner's. */

@@ -18,7 +18,7 @@ class Params(C.Structure):
     """mrd_params of include/mrd.h."""
     _fields_ = [("gamma", C.c_double), ("cfl", C.c_double), ("scheme", C.c_int32), ("time_order", C.c_int32),
                 ("precision", C.c_int32), ("reorder", C.c_int32), ("period_x", C.c_double), ("period_y", C.c_double),
-                ("tile", C.c_int32), ("lumping", C.c_int32)]
+                ("tile", C.c_int32), ("lumping", C.c_int32), ("domain_size", C.c_double)]
 
 
 class MrdError(RuntimeError):
@@ -73,6 +73,9 @@ def lib():
         L.mrd_phase_end.argtypes = [vp, vp, _lp, _dp, _dp]
         L.mrd_dt_get.argtypes = [vp, vp, vp]
         L.mrd_dt_set.argtypes = [vp, vp, vp]
+        L.mrd_status_get.argtypes = [vp, vp, vp]
+        L.mrd_status_set.argtypes = [vp, vp, vp]
+        L.mrd_partition_domain_size.argtypes = [vp, _dp]
         L.mrd_halo_pack.argtypes = [vp, vp, vp]
         L.mrd_range_get.argtypes = [vp, C.c_int32, vp, vp]
         L.mrd_range_set.argtypes = [vp, C.c_int32, vp, vp]
@@ -119,9 +122,9 @@ def _mesh_args(xy, tri, vertex_flag, wall_edge):
 
 
 def make_params(gamma=1.4, cfl=0.5, scheme=SCHEME_B, time_order=2, precision=FP64, reorder=True,
-                period=(0.0, 0.0), tile=0, lumping=0) -> Params:
+                period=(0.0, 0.0), tile=0, lumping=0, domain_size=0.0) -> Params:
     return Params(float(gamma), float(cfl), int(scheme), int(time_order), int(precision), int(bool(reorder)),
-                  float(period[0]), float(period[1]), int(tile), int(lumping))
+                  float(period[0]), float(period[1]), int(tile), int(lumping), float(domain_size))
 
 
 class Layout:
@@ -181,6 +184,9 @@ class Partition:
             n = [int(x) for x in n]
             (self.n_local, self.n_owned, self.n_tri, self.n_wall, self.n_neighbour, self.n_send, self.n_recv,
              self.n_global) = n
+            ds = C.c_double()
+            _check(lib().mrd_partition_domain_size(h, C.byref(ds)))
+            self.domain_size = ds.value
             for name, dt, shape in self._ARRAYS:
                 a = np.empty(shape(n), dtype=dt)
                 _check(lib().mrd_partition_get(h, name.encode(), C.c_void_p(a.ctypes.data), a.nbytes))
@@ -321,6 +327,14 @@ class Mesh:
     def dt_set(self, d, stream=None):
         self._check_buf(d, 2, self._torch.float64)
         _check(lib().mrd_dt_set(self._h, C.c_void_p(d.data_ptr()), _stream_ptr(stream)))
+
+    def status_get(self, d, stream=None):
+        self._check_buf(d, 1, self._torch.float64)
+        _check(lib().mrd_status_get(self._h, C.c_void_p(d.data_ptr()), _stream_ptr(stream)))
+
+    def status_set(self, d, stream=None):
+        self._check_buf(d, 1, self._torch.float64)
+        _check(lib().mrd_status_set(self._h, C.c_void_p(d.data_ptr()), _stream_ptr(stream)))
 
     def range_get(self, stage, d, stream=None):
         self._check_buf(d, 2, self._torch.float64)

@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <map>
 #include <string>
 #include <vector>
 
@@ -65,15 +66,18 @@ struct mrd_mesh {
   // fused tile path (mrd_tile.cuh): tile plan + one partial per slot
   bool fused = false;
   bool dbg = false;               // dump: tile kernels also write per-triangle residuals to d_phi / d_sT
-  int2 *d_tile_info = nullptr;    // [ntile+1]: first slot, first geometry record
+  int4 *d_tile_info = nullptr;    // [ntile+1]: first slot, first geometry record, plan record
   void *d_shape_geom = nullptr;   // R [nshape][12] (geometry-table kernels)
   int32_t *d_vslot_off = nullptr, *d_vslot_ent = nullptr;
-  uint16_t *d_plan = nullptr;     // [ntile][plan_stride]
+  uint16_t *d_plan = nullptr;     // [nplan][plan_stride]: distinct plan records
   void *d_slot_xy = nullptr;      // R [nslot][2]
   void *d_part = nullptr, *d_partS = nullptr;  // Vec4<R> [nslot], R [nslot]
   void *d_slotZ[2] = {nullptr, nullptr}, *d_slotS[2] = {nullptr, nullptr}, *d_slotD = nullptr;  // slot-major Z, |v|+c, dW/dt
-  void *d_phi16 = nullptr;        // R [ntile][16][T]: phi^N(W^n) (12) and phi^T(W^n) (4), component-major per tile
+  void *d_phi12 = nullptr;        // R [ntile][12 T]: phi_0^N, phi_1^N, phi^T of W^n in the cell layout of mrd_tile.cuh
   int nsm = 0;
+  std::map<const void *, unsigned> tile_grid;  // persistent grid of each tile-kernel instantiation (launch_tile)
+  int launch_rc = 0;              // first error met while ENQUEUEING kernels (enqueue_step is void); returned and cleared by take_launch_rc
+  void note(int rc) { if (rc && !launch_rc) launch_rc = rc; }
   // CUDA graphs for launch-bound (small) meshes: two consecutive steps (buffer parity a, then a^1) captured once per
   // starting parity on an internal stream and replayed; forked from / joined to the caller's stream by events
   cudaStream_t s_int = nullptr;
@@ -143,10 +147,12 @@ template <class R> mrd::TileDev<R> tile_dev(const mrd_mesh *m) {
   t.tile = m->L.tile;
   t.maxslots = m->L.maxslots;
   t.offn = m->L.offn;
+  t.maxbatch = m->L.maxbatch;
   t.plan_stride = m->L.plan_stride;
   t.ntile = m->L.ntile;
   t.nslot = m->L.nslot;
   t.nt = m->L.nt;
+  t.nv = m->L.nv;
   t.maxshapes = m->L.geom_table ? m->L.maxshapes : 0;
   t.tile_info = m->d_tile_info;
   t.shape_geom = (const R *)m->d_shape_geom;
@@ -215,8 +221,9 @@ template <class R> int upload_impl(mrd_mesh *m) {
     if ((rc = dev_upload(m, &m->d_csr_ent, L.csr_ent.data(), 3 * nt))) return rc;
   } else {
     {
-      std::vector<int2> info(L.ntile + 1);
-      for (int64_t b = 0; b <= L.ntile; ++b) info[b] = make_int2(L.tile_slot_off[b], L.geom_table ? L.tile_shape_off[b] : 0);
+      std::vector<int4> info(L.ntile + 1);
+      for (int64_t b = 0; b <= L.ntile; ++b)
+        info[b] = make_int4(L.tile_slot_off[b], L.geom_table ? L.tile_shape_off[b] : 0, b < L.ntile ? L.tile_plan_idx[b] : 0, 0);
       if ((rc = dev_upload(m, &m->d_tile_info, info.data(), L.ntile + 1))) return rc;
     }
     if (L.geom_table && (rc = dev_upload_real<R>(m, &m->d_shape_geom, L.shape_geom.data(), (int64_t)L.shape_geom.size()))) return rc;
@@ -225,11 +232,11 @@ template <class R> int upload_impl(mrd_mesh *m) {
     if ((rc = dev_upload(m, &m->d_vslot_off, L.vslot_off.data(), nv + 1))) return rc;
     if ((rc = dev_upload(m, &m->d_vslot_ent, L.vslot_ent.data(), (int64_t)L.vslot_ent.size()))) return rc;
     V4 *pp = nullptr, *sd = nullptr;
-    R *ps = nullptr, *p16 = nullptr;
+    R *ps = nullptr, *p12 = nullptr;
     if ((rc = dev_alloc(m, &pp, L.nslot)) || (rc = dev_alloc(m, &ps, L.nslot)) || (rc = dev_alloc(m, &sd, L.nslot))) return rc;
-    if ((rc = dev_alloc(m, &p16, L.ntile * 16 * L.tile))) return rc;
+    if ((rc = dev_alloc(m, &p12, L.ntile * 12 * L.tile))) return rc;
     CUDA_TRY(cudaMemset(sd, 0, sizeof(V4) * L.nslot));
-    m->d_slotD = sd; m->d_phi16 = p16;
+    m->d_slotD = sd; m->d_phi12 = p12;
     for (int b = 0; b < 2; ++b) {
       V4 *z = nullptr;
       R *sp = nullptr;
@@ -325,20 +332,31 @@ template <class R> int get_state_impl(mrd_mesh *m, R *W_dev, cudaStream_t s) {
   return MRD_OK;
 }
 
-// persistent launch of a tile kernel: dynamic shared memory opt-in, grid = SMs x resident blocks (<= ntile)
-template <class K, class... Args> void launch_tile(mrd_mesh *m, K kernel, size_t sh, cudaStream_t s, Args... args) {
+// persistent launch of a tile kernel: dynamic shared memory opt-in, grid = SMs x resident blocks (<= ntile).  The opt-in
+// and the occupancy query run once per (kernel instantiation, mesh); their result is cached in the mesh.
+template <class K, class... Args> int launch_tile(mrd_mesh *m, K kernel, size_t sh, cudaStream_t s, Args... args) {
   const int T = m->L.tile;
-  cudaFuncSetAttribute((const void *)kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh);
-  int occ = 1;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, T, sh);
-  if (occ < 1) occ = 1;
-  if (const char *cap = std::getenv("MRD_TILE_OCC")) {  // tuning knob: cap the resident blocks per SM of the tile kernels
-    int c = std::atoi(cap);
-    if (c >= 1 && c < occ) occ = c;
+  const void *key = (const void *)kernel;
+  auto it = m->tile_grid.find(key);
+  if (it == m->tile_grid.end()) {
+    cudaError_t e = cudaFuncSetAttribute(key, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh);
+    if (e != cudaSuccess)
+      return fail(MRD_ECUDA, "tile kernel: cannot opt in to " + std::to_string(sh) + " bytes of dynamic shared memory: " + cudaGetErrorString(e));
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, T, sh);
+    if (e != cudaSuccess || occ < 1)
+      return fail(MRD_ECUDA, std::string("tile kernel: no resident block fits (") + std::to_string(sh) + " bytes of shared memory): " + cudaGetErrorString(e));
+#ifdef MRD_DEBUG_KNOBS
+    if (const char *cap = std::getenv("MRD_TILE_OCC")) {  // tuning knob (debug builds only): cap the resident blocks per SM
+      int c = std::atoi(cap);
+      if (c >= 1 && c < occ) occ = c;
+    }
+#endif
+    it = m->tile_grid.emplace(key, (unsigned)std::min<int64_t>(m->L.ntile, (int64_t)m->nsm * occ)).first;
   }
-  int64_t grid = std::min<int64_t>(m->L.ntile, (int64_t)m->nsm * occ);
-  kernel<<<(unsigned)grid, T, sh, s>>>(args...);
+  kernel<<<it->second, T, sh, s>>>(args...);
   m->launches++;
+  return MRD_OK;
 }
 // tile sizes the fused kernels are compiled for
 #define MRD_TILE_DISPATCH_G(T, CALL)                      \
@@ -349,22 +367,27 @@ template <class K, class... Args> void launch_tile(mrd_mesh *m, K kernel, size_t
 #define MRD_TILE_DISPATCH(T, CALL)                                      \
   if (m->L.geom_table) { constexpr bool GTAB = true; MRD_TILE_DISPATCH_G(T, CALL) } \
   else { constexpr bool GTAB = false; MRD_TILE_DISPATCH_G(T, CALL) }
+// `a`: buffer pair holding W^n.  Fused path: residuals of W^n -> one partial per tile slot; unfused path: per-triangle
+// residuals d_phi, s_T.
 template <class R, int SCHEME> void launch_stage1(mrd_mesh *m, bool store, int a, cudaStream_t s) {
   using V4 = mrd::Vec4<R>;
   const R gamma = (R)m->L.p.gamma;
   if (m->fused) {
     auto td = tile_dev<R>(m);
 #define MRD_SMEM(STAGE) mrd::TileSmem<R, STAGE, GTAB>(td.tile, td.maxslots, td.plan_stride, td.maxshapes)
-    V4 *dbg = m->dbg ? (V4 *)m->d_phi : nullptr;
-    R *dbgs = m->dbg ? (R *)m->d_sT : nullptr;
+    mrd::TileIO<R> io{};
+    io.slotZ = (const V4 *)m->d_slotZ[a];
+    io.slotS = (const R *)m->d_slotS[a];
+    io.slotD = (const V4 *)m->d_slotD;
+    io.phi12 = (R *)m->d_phi12;
+    io.part = (V4 *)m->d_part;
+    io.partS = (R *)m->d_partS;
+    io.phi_dbg = m->dbg ? (V4 *)m->d_phi : nullptr;
+    io.sT_dbg = m->dbg ? (R *)m->d_sT : nullptr;
     if (store) {
-      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, true, TILE, GTAB>, MRD_SMEM(1).total, s, td, MRD_SMEM(1), gamma, (const mrd::Ctl *)m->d_ctl,
-                                              (const V4 *)m->d_slotZ[a], (const R *)m->d_slotS[a], (const V4 *)m->d_slotD, (R *)m->d_phi16,
-                                              (V4 *)m->d_part, (R *)m->d_partS, dbg, dbgs, m->d_flag)))
+      MRD_TILE_DISPATCH(td.tile, m->note(launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, true, TILE, GTAB>, MRD_SMEM(1).total, s, td, MRD_SMEM(1), gamma, (const mrd::Ctl *)m->d_ctl, io, m->d_flag)))
     } else {
-      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, false, TILE, GTAB>, MRD_SMEM(1).total, s, td, MRD_SMEM(1), gamma, (const mrd::Ctl *)m->d_ctl,
-                                              (const V4 *)m->d_slotZ[a], (const R *)m->d_slotS[a], (const V4 *)m->d_slotD, (R *)m->d_phi16,
-                                              (V4 *)m->d_part, (R *)m->d_partS, dbg, dbgs, m->d_flag)))
+      MRD_TILE_DISPATCH(td.tile, m->note(launch_tile(m, mrd::tile_kernel<R, SCHEME, 1, false, TILE, GTAB>, MRD_SMEM(1).total, s, td, MRD_SMEM(1), gamma, (const mrd::Ctl *)m->d_ctl, io, m->d_flag)))
     }
     return;
   }
@@ -378,22 +401,23 @@ template <class R, int SCHEME> void launch_stage1(mrd_mesh *m, bool store, int a
                                                              (V4 *)m->d_phi, (V4 *)m->d_phiN, (V4 *)m->d_phiT, (R *)m->d_sT, m->d_flag);
   m->launches++;
 }
+// `b`: buffer pair holding W*.  Total residuals of eq. 61-65 -> one partial per tile slot (fused) / d_phi (unfused).
 template <class R, int SCHEME> void launch_stage2(mrd_mesh *m, int b, cudaStream_t s) {
   using V4 = mrd::Vec4<R>;
   const R gamma = (R)m->L.p.gamma;
   if (m->fused) {
     auto td = tile_dev<R>(m);
-
+    mrd::TileIO<R> io{};
+    io.slotZ = (const V4 *)m->d_slotZ[b];
+    io.slotD = (const V4 *)m->d_slotD;
+    io.phi12 = (R *)m->d_phi12;
+    io.part = (V4 *)m->d_part;
     if (m->L.p.lumping) {
       constexpr bool LUMP = true;
-      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, LUMP, TILE, GTAB>, MRD_SMEM(2).total, s, td, MRD_SMEM(2), gamma, (const mrd::Ctl *)m->d_ctl,
-                                              (const V4 *)m->d_slotZ[b], (const R *)nullptr, (const V4 *)m->d_slotD, (R *)m->d_phi16,
-                                              (V4 *)m->d_part, (R *)nullptr, (V4 *)nullptr, (R *)nullptr, m->d_flag)))
+      MRD_TILE_DISPATCH(td.tile, m->note(launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, LUMP, TILE, GTAB>, MRD_SMEM(2).total, s, td, MRD_SMEM(2), gamma, (const mrd::Ctl *)m->d_ctl, io, m->d_flag)))
     } else {
       constexpr bool LUMP = false;
-      MRD_TILE_DISPATCH(td.tile, (launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, LUMP, TILE, GTAB>, MRD_SMEM(2).total, s, td, MRD_SMEM(2), gamma, (const mrd::Ctl *)m->d_ctl,
-                                              (const V4 *)m->d_slotZ[b], (const R *)nullptr, (const V4 *)m->d_slotD, (R *)m->d_phi16,
-                                              (V4 *)m->d_part, (R *)nullptr, (V4 *)nullptr, (R *)nullptr, m->d_flag)))
+      MRD_TILE_DISPATCH(td.tile, m->note(launch_tile(m, mrd::tile_kernel<R, SCHEME, 2, LUMP, TILE, GTAB>, MRD_SMEM(2).total, s, td, MRD_SMEM(2), gamma, (const mrd::Ctl *)m->d_ctl, io, m->d_flag)))
     }
     return;
   }
@@ -512,13 +536,30 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
     m->launches++;
     PROF_MARK(MRD_PROF_CTL)
   }
+  // a launch that could not be enqueued (bad configuration, shared-memory opt-in refused) is reported by the caller
+  cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess) m->note(fail(MRD_ECUDA, std::string("kernel launch: ") + cudaGetErrorString(e)));
+}
+// kernel launches of one step (the CUDA-graph replay counts them without launching)
+inline int64_t launches_per_step(const mrd_mesh *m, int scheme) {
+  const bool rk2 = m->L.p.time_order == 2;
+  int64_t n = rk2 ? 6 : 4;
+  if (m->nwv > 0) n += rk2 ? 2 : 1;
+  if (scheme == MRD_SCHEME_BX) n += m->L.p.time_order;
+  return n;
+}
+// the first error met while enqueueing since the last call (0 if none)
+int take_launch_rc(mrd_mesh *m) {
+  const int rc = m->launch_rc;
+  m->launch_rc = 0;
+  return rc;
 }
 
 // n consecutive steps starting from buffer pair `a` (updated).  Small meshes replay a captured two-step graph.
 template <class R> int run_steps(mrd_mesh *m, int scheme, int64_t n, int &a, cudaStream_t s) {
   if (!m->graph_ok || n < 2) {
     for (int64_t k = 0; k < n; ++k, a ^= 1) enqueue_step<R>(m, scheme, a, s);
-    return MRD_OK;
+    return take_launch_rc(m);
   }
   CUDA_TRY(cudaEventRecord(m->ev_in, s));
   CUDA_TRY(cudaStreamWaitEvent(m->s_int, m->ev_in, 0));
@@ -542,8 +583,7 @@ template <class R> int run_steps(mrd_mesh *m, int scheme, int64_t n, int &a, cud
       if (e != cudaSuccess) return fail(MRD_ECUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e));
     }
   }
-  const int64_t per_step = (m->L.p.time_order == 2 ? 6 : 4) + (m->nwv > 0 ? (m->L.p.time_order == 2 ? 2 : 1) : 0) +
-                           (scheme == MRD_SCHEME_BX ? m->L.p.time_order : 0);
+  const int64_t per_step = launches_per_step(m, scheme);
   for (int64_t k = 0; k + 1 < n; k += 2) {
     CUDA_TRY(cudaGraphLaunch(m->gexec[a], m->s_int));
     m->launches += 2 * per_step;
@@ -554,7 +594,7 @@ template <class R> int run_steps(mrd_mesh *m, int scheme, int64_t n, int &a, cud
   }
   CUDA_TRY(cudaEventRecord(m->ev_out, m->s_int));
   CUDA_TRY(cudaStreamWaitEvent(s, m->ev_out, 0));
-  return MRD_OK;
+  return take_launch_rc(m);
 }
 
 // fetch the control block (after a stream sync) and bring the host bookkeeping up to date
@@ -567,6 +607,18 @@ int fetch_ctl(mrd_mesh *m, cudaStream_t s, mrd::Ctl *out) {
   if (done & 1) m->cur ^= 1;
   m->steps_base = out->steps;
   return MRD_OK;
+}
+
+// A step that met rho <= 0, p <= 0 or c^2 <= 0 was discarded on the device (the buffer pair holding W^n is never written
+// during a step): clear the flag so that the state -- the last good step -- stays usable, and report it.
+int discard_failed_step(mrd_mesh *m, const mrd::Ctl &c, cudaStream_t s) {
+  mrd::Ctl fix = c;
+  fix.status = 0;
+  fix.active = 0;
+  CUDA_TRY(cudaMemcpyAsync(m->d_ctl, &fix, sizeof fix, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
+  CUDA_TRY(cudaStreamSynchronize(s));
+  return fail(MRD_ENONPHYSICAL, "non-physical state (rho <= 0, p <= 0 or c^2 <= 0) met; state left at the last good step");
 }
 
 template <class R> int step_impl(mrd_mesh *m, int64_t max_steps, double t_end, cudaStream_t s, bool sync,
@@ -606,24 +658,14 @@ template <class R> int step_impl(mrd_mesh *m, int64_t max_steps, double t_end, c
   if (steps_done) *steps_done = c.steps - steps0;
   if (t) *t = c.t;
   if (dt_last) *dt_last = c.dt;
-  if (c.status) {
-    // the failed step is discarded: clear the flag so that the state (last good step) stays usable
-    mrd::Ctl fix = c;
-    fix.status = 0;
-    fix.active = 0;
-    CUDA_TRY(cudaMemcpyAsync(m->d_ctl, &fix, sizeof fix, cudaMemcpyHostToDevice, s));
-    CUDA_TRY(cudaMemsetAsync(m->d_flag, 0, sizeof(int), s));
-    CUDA_TRY(cudaStreamSynchronize(s));
-    return fail(MRD_ENONPHYSICAL, "non-physical state (rho <= 0, p <= 0 or c^2 <= 0) met; state left at the last good step");
-  }
+  if (c.status) return discard_failed_step(m, c, s);
   return MRD_OK;
 }
 
 // ---- phase stepping and halo exchange (include/mrd.h "Domain decomposition") --------------------------------
 template <class R> int phase_impl(mrd_mesh *m, int phase, cudaStream_t s) {
   enqueue_step<R>(m, m->L.p.scheme, m->phase_a, s, nullptr, 1 << phase);
-  CUDA_TRY(cudaGetLastError());
-  return MRD_OK;
+  return take_launch_rc(m);
 }
 template <class R> int halo_pack_impl(mrd_mesh *m, void *buf, cudaStream_t s) {
   using V4 = mrd::Vec4<R>;
@@ -723,14 +765,22 @@ template <class R> int dump_impl(mrd_mesh *m, double *phiT, double *phiN, double
     if (pass == 1 && phiB) put3(phiB);
   }
   if (m->fused && (phiN || phiT)) {
-    // stored stage-1 values of the fused path: phi16[tile][16][T] -> the unfused [nt][3][4] / [nt][4] shapes
+    // stored stage-1 values of the fused path, phi12[tile][half][N0 | N1 | T][triangle][2] (the cell layout of mrd_tile.cuh),
+    // -> the unfused [nt][3][4] / [nt][4] shapes; phi_2^N = (phi^T - phi_0^N) - phi_1^N as both tile kernels form it
     const int T = m->L.tile;
-    std::vector<R> h16((size_t)m->L.ntile * 16 * T);
-    CUDA_TRY(cudaMemcpy(h16.data(), m->d_phi16, h16.size() * sizeof(R), cudaMemcpyDeviceToHost));
+    std::vector<R> h12((size_t)m->L.ntile * 12 * T);
+    CUDA_TRY(cudaMemcpy(h12.data(), m->d_phi12, h12.size() * sizeof(R), cudaMemcpyDeviceToHost));
     for (int64_t k = 0; k < nt; ++k) {
-      const R *o = &h16[(size_t)(k / T) * 16 * T + (k % T)];
-      for (int c = 0; c < 12; ++c) h3[12 * k + c] = o[(size_t)c * T];
-      for (int c = 0; c < 4; ++c) h1[4 * k + c] = o[(size_t)(12 + c) * T];
+      const R *o = &h12[(size_t)(k / T) * 12 * T];
+      const int lt = (int)(k % T);
+      for (int c = 0; c < 4; ++c) {
+        const int h = c >> 1, c2 = c & 1;
+        const R n0 = o[((h * 3 + 0) * T + lt) * 2 + c2], n1 = o[((h * 3 + 1) * T + lt) * 2 + c2], pt = o[((h * 3 + 2) * T + lt) * 2 + c2];
+        h3[12 * k + c] = n0;
+        h3[12 * k + 4 + c] = n1;
+        h3[12 * k + 8 + c] = (pt - n0) - n1;
+        h1[4 * k + c] = pt;
+      }
     }
   }
   if (phiN) {
@@ -802,8 +852,18 @@ template <class R> int dump_sample_impl(mrd_mesh *m, int64_t ns, const int64_t *
     R v16[16];
     if (m->fused) {
       const int T = m->L.tile;
-      const R *o = (const R *)m->d_phi16 + (size_t)(k / T) * 16 * T + (k % T);
-      CUDA_TRY(cudaMemcpy2D(v16, sizeof(R), o, sizeof(R) * T, sizeof(R), 16, cudaMemcpyDeviceToHost));
+      const int lt = (int)(k % T);
+      const R *o = (const R *)m->d_phi12 + (size_t)(k / T) * 12 * T;
+      R c6[6][2];   // cells (half, N0 | N1 | T) of this triangle
+      for (int hc = 0; hc < 6; ++hc) CUDA_TRY(cudaMemcpy(c6[hc], o + ((size_t)hc * T + lt) * 2, sizeof(R) * 2, cudaMemcpyDeviceToHost));
+      for (int c = 0; c < 4; ++c) {
+        const int h = c >> 1, c2 = c & 1;
+        const R n0 = c6[h * 3 + 0][c2], n1 = c6[h * 3 + 1][c2], pt = c6[h * 3 + 2][c2];
+        v16[c] = n0;
+        v16[4 + c] = n1;
+        v16[8 + c] = (pt - n0) - n1;
+        v16[12 + c] = pt;
+      }
     } else {
       CUDA_TRY(cudaMemcpy(v16, (const R *)m->d_phiN + 12 * k, sizeof(R) * 12, cudaMemcpyDeviceToHost));
       CUDA_TRY(cudaMemcpy(v16 + 12, (const R *)m->d_phiT + 4 * k, sizeof(R) * 4, cudaMemcpyDeviceToHost));
@@ -894,7 +954,7 @@ int mrd_mesh_create(mrd_mesh **out, const mrd_params *p, int64_t nv, const doubl
   }
   if (rc) { mrd_mesh_destroy(m); return rc; }
   // launch-bound regime: below ~4M triangles a step is tens of microseconds, comparable to 6 kernel launches
-  if (m->L.nt <= (int64_t(1) << 22) && !std::getenv("MRD_NO_GRAPH")) {
+  if (m->L.nt <= (int64_t(1) << 22)) {
     if (cudaStreamCreateWithFlags(&m->s_int, cudaStreamNonBlocking) == cudaSuccess &&
         cudaEventCreateWithFlags(&m->ev_in, cudaEventDisableTiming) == cudaSuccess &&
         cudaEventCreateWithFlags(&m->ev_out, cudaEventDisableTiming) == cudaSuccess)
@@ -981,7 +1041,7 @@ int mrd_sync(mrd_mesh *m, void *stream, int64_t *steps_total, double *t, double 
   if (steps_total) *steps_total = c.steps;
   if (t) *t = c.t;
   if (dt_last) *dt_last = c.dt;
-  if (c.status) return fail(MRD_ENONPHYSICAL, "non-physical state met in an asynchronous step");
+  if (c.status) return discard_failed_step(m, c, (cudaStream_t)stream);
   return MRD_OK;
 }
 
@@ -1028,7 +1088,8 @@ int mrd_step_profile(mrd_mesh *m, void *stream, float ms[MRD_PROFILE_SLOTS]) {
   prof.mark(-1, s);
   if (m->L.p.precision == MRD_FP64) enqueue_step<double>(m, m->L.p.scheme, m->cur, s, &prof);
   else enqueue_step<float>(m, m->L.p.scheme, m->cur, s, &prof);
-  rc = fetch_ctl(m, s, &c);
+  rc = take_launch_rc(m);
+  if (!rc) rc = fetch_ctl(m, s, &c);
   for (int k = 0; k < MRD_PROFILE_SLOTS; ++k) ms[k] = 0.f;
   if (!rc)
     for (int k = 1; k < prof.n; ++k) {
@@ -1061,6 +1122,11 @@ int mrd_partition_create(mrd_partition **out, int64_t nv, const double *xy, int6
   return MRD_OK;
 }
 void mrd_partition_destroy(mrd_partition *p) { delete p; }
+int mrd_partition_domain_size(const mrd_partition *p, double *L) {
+  if (!p || !L) return fail(MRD_EINVAL, "null argument");
+  *L = p->domain_size;
+  return MRD_OK;
+}
 int mrd_partition_sizes(const mrd_partition *p, int64_t n[8]) {
   if (!p || !n) return fail(MRD_EINVAL, "null argument");
   return mrd_host::partition_sizes(*p, n);
@@ -1144,7 +1210,7 @@ int mrd_phase_end(mrd_mesh *m, void *stream, int64_t *steps_done, double *t, dou
   if (steps_done) *steps_done = c.steps - m->phase_steps0;
   if (t) *t = c.t;
   if (dt_last) *dt_last = c.dt;
-  if (c.status) return fail(MRD_ENONPHYSICAL, "non-physical state (rho <= 0, p <= 0 or c^2 <= 0) met by some part; set the state again");
+  if (c.status) return discard_failed_step(m, c, s);
   return MRD_OK;
 }
 
@@ -1160,6 +1226,23 @@ int mrd_dt_set(mrd_mesh *m, const double *d_dev, void *stream) {
   if (!m || !d_dev) return fail(MRD_EINVAL, "null argument");
   if (!m->in_phases || m->phase_next != MRD_PHASE_UPDATE1) return fail(MRD_EINVAL, "mrd_dt_set must follow mrd_phase(RESIDUAL1)");
   mrd::dt_set_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(m->d_ctl, m->d_flag, d_dev);
+  m->launches++;
+  CUDA_TRY(cudaGetLastError());
+  return MRD_OK;
+}
+
+int mrd_status_get(mrd_mesh *m, double *d_dev, void *stream) {
+  if (!m || !d_dev) return fail(MRD_EINVAL, "null argument");
+  if (!m->in_phases || m->phase_next != MRD_PHASE_END) return fail(MRD_EINVAL, "mrd_status_get must precede mrd_phase(END)");
+  mrd::status_get_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(m->d_ctl, m->d_flag, d_dev);
+  m->launches++;
+  CUDA_TRY(cudaGetLastError());
+  return MRD_OK;
+}
+int mrd_status_set(mrd_mesh *m, const double *d_dev, void *stream) {
+  if (!m || !d_dev) return fail(MRD_EINVAL, "null argument");
+  if (!m->in_phases || m->phase_next != MRD_PHASE_END) return fail(MRD_EINVAL, "mrd_status_set must precede mrd_phase(END)");
+  mrd::status_set_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(m->d_flag, d_dev);
   m->launches++;
   CUDA_TRY(cudaGetLastError());
   return MRD_OK;

@@ -548,6 +548,15 @@ __global__ void dt_set_kernel(Ctl *__restrict__ c, int *__restrict__ flag, const
   if (d[1] < 0.0) *flag = 1;
 }
 
+// d[0] = 1 if a kernel of this part met a non-physical state in the step in flight (or earlier), else 0; after a
+// max-reduction over the parts, status_set raises the flag everywhere, so that every part discards the SAME step at END
+__global__ void status_get_kernel(const Ctl *__restrict__ c, const int *__restrict__ flag, double *__restrict__ d) {
+  d[0] = (*flag || c->status) ? 1.0 : 0.0;
+}
+__global__ void status_set_kernel(int *__restrict__ flag, const double *__restrict__ d) {
+  if (d[0] > 0.0) *flag = 1;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Peak micro-benchmarks (roofline denominators): FMA throughput and device copy
 // ---------------------------------------------------------------------------------------------

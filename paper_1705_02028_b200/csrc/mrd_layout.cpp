@@ -107,6 +107,7 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
   if (p->precision != MRD_FP64 && p->precision != MRD_FP32) { err = "bad precision"; return MRD_EINVAL; }
   if (p->lumping != 0 && p->lumping != 1) { err = "lumping must be 0 (global) or 1 (selective)"; return MRD_EINVAL; }
   if (p->period_x < 0.0 || p->period_y < 0.0) { err = "negative period"; return MRD_EINVAL; }
+  if (p->domain_size < 0.0 || !(p->domain_size == p->domain_size)) { err = "negative domain_size"; return MRD_EINVAL; }
   if (ne < 0 || (ne > 0 && !wall_edge)) { err = "bad wall edge list"; return MRD_EINVAL; }
   if (p->tile != -1 && p->tile != 0 && p->tile != 64 && p->tile != 128) { err = "tile must be -1, 0, 64 or 128"; return MRD_EINVAL; }
   L.p = *p;
@@ -122,6 +123,7 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
       }
     const double sx = period[0] > 0.0 ? period[0] : hi[0] - lo[0], sy = period[1] > 0.0 ? period[1] : hi[1] - lo[1];
     L.domain_size = std::max(sx, sy);
+    if (p->domain_size > 0.0) L.domain_size = p->domain_size;  // given by the caller: a part of a decomposition passes the WHOLE mesh's L
   }
   // ---- validation + orientation fix in USER numbering ------------------------------------------
   std::vector<int32_t> utri(tri, tri + 3 * nt);
@@ -291,60 +293,75 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
 // ---------------------------------------------------------------------------------------------------
 // Tile plan: tile b = internal triangles [b*tile, (b+1)*tile).  A "slot" is one (vertex, periodic image)
 // pair used by the tile; every slot carries the vertex coordinates unwrapped into the tile's frame, so the
-// fused kernel needs no minimum-image arithmetic, and receives one partial sum per stage.
+// fused kernel needs no minimum-image arithmetic, and receives one partial sum per stage.  See mrd_layout.h for the
+// plan record.
 // ---------------------------------------------------------------------------------------------------
+namespace {
+struct Hash128 {
+  uint64_t a, b;
+  bool operator<(const Hash128 &o) const { return a != o.a ? a < o.a : b < o.b; }
+  bool operator==(const Hash128 &o) const { return a == o.a && b == o.b; }
+};
+inline Hash128 hash_bytes(const void *p, size_t n) {
+  const unsigned char *c = static_cast<const unsigned char *>(p);
+  uint64_t a = 1469598103934665603ull, b = 0x9E3779B97F4A7C15ull;
+  for (size_t i = 0; i < n; ++i) {
+    a = (a ^ c[i]) * 1099511628211ull;                                  // FNV-1a
+    b = (b + c[i] + 1) * 0xD6E8FEB86659FD93ull; b ^= b >> 29;           // an independent multiplicative mix
+  }
+  return {a, b};
+}
+}  // namespace
+
 static void build_tile_plan(mrd_layout &L, const std::vector<double> &xyi) {
   const int64_t nt = L.nt, nv = L.nv;
   const int T = L.tile;
   const double period[2] = {L.p.period_x, L.p.period_y};
   const int64_t ntile = (nt + T - 1) / T;
   L.ntile = ntile;
-  L.tile_tri.assign((size_t)ntile * T * 4, 0);
-  std::vector<int32_t> nslot_of(ntile + 1, 0);
-  // pass 1 (parallel): per tile the sorted unique keys, local ids of every node
+  // pass 1 (parallel): per tile the sorted unique (vertex, image) keys
   std::vector<std::vector<int64_t>> keys(ntile);
+  std::vector<int32_t> nslot_of(ntile + 1, 0);
+  auto node_key = [&](int64_t t, int j, double ax, double ay) -> int64_t {
+    const int32_t *v = &L.tri[3 * t];
+    const double x0 = xyi[2 * v[0]], y0 = xyi[2 * v[0] + 1];
+    int sx = image_shift(x0 - ax, period[0]), sy = image_shift(y0 - ay, period[1]);
+    if (j) {
+      sx += image_shift(xyi[2 * v[j]] - x0, period[0]);
+      sy += image_shift(xyi[2 * v[j] + 1] - y0, period[1]);
+    }
+    return (int64_t)v[j] * 25 + (sx + 2) * 5 + (sy + 2);
+  };
 #pragma omp parallel for schedule(dynamic, 64)
   for (int64_t b = 0; b < ntile; ++b) {
     const int64_t t0 = b * T, t1 = std::min(nt, t0 + T);
     const int32_t anchor = L.tri[3 * t0];
     const double ax = xyi[2 * anchor], ay = xyi[2 * anchor + 1];
-    int64_t nodekey[256 * 3];
     std::vector<int64_t> &uk = keys[b];
     uk.reserve(3 * (t1 - t0));
-    for (int64_t t = t0; t < t1; ++t) {
-      const int32_t *v = &L.tri[3 * t];
-      const double x0 = xyi[2 * v[0]], y0 = xyi[2 * v[0] + 1];
-      const int tsx = image_shift(x0 - ax, period[0]), tsy = image_shift(y0 - ay, period[1]);
-      for (int j = 0; j < 3; ++j) {
-        int sx = tsx, sy = tsy;
-        if (j) {
-          sx += image_shift(xyi[2 * v[j]] - x0, period[0]);
-          sy += image_shift(xyi[2 * v[j] + 1] - y0, period[1]);
-        }
-        int64_t key = (int64_t)v[j] * 25 + (sx + 2) * 5 + (sy + 2);
-        nodekey[3 * (t - t0) + j] = key;
-        uk.push_back(key);
-      }
-    }
+    for (int64_t t = t0; t < t1; ++t)
+      for (int j = 0; j < 3; ++j) uk.push_back(node_key(t, j, ax, ay));
     std::sort(uk.begin(), uk.end());
     uk.erase(std::unique(uk.begin(), uk.end()), uk.end());
     nslot_of[b + 1] = (int32_t)((uk.size() + 3) / 4 * 4);  // padded: 16-byte granularity of the bulk copies
-    for (int64_t t = t0; t < t1; ++t)
-      for (int j = 0; j < 3; ++j) {
-        int64_t key = nodekey[3 * (t - t0) + j];
-        int loc = (int)(std::lower_bound(uk.begin(), uk.end(), key) - uk.begin());
-        L.tile_tri[((size_t)b * T + (t - t0)) * 4 + j] = (uint16_t)loc;
-      }
   }
+  // slots per vertex (a vertex with one slot has its whole fan in that tile)
+  std::vector<int32_t> vcount(nv, 0);
+  for (int64_t b = 0; b < ntile; ++b)
+    for (int64_t key : keys[b]) vcount[key / 25]++;
   L.tile_slot_off.assign(ntile + 1, 0);
   for (int64_t b = 0; b < ntile; ++b) L.tile_slot_off[b + 1] = L.tile_slot_off[b] + nslot_of[b + 1];
   const int64_t nslot = L.tile_slot_off[ntile];
   L.nslot = nslot;
   L.slot_vertex.assign(nslot, -1);  // -1 = padding slot
   L.slot_xy.assign(2 * nslot, 0.0);
-  L.slot_ent_off.assign(nslot + 1, 0);
-  L.slot_ent.resize(3 * nt);
-  // pass 2: slot records and per-slot incidence counts
+  int32_t maxs = 0;
+  for (int64_t b = 0; b < ntile; ++b) maxs = std::max(maxs, nslot_of[b + 1]);
+  L.maxslots = maxs;
+  L.offn = (maxs + 1 + 7) / 8 * 8;
+  // pass 2 (parallel): slot records, and per tile the number of incidence batches
+  // (a slot's incidences are stored 4 to a batch, the last batch padded with the sentinel entry 3 T)
+  std::vector<int32_t> nbatch_of(ntile, 0);
 #pragma omp parallel for schedule(dynamic, 64)
   for (int64_t b = 0; b < ntile; ++b) {
     const int64_t t0 = b * T, t1 = std::min(nt, t0 + T);
@@ -352,108 +369,145 @@ static void build_tile_plan(mrd_layout &L, const std::vector<double> &xyi) {
     const int32_t anchor = L.tri[3 * t0];
     const double ax = xyi[2 * anchor], ay = xyi[2 * anchor + 1];
     const std::vector<int64_t> &uk = keys[b];
+    std::vector<int> deg(uk.size(), 0);
     for (size_t q = 0; q < uk.size(); ++q) {
-      int32_t v = (int32_t)(uk[q] / 25);
-      int r = (int)(uk[q] % 25);
-      int sx = r / 5 - 2, sy = r % 5 - 2;
+      const int32_t v = (int32_t)(uk[q] / 25);
+      const int r = (int)(uk[q] % 25);
+      const int sx = r / 5 - 2, sy = r % 5 - 2;
       L.slot_vertex[s0 + q] = v;
       // relative to the tile's anchor vertex: keeps fp32 coordinates accurate to ulp(tile size), not ulp(domain)
       L.slot_xy[2 * (s0 + q)] = (xyi[2 * v] + sx * period[0]) - ax;
       L.slot_xy[2 * (s0 + q) + 1] = (xyi[2 * v + 1] + sy * period[1]) - ay;
     }
     for (int64_t t = t0; t < t1; ++t)
-      for (int j = 0; j < 3; ++j) L.slot_ent_off[s0 + L.tile_tri[((size_t)b * T + (t - t0)) * 4 + j] + 1]++;
+      for (int j = 0; j < 3; ++j) deg[std::lower_bound(uk.begin(), uk.end(), node_key(t, j, ax, ay)) - uk.begin()]++;
+    int nb = 0;
+    for (int d : deg) nb += (d + 3) / 4;
+    nbatch_of[b] = nb;
   }
-  for (int64_t s = 0; s < nslot; ++s) L.slot_ent_off[s + 1] += L.slot_ent_off[s];
+  int32_t maxb = 0;
+  for (int64_t b = 0; b < ntile; ++b) maxb = std::max(maxb, nbatch_of[b]);
+  L.maxbatch = (maxb + 1) / 2 * 2;  // 16-byte granularity
+  L.plan_stride = 4 * T + L.offn + 4 * L.maxbatch;
+
+  // geometry table: per tile the DISTINCT (bitwise) geometry records of its triangles; the record index goes into the
+  // 4th entry of the triangle's plan entry
+  std::vector<std::vector<double>> recs(ntile);
+  std::vector<int32_t> nshape_of(ntile + 1, 0);
+  std::vector<uint16_t> shape_id((size_t)ntile * T, 0);
 #pragma omp parallel for schedule(dynamic, 64)
   for (int64_t b = 0; b < ntile; ++b) {
     const int64_t t0 = b * T, t1 = std::min(nt, t0 + T);
+    const int n = (int)(t1 - t0);
+    double g[128][12];
+    int order[128];
+    for (int q = 0; q < n; ++q) {
+      const int64_t t = t0 + q;
+      for (int i = 0; i < 3; ++i) { g[q][i] = L.nx[i][t]; g[q][3 + i] = L.ny[i][t]; g[q][6 + i] = L.hl[i][t]; }
+      g[q][9] = L.area[t] / 3.0;
+      g[q][10] = L.lmax[t];
+      g[q][11] = 0.0;
+      order[q] = q;
+    }
+    std::sort(order, order + n, [&](int a, int c) { return std::memcmp(g[a], g[c], sizeof g[0]) < 0; });
+    std::vector<double> &out = recs[b];
+    int ns = 0;
+    for (int q = 0; q < n; ++q) {
+      if (q == 0 || std::memcmp(g[order[q]], g[order[q - 1]], sizeof g[0]) != 0) {
+        out.insert(out.end(), g[order[q]], g[order[q]] + 12);
+        ++ns;
+      }
+      shape_id[(size_t)b * T + order[q]] = (uint16_t)(ns - 1);
+    }
+    nshape_of[b + 1] = ns;
+  }
+  L.tile_shape_off.assign(ntile + 1, 0);
+  int32_t maxsh = 0;
+  for (int64_t b = 0; b < ntile; ++b) {
+    L.tile_shape_off[b + 1] = L.tile_shape_off[b] + nshape_of[b + 1];
+    maxsh = std::max(maxsh, nshape_of[b + 1]);
+  }
+  const int64_t nshape = L.tile_shape_off[ntile];
+  // it pays when the table is much smaller than per-triangle geometry: 96 B per record against ~60 fp64
+  // instructions per triangle and stage
+  L.geom_table = nshape * 8 <= nt;
+  L.maxshapes = maxsh;
+  if (L.geom_table) {
+    L.shape_geom.resize((size_t)nshape * 12);
+#pragma omp parallel for schedule(static)
+    for (int64_t b = 0; b < ntile; ++b)
+      std::memcpy(&L.shape_geom[(size_t)L.tile_shape_off[b] * 12], recs[b].data(), sizeof(double) * recs[b].size());
+  }
+  recs.clear();
+  recs.shrink_to_fit();
+
+  // per-tile plan record (one bulk copy): [T x 4] local slots of the three nodes + geometry record, [offn] first
+  // incidence batch of each slot, [4 maxbatch] incidence entries node * T + local triangle, 4 to a batch, ascending.
+  // Tiles with the same record share it (uniform meshes: a handful of distinct records): pass A hashes every tile's
+  // record, pass B writes one copy per distinct hash.
+  auto make_record = [&](int64_t b, uint16_t *rec) {
+    const int64_t t0 = b * T, t1 = std::min(nt, t0 + T);
     const int32_t s0 = L.tile_slot_off[b];
-    const int ns = L.tile_slot_off[b + 1] - s0;
-    std::vector<int32_t> cur(ns);
-    for (int q = 0; q < ns; ++q) cur[q] = L.slot_ent_off[s0 + q];
+    const int32_t anchor = L.tri[3 * t0];
+    const double ax = xyi[2 * anchor], ay = xyi[2 * anchor + 1];
+    const std::vector<int64_t> &uk = keys[b];
+    const int nsl = (int)uk.size(), ns_pad = L.tile_slot_off[b + 1] - s0;
+    std::fill(rec, rec + L.plan_stride, (uint16_t)0);
+    std::vector<std::vector<uint16_t>> inc(nsl);
     for (int64_t t = t0; t < t1; ++t)
       for (int j = 0; j < 3; ++j) {
-        int loc = L.tile_tri[((size_t)b * T + (t - t0)) * 4 + j];
-        L.slot_ent[cur[loc]++] = (uint16_t)((t - t0) * 4 + j);
+        const int loc = (int)(std::lower_bound(uk.begin(), uk.end(), node_key(t, j, ax, ay)) - uk.begin());
+        rec[4 * (t - t0) + j] = (uint16_t)loc;
+        inc[loc].push_back((uint16_t)(j * T + (t - t0)));
       }
+    for (int64_t t = t0; t < t1; ++t) rec[4 * (t - t0) + 3] = L.geom_table ? shape_id[(size_t)b * T + (t - t0)] : (uint16_t)0;
+    uint16_t *boff = rec + 4 * T, *ent = rec + 4 * T + L.offn;
+    int nb = 0;
+    for (int q = 0; q < L.offn; ++q) {
+      boff[q] = (uint16_t)nb;
+      if (q < nsl) {
+        std::vector<uint16_t> &e = inc[q];
+        std::sort(e.begin(), e.end(), [&](uint16_t a, uint16_t c) {  // ascending (local triangle, node): the fixed summation order
+          return (a % T) != (c % T) ? (a % T) < (c % T) : a < c;
+        });
+        for (size_t k = 0; k < (e.size() + 3) / 4 * 4; ++k) ent[4 * nb + k] = k < e.size() ? e[k] : (uint16_t)(3 * T);
+        nb += (int)((e.size() + 3) / 4);
+      }
+    }
+    (void)ns_pad;
+  };
+  std::vector<Hash128> hashes(ntile);
+#pragma omp parallel
+  {
+    std::vector<uint16_t> rec(L.plan_stride);
+#pragma omp for schedule(dynamic, 64)
+    for (int64_t b = 0; b < ntile; ++b) {
+      make_record(b, rec.data());
+      hashes[b] = hash_bytes(rec.data(), sizeof(uint16_t) * L.plan_stride);
+    }
   }
+  std::vector<int64_t> order(ntile);
+  std::iota(order.begin(), order.end(), 0);
+  std::sort(order.begin(), order.end(), [&](int64_t a, int64_t c) { return hashes[a] < hashes[c] || (hashes[a] == hashes[c] && a < c); });
+  L.tile_plan_idx.assign(ntile, 0);
+  std::vector<int64_t> reps;
+  for (int64_t q = 0; q < ntile; ++q) {
+    if (q == 0 || !(hashes[order[q]] == hashes[order[q - 1]])) reps.push_back(order[q]);
+    L.tile_plan_idx[order[q]] = (int32_t)(reps.size() - 1);
+  }
+  L.nplan = (int64_t)reps.size();
+  L.tile_plan.assign((size_t)L.nplan * L.plan_stride, 0);
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int64_t q = 0; q < L.nplan; ++q) make_record(reps[q], &L.tile_plan[(size_t)q * L.plan_stride]);
+
   // vertex -> slots, ascending (slots are tile-major, so this is ascending triangle order)
   L.vslot_off.assign(nv + 1, 0);
-  for (int64_t s = 0; s < nslot; ++s)
-    if (L.slot_vertex[s] >= 0) L.vslot_off[L.slot_vertex[s] + 1]++;
-  for (int64_t i = 0; i < nv; ++i) L.vslot_off[i + 1] += L.vslot_off[i];
-  L.vslot_ent.resize(nslot);
+  for (int64_t i = 0; i < nv; ++i) L.vslot_off[i + 1] = L.vslot_off[i] + vcount[i];
+  L.vslot_ent.resize(L.vslot_off[nv]);
   {
     std::vector<int32_t> cur(L.vslot_off.begin(), L.vslot_off.end() - 1);
     for (int64_t s = 0; s < nslot; ++s)
       if (L.slot_vertex[s] >= 0) L.vslot_ent[cur[L.slot_vertex[s]]++] = (int32_t)s;
-  }
-  L.vslot_ent.resize(L.vslot_off[nv]);
-  // per-tile plan record, one bulk copy: [T x 4] local slots of the triangle nodes, [3T] incidence entries grouped
-  // by slot, [offn] first entry of each slot (tile-local; padded with the end value)
-  int32_t maxs = 0;
-  for (int64_t b = 0; b < ntile; ++b) maxs = std::max(maxs, L.tile_slot_off[b + 1] - L.tile_slot_off[b]);
-  L.maxslots = maxs;
-  L.offn = (maxs + 1 + 7) / 8 * 8;
-  L.plan_stride = 7 * T + L.offn;
-  L.tile_plan.assign((size_t)ntile * L.plan_stride, 0);
-#pragma omp parallel for schedule(static)
-  for (int64_t b = 0; b < ntile; ++b) {
-    uint16_t *rec = &L.tile_plan[(size_t)b * L.plan_stride];
-    std::memcpy(rec, &L.tile_tri[(size_t)b * T * 4], sizeof(uint16_t) * 4 * T);
-    const int64_t e0 = 3 * b * T, e1 = std::min<int64_t>(3 * nt, e0 + 3 * T);
-    std::memcpy(rec + 4 * T, &L.slot_ent[e0], sizeof(uint16_t) * (e1 - e0));
-    const int32_t s0 = L.tile_slot_off[b], ns = L.tile_slot_off[b + 1] - s0;
-    for (int j = 0; j < L.offn; ++j) rec[7 * T + j] = (uint16_t)(L.slot_ent_off[s0 + std::min(j, ns)] - e0);
-  }
-  // geometry table: distinct (bitwise) geometry records per tile; the record index goes into the 4th entry of tile_tri
-  {
-    std::vector<std::vector<double>> recs(ntile);
-    std::vector<int32_t> nshape_of(ntile + 1, 0);
-#pragma omp parallel for schedule(dynamic, 64)
-    for (int64_t b = 0; b < ntile; ++b) {
-      const int64_t t0 = b * T, t1 = std::min(nt, t0 + T);
-      const int n = (int)(t1 - t0);
-      double g[128][12];
-      int order[128];
-      for (int q = 0; q < n; ++q) {
-        const int64_t t = t0 + q;
-        for (int i = 0; i < 3; ++i) { g[q][i] = L.nx[i][t]; g[q][3 + i] = L.ny[i][t]; g[q][6 + i] = L.hl[i][t]; }
-        g[q][9] = L.area[t] / 3.0;
-        g[q][10] = L.lmax[t];
-        g[q][11] = 0.0;
-        order[q] = q;
-      }
-      std::sort(order, order + n, [&](int a, int c) { return std::memcmp(g[a], g[c], sizeof g[0]) < 0; });
-      std::vector<double> &out = recs[b];
-      int ns = 0;
-      for (int q = 0; q < n; ++q) {
-        if (q == 0 || std::memcmp(g[order[q]], g[order[q - 1]], sizeof g[0]) != 0) {
-          out.insert(out.end(), g[order[q]], g[order[q]] + 12);
-          ++ns;
-        }
-        L.tile_plan[(size_t)b * L.plan_stride + 4 * order[q] + 3] = (uint16_t)(ns - 1);
-      }
-      nshape_of[b + 1] = ns;
-    }
-    L.tile_shape_off.assign(ntile + 1, 0);
-    int32_t maxsh = 0;
-    for (int64_t b = 0; b < ntile; ++b) {
-      L.tile_shape_off[b + 1] = L.tile_shape_off[b] + nshape_of[b + 1];
-      maxsh = std::max(maxsh, nshape_of[b + 1]);
-    }
-    const int64_t nshape = L.tile_shape_off[ntile];
-    // it pays when the table is much smaller than per-triangle geometry: 96 B per record against ~60 fp64
-    // instructions per triangle and stage
-    L.geom_table = nshape * 8 <= nt;
-    L.maxshapes = maxsh;
-    if (L.geom_table) {
-      L.shape_geom.resize((size_t)nshape * 12);
-#pragma omp parallel for schedule(static)
-      for (int64_t b = 0; b < ntile; ++b)
-        std::memcpy(&L.shape_geom[(size_t)L.tile_shape_off[b] * 12], recs[b].data(), sizeof(double) * recs[b].size());
-    }
   }
 }
 

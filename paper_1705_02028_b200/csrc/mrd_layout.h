@@ -33,15 +33,18 @@ struct mrd_layout {
   // ---- tile plan of the fused kernels ----
   int32_t tile = 0;                    // triangles per tile (0: no plan built)
   int64_t ntile = 0, nslot = 0;
-  std::vector<int32_t> tile_slot_off;  // [ntile+1]: first slot of each tile
-  std::vector<int32_t> slot_vertex;    // [nslot]: internal vertex of each (tile-local vertex) slot
+  std::vector<int32_t> tile_slot_off;  // [ntile+1]: first slot of each tile (slot counts padded to multiples of 4)
+  std::vector<int32_t> slot_vertex;    // [nslot]: internal vertex of each (tile-local vertex) slot, -1 = padding
   std::vector<double> slot_xy;         // [nslot][2]: coordinates unwrapped into the tile's frame
-  std::vector<uint16_t> tile_tri;      // [ntile*tile][4]: tile-local vertex of nodes 0..2 (+ pad)
-  std::vector<int32_t> slot_ent_off;   // [nslot+1]: tile-local incidence of each slot ...
-  std::vector<uint16_t> slot_ent;      // ... entries (local triangle)*4 + node, ascending
   std::vector<int32_t> vslot_off, vslot_ent;  // vertex -> its slots, ascending: [nv+1], [#real slots]
-  int32_t maxslots = 0, offn = 0, plan_stride = 0;  // largest (padded) slot count of a tile; plan record sizes
-  std::vector<uint16_t> tile_plan;     // [ntile][plan_stride]: tile_tri | slot_ent | tile-local slot offsets
+  // plan record of a tile (uint16 units; one bulk copy): [4 T] per triangle the tile-local slots of its three nodes and
+  // its geometry record, [offn] first incidence batch of each slot (slot j: batches boff[j] .. boff[j+1]), [4 maxbatch]
+  // incidence entries `node * T + local triangle` in ascending (triangle, node) order, four to a batch, the last batch of a
+  // slot padded with the sentinel 3 T (which the kernels map to a zero residual).  Identical records are stored once.
+  int32_t maxslots = 0, offn = 0, maxbatch = 0, plan_stride = 0;
+  int64_t nplan = 0;                   // distinct plan records
+  std::vector<int32_t> tile_plan_idx;  // [ntile]: plan record of each tile
+  std::vector<uint16_t> tile_plan;     // [nplan][plan_stride]
   // geometry table: per tile the DISTINCT geometry records of its triangles (bitwise; uniform meshes have 2 per tile).
   // Record = nx[3], ny[3], hl[3], |T|/3, l_max, pad (12 values). Used by the tile kernels when it pays (geom_table).
   bool geom_table = false;
@@ -54,6 +57,7 @@ struct mrd_layout {
 struct mrd_partition {
   int64_t nv_g = 0, nt_g = 0, n_owned = 0;
   int32_t n_part = 1, part = 0;
+  double domain_size = 0.0;            // L of eq. 56 of the WHOLE mesh (reading C25), for the parts' mrd_params.domain_size
   std::vector<int32_t> owner;          // [nv_g]
   std::vector<int32_t> vertex_global;  // local -> global: owned (ascending), then halo (ascending)
   std::vector<double> xy;

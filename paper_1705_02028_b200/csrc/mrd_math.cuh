@@ -182,6 +182,7 @@ template <class R> struct TriCore {
   // N-hat (eq. 49): symmetric 3x3 inverse (00,01,02,11,12,22) and the entropy reciprocal
   R n00, n01, n02, n11, n12, n22, ns;
   bool ok;
+  bool stagnant;  // stagnation rule C8 applied: the entropy part of N-hat is 0
 };
 
 // y = K x in the rotated frame of edge (nx, ny) with coefficients (a, b, l3):
@@ -309,22 +310,25 @@ __device__ __forceinline__ void triangle_core(R gamma, const Vec4<R> Z[3], const
     k.ap[i] = ap;
     k.bp[i] = bp;
     k.l3p[i] = l3p;
+    // with nxx + nyy = 1: s11 = sum_j (a- - l3-) nxx + sum_j l3-, s22 likewise with nyy (two instructions fewer per edge
+    // than accumulating a- nxx + l3- nyy); the entropy sum s33 is added after the loop
     R nxx = nx * nx, nyy = ny * ny, nxy = nx * ny;
+    R dm = am - l3m;
     if (i == 0) {  // (0 + x is not x for x = -0, so the compiler keeps additions to a zero accumulator)
       s00 = am;
       s01 = bm * nx;
       s02 = bm * ny;
-      s11 = F::fma_(am, nxx, l3m * nyy);
-      s12 = (am - l3m) * nxy;
-      s22 = F::fma_(am, nyy, l3m * nxx);
+      s11 = dm * nxx;
+      s12 = dm * nxy;
+      s22 = dm * nyy;
       s33 = l3m;
     } else {
       s00 += am;
       s01 = F::fma_(bm, nx, s01);
       s02 = F::fma_(bm, ny, s02);
-      s11 = F::fma_(am, nxx, F::fma_(l3m, nyy, s11));
-      s12 = F::fma_(am - l3m, nxy, s12);
-      s22 = F::fma_(am, nyy, F::fma_(l3m, nxx, s22));
+      s11 = F::fma_(dm, nxx, s11);
+      s12 = F::fma_(dm, nxy, s12);
+      s22 = F::fma_(dm, nyy, s22);
       s33 += l3m;
     }
     if (i == 1) {
@@ -336,6 +340,8 @@ __device__ __forceinline__ void triangle_core(R gamma, const Vec4<R> Z[3], const
     }
   }
 
+  s11 += s33;
+  s22 += s33;
   // O5: N-hat = (sum K^-)^-1: cofactor inverse of the symmetric 3x3 block, reciprocal of the entropy
   // scalar; stagnation rule (reading C8): u^2 + v^2 <= (1e-14 c)^2 -> entropy part of N-hat = 0
   R c00 = s11 * s22 - s12 * s12;
@@ -349,7 +355,8 @@ __device__ __forceinline__ void triangle_core(R gamma, const Vec4<R> Z[3], const
   k.n00 = c00 * idet; k.n01 = c01 * idet; k.n02 = c02 * idet;
   k.n11 = c11 * idet; k.n12 = c12 * idet; k.n22 = c22 * idet;
   const R eps = R(1e-14);
-  bool stagnant = (R(2) * k.hq2 <= (eps * eps) * c2) || !(s33 < R(0));
+  const bool stagnant = (R(2) * k.hq2 <= (eps * eps) * c2) || !(s33 < R(0));
+  k.stagnant = stagnant;
   k.ns = stagnant ? R(0) : F::rcp(stagnant ? R(-1) : s33);
 
   // eq. 48: phi_i^N = K_i^+ (dq_i - N-hat sum_j K_j^- dq_j)
@@ -375,22 +382,34 @@ __device__ __forceinline__ void triangle_core(R gamma, const Vec4<R> Z[3], const
 }
 
 // eq. 50-51: out_i = beta_i X = -K_i^+ N-hat X for a conserved-variable vector X (phi^T in stage 1,
-// Phi^T in stage 2: eq. 63 with eq. 65, reading C12)
+// Phi^T in stage 2: eq. 63 with eq. 65, reading C12).  Nodes 0 and 1 directly; node 2 from sum_i beta_i = I, which holds
+// identically (sum_i K_i^+ = -sum_j K_j^- and N-hat is its inverse) except for the entropy component under the
+// stagnation rule C8, where that part of N-hat is 0: there the three residuals add up to X minus its entropy part
+// M (0, 0, 0, q_3) = -(q_3 / c^2) (1, u, v, (u^2 + v^2)/2).  8-13 instructions instead of the ~22 of a third projection.
 template <class R>
-__device__ __forceinline__ void apply_beta(R gamma, const TriCore<R> &k, const TriGeom<R> &g, const R X[4], R out[3][4]) {
-  R q[4];
-  to_symmetrising(gamma - R(1), k, X, q);
+__device__ __forceinline__ void lda_from_symmetrised(const TriCore<R> &k, const TriGeom<R> &g, const R X[4], const R q[4], R out[3][4]) {
   R y[4];
   y[0] = -(k.n00 * q[0] + k.n01 * q[1] + k.n02 * q[2]);
   y[1] = -(k.n01 * q[0] + k.n11 * q[1] + k.n12 * q[2]);
   y[2] = -(k.n02 * q[0] + k.n12 * q[1] + k.n22 * q[2]);
   y[3] = -(k.ns * q[3]);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) {
+  for (int i = 0; i < 2; ++i) {
     R z[4];
     apply_split<false>(k.ap[i], k.bp[i], k.l3p[i], g.nx[i], g.ny[i], y, z);
     to_conserved(k, z, out[i]);
   }
+  const R e3 = k.stagnant ? q[3] * k.ic2 : R(0);
+  out[2][0] = ((X[0] + e3) - out[0][0]) - out[1][0];
+  out[2][1] = (Fast<R>::fma_(k.u, e3, X[1]) - out[0][1]) - out[1][1];
+  out[2][2] = (Fast<R>::fma_(k.v, e3, X[2]) - out[0][2]) - out[1][2];
+  out[2][3] = (Fast<R>::fma_(k.hq2, e3, X[3]) - out[0][3]) - out[1][3];
+}
+template <class R>
+__device__ __forceinline__ void apply_beta(R gamma, const TriCore<R> &k, const TriGeom<R> &g, const R X[4], R out[3][4]) {
+  R q[4];
+  to_symmetrising(gamma - R(1), k, X, q);
+  lda_from_symmetrised(k, g, X, q, out);
 }
 
 // eq. 52-53 (+ reading C10): Theta_kk = min(1, |X_k| / sum_j |N_j,k|), 0 when the denominator is 0;
@@ -399,14 +418,43 @@ __device__ __forceinline__ void apply_beta(R gamma, const TriCore<R> &k, const T
 // L503)
 template <class R> __device__ __forceinline__ void blend_theta(const R X[4], const R N[3][4], int bvar, R th[4]) {
   using F = Fast<R>;
+  // Theta = min(1, |X| / den), and 0 on a zero denominator (C10).  den = 0 means every nodal residual is exactly 0,
+  // which makes X and the LDA residuals exactly 0 too, so the value taken there (1) changes nothing: B_i = 0.
+  R den[4];
 #pragma unroll
-  for (int c = 0; c < 4; ++c) {
-    // Theta = min(1, |X| / den), and 0 on a zero denominator (C10).  den = 0 means every nodal residual is exactly 0,
-    // which makes X and the LDA residuals exactly 0 too, so the value taken there (1) changes nothing: B_i = 0.
-    R den = F::abs(N[0][c]) + F::abs(N[1][c]) + F::abs(N[2][c]);
-    // Written so that a zero or denormal denominator (reciprocal inf, product inf or NaN) also lands on 1.
-    R t = F::abs(X[c]) * F::rcp(den);
-    th[c] = t < R(1) ? t : R(1);
+  for (int c = 0; c < 4; ++c) den[c] = F::abs(N[0][c]) + F::abs(N[1][c]) + F::abs(N[2][c]);
+  if (sizeof(R) == 8) {
+    // fp64: the four reciprocals from ONE (seed + Newton) reciprocal of the product of the denominators (the seed
+    // instruction and its fix-ups are the expensive part): 1/d_0 = d_1 (d_2 d_3) / P, ...  Zero denominators are replaced
+    // by 1 (their Theta is 1 whatever the quotient); should the product leave the normal range (denominators below
+    // ~1e-75 each), the components fall back to one reciprocal each.
+    R d[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) d[c] = den[c] > R(0) ? den[c] : R(1);
+    const R p01 = d[0] * d[1], p23 = d[2] * d[3], P = p01 * p23;
+    if (P > R(1e-290) && P < R(1e290)) {
+      const R r = F::rcp(P);
+      const R r01 = r * p23, r23 = r * p01;   // 1 / (d0 d1), 1 / (d2 d3)
+      const R inv[4] = {r01 * d[1], r01 * d[0], r23 * d[3], r23 * d[2]};
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        R t = F::abs(X[c]) * inv[c];
+        th[c] = (den[c] > R(0) && t < R(1)) ? t : R(1);
+      }
+    } else {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        R t = F::abs(X[c]) * F::rcp(d[c]);
+        th[c] = (den[c] > R(0) && t < R(1)) ? t : R(1);
+      }
+    }
+  } else {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      // Written so that a zero or denormal denominator (reciprocal inf, product inf or NaN) also lands on 1.
+      R t = F::abs(X[c]) * F::rcp(den[c]);
+      th[c] = t < R(1) ? t : R(1);
+    }
   }
   if (bvar != 0) {
     R hi = F::max(F::max(th[0], th[1]), F::max(th[2], th[3]));

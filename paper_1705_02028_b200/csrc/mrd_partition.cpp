@@ -29,6 +29,15 @@ int partition_build(mrd_partition &P, int64_t nv, const double *xy, int64_t nt, 
   for (int64_t e = 0; e < 2 * ne; ++e)
     if (wall_edge[e] < 0 || wall_edge[e] >= nv) { err = "bad wall edge"; return MRD_EINVAL; }
   P.nv_g = nv; P.nt_g = nt; P.n_part = n_part; P.part = part;
+  {  // L of the Bx sensor (eq. 56, reading C25) of the WHOLE mesh: every part must use the same value
+    double lo[2] = {xy[0], xy[1]}, hi[2] = {xy[0], xy[1]};
+    for (int64_t i = 0; i < nv; ++i)
+      for (int d = 0; d < 2; ++d) {
+        lo[d] = std::min(lo[d], xy[2 * i + d]);
+        hi[d] = std::max(hi[d], xy[2 * i + d]);
+      }
+    P.domain_size = std::max(period_x > 0.0 ? period_x : hi[0] - lo[0], period_y > 0.0 ? period_y : hi[1] - lo[1]);
+  }
 
   // owners: part q owns positions [q nv / P, (q+1) nv / P) of the Morton order
   {

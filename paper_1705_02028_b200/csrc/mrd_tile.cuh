@@ -3,29 +3,33 @@
 // walk over tiles with a two-deep software pipeline:
 //
 //   stage-in : everything a tile needs lives in CONTIGUOUS global ranges (slot-major copies of Z, |v|+c,
-//              dW/dt written by the vertex kernels; tile-frame coordinates; the tile's plan record; for
-//              stage 2 the stored phi^N(W^n), phi^T(W^n)), so one thread brings the tile AFTER NEXT in with a
-//              handful of TMA bulk copies (cp.async.bulk + mbarrier complete_tx) as soon as the last warp has
-//              left the buffer it goes into -- no gather by vertex index, no dependent global latency;
-//   body     : one thread per triangle; geometry of eq. 35 (L397-L399) from the staged coordinates, then
-//              S2-S5 / S9 of SURVEY 8a with the same device functions as the unfused kernels;
-//   epilogue : distributed residuals -> shared memory; every slot sums its incident (triangle, node) entries
-//              in ascending order; ONE partial per slot leaves the SM (deterministic; replaces the float
-//              atomics of L734 and the 3 x 4 values per triangle of the unfused design).  One block barrier
-//              per tile (between the residuals and their sums); warps that are done move on to the next tile.
-// The vertex kernels add a vertex's few partials (ascending slot = ascending triangle order) and scatter
-// the new per-vertex quantities back to the vertex's slots.
+//              dW/dt written by the vertex side; tile-frame coordinates or geometry records; the tile's plan
+//              record; for stage 2 the stored phi^N(W^n), phi^T(W^n)), so one thread brings the tile AFTER NEXT
+//              in with a handful of TMA bulk copies (cp.async.bulk + mbarrier complete_tx) as soon as the last
+//              warp has left the buffer it goes into -- no gather by vertex index, no dependent global latency;
+//   body     : one thread per triangle; geometry of eq. 35 (L397-L399) from the geometry table or the staged
+//              coordinates, then S2-S5 / S9 of SURVEY 8a with the device functions of mrd_math.cuh;
+//   epilogue : distributed residuals -> shared memory (16-byte cells); every slot sums its incident (triangle,
+//              node) entries in ascending order, four to a batch with all loads issued before the first add; ONE
+//              partial per slot leaves the SM (deterministic; replaces the float atomics of L734 and the 3 x 4
+//              values per triangle of the unfused design).
+// The vertex kernels add a vertex's few partials (ascending slot = ascending triangle order) and scatter the new
+// per-vertex quantities back to the vertex's slots.  (Finishing the vertices inside the tile kernels -- directly for
+// the 77 % whose fan lies in one tile, by the last tile to arrive for the rest -- was built and measured in round 2:
+// the arithmetic of a vertex update costs the fp64-bound tile kernels what it costs, the vertex kernels hide it under
+// their HBM time, and the arrival protocol adds a chain of L2 round trips per tile; see profiles/r02_experiments.md.)
+// One block barrier per tile (between the residuals and their sums); warps that are done move on to the next tile.
 #pragma once
 #include "mrd_kernels.cuh"
 
 namespace mrd {
 
 template <class R> struct TileDev {
-  int32_t tile, maxslots, offn, plan_stride, maxshapes;
-  int64_t ntile, nslot, nt;
-  const int2 *tile_info;         // [ntile+1]: .x first slot (padded slot counts: multiples of 4), .y first geometry record
+  int32_t tile, maxslots, offn, maxbatch, plan_stride, maxshapes;
+  int64_t ntile, nslot, nt, nv;
+  const int4 *tile_info;         // [ntile+1]: .x first slot (padded slot counts: multiples of 4), .y first geometry record, .z plan record
   const R *shape_geom;           // [nshape][12] geometry records (GTAB kernels), else null
-  const uint16_t *plan;          // [ntile][plan_stride]: tile_tri[T][4] | ent[3T] | off[offn]
+  const uint16_t *plan;          // [nplan][plan_stride]: tri[T][4] | boff[offn] | ent[4 maxbatch]  (mrd_layout.h)
   const R *slot_xy;              // [nslot][2], relative to the tile's anchor vertex
   const int32_t *vslot_off;      // [nv+1]
   const int32_t *vslot_ent;      // [#real slots]
@@ -60,19 +64,25 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned by
 // tile_info prefetch: a plain (per-thread register) global load whose result is handed over through an opaque
 // move at the point of use.  Without this the compiler turns the block-uniform value into a uniform register
 // right after the load (R2UR), stalling every warp on the global latency once per tile (10 % of all stall samples).
-__device__ __forceinline__ int2 ld_info(const int2 *p) {
-  int2 v;
-  asm volatile("ld.global.nc.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+__device__ __forceinline__ int4 ld_info(const int4 *p) {
+  int4 v;
+  asm volatile("ld.global.nc.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
   return v;
 }
-__device__ __forceinline__ int2 use_info(int2 v) {
-  int2 o;
-  asm volatile("mov.b32 %0, %2;\n\tmov.b32 %1, %3;" : "=r"(o.x), "=r"(o.y) : "r"(v.x), "r"(v.y));
+__device__ __forceinline__ int4 use_info(int4 v) {
+  int4 o;
+  asm volatile("mov.b32 %0, %4;\n\tmov.b32 %1, %5;\n\tmov.b32 %2, %6;\n\tmov.b32 %3, %7;"
+               : "=r"(o.x), "=r"(o.y), "=r"(o.z), "=r"(o.w)
+               : "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w));
   return o;
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
+// shared-memory cells of the residual exchange (two components each: 16 bytes in fp64)
+template <class R> struct Cell;
+template <> struct __align__(16) Cell<double> { double a, b; };
+template <> struct __align__(8) Cell<float> { float a, b; };
 // geometry of one CCW triangle from its vertex coordinates (eq. 35; reading C4):
 // the edge opposite node i runs from node i+1 to node i+2, inward normal (-e_y, e_x)
 template <class R>
@@ -95,26 +105,37 @@ __device__ __forceinline__ void tile_geometry(const R x[3], const R y[3], TriGeo
 }
 
 // ---- shared-memory carve-up (dynamic).  Two stage-in buffers + the residual exchange area ----------------
+// Residual cells of one tile (T triangles): cell (half h, node i, triangle t) at index h HOFF + i T + t holds the
+// components (2h, 2h + 1) of the residual sent to node i; HOFF = 3T + 1 (fp64; 3T + 2 in fp32, which keeps the second half
+// 16-byte aligned for the bulk copies).  The cells 3T and HOFF + 3T stay zero: they are what the sentinel incidence entry
+// 3T of the plan reads.
+template <class R, int T> struct CellGeom {
+  static constexpr int HOFF = 3 * T + 16 / (int)sizeof(Cell<R>);
+  static constexpr int NCELL = HOFF + 3 * T + 1;
+};
 template <class R, int STAGE, bool GTAB> struct TileSmem {
   // computed once on the host and passed to the kernel by value (the device code recomputed it every tile otherwise)
   uint32_t oZ, oD, oS, oXY, oPlan, oPhi, buf_bytes;  // per buffer (oXY holds the geometry records when GTAB)
-  uint32_t oRes, oST, oBar, total;                   // shared
+  uint32_t oRes, oST, oBar, total;                          // shared
+  uint32_t res_bytes, st_bytes;
   __host__ __device__ static uint32_t up16(size_t x) { return (uint32_t)((x + 15) & ~size_t(15)); }
   __host__ __device__ TileSmem(int T, int maxslots, int plan_stride, int maxshapes) {
     uint32_t o = 0;
+    res_bytes = up16(sizeof(Cell<R>) * (6 * T + 16 / sizeof(Cell<R>) + 1));
+    st_bytes = up16(sizeof(R) * (3 * T + 1));
     oZ = o; o += up16(sizeof(Vec4<R>) * maxslots);
     oD = o; if (STAGE == 2) o += up16(sizeof(Vec4<R>) * maxslots);
     oS = o; if (STAGE == 1) o += up16(sizeof(R) * maxslots);
     oXY = o; o += GTAB ? up16(sizeof(R) * 12 * maxshapes) : up16(sizeof(R) * 2 * maxslots);
     oPlan = o; o += up16(sizeof(uint16_t) * plan_stride);
-    oPhi = o; if (STAGE == 2) o += up16(sizeof(R) * 16 * T);
+    // stage 2: the stored stage-1 residuals arrive in the cell layout, and the residual exchange area IS that block --
+    // thread `tid` only overwrites the six cells it has consumed itself (saves 12 KB: 4 blocks per SM)
+    oPhi = o; if (STAGE == 2) o += res_bytes;
     buf_bytes = (o + 31u) & ~31u;
     uint32_t s = 2 * buf_bytes;
-    // stage 2: the residual exchange area aliases the current buffer's phi16 block -- thread `tid` only overwrites the
-    // 12 entries [c][tid] it has consumed itself, so no other thread's data is touched (saves 12 KB: 4 blocks per SM)
     // stage 1: two residual areas (tile k's epilogue may still read one while a faster warp writes tile k+1's)
-    oRes = s; if (STAGE == 1) s += 2 * (uint32_t)(sizeof(R) * 12 * T);
-    oST = s; if (STAGE == 1) s += 2 * up16(sizeof(R) * T);
+    oRes = s; if (STAGE == 1) s += 2 * res_bytes;
+    oST = s; if (STAGE == 1) s += 2 * st_bytes;
     oBar = s; s += 32;  // two mbarriers, two "warps done with the buffer" counters
     total = s;
   }
@@ -123,106 +144,110 @@ template <class R, int STAGE, bool GTAB> struct TileSmem {
 // bring tile b into buffer `buf` (one thread): expect_tx, then the bulk copies
 template <class R, int STAGE, bool GTAB>
 __device__ __forceinline__ void tile_stage_in(const TileDev<R> &td, const TileSmem<R, STAGE, GTAB> &L, unsigned char *buf,
-                                              uint64_t *bar, int64_t b, int2 i0, int2 i1, const Vec4<R> *slotZ,
-                                              const R *slotS, const Vec4<R> *slotD, const R *phi16) {
+                                              uint64_t *bar, int64_t b, int4 i0, int4 i1, const Vec4<R> *slotZ,
+                                              const R *slotS, const Vec4<R> *slotD, const R *phi12) {
   const int T = td.tile;
   const int s0 = i0.x, ns = i1.x - i0.x;
   const unsigned bZ = sizeof(Vec4<R>) * ns, bS = sizeof(R) * ns;
   const unsigned bXY = GTAB ? sizeof(R) * 12 * (i1.y - i0.y) : sizeof(R) * 2 * ns;
-  const unsigned bPlan = sizeof(uint16_t) * td.plan_stride, bPhi = sizeof(R) * 16 * T;
-  unsigned total = bZ + bXY + bPlan + (STAGE == 1 ? bS : bZ + bPhi);
+  const unsigned bPlan = sizeof(uint16_t) * td.plan_stride, bHalf = sizeof(Cell<R>) * 3 * T;
+  unsigned total = bZ + bXY + bPlan + (STAGE == 1 ? bS : bZ + 2 * bHalf);
   mbar_expect_tx(bar, total);
   bulk_g2s(buf + L.oZ, slotZ + s0, bZ, bar);
   if (GTAB) bulk_g2s(buf + L.oXY, td.shape_geom + 12 * (int64_t)i0.y, bXY, bar);
   else bulk_g2s(buf + L.oXY, td.slot_xy + 2 * (int64_t)s0, bXY, bar);
-  bulk_g2s(buf + L.oPlan, td.plan + b * td.plan_stride, bPlan, bar);
+  bulk_g2s(buf + L.oPlan, td.plan + (int64_t)i0.z * td.plan_stride, bPlan, bar);
   if (STAGE == 1) {
     bulk_g2s(buf + L.oS, slotS + s0, bS, bar);
   } else {
     bulk_g2s(buf + L.oD, slotD + s0, bZ, bar);
-    bulk_g2s(buf + L.oPhi, phi16 + b * 16 * T, bPhi, bar);
+    const R *src = phi12 + b * 12 * T;                       // [half][3 T] cells of two values
+    bulk_g2s(buf + L.oPhi, src, bHalf, bar);
+    bulk_g2s(buf + L.oPhi + sizeof(Cell<R>) * (3 * T + 16 / sizeof(Cell<R>)), src + 6 * T, bHalf, bar);
   }
 }
 
-// epilogue shared by both stages: per slot, ascending sum of its tile-local incidences (all from shared memory).
-// (A (slot, component)-parallel variant was measured: 15 % slower -- the kernel is issue-bound, not barrier-bound.)
-template <class R, bool WITH_ST>
-__device__ __forceinline__ void tile_epilogue(int T, const R *res, const R *sT, const uint16_t *ent, const uint16_t *off,
-                                              int s0, int ns, Vec4<R> *__restrict__ part, R *__restrict__ partS) {
-  // The incidences of a slot are fetched EPI at a time, all loads issued before the first add: the plain loop is a chain of
-  // dependent shared-memory loads (entry -> residual -> add) per incidence, ~70 cycles each, and every warp of the block
-  // waits for the slowest one at the barrier before this.  Missing incidences add +0.0, which changes nothing.
-  constexpr int EPI = 8;
-  for (int j = threadIdx.x; j < ns; j += T) {
-    const int q0 = off[j], q1 = off[j + 1];
-    R a0 = 0, a1 = 0, a2 = 0, a3 = 0, S = 0;
-    for (int q = q0; q < q1; q += EPI) {
-      R v[EPI][4], sv[EPI];
+// sum of the tile-local incidences of one slot, in ascending (triangle, node) order, from the residual cells
+template <class R, int T, bool WITH_ST>
+__device__ __forceinline__ void slot_sum(const Cell<R> *cell, const R *sTx, const uint16_t *ent, int b0, int b1, R a[4], R &S) {
+  a[0] = a[1] = a[2] = a[3] = R(0);
+  S = R(0);
+  for (int q = b0; q < b1; ++q) {
+    const uint2 pk = *reinterpret_cast<const uint2 *>(ent + 4 * q);   // four entries; all loads issued before the first add
+    const unsigned e[4] = {pk.x & 0xFFFFu, pk.x >> 16, pk.y & 0xFFFFu, pk.y >> 16};
+    Cell<R> lo[4], hi[4];
+    R sv[4];
 #pragma unroll
-      for (int u = 0; u < EPI; ++u) {
-        const bool on = q + u < q1;
-        const int e = on ? ent[q + u] : 0;
-        const int lt = e >> 2, nd = e & 3;
-        const R *r = res + (nd * 4) * T + lt;
-        v[u][0] = on ? r[0] : R(0);
-        v[u][1] = on ? r[T] : R(0);
-        v[u][2] = on ? r[2 * T] : R(0);
-        v[u][3] = on ? r[3 * T] : R(0);
-        if (WITH_ST) sv[u] = on ? sT[lt] : R(0);
-      }
-#pragma unroll
-      for (int u = 0; u < EPI; ++u) {
-        a0 += v[u][0];
-        a1 += v[u][1];
-        a2 += v[u][2];
-        a3 += v[u][3];
-        if (WITH_ST) S += sv[u];
-      }
+    for (int u = 0; u < 4; ++u) {
+      lo[u] = cell[e[u]];
+      hi[u] = cell[e[u] + CellGeom<R, T>::HOFF];
+      if (WITH_ST) sv[u] = sTx[e[u]];
     }
-    st4(&part[s0 + j], Vec4<R>{a0, a1, a2, a3});
-    if (WITH_ST) partS[s0 + j] = S;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      a[0] += lo[u].a;
+      a[1] += lo[u].b;
+      a[2] += hi[u].a;
+      a[3] += hi[u].b;
+      if (WITH_ST) S += sv[u];
+    }
   }
 }
 
-// STAGE 1: SCHEME residuals of W^n -> partials, s_T sums, and (STORE) phi^N(W^n), phi^T(W^n) as phi16[tile][16][T]
+// STAGE 1: SCHEME residuals of W^n -> partials, s_T sums, and (STORE) phi^N(W^n), phi^T(W^n) as phi12
 // STAGE 2: total residuals (eq. 57, 61-65; reading C12) -> partials
 #ifndef MRD_TILE_MINB
 #define MRD_TILE_MINB 4
 #endif
+template <class R> struct TileIO {
+  const Vec4<R> *slotZ;    // Z of the state the stage reads (slot-major)
+  const R *slotS;          // stage 1: |v| + c
+  const Vec4<R> *slotD;    // stage 2: dW/dt of stage 1
+  R *phi12;                // [ntile][12 T]: phi_0^N, phi_1^N, phi^T of W^n in the cell layout (written by stage 1, read by stage 2)
+  Vec4<R> *part;           // [nslot] out: one partial residual sum per slot
+  R *partS;                // [nslot] out, stage 1: partial s_T sums
+  Vec4<R> *phi_dbg;        // dumps: per-triangle distributed residuals [nt][3], or null
+  R *sT_dbg;
+};
 // STORE: stage 1 keeps phi^N(W^n), phi^T(W^n) for stage 2; stage 2 reuses the flag for selective lumping (eq. 66-67), a
 // compile-time switch because the extra live ranges of a run-time branch cost the headline configuration 8 %.
 template <class R, int SCHEME, int STAGE, bool STORE, int TILE, bool GTAB>
 __global__ void __launch_bounds__(TILE, (MRD_TILE_MINB * 128) / TILE)
-tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl *__restrict__ ctl, const Vec4<R> *__restrict__ slotZ,
-            const R *__restrict__ slotS, const Vec4<R> *__restrict__ slotD, R *__restrict__ phi16,
-            Vec4<R> *__restrict__ part, R *__restrict__ partS, Vec4<R> *__restrict__ phi_dbg, R *__restrict__ sT_dbg,
-            int *status) {
+tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl *__restrict__ ctl, TileIO<R> io, int *status) {
   MRD_CTL_GUARD(ctl)
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  constexpr int T = TILE;  // compile-time tile size: shared-memory and phi16 strides become immediates
+  constexpr int T = TILE;  // compile-time tile size: shared-memory and cell strides become immediates
+  constexpr int HOFF = CellGeom<R, TILE>::HOFF;
   const int tid = threadIdx.x;
-  R *res1 = reinterpret_cast<R *>(smem_raw + L.oRes);
-  R *sST = reinterpret_cast<R *>(smem_raw + L.oST);
   uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + L.oBar);
   unsigned *done = reinterpret_cast<unsigned *>(smem_raw + L.oBar + 16);
   constexpr unsigned NW = TILE / 32;
   int64_t b = blockIdx.x;
   // slot / geometry-record range of the tile in flight (i0, i1); the next tile's range is fetched one iteration ahead
-  int2 i0 = __ldg(td.tile_info + b), i1 = __ldg(td.tile_info + b + 1);
+  int4 i0 = __ldg(td.tile_info + b), i1 = __ldg(td.tile_info + b + 1);
   if (tid == 0) {
     mbar_init(&bar[0], 1);
     mbar_init(&bar[1], 1);
     done[0] = done[1] = 0;
     fence_mbar_init();
     // the first two tiles of this block; every later copy is issued by the last warp to leave the buffer it refills
-    tile_stage_in<R, STAGE, GTAB>(td, L, smem_raw, &bar[0], b, i0, i1, slotZ, slotS, slotD, phi16);
+    tile_stage_in<R, STAGE, GTAB>(td, L, smem_raw, &bar[0], b, i0, i1, io.slotZ, io.slotS, io.slotD, io.phi12);
     const int64_t b1 = b + gridDim.x;
     if (b1 < td.ntile)
       tile_stage_in<R, STAGE, GTAB>(td, L, smem_raw + L.buf_bytes, &bar[1], b1, __ldg(td.tile_info + b1), __ldg(td.tile_info + b1 + 1),
-                                    slotZ, slotS, slotD, phi16);
+                                    io.slotZ, io.slotS, io.slotD, io.phi12);
+  }
+  // the zero cells (what the sentinel incidence entry reads) of both residual areas; nothing ever writes them again
+  if (tid < 2) {
+    for (int k = 0; k < 2; ++k) {
+      unsigned char *area = STAGE == 1 ? smem_raw + L.oRes + k * L.res_bytes : smem_raw + k * L.buf_bytes + L.oPhi;
+      Cell<R> *c = reinterpret_cast<Cell<R> *>(area);
+      c[tid == 0 ? 3 * T : CellGeom<R, T>::HOFF + 3 * T] = Cell<R>{R(0), R(0)};
+      if (STAGE == 1 && tid == 0) reinterpret_cast<R *>(smem_raw + L.oST + k * L.st_bytes)[3 * T] = R(0);
+    }
   }
   __syncthreads();
-  int2 n0 = make_int2(0, 0), n1 = make_int2(0, 0);
+  int4 n0 = make_int4(0, 0, 0, 0), n1 = n0;
   const int bvar = ctl->bvar;
   const R bxL = (R)ctl->bx_L, bxInv = SCHEME == MRD_SCHEME_BX ? (R)bx_inv_range(ctl, STAGE - 1) : R(0);
   constexpr bool lump = STAGE == 2 && STORE;
@@ -240,14 +265,14 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
     const Vec4<R> *sZ = reinterpret_cast<const Vec4<R> *>(buf + L.oZ);
     const R *sXY = reinterpret_cast<const R *>(buf + L.oXY);
     const uint16_t *plan = reinterpret_cast<const uint16_t *>(buf + L.oPlan);
-    R *res = STAGE == 1 ? res1 + cur * (12 * T) : reinterpret_cast<R *>(buf + L.oPhi);
-    R *sSTc = sST + cur * T;
+    Cell<R> *cell = reinterpret_cast<Cell<R> *>(STAGE == 1 ? smem_raw + L.oRes + cur * L.res_bytes : buf + L.oPhi);
+    R *sTx = reinterpret_cast<R *>(smem_raw + L.oST + cur * L.st_bytes);
     const int64_t t = b * T + tid;
-    R pN[3][4];
     R st = R(0);
     // (no branch around the body: a padding triangle of the last tile computes on triangle 0 and its results are zeroed)
     const bool valid = t < td.nt;
     {
+      R pN[3][4];
       const ushort4 lv = reinterpret_cast<const ushort4 *>(plan)[valid ? tid : 0];
       const int l[3] = {lv.x, lv.y, lv.z};
       Vec4<R> z[3] = {sZ[l[0]], sZ[l[1]], sZ[l[2]]};
@@ -271,21 +296,30 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
       if (STAGE == 1) {
         const R *sS = reinterpret_cast<const R *>(buf + L.oS);
         st = lmax * Fast<R>::max(sS[l[0]], Fast<R>::max(sS[l[1]], sS[l[2]]));  // eq. 44-45
-        if (STORE) {
-          R *o = phi16 + b * 16 * T + tid;
+        if (STORE) {  // phi_0^N, phi_1^N and phi^T of W^n (phi_2^N follows from them, mrd_math.cuh): 12 values per triangle
+          Cell<R> *o = reinterpret_cast<Cell<R> *>(io.phi12 + b * 12 * T) + tid;
 #pragma unroll
-          for (int i = 0; i < 3; ++i)
-#pragma unroll
-            for (int c = 0; c < 4; ++c) o[(i * 4 + c) * T] = pN[i][c];
-#pragma unroll
-          for (int c = 0; c < 4; ++c) o[(12 + c) * T] = pT[c];
+          for (int h = 0; h < 2; ++h) {
+            o[(h * 3 + 0) * T] = Cell<R>{pN[0][2 * h], pN[0][2 * h + 1]};
+            o[(h * 3 + 1) * T] = Cell<R>{pN[1][2 * h], pN[1][2 * h + 1]};
+            o[(h * 3 + 2) * T] = Cell<R>{pT[2 * h], pT[2 * h + 1]};
+          }
         }
       } else {
         // eq. 57 / 61: Phi^T = |T|/3 sum_j dW_j/dt + (phi^T(W^n) + phi^T(W*))/2;  eq. 62 per node
         const Vec4<R> *sD = reinterpret_cast<const Vec4<R> *>(buf + L.oD);
-        const R *sP = reinterpret_cast<const R *>(buf + L.oPhi) + tid;
+        R oN[3][4], oT[4];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) X[c] = R(0.5) * (sP[(12 + c) * T] + pT[c]);
+        for (int h = 0; h < 2; ++h) {
+          const Cell<R> c0 = cell[h * HOFF + tid], c1 = cell[h * HOFF + T + tid], c2 = cell[h * HOFF + 2 * T + tid];
+          oN[0][2 * h] = c0.a; oN[0][2 * h + 1] = c0.b;
+          oN[1][2 * h] = c1.a; oN[1][2 * h + 1] = c1.b;
+          oT[2 * h] = c2.a; oT[2 * h + 1] = c2.b;
+        }
+#pragma unroll
+        for (int c = 0; c < 4; ++c) oN[2][c] = (oT[c] - oN[0][c]) - oN[1][c];   // as stage 1 formed phi_2^N: bitwise its value
+#pragma unroll
+        for (int c = 0; c < 4; ++c) X[c] = R(0.5) * (oT[c] + pT[c]);
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
           Vec4<R> d = sD[l[i]];
@@ -293,7 +327,7 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
 #pragma unroll
           for (int c = 0; c < 4; ++c) {
             X[c] += m[c];
-            pN[i][c] = m[c] + R(0.5) * (pN[i][c] + sP[(i * 4 + c) * T]);
+            pN[i][c] = m[c] + R(0.5) * (pN[i][c] + oN[i][c]);
           }
         }
         if (lump) {  // selective lumping (eq. 66-67): E_i = sum_j (|T| d_ij/3 - m^G_ij) dW_j/dt = |T|/12 (3 dW_i - sum_j dW_j)
@@ -309,60 +343,77 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
         }
       }
       // The nodal N residuals go to shared memory now (their final place for scheme N); the LDA residuals are then
-      // produced node by node and blended in place -- 24 fewer values live at once than blending from registers.
+      // produced and blended in place -- 24 fewer values live at once than blending from registers.
       R th[4] = {0, 0, 0, 0};
       if (SCHEME == MRD_SCHEME_B) blend_theta(X, pN, bvar, th);  // eq. 53 (+ C10); Bmax / Bmin: L503
       if (SCHEME == MRD_SCHEME_BX)                               // eq. 54-56: one theta from the shock sensor of this stage's state
         th[0] = th[1] = th[2] = th[3] = bx_theta(z, g, a3, lmax, bxL, bxInv);
 #pragma unroll
-      for (int c = 0; c < 4; ++c)
+      for (int i = 0; i < 3; ++i)
 #pragma unroll
-        for (int i = 0; i < 3; ++i) res[(i * 4 + c) * T + tid] = pN[i][c];
+        for (int h = 0; h < 2; ++h) cell[h * HOFF + i * T + tid] = Cell<R>{pN[i][2 * h], pN[i][2 * h + 1]};
       if (SCHEME != MRD_SCHEME_N) {
         // eq. 50-51 (stage 2: eq. 63 with eq. 65): L_i = -K_i^+ N-hat X;  eq. 52: B_i = L_i + Theta (N_i - L_i)
-        R q[4], y[4];
+        R q[4], Lw[3][4];
         to_symmetrising(gamma - R(1), kk, X, q);
-        y[0] = -(kk.n00 * q[0] + kk.n01 * q[1] + kk.n02 * q[2]);
-        y[1] = -(kk.n01 * q[0] + kk.n11 * q[1] + kk.n12 * q[2]);
-        y[2] = -(kk.n02 * q[0] + kk.n12 * q[1] + kk.n22 * q[2]);
-        y[3] = -(kk.ns * q[3]);
+        lda_from_symmetrised(kk, g, X, q, Lw);
+        if (lump) {  // the same anti-diffusive term on the LDA residual (L567)
+          const Vec4<R> *sD = reinterpret_cast<const Vec4<R> *>(buf + L.oD);
+          Vec4<R> d0 = sD[l[0]], d1 = sD[l[1]], d2 = sD[l[2]];
+          R sm[4] = {d0.x + d1.x + d2.x, d0.y + d1.y + d2.y, d0.z + d1.z + d2.z, d0.w + d1.w + d2.w};
 #pragma unroll
-        for (int i = 0; i < 3; ++i) {
-          R z[4], Lw[4];
-          apply_split<false>(kk.ap[i], kk.bp[i], kk.l3p[i], g.nx[i], g.ny[i], y, z);
-          to_conserved(kk, z, Lw);
-          if (STAGE == 2 && lump) {  // the same anti-diffusive term on the LDA residual (L567)
-            const Vec4<R> *sD = reinterpret_cast<const Vec4<R> *>(buf + L.oD);
-            Vec4<R> d0 = sD[l[0]], d1 = sD[l[1]], d2 = sD[l[2]], d = sD[l[i]];
-            Lw[0] += (R(0.25) * a3) * (R(3) * d.x - (d0.x + d1.x + d2.x));
-            Lw[1] += (R(0.25) * a3) * (R(3) * d.y - (d0.y + d1.y + d2.y));
-            Lw[2] += (R(0.25) * a3) * (R(3) * d.z - (d0.z + d1.z + d2.z));
-            Lw[3] += (R(0.25) * a3) * (R(3) * d.w - (d0.w + d1.w + d2.w));
-          }
+          for (int i = 0; i < 3; ++i) {
+            Vec4<R> d = sD[l[i]];
+            R dv[4] = {d.x, d.y, d.z, d.w};
 #pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            R *r = res + (i * 4 + c) * T + tid;
-            *r = (SCHEME == MRD_SCHEME_B || SCHEME == MRD_SCHEME_BX) ? Lw[c] + th[c] * (*r - Lw[c]) : Lw[c];
+            for (int c = 0; c < 4; ++c) Lw[i][c] += (R(0.25) * a3) * (R(3) * dv[c] - sm[c]);
           }
         }
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            Cell<R> *r = cell + h * HOFF + i * T + tid;
+            if (SCHEME == MRD_SCHEME_B || SCHEME == MRD_SCHEME_BX) {
+              const Cell<R> n = *r;
+              *r = Cell<R>{Lw[i][2 * h] + th[2 * h] * (n.a - Lw[i][2 * h]), Lw[i][2 * h + 1] + th[2 * h + 1] * (n.b - Lw[i][2 * h + 1])};
+            } else {
+              *r = Cell<R>{Lw[i][2 * h], Lw[i][2 * h + 1]};
+            }
+          }
       }
-      if (STAGE == 1 && phi_dbg && valid) {
+      if (STAGE == 1 && io.phi_dbg && valid) {
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
-          const R *r = res + (i * 4) * T + tid;
-          st4(&phi_dbg[3 * t + i], Vec4<R>{r[0], r[T], r[2 * T], r[3 * T]});
+          const Cell<R> c0 = cell[i * T + tid], c1 = cell[HOFF + i * T + tid];
+          st4(&io.phi_dbg[3 * t + i], Vec4<R>{c0.a, c0.b, c1.a, c1.b});
         }
-        sT_dbg[t] = st;
+        io.sT_dbg[t] = st;
       }
     }
     if (!valid) {  // padding thread of the last tile: contributes nothing
 #pragma unroll
-      for (int i = 0; i < 12; ++i) res[i * T + tid] = R(0);
+      for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int h = 0; h < 2; ++h) cell[h * HOFF + i * T + tid] = Cell<R>{R(0), R(0)};
       st = R(0);
     }
-    if (STAGE == 1) sSTc[tid] = st;
+    if (STAGE == 1) {
+      sTx[tid] = st;
+      sTx[T + tid] = st;
+      sTx[2 * T + tid] = st;
+    }
     __syncthreads();
-    tile_epilogue<R, STAGE == 1>(T, res, sSTc, plan + 4 * T, plan + 7 * T, s0, ns, part, partS);
+    // ---- epilogue: per slot the ascending sum of its tile-local incidences; one partial per slot leaves the SM
+    {
+      const uint16_t *boff = plan + 4 * T, *ent = plan + 4 * T + td.offn;
+      for (int j = tid; j < ns; j += T) {   // (padding slots have no incidences: their partial is zero and nobody reads it)
+        R a[4], S;
+        slot_sum<R, T, STAGE == 1>(cell, sTx, ent, boff[j], boff[j + 1], a, S);
+        st4(&io.part[s0 + j], Vec4<R>{a[0], a[1], a[2], a[3]});
+        if (STAGE == 1) io.partS[s0 + j] = S;
+      }
+    }
     // No second block barrier: a warp that is done goes on to the next tile (the other buffer, the other residual
     // area) while slower warps finish this epilogue; the LAST warp to leave refills buffer `cur` with tile k+2.
     // (Nobody runs more than one tile ahead: the barrier above needs every warp.)
@@ -375,8 +426,8 @@ tile_kernel(TileDev<R> td, const TileSmem<R, STAGE, GTAB> L, R gamma, const Ctl 
         const int64_t b2 = nb + gridDim.x;
         if (b2 < td.ntile) {
           fence_proxy_async();  // buffer `cur` was read through the generic proxy
-          tile_stage_in<R, STAGE, GTAB>(td, L, buf, &bar[cur], b2, __ldg(td.tile_info + b2), __ldg(td.tile_info + b2 + 1), slotZ, slotS,
-                                        slotD, phi16);
+          tile_stage_in<R, STAGE, GTAB>(td, L, buf, &bar[cur], b2, __ldg(td.tile_info + b2), __ldg(td.tile_info + b2 + 1), io.slotZ, io.slotS,
+                                        io.slotD, io.phi12);
         }
       }
     }

@@ -7,7 +7,9 @@ phases; between the phases this module moves bytes and nothing else:
   * after RESIDUAL1: all-reduce(min) of two doubles (eq. 44: the global minimum of 2 V_i / sum s_T; the
     non-physical flag rides along),
   * after UPDATE1 and after STAGE2: neighbour exchange of the conserved state of the vertices on the cut
-    (`mrd_halo_pack` -> send/recv -> `mrd_halo_unpack`).
+    (`mrd_halo_pack` -> send/recv -> `mrd_halo_unpack`),
+  * before END: all-reduce(max) of one double, the non-physical flag of the whole step, so that every rank commits
+    or discards the same step (and `step` returns the same (steps, t) or raises the same error everywhere).
 
 With the `nccl` backend the packed buffers go device to device over NVLink; with `gloo` (tests on a box with
 one GPU, or none for the host logic) they are staged through host memory.  No arithmetic of the method lives
@@ -84,6 +86,7 @@ class DistributedMesh:
         self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
         period = params.get("period", (0.0, 0.0))
         P = self.part = Partition(xy, tri, self.world, self.rank, vertex_flag=vertex_flag, wall_edge=wall_edge, period=period)
+        params = dict(params, domain_size=P.domain_size)     # Bx: L of eq. 56 is the WHOLE mesh's, not the part's
         self.mesh = Mesh(P.xy, P.tri, vertex_flag=P.vertex_flag, wall_edge=P.wall_edge if P.n_wall else None, **params)
         self.mesh.halo_set(P.send_idx, P.recv_idx)
         self.nv, self.dtype, self.np_dtype = P.n_global, self.mesh.dtype, self.mesh.np_dtype
@@ -95,6 +98,7 @@ class DistributedMesh:
         self._rk2 = self.mesh.params.time_order == 2
         self._bx = self.mesh.params.scheme == 5   # Bx: the speed range of eq. 56 is reduced over all parts
         self._r = torch.empty(2, dtype=torch.float64, device="cuda")
+        self._f = torch.empty(1, dtype=torch.float64, device="cuda")
         self._open = False
 
     def close(self):
@@ -161,6 +165,9 @@ class DistributedMesh:
                 self._range(2)
             m.phase(m.PHASE_STAGE2)
             self._exchange()
+        m.status_get(self._f)                 # a rank that met rho <= 0, p <= 0 or c^2 <= 0 anywhere in this step ...
+        self.comm.allreduce_max(self._f)
+        m.status_set(self._f)                 # ... makes every rank discard it
         m.phase(m.PHASE_END)
         if self._bx:
             self._range(1)

@@ -33,7 +33,19 @@ def cases():
     out["vortex_bx_n1"] = (m, wl.vortex_state(m, advect=(0.3, 0.1)), None, None, dict(scheme=5, time_order=1), 6, 0.0)
     r = wl.make_config("riemann4", n=40)
     out["riemann4_frozen"] = (r.mesh, r.W0, r.vertex_flag, None, dict(scheme=2, time_order=2), 6, 0.0)
+    # Bx on a BOUNDED domain: L of eq. 56 must be the whole tube's length on every part, not the part's bounding box
+    out["sod_bx_walls"] = (c.mesh, c.W0, c.vertex_flag, c.wall_edge, dict(scheme=5, time_order=2), 8, 0.0)
     return out
+
+
+def nonphysical_case():
+    """A state that stays physical for one step and turns non-physical in STAGE 2 of the second one, at an interior vertex
+    of the first Morton range only (a Mach-3 momentum spike at one vertex of a gas at rest): (mesh, W0, steps asked for)."""
+    m = wl.uniform_mesh(32, 32, 1.0, 1.0, periodic=True)
+    rho, u, v, p = np.ones(m.nv), np.zeros(m.nv), np.zeros(m.nv), np.ones(m.nv)
+    i0 = 5 * 32 + 6
+    u[i0], p[i0] = 4.0, 0.2
+    return m, wl.primitive_to_conserved(rho, u, v, p), 5
 
 
 def main():
@@ -60,6 +72,24 @@ def main():
         res[name + "/scalars"] = np.array([n1, t1, dt1, n, t, dt, mr, mp, dm.part.n_owned, dm.part.n_recv, dm.launch_count()], dtype=np.float64)
         res[name + "/totals"] = tot
         dm.close()
+    # a step that fails on ONE part must be discarded by ALL of them: same (error, steps, t) everywhere, state still usable
+    from paper_1705_02028_b200 import MrdError
+    mesh, W0, steps = nonphysical_case()
+    dm = DistributedMesh(mesh.xy, mesh.tri, period=mesh.period, scheme=2, time_order=2)
+    dm.set_state(W0)
+    code = 0
+    try:
+        dm.step(steps)
+    except MrdError as e:
+        code = e.code
+    n_tot, t_tot, _ = dm.mesh.sync()
+    mine = [float(code), float(n_tot), float(t_tot)]
+    everyone = [None] * dist.get_world_size()
+    dist.all_gather_object(everyone, mine)
+    res["nonphysical/ranks"] = np.array(everyone, dtype=np.float64)
+    res["nonphysical/W"] = dm.get_state()                       # collective: hangs if the ranks disagree about the step
+    n_more = dm.step(1) if code == 0 else None                  # (not reached in the failing case)
+    dm.close()
     dist.barrier()
     if rank == 0:
         np.savez(args.out, **res)

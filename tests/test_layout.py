@@ -22,8 +22,8 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_params_struct_matches_header_size():
-    # 2 doubles + 4 int32 + 2 doubles + 2 int32
-    assert C.sizeof(mrd.Params) == 16 + 16 + 16 + 8
+    # 2 doubles + 4 int32 + 2 doubles + 2 int32 + 1 double (domain_size)
+    assert C.sizeof(mrd.Params) == 16 + 16 + 16 + 8 + 8
 
 
 MESHES = {

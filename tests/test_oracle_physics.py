@@ -1,59 +1,15 @@
 """Physics-level pins for the oracle: Sod shock tube against the exact Riemann solution (PAPER.md
 §5.1.2) and second-order convergence on the stationary isentropic vortex (§5.2.1).
-The exact Riemann solver below is the textbook construction (two-shock/rarefaction pressure
+The exact Riemann solver (tests/helpers.py) is the textbook construction (two-shock/rarefaction pressure
 function, Newton iteration), independent of the oracle."""
 import numpy as np
 import pytest
 
 import oracle
 import workloads as wl
+from helpers import exact_riemann
 
 GAMMA = 1.4
-
-
-def exact_riemann(rl, ul, pl, rr, ur, pr, xi, g=GAMMA):
-    """Exact solution of the 1D Riemann problem sampled at xi = (x - x0)/t."""
-    cl, cr = np.sqrt(g * pl / rl), np.sqrt(g * pr / rr)
-
-    def f(p, r, pk, c):
-        if p > pk:   # shock
-            A, B = 2 / ((g + 1) * r), (g - 1) / (g + 1) * pk
-            return (p - pk) * np.sqrt(A / (p + B)), np.sqrt(A / (p + B)) * (1 - 0.5 * (p - pk) / (p + B))
-        return 2 * c / (g - 1) * ((p / pk) ** ((g - 1) / (2 * g)) - 1), 1 / (r * c) * (p / pk) ** (-(g + 1) / (2 * g))
-
-    p = 0.5 * (pl + pr)
-    for _ in range(100):
-        fl, dfl = f(p, rl, pl, cl)
-        fr, dfr = f(p, rr, pr, cr)
-        dp = (fl + fr + ur - ul) / (dfl + dfr)
-        p = max(p - dp, 1e-12)
-        if abs(dp) < 1e-15 * p:
-            break
-    us = 0.5 * (ul + ur) + 0.5 * (f(p, rr, pr, cr)[0] - f(p, rl, pl, cl)[0])
-    rho = np.empty_like(xi)
-    # left of the contact
-    if p > pl:
-        rsl = rl * ((p / pl + (g - 1) / (g + 1)) / ((g - 1) / (g + 1) * p / pl + 1))
-        sl = ul - cl * np.sqrt((g + 1) / (2 * g) * p / pl + (g - 1) / (2 * g))
-        left = np.where(xi < sl, rl, rsl)
-    else:
-        rsl = rl * (p / pl) ** (1 / g)
-        csl = cl * (p / pl) ** ((g - 1) / (2 * g))
-        head, tail = ul - cl, us - csl
-        fan = rl * (2 / (g + 1) + (g - 1) / ((g + 1) * cl) * (ul - xi)) ** (2 / (g - 1))
-        left = np.where(xi < head, rl, np.where(xi < tail, fan, rsl))
-    if p > pr:
-        rsr = rr * ((p / pr + (g - 1) / (g + 1)) / ((g - 1) / (g + 1) * p / pr + 1))
-        sr = ur + cr * np.sqrt((g + 1) / (2 * g) * p / pr + (g - 1) / (2 * g))
-        right = np.where(xi > sr, rr, rsr)
-    else:
-        rsr = rr * (p / pr) ** (1 / g)
-        csr = cr * (p / pr) ** ((g - 1) / (2 * g))
-        head, tail = ur + cr, us + csr
-        fan = rr * (2 / (g + 1) - (g - 1) / ((g + 1) * cr) * (ur - xi)) ** (2 / (g - 1))
-        right = np.where(xi > head, rr, np.where(xi > tail, fan, rsr))
-    rho = np.where(xi < us, left, right)
-    return rho, p, us
 
 
 def test_exact_solver_reproduces_the_standard_sod_star_state():
