@@ -133,6 +133,13 @@ def build_workload(n: int, numbering: str, kind: str = "uniform"):
     """config 5; kind 'jitter' moves every vertex by up to 0.2 cell widths (no two triangles alike), 'flip' also flips a seeded
     third of the edges (valence 4...10): the second, genuinely unstructured workload of SURVEY 8f-2."""
     import workloads as wl
+    if kind == "delaunay":
+        # the paper's unstructured mesh shape (L685: 1.3 M vertices): seeded Delaunay triangulation, graded 100:1, frozen ring
+        cfg = wl.make_config("sweep", n=32, numbering="natural")
+        cfg.mesh = wl.delaunay_mesh(n * n, seed=1)
+        cfg.vertex_flag = cfg.mesh.boundary
+        cfg.W0 = wl.vortex_state(cfg.mesh)
+        return cfg
     cfg = wl.make_config("sweep", n=n, numbering=numbering)
     if kind in ("jitter", "flip"):
         cfg.mesh = wl.jitter_mesh(cfg.mesh, 0.2, seed=7)
@@ -141,6 +148,28 @@ def build_workload(n: int, numbering: str, kind: str = "uniform"):
     if kind != "uniform":
         cfg.W0 = wl.vortex_state(cfg.mesh)     # the same vortex, sampled at the moved vertices
     return cfg
+
+
+def setup_part(n: int, world: int, rank: int):
+    """Host-side set-up of ONE rank of the N-GPU run, from local pieces only (needs no GPU): the part of the periodic strip of
+    `world` vortex squares (workloads.uniform_strip_part -> mrd_partition_create_local) and its initial state.
+    Returns (Partition, W_local [4][n_local] in the part's vertex order, stats)."""
+    import resource
+    from types import SimpleNamespace
+    import workloads as wl
+    import paper_1705_02028_b200 as mrd
+    t0 = time.perf_counter()
+    pc = wl.uniform_strip_part(n, world, rank)
+    part = mrd.Partition.from_local(pc["n_vertex_global"], pc["vertex_global"], pc["owner"], pc["xy"], pc["tri"], pc["tri_global"],
+                                    world, rank, period=pc["period"], domain_size=pc["domain_size"])
+    L = pc["period"][0]
+    # the vortex of every square: the state at (x, y mod L) of the single-square workload
+    sq = SimpleNamespace(xy=np.stack([part.xy[:, 0], np.mod(part.xy[:, 1], L)], axis=1), lengths=(L, L), period=(L, L),
+                         nv=part.n_local)
+    W_local = wl.vortex_state(sq)
+    stats = dict(n_vertex_global=pc["n_vertex_global"], n_triangle_global=pc["n_triangle_global"],
+                 setup_s=time.perf_counter() - t0, host_rss_gb=resource.getrusage(resource.RUSAGE_SELF).ru_maxrss / 1e6)
+    return part, W_local, stats
 
 
 # ------------------------------------------------------------------------------------------------------
@@ -222,34 +251,32 @@ def run_mrd(args):
     params = dict(gamma=1.4, cfl=0.5, scheme=mrd.SCHEME_B, time_order=2, precision=mrd.FP64 if prec == "fp64" else mrd.FP32,
                   reorder=bool(args.reorder), tile=args.tile)
     t0 = time.perf_counter()
+    setup = None
     if not halo:
         # one GPU, or N independent replicas of the single-GPU workload
         cfg = build_workload(args.n, args.numbering, args.mesh)
         mesh = cfg.mesh
         nt, nv = mesh.nt, mesh.nv                 # units per rank
         nt_job, nv_job = world * nt, world * nv
-        gm = sim = mrd.Mesh(mesh.xy, mesh.tri, period=mesh.period, **params)
+        gm = sim = mrd.Mesh(mesh.xy, mesh.tri, vertex_flag=cfg.vertex_flag, period=mesh.period, **params)
         layout_s = time.perf_counter() - t0
         gm.set_state(torch.tensor(cfg.W0, dtype=tdtype, device="cuda"))
         parallelism = "1 GPU" if world == 1 else f"{world} independent replicas"
     else:
         # ONE mesh over N GPUs (weak scaling): a periodic strip of N copies of the single-GPU workload stacked in y, cut into
-        # N Morton ranges (= the N squares); one halo exchange per stage and one min-reduction per step over NCCL
-        import workloads as wl
+        # its N squares; one halo exchange per stage and two scalar reductions per step over NCCL.  Every rank builds ITS part
+        # only (setup_part): no array of the whole mesh exists anywhere, so start-up time and host memory do not grow with N.
         from paper_1705_02028_b200.distributed import DistributedMesh
-        n = args.n
-        cell = build_workload(n, "natural")
-        mesh = wl.uniform_mesh(n, n * world, 10.0, 10.0 * world, periodic=True)
-        W0 = np.ascontiguousarray(np.tile(cell.W0.reshape(4, n, n), (1, world, 1)).reshape(4, -1))
-        sim = DistributedMesh(mesh.xy, mesh.tri, period=mesh.period, **params)
+        part, W_local, setup = setup_part(args.n, world, rank)
+        sim = DistributedMesh(None, None, part=part, period=part.period, **params)
         gm = sim.mesh                             # this rank's part (owned + halo vertices, cut triangles on both sides)
-        nt_job, nv_job = mesh.nt, mesh.nv         # unique triangles / vertices of the whole mesh
+        nt_job, nv_job = setup["n_triangle_global"], setup["n_vertex_global"]   # unique triangles / vertices of the whole mesh
         nt, nv = gm.nt, gm.nv                     # this rank's share (kernel-level numbers)
         layout_s = time.perf_counter() - t0
-        sim.set_state(W0)
-        parallelism = (f"one mesh over {world} GPUs: Morton-range domain decomposition, {sim.part.n_send} halo vertices sent per "
-                       f"rank per stage to {sim.part.n_neighbour} neighbours, 1 all-reduce(min) per step")
-        del W0, cell
+        sim.set_state_local(W_local)
+        parallelism = (f"one mesh over {world} GPUs: row-band domain decomposition built locally per rank, {sim.part.n_send} halo vertices "
+                       f"sent per rank per stage to {sim.part.n_neighbour} neighbours, 2 scalar all-reduces per step")
+        del W_local
     stream = torch.cuda.current_stream()
 
     # ---- device-resident throughput: W warm-up steps, then exactly K timed steps -------------------------
@@ -369,7 +396,9 @@ def run_mrd(args):
                        "l2": "inputs larger than L2 (state %.0f MB, per-triangle arrays %.1f GB)" % (
                            state_bytes / 1e6, gm.device_bytes() / 1e9),
                        "parallelism": parallelism,
-                       "layout_s": layout_s, "device_gb": gm.device_bytes() / 1e9, "t_sim": t_sim},
+                       "layout_s": layout_s, "device_gb": gm.device_bytes() / 1e9, "t_sim": t_sim,
+                       "host_rss_gb": __import__("resource").getrusage(__import__("resource").RUSAGE_SELF).ru_maxrss / 1e6,
+                       "part_setup_s": None if setup is None else setup["setup_s"]},
             "vertex_updates_per_s": nv_job * args.steps / (ms_total * 1e-3),
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
@@ -392,8 +421,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--traffic", type=float, default=None, help="dram bytes per launch of the dominant kernel (ncu)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--mesh", default="uniform", choices=["uniform", "jitter", "flip"],
-                    help="uniform triangulation (config 5), jittered vertices, or jittered + flipped edges (variable valence)")
+    ap.add_argument("--mesh", default="uniform", choices=["uniform", "jitter", "flip", "delaunay"],
+                    help="uniform triangulation (config 5), jittered vertices, jittered + flipped edges (variable valence), or a seeded "
+                         "graded Delaunay triangulation of --size^2 points with a frozen boundary ring (--size 1140: the paper's 1.3 M vertices)")
     ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
                     help="N > 1: torch.distributed backend (gloo stages the halo rows through host memory; functional tests only)")
     ap.add_argument("--decomposition", default="halo", choices=["halo", "replicas"],

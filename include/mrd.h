@@ -196,12 +196,35 @@ int mrd_step_profile(mrd_mesh *m, void *stream, float ms[MRD_PROFILE_SLOTS]);
  *   "send_off"      int32[n4+1], "send_idx" int32[n5]: owned local vertices whose state neighbour k needs,
  *   "recv_off"      int32[n4+1], "recv_idx" int32[n6]: halo local vertices owned by neighbour k; both lists
  *                   ascending in global id per neighbour, so that send list of a for b == recv list of b from a
- *   "owner"         int32[n7]    owning part of every global vertex
+ *   "owner"         int32[n7]    owning part of every global vertex (empty, 0 bytes, for mrd_partition_create_local)
  * ---------------------------------------------------------------------------------------------- */
 typedef struct mrd_partition mrd_partition;
 int mrd_partition_create(mrd_partition **out, int64_t n_vertex, const double *xy, int64_t n_triangle,
                          const int32_t *tri, const uint8_t *vertex_flag, int64_t n_wall_edge,
                          const int32_t *wall_edge, double period_x, double period_y, int32_t n_part, int32_t part);
+/* As mrd_partition_create with the owning part of every vertex given by the caller (owner: host int32[n_vertex], values in
+ * [0, n_part)) instead of the Morton ranges: any decomposition into connected pieces works the same way. */
+int mrd_partition_create_owned(mrd_partition **out, int64_t n_vertex, const double *xy, int64_t n_triangle,
+                               const int32_t *tri, const uint8_t *vertex_flag, int64_t n_wall_edge,
+                               const int32_t *wall_edge, double period_x, double period_y, int32_t n_part, int32_t part,
+                               const int32_t *owner);
+/* The same part assembled from LOCAL pieces, for meshes whose arrays should never exist in full on one host (the start-up of an
+ * N-GPU run then costs each rank its own share only).  The caller passes the vertices and triangles it knows -- at least every
+ * triangle incident to a vertex owned by `part`, with all three vertices of each -- and for each vertex its global id and
+ * owning part (all host arrays, copied):
+ *   vertex_global int32[n_local_vertex]   global vertex ids (unique, any order), < n_vertex_global
+ *   owner         int32[n_local_vertex]   owning part of each of these vertices
+ *   xy            double[n_local_vertex][2];  vertex_flag uint8[n_local_vertex] or NULL (0 free, 1 frozen)
+ *   tri           int32[n_local_triangle][3]  indices INTO the arrays above;  tri_global int32[n_local_triangle] global triangle ids
+ *   wall_edge     int32[n_wall_edge][2] or NULL, indices into the arrays above
+ *   domain_size   L of eq. 56 of the whole mesh (reading C25; only MRD_SCHEME_BX uses it)
+ * Triangles without a vertex of `part` and vertices used by no kept triangle are dropped.  The result is what
+ * mrd_partition_create_owned gives for the whole mesh with the same owners (same local numbering, same exchange lists:
+ * they are sorted by global id), except that "owner" (a whole-mesh array) is empty.  Errors as mrd_partition_create. */
+int mrd_partition_create_local(mrd_partition **out, int64_t n_vertex_global, double domain_size, int64_t n_local_vertex,
+                               const int32_t *vertex_global, const int32_t *owner, const double *xy, const uint8_t *vertex_flag,
+                               int64_t n_local_triangle, const int32_t *tri, const int32_t *tri_global, int64_t n_wall_edge,
+                               const int32_t *wall_edge, int32_t n_part, int32_t part);
 void mrd_partition_destroy(mrd_partition *p);
 int mrd_partition_sizes(const mrd_partition *p, int64_t n[8]);
 /* L of eq. 56 (reading C25) of the WHOLE mesh the partition was made from (host out): goes into the

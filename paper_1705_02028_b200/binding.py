@@ -63,6 +63,10 @@ def lib():
         L.mrd_step_profile.argtypes = [vp, vp, C.POINTER(C.c_float)]
         L.mrd_partition_create.argtypes = [C.POINTER(vp), C.c_int64, _dp, C.c_int64, _ip, _bp, C.c_int64, _ip, C.c_double,
                                            C.c_double, C.c_int32, C.c_int32]
+        L.mrd_partition_create_owned.argtypes = [C.POINTER(vp), C.c_int64, _dp, C.c_int64, _ip, _bp, C.c_int64, _ip, C.c_double,
+                                                 C.c_double, C.c_int32, C.c_int32, _ip]
+        L.mrd_partition_create_local.argtypes = [C.POINTER(vp), C.c_int64, C.c_double, C.c_int64, _ip, _ip, _dp, _bp, C.c_int64, _ip,
+                                                 _ip, C.c_int64, _ip, C.c_int32, C.c_int32]
         L.mrd_partition_destroy.argtypes = [vp]
         L.mrd_partition_destroy.restype = None
         L.mrd_partition_sizes.argtypes = [vp, _lp]
@@ -174,10 +178,43 @@ class Partition:
                ("send_idx", np.int32, lambda n: (n[5],)), ("recv_off", np.int32, lambda n: (n[4] + 1,)),
                ("recv_idx", np.int32, lambda n: (n[6],)), ("owner", np.int32, lambda n: (n[7],)))
 
-    def __init__(self, xy, tri, n_part, part, vertex_flag=None, wall_edge=None, period=(0.0, 0.0)):
+    def __init__(self, xy, tri, n_part, part, vertex_flag=None, wall_edge=None, period=(0.0, 0.0), owner=None):
+        """Part `part` of `n_part` of the WHOLE mesh (xy, tri, ...): owners = contiguous ranges of the vertices' Morton order,
+        or the `owner` array (int32 [nv]) when given."""
         keep, args = _mesh_args(xy, tri, vertex_flag, wall_edge)
         h = C.c_void_p()
-        _check(lib().mrd_partition_create(C.byref(h), *args, float(period[0]), float(period[1]), int(n_part), int(part)))
+        if owner is None:
+            _check(lib().mrd_partition_create(C.byref(h), *args, float(period[0]), float(period[1]), int(n_part), int(part)))
+        else:
+            own = np.ascontiguousarray(owner, dtype=np.int32)
+            assert own.shape == (args[0],)
+            _check(lib().mrd_partition_create_owned(C.byref(h), *args, float(period[0]), float(period[1]), int(n_part), int(part),
+                                                    _np_ptr(own, C.c_int32)))
+        self._load(h, n_part, part, period, has_owner=True)
+
+    @classmethod
+    def from_local(cls, n_vertex_global, vertex_global, owner, xy, tri, tri_global, n_part, part, vertex_flag=None, wall_edge=None,
+                   period=(0.0, 0.0), domain_size=0.0):
+        """mrd_partition_create_local: the part assembled from local pieces (no whole-mesh array); `tri` / `wall_edge` index the
+        local arrays.  `self.owner` is None."""
+        vg = np.ascontiguousarray(vertex_global, dtype=np.int32)
+        own = np.ascontiguousarray(owner, dtype=np.int32)
+        xy = np.ascontiguousarray(xy, dtype=np.float64)
+        tri = np.ascontiguousarray(tri, dtype=np.int32)
+        tg = np.ascontiguousarray(tri_global, dtype=np.int32)
+        flag = None if vertex_flag is None else np.ascontiguousarray(vertex_flag, dtype=np.uint8)
+        wedge = None if wall_edge is None else np.ascontiguousarray(wall_edge, dtype=np.int32)
+        assert vg.shape == own.shape == (xy.shape[0],) and tri.shape == (tg.shape[0], 3)
+        self = cls.__new__(cls)
+        h = C.c_void_p()
+        _check(lib().mrd_partition_create_local(C.byref(h), int(n_vertex_global), float(domain_size), xy.shape[0], _np_ptr(vg, C.c_int32),
+                                                _np_ptr(own, C.c_int32), _np_ptr(xy, C.c_double), _np_ptr(flag, C.c_uint8),
+                                                tri.shape[0], _np_ptr(tri, C.c_int32), _np_ptr(tg, C.c_int32),
+                                                0 if wedge is None else wedge.shape[0], _np_ptr(wedge, C.c_int32), int(n_part), int(part)))
+        self._load(h, n_part, part, period, has_owner=False)
+        return self
+
+    def _load(self, h, n_part, part, period, has_owner):
         try:
             n = (C.c_int64 * 8)()
             _check(lib().mrd_partition_sizes(h, n))
@@ -188,6 +225,9 @@ class Partition:
             _check(lib().mrd_partition_domain_size(h, C.byref(ds)))
             self.domain_size = ds.value
             for name, dt, shape in self._ARRAYS:
+                if name == "owner" and not has_owner:
+                    self.owner = None
+                    continue
                 a = np.empty(shape(n), dtype=dt)
                 _check(lib().mrd_partition_get(h, name.encode(), C.c_void_p(a.ctypes.data), a.nbytes))
                 setattr(self, name, a)

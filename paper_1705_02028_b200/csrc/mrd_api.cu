@@ -1112,7 +1112,45 @@ int mrd_partition_create(mrd_partition **out, int64_t nv, const double *xy, int6
   std::string err;
   int rc;
   try {
-    rc = mrd_host::partition_build(*P, nv, xy, nt, tri, vertex_flag, ne, wall_edge, period_x, period_y, n_part, part, err);
+    rc = mrd_host::partition_build(*P, nv, xy, nt, tri, vertex_flag, ne, wall_edge, period_x, period_y, n_part, part, nullptr, err);
+  } catch (const std::bad_alloc &) {
+    rc = MRD_ENOMEM;
+    err = "out of host memory in the partitioner";
+  }
+  if (rc) { delete P; return fail(rc, err); }
+  *out = P;
+  return MRD_OK;
+}
+int mrd_partition_create_owned(mrd_partition **out, int64_t nv, const double *xy, int64_t nt, const int32_t *tri,
+                               const uint8_t *vertex_flag, int64_t ne, const int32_t *wall_edge, double period_x, double period_y,
+                               int32_t n_part, int32_t part, const int32_t *owner) {
+  if (!out || !owner) return fail(MRD_EINVAL, "null argument");
+  mrd_partition *P = new (std::nothrow) mrd_partition();
+  if (!P) return fail(MRD_ENOMEM, "out of memory");
+  std::string err;
+  int rc;
+  try {
+    rc = mrd_host::partition_build(*P, nv, xy, nt, tri, vertex_flag, ne, wall_edge, period_x, period_y, n_part, part, owner, err);
+  } catch (const std::bad_alloc &) {
+    rc = MRD_ENOMEM;
+    err = "out of host memory in the partitioner";
+  }
+  if (rc) { delete P; return fail(rc, err); }
+  *out = P;
+  return MRD_OK;
+}
+int mrd_partition_create_local(mrd_partition **out, int64_t nv_global, double domain_size, int64_t n_local_vertex,
+                               const int32_t *vertex_global, const int32_t *owner, const double *xy, const uint8_t *vertex_flag,
+                               int64_t n_local_triangle, const int32_t *tri, const int32_t *tri_global, int64_t n_wall_edge,
+                               const int32_t *wall_edge, int32_t n_part, int32_t part) {
+  if (!out) return fail(MRD_EINVAL, "null output pointer");
+  mrd_partition *P = new (std::nothrow) mrd_partition();
+  if (!P) return fail(MRD_ENOMEM, "out of memory");
+  std::string err;
+  int rc;
+  try {
+    rc = mrd_host::partition_build_local(*P, nv_global, domain_size, n_local_vertex, vertex_global, owner, xy, vertex_flag,
+                                         n_local_triangle, tri, tri_global, n_wall_edge, wall_edge, n_part, part, err);
   } catch (const std::bad_alloc &) {
     rc = MRD_ENOMEM;
     err = "out of host memory in the partitioner";

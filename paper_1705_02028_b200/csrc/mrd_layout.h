@@ -75,7 +75,11 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
 void morton_order_vertices(int64_t nv, const double *xy, const double period[2], std::vector<int32_t> &perm);
 int partition_build(mrd_partition &P, int64_t nv, const double *xy, int64_t nt, const int32_t *tri,
                     const uint8_t *vertex_flag, int64_t ne, const int32_t *wall_edge, double period_x, double period_y,
-                    int32_t n_part, int32_t part, std::string &err);
+                    int32_t n_part, int32_t part, const int32_t *owner /* [nv] or null: Morton ranges */, std::string &err);
+int partition_build_local(mrd_partition &P, int64_t nv_global, double domain_size, int64_t nlv, const int32_t *vertex_global,
+                          const int32_t *owner, const double *xy, const uint8_t *vertex_flag, int64_t nlt, const int32_t *tri,
+                          const int32_t *tri_global, int64_t ne, const int32_t *wall_edge, int32_t n_part, int32_t part,
+                          std::string &err);
 int partition_sizes(const mrd_partition &P, int64_t n[8]);
 int partition_get(const mrd_partition &P, const char *name, void *dst, int64_t bytes, std::string &err);
 }

@@ -79,13 +79,18 @@ class DistributedMesh:
     Every rank passes the same global arrays (`xy`, `tri`, `vertex_flag`, `wall_edge`) and parameters; the state
     crosses this interface in GLOBAL user numbering.  Call from every rank in the same order."""
 
-    def __init__(self, xy, tri, vertex_flag=None, wall_edge=None, group=None, **params):
+    def __init__(self, xy, tri, vertex_flag=None, wall_edge=None, group=None, part=None, **params):
+        """Either the whole mesh (every rank passes the same global arrays; fine up to a few 10^7 triangles), or `part`, a
+        `Partition` each rank made for itself (`Partition.from_local`: no whole-mesh array anywhere; xy and tri are ignored)."""
         import torch
         import torch.distributed as dist
         self._torch, self._dist, self.group = torch, dist, group
         self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
         period = params.get("period", (0.0, 0.0))
-        P = self.part = Partition(xy, tri, self.world, self.rank, vertex_flag=vertex_flag, wall_edge=wall_edge, period=period)
+        if part is None:
+            part = Partition(xy, tri, self.world, self.rank, vertex_flag=vertex_flag, wall_edge=wall_edge, period=period)
+        assert part.n_part == self.world and part.part == self.rank
+        P = self.part = part
         params = dict(params, domain_size=P.domain_size)     # Bx: L of eq. 56 is the WHOLE mesh's, not the part's
         self.mesh = Mesh(P.xy, P.tri, vertex_flag=P.vertex_flag, wall_edge=P.wall_edge if P.n_wall else None, **params)
         self.mesh.halo_set(P.send_idx, P.recv_idx)
@@ -120,23 +125,33 @@ class DistributedMesh:
         no = self.part.n_owned
         return self.part.vertex_global[:no], self.mesh.get_state()[:, :no].contiguous()
 
+    def set_state_local(self, W_local):
+        """W_local: [4][n_local] in the part's own vertex order (`part.vertex_global`): nothing global is touched."""
+        t = self._torch
+        loc = t.as_tensor(np.ascontiguousarray(W_local, dtype=self.np_dtype), device="cuda") if not isinstance(W_local, t.Tensor) \
+            else W_local.to("cuda", self.dtype).contiguous()
+        self.mesh.set_state(loc)
+
     def get_state(self):
-        """The whole state [4][nv_global] (host, numpy) on every rank."""
+        """The whole state [4][nv_global] (host, numpy) on every rank (small meshes: tests, output)."""
         t, dist = self._torch, self._dist
-        owner = self.part.owner
-        counts = np.bincount(owner, minlength=self.world)
-        width = int(counts.max())
-        _, W = self.owned_state()
+        ids, W = self.owned_state()
+        counts = [None] * self.world
+        dist.all_gather_object(counts, int(len(ids)), group=self.group)
+        width = max(counts)
         pad = t.zeros((4, width), dtype=self.dtype, device="cuda")
         pad[:, :W.shape[1]] = W
+        pid = t.zeros(width, dtype=t.int32, device="cuda")
+        pid[:len(ids)] = t.as_tensor(ids, device="cuda")
         if self.comm.staged:
-            pad = pad.cpu()
+            pad, pid = pad.cpu(), pid.cpu()
         parts = [t.empty_like(pad) for _ in range(self.world)]
+        pids = [t.empty_like(pid) for _ in range(self.world)]
         dist.all_gather(parts, pad, group=self.group)
+        dist.all_gather(pids, pid, group=self.group)
         out = np.empty((4, self.nv), dtype=self.np_dtype)
         for q in range(self.world):
-            ids = np.nonzero(owner == q)[0]  # ascending, the order of vertex_global[:n_owned] on rank q
-            out[:, ids] = parts[q][:, :len(ids)].cpu().numpy()
+            out[:, pids[q][:counts[q]].cpu().numpy()] = parts[q][:, :counts[q]].cpu().numpy()
         return out
 
     # ---- stepping ----

@@ -5,6 +5,7 @@ import os
 import subprocess
 import sys
 
+import numpy as np
 import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -62,3 +63,24 @@ def test_reference_arm_prints_one_json_line_under_torchrun():
     assert d["impl"] == "reference" and d["metric"] == "triangle_updates_per_s_rk2_step" and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"] and d["higher_is_better"] is True
+
+
+def test_n_gpu_setup_builds_only_the_local_part():
+    """bench.py --gpus N: the host side of one rank's set-up (no GPU needed) touches (n + 2) n vertices whatever N is."""
+    import bench
+    n, world = 256, 8
+    sizes = []
+    for rank in (0, 3, 7):
+        part, W, stats = bench.setup_part(n, world, rank)
+        assert part.n_part == world and part.part == rank and part.n_owned == n * n and part.n_local == (n + 2) * n
+        assert part.n_tri == 2 * (n + 1) * n and part.n_neighbour == 2 and part.n_send == part.n_recv == 2 * n
+        assert sorted(part.neighbour.tolist()) == sorted({(rank - 1) % world, (rank + 1) % world})
+        assert W.shape == (4, part.n_local) and np.isfinite(W).all() and W[0].min() > 0.4
+        assert stats["n_vertex_global"] == n * n * world and stats["n_triangle_global"] == 2 * n * n * world
+        sizes.append(part.n_local)
+        # every square carries the same vortex: the owned block of rank r equals that of rank 0
+        if rank == 0:
+            W_first = W[:, :part.n_owned].copy()
+        else:
+            assert np.abs(W[:, :part.n_owned] - W_first).max() < 1e-12
+    assert len(set(sizes)) == 1

@@ -160,3 +160,40 @@ def test_halo_exchange_gloo_world_size_2():
     for rank, ok, d, nrecv in res:
         assert nrecv > 0 and ok          # every halo row arrived from the right peer at the right offset
         assert d == [3.0, -1.0]          # the minimum over ranks of both doubles (dt bound, non-physical flag)
+
+
+@pytest.mark.parametrize("world", [2, 3, 8])
+def test_part_made_from_local_pieces_equals_the_part_of_the_whole_mesh(world):
+    """N > 1 start-up without any whole-mesh array: `uniform_strip_part` + `Partition.from_local` give exactly what
+    the partitioner gives for the whole strip with the same owners -- local numbering, triangles, flags and exchange lists."""
+    n = 16
+    whole = wl.uniform_mesh(n, n * world, 10.0, 10.0 * world, periodic=True)
+    owner = (np.arange(whole.nv) // n // n).astype(np.int32)               # row bands of n vertex rows
+    for rank in range(world):
+        pc = wl.uniform_strip_part(n, world, rank)
+        assert pc["n_vertex_global"] == whole.nv and len(pc["vertex_global"]) == (n + 2) * n and len(pc["tri"]) == 2 * (n + 1) * n
+        assert np.array_equal(whole.xy[pc["vertex_global"]], pc["xy"])
+        assert np.array_equal(whole.tri[pc["tri_global"]], pc["vertex_global"][pc["tri"]])
+        loc = mrd.Partition.from_local(pc["n_vertex_global"], pc["vertex_global"], pc["owner"], pc["xy"], pc["tri"], pc["tri_global"],
+                                       world, rank, period=pc["period"], domain_size=pc["domain_size"])
+        ref = mrd.Partition(whole.xy, whole.tri, world, rank, period=whole.period, owner=owner)
+        for name in ("vertex_global", "xy", "tri", "tri_global", "vertex_flag", "wall_edge", "neighbour", "send_off", "send_idx",
+                     "recv_off", "recv_idx"):
+            assert np.array_equal(getattr(loc, name), getattr(ref, name)), (name, rank)
+        assert (loc.n_owned, loc.n_send, loc.n_recv, loc.n_global) == (ref.n_owned, ref.n_send, ref.n_recv, ref.n_global)
+        assert loc.owner is None and loc.domain_size == ref.domain_size == 10.0 * world
+
+
+def test_local_part_rejects_bad_input():
+    pc = wl.uniform_strip_part(6, 2, 0)
+    args = (pc["n_vertex_global"], pc["vertex_global"], pc["owner"], pc["xy"], pc["tri"], pc["tri_global"], 2, 0)
+    bad = pc["tri"].copy()
+    bad[0, 0] = 10 ** 6
+    with pytest.raises(mrd.MrdError):
+        mrd.Partition.from_local(args[0], args[1], args[2], args[3], bad, args[5], 2, 0)
+    dup = pc["vertex_global"].copy()
+    dup[1] = dup[0]
+    with pytest.raises(mrd.MrdError):
+        mrd.Partition.from_local(args[0], dup, *args[2:])
+    with pytest.raises(mrd.MrdError):                                      # a part that owns nothing of what it was given
+        mrd.Partition.from_local(args[0], args[1], np.ones_like(pc["owner"]), *args[3:])

@@ -13,6 +13,10 @@ from .meshes import (  # noqa: F401
     morton_order_mesh,
     jitter_mesh,
     flip_edges,
+    delaunay_mesh,
+    uniform_strip_part,
+    read_triangle_files,
+    write_triangle_files,
     boundary_vertices,
     wall_edges_y,
     UniformMesh,

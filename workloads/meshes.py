@@ -215,3 +215,127 @@ def wall_edges_y(mesh: UniformMesh) -> np.ndarray:
     bot = np.stack([rank[0, i0], rank[0, i1]], axis=1)
     top = np.stack([rank[nvy - 1, i0], rank[nvy - 1, i1]], axis=1)
     return np.ascontiguousarray(np.concatenate([bot, top], axis=0).astype(np.int32))
+
+
+def delaunay_mesh(n_points: int = 20000, seed: int = 1, grading: float = 10.0) -> UniformMesh:
+    """A genuinely unstructured, bounded triangulation (stand-in for the paper's Delaunay meshes, which are
+    not in the container): the Delaunay triangulation (scipy.spatial.Delaunay, i.e. Qhull) of seeded random points.
+
+    Points: one uniformly random point in every cell of an m x m stratification of the parameter square (m^2 ~ n_points;
+    valences 3...12, no two triangles alike), plus a ring of points ON the four sides (the boundary vertices, returned as
+    flag 1 by `boundary_vertices`).  The triangulation is made in the parameter square and then carried to physical space
+    by the conformal map w = exp(c (u + i v)), c = ln(grading): angles are kept, lengths grow by e^{c u}, so that the
+    largest triangles have ~grading^2 times the area of the smallest (100:1 by default) -- non-uniform V_i, an annular-
+    sector domain.  `grid_ij`, `shape`, `cells` are None: nothing here is a grid."""
+    rng = np.random.default_rng(seed)
+    m = max(4, int(round(np.sqrt(n_points))))
+    jj, ii = np.meshgrid(np.arange(m), np.arange(m), indexing="ij")
+    u = (ii + rng.random((m, m))) / m
+    v = (jj + rng.random((m, m))) / m
+    # keep the interior points a quarter of a cell away from the sides, so that the ring below IS the boundary
+    pad = 0.25 / m
+    u, v = np.clip(u, pad, 1.0 - pad).ravel(), np.clip(v, pad, 1.0 - pad).ravel()
+    s = (np.arange(m) + 0.5) / m
+    ring = np.concatenate([
+        np.stack([s, np.zeros(m)], axis=1), np.stack([s, np.ones(m)], axis=1),
+        np.stack([np.zeros(m), s], axis=1), np.stack([np.ones(m), s], axis=1),
+        np.array([[0.0, 0.0], [1.0, 0.0], [0.0, 1.0], [1.0, 1.0]])])
+    uv = np.concatenate([np.stack([u, v], axis=1), ring], axis=0)
+    from scipy.spatial import Delaunay
+    tri = Delaunay(uv).simplices.astype(np.int64)
+    # drop the slivers Qhull makes of (nearly) collinear boundary points
+    a, b, c = uv[tri[:, 0]], uv[tri[:, 1]], uv[tri[:, 2]]
+    area = 0.5 * ((b[:, 0] - a[:, 0]) * (c[:, 1] - a[:, 1]) - (b[:, 1] - a[:, 1]) * (c[:, 0] - a[:, 0]))
+    tri = tri[np.abs(area) > 1e-12 / (m * m)]
+    area = area[np.abs(area) > 1e-12 / (m * m)]
+    tri[area < 0] = tri[area < 0][:, [0, 2, 1]]                      # counter-clockwise
+    cgr = np.log(grading)
+    w = np.exp(cgr * (uv[:, 0] + 1j * uv[:, 1]))
+    xy = np.ascontiguousarray(np.stack([w.real, w.imag], axis=1))
+    xy -= xy.min(axis=0)
+    lengths = tuple(float(x) for x in xy.max(axis=0))
+    mesh = UniformMesh(xy, np.ascontiguousarray(tri.astype(np.int32)), (0.0, 0.0), None, None, None, lengths)
+    mesh.boundary = np.zeros(len(xy), dtype=np.uint8)
+    mesh.boundary[len(u):] = 1
+    return mesh
+
+
+def write_triangle_files(mesh: UniformMesh, stem: str, vertex_flag=None) -> None:
+    """Write `stem.node` / `stem.ele` in the ASCII format of the mesh generator Triangle (vertices with one boundary
+    marker, triangles by 1-based vertex number): the ingest format for externally generated meshes."""
+    flag = np.zeros(mesh.nv, dtype=np.int64) if vertex_flag is None else np.asarray(vertex_flag, dtype=np.int64)
+    with open(stem + ".node", "w") as f:
+        f.write(f"{mesh.nv} 2 0 1\n")
+        for k in range(mesh.nv):
+            f.write(f"{k + 1} {float(mesh.xy[k, 0])!r} {float(mesh.xy[k, 1])!r} {flag[k]}\n")
+    with open(stem + ".ele", "w") as f:
+        f.write(f"{mesh.nt} 3 0\n")
+        for k in range(mesh.nt):
+            f.write(f"{k + 1} {mesh.tri[k, 0] + 1} {mesh.tri[k, 1] + 1} {mesh.tri[k, 2] + 1}\n")
+
+
+def read_triangle_files(stem: str):
+    """Read a mesh written by an external generator in Triangle's `.node` / `.ele` format (comments `#`, 0- or 1-based
+    numbering, optional attributes; 3-node triangles).  Returns (mesh, vertex_flag) with the boundary markers as flags
+    (non-zero marker -> 1), ready for `Mesh(mesh.xy, mesh.tri, vertex_flag=...)`."""
+    def rows(path):
+        with open(path) as f:
+            for line in f:
+                line = line.split("#", 1)[0].split()
+                if line:
+                    yield line
+    it = rows(stem + ".node")
+    nv, dim, nattr, nmark = (int(x) for x in next(it))
+    assert dim == 2
+    ids, xy, flag = np.empty(nv, dtype=np.int64), np.empty((nv, 2)), np.zeros(nv, dtype=np.uint8)
+    for k in range(nv):
+        r = next(it)
+        ids[k] = int(r[0])
+        xy[k] = float(r[1]), float(r[2])
+        if nmark:
+            flag[k] = 1 if int(r[3 + nattr]) != 0 else 0
+    base = int(ids.min())
+    assert np.array_equal(ids, np.arange(base, base + nv)), "vertices must be numbered consecutively"
+    it = rows(stem + ".ele")
+    nt, nodes = (int(x) for x in next(it)[:2])
+    assert nodes == 3, "3-node triangles only"
+    tri = np.empty((nt, 3), dtype=np.int32)
+    for k in range(nt):
+        r = next(it)
+        tri[k] = int(r[1]) - base, int(r[2]) - base, int(r[3]) - base
+    xy = np.ascontiguousarray(xy)
+    lo = xy.min(axis=0)
+    lengths = tuple(float(x) for x in (xy.max(axis=0) - lo))
+    mesh = UniformMesh(xy, np.ascontiguousarray(tri), (0.0, 0.0), None, None, None, lengths)
+    mesh.boundary = flag
+    return mesh, flag
+
+
+def uniform_strip_part(n: int, world: int, rank: int, L: float = 10.0):
+    """The pieces of ONE part of the N-GPU bench workload, made without the whole mesh: the periodic strip of `world` squares
+    of n x n cells stacked in y (`uniform_mesh(n, n * world, L, L * world, periodic=True)`, natural numbering), cut into
+    the `world` row bands of n vertex rows.  Returns a dict with what `Partition.from_local` takes: the band's n rows plus the
+    row below and the row above (the vertices of every triangle that touches the band), their global ids and owners, and the
+    n + 1 rows of cells between them -- (n + 2) n vertices and 2 (n + 1) n triangles however large `world` is."""
+    assert world >= 2 and n >= 3
+    nvy = n * world
+    h = L / n
+    j0 = rank * n
+    rows = (np.arange(j0 - 1, j0 + n + 1, dtype=np.int64)) % nvy            # global vertex row of each local row
+    ii = np.arange(n, dtype=np.int64)
+    gid = (rows[:, None] * n + ii[None, :]).ravel()
+    owner = np.repeat(rows // n, n)
+    xy = np.stack([np.tile(ii * h, n + 2), np.repeat(rows * h, n)], axis=1).astype(np.float64)
+    lc, ci = np.meshgrid(np.arange(n + 1, dtype=np.int64), ii, indexing="ij")  # local cell row, column
+    lc, ci = lc.ravel(), ci.ravel()
+    ip = (ci + 1) % n
+    v00, v10, v01, v11 = lc * n + ci, lc * n + ip, (lc + 1) * n + ci, (lc + 1) * n + ip
+    tri = np.empty((2 * (n + 1) * n, 3), dtype=np.int32)
+    tri[0::2] = np.stack([v00, v10, v11], axis=1)
+    tri[1::2] = np.stack([v00, v11, v01], axis=1)
+    cell = rows[lc] * n + ci                                                  # global cell = global row of its lower vertices
+    tri_global = np.empty(2 * (n + 1) * n, dtype=np.int64)
+    tri_global[0::2], tri_global[1::2] = 2 * cell, 2 * cell + 1
+    return dict(n_vertex_global=n * nvy, n_triangle_global=2 * n * nvy, vertex_global=gid.astype(np.int32), owner=owner.astype(np.int32),
+                xy=np.ascontiguousarray(xy), tri=tri, tri_global=tri_global.astype(np.int32), period=(float(L), float(L * world)),
+                domain_size=float(L * world), local_rows=rows % n)
