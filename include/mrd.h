@@ -278,6 +278,31 @@ int mrd_range_get(mrd_mesh *m, int32_t stage, double *d_dev, void *stream);
 int mrd_range_set(mrd_mesh *m, int32_t stage, const double *d_dev, void *stream);
 int mrd_halo_unpack(mrd_mesh *m, const void *buf_dev, void *stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * Mesh generation, first slice (section 2.4, and 4.1.3, L665-L667): the kernels that open
+ * every iteration of the parallel Delaunay refinement, and the exact predicates the rest of it rests on.  Bounded meshes
+ * (no periodic unwrap).  All arrays are DEVICE arrays of the current device; the calls synchronise `stream`.
+ *
+ * mrd_meshgen_test_quality: for every triangle (a, b, c) = tri[t] of the counter-clockwise mesh
+ *   r[t]     circumradius, eq. 2 (L146): l_a l_b l_c / (2 det), det the determinant of eq. 3
+ *   beta[t]  r / shortest edge (L120: 2 beta = 1 / sin(smallest angle))
+ *   cc[t]    circumcentre, where the refinement inserts the new vertex (L150); double[nt][2]
+ *   bad[t]   1 if r > R (too big) or beta > B (low quality) (L150), or det <= 0 (not counter-clockwise); uint8
+ *   n_bad    HOST out (may be NULL): number of flagged triangles
+ *   xy double[nv][2], tri int32[nt][3].  Every operation is a single IEEE round-to-nearest operation in a fixed order: the
+ *   results are reproducible bit for bit (oracle/meshgen.py evaluates the same sequence).
+ * mrd_meshgen_orient2d / _incircle2d: the SIGN (+1, 0, -1; int8) of the determinants of eq. 3 (L160: positive when a, b, c are
+ *   counter-clockwise) and eq. 5 (L198: positive when d lies inside the circle through the counter-clockwise a, b, c), EXACT
+ *   for any double coordinates: a floating-point filter with a rigorous error bound, then exact expansion arithmetic for the
+ *   tests it cannot decide (L166, L206: "we need the test to give the exact result").  idx int32[n][3] / [n][4]: vertex
+ *   numbers of (a, b, c[, d]) of each test; n_exact HOST out (may be NULL): how many tests needed the exact path.
+ * Errors: MRD_EINVAL (null pointer, non-positive R or B), MRD_ENOMEM, MRD_ECUDA.
+ * ---------------------------------------------------------------------------------------------- */
+int mrd_meshgen_test_quality(int64_t n_triangle, const double *xy_dev, const int32_t *tri_dev, double R, double B,
+                             double *r_dev, double *beta_dev, double *cc_dev, uint8_t *bad_dev, int64_t *n_bad, void *stream);
+int mrd_meshgen_orient2d(int64_t n, const double *xy_dev, const int32_t *idx_dev, int8_t *sign_dev, int64_t *n_exact, void *stream);
+int mrd_meshgen_incircle2d(int64_t n, const double *xy_dev, const int32_t *idx_dev, int8_t *sign_dev, int64_t *n_exact, void *stream);
+
 /* Kernel launch counter: number of the library's own kernel launches since the mesh was created. */
 int mrd_launch_count(const mrd_mesh *m, int64_t *launches);
 

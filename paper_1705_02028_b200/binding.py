@@ -84,6 +84,9 @@ def lib():
         L.mrd_range_get.argtypes = [vp, C.c_int32, vp, vp]
         L.mrd_range_set.argtypes = [vp, C.c_int32, vp, vp]
         L.mrd_halo_unpack.argtypes = [vp, vp, vp]
+        L.mrd_meshgen_test_quality.argtypes = [C.c_int64, vp, vp, C.c_double, C.c_double, vp, vp, vp, vp, _lp, vp]
+        L.mrd_meshgen_orient2d.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
+        L.mrd_meshgen_incircle2d.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
         L.mrd_last_error.restype = C.c_char_p
         L.mrd_version.restype = C.c_char_p
         L._path = path
@@ -411,3 +414,41 @@ def measure_peaks(stream=None):
     a, b, c = C.c_double(), C.c_double(), C.c_double()
     _check(lib().mrd_measure_peaks(C.byref(a), C.byref(b), C.byref(c), _stream_ptr(stream)))
     return a.value, b.value, c.value
+
+
+# ---- mesh generation, first slice (include/mrd.h "Mesh generation"): torch CUDA tensors in, torch CUDA tensors out ----
+def meshgen_test_quality(xy, tri, R, B, stream=None):
+    """xy float64 [nv][2], tri int32 [nt][3] (CUDA tensors) -> dict(r, beta, cc, bad, n_bad)."""
+    import torch
+    assert xy.is_cuda and xy.dtype == torch.float64 and xy.is_contiguous() and tri.is_cuda and tri.dtype == torch.int32 and tri.is_contiguous()
+    nt = tri.shape[0]
+    r = torch.empty(nt, dtype=torch.float64, device="cuda")
+    beta = torch.empty(nt, dtype=torch.float64, device="cuda")
+    cc = torch.empty((nt, 2), dtype=torch.float64, device="cuda")
+    bad = torch.empty(nt, dtype=torch.uint8, device="cuda")
+    n_bad = C.c_int64(0)
+    _check(lib().mrd_meshgen_test_quality(nt, C.c_void_p(xy.data_ptr()), C.c_void_p(tri.data_ptr()), float(R), float(B),
+                                          C.c_void_p(r.data_ptr()), C.c_void_p(beta.data_ptr()), C.c_void_p(cc.data_ptr()),
+                                          C.c_void_p(bad.data_ptr()), C.byref(n_bad), _stream_ptr(stream)))
+    return dict(r=r, beta=beta, cc=cc, bad=bad, n_bad=n_bad.value)
+
+
+def _meshgen_predicate(fn, width, xy, idx, stream):
+    import torch
+    assert xy.is_cuda and xy.dtype == torch.float64 and xy.is_contiguous()
+    assert idx.is_cuda and idx.dtype == torch.int32 and idx.is_contiguous() and idx.shape[1] == width
+    sign = torch.empty(idx.shape[0], dtype=torch.int8, device="cuda")
+    n_exact = C.c_int64(0)
+    _check(fn(idx.shape[0], C.c_void_p(xy.data_ptr()), C.c_void_p(idx.data_ptr()), C.c_void_p(sign.data_ptr()), C.byref(n_exact),
+              _stream_ptr(stream)))
+    return sign, n_exact.value
+
+
+def meshgen_orient2d(xy, idx, stream=None):
+    """Exact sign of eq. 3 for every row (a, b, c) of idx: (int8 tensor, number of tests that took the exact path)."""
+    return _meshgen_predicate(lib().mrd_meshgen_orient2d, 3, xy, idx, stream)
+
+
+def meshgen_incircle2d(xy, idx, stream=None):
+    """Exact sign of eq. 5 for every row (a, b, c, d) of idx."""
+    return _meshgen_predicate(lib().mrd_meshgen_incircle2d, 4, xy, idx, stream)

@@ -755,8 +755,11 @@ template <class R> int dump_impl(mrd_mesh *m, double *phiT, double *phiN, double
   }
   m->dbg = m->fused;
   for (int pass = 0; pass < 2; ++pass) {
+    // pass 0: the LDA residuals (and the stored N residuals); pass 1: the residuals the configured scheme distributes
     if (pass == 0) launch_stage1<R, MRD_SCHEME_LDA>(m, true, a, s);
     else if (m->L.p.scheme == MRD_SCHEME_BX) launch_bx_stage1<R>(m, a, s);
+    else if (m->L.p.scheme == MRD_SCHEME_N) launch_stage1<R, MRD_SCHEME_N>(m, true, a, s);
+    else if (m->L.p.scheme == MRD_SCHEME_LDA) launch_stage1<R, MRD_SCHEME_LDA>(m, true, a, s);
     else launch_stage1<R, MRD_SCHEME_B>(m, true, a, s);
     CUDA_TRY(cudaMemcpyAsync(h3.data(), m->d_phi, h3.size() * sizeof(R), cudaMemcpyDeviceToHost, s));
     CUDA_TRY(cudaStreamSynchronize(s));
@@ -837,8 +840,11 @@ template <class R> int dump_sample_impl(mrd_mesh *m, int64_t ns, const int64_t *
     return e;
   };
   for (int pass = 0; pass < 2; ++pass) {
+    // pass 0: the LDA residuals (and the stored N residuals); pass 1: the residuals the configured scheme distributes
     if (pass == 0) launch_stage1<R, MRD_SCHEME_LDA>(m, true, a, s);
     else if (m->L.p.scheme == MRD_SCHEME_BX) launch_bx_stage1<R>(m, a, s);
+    else if (m->L.p.scheme == MRD_SCHEME_N) launch_stage1<R, MRD_SCHEME_N>(m, true, a, s);
+    else if (m->L.p.scheme == MRD_SCHEME_LDA) launch_stage1<R, MRD_SCHEME_LDA>(m, true, a, s);
     else launch_stage1<R, MRD_SCHEME_B>(m, true, a, s);
     CUDA_TRY(cudaStreamSynchronize(s));
     CUDA_TRY(cudaGetLastError());
@@ -894,6 +900,8 @@ template <class R> int dump_sample_impl(mrd_mesh *m, int64_t ns, const int64_t *
 extern "C" {
 
 const char *mrd_last_error(void) { return g_err.c_str(); }
+// error hook of the other translation units of the library (mrd_meshgen.cu): same thread-local message
+int mrd_internal_set_error(int code, const char *msg) { return fail(code, msg ? msg : ""); }
 const char *mrd_version(void) { return "mrd 0.1 (sm_100a)"; }
 
 int mrd_layout_create(mrd_layout **out, const mrd_params *p, int64_t nv, const double *xy, int64_t nt,

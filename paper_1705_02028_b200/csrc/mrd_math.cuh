@@ -416,6 +416,16 @@ __device__ __forceinline__ void apply_beta(R gamma, const TriCore<R> &k, const T
 // B_i = Theta N_i + (1 - Theta) LDA_i, written over N.
 // Theta_kk of eq. 53 for all four components; bvar 1 / 2: all entries replaced by their maximum / minimum (Bmax / Bmin,
 // L503)
+// range in which the product of the four blend denominators (and its reciprocal) is safely a normal number
+template <class R> struct ProductRange;
+template <> struct ProductRange<double> {
+  static __device__ __forceinline__ double lo() { return 1e-290; }
+  static __device__ __forceinline__ double hi() { return 1e290; }
+};
+template <> struct ProductRange<float> {   // (the fp32 variant takes one reciprocal per component: never used)
+  static __device__ __forceinline__ float lo() { return 1e-30f; }
+  static __device__ __forceinline__ float hi() { return 1e30f; }
+};
 template <class R> __device__ __forceinline__ void blend_theta(const R X[4], const R N[3][4], int bvar, R th[4]) {
   using F = Fast<R>;
   // Theta = min(1, |X| / den), and 0 on a zero denominator (C10).  den = 0 means every nodal residual is exactly 0,
@@ -432,7 +442,7 @@ template <class R> __device__ __forceinline__ void blend_theta(const R X[4], con
 #pragma unroll
     for (int c = 0; c < 4; ++c) d[c] = den[c] > R(0) ? den[c] : R(1);
     const R p01 = d[0] * d[1], p23 = d[2] * d[3], P = p01 * p23;
-    if (P > R(1e-290) && P < R(1e290)) {
+    if (P > ProductRange<R>::lo() && P < ProductRange<R>::hi()) {
       const R r = F::rcp(P);
       const R r01 = r * p23, r23 = r * p01;   // 1 / (d0 d1), 1 / (d2 d3)
       const R inv[4] = {r01 * d[1], r01 * d[0], r23 * d[3], r23 * d[2]};
