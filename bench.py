@@ -358,7 +358,7 @@ def run_mrd(args):
         ach = bytes_unit * nt / (dom_ms * 1e-3) * 1e-9
         roof = {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs}
     traffic = args.traffic
-    if traffic is None and dom in NCU_TRAFFIC_BYTES_TRI and prec in NCU_TRAFFIC_BYTES_TRI[dom] and args.tile in (0, 128):
+    if traffic is None and dom in NCU_TRAFFIC_BYTES_TRI and prec in NCU_TRAFFIC_BYTES_TRI[dom] and args.tile in (0, 256):
         traffic = NCU_TRAFFIC_BYTES_TRI[dom][prec] * nt      # per launch, from the committed ncu capture of this kernel
     roof.update({"traffic": traffic, "kernel": dom, "kernel_ms": dom_ms, "peak_source": hbm_src if roof["bound"] == "hbm"
                  else "derived: 148 SM x %d lanes x 2 x %.0f MHz" % (64 if prec == "fp64" else 128, sm_max),

@@ -55,9 +55,9 @@ typedef struct {
   int32_t reorder;    /* 1 = renumber vertices/triangles along a Morton curve (L669-L675); 0 = keep    */
   double period_x;    /* > 0: periodic in x with this period, coordinates in [0, period); 0 = bounded  */
   double period_y;    /* same for y (L584: periodicity is "handled by the mesh")                       */
-  int32_t tile;       /* triangles per thread block of the fused tile kernels: 0 = default (128), or 64, 128; -1 = the unfused kernels (one thread per triangle through
-                         global memory, kept for comparison). Results depend on it through summation order
-                         only                                                                          */
+  int32_t tile;       /* triangles (= threads) per tile of the fused tile kernels: 0 = default (256), or 64, 128, 256; -1 = the
+                         unfused kernels (one thread per triangle through global memory, kept for comparison).  Results
+                         depend on it through summation order only                                              */
   int32_t lumping;    /* 0 = global lumping (all tests of the paper, L576); 1 = selective lumping with the Galerkin
                          mass matrix (eq. 66-67), stage 2 of time_order 2 only                        */
   double domain_size; /* MRD_SCHEME_BX: "L, the domain size" of eq. 56 (L515; reading C25).  0 = take it from this mesh

@@ -212,7 +212,7 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
   if (p->period_x < 0.0 || p->period_y < 0.0) { err = "negative period"; return MRD_EINVAL; }
   if (p->domain_size < 0.0 || !(p->domain_size == p->domain_size)) { err = "negative domain_size"; return MRD_EINVAL; }
   if (ne < 0 || (ne > 0 && !wall_edge)) { err = "bad wall edge list"; return MRD_EINVAL; }
-  if (p->tile != -1 && p->tile != 0 && p->tile != 64 && p->tile != 128) { err = "tile must be -1, 0, 64 or 128"; return MRD_EINVAL; }
+  if (p->tile != -1 && p->tile != 0 && p->tile != 64 && p->tile != 128 && p->tile != 256) { err = "tile must be -1, 0, 64, 128 or 256"; return MRD_EINVAL; }
   L.p = *p;
   L.nv = nv; L.nt = nt; L.ne = ne;
   const double period[2] = {p->period_x, p->period_y};
@@ -395,7 +395,7 @@ int layout_build(mrd_layout &L, const mrd_params *p, int64_t nv, const double *x
   }
 
   MRD_PHASE(pt, "walls");
-  L.tile = p->tile == 0 ? 128 : (p->tile < 0 ? 0 : p->tile);  // 0 = default tile, -1 = unfused kernels
+  L.tile = p->tile == 0 ? 256 : (p->tile < 0 ? 0 : p->tile);  // 0 = default tile, -1 = unfused kernels
   if (L.tile > 0) build_tile_plan(L, xyi);
   MRD_PHASE(pt, "tile plan total");
   return MRD_OK;
@@ -520,8 +520,8 @@ static void build_tile_plan(mrd_layout &L, const std::vector<double> &xyi) {
   for (int64_t b = 0; b < ntile; ++b) {
     const int64_t t0 = b * T, t1 = std::min(nt, t0 + T);
     const int n = (int)(t1 - t0);
-    double g[128][12];
-    int order[128];
+    double g[256][12];
+    int order[256];
     for (int q = 0; q < n; ++q) {
       triangle_geometry(&L.tri[3 * (t0 + q)], xyi.data(), period, g[q]);
       g[q][11] = 0.0;

@@ -1,6 +1,6 @@
 """Parity of the tile kernels WITHOUT the geometry table (`tile_kernel<..., GTAB = false>`: every jittered or flipped
-mesh) at a size where the persistent loop iterates: 512^2 vertices = 524 288 triangles = 4096 tiles of 128 (8192 of
-64) on a grid of at most 148 x 8 blocks, so every block refills its buffers several times, uses the second buffer and
+mesh) at a size where the persistent loop iterates: 512^2 vertices = 524 288 triangles = 2048 tiles of 256 (the default;
+4096 of 128, 8192 of 64) on a grid of 148 x 1024 / tile blocks, so every block refills its buffers several times, uses the second buffer and
 flips the mbarrier phase (mrd_tile.cuh: the "last warp out refills" branch and the parity `(k >> 1) & 1`).  The small
 meshes of tests/test_gpu_parity.py give every block exactly one tile and never reach those branches.
 Shape: the paper's unstructured periodic mesh, scaled down; SURVEY 8(f2).
@@ -63,13 +63,13 @@ def make_pair(mrd, kind, **kw):
 
 
 @pytest.mark.parametrize("scheme", [2, 5])             # B, Bx
-@pytest.mark.parametrize("tile", [0, 64])
+@pytest.mark.parametrize("tile", [0, 64, 128])
 @pytest.mark.parametrize("kind", ["jitter", "flip", "bounded"])
 def test_non_table_tile_path_where_the_persistent_loop_iterates(mrd, kind, tile, scheme):
     import torch
     mesh, flag, W, gm, om = make_pair(mrd, kind, tile=tile, scheme=scheme)
     lay = mrd.Layout(mesh.xy, mesh.tri, vertex_flag=flag, period=mesh.period, tile=tile)
-    assert lay.ntile >= 3500                            # >= 3 tiles per block on any grid the launcher can pick
+    assert lay.ntile >= 1850                            # >= 3 tiles per block on any grid the launcher can pick (<= 148 x 1024 / tile blocks)
     if kind != "jitter":
         val = np.bincount(mesh.tri.ravel(), minlength=mesh.nv)
         assert val.max() >= 9 and val.min() <= 4

@@ -48,7 +48,7 @@ def rel(a, b):
 # per-triangle quantities
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("case", ["smooth_jitter", "vortex", "kh_permuted", "supersonic"])
-@pytest.mark.parametrize("tile", [-1, 0, 64])
+@pytest.mark.parametrize("tile", [-1, 0, 64, 128])
 def test_stage1_per_triangle_matches_oracle(mrd, case, tile):
     if case == "smooth_jitter":
         mesh = wl.jitter_mesh(wl.uniform_mesh(37, 29, 2.0, 1.5, periodic=True), 0.22, seed=3)
@@ -87,7 +87,7 @@ def test_uniform_flow_has_exactly_zero_residual_and_state_is_bitwise_kept(mrd):
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("scheme,order", [(2, 2), (0, 1), (1, 2), (0, 2), (2, 1)])
 @pytest.mark.parametrize("reorder", [True, False])
-@pytest.mark.parametrize("tile", [-1, 0, 64])
+@pytest.mark.parametrize("tile", [-1, 0, 64, 128])
 def test_one_step_and_many_steps_match_oracle(mrd, scheme, order, reorder, tile):
     mesh = wl.jitter_mesh(wl.uniform_mesh(33, 27, 1.0, 1.0, periodic=True), 0.2, seed=11)
     # LDA is not monotone (L457): at Mach 1.2 the steepening waves drive p <= 0 in the oracle too, so it gets Mach 0.5
