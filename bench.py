@@ -31,23 +31,43 @@ METRIC = "triangle_updates_per_s_rk2_step"
 UNIT = "triangle-updates/s"
 
 # ---- per-unit algorithmic figures --------------------------------
-# FLOPs per triangle per stage = min(oracle operation count, FLOPs the kernel executes).  The kernel's count
-# (2*DFMA + DADD + DMUL per thread, from ncu's smsp__sass_thread_inst_executed_op_d*_pred_on of the profiled
-# launch, profiles/) is the smaller one; the oracle's own count (orc_count_ops) is kept for context.
-FLOPS_TRI_STAGE1 = {"fp64": 677.0, "fp32": 640.0}
-FLOPS_TRI_STAGE2 = {"fp64": 753.0, "fp32": 710.0}
-FLOPS_VERTEX_STAGE = 144.0             # per triangle-update, all three vertex kernels together (ncu: 8.6 + 71.5 + 63.5)
+# FLOPs per triangle and launch = min(oracle operation count, FLOPs the kernel executes).  The kernel's count
+# (2*FMA + ADD + MUL thread instructions, predicated on, of the profiled launch) is the smaller one; it comes, with the
+# measured dram bytes per triangle, from the committed capture profiles/r02_kernel_metrics.csv (+ .md: the command).
+# The built-in figures below are that file's fp64 / fp32 rows for the uniform mesh and tiles of 256 triangles: they
+# serve when no row of the file matches the run (then `flops_source` says so and `traffic` is null).
+METRICS_CSV = os.path.join(ROOT, "profiles", "r02_kernel_metrics.csv")
+FLOPS_BUILTIN = {"fp64": {"tri_stage1": 635.2, "gather_dt": 9.6, "update": 71.4, "tri_stage2": 718.1, "gather_update": 63.4},
+                 "fp32": {"tri_stage1": 598.2, "gather_dt": 9.6, "update": 38.4, "tri_stage2": 684.2, "gather_update": 31.9}}
+STEP_KERNELS = ("tri_stage1", "gather_dt", "update", "tri_stage2", "gather_update")
 ORACLE_FLOPS_TRI = (2098.0, 2194.0)    # oracle.count_ops(stage 1 / stage 2): add+mul+div+sqrt
-# compulsory HBM bytes per triangle of one triangle-kernel launch (share of SURVEY 8d's 130 B per triangle-update):
-# state read once (32 B per vertex / 2), connectivity 12 B, coordinates 8 B; stage 2 also reads W^n (dW/dt)
-BYTES_TRI_STAGE1 = {"fp64": 36.0, "fp32": 24.0}
-BYTES_TRI_STAGE2 = {"fp64": 52.0, "fp32": 32.0}
-# bytes the fused kernels move BY DESIGN (slot copies, plan record, stored phi^N/phi^T, partials), for comparison
-# with ncu's dram__bytes (the roofline object's `traffic`)
-DESIGN_BYTES_TRI = {"tri_stage1": {"fp64": 196.0, "fp32": 106.0}, "tri_stage2": {"fp64": 207.0, "fp32": 112.0}}
-# ncu dram__bytes_read.sum + dram__bytes_write.sum per triangle of the profiled launches (profiles/*.md)
-NCU_TRAFFIC_BYTES_TRI = {"tri_stage1": {"fp64": 195.8}, "tri_stage2": {"fp64": 207.8}}
+# compulsory HBM bytes per triangle of one launch (shares of SURVEY 8d's 130 B per triangle-update):
+# tile kernels: state read once (32 B per vertex / 2), connectivity 12 B, coordinates 8 B; stage 2 also reads dW/dt;
+# vertex kernels (what is left of the 130 B): one state written per stage (32 B per vertex / 2) and V_i read (8 B / 2)
+BYTES_ALG = {"fp64": {"tri_stage1": 36.0, "tri_stage2": 52.0, "gather_dt": 2.0, "update": 20.0, "gather_update": 20.0},
+             "fp32": {"tri_stage1": 24.0, "tri_stage2": 32.0, "gather_dt": 1.0, "update": 9.5, "gather_update": 9.5}}
+# bytes the fused kernels move BY DESIGN per triangle (slot copies, stored stage-1 cells, partials),
+# for comparison with ncu's dram__bytes (the roofline object's `traffic`)
+DESIGN_BYTES_TRI = {"tri_stage1": {"fp64": 144.0, "fp32": 72.0}, "tri_stage2": {"fp64": 155.0, "fp32": 77.0}}
 B_ALG_STEP = {"fp64": 130.0, "fp32": 76.0}
+
+
+def kernel_metrics(precision: str, mesh: str, tile: int):
+    """Rows of the committed ncu capture that describe THIS run: same precision, same kind of mesh (the geometry-table
+    kernels of the uniform mesh and the coordinate kernels of every other mesh are different instantiations) and same tile
+    size.  Returns ({kernel: row}, source text) -- ({}, reason) when nothing matches."""
+    import csv
+    tile = 256 if tile == 0 else tile
+    try:
+        with open(METRICS_CSV) as f:
+            rows = [r for r in csv.DictReader(f)]
+    except OSError:
+        return {}, "none: profiles/r02_kernel_metrics.csv not found"
+    hit = {r["kernel"]: r for r in rows if r["precision"] == precision and r["mesh"] == mesh and int(r["tile"]) == tile}
+    if not hit:
+        return {}, f"none: no ncu capture of precision {precision}, mesh '{mesh}', tile {tile} in profiles/r02_kernel_metrics.csv"
+    size = next(iter(hit.values()))["size"]
+    return hit, f"profiles/r02_kernel_metrics.csv ({precision}, mesh '{mesh}' --size {size}, tile {tile}): ncu dram bytes per triangle x triangles of this run"
 
 
 def measured_peaks():
@@ -62,7 +82,7 @@ def measured_peaks():
 
 class ClockSampler:
     """SM clock and throttle reasons sampled DURING the timed region (B200_PROFILING.md), through NVML
-    (nvidia_ml_py; the same counters nvidia-smi prints) every 20 ms from a background thread."""
+    (nvidia_ml_py; the same counters nvidia-smi prints) every 5 ms from a background thread, started before the warm-up steps."""
     REASONS = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
 
     def __init__(self, index: int):
@@ -99,7 +119,7 @@ class ClockSampler:
                 self.power.append(n.nvmlDeviceGetPowerUsage(self._h) / 1000.0)
             except Exception:
                 pass
-            self._stop.wait(0.02)
+            self._stop.wait(0.005)
 
     def __exit__(self, *a):
         self._stop.set()
@@ -148,6 +168,20 @@ def build_workload(n: int, numbering: str, kind: str = "uniform"):
     if kind != "uniform":
         cfg.W0 = wl.vortex_state(cfg.mesh)     # the same vortex, sampled at the moved vertices
     return cfg
+
+
+def workload_text(args, nt: int) -> str:
+    """config.workload of the single-GPU line: what was actually built (build_workload)."""
+    tail = f"{nt} triangles, scheme B, RK2, CFL 0.5"
+    if args.mesh == "delaunay":
+        return (f"isentropic vortex on a seeded graded Delaunay triangulation ({args.n}^2 points, cell size 100:1, frozen boundary ring; the "
+                f"shape of the paper's unstructured mesh, PAPER.md L685), Morton-ordered by the layout stage, {tail}")
+    head = f"BASELINE.json config 5: isentropic vortex, periodic uniform triangulation {args.n}^2 vertices"
+    if args.mesh == "jitter":
+        head += ", every vertex moved by up to 0.2 cell widths (seed 7: no two triangles alike)"
+    if args.mesh == "flip":
+        head += ", every vertex moved by up to 0.2 cell widths and a seeded third of the edges flipped (variable valence)"
+    return f"{head}, {args.numbering} input numbering, {tail}"
 
 
 def setup_part(n: int, world: int, rank: int):
@@ -246,6 +280,7 @@ def run_mrd(args):
         torch.cuda.synchronize()
 
     prec = args.precision
+    tile_eff = 256 if args.tile == 0 else args.tile      # 0 = the library's default
     tdtype = torch.float64 if prec == "fp64" else torch.float32
     halo = world > 1 and args.decomposition == "halo"
     params = dict(gamma=1.4, cfl=0.5, scheme=mrd.SCHEME_B, time_order=2, precision=mrd.FP64 if prec == "fp64" else mrd.FP32,
@@ -258,6 +293,7 @@ def run_mrd(args):
         mesh = cfg.mesh
         nt, nv = mesh.nt, mesh.nv                 # units per rank
         nt_job, nv_job = world * nt, world * nv
+        t0 = time.perf_counter()                  # layout_s: the library's one-off stage alone (mrd_mesh_create, upload included)
         gm = sim = mrd.Mesh(mesh.xy, mesh.tri, vertex_flag=cfg.vertex_flag, period=mesh.period, **params)
         layout_s = time.perf_counter() - t0
         gm.set_state(torch.tensor(cfg.W0, dtype=tdtype, device="cuda"))
@@ -339,11 +375,18 @@ def run_mrd(args):
     hbm_gbs, hbm_src = measured_peaks()
     clocks = clk.summary()
     sm_max = clocks["sm_max_mhz"] or 1965.0
-    main = {k: v for k, v in prof.items() if k in ("tri_stage1", "tri_stage2", "gather_dt", "update", "gather_update")}
+    main = {k: v for k, v in prof.items() if k in STEP_KERNELS}
     dom = max(main, key=main.get)
     dom_ms = main[dom]
-    flops_unit = {"tri_stage1": FLOPS_TRI_STAGE1[prec], "tri_stage2": FLOPS_TRI_STAGE2[prec]}.get(dom, FLOPS_VERTEX_STAGE / 2)
-    bytes_unit = {"tri_stage1": BYTES_TRI_STAGE1[prec], "tri_stage2": BYTES_TRI_STAGE2[prec]}.get(dom, 40.0)
+    ncu, ncu_src = kernel_metrics(prec, args.mesh, args.tile)
+    if ncu:
+        flops = {k: float(ncu[k]["flops_per_triangle"]) for k in STEP_KERNELS}
+        flops_src = ncu_src.split(":")[0] + ": executed 2*FMA + MUL + ADD per triangle"
+    else:
+        flops = dict(FLOPS_BUILTIN[prec])
+        flops_src = f"built-in ({prec}, uniform mesh, tile 256, of profiles/r02_kernel_metrics.csv): {ncu_src[6:]}"
+    flops_unit, bytes_unit = flops[dom], BYTES_ALG[prec][dom]
+    flops_step = sum(flops.values())
     alu_peak = fp64_peak_nominal(sm_max, prec)
     t_alu = flops_unit * nt / (alu_peak * 1e12)
     t_hbm = bytes_unit * nt / (hbm_gbs * 1e9)
@@ -357,21 +400,28 @@ def run_mrd(args):
     else:
         ach = bytes_unit * nt / (dom_ms * 1e-3) * 1e-9
         roof = {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs}
-    traffic = args.traffic
-    if traffic is None and dom in NCU_TRAFFIC_BYTES_TRI and prec in NCU_TRAFFIC_BYTES_TRI[dom] and args.tile in (0, 256):
-        traffic = NCU_TRAFFIC_BYTES_TRI[dom][prec] * nt      # per launch, from the committed ncu capture of this kernel
-    roof.update({"traffic": traffic, "kernel": dom, "kernel_ms": dom_ms, "peak_source": hbm_src if roof["bound"] == "hbm"
+    if args.traffic is not None:
+        traffic, traffic_src = args.traffic, "--traffic (bytes per launch given on the command line)"
+    elif ncu and 0.5 <= nt / float(ncu[dom]["triangles"]) <= 4.0:
+        traffic, traffic_src = float(ncu[dom]["dram_bytes_per_triangle"]) * nt, ncu_src    # per launch, like `achieved`
+    elif ncu:
+        # (bytes per triangle depend on how much of the mesh the 126 MB L2 holds: only a capture of a comparable size counts)
+        traffic, traffic_src = None, f"none: the ncu capture of this configuration has {ncu[dom]['triangles']} triangles, this run {nt}"
+    else:
+        traffic, traffic_src = None, ncu_src
+    roof.update({"traffic": traffic, "traffic_source": traffic_src, "kernel": dom, "kernel_ms": dom_ms,
+                 "peak_source": hbm_src if roof["bound"] == "hbm"
                  else "derived: 148 SM x %d lanes x 2 x %.0f MHz" % (64 if prec == "fp64" else 128, sm_max),
-                 "alg_flops_per_triangle": flops_unit, "alg_bytes_per_triangle": bytes_unit,
+                 "alg_flops_per_triangle": flops_unit, "alg_bytes_per_triangle": bytes_unit, "flops_source": flops_src,
+                 "oracle_flops_per_triangle": {"tri_stage1": ORACLE_FLOPS_TRI[0], "tri_stage2": ORACLE_FLOPS_TRI[1]}.get(dom),
                  "alu_frac": flops_unit * nt / (dom_ms * 1e-3) * 1e-12 / alu_peak,
                  "hbm_frac": bytes_unit * nt / (dom_ms * 1e-3) * 1e-9 / hbm_gbs,
                  "measured_fma_tflops": dfma_tf if prec == "fp64" else ffma_tf, "measured_copy_gbs": copy_gbs,
-                 "design_bytes_per_triangle": DESIGN_BYTES_TRI.get(dom, {}).get(prec),
+                 "design_bytes_per_triangle": DESIGN_BYTES_TRI.get(dom, {}).get(prec) if tile_eff == 256 else None,
                  "kernels_ms": prof,
-                 "step_alg": {"flops_per_triangle_update": FLOPS_TRI_STAGE1[prec] + FLOPS_TRI_STAGE2[prec] + FLOPS_VERTEX_STAGE,
+                 "step_alg": {"flops_per_triangle_update": flops_step,
                               "bytes_per_triangle_update": B_ALG_STEP[prec],
-                              "roofline_ms": max((FLOPS_TRI_STAGE1[prec] + FLOPS_TRI_STAGE2[prec] + FLOPS_VERTEX_STAGE) * nt / (alu_peak * 1e12),
-                                                 B_ALG_STEP[prec] * nt / (hbm_gbs * 1e9)) * 1e3}})
+                              "roofline_ms": max(flops_step * nt / (alu_peak * 1e12), B_ALG_STEP[prec] * nt / (hbm_gbs * 1e9)) * 1e3}})
     roof["step_alg"]["frac"] = roof["step_alg"]["roofline_ms"] / ms_step
 
     # ---- the oracle beside it (rank 0, N = 1 only): bounded sample of the same workload --------------------
@@ -386,13 +436,11 @@ def run_mrd(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64" if prec == "fp64" else "f32", "data": "synthetic",
-            "config": {"workload": (f"BASELINE.json config 5: isentropic vortex, periodic uniform triangulation {args.n}^2 "
-                                    f"vertices, {nt} triangles, {args.numbering} input numbering, scheme B, RK2, CFL 0.5"
-                                    + ("" if args.mesh == "uniform" else f", mesh variant '{args.mesh}'")) if not halo else
+            "config": {"workload": workload_text(args, nt) if not halo else
                                    (f"BASELINE.json config 5 stacked {world} times in y: row of {world} isentropic vortices, periodic uniform "
                                     f"triangulation {args.n} x {args.n * world} vertices, {nt_job} triangles, natural input numbering, "
                                     f"scheme B, RK2, CFL 0.5"),
-                       "n_triangles": nt_job, "n_vertices": nv_job, "n_triangles_rank0": nt, "reorder": int(args.reorder), "tile": args.tile,
+                       "n_triangles": nt_job, "n_vertices": nv_job, "n_triangles_rank0": nt, "reorder": int(args.reorder), "tile": tile_eff,
                        "l2": "inputs larger than L2 (state %.0f MB, per-triangle arrays %.1f GB)" % (
                            state_bytes / 1e6, gm.device_bytes() / 1e9),
                        "parallelism": parallelism,

@@ -346,12 +346,6 @@ template <class K, class... Args> int launch_tile(mrd_mesh *m, K kernel, size_t 
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, T, sh);
     if (e != cudaSuccess || occ < 1)
       return fail(MRD_ECUDA, std::string("tile kernel: no resident block fits (") + std::to_string(sh) + " bytes of shared memory): " + cudaGetErrorString(e));
-#ifdef MRD_DEBUG_KNOBS
-    if (const char *cap = std::getenv("MRD_TILE_OCC")) {  // tuning knob (debug builds only): cap the resident blocks per SM
-      int c = std::atoi(cap);
-      if (c >= 1 && c < occ) occ = c;
-    }
-#endif
     it = m->tile_grid.emplace(key, (unsigned)std::min<int64_t>(m->L.ntile, (int64_t)m->nsm * occ)).first;
   }
   kernel<<<it->second, T, sh, s>>>(args...);
@@ -1335,58 +1329,6 @@ int mrd_halo_unpack(mrd_mesh *m, const void *buf_dev, void *stream) {
   cudaStream_t s = (cudaStream_t)stream;
   return m->L.p.precision == MRD_FP64 ? halo_unpack_impl<double>(m, buf_dev, s) : halo_unpack_impl<float>(m, buf_dev, s);
 }
-
-#ifdef MRD_DEBUG_KNOBS
-// experiment: how well do a tile kernel and a vertex kernel share the GPU?  ms[0] tile stage 2 alone (MRD_TILE_OCC blocks per
-// SM), ms[1] the stage-1 vertex update alone, ms[2] both at once on two streams (data hazards ignored: timing only)
-int mrd_debug_overlap(mrd_mesh *m, float ms[3]) {
-  using R = double;
-  using V4 = mrd::Vec4<R>;
-  if (!m || !m->fused || m->L.p.precision != MRD_FP64) return fail(MRD_EINVAL, "fp64 fused mesh only");
-  cudaStream_t sa, sb;
-  cudaStreamCreateWithFlags(&sa, cudaStreamNonBlocking);
-  cudaStreamCreateWithFlags(&sb, cudaStreamNonBlocking);
-  cudaEvent_t e[4];
-  for (auto &x : e) cudaEventCreate(&x);
-  mrd::Ctl c{};
-  fetch_ctl(m, nullptr, &c);
-  mrd::Ctl armed = c;
-  armed.active = 1;
-  cudaMemcpy(m->d_ctl, &armed, sizeof armed, cudaMemcpyHostToDevice);
-  auto md = mesh_dev<R>(m);
-  const unsigned vb = blocks_for(md.nv, 256);
-  const int a = m->cur, b = a ^ 1;
-  auto tile = [&](cudaStream_t s) { launch_stage2<R, MRD_SCHEME_B>(m, b, s); };
-  auto vert = [&](cudaStream_t s) {
-    mrd::slot_gather_update_kernel<R, 0><<<vb, 256, 0, s>>>(md, tile_dev<R>(m), (R)m->L.p.gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)nullptr,
-                                                         (const V4 *)m->d_W[a], (V4 *)m->d_W[b], sink_for<R>(m, b, false, true), m->d_flag);
-  };
-  for (int rep = 0; rep < 3; ++rep) {
-    cudaDeviceSynchronize();
-    cudaEventRecord(e[0], sa); tile(sa); cudaEventRecord(e[1], sa);
-    cudaDeviceSynchronize();
-    cudaEventElapsedTime(&ms[0], e[0], e[1]);
-    cudaEventRecord(e[0], sb); vert(sb); cudaEventRecord(e[1], sb);
-    cudaDeviceSynchronize();
-    cudaEventElapsedTime(&ms[1], e[0], e[1]);
-    cudaEventRecord(e[0], sa);
-    cudaStreamWaitEvent(sb, e[0], 0);
-    tile(sa);
-    vert(sb);
-    cudaEventRecord(e[2], sb);
-    cudaStreamWaitEvent(sa, e[2], 0);
-    cudaEventRecord(e[1], sa);
-    cudaDeviceSynchronize();
-    cudaEventElapsedTime(&ms[2], e[0], e[1]);
-  }
-  cudaMemcpy(m->d_ctl, &c, sizeof c, cudaMemcpyHostToDevice);
-  cudaMemset(m->d_flag, 0, sizeof(int));
-  for (auto &x : e) cudaEventDestroy(x);
-  cudaStreamDestroy(sa);
-  cudaStreamDestroy(sb);
-  return MRD_OK;
-}
-#endif
 
 int mrd_launch_count(const mrd_mesh *m, int64_t *launches) {
   if (!m || !launches) return fail(MRD_EINVAL, "null argument");

@@ -50,6 +50,30 @@ def test_single_process_helpers():
     assert bench.fp64_peak_nominal(1965.0, "fp64") == pytest.approx(37.2, rel=1e-2)
 
 
+def test_roofline_figures_come_from_the_committed_capture_of_the_same_configuration():
+    """`roofline.traffic` is the committed ncu capture's dram bytes per triangle only when precision, kind of mesh and tile size
+    are those of the capture; any other run gets null and a `traffic_source` that says why."""
+    from types import SimpleNamespace
+    sys.path.insert(0, ROOT)
+    import bench
+    rows, src = bench.kernel_metrics("fp64", "uniform", 0)             # tile 0 = the default, 256
+    assert set(rows) == set(bench.STEP_KERNELS) and "r02_kernel_metrics.csv" in src
+    for prec in ("fp64", "fp32"):                                      # the built-in fall-back is the same capture
+        r, _ = bench.kernel_metrics(prec, "uniform", 256)
+        for k in bench.STEP_KERNELS:
+            assert float(r[k]["flops_per_triangle"]) == bench.FLOPS_BUILTIN[prec][k]
+    total = sum(float(rows[k]["dram_bytes_per_triangle"]) for k in bench.STEP_KERNELS)
+    assert 480 < total < 500                                           # 491.6 B per triangle-update (profiles/r02_kernels_full.md)
+    assert bench.kernel_metrics("fp64", "delaunay", 0)[0]["tri_stage1"]["size"] == "1140"
+    for prec, mesh, tile in (("fp64", "uniform", 64), ("fp32", "flip", 0)):
+        rows, src = bench.kernel_metrics(prec, mesh, tile)
+        assert rows == {} and src.startswith("none:")
+    a = SimpleNamespace(mesh="delaunay", n=1140, numbering="morton")
+    assert "Delaunay" in bench.workload_text(a, 7) and "periodic uniform" not in bench.workload_text(a, 7)
+    a.mesh = "uniform"
+    assert "periodic uniform triangulation 1140^2" in bench.workload_text(a, 7)
+
+
 @pytest.mark.slow
 def test_reference_arm_prints_one_json_line_under_torchrun():
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
