@@ -379,6 +379,8 @@ def run_mrd(args):
     dom = max(main, key=main.get)
     dom_ms = main[dom]
     ncu, ncu_src = kernel_metrics(prec, args.mesh, args.tile)
+    if not args.reorder and args.numbering != "morton":
+        ncu, ncu_src = {}, "none: the ncu captures are of Morton-ordered layouts (--reorder 0 on a non-Morton numbering moves other bytes)"
     if ncu:
         flops = {k: float(ncu[k]["flops_per_triangle"]) for k in STEP_KERNELS}
         flops_src = ncu_src.split(":")[0] + ": executed 2*FMA + MUL + ADD per triangle"
