@@ -303,6 +303,44 @@ int mrd_meshgen_test_quality(int64_t n_triangle, const double *xy_dev, const int
 int mrd_meshgen_orient2d(int64_t n, const double *xy_dev, const int32_t *idx_dev, int8_t *sign_dev, int64_t *n_exact, void *stream);
 int mrd_meshgen_incircle2d(int64_t n, const double *xy_dev, const int32_t *idx_dev, int8_t *sign_dev, int64_t *n_exact, void *stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * Mesh generation, second slice: the mesh data structure of section 4.1.2 (L656-L663), the Delaunay triangulator of
+ * section 2.4.6 (L186-L208) / 4.1.5 (L677-L681), and the search for the triangle that contains a new vertex (section 2.4.2,
+ * L152-L168).  Bounded meshes; all arrays DEVICE arrays of the current device; the calls synchronise `stream`.
+ *
+ * Data structure (the paper's four arrays): xy double[nv][2] (vertexCoordinates), tv int32[nt][3] (triangleVertices,
+ * counter-clockwise), te int32[nt][3] (triangleEdges), et int32[ne][2] (edgeTriangles).  Conventions the paper leaves open:
+ * edge k of a triangle is the one OPPOSITE its local vertex k (it joins local vertices k+1 and k+2); a boundary edge (a
+ * segment, L663) has -1 as its second triangle.
+ *
+ * mrd_meshgen_build_edges: te and et from tv.  Edges are numbered in ascending order of (smaller vertex, larger vertex); et
+ *   lists the two neighbours in ascending triangle order.  et_dev must hold 3 * n_triangle pairs (the upper bound); *n_edge
+ *   (HOST out) receives the number of edges.  MRD_EINVAL if an edge belongs to more than two triangles.
+ * mrd_meshgen_delaunay_flip: transforms the valid triangulation (tv, te, et), IN PLACE, into the Delaunay triangulation of its
+ *   vertices by edge flips ("start with any valid triangulation, and perform edge flips until all edges are locally Delaunay",
+ *   L112).  Per iteration (section 4.1.5): the exact INCIRCLE2D test of eq. 5 on every edge whose containing quadrilateral
+ *   changed (all edges in the first iteration) lists the edges that are not Delaunay; of those, an independent set -- no two in
+ *   the same triangle; the higher edge number wins a contested triangle -- is flipped in parallel; edgeTriangles of the edges
+ *   that change sides is repaired in the same pass.  A flipped edge keeps its number and its two triangles: with a opposite E
+ *   in t1 = (a, b, c) and d opposite E in t2 = (d, c, b), t1 becomes (a, b, d) and t2 (a, d, c).  Edges with INCIRCLE2D = 0
+ *   (four cocircular vertices) are left alone.  The result is unique as a set of triangles when no four vertices are
+ *   cocircular (L96), and deterministic (bitwise the same arrays on every run) in any case.
+ *   HOST outs (may be NULL): n_flips, n_iterations, n_exact (INCIRCLE2D tests that needed the exact path).
+ * mrd_meshgen_find_triangle: for every point p[i] (double[n][2]) the triangle that contains it, by walking from t0[i] across
+ *   the first edge -- tried in the order (a, b), (b, c), (c, a) -- that has p strictly on its outer side (exact ORIENT2D,
+ *   eq. 3).  t[i] >= 0: found, with code[i] = 0 strictly inside, 1 + k on edge k of t, 4 + k on local vertex k (L168);
+ *   t[i] = -1 - t_last: the walk left the triangulation through a boundary edge of t_last.  The walk terminates on Delaunay
+ *   triangulations; MRD_EINVAL if a walk exceeds n_triangle + 16 steps (not a Delaunay triangulation).
+ * Errors: MRD_EINVAL (null pointer, inconsistent structure), MRD_ENOMEM, MRD_ECUDA.
+ * ---------------------------------------------------------------------------------------------- */
+int mrd_meshgen_build_edges(int64_t n_triangle, const int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_edge,
+                            void *stream);
+int mrd_meshgen_delaunay_flip(int64_t n_triangle, int64_t n_edge, const double *xy_dev, int32_t *tv_dev, int32_t *te_dev,
+                              int32_t *et_dev, int64_t *n_flips, int64_t *n_iterations, int64_t *n_exact, void *stream);
+int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_t *t0_dev, int64_t n_triangle,
+                              const double *xy_dev, const int32_t *tv_dev, const int32_t *te_dev, const int32_t *et_dev,
+                              int32_t *t_dev, int8_t *code_dev, void *stream);
+
 /* Kernel launch counter: number of the library's own kernel launches since the mesh was created. */
 int mrd_launch_count(const mrd_mesh *m, int64_t *launches);
 

@@ -87,6 +87,9 @@ def lib():
         L.mrd_meshgen_test_quality.argtypes = [C.c_int64, vp, vp, C.c_double, C.c_double, vp, vp, vp, vp, _lp, vp]
         L.mrd_meshgen_orient2d.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
         L.mrd_meshgen_incircle2d.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
+        L.mrd_meshgen_build_edges.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
+        L.mrd_meshgen_delaunay_flip.argtypes = [C.c_int64, C.c_int64, vp, vp, vp, vp, _lp, _lp, _lp, vp]
+        L.mrd_meshgen_find_triangle.argtypes = [C.c_int64, vp, vp, C.c_int64, vp, vp, vp, vp, vp, vp, vp]
         L.mrd_last_error.restype = C.c_char_p
         L.mrd_version.restype = C.c_char_p
         L._path = path
@@ -452,3 +455,44 @@ def meshgen_orient2d(xy, idx, stream=None):
 def meshgen_incircle2d(xy, idx, stream=None):
     """Exact sign of eq. 5 for every row (a, b, c, d) of idx."""
     return _meshgen_predicate(lib().mrd_meshgen_incircle2d, 4, xy, idx, stream)
+
+
+def _dev(t, dtype, cols):
+    import torch
+    assert t.is_cuda and t.dtype == dtype and t.is_contiguous() and t.ndim == 2 and t.shape[1] == cols, (t.dtype, t.shape)
+    return C.c_void_p(t.data_ptr())
+
+
+def meshgen_build_edges(tv, stream=None):
+    """triangleEdges te int32 [nt][3] and edgeTriangles et int32 [ne][2] (section 4.1.2) from triangleVertices tv (CUDA tensor)."""
+    import torch
+    nt = tv.shape[0]
+    te = torch.empty((nt, 3), dtype=torch.int32, device="cuda")
+    et = torch.empty((3 * nt, 2), dtype=torch.int32, device="cuda")
+    ne = C.c_int64(0)
+    _check(lib().mrd_meshgen_build_edges(nt, _dev(tv, torch.int32, 3), C.c_void_p(te.data_ptr()), C.c_void_p(et.data_ptr()),
+                                         C.byref(ne), _stream_ptr(stream)))
+    return te, et[:ne.value].clone()
+
+
+def meshgen_delaunay_flip(xy, tv, te, et, stream=None):
+    """Flip (tv, te, et) IN PLACE to the Delaunay triangulation of xy; returns dict(flips, iterations, exact)."""
+    import torch
+    f, it, ex = C.c_int64(0), C.c_int64(0), C.c_int64(0)
+    _check(lib().mrd_meshgen_delaunay_flip(tv.shape[0], et.shape[0], _dev(xy, torch.float64, 2), _dev(tv, torch.int32, 3),
+                                           _dev(te, torch.int32, 3), _dev(et, torch.int32, 2), C.byref(f), C.byref(it), C.byref(ex),
+                                           _stream_ptr(stream)))
+    return dict(flips=f.value, iterations=it.value, exact=ex.value)
+
+
+def meshgen_find_triangle(xy, tv, te, et, p, t0, stream=None):
+    """For every point p[i] the containing triangle, walking from t0[i]: (t int32 [n], code int8 [n]); see include/mrd.h."""
+    import torch
+    n = p.shape[0]
+    assert t0.is_cuda and t0.dtype == torch.int32 and t0.is_contiguous() and t0.shape == (n,)
+    t = torch.empty(n, dtype=torch.int32, device="cuda")
+    code = torch.empty(n, dtype=torch.int8, device="cuda")
+    _check(lib().mrd_meshgen_find_triangle(n, _dev(p, torch.float64, 2), C.c_void_p(t0.data_ptr()), tv.shape[0], _dev(xy, torch.float64, 2),
+                                           _dev(tv, torch.int32, 3), _dev(te, torch.int32, 3), _dev(et, torch.int32, 2),
+                                           C.c_void_p(t.data_ptr()), C.c_void_p(code.data_ptr()), _stream_ptr(stream)))
+    return t, code

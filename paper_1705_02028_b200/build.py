@@ -13,7 +13,7 @@ CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(os.path.dirname(HERE), "include")
 SRC = [os.path.join(CSRC, "mrd_api.cu"), os.path.join(CSRC, "mrd_meshgen.cu"), os.path.join(CSRC, "mrd_layout.cpp"),
        os.path.join(CSRC, "mrd_partition.cpp")]
-DEPS = SRC + [os.path.join(CSRC, f) for f in ("mrd_kernels.cuh", "mrd_tile.cuh", "mrd_math.cuh", "mrd_layout.h")] + [
+DEPS = SRC + [os.path.join(CSRC, f) for f in ("mrd_kernels.cuh", "mrd_tile.cuh", "mrd_math.cuh", "mrd_layout.h", "mrd_predicates.cuh")] + [
     os.path.join(INC, "mrd.h")]
 LIB = os.path.join(HERE, "libmrd.so")
 

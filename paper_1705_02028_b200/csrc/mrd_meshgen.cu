@@ -15,10 +15,14 @@
 // zero elimination).  The sign of an expansion is the sign of its largest component.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdint>
+#include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
 #include <string>
 
 #include "../../include/mrd.h"
+#include "mrd_predicates.cuh"
 
 namespace mrdgen {
 
@@ -62,142 +66,16 @@ test_quality_kernel(int64_t nt, const double2 *__restrict__ xy, const int32_t *_
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// Expansion arithmetic (device).  An expansion is a sum of doubles e[0..n) that do not overlap, in increasing magnitude, zeros
-// removed.  All operations below are exact.
-// ------------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void two_sum(double a, double b, double &s, double &e) {
-  s = __dadd_rn(a, b);
-  const double bb = __dsub_rn(s, a);
-  e = __dadd_rn(__dsub_rn(a, __dsub_rn(s, bb)), __dsub_rn(b, bb));
-}
-__device__ __forceinline__ void two_diff(double a, double b, double &s, double &e) { two_sum(a, -b, s, e); }
-__device__ __forceinline__ void two_prod(double a, double b, double &p, double &e) {
-  p = __dmul_rn(a, b);
-  e = __fma_rn(a, b, -p);
-}
-// h = e + b (e: expansion of length n, b: any double); returns the new length.  h may alias e.
-__device__ int grow(const double *e, int n, double b, double *h) {
-  double Q = b;
-  int m = 0;
-  for (int i = 0; i < n; ++i) {
-    double s, lo;
-    two_sum(Q, e[i], s, lo);
-    Q = s;
-    if (lo != 0.0) h[m++] = lo;
-  }
-  if (Q != 0.0 || m == 0) h[m++] = Q;
-  return m;
-}
-// e += f (both expansions); e must have room for n + m components
-__device__ int expansion_add(double *e, int n, const double *f, int m) {
-  for (int j = 0; j < m; ++j) n = grow(e, n, f[j], e);
-  return n;
-}
-// acc += s * (e[0..n) * b): the exact products go in one component at a time
-__device__ int add_scaled(double *acc, int na, const double *e, int n, double b, double s) {
-  for (int i = 0; i < n; ++i) {
-    double p, lo;
-    two_prod(e[i], b, p, lo);
-    if (lo != 0.0) na = grow(acc, na, s * lo, acc);
-    if (p != 0.0) na = grow(acc, na, s * p, acc);
-  }
-  return na;
-}
-// acc += s * (e * f), e and f expansions
-__device__ int add_product(double *acc, int na, const double *e, int n, const double *f, int m, double s) {
-  for (int j = 0; j < m; ++j) na = add_scaled(acc, na, e, n, f[j], s);
-  return na;
-}
-__device__ __forceinline__ int sign_of(const double *e, int n) {
-  const double top = e[n - 1];
-  return top > 0.0 ? 1 : (top < 0.0 ? -1 : 0);
-}
-
-// orient2d, exact: (ax - cx)(by - cy) - (ay - cy)(bx - cx) with every difference a two-component expansion
-__device__ int orient2d_exact(double2 a, double2 b, double2 c) {
-  double A[2][2], Bv[2][2];
-  int nA[2], nB[2];
-  const double av[2] = {a.x, a.y}, bv[2] = {b.x, b.y}, cv[2] = {c.x, c.y};
-  for (int k = 0; k < 2; ++k) {
-    double s, lo;
-    two_diff(av[k], cv[k], s, lo);
-    nA[k] = 0;
-    if (lo != 0.0) A[k][nA[k]++] = lo;
-    if (s != 0.0 || nA[k] == 0) A[k][nA[k]++] = s;
-    two_diff(bv[k], cv[k], s, lo);
-    nB[k] = 0;
-    if (lo != 0.0) Bv[k][nB[k]++] = lo;
-    if (s != 0.0 || nB[k] == 0) Bv[k][nB[k]++] = s;
-  }
-  double acc[20];
-  acc[0] = 0.0;
-  int n = 1;
-  n = add_product(acc, n, A[0], nA[0], Bv[1], nB[1], 1.0);    // + (ax - cx)(by - cy)
-  n = add_product(acc, n, A[1], nA[1], Bv[0], nB[0], -1.0);   // - (ay - cy)(bx - cx)
-  return sign_of(acc, n);
-}
-
-// incircle2d, exact (eq. 5): sum over the rows (a, b, c) of lift_row * minor_row with the rows translated by d
-constexpr int MAXE = 1200;   // 3 x (12 x 16 x 2) = 1152 components at most
-__device__ int incircle2d_exact(double2 a, double2 b, double2 c, double2 d, double *acc, double *tmp) {
-  const double px[3] = {a.x, b.x, c.x}, py[3] = {a.y, b.y, c.y};
-  double X[3][2], Y[3][2];
-  int nX[3], nY[3];
-  for (int k = 0; k < 3; ++k) {
-    double s, lo;
-    two_diff(px[k], d.x, s, lo);
-    nX[k] = 0;
-    if (lo != 0.0) X[k][nX[k]++] = lo;
-    if (s != 0.0 || nX[k] == 0) X[k][nX[k]++] = s;
-    two_diff(py[k], d.y, s, lo);
-    nY[k] = 0;
-    if (lo != 0.0) Y[k][nY[k]++] = lo;
-    if (s != 0.0 || nY[k] == 0) Y[k][nY[k]++] = s;
-  }
-  acc[0] = 0.0;
-  int na = 1;
-  for (int k = 0; k < 3; ++k) {
-    const int i = (k + 1) % 3, j = (k + 2) % 3;   // cofactor of row k: + (x_i y_j - y_i x_j) for k = 0, 1, 2 (cyclic)
-    double lift[16], minor[20];
-    lift[0] = 0.0;
-    int nl = 1;
-    nl = add_product(lift, nl, X[k], nX[k], X[k], nX[k], 1.0);
-    nl = add_product(lift, nl, Y[k], nY[k], Y[k], nY[k], 1.0);
-    minor[0] = 0.0;
-    int nm = 1;
-    nm = add_product(minor, nm, X[i], nX[i], Y[j], nY[j], 1.0);
-    nm = add_product(minor, nm, Y[i], nY[i], X[j], nX[j], -1.0);
-    // acc += lift * minor, through tmp so that the inner sums stay short
-    tmp[0] = 0.0;
-    int nt = 1;
-    nt = add_product(tmp, nt, lift, nl, minor, nm, 1.0);
-    na = expansion_add(acc, na, tmp, nt);
-  }
-  return sign_of(acc, na);
-}
-
-// ------------------------------------------------------------------------------------------------------------------
 // Filter kernels: the determinant in plain fp64 and a bound on its rounding error; undecided tests go to a work list
 // ------------------------------------------------------------------------------------------------------------------
-constexpr double EPS = 1.1102230246251565e-16;   // 2^-53
-
 __global__ void __launch_bounds__(256)
 orient_filter_kernel(int64_t n, const double2 *__restrict__ xy, const int32_t *__restrict__ idx, int8_t *__restrict__ sign,
                      int32_t *__restrict__ work, unsigned long long *__restrict__ n_work) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= n) return;
-  const double2 a = xy[idx[3 * k]], b = xy[idx[3 * k + 1]], c = xy[idx[3 * k + 2]];
-  const double l = __dmul_rn(__dsub_rn(a.x, c.x), __dsub_rn(b.y, c.y)), r = __dmul_rn(__dsub_rn(a.y, c.y), __dsub_rn(b.x, c.x));
-  const double det = __dsub_rn(l, r);
-  // each product carries three roundings (two differences, one product), the difference one more: |error| <= 4 eps (|l| + |r|)
-  // to first order; 8 eps covers the higher orders with a wide margin
-  const double bound = 8.0 * EPS * (fabs(l) + fabs(r));
-  if (det > bound) sign[k] = 1;
-  else if (det < -bound) sign[k] = -1;
-  else {
-    sign[k] = 2;
-    work[atomicAdd(n_work, 1ull)] = (int32_t)k;
-  }
+  const int sg = orient2d_filter(xy[idx[3 * k]], xy[idx[3 * k + 1]], xy[idx[3 * k + 2]]);
+  sign[k] = (int8_t)sg;
+  if (sg == 2) work[atomicAdd(n_work, 1ull)] = (int32_t)k;
 }
 __global__ void orient_exact_kernel(const unsigned long long *__restrict__ n_work, const int32_t *__restrict__ work,
                                     const double2 *__restrict__ xy, const int32_t *__restrict__ idx, int8_t *__restrict__ sign) {
@@ -213,22 +91,9 @@ incircle_filter_kernel(int64_t n, const double2 *__restrict__ xy, const int32_t 
                        int32_t *__restrict__ work, unsigned long long *__restrict__ n_work) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= n) return;
-  const double2 a = xy[idx[4 * k]], b = xy[idx[4 * k + 1]], c = xy[idx[4 * k + 2]], d = xy[idx[4 * k + 3]];
-  const double ax = a.x - d.x, ay = a.y - d.y, bx = b.x - d.x, by = b.y - d.y, cx = c.x - d.x, cy = c.y - d.y;
-  const double al = ax * ax + ay * ay, bl = bx * bx + by * by, cl = cx * cx + cy * cy;
-  const double bc1 = bx * cy, bc2 = by * cx, ca1 = cx * ay, ca2 = cy * ax, ab1 = ax * by, ab2 = ay * bx;
-  const double det = al * (bc1 - bc2) + bl * (ca1 - ca2) + cl * (ab1 - ab2);
-  // every one of the six monomial groups lift * product goes through at most 9 roundings (a difference, a square or product,
-  // the sums, the final products and additions); |error| <= 10 eps * permanent to first order, 16 eps with margin
-  // (whatever contraction into FMAs the compiler applies only removes roundings)
-  const double perm = al * (fabs(bc1) + fabs(bc2)) + bl * (fabs(ca1) + fabs(ca2)) + cl * (fabs(ab1) + fabs(ab2));
-  const double bound = 16.0 * EPS * perm;
-  if (det > bound) sign[k] = 1;
-  else if (det < -bound) sign[k] = -1;
-  else {
-    sign[k] = 2;
-    work[atomicAdd(n_work, 1ull)] = (int32_t)k;
-  }
+  const int sg = incircle2d_filter(xy[idx[4 * k]], xy[idx[4 * k + 1]], xy[idx[4 * k + 2]], xy[idx[4 * k + 3]]);
+  sign[k] = (int8_t)sg;
+  if (sg == 2) work[atomicAdd(n_work, 1ull)] = (int32_t)k;
 }
 __global__ void __launch_bounds__(32)
 incircle_exact_kernel(const unsigned long long *__restrict__ n_work, const int32_t *__restrict__ work, const double2 *__restrict__ xy,
@@ -240,6 +105,183 @@ incircle_exact_kernel(const unsigned long long *__restrict__ n_work, const int32
     const int64_t k = work[q];
     sign[k] = (int8_t)incircle2d_exact(xy[idx[4 * k]], xy[idx[4 * k + 1]], xy[idx[4 * k + 2]], xy[idx[4 * k + 3]], acc, tmp);
   }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Mesh data structure (section 4.1.2): triangleEdges and edgeTriangles from triangleVertices
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+edge_keys_kernel(int64_t n, const int32_t *__restrict__ tv, unsigned long long *__restrict__ key, int32_t *__restrict__ val) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int64_t t = i / 3;
+  const int k = (int)(i - 3 * t);
+  const unsigned a = (unsigned)tv[3 * t + (k + 1) % 3], b = (unsigned)tv[3 * t + (k + 2) % 3];   // edge k is opposite local vertex k
+  key[i] = ((unsigned long long)min(a, b) << 32) | max(a, b);
+  val[i] = (int32_t)i;
+}
+__global__ void __launch_bounds__(256)
+edge_heads_kernel(int64_t n, const unsigned long long *__restrict__ key, int32_t *__restrict__ head) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) head[i] = (i == 0 || key[i] != key[i - 1]) ? 1 : 0;
+}
+// incl = inclusive sum of head: sorted entry i belongs to edge incl[i] - 1
+__global__ void __launch_bounds__(256)
+edge_fill_kernel(int64_t n, const unsigned long long *__restrict__ key, const int32_t *__restrict__ val, const int32_t *__restrict__ incl,
+                 int32_t *__restrict__ te, int32_t *__restrict__ et, int *__restrict__ err) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int32_t e = incl[i] - 1;
+  const int slot = (i > 0 && key[i] == key[i - 1]) ? 1 : 0;
+  if (i > 1 && key[i] == key[i - 2]) { *err = 1; return; }      // an edge with three triangles
+  te[val[i]] = e;
+  et[2 * (int64_t)e + slot] = val[i] / 3;                        // (the sort is stable: ascending triangle order)
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Delaunay triangulator (section 2.4.6, 4.1.5)
+// ------------------------------------------------------------------------------------------------------------------
+struct FlipCounters { unsigned long long n_work, n_bad, n_flip, n_next, n_exact; };
+
+struct Quad { int32_t t1, t2; double2 a, b, c, d; };
+static __device__ __forceinline__ bool load_quad(int32_t e, const double2 *xy, const int32_t *tv, const int32_t *te, const int32_t *et, Quad &q) {
+  q.t1 = et[2 * (int64_t)e];
+  q.t2 = et[2 * (int64_t)e + 1];
+  if (q.t2 < 0) return false;                                    // a boundary edge: Delaunay by definition
+  const int32_t *e2 = te + 3 * (int64_t)q.t2;
+  const int k2 = e2[0] == e ? 0 : (e2[1] == e ? 1 : 2);
+  const int32_t *v1 = tv + 3 * (int64_t)q.t1;
+  q.a = xy[v1[0]]; q.b = xy[v1[1]]; q.c = xy[v1[2]];
+  q.d = xy[tv[3 * (int64_t)q.t2 + k2]];                          // "the one vertex of T' that is not part of T" (L192)
+  return true;
+}
+// E is not Delaunay: note it and bid for its two triangles (independent set of section 4.1.5: the higher edge number wins;
+// the iteration stamp in the upper half outbids every bid of an earlier iteration, so the locks are never reset)
+static __device__ __forceinline__ void mark_bad(int32_t e, const Quad &q, unsigned long long stamp, int8_t *state,
+                                                unsigned long long *lock, FlipCounters *c) {
+  state[e] = 1;
+  atomicMax(lock + q.t1, stamp | (unsigned)e);
+  atomicMax(lock + q.t2, stamp | (unsigned)e);
+  atomicAdd(&c->n_bad, 1ull);
+}
+__global__ void __launch_bounds__(256)
+check_edge_kernel(int64_t n, const int32_t *__restrict__ cand, const double2 *__restrict__ xy, const int32_t *__restrict__ tv,
+                  const int32_t *__restrict__ te, const int32_t *__restrict__ et, int8_t *__restrict__ state,
+                  unsigned long long *__restrict__ lock, unsigned long long stamp, int32_t *__restrict__ work, FlipCounters *c) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int32_t e = cand ? cand[i] : (int32_t)i;
+  Quad q;
+  if (!load_quad(e, xy, tv, te, et, q)) { state[e] = 0; return; }
+  const int sg = incircle2d_filter(q.a, q.b, q.c, q.d);
+  if (sg == 2) work[atomicAdd(&c->n_work, 1ull)] = e;
+  else if (sg == 1) mark_bad(e, q, stamp, state, lock, c);
+  else state[e] = 0;
+}
+__global__ void __launch_bounds__(32)
+check_edge_exact_kernel(const int32_t *__restrict__ work, const double2 *__restrict__ xy, const int32_t *__restrict__ tv,
+                        const int32_t *__restrict__ te, const int32_t *__restrict__ et, int8_t *__restrict__ state,
+                        unsigned long long *__restrict__ lock, unsigned long long stamp, FlipCounters *c, double *__restrict__ scratch) {
+  const int64_t nw = (int64_t)c->n_work;
+  const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  double *acc = scratch + tid * (2 * MAXE), *tmp = acc + MAXE;
+  for (int64_t w = tid; w < nw; w += (int64_t)gridDim.x * blockDim.x) {
+    const int32_t e = work[w];
+    Quad q;
+    load_quad(e, xy, tv, te, et, q);
+    if (incircle2d_exact(q.a, q.b, q.c, q.d, acc, tmp) > 0) mark_bad(e, q, stamp, state, lock, c);
+    else state[e] = 0;                                           // zero: four cocircular vertices, left alone
+  }
+  if (tid == 0) c->n_exact += (unsigned long long)nw;
+}
+// candidate for the next iteration, once
+static __device__ __forceinline__ void push_next(int32_t f, int32_t iter, int32_t *mark, int32_t *next, FlipCounters *c) {
+  if (atomicExch(mark + f, iter) != iter) next[atomicAdd(&c->n_next, 1ull)] = f;
+}
+__global__ void __launch_bounds__(256)
+flip_kernel(int64_t n, const int32_t *__restrict__ cand, int32_t *__restrict__ tv, int32_t *__restrict__ te, int32_t *__restrict__ et,
+            int8_t *__restrict__ state, const unsigned long long *__restrict__ lock, unsigned long long stamp, int32_t iter,
+            int32_t *__restrict__ mark, int32_t *__restrict__ next, FlipCounters *c) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int32_t e = cand ? cand[i] : (int32_t)i;
+  if (state[e] != 1) return;
+  const int32_t t1 = et[2 * (int64_t)e], t2 = et[2 * (int64_t)e + 1];
+  const unsigned long long mine = stamp | (unsigned)e;
+  if (lock[t1] != mine || lock[t2] != mine) {                    // lost a triangle to another edge: try again next iteration
+    push_next(e, iter, mark, next, c);
+    return;
+  }
+  // flip (L102): a opposite E in t1 = (a, b, c), d opposite E in t2 = (d, c, b)  ->  t1 = (a, b, d), t2 = (a, d, c)
+  int32_t *v1 = tv + 3 * (int64_t)t1, *v2 = tv + 3 * (int64_t)t2, *e1 = te + 3 * (int64_t)t1, *e2 = te + 3 * (int64_t)t2;
+  const int i1 = e1[0] == e ? 0 : (e1[1] == e ? 1 : 2), i2 = e2[0] == e ? 0 : (e2[1] == e ? 1 : 2);
+  const int32_t a = v1[i1], b = v1[(i1 + 1) % 3], cc = v1[(i1 + 2) % 3], d = v2[i2];
+  const int32_t e_ca = e1[(i1 + 1) % 3], e_ab = e1[(i1 + 2) % 3], e_bd = e2[(i2 + 1) % 3], e_dc = e2[(i2 + 2) % 3];
+  v1[0] = a; v1[1] = b; v1[2] = d;
+  e1[0] = e_bd; e1[1] = e; e1[2] = e_ab;
+  v2[0] = a; v2[1] = d; v2[2] = cc;
+  e2[0] = e_dc; e2[1] = e_ca; e2[2] = e;
+  // repair edgeTriangles of the two edges that changed sides (section 4.1.5; in place: every thread rewrites only the entry
+  // that names one of ITS two triangles, which no other flip of this iteration can name)
+  int32_t *f = et + 2 * (int64_t)e_bd;
+  f[f[0] == t2 ? 0 : 1] = t1;
+  f = et + 2 * (int64_t)e_ca;
+  f[f[0] == t1 ? 0 : 1] = t2;
+  state[e] = 0;                                                  // "E' would be locally Delaunay" (L102)
+  push_next(e_ca, iter, mark, next, c);
+  push_next(e_ab, iter, mark, next, c);
+  push_next(e_bd, iter, mark, next, c);
+  push_next(e_dc, iter, mark, next, c);
+  atomicAdd(&c->n_flip, 1ull);
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Point location (section 2.4.2)
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+find_triangle_kernel(int64_t np, const double2 *__restrict__ p, const int32_t *__restrict__ t0, int64_t max_steps,
+                     const double2 *__restrict__ xy, const int32_t *__restrict__ tv, const int32_t *__restrict__ te,
+                     const int32_t *__restrict__ et, int32_t *__restrict__ t_out, int8_t *__restrict__ code_out, int *__restrict__ err) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= np) return;
+  const double2 P = p[i];
+  int32_t t = t0[i];
+  for (int64_t step = 0; step < max_steps; ++step) {
+    const int32_t *v = tv + 3 * (int64_t)t;
+    const double2 A = xy[v[0]], B = xy[v[1]], C = xy[v[2]];
+    // the edge (a, b) is opposite local vertex 2, (b, c) opposite 0, (c, a) opposite 1; cross the first with p strictly outside
+    int s[3];
+    int out = -1;
+    s[0] = orient2d_sign(A, B, P);
+    if (s[0] < 0) out = 2;
+    else {
+      s[1] = orient2d_sign(B, C, P);
+      if (s[1] < 0) out = 0;
+      else {
+        s[2] = orient2d_sign(C, A, P);
+        if (s[2] < 0) out = 1;
+      }
+    }
+    if (out < 0) {
+      const int z0 = s[0] == 0, z1 = s[1] == 0, z2 = s[2] == 0;
+      int code = 0;
+      if (z0 + z1 + z2 == 1) code = 1 + (z0 ? 2 : (z1 ? 0 : 1));
+      else if (z0 + z1 + z2 >= 2) code = 4 + ((z0 && z1) ? 1 : ((z1 && z2) ? 2 : 0));   // the vertex the two edges share
+      t_out[i] = t;
+      code_out[i] = (int8_t)code;
+      return;
+    }
+    const int32_t e = te[3 * (int64_t)t + out];
+    const int32_t n0 = et[2 * (int64_t)e], n1 = et[2 * (int64_t)e + 1];
+    const int32_t nxt = n0 != t ? n0 : n1;
+    if (nxt < 0) {
+      t_out[i] = -1 - t;
+      code_out[i] = 0;
+      return;
+    }
+    t = nxt;
+  }
+  *err = 1;
 }
 
 }  // namespace mrdgen
@@ -320,6 +362,144 @@ int mrd_meshgen_orient2d(int64_t n, const double *xy_dev, const int32_t *idx_dev
 }
 int mrd_meshgen_incircle2d(int64_t n, const double *xy_dev, const int32_t *idx_dev, int8_t *sign_dev, int64_t *n_exact, void *stream) {
   return predicate_impl(1, n, xy_dev, idx_dev, sign_dev, n_exact, stream);
+}
+
+int mrd_meshgen_build_edges(int64_t n_triangle, const int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_edge, void *stream) {
+  if (n_triangle < 0 || !n_edge || (n_triangle > 0 && (!tv_dev || !te_dev || !et_dev))) return gen_fail(MRD_EINVAL, "null argument");
+  if (3 * n_triangle > 0x7FFFFFF0ll) return gen_fail(MRD_EINVAL, "too many triangles for 32-bit edge numbers");
+  *n_edge = 0;
+  if (n_triangle == 0) return MRD_OK;
+  cudaStream_t s = (cudaStream_t)stream;
+  const int64_t n = 3 * n_triangle;
+  unsigned long long *key[2] = {nullptr, nullptr};
+  int32_t *val[2] = {nullptr, nullptr}, *head = nullptr, *incl = nullptr;
+  int *err = nullptr;
+  void *tmp = nullptr;
+  size_t tmp_sort = 0, tmp_scan = 0;
+  cub::DeviceRadixSort::SortPairs(nullptr, tmp_sort, key[0], key[1], val[0], val[1], n, 0, 64, s);
+  cub::DeviceScan::InclusiveSum(nullptr, tmp_scan, head, incl, n, s);
+  cudaError_t e = cudaSuccess;
+  auto alloc = [&](void **p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
+  for (int j = 0; j < 2; ++j) {
+    alloc((void **)&key[j], sizeof(unsigned long long) * n);
+    alloc((void **)&val[j], sizeof(int32_t) * n);
+  }
+  alloc((void **)&head, sizeof(int32_t) * n);
+  alloc((void **)&incl, sizeof(int32_t) * n);
+  alloc((void **)&err, sizeof(int));
+  alloc(&tmp, std::max(tmp_sort, tmp_scan));
+  int h_err = 0;
+  int32_t h_ne = 0;
+  if (e == cudaSuccess) {
+    const unsigned nb = (unsigned)((n + 255) / 256);
+    cudaMemsetAsync(err, 0, sizeof(int), s);
+    cudaMemsetAsync(et_dev, 0xFF, sizeof(int32_t) * 2 * (size_t)n, s);   // -1: no second triangle
+    mrdgen::edge_keys_kernel<<<nb, 256, 0, s>>>(n, tv_dev, key[0], val[0]);
+    cub::DeviceRadixSort::SortPairs(tmp, tmp_sort, key[0], key[1], val[0], val[1], n, 0, 64, s);
+    mrdgen::edge_heads_kernel<<<nb, 256, 0, s>>>(n, key[1], head);
+    cub::DeviceScan::InclusiveSum(tmp, tmp_scan, head, incl, n, s);
+    mrdgen::edge_fill_kernel<<<nb, 256, 0, s>>>(n, key[1], val[1], incl, te_dev, et_dev, err);
+    cudaMemcpyAsync(&h_err, err, sizeof(int), cudaMemcpyDeviceToHost, s);
+    cudaMemcpyAsync(&h_ne, incl + (n - 1), sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+    e = cudaStreamSynchronize(s);
+    if (e == cudaSuccess) e = cudaGetLastError();
+  }
+  for (int j = 0; j < 2; ++j) { cudaFree(key[j]); cudaFree(val[j]); }
+  cudaFree(head); cudaFree(incl); cudaFree(err); cudaFree(tmp);
+  if (e != cudaSuccess) return gen_fail(e == cudaErrorMemoryAllocation ? MRD_ENOMEM : MRD_ECUDA, std::string("build_edges: ") + cudaGetErrorString(e));
+  if (h_err) return gen_fail(MRD_EINVAL, "build_edges: an edge belongs to more than two triangles");
+  *n_edge = h_ne;
+  return MRD_OK;
+}
+
+int mrd_meshgen_delaunay_flip(int64_t n_triangle, int64_t n_edge, const double *xy_dev, int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev,
+                              int64_t *n_flips, int64_t *n_iterations, int64_t *n_exact, void *stream) {
+  if (n_triangle < 0 || n_edge < 0 || ((n_triangle > 0 || n_edge > 0) && (!xy_dev || !tv_dev || !te_dev || !et_dev)))
+    return gen_fail(MRD_EINVAL, "null argument");
+  if (n_edge > 0x7FFFFFF0ll) return gen_fail(MRD_EINVAL, "too many edges");
+  if (n_flips) *n_flips = 0;
+  if (n_iterations) *n_iterations = 0;
+  if (n_exact) *n_exact = 0;
+  if (n_edge == 0) return MRD_OK;
+  using mrdgen::FlipCounters;
+  cudaStream_t s = (cudaStream_t)stream;
+  const int exact_blocks = 148 * 4, exact_threads = 32;
+  int8_t *state = nullptr;
+  unsigned long long *lock = nullptr;
+  int32_t *mark = nullptr, *list[2] = {nullptr, nullptr}, *work = nullptr;
+  FlipCounters *cnt = nullptr;
+  double *scratch = nullptr;
+  cudaError_t e = cudaSuccess;
+  auto alloc = [&](void **p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
+  alloc((void **)&state, (size_t)n_edge);
+  alloc((void **)&lock, sizeof(unsigned long long) * (size_t)std::max<int64_t>(n_triangle, 1));
+  alloc((void **)&mark, sizeof(int32_t) * (size_t)n_edge);
+  alloc((void **)&list[0], sizeof(int32_t) * (size_t)n_edge);
+  alloc((void **)&list[1], sizeof(int32_t) * (size_t)n_edge);
+  alloc((void **)&work, sizeof(int32_t) * (size_t)n_edge);
+  alloc((void **)&cnt, sizeof(FlipCounters));
+  alloc((void **)&scratch, sizeof(double) * 2 * mrdgen::MAXE * (size_t)exact_blocks * exact_threads);
+  int64_t flips = 0, iters = 0, exact = 0;
+  int rc = MRD_OK;
+  if (e == cudaSuccess) {
+    cudaMemsetAsync(state, 0, (size_t)n_edge, s);
+    cudaMemsetAsync(lock, 0, sizeof(unsigned long long) * (size_t)std::max<int64_t>(n_triangle, 1), s);
+    cudaMemsetAsync(mark, 0, sizeof(int32_t) * (size_t)n_edge, s);
+    int64_t n = n_edge;
+    const int32_t *cand = nullptr;                               // first iteration: every edge
+    const double2 *xy = (const double2 *)xy_dev;
+    for (int32_t iter = 1;; ++iter) {
+      if (iter > 100000) { rc = gen_fail(MRD_EINVAL, "delaunay_flip: no convergence (is the input a valid triangulation?)"); break; }
+      const unsigned long long stamp = (unsigned long long)iter << 32;
+      int32_t *next = list[iter & 1];
+      const unsigned nb = (unsigned)((n + 255) / 256);
+      cudaMemsetAsync(cnt, 0, sizeof(FlipCounters), s);
+      mrdgen::check_edge_kernel<<<nb, 256, 0, s>>>(n, cand, xy, tv_dev, te_dev, et_dev, state, lock, stamp, work, cnt);
+      mrdgen::check_edge_exact_kernel<<<exact_blocks, exact_threads, 0, s>>>(work, xy, tv_dev, te_dev, et_dev, state, lock, stamp, cnt, scratch);
+      mrdgen::flip_kernel<<<nb, 256, 0, s>>>(n, cand, tv_dev, te_dev, et_dev, state, lock, stamp, iter, mark, next, cnt);
+      FlipCounters h;
+      e = cudaMemcpyAsync(&h, cnt, sizeof h, cudaMemcpyDeviceToHost, s);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+      if (e == cudaSuccess) e = cudaGetLastError();
+      if (e != cudaSuccess) break;
+      iters++;
+      flips += (int64_t)h.n_flip;
+      exact += (int64_t)h.n_exact;
+      if (h.n_bad == 0) break;                                   // every edge is locally Delaunay
+      cand = next;
+      n = (int64_t)h.n_next;
+    }
+  }
+  cudaFree(state); cudaFree(lock); cudaFree(mark); cudaFree(list[0]); cudaFree(list[1]); cudaFree(work); cudaFree(cnt); cudaFree(scratch);
+  if (e != cudaSuccess) return gen_fail(e == cudaErrorMemoryAllocation ? MRD_ENOMEM : MRD_ECUDA, std::string("delaunay_flip: ") + cudaGetErrorString(e));
+  if (rc != MRD_OK) return rc;
+  if (n_flips) *n_flips = flips;
+  if (n_iterations) *n_iterations = iters;
+  if (n_exact) *n_exact = exact;
+  return MRD_OK;
+}
+
+int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_t *t0_dev, int64_t n_triangle, const double *xy_dev,
+                              const int32_t *tv_dev, const int32_t *te_dev, const int32_t *et_dev, int32_t *t_dev, int8_t *code_dev,
+                              void *stream) {
+  if (n_point < 0 || n_triangle < 0 || (n_point > 0 && (!p_dev || !t0_dev || !xy_dev || !tv_dev || !te_dev || !et_dev || !t_dev || !code_dev)))
+    return gen_fail(MRD_EINVAL, "null argument");
+  if (n_point == 0) return MRD_OK;
+  if (n_triangle == 0) return gen_fail(MRD_EINVAL, "find_triangle: empty triangulation");
+  cudaStream_t s = (cudaStream_t)stream;
+  int *err = nullptr;
+  GEN_TRY(cudaMalloc(&err, sizeof(int)));
+  cudaMemsetAsync(err, 0, sizeof(int), s);
+  mrdgen::find_triangle_kernel<<<(unsigned)((n_point + 127) / 128), 128, 0, s>>>(n_point, (const double2 *)p_dev, t0_dev, n_triangle + 16,
+                                                                                   (const double2 *)xy_dev, tv_dev, te_dev, et_dev, t_dev, code_dev, err);
+  int h = 0;
+  cudaError_t e = cudaMemcpyAsync(&h, err, sizeof(int), cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaFree(err);
+  if (e != cudaSuccess) return gen_fail(MRD_ECUDA, std::string("find_triangle: ") + cudaGetErrorString(e));
+  if (h) return gen_fail(MRD_EINVAL, "find_triangle: a walk did not end (not a Delaunay triangulation, or a start triangle out of range)");
+  return MRD_OK;
 }
 
 }  // extern "C"

@@ -10,11 +10,8 @@ import workloads as wl
 from oracle import meshgen as mg
 
 
-def scrambled(nx, ny, seed, amplitude=0.25, rounds=3):
-    """A valid but far-from-Delaunay triangulation of points in general position inside a rectangle: jittered grid (boundary
-    vertices slide along the boundary, so the hull stays the rectangle), then seeded random flips of convex quadrilaterals."""
-    m = wl.jitter_mesh(wl.uniform_mesh(nx, ny, 2.0, 1.5, periodic=False), amplitude, seed=seed)
-    m = wl.flip_edges(m, fraction=0.5, seed=seed + 1, rounds=rounds)
+def scrambled(nx, ny, seed):
+    m = wl.scrambled_triangulation(nx, ny, seed)
     return m.xy, m.tri.astype(np.int32)
 
 

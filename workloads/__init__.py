@@ -13,6 +13,7 @@ from .meshes import (  # noqa: F401
     morton_order_mesh,
     jitter_mesh,
     flip_edges,
+    scrambled_triangulation,
     delaunay_mesh,
     uniform_strip_part,
     read_triangle_files,

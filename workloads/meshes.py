@@ -190,6 +190,16 @@ def flip_edges(mesh: UniformMesh, fraction: float = 0.35, seed: int = 11, rounds
     return replace(mesh, tri=np.ascontiguousarray(tri.astype(np.int32)))
 
 
+def scrambled_triangulation(ncx: int, ncy: int, seed: int = 1, amplitude: float = 0.25, rounds: int = 3, Lx: float = 2.0,
+                            Ly: float = 1.5) -> UniformMesh:
+    """Input of the Delaunay triangulator (section 2.4.6): a VALID but far-from-Delaunay triangulation of points in
+    general position inside a rectangle -- a jittered ncx x ncy-cell grid (boundary vertices slide along the boundary, so the
+    hull stays the rectangle and the Delaunay triangulation of the points is the triangulation of the domain), then `rounds`
+    rounds of seeded flips of strictly convex quadrilaterals (every second edge a candidate)."""
+    m = jitter_mesh(uniform_mesh(ncx, ncy, Lx, Ly, periodic=False), amplitude, seed=seed)
+    return flip_edges(m, fraction=0.5, seed=seed + 1, rounds=rounds)
+
+
 def boundary_vertices(mesh: UniformMesh, x_ends: bool = True, y_ends: bool = True) -> np.ndarray:
     """uint8 [nv] flag: 1 on the requested boundary rows/columns of a bounded mesh (PAPER.md L582:
     boundary vertices promoted to ghost vertices that keep the initial condition)."""
