@@ -331,8 +331,12 @@ int mrd_meshgen_incircle2d(int64_t n, const double *xy_dev, const int32_t *idx_d
  *   eq. 3).  t[i] >= 0: found, with code[i] = 0 strictly inside, 1 + k on edge k of t, 4 + k on local vertex k (L168);
  *   t[i] = -1 - t_last: the walk left the triangulation through a boundary edge of t_last.  The walk terminates on Delaunay
  *   triangulations; MRD_EINVAL if a walk exceeds n_triangle + 16 steps (not a Delaunay triangulation).
+ * Work space: the mrd_meshgen_* calls keep one device block (grown on demand; ~200 MB for the scratch of the exact
+ *   predicates plus ~40 B per edge) and a small pinned host block between calls, because allocating them costs more than the
+ *   kernels; calls are serialised by a lock.  mrd_meshgen_release frees both (they come back on the next call).
  * Errors: MRD_EINVAL (null pointer, inconsistent structure), MRD_ENOMEM, MRD_ECUDA.
  * ---------------------------------------------------------------------------------------------- */
+int mrd_meshgen_release(void);
 int mrd_meshgen_build_edges(int64_t n_triangle, const int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_edge,
                             void *stream);
 int mrd_meshgen_delaunay_flip(int64_t n_triangle, int64_t n_edge, const double *xy_dev, int32_t *tv_dev, int32_t *te_dev,

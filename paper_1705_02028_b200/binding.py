@@ -87,6 +87,7 @@ def lib():
         L.mrd_meshgen_test_quality.argtypes = [C.c_int64, vp, vp, C.c_double, C.c_double, vp, vp, vp, vp, _lp, vp]
         L.mrd_meshgen_orient2d.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
         L.mrd_meshgen_incircle2d.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
+        L.mrd_meshgen_release.argtypes = []
         L.mrd_meshgen_build_edges.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
         L.mrd_meshgen_delaunay_flip.argtypes = [C.c_int64, C.c_int64, vp, vp, vp, vp, _lp, _lp, _lp, vp]
         L.mrd_meshgen_find_triangle.argtypes = [C.c_int64, vp, vp, C.c_int64, vp, vp, vp, vp, vp, vp, vp]
@@ -496,3 +497,8 @@ def meshgen_find_triangle(xy, tv, te, et, p, t0, stream=None):
                                            _dev(tv, torch.int32, 3), _dev(te, torch.int32, 3), _dev(et, torch.int32, 2),
                                            C.c_void_p(t.data_ptr()), C.c_void_p(code.data_ptr()), _stream_ptr(stream)))
     return t, code
+
+
+def meshgen_release():
+    """Free the work space the mrd_meshgen_* calls keep between calls."""
+    _check(lib().mrd_meshgen_release())

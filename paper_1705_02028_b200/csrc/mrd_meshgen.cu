@@ -19,6 +19,7 @@
 #include <cstdint>
 #include <cub/device/device_radix_sort.cuh>
 #include <cub/device/device_scan.cuh>
+#include <mutex>
 #include <string>
 
 #include "../../include/mrd.h"
@@ -157,26 +158,31 @@ static __device__ __forceinline__ bool load_quad(int32_t e, const double2 *xy, c
 }
 // E is not Delaunay: note it and bid for its two triangles (independent set of section 4.1.5: the higher edge number wins;
 // the iteration stamp in the upper half outbids every bid of an earlier iteration, so the locks are never reset)
-static __device__ __forceinline__ void mark_bad(int32_t e, const Quad &q, unsigned long long stamp, int8_t *state,
-                                                unsigned long long *lock, FlipCounters *c) {
+static __device__ __forceinline__ void bid(int32_t e, const Quad &q, unsigned long long stamp, int8_t *state, unsigned long long *lock) {
   state[e] = 1;
   atomicMax(lock + q.t1, stamp | (unsigned)e);
   atomicMax(lock + q.t2, stamp | (unsigned)e);
-  atomicAdd(&c->n_bad, 1ull);
 }
+// (counters: one atomic per warp, not per thread -- millions of increments of one address serialise in L2)
 __global__ void __launch_bounds__(256)
 check_edge_kernel(int64_t n, const int32_t *__restrict__ cand, const double2 *__restrict__ xy, const int32_t *__restrict__ tv,
                   const int32_t *__restrict__ te, const int32_t *__restrict__ et, int8_t *__restrict__ state,
                   unsigned long long *__restrict__ lock, unsigned long long stamp, int32_t *__restrict__ work, FlipCounters *c) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const int32_t e = cand ? cand[i] : (int32_t)i;
-  Quad q;
-  if (!load_quad(e, xy, tv, te, et, q)) { state[e] = 0; return; }
-  const int sg = incircle2d_filter(q.a, q.b, q.c, q.d);
-  if (sg == 2) work[atomicAdd(&c->n_work, 1ull)] = e;
-  else if (sg == 1) mark_bad(e, q, stamp, state, lock, c);
-  else state[e] = 0;
+  bool bad = false;
+  if (i < n) {
+    const int32_t e = cand ? cand[i] : (int32_t)i;
+    Quad q;
+    if (!load_quad(e, xy, tv, te, et, q)) state[e] = 0;
+    else {
+      const int sg = incircle2d_filter(q.a, q.b, q.c, q.d);
+      if (sg == 2) work[atomicAdd(&c->n_work, 1ull)] = e;          // rare
+      else if (sg == 1) { bid(e, q, stamp, state, lock); bad = true; }
+      else state[e] = 0;
+    }
+  }
+  const unsigned m = __ballot_sync(0xFFFFFFFFu, bad);
+  if ((threadIdx.x & 31) == 0 && m) atomicAdd(&c->n_bad, (unsigned long long)__popc(m));
 }
 __global__ void __launch_bounds__(32)
 check_edge_exact_kernel(const int32_t *__restrict__ work, const double2 *__restrict__ xy, const int32_t *__restrict__ tv,
@@ -189,50 +195,66 @@ check_edge_exact_kernel(const int32_t *__restrict__ work, const double2 *__restr
     const int32_t e = work[w];
     Quad q;
     load_quad(e, xy, tv, te, et, q);
-    if (incircle2d_exact(q.a, q.b, q.c, q.d, acc, tmp) > 0) mark_bad(e, q, stamp, state, lock, c);
-    else state[e] = 0;                                           // zero: four cocircular vertices, left alone
+    if (incircle2d_exact(q.a, q.b, q.c, q.d, acc, tmp) > 0) {
+      bid(e, q, stamp, state, lock);
+      atomicAdd(&c->n_bad, 1ull);
+    } else state[e] = 0;                                         // zero: four cocircular vertices, left alone
   }
   if (tid == 0) c->n_exact += (unsigned long long)nw;
-}
-// candidate for the next iteration, once
-static __device__ __forceinline__ void push_next(int32_t f, int32_t iter, int32_t *mark, int32_t *next, FlipCounters *c) {
-  if (atomicExch(mark + f, iter) != iter) next[atomicAdd(&c->n_next, 1ull)] = f;
 }
 __global__ void __launch_bounds__(256)
 flip_kernel(int64_t n, const int32_t *__restrict__ cand, int32_t *__restrict__ tv, int32_t *__restrict__ te, int32_t *__restrict__ et,
             int8_t *__restrict__ state, const unsigned long long *__restrict__ lock, unsigned long long stamp, int32_t iter,
             int32_t *__restrict__ mark, int32_t *__restrict__ next, FlipCounters *c) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const int32_t e = cand ? cand[i] : (int32_t)i;
-  if (state[e] != 1) return;
-  const int32_t t1 = et[2 * (int64_t)e], t2 = et[2 * (int64_t)e + 1];
-  const unsigned long long mine = stamp | (unsigned)e;
-  if (lock[t1] != mine || lock[t2] != mine) {                    // lost a triangle to another edge: try again next iteration
-    push_next(e, iter, mark, next, c);
-    return;
+  int32_t items[4];                                              // this thread's candidates for the next iteration
+  int cnt = 0;
+  bool flipped = false;
+  const int32_t e = i < n ? (cand ? cand[i] : (int32_t)i) : -1;
+  if (e >= 0 && state[e] == 1) {
+    const int32_t t1 = et[2 * (int64_t)e], t2 = et[2 * (int64_t)e + 1];
+    const unsigned long long mine = stamp | (unsigned)e;
+    if (lock[t1] != mine || lock[t2] != mine) {                  // lost a triangle to another edge: try again next iteration
+      if (atomicExch(mark + e, iter) != iter) items[cnt++] = e;
+    } else {
+      // flip (L102): a opposite E in t1 = (a, b, c), d opposite E in t2 = (d, c, b)  ->  t1 = (a, b, d), t2 = (a, d, c)
+      int32_t *v1 = tv + 3 * (int64_t)t1, *v2 = tv + 3 * (int64_t)t2, *e1 = te + 3 * (int64_t)t1, *e2 = te + 3 * (int64_t)t2;
+      const int i1 = e1[0] == e ? 0 : (e1[1] == e ? 1 : 2), i2 = e2[0] == e ? 0 : (e2[1] == e ? 1 : 2);
+      const int32_t a = v1[i1], b = v1[(i1 + 1) % 3], cc = v1[(i1 + 2) % 3], d = v2[i2];
+      const int32_t e_ca = e1[(i1 + 1) % 3], e_ab = e1[(i1 + 2) % 3], e_bd = e2[(i2 + 1) % 3], e_dc = e2[(i2 + 2) % 3];
+      v1[0] = a; v1[1] = b; v1[2] = d;
+      e1[0] = e_bd; e1[1] = e; e1[2] = e_ab;
+      v2[0] = a; v2[1] = d; v2[2] = cc;
+      e2[0] = e_dc; e2[1] = e_ca; e2[2] = e;
+      // repair edgeTriangles of the two edges that changed sides (section 4.1.5; in place: every thread rewrites only the
+      // entry that names one of ITS two triangles, which no other flip of this iteration can name)
+      int32_t *f = et + 2 * (int64_t)e_bd;
+      f[f[0] == t2 ? 0 : 1] = t1;
+      f = et + 2 * (int64_t)e_ca;
+      f[f[0] == t1 ? 0 : 1] = t2;
+      state[e] = 0;                                              // "E' would be locally Delaunay" (L102)
+      const int32_t outer[4] = {e_ca, e_ab, e_bd, e_dc};         // their quadrilaterals changed: check them next
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        if (atomicExch(mark + outer[j], iter) != iter) items[cnt++] = outer[j];
+      flipped = true;
+    }
   }
-  // flip (L102): a opposite E in t1 = (a, b, c), d opposite E in t2 = (d, c, b)  ->  t1 = (a, b, d), t2 = (a, d, c)
-  int32_t *v1 = tv + 3 * (int64_t)t1, *v2 = tv + 3 * (int64_t)t2, *e1 = te + 3 * (int64_t)t1, *e2 = te + 3 * (int64_t)t2;
-  const int i1 = e1[0] == e ? 0 : (e1[1] == e ? 1 : 2), i2 = e2[0] == e ? 0 : (e2[1] == e ? 1 : 2);
-  const int32_t a = v1[i1], b = v1[(i1 + 1) % 3], cc = v1[(i1 + 2) % 3], d = v2[i2];
-  const int32_t e_ca = e1[(i1 + 1) % 3], e_ab = e1[(i1 + 2) % 3], e_bd = e2[(i2 + 1) % 3], e_dc = e2[(i2 + 2) % 3];
-  v1[0] = a; v1[1] = b; v1[2] = d;
-  e1[0] = e_bd; e1[1] = e; e1[2] = e_ab;
-  v2[0] = a; v2[1] = d; v2[2] = cc;
-  e2[0] = e_dc; e2[1] = e_ca; e2[2] = e;
-  // repair edgeTriangles of the two edges that changed sides (section 4.1.5; in place: every thread rewrites only the entry
-  // that names one of ITS two triangles, which no other flip of this iteration can name)
-  int32_t *f = et + 2 * (int64_t)e_bd;
-  f[f[0] == t2 ? 0 : 1] = t1;
-  f = et + 2 * (int64_t)e_ca;
-  f[f[0] == t1 ? 0 : 1] = t2;
-  state[e] = 0;                                                  // "E' would be locally Delaunay" (L102)
-  push_next(e_ca, iter, mark, next, c);
-  push_next(e_ab, iter, mark, next, c);
-  push_next(e_bd, iter, mark, next, c);
-  push_next(e_dc, iter, mark, next, c);
-  atomicAdd(&c->n_flip, 1ull);
+  // append to the next list: warp prefix sum, one atomic per warp
+  const int lane = threadIdx.x & 31;
+  int incl = cnt;
+#pragma unroll
+  for (int dlt = 1; dlt < 32; dlt <<= 1) {
+    const int v = __shfl_up_sync(0xFFFFFFFFu, incl, dlt);
+    if (lane >= dlt) incl += v;
+  }
+  const int total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+  unsigned long long base = 0;
+  if (lane == 31 && total) base = atomicAdd(&c->n_next, (unsigned long long)total);
+  base = __shfl_sync(0xFFFFFFFFu, base, 31);
+  for (int j = 0; j < cnt; ++j) next[base + incl - cnt + j] = items[j];
+  const unsigned fm = __ballot_sync(0xFFFFFFFFu, flipped);
+  if (lane == 0 && fm) atomicAdd(&c->n_flip, (unsigned long long)__popc(fm));
 }
 
 // ------------------------------------------------------------------------------------------------------------------
@@ -293,13 +315,62 @@ int mrd_internal_set_error(int code, const char *msg);
 
 namespace {
 int gen_fail(int code, const std::string &msg) { return mrd_internal_set_error(code, msg.c_str()); }
-#define GEN_TRY(expr)                                                                                   \
-  do {                                                                                                  \
-    cudaError_t e_ = (expr);                                                                            \
-    if (e_ != cudaSuccess) return gen_fail(e_ == cudaErrorMemoryAllocation ? MRD_ENOMEM : MRD_ECUDA,    \
-                                           std::string(#expr) + ": " + cudaGetErrorString(e_));         \
-  } while (0)
+int cuda_fail(const char *what, cudaError_t e) {
+  return gen_fail(e == cudaErrorMemoryAllocation ? MRD_ENOMEM : MRD_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+// Work space kept between calls: cudaMalloc / cudaFree of the scratch arrays cost milliseconds, the kernels microseconds.
+// One block per process, grown on demand, carved up by every call (which holds the lock until it has synchronised its
+// stream); a small pinned host block receives the counters.  mrd_meshgen_release() frees both.
+struct Arena {
+  std::mutex mu;
+  int dev = -1;
+  char *base = nullptr;
+  size_t cap = 0;
+  unsigned long long *pinned = nullptr;   // 16 words
+  cudaError_t reserve(size_t bytes) {
+    int d = 0;
+    cudaError_t e = cudaGetDevice(&d);
+    if (e != cudaSuccess) return e;
+    if (d != dev || bytes > cap) {
+      if (base) cudaFree(base);
+      base = nullptr;
+      cap = 0;
+      dev = d;
+      e = cudaMalloc(&base, bytes);
+      if (e != cudaSuccess) return e;
+      cap = bytes;
+    }
+    if (!pinned) e = cudaHostAlloc(&pinned, 16 * sizeof(unsigned long long), cudaHostAllocDefault);
+    return e;
+  }
+  void release() {
+    if (base) cudaFree(base);
+    if (pinned) cudaFreeHost(pinned);
+    base = nullptr;
+    pinned = nullptr;
+    cap = 0;
+    dev = -1;
+  }
+};
+Arena g_arena;
+struct Carve {   // offsets first (so that one reserve() covers the call), pointers after
+  size_t total = 0;
+  size_t add(size_t bytes) {
+    const size_t o = total;
+    total += (bytes + 255) & ~size_t(255);
+    return o;
+  }
+};
+constexpr int EXACT_BLOCKS = 148 * 2, EXACT_THREADS = 32;
+constexpr size_t EXACT_SCRATCH = sizeof(double) * 2 * mrdgen::MAXE * (size_t)EXACT_BLOCKS * EXACT_THREADS;   // 182 MB
 }  // namespace
+
+int mrd_meshgen_release(void) {
+  std::lock_guard<std::mutex> g(g_arena.mu);
+  g_arena.release();
+  return MRD_OK;
+}
 
 int mrd_meshgen_test_quality(int64_t n_triangle, const double *xy_dev, const int32_t *tri_dev, double R, double B, double *r_dev,
                              double *beta_dev, double *cc_dev, uint8_t *bad_dev, int64_t *n_bad, void *stream) {
@@ -307,19 +378,19 @@ int mrd_meshgen_test_quality(int64_t n_triangle, const double *xy_dev, const int
     return gen_fail(MRD_EINVAL, "null argument");
   if (!(R > 0.0) || !(B > 0.0)) return gen_fail(MRD_EINVAL, "R and B must be positive");
   cudaStream_t s = (cudaStream_t)stream;
-  unsigned long long *cnt = nullptr;
-  GEN_TRY(cudaMalloc(&cnt, sizeof *cnt));
-  GEN_TRY(cudaMemsetAsync(cnt, 0, sizeof *cnt, s));
+  std::lock_guard<std::mutex> g(g_arena.mu);
+  cudaError_t e = g_arena.reserve(256);
+  if (e != cudaSuccess) return cuda_fail("test_quality", e);
+  unsigned long long *cnt = (unsigned long long *)g_arena.base;
+  cudaMemsetAsync(cnt, 0, sizeof *cnt, s);
   if (n_triangle > 0)
     mrdgen::test_quality_kernel<<<(unsigned)((n_triangle + 255) / 256), 256, 0, s>>>(n_triangle, (const double2 *)xy_dev, tri_dev, R, B, r_dev, beta_dev,
                                                                                      (double2 *)cc_dev, bad_dev, cnt);
-  unsigned long long h = 0;
-  cudaError_t e = cudaMemcpyAsync(&h, cnt, sizeof h, cudaMemcpyDeviceToHost, s);
+  e = cudaMemcpyAsync(g_arena.pinned, cnt, sizeof *cnt, cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e == cudaSuccess) e = cudaGetLastError();
-  cudaFree(cnt);
-  if (e != cudaSuccess) return gen_fail(MRD_ECUDA, std::string("test_quality: ") + cudaGetErrorString(e));
-  if (n_bad) *n_bad = (int64_t)h;
+  if (e != cudaSuccess) return cuda_fail("test_quality", e);
+  if (n_bad) *n_bad = (int64_t)g_arena.pinned[0];
   return MRD_OK;
 }
 
@@ -327,33 +398,31 @@ static int predicate_impl(int which, int64_t n, const double *xy_dev, const int3
   if (n < 0 || (n > 0 && (!xy_dev || !idx_dev || !sign_dev))) return gen_fail(MRD_EINVAL, "null argument");
   if (n > 0x7FFFFFF0ll) return gen_fail(MRD_EINVAL, "too many tests for 32-bit work lists");
   cudaStream_t s = (cudaStream_t)stream;
-  unsigned long long *cnt = nullptr;
-  int32_t *work = nullptr;
-  double *scratch = nullptr;
-  GEN_TRY(cudaMalloc(&cnt, sizeof *cnt));
-  cudaError_t e = cudaMalloc(&work, sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
-  const int exact_blocks = 148 * 4, exact_threads = 32;
-  if (e == cudaSuccess && which == 1) e = cudaMalloc(&scratch, sizeof(double) * 2 * mrdgen::MAXE * (size_t)exact_blocks * exact_threads);
-  if (e == cudaSuccess) e = cudaMemsetAsync(cnt, 0, sizeof *cnt, s);
-  if (e == cudaSuccess && n > 0) {
+  Carve c;
+  const size_t o_cnt = c.add(sizeof(unsigned long long)), o_work = c.add(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+  const size_t o_scr = which == 1 ? c.add(EXACT_SCRATCH) : 0;
+  std::lock_guard<std::mutex> g(g_arena.mu);
+  cudaError_t e = g_arena.reserve(c.total);
+  if (e != cudaSuccess) return cuda_fail("predicate", e);
+  unsigned long long *cnt = (unsigned long long *)(g_arena.base + o_cnt);
+  int32_t *work = (int32_t *)(g_arena.base + o_work);
+  double *scratch = (double *)(g_arena.base + o_scr);
+  cudaMemsetAsync(cnt, 0, sizeof *cnt, s);
+  if (n > 0) {
     const unsigned nb = (unsigned)((n + 255) / 256);
     if (which == 0) {
       mrdgen::orient_filter_kernel<<<nb, 256, 0, s>>>(n, (const double2 *)xy_dev, idx_dev, sign_dev, work, cnt);
-      mrdgen::orient_exact_kernel<<<exact_blocks, 128, 0, s>>>(cnt, work, (const double2 *)xy_dev, idx_dev, sign_dev);
+      mrdgen::orient_exact_kernel<<<EXACT_BLOCKS, 128, 0, s>>>(cnt, work, (const double2 *)xy_dev, idx_dev, sign_dev);
     } else {
       mrdgen::incircle_filter_kernel<<<nb, 256, 0, s>>>(n, (const double2 *)xy_dev, idx_dev, sign_dev, work, cnt);
-      mrdgen::incircle_exact_kernel<<<exact_blocks, exact_threads, 0, s>>>(cnt, work, (const double2 *)xy_dev, idx_dev, sign_dev, scratch);
+      mrdgen::incircle_exact_kernel<<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cnt, work, (const double2 *)xy_dev, idx_dev, sign_dev, scratch);
     }
   }
-  unsigned long long h = 0;
-  if (e == cudaSuccess) e = cudaMemcpyAsync(&h, cnt, sizeof h, cudaMemcpyDeviceToHost, s);
+  e = cudaMemcpyAsync(g_arena.pinned, cnt, sizeof *cnt, cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e == cudaSuccess) e = cudaGetLastError();
-  cudaFree(cnt);
-  cudaFree(work);
-  if (scratch) cudaFree(scratch);
-  if (e != cudaSuccess) return gen_fail(e == cudaErrorMemoryAllocation ? MRD_ENOMEM : MRD_ECUDA, std::string("predicate: ") + cudaGetErrorString(e));
-  if (n_exact) *n_exact = (int64_t)h;
+  if (e != cudaSuccess) return cuda_fail("predicate", e);
+  if (n_exact) *n_exact = (int64_t)g_arena.pinned[0];
   return MRD_OK;
 }
 
@@ -371,44 +440,39 @@ int mrd_meshgen_build_edges(int64_t n_triangle, const int32_t *tv_dev, int32_t *
   if (n_triangle == 0) return MRD_OK;
   cudaStream_t s = (cudaStream_t)stream;
   const int64_t n = 3 * n_triangle;
-  unsigned long long *key[2] = {nullptr, nullptr};
-  int32_t *val[2] = {nullptr, nullptr}, *head = nullptr, *incl = nullptr;
-  int *err = nullptr;
-  void *tmp = nullptr;
   size_t tmp_sort = 0, tmp_scan = 0;
-  cub::DeviceRadixSort::SortPairs(nullptr, tmp_sort, key[0], key[1], val[0], val[1], n, 0, 64, s);
-  cub::DeviceScan::InclusiveSum(nullptr, tmp_scan, head, incl, n, s);
-  cudaError_t e = cudaSuccess;
-  auto alloc = [&](void **p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
-  for (int j = 0; j < 2; ++j) {
-    alloc((void **)&key[j], sizeof(unsigned long long) * n);
-    alloc((void **)&val[j], sizeof(int32_t) * n);
-  }
-  alloc((void **)&head, sizeof(int32_t) * n);
-  alloc((void **)&incl, sizeof(int32_t) * n);
-  alloc((void **)&err, sizeof(int));
-  alloc(&tmp, std::max(tmp_sort, tmp_scan));
-  int h_err = 0;
-  int32_t h_ne = 0;
-  if (e == cudaSuccess) {
-    const unsigned nb = (unsigned)((n + 255) / 256);
-    cudaMemsetAsync(err, 0, sizeof(int), s);
-    cudaMemsetAsync(et_dev, 0xFF, sizeof(int32_t) * 2 * (size_t)n, s);   // -1: no second triangle
-    mrdgen::edge_keys_kernel<<<nb, 256, 0, s>>>(n, tv_dev, key[0], val[0]);
-    cub::DeviceRadixSort::SortPairs(tmp, tmp_sort, key[0], key[1], val[0], val[1], n, 0, 64, s);
-    mrdgen::edge_heads_kernel<<<nb, 256, 0, s>>>(n, key[1], head);
-    cub::DeviceScan::InclusiveSum(tmp, tmp_scan, head, incl, n, s);
-    mrdgen::edge_fill_kernel<<<nb, 256, 0, s>>>(n, key[1], val[1], incl, te_dev, et_dev, err);
-    cudaMemcpyAsync(&h_err, err, sizeof(int), cudaMemcpyDeviceToHost, s);
-    cudaMemcpyAsync(&h_ne, incl + (n - 1), sizeof(int32_t), cudaMemcpyDeviceToHost, s);
-    e = cudaStreamSynchronize(s);
-    if (e == cudaSuccess) e = cudaGetLastError();
-  }
-  for (int j = 0; j < 2; ++j) { cudaFree(key[j]); cudaFree(val[j]); }
-  cudaFree(head); cudaFree(incl); cudaFree(err); cudaFree(tmp);
-  if (e != cudaSuccess) return gen_fail(e == cudaErrorMemoryAllocation ? MRD_ENOMEM : MRD_ECUDA, std::string("build_edges: ") + cudaGetErrorString(e));
-  if (h_err) return gen_fail(MRD_EINVAL, "build_edges: an edge belongs to more than two triangles");
-  *n_edge = h_ne;
+  cub::DeviceRadixSort::SortPairs(nullptr, tmp_sort, (unsigned long long *)nullptr, (unsigned long long *)nullptr, (int32_t *)nullptr,
+                                  (int32_t *)nullptr, n, 0, 64, s);
+  cub::DeviceScan::InclusiveSum(nullptr, tmp_scan, (int32_t *)nullptr, (int32_t *)nullptr, n, s);
+  Carve c;
+  const size_t o_k0 = c.add(sizeof(unsigned long long) * n), o_k1 = c.add(sizeof(unsigned long long) * n);
+  const size_t o_v0 = c.add(sizeof(int32_t) * n), o_v1 = c.add(sizeof(int32_t) * n);
+  const size_t o_head = c.add(sizeof(int32_t) * n), o_incl = c.add(sizeof(int32_t) * n), o_err = c.add(sizeof(int));
+  const size_t o_tmp = c.add(std::max(tmp_sort, tmp_scan));
+  std::lock_guard<std::mutex> g(g_arena.mu);
+  cudaError_t e = g_arena.reserve(c.total);
+  if (e != cudaSuccess) return cuda_fail("build_edges", e);
+  char *b = g_arena.base;
+  unsigned long long *k0 = (unsigned long long *)(b + o_k0), *k1 = (unsigned long long *)(b + o_k1);
+  int32_t *v0 = (int32_t *)(b + o_v0), *v1 = (int32_t *)(b + o_v1), *head = (int32_t *)(b + o_head), *incl = (int32_t *)(b + o_incl);
+  int *err = (int *)(b + o_err);
+  const unsigned nb = (unsigned)((n + 255) / 256);
+  cudaMemsetAsync(err, 0, sizeof(int), s);
+  cudaMemsetAsync(et_dev, 0xFF, sizeof(int32_t) * 2 * (size_t)n, s);   // -1: no second triangle
+  mrdgen::edge_keys_kernel<<<nb, 256, 0, s>>>(n, tv_dev, k0, v0);
+  // (vertex numbers are below 2^31: the keys have 63 significant bits)
+  cub::DeviceRadixSort::SortPairs(b + o_tmp, tmp_sort, k0, k1, v0, v1, n, 0, 63, s);
+  mrdgen::edge_heads_kernel<<<nb, 256, 0, s>>>(n, k1, head);
+  cub::DeviceScan::InclusiveSum(b + o_tmp, tmp_scan, head, incl, n, s);
+  mrdgen::edge_fill_kernel<<<nb, 256, 0, s>>>(n, k1, v1, incl, te_dev, et_dev, err);
+  int32_t *h = (int32_t *)g_arena.pinned;
+  cudaMemcpyAsync(h, err, sizeof(int), cudaMemcpyDeviceToHost, s);
+  cudaMemcpyAsync(h + 1, incl + (n - 1), sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+  e = cudaStreamSynchronize(s);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("build_edges", e);
+  if (h[0]) return gen_fail(MRD_EINVAL, "build_edges: an edge belongs to more than two triangles");
+  *n_edge = h[1];
   return MRD_OK;
 }
 
@@ -423,56 +487,49 @@ int mrd_meshgen_delaunay_flip(int64_t n_triangle, int64_t n_edge, const double *
   if (n_edge == 0) return MRD_OK;
   using mrdgen::FlipCounters;
   cudaStream_t s = (cudaStream_t)stream;
-  const int exact_blocks = 148 * 4, exact_threads = 32;
-  int8_t *state = nullptr;
-  unsigned long long *lock = nullptr;
-  int32_t *mark = nullptr, *list[2] = {nullptr, nullptr}, *work = nullptr;
-  FlipCounters *cnt = nullptr;
-  double *scratch = nullptr;
-  cudaError_t e = cudaSuccess;
-  auto alloc = [&](void **p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
-  alloc((void **)&state, (size_t)n_edge);
-  alloc((void **)&lock, sizeof(unsigned long long) * (size_t)std::max<int64_t>(n_triangle, 1));
-  alloc((void **)&mark, sizeof(int32_t) * (size_t)n_edge);
-  alloc((void **)&list[0], sizeof(int32_t) * (size_t)n_edge);
-  alloc((void **)&list[1], sizeof(int32_t) * (size_t)n_edge);
-  alloc((void **)&work, sizeof(int32_t) * (size_t)n_edge);
-  alloc((void **)&cnt, sizeof(FlipCounters));
-  alloc((void **)&scratch, sizeof(double) * 2 * mrdgen::MAXE * (size_t)exact_blocks * exact_threads);
+  const size_t nt = (size_t)std::max<int64_t>(n_triangle, 1), ne = (size_t)n_edge;
+  Carve c;
+  const size_t o_cnt = c.add(sizeof(FlipCounters)), o_state = c.add(ne), o_lock = c.add(sizeof(unsigned long long) * nt);
+  const size_t o_mark = c.add(sizeof(int32_t) * ne), o_l0 = c.add(sizeof(int32_t) * ne), o_l1 = c.add(sizeof(int32_t) * ne);
+  const size_t o_work = c.add(sizeof(int32_t) * ne), o_scr = c.add(EXACT_SCRATCH);
+  std::lock_guard<std::mutex> g(g_arena.mu);
+  cudaError_t e = g_arena.reserve(c.total);
+  if (e != cudaSuccess) return cuda_fail("delaunay_flip", e);
+  char *b = g_arena.base;
+  FlipCounters *cnt = (FlipCounters *)(b + o_cnt);
+  int8_t *state = (int8_t *)(b + o_state);
+  unsigned long long *lock = (unsigned long long *)(b + o_lock);
+  int32_t *mark = (int32_t *)(b + o_mark), *list[2] = {(int32_t *)(b + o_l0), (int32_t *)(b + o_l1)}, *work = (int32_t *)(b + o_work);
+  double *scratch = (double *)(b + o_scr);
+  static_assert(sizeof(FlipCounters) <= 16 * sizeof(unsigned long long), "pinned block too small");
+  const FlipCounters *h = (const FlipCounters *)g_arena.pinned;
   int64_t flips = 0, iters = 0, exact = 0;
-  int rc = MRD_OK;
-  if (e == cudaSuccess) {
-    cudaMemsetAsync(state, 0, (size_t)n_edge, s);
-    cudaMemsetAsync(lock, 0, sizeof(unsigned long long) * (size_t)std::max<int64_t>(n_triangle, 1), s);
-    cudaMemsetAsync(mark, 0, sizeof(int32_t) * (size_t)n_edge, s);
-    int64_t n = n_edge;
-    const int32_t *cand = nullptr;                               // first iteration: every edge
-    const double2 *xy = (const double2 *)xy_dev;
-    for (int32_t iter = 1;; ++iter) {
-      if (iter > 100000) { rc = gen_fail(MRD_EINVAL, "delaunay_flip: no convergence (is the input a valid triangulation?)"); break; }
-      const unsigned long long stamp = (unsigned long long)iter << 32;
-      int32_t *next = list[iter & 1];
-      const unsigned nb = (unsigned)((n + 255) / 256);
-      cudaMemsetAsync(cnt, 0, sizeof(FlipCounters), s);
-      mrdgen::check_edge_kernel<<<nb, 256, 0, s>>>(n, cand, xy, tv_dev, te_dev, et_dev, state, lock, stamp, work, cnt);
-      mrdgen::check_edge_exact_kernel<<<exact_blocks, exact_threads, 0, s>>>(work, xy, tv_dev, te_dev, et_dev, state, lock, stamp, cnt, scratch);
-      mrdgen::flip_kernel<<<nb, 256, 0, s>>>(n, cand, tv_dev, te_dev, et_dev, state, lock, stamp, iter, mark, next, cnt);
-      FlipCounters h;
-      e = cudaMemcpyAsync(&h, cnt, sizeof h, cudaMemcpyDeviceToHost, s);
-      if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-      if (e == cudaSuccess) e = cudaGetLastError();
-      if (e != cudaSuccess) break;
-      iters++;
-      flips += (int64_t)h.n_flip;
-      exact += (int64_t)h.n_exact;
-      if (h.n_bad == 0) break;                                   // every edge is locally Delaunay
-      cand = next;
-      n = (int64_t)h.n_next;
-    }
+  cudaMemsetAsync(state, 0, ne, s);
+  cudaMemsetAsync(lock, 0, sizeof(unsigned long long) * nt, s);
+  cudaMemsetAsync(mark, 0, sizeof(int32_t) * ne, s);
+  int64_t n = n_edge;
+  const int32_t *cand = nullptr;                                 // first iteration: every edge
+  const double2 *xy = (const double2 *)xy_dev;
+  for (int32_t iter = 1;; ++iter) {
+    if (iter > 100000) return gen_fail(MRD_EINVAL, "delaunay_flip: no convergence (is the input a valid triangulation?)");
+    const unsigned long long stamp = (unsigned long long)iter << 32;
+    int32_t *next = list[iter & 1];
+    const unsigned nb = (unsigned)((n + 255) / 256);
+    cudaMemsetAsync(cnt, 0, sizeof(FlipCounters), s);
+    mrdgen::check_edge_kernel<<<nb, 256, 0, s>>>(n, cand, xy, tv_dev, te_dev, et_dev, state, lock, stamp, work, cnt);
+    mrdgen::check_edge_exact_kernel<<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(work, xy, tv_dev, te_dev, et_dev, state, lock, stamp, cnt, scratch);
+    mrdgen::flip_kernel<<<nb, 256, 0, s>>>(n, cand, tv_dev, te_dev, et_dev, state, lock, stamp, iter, mark, next, cnt);
+    e = cudaMemcpyAsync(g_arena.pinned, cnt, sizeof(FlipCounters), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail("delaunay_flip", e);
+    iters++;
+    flips += (int64_t)h->n_flip;
+    exact += (int64_t)h->n_exact;
+    if (h->n_bad == 0) break;                                    // every edge is locally Delaunay
+    cand = next;
+    n = (int64_t)h->n_next;
   }
-  cudaFree(state); cudaFree(lock); cudaFree(mark); cudaFree(list[0]); cudaFree(list[1]); cudaFree(work); cudaFree(cnt); cudaFree(scratch);
-  if (e != cudaSuccess) return gen_fail(e == cudaErrorMemoryAllocation ? MRD_ENOMEM : MRD_ECUDA, std::string("delaunay_flip: ") + cudaGetErrorString(e));
-  if (rc != MRD_OK) return rc;
   if (n_flips) *n_flips = flips;
   if (n_iterations) *n_iterations = iters;
   if (n_exact) *n_exact = exact;
@@ -487,18 +544,18 @@ int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_
   if (n_point == 0) return MRD_OK;
   if (n_triangle == 0) return gen_fail(MRD_EINVAL, "find_triangle: empty triangulation");
   cudaStream_t s = (cudaStream_t)stream;
-  int *err = nullptr;
-  GEN_TRY(cudaMalloc(&err, sizeof(int)));
+  std::lock_guard<std::mutex> g(g_arena.mu);
+  cudaError_t e = g_arena.reserve(256);
+  if (e != cudaSuccess) return cuda_fail("find_triangle", e);
+  int *err = (int *)g_arena.base;
   cudaMemsetAsync(err, 0, sizeof(int), s);
   mrdgen::find_triangle_kernel<<<(unsigned)((n_point + 127) / 128), 128, 0, s>>>(n_point, (const double2 *)p_dev, t0_dev, n_triangle + 16,
                                                                                    (const double2 *)xy_dev, tv_dev, te_dev, et_dev, t_dev, code_dev, err);
-  int h = 0;
-  cudaError_t e = cudaMemcpyAsync(&h, err, sizeof(int), cudaMemcpyDeviceToHost, s);
+  e = cudaMemcpyAsync(g_arena.pinned, err, sizeof(int), cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e == cudaSuccess) e = cudaGetLastError();
-  cudaFree(err);
-  if (e != cudaSuccess) return gen_fail(MRD_ECUDA, std::string("find_triangle: ") + cudaGetErrorString(e));
-  if (h) return gen_fail(MRD_EINVAL, "find_triangle: a walk did not end (not a Delaunay triangulation, or a start triangle out of range)");
+  if (e != cudaSuccess) return cuda_fail("find_triangle", e);
+  if (*(const int *)g_arena.pinned) return gen_fail(MRD_EINVAL, "find_triangle: a walk did not end (not a Delaunay triangulation, or a start triangle out of range)");
   return MRD_OK;
 }
 

@@ -157,6 +157,9 @@ def test_delaunay_flip_leaves_cocircular_points_alone_and_handles_degenerate_siz
     assert mrdb.meshgen_delaunay_flip(dev(np.array([[0.0, 0.0], [1.0, 0.0], [0.0, 1.0]]), torch.float64), one, te1, et1)["flips"] == 0
     empty = torch.empty((0, 3), dtype=torch.int32, device="cuda")
     assert mrdb.meshgen_delaunay_flip(xy, empty, empty.clone(), torch.empty((0, 2), dtype=torch.int32, device="cuda"))["flips"] == 0
+    mrdb.meshgen_release()                                         # the kept work space comes back on the next call
+    te, et = mrdb.meshgen_build_edges(tv)
+    assert mrdb.meshgen_delaunay_flip(xy, tv, te, et)["flips"] == 0
 
 
 def test_find_triangle_matches_the_oracle(mrdb):
