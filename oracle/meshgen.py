@@ -181,3 +181,210 @@ def find_triangle(xy, tv, te, et, p, t0, max_steps=10 ** 7):
             return -1 - t, 0
         t = nxt
     raise RuntimeError("find_triangle did not terminate")
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# Delaunay refinement (section 2.4) with the parallel insertion set of section 4.1.1 (L634-L654), bounded domains
+# ----------------------------------------------------------------------------------------------------------------------
+CAVITY_MAX = 64     # reading M11: a candidate whose cavity has more triangles than this waits for a later iteration
+KIND_NONE, KIND_TRI, KIND_EDGE, KIND_SEG = 0, 1, 2, 3
+
+
+def priority(seed: int, iteration: int, t: int) -> int:
+    """The "unique random integer" i(v) of L648 for the candidate of bad triangle t (reading M10): a 32-bit mix of (seed,
+    iteration, t) in the upper half, t itself in the lower half (which makes it unique).  Integer arithmetic modulo 2^32."""
+    m = 0xFFFFFFFF
+    x = (t * 2654435761 + iteration * 40503 + seed) & m
+    x ^= x >> 15
+    x = (x * 2246822519) & m
+    x ^= x >> 13
+    x = (x * 3266489917) & m
+    x ^= x >> 16
+    return (x << 32) | t
+
+
+def _encroaches(xy, u, w, p) -> bool:
+    """eq. 4 (L172), one IEEE operation at a time: (r_u - p) . (r_w - p) < 0  -- "no need for exact predicates" (L174)."""
+    ux, uy, wx, wy = xy[u][0] - p[0], xy[u][1] - p[1], xy[w][0] - p[0], xy[w][1] - p[1]
+    return ux * wx + uy * wy < 0.0
+
+
+def _edge_ends(tv, te, t, e):
+    k = _opposite(te, t, e)
+    return int(tv[t, (k + 1) % 3]), int(tv[t, (k + 2) % 3])
+
+
+def _midpoint(xy, u, w):
+    return (0.5 * (xy[u][0] + xy[w][0]), 0.5 * (xy[u][1] + xy[w][1]))
+
+
+def candidate(xy, tv, te, et, t_bad, cc):
+    """Sections 2.4.2-2.4.3 for the circumcentre cc of the bad triangle t_bad: where, and as what, a vertex would go in.
+    Returns (kind, p, t_ins, e): KIND_TRI inside triangle t_ins; KIND_EDGE on the interior edge e (t_ins = et[e][0]);
+    KIND_SEG: the midpoint of segment e (boundary edge of t_ins) -- because the walk left the triangulation through e
+    (reading M8: "if the circumcentre happens to be outside the triangulation ... somewhere a segment is encroached", L140),
+    because cc lies on e, or because cc encroaches upon e (eq. 4; of several encroached segments the one with the lowest edge
+    number, reading M9); KIND_NONE when cc coincides with an existing vertex."""
+    t, code = find_triangle(xy, tv, te, et, cc, t_bad)
+    if t < 0:
+        t_last = -1 - t
+        a, b, c = (int(v) for v in tv[t_last])
+        # the walk crosses the first edge with cc strictly outside; at a boundary edge that is where it left
+        s = (orient2d(xy[a], xy[b], cc), orient2d(xy[b], xy[c], cc), orient2d(xy[c], xy[a], cc))
+        k = (2, 0, 1)[[j for j in range(3) if s[j] < 0][0]]
+        e = int(te[t_last, k])
+        return KIND_SEG, _midpoint(xy, *_edge_ends(tv, te, t_last, e)), t_last, e
+    if code >= 4:
+        return KIND_NONE, (float(cc[0]), float(cc[1])), t, -1
+    if code >= 1:
+        e = int(te[t, code - 1])
+        if int(et[e, 1]) < 0:
+            return KIND_SEG, _midpoint(xy, *_edge_ends(tv, te, t, e)), t, e
+        kind, tris = KIND_EDGE, [int(et[e, 0]), int(et[e, 1])]
+    else:
+        e, kind, tris = -1, KIND_TRI, [t]
+    # eq. 4 against every segment of "all triangles that have either a, b or c as a vertex" (L176-L178)
+    verts = set(int(v) for tt in tris for v in tv[tt])
+    hit = []
+    for tt in range(tv.shape[0]):
+        if verts & set(int(v) for v in tv[tt]):
+            for k in range(3):
+                s = int(te[tt, k])
+                if int(et[s, 1]) < 0 and _encroaches(xy, *_edge_ends(tv, te, tt, s), cc):
+                    hit.append((s, tt))
+    if hit:
+        s, tt = min(hit)
+        return KIND_SEG, _midpoint(xy, *_edge_ends(tv, te, tt, s)), tt, s
+    return kind, (float(cc[0]), float(cc[1])), tris[0], e
+
+
+def cavity(xy, tv, te, et, p, start):
+    """Section 4.1.1 (L640-L644): the triangles whose circumcircles contain p (exact INCIRCLE2D > 0), reached from the insertion
+    triangle(s) through shared edges.  Returns a sorted list."""
+    seen, todo = set(start), list(start)
+    while todo:
+        t = todo.pop()
+        for k in range(3):
+            e = int(te[t, k])
+            n = int(et[e, 0]) if int(et[e, 0]) != t else int(et[e, 1])
+            if n >= 0 and n not in seen and incircle2d(*(xy[int(v)] for v in tv[n]), p) > 0:
+                seen.add(n)
+                todo.append(n)
+    return sorted(seen)
+
+
+def _replace(et, e, old, new):
+    j = 0 if int(et[e, 0]) == old else 1
+    assert int(et[e, j]) == old
+    et[e, j] = new
+
+
+def insert_vertex(tv, te, et, kind, t, e, v, nt, ne):
+    """Section 2.4.4 (L180-L184) for new vertex v, with the new triangles numbered from nt and the new edges from ne.
+    KIND_TRI: T = (a, b, c) becomes (a, b, v), (b, c, v), (c, a, v): "adds two triangles".  KIND_EDGE: the two triangles
+    sharing E are each split into two.  KIND_SEG: "the single triangle of which the segment is part is split into two".
+    tv, te, et must have room.  Returns (triangles added, edges added)."""
+    if kind == KIND_TRI:
+        a, b, c = (int(x) for x in tv[t])
+        e0, e1, e2 = (int(x) for x in te[t])
+        t1, t2, f0, f1, f2 = nt, nt + 1, ne, ne + 1, ne + 2       # f0 = (v, a), f1 = (v, b), f2 = (v, c)
+        tv[t], te[t] = (a, b, v), (f1, f0, e2)
+        tv[t1], te[t1] = (b, c, v), (f2, f1, e0)
+        tv[t2], te[t2] = (c, a, v), (f0, f2, e1)
+        et[f0], et[f1], et[f2] = (t, t2), (t, t1), (t1, t2)
+        _replace(et, e0, t, t1)
+        _replace(et, e1, t, t2)
+        return 2, 3
+    t1 = t
+    i1 = _opposite(te, t1, e)
+    a, b, c = (int(tv[t1, (i1 + j) % 3]) for j in range(3))      # E = (b, c), a opposite
+    e_ca, e_ab = int(te[t1, (i1 + 1) % 3]), int(te[t1, (i1 + 2) % 3])
+    if kind == KIND_SEG:
+        n1, g0, g1 = nt, ne, ne + 1                               # E becomes (b, v); g0 = (v, c) is the other half; g1 = (a, v)
+        tv[t1], te[t1] = (a, b, v), (e, g1, e_ab)
+        tv[n1], te[n1] = (a, v, c), (g0, e_ca, g1)
+        et[g0], et[g1] = (n1, -1), (t1, n1)
+        _replace(et, e_ca, t1, n1)
+        return 1, 2
+    t2 = int(et[e, 0]) if int(et[e, 0]) != t1 else int(et[e, 1])
+    i2 = _opposite(te, t2, e)
+    d = int(tv[t2, i2])
+    e_bd, e_dc = int(te[t2, (i2 + 1) % 3]), int(te[t2, (i2 + 2) % 3])
+    n1, n2, g0, g1, g2 = nt, nt + 1, ne, ne + 1, ne + 2           # E becomes (b, v); g0 = (v, c), g1 = (a, v), g2 = (v, d)
+    tv[t1], te[t1] = (a, b, v), (e, g1, e_ab)
+    tv[n1], te[n1] = (a, v, c), (g0, e_ca, g1)
+    tv[t2], te[t2] = (d, v, b), (e, e_bd, g2)
+    tv[n2], te[n2] = (d, c, v), (g0, g2, e_dc)
+    et[g0], et[g1], et[g2] = (n1, n2), (t1, n1), (t2, n2)
+    _replace(et, e_ca, t1, n1)
+    _replace(et, e_dc, t2, n2)
+    return 2, 3
+
+
+def flip_to_delaunay(xy, tv, te, et):
+    """delaunay_flip on an existing structure, in place; returns the number of flips."""
+    flips = 0
+    while True:
+        done = True
+        for e in range(et.shape[0]):
+            if check_edge(xy, tv, te, et, e):
+                flip_edge(tv, te, et, e)
+                flips += 1
+                done = False
+        if done:
+            return flips
+
+
+def refine_iteration(xy, tv, te, et, R, B, seed, iteration):
+    """One iteration of section 2.4 on a Delaunay triangulation: TestQuality; for every bad triangle, in ascending order, its
+    candidate; cavities and the independent set of section 4.1.1 (a triangle claimed by several cavities goes to the highest
+    priority; a candidate is selected when it holds every triangle of its cavity); the selected vertices are numbered, and
+    their triangles and edges appended, in ascending order of their bad triangle; flips restore the Delaunay property.
+    Returns (xy, tv, te, et, info) as new arrays; info: n_bad, n_selected, kinds of the selected, flips."""
+    xy = np.asarray(xy, dtype=np.float64)
+    q = test_quality(xy, tv, R, B)
+    bad = np.nonzero(q["bad"])[0]
+    cands = []
+    for t in bad:
+        kind, p, t_ins, e = candidate(xy, tv, te, et, int(t), q["cc"][t])
+        if kind == KIND_NONE:
+            continue
+        start = [int(et[e, 0]), int(et[e, 1])] if kind == KIND_EDGE else [t_ins]
+        cav = cavity(xy, tv, te, et, p, start)
+        if len(cav) > CAVITY_MAX:
+            continue
+        cands.append((int(t), kind, p, t_ins, e, cav))
+    lock = {}
+    for t, kind, p, t_ins, e, cav in cands:
+        pr = priority(seed, iteration, t)
+        for c in cav:
+            lock[c] = max(lock.get(c, 0), pr)
+    sel = [cd for cd in cands if all(lock[c] == priority(seed, iteration, cd[0]) for c in cd[5])]
+    nv, nt, ne = xy.shape[0], tv.shape[0], et.shape[0]
+    add_t = sum(1 if cd[1] == KIND_SEG else 2 for cd in sel)
+    add_e = sum(2 if cd[1] == KIND_SEG else 3 for cd in sel)
+    xy2 = np.concatenate([xy, np.array([cd[2] for cd in sel], dtype=np.float64).reshape(-1, 2)])
+    tv2 = np.concatenate([np.array(tv, dtype=np.int32), np.full((add_t, 3), -1, np.int32)])
+    te2 = np.concatenate([np.array(te, dtype=np.int32), np.full((add_t, 3), -1, np.int32)])
+    et2 = np.concatenate([np.array(et, dtype=np.int32), np.full((add_e, 2), -1, np.int32)])
+    for j, (t, kind, p, t_ins, e, cav) in enumerate(sel):
+        dt, de = insert_vertex(tv2, te2, et2, kind, t_ins, e, nv + j, nt, ne)
+        nt, ne = nt + dt, ne + de
+    flips = flip_to_delaunay(xy2, tv2, te2, et2)
+    info = dict(n_bad=len(bad), n_candidates=len(cands), n_selected=len(sel), kinds=[cd[1] for cd in sel], flips=flips,
+                selected=[(cd[0], cd[1], cd[2], cd[5]) for cd in sel])
+    return xy2, tv2, te2, et2, info
+
+
+def refine(xy, tv, R, B, seed=0, max_iterations=10 ** 6):
+    """Section 2.4: iterate "until no more vertices need to be inserted".  The input is made Delaunay first.
+    Returns (xy, tv, te, et, number of iterations that inserted something)."""
+    xy = np.asarray(xy, dtype=np.float64)
+    tv, te, et, _ = delaunay_flip(xy, tv)
+    it = 0
+    while it < max_iterations:
+        xy, tv, te, et, info = refine_iteration(xy, tv, te, et, R, B, seed, it)
+        if info["n_bad"] == 0:
+            break
+        it += 1
+    return xy, tv, te, et, it

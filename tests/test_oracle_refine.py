@@ -1,0 +1,186 @@
+"""Pins of the oracle's Delaunay refinement (oracle/meshgen.py; section 2.3-2.4, 4.1.1): what the paper and geometry
+fix -- the three ways of inserting a vertex keep a valid structure and add 2 / 2 / 1 triangles (L180-L184); a cavity is exactly
+the set of triangles whose circumcircles contain the new vertex (L640); eq. 4 is the diametric-circle test (L136); selected
+cavities do not overlap (L642) and inserting the selected vertices gives THE Delaunay triangulation of the enlarged vertex set
+(checked against the library triangulation); the finished mesh has no triangle with r > R or beta > B, hence no angle below
+arcsin(1 / 2B) (L120), is Delaunay, covers the same rectangle, keeps the input vertices, and has no encroached segment."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from oracle import meshgen as mg
+from test_oracle_triangulator import angles, assert_structure
+
+
+def start_mesh(seed=3, shape=(6, 5)):
+    m = wl.scrambled_triangulation(*shape, seed=seed)
+    tv, te, et, _ = mg.delaunay_flip(m.xy, m.tri)
+    return m.xy, tv, te, et
+
+
+def area(xy, tv):
+    p = xy[tv]
+    return 0.5 * ((p[:, 1, 0] - p[:, 0, 0]) * (p[:, 2, 1] - p[:, 0, 1]) - (p[:, 1, 1] - p[:, 0, 1]) * (p[:, 2, 0] - p[:, 0, 0]))
+
+
+def grown(tv, te, et, dt, de):
+    return (np.concatenate([tv, np.full((dt, 3), -1, np.int32)]), np.concatenate([te, np.full((dt, 3), -1, np.int32)]),
+            np.concatenate([et, np.full((de, 2), -1, np.int32)]))
+
+
+def library_triangulation(xy):
+    from scipy.spatial import Delaunay
+    lib = Delaunay(xy).simplices
+    cw = np.array([mg.orient2d(*xy[s]) for s in lib]) < 0
+    lib[cw] = lib[cw][:, [0, 2, 1]]
+    return mg.triangle_set(lib)
+
+
+def test_the_three_insertions_keep_a_valid_structure_and_add_2_2_1_triangles():
+    xy, tv, te, et = start_mesh()
+    nv, nt, ne = xy.shape[0], tv.shape[0], et.shape[0]
+    total = area(xy, tv).sum()
+    # inside a triangle: its centroid
+    t = 7
+    p = xy[tv[t]].mean(axis=0)
+    tv2, te2, et2 = grown(tv, te, et, 2, 3)
+    assert mg.insert_vertex(tv2, te2, et2, mg.KIND_TRI, t, -1, nv, nt, ne) == (2, 3)
+    xy2 = np.vstack([xy, p])
+    assert_structure(xy2, tv2, te2, et2)
+    assert abs(area(xy2, tv2).sum() - total) < 1e-13 and (tv2 == nv).sum() == 3
+    # on an interior edge: its midpoint (exactly representable halves are not needed: orientation of the four pieces is what counts)
+    e = int(np.nonzero(et[:, 1] >= 0)[0][5])
+    t1 = int(et[e, 0])
+    u, w = mg._edge_ends(tv, te, t1, e)
+    xyg = xy.copy()
+    xyg[[u, w]] = np.round(xyg[[u, w]] * 1024) / 1024                # make the midpoint exact, so that it IS on the edge
+    p = 0.5 * (xyg[u] + xyg[w])
+    assert mg.orient2d(xyg[u], xyg[w], p) == 0
+    tv2, te2, et2 = grown(tv, te, et, 2, 3)
+    assert mg.insert_vertex(tv2, te2, et2, mg.KIND_EDGE, t1, e, nv, nt, ne) == (2, 3)
+    xy2 = np.vstack([xyg, p])
+    assert_structure(xy2, tv2, te2, et2)
+    assert (tv2 == nv).sum() == 4 and abs(area(xy2, tv2).sum() - area(xyg, tv).sum()) < 1e-13
+    # on a segment: "the single triangle of which the segment is part is split into two"
+    s = int(np.nonzero(et[:, 1] < 0)[0][3])
+    t1 = int(et[s, 0])
+    p = np.array(mg._midpoint(xy, *mg._edge_ends(tv, te, t1, s)))
+    tv2, te2, et2 = grown(tv, te, et, 1, 2)
+    assert mg.insert_vertex(tv2, te2, et2, mg.KIND_SEG, t1, s, nv, nt, ne) == (1, 2)
+    xy2 = np.vstack([xy, p])
+    assert_structure(xy2, tv2, te2, et2)
+    assert (tv2 == nv).sum() == 2 and (et2[:, 1] < 0).sum() == (et[:, 1] < 0).sum() + 1
+    assert abs(area(xy2, tv2).sum() - total) < 1e-13
+
+
+def test_cavity_is_every_triangle_whose_circumcircle_contains_the_point():
+    xy, tv, te, et = start_mesh(seed=5, shape=(9, 7))
+    rng = np.random.default_rng(1)
+    for p in rng.random((40, 2)) * np.array([2.0, 1.5]):
+        t, code = mg.find_triangle(xy, tv, te, et, p, 0)
+        assert code == 0
+        brute = [k for k in range(tv.shape[0]) if mg.incircle2d(*xy[tv[k]], p) > 0]
+        cav = mg.cavity(xy, tv, te, et, p, [t])
+        assert cav == brute and t in cav and len(cav) >= 1        # connected: the walk from t finds them all (L644)
+
+
+def test_eq_4_is_the_diametric_circle():
+    rng = np.random.default_rng(2)
+    xy = rng.random((2, 2))
+    m, r = xy.mean(axis=0), 0.5 * np.hypot(*(xy[0] - xy[1]))
+    n = 0
+    for p in rng.random((2000, 2)) * 2 - 0.5:
+        d = np.hypot(*(p - m))
+        if abs(d - r) > 1e-9:
+            assert mg._encroaches(xy, 0, 1, p) == (d < r)         # L136: "if any vertex lies inside the diametric circle"
+            n += d < r
+    assert n > 50
+
+
+def test_candidates_of_constructed_cases():
+    # two right isosceles triangles: both circumcentres are the midpoint of the shared diagonal -> on the interior edge
+    xy = np.array([[0.0, 0.0], [1.0, 0.0], [0.0, 1.0], [1.0, 1.0]])
+    tv = np.array([[0, 1, 2], [1, 3, 2]], dtype=np.int32)
+    te, et = mg.build_edges(tv)
+    q = mg.test_quality(xy, tv, 1.0, 0.5)
+    kind, p, t, e = mg.candidate(xy, tv, te, et, 0, q["cc"][0])
+    assert kind == mg.KIND_EDGE and p == (0.5, 0.5) and int(et[e, 1]) >= 0
+    # an obtuse triangle at the boundary: the circumcentre is outside the domain -> the walk leaves through a segment,
+    # which is split at its midpoint
+    xy = np.array([[0.0, 0.0], [4.0, 0.0], [2.0, 0.5], [2.0, 3.0]])
+    tv = np.array([[0, 1, 2], [1, 3, 2], [3, 0, 2]], dtype=np.int32)
+    te, et = mg.build_edges(tv)
+    q = mg.test_quality(xy, tv, 10.0, 1.0)
+    assert q["cc"][0][1] < 0                                       # below the edge (0, 1)
+    kind, p, t, e = mg.candidate(xy, tv, te, et, 0, q["cc"][0])
+    assert kind == mg.KIND_SEG and p == (2.0, 0.0) and t == 0 and set(mg._edge_ends(tv, te, t, e)) == {0, 1}
+    # a point inside the domain but inside the diametric circle of a segment: the segment is split, not the triangle
+    cc = np.array([2.0, 0.2])
+    assert mg.find_triangle(xy, tv, te, et, cc, 1) == (0, 0)
+    kind, p, t, e = mg.candidate(xy, tv, te, et, 1, cc)
+    assert kind == mg.KIND_SEG and p == (2.0, 0.0)
+    # well inside a larger domain, far from every segment: into the triangle that contains it
+    xyb, tvb, teb, etb = start_mesh()
+    cc = np.array([1.03, 0.77])
+    kind, p, t, e = mg.candidate(xyb, tvb, teb, etb, 0, cc)
+    assert kind == mg.KIND_TRI and p == (1.03, 0.77) and e == -1 and mg.find_triangle(xyb, tvb, teb, etb, cc, 5) == (t, 0)
+    # exactly on a vertex: nothing to insert
+    assert mg.candidate(xy, tv, te, et, 0, xy[2])[0] == mg.KIND_NONE
+
+
+def test_priority_is_unique_reproducible_and_mixes():
+    pr = [mg.priority(7, 2, t) for t in range(4000)]
+    assert len(set(pr)) == 4000 and all(p & 0xFFFFFFFF == t for t, p in enumerate(pr))
+    hi = np.array([p >> 32 for p in pr], dtype=np.float64)
+    assert 0.45 < hi.mean() / 2 ** 32 < 0.55 and abs(np.corrcoef(hi[:-1], hi[1:])[0, 1]) < 0.1
+    assert mg.priority(7, 2, 5) != mg.priority(7, 3, 5) != mg.priority(8, 3, 5) and mg.priority(7, 2, 5) == pr[5]
+    assert mg.priority(0, 0, 0) == 0                              # the mix maps 0 to 0
+
+
+def test_one_iteration_inserts_an_independent_set_and_stays_delaunay():
+    xy, tv, te, et = start_mesh()
+    xy2, tv2, te2, et2, info = mg.refine_iteration(xy, tv, te, et, 0.06, 1.0, seed=3, iteration=0)
+    assert 0 < info["n_selected"] < info["n_candidates"] <= info["n_bad"]
+    cavs = [set(c[3]) for c in info["selected"]]
+    for i in range(len(cavs)):
+        for j in range(i):
+            assert not (cavs[i] & cavs[j])                        # L642: "their cavities do not overlap"
+    assert [c[0] for c in info["selected"]] == sorted(c[0] for c in info["selected"])
+    assert np.array_equal(xy2[:xy.shape[0]], xy) and xy2.shape[0] == xy.shape[0] + info["n_selected"]
+    assert np.array_equal(xy2[xy.shape[0]:], np.array([c[2] for c in info["selected"]]))
+    kinds = np.bincount(info["kinds"], minlength=4)
+    assert tv2.shape[0] == tv.shape[0] + 2 * (kinds[1] + kinds[2]) + kinds[3] and kinds[1] > 0 and kinds[3] > 0
+    assert_structure(xy2, tv2, te2, et2)
+    assert mg.triangle_set(tv2) == library_triangulation(xy2)     # THE Delaunay triangulation of the enlarged vertex set
+    # a loser of this iteration is a candidate again in the next one, and another seed picks another set
+    other = mg.refine_iteration(xy, tv, te, et, 0.06, 1.0, seed=4, iteration=0)[4]
+    assert [c[0] for c in other["selected"]] != [c[0] for c in info["selected"]]
+
+
+@pytest.mark.parametrize("B,R,seed", [(1.0, 0.09, 1), (np.sqrt(2.0), 0.07, 2)])
+def test_refinement_ends_with_the_guarantees_of_section_2_3(B, R, seed):
+    xy0, tv0, te0, et0 = start_mesh(seed=seed)
+    xy, tv, te, et, it = mg.refine(xy0, tv0, R, B, seed=seed)
+    assert 3 <= it < 60 and xy.shape[0] > 3 * xy0.shape[0]
+    q = mg.test_quality(xy, tv, R, B)
+    assert q["bad"].sum() == 0 and q["r"].max() <= R and q["beta"].max() <= B
+    assert angles(xy, tv).min() >= np.arcsin(1.0 / (2.0 * B)) - 1e-12          # L120: 2 beta = 1 / sin(alpha)
+    assert_structure(xy, tv, te, et)
+    assert all(not mg.check_edge(xy, tv, te, et, e) for e in range(et.shape[0]))
+    assert mg.triangle_set(tv) == library_triangulation(xy)
+    assert np.array_equal(xy[:xy0.shape[0]], xy0)
+    assert abs(area(xy, tv).sum() - 2.0 * 1.5) < 1e-12            # the rectangle of the workload, no more, no less
+    seg = np.nonzero(et[:, 1] < 0)[0]
+    ends = np.array([mg._edge_ends(tv, te, int(et[s, 0]), int(s)) for s in seg])
+    on_boundary = np.unique(ends)
+    b = xy[on_boundary]
+    assert (np.isin(b[:, 0], [0.0, 2.0]) | np.isin(b[:, 1], [0.0, 1.5])).all()   # segments stay on the sides (midpoints are exact there)
+    mid, rad = 0.5 * (xy[ends[:, 0]] + xy[ends[:, 1]]), 0.5 * np.hypot(*(xy[ends[:, 0]] - xy[ends[:, 1]]).T)
+    d = np.hypot(xy[:, None, 0] - mid[None, :, 0], xy[:, None, 1] - mid[None, :, 1])
+    assert (d >= rad[None, :] * (1 - 1e-12)).all()               # L136: no vertex inside a diametric circle -- no encroached segment
+    # "the resulting mesh ... is not unique ... the locations of the vertices depend on the order" (L144), the guarantees do not
+    xy_b, tv_b, _, _, _ = mg.refine(xy0, tv0, R, B, seed=seed + 10)
+    assert xy_b.shape != xy.shape or not np.array_equal(xy_b, xy)
+    assert mg.test_quality(xy_b, tv_b, R, B)["bad"].sum() == 0
+    xy_c, tv_c, _, _, _ = mg.refine(xy0, tv0, R, B, seed=seed)
+    assert np.array_equal(xy_c, xy) and np.array_equal(tv_c, tv)
