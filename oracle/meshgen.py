@@ -335,11 +335,22 @@ def flip_to_delaunay(xy, tv, te, et):
             return flips
 
 
+def canonical_order(tv):
+    """Reading M12: every iteration ends with the triangles renumbered -- each rotated so that its smallest vertex comes first,
+    all sorted by (first, second, third) vertex -- and the edge arrays rebuilt (build_edges numbers edges by their end points).
+    The paper re-sorts vertices, edges and triangles after every insertion step too (section 4.1.4, by Morton value); this
+    order has no ties, which makes the numbering, and with it the priorities of the next iteration, independent of the order
+    in which the flips happened."""
+    rows = sorted(triangle_set(tv))
+    return np.array(rows, dtype=np.int32).reshape(-1, 3)
+
+
 def refine_iteration(xy, tv, te, et, R, B, seed, iteration):
     """One iteration of section 2.4 on a Delaunay triangulation: TestQuality; for every bad triangle, in ascending order, its
     candidate; cavities and the independent set of section 4.1.1 (a triangle claimed by several cavities goes to the highest
     priority; a candidate is selected when it holds every triangle of its cavity); the selected vertices are numbered, and
-    their triangles and edges appended, in ascending order of their bad triangle; flips restore the Delaunay property.
+    their triangles and edges appended, in ascending order of their bad triangle; flips restore the Delaunay property; the
+    triangles are put in canonical order (reading M12).
     Returns (xy, tv, te, et, info) as new arrays; info: n_bad, n_selected, kinds of the selected, flips."""
     xy = np.asarray(xy, dtype=np.float64)
     q = test_quality(xy, tv, R, B)
@@ -371,6 +382,8 @@ def refine_iteration(xy, tv, te, et, R, B, seed, iteration):
         dt, de = insert_vertex(tv2, te2, et2, kind, t_ins, e, nv + j, nt, ne)
         nt, ne = nt + dt, ne + de
     flips = flip_to_delaunay(xy2, tv2, te2, et2)
+    tv2 = canonical_order(tv2)
+    te2, et2 = build_edges(tv2)
     info = dict(n_bad=len(bad), n_candidates=len(cands), n_selected=len(sel), kinds=[cd[1] for cd in sel], flips=flips,
                 selected=[(cd[0], cd[1], cd[2], cd[5]) for cd in sel])
     return xy2, tv2, te2, et2, info
@@ -380,7 +393,8 @@ def refine(xy, tv, R, B, seed=0, max_iterations=10 ** 6):
     """Section 2.4: iterate "until no more vertices need to be inserted".  The input is made Delaunay first.
     Returns (xy, tv, te, et, number of iterations that inserted something)."""
     xy = np.asarray(xy, dtype=np.float64)
-    tv, te, et, _ = delaunay_flip(xy, tv)
+    tv = canonical_order(delaunay_flip(xy, tv)[0])
+    te, et = build_edges(tv)
     it = 0
     while it < max_iterations:
         xy, tv, te, et, info = refine_iteration(xy, tv, te, et, R, B, seed, it)

@@ -184,3 +184,17 @@ def test_refinement_ends_with_the_guarantees_of_section_2_3(B, R, seed):
     assert mg.test_quality(xy_b, tv_b, R, B)["bad"].sum() == 0
     xy_c, tv_c, _, _, _ = mg.refine(xy0, tv0, R, B, seed=seed)
     assert np.array_equal(xy_c, xy) and np.array_equal(tv_c, tv)
+
+
+def test_canonical_order_renumbers_without_changing_the_triangulation():
+    xy, tv, te, et = start_mesh(seed=8)
+    rng = np.random.default_rng(0)
+    shuffled = tv[rng.permutation(tv.shape[0])]
+    rot = rng.integers(0, 3, size=tv.shape[0])
+    shuffled = np.stack([shuffled[np.arange(len(rot)), (rot + j) % 3] for j in range(3)], axis=1).astype(np.int32)
+    c = mg.canonical_order(shuffled)
+    assert mg.triangle_set(c) == mg.triangle_set(tv) and np.array_equal(c, mg.canonical_order(tv))
+    assert (c[:, 0] < c[:, 1]).all() and (c[:, 0] < c[:, 2]).all()
+    assert (np.lexsort((c[:, 2], c[:, 1], c[:, 0])) == np.arange(len(c))).all()
+    assert all(mg.orient2d(*xy[t]) == 1 for t in c)               # rotation only: every triangle stays counter-clockwise
+    assert np.array_equal(mg.canonical_order(c), c)
