@@ -345,6 +345,46 @@ int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_
                               const double *xy_dev, const int32_t *tv_dev, const int32_t *te_dev, const int32_t *et_dev,
                               int32_t *t_dev, int8_t *code_dev, void *stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * Mesh generation, third slice: Delaunay refinement of a bounded domain (section 2.3-2.4) with the parallel insertion
+ * set of section 4.1.1 (L634-L654).  The boundary edges of the input triangulation are the segments (L128-L140).
+ *
+ * mrd_meshgen_refine: repeats, at most max_iterations times and until no triangle is bad,
+ *   1. TestQuality (eq. 2): every triangle with circumradius r > R or r / shortest edge > B is bad; its circumcentre is a
+ *      candidate vertex (2.4.1);
+ *   2. the triangle containing the candidate, by the walk of mrd_meshgen_find_triangle from the bad triangle (2.4.2).  A
+ *      candidate outside the triangulation becomes the midpoint of the segment the walk left through; one on a segment the
+ *      midpoint of that segment; one that coincides with a vertex is dropped;
+ *   3. encroachment (2.4.3, eq. 4 in plain IEEE arithmetic): against the segments of all triangles that have a vertex of the
+ *      insertion triangle(s) as a vertex; a candidate that encroaches becomes the midpoint of the encroached segment with
+ *      the lowest edge number;
+ *   4. the cavity of every candidate -- the triangles whose circumcircles contain it (exact INCIRCLE2D), reached from the
+ *      insertion triangle(s) through shared edges -- claims its triangles with the candidate's priority i(v) (atomicMax, L648);
+ *      a candidate is selected when it holds all of them (4.1.1).  i(v) = mix32(seed, iteration, bad triangle) * 2^32 + bad
+ *      triangle; mix32(x): x ^= x >> 15, x *= 2246822519, x ^= x >> 13, x *= 3266489917, x ^= x >> 16 on
+ *      x = t * 2654435761 + iteration * 40503 + seed (mod 2^32).  A cavity of more than 64 triangles waits;
+ *   5. the selected vertices are inserted (2.4.4: a triangle split in three, the two triangles at an edge split in two each, the
+ *      one triangle at a segment split in two), numbered -- like their new triangles and edges -- in ascending order of
+ *      their bad triangle;
+ *   6. flips restore the Delaunay property (2.4.6);
+ *   7. the triangles are renumbered canonically (each rotated to its smallest vertex, sorted by vertex triple) and te, et
+ *      rebuilt as by mrd_meshgen_build_edges (the paper re-sorts after every insertion step too, 4.1.4).
+ *   Every step is deterministic and independent of the order in which threads run: the result is, array for array, the one
+ *   of oracle/meshgen.py: refine.
+ *   In: a Delaunay triangulation (xy, tv, te, et) with *n_vertex, *n_triangle, *n_edge entries in device arrays with room
+ *   for cap_vertex / cap_triangle / cap_edge (cap_edge >= 3 * cap_triangle); first_iteration: the iteration number the
+ *   priorities start from.  Out: the refined mesh in the same arrays, the three counts, *n_iterations (iterations that
+ *   inserted vertices), *n_bad_left (bad triangles remaining: 0 when finished).  HOST pointers for all counts.
+ *   Guarantees on completion (section 2.3): no triangle with r > R or beta > B, hence no angle below arcsin(1 / 2B); Delaunay;
+ *   no encroached segment.  Termination is guaranteed for B >= sqrt(2) and domains without small angles (L126).
+ *   MRD_ENOMEM when the next insertion would exceed a capacity (the arrays then hold a valid Delaunay mesh, partly
+ *   refined); MRD_EINVAL for an input that is not a Delaunay triangulation (a walk that does not end).
+ * ---------------------------------------------------------------------------------------------- */
+int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteration, int64_t max_iterations, int64_t cap_vertex,
+                       int64_t cap_triangle, int64_t cap_edge, int64_t *n_vertex, int64_t *n_triangle, int64_t *n_edge,
+                       double *xy_dev, int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_iterations,
+                       int64_t *n_bad_left, void *stream);
+
 /* Kernel launch counter: number of the library's own kernel launches since the mesh was created. */
 int mrd_launch_count(const mrd_mesh *m, int64_t *launches);
 

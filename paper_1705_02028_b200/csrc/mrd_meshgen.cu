@@ -19,8 +19,10 @@
 #include <cstdint>
 #include <cub/device/device_radix_sort.cuh>
 #include <cub/device/device_scan.cuh>
+#include <cub/device/device_select.cuh>
 #include <mutex>
 #include <string>
+#include <thrust/iterator/counting_iterator.h>
 
 #include "../../include/mrd.h"
 #include "mrd_predicates.cuh"
@@ -306,6 +308,290 @@ find_triangle_kernel(int64_t np, const double2 *__restrict__ p, const int32_t *_
   *err = 1;
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Delaunay refinement (section 2.4) with the parallel insertion set of section 4.1.1
+// ------------------------------------------------------------------------------------------------------------------
+constexpr int CAVITY_MAX = 64;   // reading M11
+enum { KIND_NONE = 0, KIND_TRI = 1, KIND_EDGE = 2, KIND_SEG = 3 };
+
+// i(v) of L648 (reading M10): 32-bit mix of (seed, iteration, bad triangle) above the bad triangle's number
+static __device__ __forceinline__ unsigned long long priority_of(unsigned seed, unsigned iteration, unsigned t) {
+  unsigned x = t * 2654435761u + iteration * 40503u + seed;
+  x ^= x >> 15;
+  x *= 2246822519u;
+  x ^= x >> 13;
+  x *= 3266489917u;
+  x ^= x >> 16;
+  return ((unsigned long long)x << 32) | t;
+}
+static __device__ __forceinline__ int local_of(const int32_t *row, int32_t x) { return row[0] == x ? 0 : (row[1] == x ? 1 : 2); }
+static __device__ __forceinline__ int32_t across(const int32_t *et, int32_t e, int32_t t) {
+  const int32_t n0 = et[2 * (int64_t)e], n1 = et[2 * (int64_t)e + 1];
+  return n0 != t ? n0 : n1;
+}
+// eq. 4 (L172), one IEEE operation at a time
+static __device__ __forceinline__ bool encroaches(double2 u, double2 w, double2 p) {
+  const double ux = __dsub_rn(u.x, p.x), uy = __dsub_rn(u.y, p.y), wx = __dsub_rn(w.x, p.x), wy = __dsub_rn(w.y, p.y);
+  return __dadd_rn(__dmul_rn(ux, wx), __dmul_rn(uy, wy)) < 0.0;
+}
+// the segments of triangle t that p encroaches upon: lowest edge number so far in (best_e, best_t)
+static __device__ __forceinline__ void test_segments(int32_t t, double2 p, const double2 *xy, const int32_t *tv, const int32_t *te,
+                                                     const int32_t *et, int32_t &best_e, int32_t &best_t) {
+  const int32_t *v = tv + 3 * (int64_t)t, *ed = te + 3 * (int64_t)t;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const int32_t e = ed[k];
+    if (et[2 * (int64_t)e + 1] < 0 && (best_e < 0 || e < best_e) && encroaches(xy[v[(k + 1) % 3]], xy[v[(k + 2) % 3]], p)) {
+      best_e = e;
+      best_t = t;
+    }
+  }
+}
+// all triangles that have x as a vertex (L176), starting from t: around x one way until back at t or at the boundary, then
+// the other way
+static __device__ void around_vertex(int32_t x, int32_t t, double2 p, const double2 *xy, const int32_t *tv, const int32_t *te,
+                                     const int32_t *et, int32_t &best_e, int32_t &best_t) {
+  test_segments(t, p, xy, tv, te, et, best_e, best_t);
+  for (int dir = 1; dir <= 2; ++dir) {
+    int32_t cur = t;
+    for (int guard = 0; guard < 4096; ++guard) {
+      const int k = local_of(tv + 3 * (int64_t)cur, x);
+      const int32_t nxt = across(et, te[3 * (int64_t)cur + (k + dir) % 3], cur);   // both edges opposite k+1 and k+2 contain x
+      if (nxt < 0) break;
+      if (nxt == t) return;                                        // closed fan: everything seen
+      test_segments(nxt, p, xy, tv, te, et, best_e, best_t);
+      cur = nxt;
+    }
+  }
+}
+static __device__ __forceinline__ double2 midpoint(double2 u, double2 w) {
+  return make_double2(__dmul_rn(0.5, __dadd_rn(u.x, w.x)), __dmul_rn(0.5, __dadd_rn(u.y, w.y)));
+}
+// sections 2.4.2-2.4.3 for the circumcentre of every bad triangle (oracle/meshgen.py: candidate)
+__global__ void __launch_bounds__(128)
+candidate_kernel(int64_t nc, const int32_t *__restrict__ cand, const double2 *__restrict__ cc, int64_t max_steps,
+                 const double2 *__restrict__ xy, const int32_t *__restrict__ tv, const int32_t *__restrict__ te,
+                 const int32_t *__restrict__ et, int8_t *__restrict__ kind, double2 *__restrict__ pt, int32_t *__restrict__ t_ins,
+                 int32_t *__restrict__ e_ins, int *__restrict__ err) {
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= nc) return;
+  const int32_t tb = cand[j];
+  const double2 P = cc[tb];
+  int32_t t = tb;
+  int code = -1, out = -1;
+  for (int64_t step = 0; step < max_steps; ++step) {               // the walk of find_triangle_kernel, keeping the exit edge
+    const int32_t *v = tv + 3 * (int64_t)t;
+    const double2 A = xy[v[0]], B = xy[v[1]], C = xy[v[2]];
+    int s0, s1 = 1, s2 = 1;
+    out = -1;
+    s0 = orient2d_sign(A, B, P);
+    if (s0 < 0) out = 2;
+    else {
+      s1 = orient2d_sign(B, C, P);
+      if (s1 < 0) out = 0;
+      else {
+        s2 = orient2d_sign(C, A, P);
+        if (s2 < 0) out = 1;
+      }
+    }
+    if (out < 0) {
+      const int z0 = s0 == 0, z1 = s1 == 0, z2 = s2 == 0;
+      code = 0;
+      if (z0 + z1 + z2 == 1) code = 1 + (z0 ? 2 : (z1 ? 0 : 1));
+      else if (z0 + z1 + z2 >= 2) code = 4;
+      break;
+    }
+    const int32_t nxt = across(et, te[3 * (int64_t)t + out], t);
+    if (nxt < 0) break;                                            // left the triangulation through edge `out` of t
+    t = nxt;
+    out = -1;
+  }
+  int8_t kd = KIND_NONE;
+  double2 p = P;
+  int32_t ti = t, ei = -1;
+  if (code < 0 && out < 0) { *err = 1; return; }                    // the walk did not end
+  if (code < 0) {                                                  // outside: split the segment it left through (M8)
+    ei = te[3 * (int64_t)t + out];
+    const int32_t *v = tv + 3 * (int64_t)t;
+    p = midpoint(xy[v[(out + 1) % 3]], xy[v[(out + 2) % 3]]);
+    kd = KIND_SEG;
+  } else if (code >= 4) {
+    kd = KIND_NONE;
+  } else {
+    int32_t t2 = -1;
+    if (code >= 1) {
+      ei = te[3 * (int64_t)t + code - 1];
+      if (et[2 * (int64_t)ei + 1] < 0) {                           // on a segment: split it
+        const int32_t *v = tv + 3 * (int64_t)t;
+        p = midpoint(xy[v[code % 3]], xy[v[(code + 1) % 3]]);
+        kd = KIND_SEG;
+      } else {
+        kd = KIND_EDGE;
+        ti = et[2 * (int64_t)ei];
+        t2 = et[2 * (int64_t)ei + 1];
+      }
+    } else kd = KIND_TRI;
+    if (kd != KIND_SEG) {                                          // eq. 4 around every vertex of the insertion triangle(s)
+      int32_t best_e = -1, best_t = -1;
+      const int32_t *v = tv + 3 * (int64_t)ti;
+      for (int k = 0; k < 3; ++k) around_vertex(v[k], ti, P, xy, tv, te, et, best_e, best_t);
+      if (t2 >= 0) {
+        const int32_t *w = tv + 3 * (int64_t)t2;
+        around_vertex(w[local_of(te + 3 * (int64_t)t2, ei)], t2, P, xy, tv, te, et, best_e, best_t);   // the fourth vertex
+      }
+      if (best_e >= 0) {
+        const int k = local_of(te + 3 * (int64_t)best_t, best_e);
+        const int32_t *u = tv + 3 * (int64_t)best_t;
+        p = midpoint(xy[u[(k + 1) % 3]], xy[u[(k + 2) % 3]]);
+        kd = KIND_SEG;
+        ti = best_t;
+        ei = best_e;
+      }
+    }
+  }
+  kind[j] = kd;
+  pt[j] = p;
+  t_ins[j] = ti;
+  e_ins[j] = ei;
+}
+
+// section 4.1.1: the cavity of p from its insertion triangle(s); returns its size, or -1 when it exceeds CAVITY_MAX
+static __device__ int cavity_of(double2 p, int8_t kd, int32_t ti, int32_t ei, const double2 *xy, const int32_t *tv, const int32_t *te,
+                                const int32_t *et, int32_t *list, double *acc, double *tmp) {
+  int n = 0;
+  if (kd == KIND_EDGE) { list[n++] = et[2 * (int64_t)ei]; list[n++] = et[2 * (int64_t)ei + 1]; }
+  else list[n++] = ti;
+  for (int head = 0; head < n; ++head) {
+    const int32_t t = list[head];
+    for (int k = 0; k < 3; ++k) {
+      const int32_t nb = across(et, te[3 * (int64_t)t + k], t);
+      if (nb < 0) continue;
+      bool seen = false;
+      for (int q = 0; q < n; ++q) seen |= list[q] == nb;
+      if (seen) continue;
+      const int32_t *v = tv + 3 * (int64_t)nb;
+      const double2 A = xy[v[0]], B = xy[v[1]], C = xy[v[2]];
+      int sg = incircle2d_filter(A, B, C, p);
+      if (sg == 2) sg = incircle2d_exact(A, B, C, p, acc, tmp);
+      if (sg > 0) {
+        if (n == CAVITY_MAX) return -1;
+        list[n++] = nb;
+      }
+    }
+  }
+  return n;
+}
+// pass 1: claim the cavity's triangles; pass 2: selected when every one of them still carries this candidate's priority.
+// Grid-stride with few threads: every thread owns a slice of the expansion scratch.
+template <int PASS>
+__global__ void __launch_bounds__(32)
+cavity_kernel(int64_t nc, const int32_t *__restrict__ cand, int8_t *__restrict__ kind, const double2 *__restrict__ pt,
+              const int32_t *__restrict__ t_ins, const int32_t *__restrict__ e_ins, const double2 *__restrict__ xy,
+              const int32_t *__restrict__ tv, const int32_t *__restrict__ te, const int32_t *__restrict__ et,
+              unsigned long long *__restrict__ claim, unsigned seed, unsigned iteration, int32_t *__restrict__ sel,
+              int32_t *__restrict__ seg, double *__restrict__ scratch) {
+  const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  double *acc = scratch + tid * (2 * MAXE), *tmp = acc + MAXE;
+  int32_t list[CAVITY_MAX];
+  for (int64_t j = tid; j < nc; j += (int64_t)gridDim.x * blockDim.x) {
+    const int8_t kd = kind[j];
+    int n = kd == KIND_NONE ? -1 : cavity_of(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, list, acc, tmp);
+    const unsigned long long pr = priority_of(seed, iteration, (unsigned)cand[j]);
+    if (PASS == 1) {
+      if (n < 0) kind[j] = KIND_NONE;                              // too large (M11) or nothing to insert: waits
+      for (int q = 0; q < n; ++q) atomicMax(claim + list[q], pr);
+    } else {
+      bool mine = n > 0;
+      for (int q = 0; q < n; ++q) mine &= claim[list[q]] == pr;
+      sel[j] = mine ? 1 : 0;
+      seg[j] = (mine && kd == KIND_SEG) ? 1 : 0;
+    }
+  }
+}
+static __device__ __forceinline__ void swap_side(int32_t *et, int32_t e, int32_t from, int32_t to) {
+  int32_t *f = et + 2 * (int64_t)e;
+  f[f[0] == from ? 0 : 1] = to;
+}
+static __device__ __forceinline__ void put3(int32_t *row, int32_t a, int32_t b, int32_t c) { row[0] = a; row[1] = b; row[2] = c; }
+// section 2.4.4 for every selected candidate (oracle/meshgen.py: insert_vertex); rank / segrank: exclusive sums of sel / seg
+__global__ void __launch_bounds__(128)
+insert_kernel(int64_t nc, const int8_t *__restrict__ kind, const double2 *__restrict__ pt, const int32_t *__restrict__ t_ins,
+              const int32_t *__restrict__ e_ins, const int32_t *__restrict__ sel, const int32_t *__restrict__ rank,
+              const int32_t *__restrict__ segrank, int32_t nv, int32_t nt, int32_t ne, double2 *__restrict__ xy,
+              int32_t *__restrict__ tv, int32_t *__restrict__ te, int32_t *__restrict__ et) {
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= nc || !sel[j]) return;
+  const int32_t v = nv + rank[j];
+  const int32_t tn = nt + 2 * rank[j] - segrank[j], en = ne + 3 * rank[j] - segrank[j];   // SEG adds 1 / 2, the others 2 / 3
+  xy[v] = pt[j];
+  const int32_t t = t_ins[j], e = e_ins[j];
+  int32_t *V = tv + 3 * (int64_t)t, *E = te + 3 * (int64_t)t;
+  if (kind[j] == KIND_TRI) {
+    const int32_t a = V[0], b = V[1], c = V[2], e0 = E[0], e1 = E[1], e2 = E[2];
+    const int32_t t1 = tn, t2 = tn + 1, f0 = en, f1 = en + 1, f2 = en + 2;      // f0 = (v, a), f1 = (v, b), f2 = (v, c)
+    put3(V, a, b, v); put3(E, f1, f0, e2);
+    put3(tv + 3 * (int64_t)t1, b, c, v); put3(te + 3 * (int64_t)t1, f2, f1, e0);
+    put3(tv + 3 * (int64_t)t2, c, a, v); put3(te + 3 * (int64_t)t2, f0, f2, e1);
+    et[2 * (int64_t)f0] = t; et[2 * (int64_t)f0 + 1] = t2;
+    et[2 * (int64_t)f1] = t; et[2 * (int64_t)f1 + 1] = t1;
+    et[2 * (int64_t)f2] = t1; et[2 * (int64_t)f2 + 1] = t2;
+    swap_side(et, e0, t, t1);
+    swap_side(et, e1, t, t2);
+    return;
+  }
+  const int i1 = local_of(E, e);
+  const int32_t a = V[i1], b = V[(i1 + 1) % 3], c = V[(i1 + 2) % 3];           // E = (b, c), a opposite
+  const int32_t e_ca = E[(i1 + 1) % 3], e_ab = E[(i1 + 2) % 3];
+  if (kind[j] == KIND_SEG) {
+    const int32_t n1 = tn, g0 = en, g1 = en + 1;                               // E becomes (b, v); g0 = (v, c); g1 = (a, v)
+    put3(V, a, b, v); put3(E, e, g1, e_ab);
+    put3(tv + 3 * (int64_t)n1, a, v, c); put3(te + 3 * (int64_t)n1, g0, e_ca, g1);
+    et[2 * (int64_t)g0] = n1; et[2 * (int64_t)g0 + 1] = -1;
+    et[2 * (int64_t)g1] = t; et[2 * (int64_t)g1 + 1] = n1;
+    swap_side(et, e_ca, t, n1);
+    return;
+  }
+  const int32_t t2 = across(et, e, t);
+  int32_t *V2 = tv + 3 * (int64_t)t2, *E2 = te + 3 * (int64_t)t2;
+  const int i2 = local_of(E2, e);
+  const int32_t d = V2[i2], e_bd = E2[(i2 + 1) % 3], e_dc = E2[(i2 + 2) % 3];
+  const int32_t n1 = tn, n2 = tn + 1, g0 = en, g1 = en + 1, g2 = en + 2;       // g0 = (v, c), g1 = (a, v), g2 = (v, d)
+  put3(V, a, b, v); put3(E, e, g1, e_ab);
+  put3(tv + 3 * (int64_t)n1, a, v, c); put3(te + 3 * (int64_t)n1, g0, e_ca, g1);
+  put3(V2, d, v, b); put3(E2, e, e_bd, g2);
+  put3(tv + 3 * (int64_t)n2, d, c, v); put3(te + 3 * (int64_t)n2, g0, g2, e_dc);
+  et[2 * (int64_t)g0] = n1; et[2 * (int64_t)g0 + 1] = n2;
+  et[2 * (int64_t)g1] = t; et[2 * (int64_t)g1 + 1] = n1;
+  et[2 * (int64_t)g2] = t2; et[2 * (int64_t)g2 + 1] = n2;
+  swap_side(et, e_ca, t, n1);
+  swap_side(et, e_dc, t2, n2);
+}
+// canonical order (reading M12): rotate every triangle to its smallest vertex; sort keys (second, third) and (first)
+__global__ void __launch_bounds__(256)
+canonical_keys_kernel(int64_t nt, int32_t *__restrict__ tv, unsigned long long *__restrict__ key_lo, int32_t *__restrict__ idx) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nt) return;
+  int32_t *v = tv + 3 * t;
+  const int32_t a = v[0], b = v[1], c = v[2];
+  const int r = (a < b && a < c) ? 0 : ((b < a && b < c) ? 1 : 2);
+  const int32_t x = r == 0 ? a : (r == 1 ? b : c), y = r == 0 ? b : (r == 1 ? c : a), z = r == 0 ? c : (r == 1 ? a : b);
+  v[0] = x; v[1] = y; v[2] = z;
+  key_lo[t] = ((unsigned long long)(unsigned)y << 32) | (unsigned)z;
+  idx[t] = (int32_t)t;
+}
+__global__ void __launch_bounds__(256)
+gather_first_kernel(int64_t nt, const int32_t *__restrict__ tv, const int32_t *__restrict__ idx, unsigned *__restrict__ key_hi) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < nt) key_hi[i] = (unsigned)tv[3 * (int64_t)idx[i]];
+}
+__global__ void __launch_bounds__(256)
+gather_rows_kernel(int64_t nt, const int32_t *__restrict__ src, const int32_t *__restrict__ idx, int32_t *__restrict__ dst) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nt) return;
+  const int32_t *s = src + 3 * (int64_t)idx[i];
+  dst[3 * i] = s[0]; dst[3 * i + 1] = s[1]; dst[3 * i + 2] = s[2];
+}
+
 }  // namespace mrdgen
 
 extern "C" {
@@ -433,47 +719,126 @@ int mrd_meshgen_incircle2d(int64_t n, const double *xy_dev, const int32_t *idx_d
   return predicate_impl(1, n, xy_dev, idx_dev, sign_dev, n_exact, stream);
 }
 
+namespace {
+// work space of build_edges for n = 3 * triangles entries
+struct EdgeWork {
+  size_t o_k0, o_k1, o_v0, o_v1, o_head, o_incl, o_err, o_tmp, tmp_sort, tmp_scan;
+  void plan(Carve &c, int64_t n, cudaStream_t s) {
+    tmp_sort = tmp_scan = 0;
+    cub::DeviceRadixSort::SortPairs(nullptr, tmp_sort, (unsigned long long *)nullptr, (unsigned long long *)nullptr, (int32_t *)nullptr,
+                                    (int32_t *)nullptr, n, 0, 64, s);
+    cub::DeviceScan::InclusiveSum(nullptr, tmp_scan, (int32_t *)nullptr, (int32_t *)nullptr, n, s);
+    o_k0 = c.add(sizeof(unsigned long long) * n);
+    o_k1 = c.add(sizeof(unsigned long long) * n);
+    o_v0 = c.add(sizeof(int32_t) * n);
+    o_v1 = c.add(sizeof(int32_t) * n);
+    o_head = c.add(sizeof(int32_t) * n);
+    o_incl = c.add(sizeof(int32_t) * n);
+    o_err = c.add(sizeof(int));
+    o_tmp = c.add(std::max(tmp_sort, tmp_scan));
+  }
+};
+// te, et from tv (arena reserved and locked by the caller); synchronises s
+int build_edges_run(const EdgeWork &w, int64_t n_triangle, const int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_edge, cudaStream_t s) {
+  const int64_t n = 3 * n_triangle;
+  char *b = g_arena.base;
+  unsigned long long *k0 = (unsigned long long *)(b + w.o_k0), *k1 = (unsigned long long *)(b + w.o_k1);
+  int32_t *v0 = (int32_t *)(b + w.o_v0), *v1 = (int32_t *)(b + w.o_v1), *head = (int32_t *)(b + w.o_head), *incl = (int32_t *)(b + w.o_incl);
+  int *err = (int *)(b + w.o_err);
+  const unsigned nb = (unsigned)((n + 255) / 256);
+  size_t tmp_sort = w.tmp_sort, tmp_scan = w.tmp_scan;
+  cudaMemsetAsync(err, 0, sizeof(int), s);
+  cudaMemsetAsync(et_dev, 0xFF, sizeof(int32_t) * 2 * (size_t)n, s);   // -1: no second triangle
+  mrdgen::edge_keys_kernel<<<nb, 256, 0, s>>>(n, tv_dev, k0, v0);
+  // (vertex numbers are below 2^31: the keys have 63 significant bits)
+  cub::DeviceRadixSort::SortPairs(b + w.o_tmp, tmp_sort, k0, k1, v0, v1, n, 0, 63, s);
+  mrdgen::edge_heads_kernel<<<nb, 256, 0, s>>>(n, k1, head);
+  cub::DeviceScan::InclusiveSum(b + w.o_tmp, tmp_scan, head, incl, n, s);
+  mrdgen::edge_fill_kernel<<<nb, 256, 0, s>>>(n, k1, v1, incl, te_dev, et_dev, err);
+  int32_t *h = (int32_t *)g_arena.pinned;
+  cudaMemcpyAsync(h, err, sizeof(int), cudaMemcpyDeviceToHost, s);
+  cudaMemcpyAsync(h + 1, incl + (n - 1), sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+  cudaError_t e = cudaStreamSynchronize(s);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("build_edges", e);
+  if (h[0]) return gen_fail(MRD_EINVAL, "build_edges: an edge belongs to more than two triangles");
+  *n_edge = h[1];
+  return MRD_OK;
+}
+
+// work space of the flip loop for up to nt triangles and ne edges
+struct FlipWork {
+  size_t o_cnt, o_state, o_lock, o_mark, o_l0, o_l1, o_work, o_scr;
+  void plan(Carve &c, size_t nt, size_t ne, bool with_scratch) {
+    o_cnt = c.add(sizeof(mrdgen::FlipCounters));
+    o_state = c.add(ne);
+    o_lock = c.add(sizeof(unsigned long long) * nt);
+    o_mark = c.add(sizeof(int32_t) * ne);
+    o_l0 = c.add(sizeof(int32_t) * ne);
+    o_l1 = c.add(sizeof(int32_t) * ne);
+    o_work = c.add(sizeof(int32_t) * ne);
+    o_scr = with_scratch ? c.add(EXACT_SCRATCH) : 0;
+  }
+};
+// flips (tv, te, et) to the Delaunay triangulation (arena reserved and locked by the caller); synchronises s every iteration
+int flip_run(const FlipWork &w, size_t o_scratch, int64_t n_triangle, int64_t n_edge, const double2 *xy, int32_t *tv_dev, int32_t *te_dev,
+             int32_t *et_dev, int64_t *flips_out, int64_t *iters_out, int64_t *exact_out, cudaStream_t s) {
+  using mrdgen::FlipCounters;
+  const size_t nt = (size_t)std::max<int64_t>(n_triangle, 1), ne = (size_t)n_edge;
+  char *b = g_arena.base;
+  FlipCounters *cnt = (FlipCounters *)(b + w.o_cnt);
+  int8_t *state = (int8_t *)(b + w.o_state);
+  unsigned long long *lock = (unsigned long long *)(b + w.o_lock);
+  int32_t *mark = (int32_t *)(b + w.o_mark), *list[2] = {(int32_t *)(b + w.o_l0), (int32_t *)(b + w.o_l1)}, *work = (int32_t *)(b + w.o_work);
+  double *scratch = (double *)(b + o_scratch);
+  static_assert(sizeof(FlipCounters) <= 16 * sizeof(unsigned long long), "pinned block too small");
+  const FlipCounters *h = (const FlipCounters *)g_arena.pinned;
+  int64_t flips = 0, iters = 0, exact = 0;
+  cudaMemsetAsync(state, 0, ne, s);
+  cudaMemsetAsync(lock, 0, sizeof(unsigned long long) * nt, s);
+  cudaMemsetAsync(mark, 0, sizeof(int32_t) * ne, s);
+  int64_t n = n_edge;
+  const int32_t *cand = nullptr;                                 // first iteration: every edge
+  for (int32_t iter = 1;; ++iter) {
+    if (iter > 100000) return gen_fail(MRD_EINVAL, "delaunay_flip: no convergence (is the input a valid triangulation?)");
+    const unsigned long long stamp = (unsigned long long)iter << 32;
+    int32_t *next = list[iter & 1];
+    const unsigned nb = (unsigned)((n + 255) / 256);
+    cudaMemsetAsync(cnt, 0, sizeof(FlipCounters), s);
+    mrdgen::check_edge_kernel<<<nb, 256, 0, s>>>(n, cand, xy, tv_dev, te_dev, et_dev, state, lock, stamp, work, cnt);
+    mrdgen::check_edge_exact_kernel<<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(work, xy, tv_dev, te_dev, et_dev, state, lock, stamp, cnt, scratch);
+    mrdgen::flip_kernel<<<nb, 256, 0, s>>>(n, cand, tv_dev, te_dev, et_dev, state, lock, stamp, iter, mark, next, cnt);
+    cudaError_t e = cudaMemcpyAsync(g_arena.pinned, cnt, sizeof(FlipCounters), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail("delaunay_flip", e);
+    iters++;
+    flips += (int64_t)h->n_flip;
+    exact += (int64_t)h->n_exact;
+    if (h->n_bad == 0) break;                                    // every edge is locally Delaunay
+    cand = next;
+    n = (int64_t)h->n_next;
+  }
+  if (flips_out) *flips_out = flips;
+  if (iters_out) *iters_out = iters;
+  if (exact_out) *exact_out = exact;
+  return MRD_OK;
+}
+}  // namespace
+
 int mrd_meshgen_build_edges(int64_t n_triangle, const int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_edge, void *stream) {
   if (n_triangle < 0 || !n_edge || (n_triangle > 0 && (!tv_dev || !te_dev || !et_dev))) return gen_fail(MRD_EINVAL, "null argument");
   if (3 * n_triangle > 0x7FFFFFF0ll) return gen_fail(MRD_EINVAL, "too many triangles for 32-bit edge numbers");
   *n_edge = 0;
   if (n_triangle == 0) return MRD_OK;
   cudaStream_t s = (cudaStream_t)stream;
-  const int64_t n = 3 * n_triangle;
-  size_t tmp_sort = 0, tmp_scan = 0;
-  cub::DeviceRadixSort::SortPairs(nullptr, tmp_sort, (unsigned long long *)nullptr, (unsigned long long *)nullptr, (int32_t *)nullptr,
-                                  (int32_t *)nullptr, n, 0, 64, s);
-  cub::DeviceScan::InclusiveSum(nullptr, tmp_scan, (int32_t *)nullptr, (int32_t *)nullptr, n, s);
   Carve c;
-  const size_t o_k0 = c.add(sizeof(unsigned long long) * n), o_k1 = c.add(sizeof(unsigned long long) * n);
-  const size_t o_v0 = c.add(sizeof(int32_t) * n), o_v1 = c.add(sizeof(int32_t) * n);
-  const size_t o_head = c.add(sizeof(int32_t) * n), o_incl = c.add(sizeof(int32_t) * n), o_err = c.add(sizeof(int));
-  const size_t o_tmp = c.add(std::max(tmp_sort, tmp_scan));
+  EdgeWork w;
+  w.plan(c, 3 * n_triangle, s);
   std::lock_guard<std::mutex> g(g_arena.mu);
   cudaError_t e = g_arena.reserve(c.total);
   if (e != cudaSuccess) return cuda_fail("build_edges", e);
-  char *b = g_arena.base;
-  unsigned long long *k0 = (unsigned long long *)(b + o_k0), *k1 = (unsigned long long *)(b + o_k1);
-  int32_t *v0 = (int32_t *)(b + o_v0), *v1 = (int32_t *)(b + o_v1), *head = (int32_t *)(b + o_head), *incl = (int32_t *)(b + o_incl);
-  int *err = (int *)(b + o_err);
-  const unsigned nb = (unsigned)((n + 255) / 256);
-  cudaMemsetAsync(err, 0, sizeof(int), s);
-  cudaMemsetAsync(et_dev, 0xFF, sizeof(int32_t) * 2 * (size_t)n, s);   // -1: no second triangle
-  mrdgen::edge_keys_kernel<<<nb, 256, 0, s>>>(n, tv_dev, k0, v0);
-  // (vertex numbers are below 2^31: the keys have 63 significant bits)
-  cub::DeviceRadixSort::SortPairs(b + o_tmp, tmp_sort, k0, k1, v0, v1, n, 0, 63, s);
-  mrdgen::edge_heads_kernel<<<nb, 256, 0, s>>>(n, k1, head);
-  cub::DeviceScan::InclusiveSum(b + o_tmp, tmp_scan, head, incl, n, s);
-  mrdgen::edge_fill_kernel<<<nb, 256, 0, s>>>(n, k1, v1, incl, te_dev, et_dev, err);
-  int32_t *h = (int32_t *)g_arena.pinned;
-  cudaMemcpyAsync(h, err, sizeof(int), cudaMemcpyDeviceToHost, s);
-  cudaMemcpyAsync(h + 1, incl + (n - 1), sizeof(int32_t), cudaMemcpyDeviceToHost, s);
-  e = cudaStreamSynchronize(s);
-  if (e == cudaSuccess) e = cudaGetLastError();
-  if (e != cudaSuccess) return cuda_fail("build_edges", e);
-  if (h[0]) return gen_fail(MRD_EINVAL, "build_edges: an edge belongs to more than two triangles");
-  *n_edge = h[1];
-  return MRD_OK;
+  return build_edges_run(w, n_triangle, tv_dev, te_dev, et_dev, n_edge, s);
 }
 
 int mrd_meshgen_delaunay_flip(int64_t n_triangle, int64_t n_edge, const double *xy_dev, int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev,
@@ -485,55 +850,136 @@ int mrd_meshgen_delaunay_flip(int64_t n_triangle, int64_t n_edge, const double *
   if (n_iterations) *n_iterations = 0;
   if (n_exact) *n_exact = 0;
   if (n_edge == 0) return MRD_OK;
-  using mrdgen::FlipCounters;
   cudaStream_t s = (cudaStream_t)stream;
-  const size_t nt = (size_t)std::max<int64_t>(n_triangle, 1), ne = (size_t)n_edge;
   Carve c;
-  const size_t o_cnt = c.add(sizeof(FlipCounters)), o_state = c.add(ne), o_lock = c.add(sizeof(unsigned long long) * nt);
-  const size_t o_mark = c.add(sizeof(int32_t) * ne), o_l0 = c.add(sizeof(int32_t) * ne), o_l1 = c.add(sizeof(int32_t) * ne);
-  const size_t o_work = c.add(sizeof(int32_t) * ne), o_scr = c.add(EXACT_SCRATCH);
+  FlipWork w;
+  w.plan(c, (size_t)std::max<int64_t>(n_triangle, 1), (size_t)n_edge, true);
   std::lock_guard<std::mutex> g(g_arena.mu);
   cudaError_t e = g_arena.reserve(c.total);
   if (e != cudaSuccess) return cuda_fail("delaunay_flip", e);
+  return flip_run(w, w.o_scr, n_triangle, n_edge, (const double2 *)xy_dev, tv_dev, te_dev, et_dev, n_flips, n_iterations, n_exact, s);
+}
+
+int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteration, int64_t max_iterations, int64_t cap_vertex,
+                       int64_t cap_triangle, int64_t cap_edge, int64_t *n_vertex, int64_t *n_triangle, int64_t *n_edge, double *xy_dev,
+                       int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_iterations, int64_t *n_bad_left, void *stream) {
+  if (!n_vertex || !n_triangle || !n_edge || !xy_dev || !tv_dev || !te_dev || !et_dev) return gen_fail(MRD_EINVAL, "null argument");
+  if (!(R > 0.0) || !(B > 0.0)) return gen_fail(MRD_EINVAL, "R and B must be positive");
+  int64_t nv = *n_vertex, nt = *n_triangle, ne = *n_edge;
+  if (nv < 3 || nt < 1 || ne < 3 || nv > cap_vertex || nt > cap_triangle || ne > cap_edge || first_iteration < 0 || max_iterations < 0)
+    return gen_fail(MRD_EINVAL, "refine: sizes out of range");
+  if (cap_edge > 0x7FFFFFF0ll / 2 || 3 * cap_triangle > 0x7FFFFFF0ll) return gen_fail(MRD_EINVAL, "refine: capacity beyond 32-bit numbering");
+  if (cap_edge < 3 * cap_triangle) return gen_fail(MRD_EINVAL, "refine: et must hold 3 * cap_triangle pairs (mrd_meshgen_build_edges writes that many)");
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t ct = (size_t)cap_triangle, ce = (size_t)cap_edge;
+  Carve c;
+  EdgeWork ew;
+  ew.plan(c, 3 * cap_triangle, s);
+  FlipWork fw;
+  fw.plan(c, ct, ce, false);
+  const size_t o_scr = c.add(EXACT_SCRATCH);
+  const size_t o_cnt = c.add(sizeof(unsigned long long)), o_err = c.add(sizeof(int)), o_nsel = c.add(sizeof(int32_t));
+  const size_t o_r = c.add(sizeof(double) * ct), o_beta = c.add(sizeof(double) * ct), o_cc = c.add(sizeof(double2) * ct), o_bad = c.add(ct);
+  const size_t o_cand = c.add(sizeof(int32_t) * ct), o_kind = c.add(ct), o_pt = c.add(sizeof(double2) * ct);
+  const size_t o_tins = c.add(sizeof(int32_t) * ct), o_eins = c.add(sizeof(int32_t) * ct), o_claim = c.add(sizeof(unsigned long long) * ct);
+  const size_t o_sel = c.add(sizeof(int32_t) * ct), o_seg = c.add(sizeof(int32_t) * ct), o_rank = c.add(sizeof(int32_t) * ct), o_srank = c.add(sizeof(int32_t) * ct);
+  const size_t o_klo0 = c.add(sizeof(unsigned long long) * ct), o_klo1 = c.add(sizeof(unsigned long long) * ct);
+  const size_t o_khi0 = c.add(sizeof(unsigned) * ct), o_khi1 = c.add(sizeof(unsigned) * ct);
+  const size_t o_i0 = c.add(sizeof(int32_t) * ct), o_i1 = c.add(sizeof(int32_t) * ct), o_tv2 = c.add(sizeof(int32_t) * 3 * ct);
+  size_t tmp_sel = 0, tmp_scan = 0, tmp_s64 = 0, tmp_s32 = 0;
+  cub::DeviceSelect::Flagged(nullptr, tmp_sel, thrust::counting_iterator<int32_t>(0), (const uint8_t *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, s);
+  cub::DeviceScan::ExclusiveSum(nullptr, tmp_scan, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, s);
+  cub::DeviceRadixSort::SortPairs(nullptr, tmp_s64, (unsigned long long *)nullptr, (unsigned long long *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, 0, 64, s);
+  cub::DeviceRadixSort::SortPairs(nullptr, tmp_s32, (unsigned *)nullptr, (unsigned *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, 0, 32, s);
+  const size_t o_tmp = c.add(std::max(std::max(tmp_sel, tmp_scan), std::max(tmp_s64, tmp_s32)));
+  std::lock_guard<std::mutex> g(g_arena.mu);
+  cudaError_t e = g_arena.reserve(c.total);
+  if (e != cudaSuccess) return cuda_fail("refine", e);
   char *b = g_arena.base;
-  FlipCounters *cnt = (FlipCounters *)(b + o_cnt);
-  int8_t *state = (int8_t *)(b + o_state);
-  unsigned long long *lock = (unsigned long long *)(b + o_lock);
-  int32_t *mark = (int32_t *)(b + o_mark), *list[2] = {(int32_t *)(b + o_l0), (int32_t *)(b + o_l1)}, *work = (int32_t *)(b + o_work);
-  double *scratch = (double *)(b + o_scr);
-  static_assert(sizeof(FlipCounters) <= 16 * sizeof(unsigned long long), "pinned block too small");
-  const FlipCounters *h = (const FlipCounters *)g_arena.pinned;
-  int64_t flips = 0, iters = 0, exact = 0;
-  cudaMemsetAsync(state, 0, ne, s);
-  cudaMemsetAsync(lock, 0, sizeof(unsigned long long) * nt, s);
-  cudaMemsetAsync(mark, 0, sizeof(int32_t) * ne, s);
-  int64_t n = n_edge;
-  const int32_t *cand = nullptr;                                 // first iteration: every edge
-  const double2 *xy = (const double2 *)xy_dev;
-  for (int32_t iter = 1;; ++iter) {
-    if (iter > 100000) return gen_fail(MRD_EINVAL, "delaunay_flip: no convergence (is the input a valid triangulation?)");
-    const unsigned long long stamp = (unsigned long long)iter << 32;
-    int32_t *next = list[iter & 1];
-    const unsigned nb = (unsigned)((n + 255) / 256);
-    cudaMemsetAsync(cnt, 0, sizeof(FlipCounters), s);
-    mrdgen::check_edge_kernel<<<nb, 256, 0, s>>>(n, cand, xy, tv_dev, te_dev, et_dev, state, lock, stamp, work, cnt);
-    mrdgen::check_edge_exact_kernel<<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(work, xy, tv_dev, te_dev, et_dev, state, lock, stamp, cnt, scratch);
-    mrdgen::flip_kernel<<<nb, 256, 0, s>>>(n, cand, tv_dev, te_dev, et_dev, state, lock, stamp, iter, mark, next, cnt);
-    e = cudaMemcpyAsync(g_arena.pinned, cnt, sizeof(FlipCounters), cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    if (e == cudaSuccess) e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail("delaunay_flip", e);
-    iters++;
-    flips += (int64_t)h->n_flip;
-    exact += (int64_t)h->n_exact;
-    if (h->n_bad == 0) break;                                    // every edge is locally Delaunay
-    cand = next;
-    n = (int64_t)h->n_next;
+  unsigned long long *cnt = (unsigned long long *)(b + o_cnt), *claim = (unsigned long long *)(b + o_claim);
+  int *err = (int *)(b + o_err);
+  int32_t *d_nsel = (int32_t *)(b + o_nsel);
+  double *r = (double *)(b + o_r), *beta = (double *)(b + o_beta), *scratch = (double *)(b + o_scr);
+  double2 *cc = (double2 *)(b + o_cc), *pt = (double2 *)(b + o_pt), *xy = (double2 *)xy_dev;
+  uint8_t *bad = (uint8_t *)(b + o_bad);
+  int8_t *kind = (int8_t *)(b + o_kind);
+  int32_t *cand = (int32_t *)(b + o_cand), *tins = (int32_t *)(b + o_tins), *eins = (int32_t *)(b + o_eins);
+  int32_t *sel = (int32_t *)(b + o_sel), *seg = (int32_t *)(b + o_seg), *rank = (int32_t *)(b + o_rank), *srank = (int32_t *)(b + o_srank);
+  unsigned long long *klo0 = (unsigned long long *)(b + o_klo0), *klo1 = (unsigned long long *)(b + o_klo1);
+  unsigned *khi0 = (unsigned *)(b + o_khi0), *khi1 = (unsigned *)(b + o_khi1);
+  int32_t *i0 = (int32_t *)(b + o_i0), *i1 = (int32_t *)(b + o_i1), *tv2 = (int32_t *)(b + o_tv2);
+  void *tmp = b + o_tmp;
+  volatile unsigned long long *hp = g_arena.pinned;
+  auto sync = [&](const char *what) -> int {
+    cudaError_t e2 = cudaStreamSynchronize(s);
+    if (e2 == cudaSuccess) e2 = cudaGetLastError();
+    return e2 == cudaSuccess ? MRD_OK : cuda_fail(what, e2);
+  };
+  int64_t done = 0, left = 0;
+  int rc = MRD_OK;
+  for (int64_t it = 0;; ++it) {
+    // 2.4.1: bad triangles and their circumcentres
+    cudaMemsetAsync(cnt, 0, sizeof *cnt, s);
+    mrdgen::test_quality_kernel<<<(unsigned)((nt + 255) / 256), 256, 0, s>>>(nt, xy, tv_dev, R, B, r, beta, cc, bad, cnt);
+    cudaMemcpyAsync((void *)hp, cnt, sizeof *cnt, cudaMemcpyDeviceToHost, s);
+    if ((rc = sync("refine: test_quality")) != MRD_OK) return rc;
+    const int64_t nc = (int64_t)hp[0];
+    left = nc;
+    if (nc == 0 || it >= max_iterations) break;
+    // candidates in ascending order of their bad triangle; 2.4.2-2.4.3
+    size_t tb = tmp_sel;
+    cub::DeviceSelect::Flagged(tmp, tb, thrust::counting_iterator<int32_t>(0), (const uint8_t *)bad, cand, d_nsel, nt, s);
+    cudaMemsetAsync(err, 0, sizeof(int), s);
+    mrdgen::candidate_kernel<<<(unsigned)((nc + 127) / 128), 128, 0, s>>>(nc, cand, cc, nt + 16, xy, tv_dev, te_dev, et_dev, kind, pt, tins, eins, err);
+    // 4.1.1: cavities, claims, selection
+    cudaMemsetAsync(claim, 0, sizeof(unsigned long long) * (size_t)nt, s);
+    const unsigned itn = (unsigned)(first_iteration + it);
+    mrdgen::cavity_kernel<1><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch);
+    mrdgen::cavity_kernel<2><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch);
+    tb = tmp_scan;
+    cub::DeviceScan::ExclusiveSum(tmp, tb, sel, rank, nc, s);
+    tb = tmp_scan;
+    cub::DeviceScan::ExclusiveSum(tmp, tb, seg, srank, nc, s);
+    int32_t *h32 = (int32_t *)hp;
+    cudaMemcpyAsync(h32 + 0, err, sizeof(int), cudaMemcpyDeviceToHost, s);
+    cudaMemcpyAsync(h32 + 1, rank + (nc - 1), sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+    cudaMemcpyAsync(h32 + 2, sel + (nc - 1), sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+    cudaMemcpyAsync(h32 + 3, srank + (nc - 1), sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+    cudaMemcpyAsync(h32 + 4, seg + (nc - 1), sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+    if ((rc = sync("refine: candidates")) != MRD_OK) return rc;
+    if (h32[0]) return gen_fail(MRD_EINVAL, "refine: a point-location walk did not end (the input is not a Delaunay triangulation)");
+    const int64_t nsel = (int64_t)h32[1] + h32[2], nseg = (int64_t)h32[3] + h32[4];
+    if (nsel == 0) return gen_fail(MRD_EINVAL, "refine: bad triangles remain but no vertex can be inserted (cavities beyond 64 triangles or circumcentres on vertices)");
+    const int64_t nv2 = nv + nsel, nt2 = nt + 2 * nsel - nseg, ne2 = ne + 3 * nsel - nseg;
+    if (nv2 > cap_vertex || nt2 > cap_triangle || ne2 > cap_edge) {
+      rc = gen_fail(MRD_ENOMEM, "refine: capacity of the mesh arrays reached (the mesh is valid and Delaunay; call again with larger arrays)");
+      break;
+    }
+    // 2.4.4: insert; 2.4.6: flips
+    mrdgen::insert_kernel<<<(unsigned)((nc + 127) / 128), 128, 0, s>>>(nc, kind, pt, tins, eins, sel, rank, srank, (int32_t)nv, (int32_t)nt, (int32_t)ne, xy, tv_dev, te_dev, et_dev);
+    nv = nv2; nt = nt2; ne = ne2;
+    if ((rc = flip_run(fw, o_scr, nt, ne, xy, tv_dev, te_dev, et_dev, nullptr, nullptr, nullptr, s)) != MRD_OK) return rc;
+    // canonical order (M12) and the edge arrays that go with it
+    const unsigned nbt = (unsigned)((nt + 255) / 256);
+    mrdgen::canonical_keys_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, klo0, i0);
+    tb = tmp_s64;
+    cub::DeviceRadixSort::SortPairs(tmp, tb, klo0, klo1, i0, i1, nt, 0, 64, s);
+    mrdgen::gather_first_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, i1, khi0);
+    tb = tmp_s32;
+    cub::DeviceRadixSort::SortPairs(tmp, tb, khi0, khi1, i1, i0, nt, 0, 32, s);
+    mrdgen::gather_rows_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, i0, tv2);
+    cudaMemcpyAsync(tv_dev, tv2, sizeof(int32_t) * 3 * (size_t)nt, cudaMemcpyDeviceToDevice, s);
+    int64_t ne_built = 0;
+    if ((rc = build_edges_run(ew, nt, tv_dev, te_dev, et_dev, &ne_built, s)) != MRD_OK) return rc;
+    if (ne_built != ne) return gen_fail(MRD_EINVAL, "refine: edge count changed under renumbering (internal error)");
+    done++;
   }
-  if (n_flips) *n_flips = flips;
-  if (n_iterations) *n_iterations = iters;
-  if (n_exact) *n_exact = exact;
-  return MRD_OK;
+  *n_vertex = nv;
+  *n_triangle = nt;
+  *n_edge = ne;
+  if (n_iterations) *n_iterations = done;
+  if (n_bad_left) *n_bad_left = left;
+  return rc;
 }
 
 int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_t *t0_dev, int64_t n_triangle, const double *xy_dev,

@@ -1,0 +1,156 @@
+"""GPU parity of the Delaunay refinement (section 2.3-2.4, 4.1.1) against oracle/meshgen.py: refine.
+Integer and index work with IEEE-exact coordinates: the refined mesh must be the oracle's ARRAY FOR ARRAY (vertex coordinates
+bit for bit, triangleVertices, triangleEdges, edgeTriangles) -- iteration by iteration and for the whole run -- because every
+decision is exact (ORIENT2D, INCIRCLE2D), prescribed (eq. 2 and eq. 4 one IEEE operation at a time) or an integer rule
+(priorities, numbering, canonical order).  At sizes beyond the oracle: the guarantees of section 2.3 and the library
+triangulation of the final vertex set."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from oracle import meshgen as mg
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mrdb():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_1705_02028_b200.binding as b
+    return b
+
+
+def dev(a, dtype):
+    import torch
+    return torch.tensor(np.ascontiguousarray(a), dtype=dtype, device="cuda")
+
+
+def start(seed, shape):
+    m = wl.scrambled_triangulation(*shape, seed=seed)
+    tv = mg.canonical_order(mg.delaunay_flip(m.xy, m.tri)[0])
+    te, et = mg.build_edges(tv)
+    return m.xy, tv, te, et
+
+
+def to_dev(xy, tv, te, et):
+    import torch
+    return dev(xy, torch.float64), dev(tv, torch.int32), dev(te, torch.int32), dev(et, torch.int32)
+
+
+def same(g, o):
+    return all(np.array_equal(a.cpu().numpy(), b) for a, b in zip(g, o))
+
+
+@pytest.mark.parametrize("B,R,seed,shape", [(1.0, 0.09, 1, (6, 5)), (np.sqrt(2.0), 0.05, 2, (6, 5)), (1.2, 0.04, 3, (9, 7))])
+def test_every_iteration_and_the_whole_run_match_the_oracle(mrdb, B, R, seed, shape):
+    xy, tv, te, et = start(seed, shape)
+    state = (xy, tv, te, et)
+    kinds = np.zeros(4, dtype=int)
+    for it in range(100):                                          # iteration by iteration, from the oracle's state
+        o = mg.refine_iteration(*state, R, B, seed, it)
+        g = mrdb.meshgen_refine(*to_dev(*state), R, B, seed=seed, first_iteration=it, max_iterations=1)
+        assert same(g[:4], o[:4]), it
+        assert g[4]["iterations"] == (1 if o[4]["n_bad"] else 0)
+        kinds += np.bincount(o[4]["kinds"], minlength=4)
+        if o[4]["n_bad"] == 0:
+            assert g[4]["bad_left"] == 0
+            break
+        state = o[:4]
+    assert it >= 4 and kinds[mg.KIND_TRI] > 20 and kinds[mg.KIND_SEG] > 5     # both common kinds of insertion were exercised
+    g = mrdb.meshgen_refine(*to_dev(xy, tv, te, et), R, B, seed=seed)          # free-running
+    assert same(g[:4], state) and g[4] == dict(iterations=it, bad_left=0)
+    assert g[0].shape[0] > 3 * xy.shape[0]
+
+
+def test_edge_insertions_on_a_uniform_mesh(mrdb):
+    """Right isosceles triangles: every circumcentre is the midpoint of a hypotenuse -- on an interior edge (KIND_EDGE) or on a
+    segment -- and every interior edge has four cocircular vertices (all INCIRCLE2D tests take the exact path)."""
+    m = wl.uniform_mesh(5, 4, 2.0, 1.5, periodic=False)
+    tv = mg.canonical_order(m.tri)
+    te, et = mg.build_edges(tv)
+    state = (m.xy, tv, te, et)
+    seen = np.zeros(4, dtype=int)
+    for it in range(3):
+        o = mg.refine_iteration(*state, 0.12, 0.6, 5, it)
+        g = mrdb.meshgen_refine(*to_dev(*state), 0.12, 0.6, seed=5, first_iteration=it, max_iterations=1)
+        assert same(g[:4], o[:4]), it
+        seen += np.bincount(o[4]["kinds"], minlength=4)
+        state = o[:4]
+    assert seen[mg.KIND_EDGE] > 5
+
+
+def test_refinement_at_size_keeps_the_guarantees_of_section_2_3(mrdb):
+    """40 x 30 cells refined to ~10^5 vertices (beyond the sequential oracle): no bad triangle, no angle below arcsin(1 / 2B),
+    THE Delaunay triangulation of its vertices (library), same domain, input vertices kept, no encroached segment."""
+    import torch
+    from scipy.spatial import Delaunay
+    m = wl.scrambled_triangulation(40, 30, seed=4)
+    xy, tv = dev(m.xy, torch.float64), dev(m.tri, torch.int32)
+    te, et = mrdb.meshgen_build_edges(tv)
+    mrdb.meshgen_delaunay_flip(xy, tv, te, et)
+    B, R = np.sqrt(2.0), 0.004
+    gx, gt, gte, get, info = mrdb.meshgen_refine(xy, tv, te, et, R, B, seed=9, cap_vertex=400000)
+    assert info["bad_left"] == 0 and 10 < info["iterations"] < 200
+    X, T, TE, ET = gx.cpu().numpy(), gt.cpu().numpy(), gte.cpu().numpy(), get.cpu().numpy()
+    assert X.shape[0] > 50000 and np.array_equal(X[:m.nv], m.xy)
+    q = mg.test_quality(X, T, R, B)
+    assert q["bad"].sum() == 0
+    p = X[T]
+    ang = []
+    for k in range(3):
+        u, v = p[:, (k + 1) % 3] - p[:, k], p[:, (k + 2) % 3] - p[:, k]
+        ang.append(np.arccos(np.clip((u * v).sum(1) / np.hypot(*u.T) / np.hypot(*v.T), -1, 1)))
+    assert np.min(ang) >= np.arcsin(1 / (2 * B)) - 1e-9
+    area = 0.5 * ((p[:, 1, 0] - p[:, 0, 0]) * (p[:, 2, 1] - p[:, 0, 1]) - (p[:, 1, 1] - p[:, 0, 1]) * (p[:, 2, 0] - p[:, 0, 0]))
+    assert (area > 0).all() and abs(area.sum() - 3.0) < 1e-10
+    lib = Delaunay(X).simplices.astype(np.int32)
+    pl = X[lib]
+    cw = (pl[:, 0, 0] - pl[:, 2, 0]) * (pl[:, 1, 1] - pl[:, 2, 1]) - (pl[:, 0, 1] - pl[:, 2, 1]) * (pl[:, 1, 0] - pl[:, 2, 0]) < 0
+    lib[cw] = lib[cw][:, [0, 2, 1]]
+    r = np.argmin(lib, axis=1)
+    lib = np.stack([lib[np.arange(len(lib)), (r + j) % 3] for j in range(3)], axis=1)
+    lib = lib[np.lexsort((lib[:, 2], lib[:, 1], lib[:, 0]))]
+    # All edges locally Delaunay <=> Delaunay (L100): the exact INCIRCLE2D of every interior edge (the predicate kernel, itself
+    # under parity in test_gpu_meshgen.py; a sample again through the oracle's rational arithmetic).  The library triangulation
+    # (Qhull: floating-point with tolerances, and this vertex set has exactly cocircular quadruples and thousands of collinear
+    # boundary points, where the Delaunay triangulation is not unique, L96) must agree on all but a few triangles.
+    lib_set = set(map(tuple, lib.tolist()))
+    extra = [t for t, row in enumerate(T.tolist()) if tuple(row) not in lib_set]
+    assert len(lib) == len(T) and len(extra) < 0.005 * len(T)
+    inner = np.nonzero(ET[:, 1] >= 0)[0]
+    t1, t2 = ET[inner, 0], ET[inner, 1]
+    k2 = (TE[t2] == inner[:, None]).argmax(axis=1)
+    quads = np.concatenate([T[t1], T[t2, k2][:, None]], axis=1).astype(np.int32)
+    sgn, _ = mrdb.meshgen_incircle2d(gx, dev(quads, torch.int32))
+    assert (sgn <= 0).all().item()
+    rng = np.random.default_rng(3)
+    for qd in quads[rng.choice(len(quads), 300, replace=False)]:
+        assert mg.incircle2d(*X[qd]) <= 0
+    seg = np.nonzero(ET[:, 1] < 0)[0]
+    tri_of = ET[seg, 0]
+    k = (TE[tri_of] == seg[:, None]).argmax(axis=1)
+    u, w = T[tri_of, (k + 1) % 3], T[tri_of, (k + 2) % 3]
+    on = np.unique(np.concatenate([u, w]))
+    assert (np.isin(X[on, 0], [0.0, 2.0]) | np.isin(X[on, 1], [0.0, 1.5])).all()
+    mid, rad = 0.5 * (X[u] + X[w]), 0.5 * np.hypot(*(X[u] - X[w]).T)
+    near = X[(X[:, 0] < 0.05) | (X[:, 0] > 1.95) | (X[:, 1] < 0.05) | (X[:, 1] > 1.45)]     # only vertices near the sides can encroach
+    d = np.hypot(near[:, None, 0] - mid[None, :, 0], near[:, None, 1] - mid[None, :, 1])
+    assert (d >= rad[None, :] * (1 - 1e-12)).all()
+    # deterministic
+    g2 = mrdb.meshgen_refine(xy, tv, te, et, R, B, seed=9, cap_vertex=400000)
+    assert all(torch.equal(a, b) for a, b in zip((gx, gt, gte, get), g2[:4]))
+
+
+def test_capacity_and_bad_input_are_reported(mrdb):
+    xy, tv, te, et = start(1, (6, 5))
+    d = to_dev(xy, tv, te, et)
+    with pytest.raises(mrdb.MrdError) as ex:
+        mrdb.meshgen_refine(*d, 0.02, 1.0, cap_vertex=xy.shape[0] + 20)
+    assert ex.value.code == mrdb.MRD_ENOMEM
+    g = mrdb.meshgen_refine(*d, 0.5, 10.0)                         # nothing is bad: nothing happens
+    assert g[4] == dict(iterations=0, bad_left=0) and same(g[:4], (xy, tv, te, et))
+    g = mrdb.meshgen_refine(*d, 0.05, 1.0, max_iterations=2)       # stopped early: still a valid mesh, and says what is left
+    assert g[4]["iterations"] == 2 and g[4]["bad_left"] > 0
+    with pytest.raises(mrdb.MrdError):
+        mrdb.meshgen_refine(*d, -1.0, 1.0)
