@@ -114,13 +114,13 @@ incircle_exact_kernel(const unsigned long long *__restrict__ n_work, const int32
 // Mesh data structure (section 4.1.2): triangleEdges and edgeTriangles from triangleVertices
 // ------------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-edge_keys_kernel(int64_t n, const int32_t *__restrict__ tv, unsigned long long *__restrict__ key, int32_t *__restrict__ val) {
+edge_keys_kernel(int64_t n, const int32_t *__restrict__ tv, int bits, unsigned long long *__restrict__ key, int32_t *__restrict__ val) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int64_t t = i / 3;
   const int k = (int)(i - 3 * t);
   const unsigned a = (unsigned)tv[3 * t + (k + 1) % 3], b = (unsigned)tv[3 * t + (k + 2) % 3];   // edge k is opposite local vertex k
-  key[i] = ((unsigned long long)min(a, b) << 32) | max(a, b);
+  key[i] = ((unsigned long long)min(a, b) << bits) | max(a, b);   // `bits` >= the width of a vertex number: sorts by (smaller, larger)
   val[i] = (int32_t)i;
 }
 __global__ void __launch_bounds__(256)
@@ -455,7 +455,9 @@ candidate_kernel(int64_t nc, const int32_t *__restrict__ cand, const double2 *__
   e_ins[j] = ei;
 }
 
-// section 4.1.1: the cavity of p from its insertion triangle(s); returns its size, or -1 when it exceeds CAVITY_MAX
+// section 4.1.1: the cavity of p from its insertion triangle(s); returns its size, -1 when it exceeds CAVITY_MAX, and -2 when
+// EXACT is false and the filter could not decide one of the INCIRCLE2D tests (the candidate then goes to the exact kernel)
+template <bool EXACT>
 static __device__ int cavity_of(double2 p, int8_t kd, int32_t ti, int32_t ei, const double2 *xy, const int32_t *tv, const int32_t *te,
                                 const int32_t *et, int32_t *list, double *acc, double *tmp) {
   int n = 0;
@@ -472,7 +474,10 @@ static __device__ int cavity_of(double2 p, int8_t kd, int32_t ti, int32_t ei, co
       const int32_t *v = tv + 3 * (int64_t)nb;
       const double2 A = xy[v[0]], B = xy[v[1]], C = xy[v[2]];
       int sg = incircle2d_filter(A, B, C, p);
-      if (sg == 2) sg = incircle2d_exact(A, B, C, p, acc, tmp);
+      if (sg == 2) {
+        if (!EXACT) return -2;
+        sg = incircle2d_exact(A, B, C, p, acc, tmp);
+      }
       if (sg > 0) {
         if (n == CAVITY_MAX) return -1;
         list[n++] = nb;
@@ -481,31 +486,53 @@ static __device__ int cavity_of(double2 p, int8_t kd, int32_t ti, int32_t ei, co
   }
   return n;
 }
-// pass 1: claim the cavity's triangles; pass 2: selected when every one of them still carries this candidate's priority.
-// Grid-stride with few threads: every thread owns a slice of the expansion scratch.
+// pass 1: claim the cavity's triangles; pass 2: selected when every one of them still carries this candidate's priority
 template <int PASS>
-__global__ void __launch_bounds__(32)
+static __device__ __forceinline__ void cavity_act(int64_t j, int n, const int32_t *list, int8_t kd, unsigned long long pr, int8_t *kind,
+                                                  unsigned long long *claim, int32_t *sel, int32_t *seg) {
+  if (PASS == 1) {
+    if (n < 0) kind[j] = KIND_NONE;                                // too large (M11) or nothing to insert: waits
+    for (int q = 0; q < n; ++q) atomicMax(claim + list[q], pr);
+  } else {
+    bool mine = n > 0;
+    for (int q = 0; q < n; ++q) mine &= claim[list[q]] == pr;
+    sel[j] = mine ? 1 : 0;
+    seg[j] = (mine && kd == KIND_SEG) ? 1 : 0;
+  }
+}
+// one thread per candidate, filter only; the candidates with an undecided test are listed for cavity_exact_kernel
+template <int PASS>
+__global__ void __launch_bounds__(128)
 cavity_kernel(int64_t nc, const int32_t *__restrict__ cand, int8_t *__restrict__ kind, const double2 *__restrict__ pt,
               const int32_t *__restrict__ t_ins, const int32_t *__restrict__ e_ins, const double2 *__restrict__ xy,
               const int32_t *__restrict__ tv, const int32_t *__restrict__ te, const int32_t *__restrict__ et,
               unsigned long long *__restrict__ claim, unsigned seed, unsigned iteration, int32_t *__restrict__ sel,
-              int32_t *__restrict__ seg, double *__restrict__ scratch) {
-  const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+              int32_t *__restrict__ seg, int32_t *__restrict__ work, unsigned long long *__restrict__ n_work) {
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= nc) return;
+  int32_t list[CAVITY_MAX];
+  const int8_t kd = kind[j];
+  const int n = kd == KIND_NONE ? -1 : cavity_of<false>(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, list, nullptr, nullptr);
+  if (n == -2) { work[atomicAdd(n_work, 1ull)] = (int32_t)j; return; }
+  cavity_act<PASS>(j, n, list, kd, priority_of(seed, iteration, (unsigned)cand[j]), kind, claim, sel, seg);
+}
+// the listed candidates again, with the exact INCIRCLE2D where the filter fails.  Grid-stride with few threads: every thread
+// owns a slice of the expansion scratch.
+template <int PASS>
+__global__ void __launch_bounds__(32)
+cavity_exact_kernel(const unsigned long long *__restrict__ n_work, const int32_t *__restrict__ work, const int32_t *__restrict__ cand,
+                    int8_t *__restrict__ kind, const double2 *__restrict__ pt, const int32_t *__restrict__ t_ins,
+                    const int32_t *__restrict__ e_ins, const double2 *__restrict__ xy, const int32_t *__restrict__ tv,
+                    const int32_t *__restrict__ te, const int32_t *__restrict__ et, unsigned long long *__restrict__ claim, unsigned seed,
+                    unsigned iteration, int32_t *__restrict__ sel, int32_t *__restrict__ seg, double *__restrict__ scratch) {
+  const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, nw = (int64_t)*n_work;
   double *acc = scratch + tid * (2 * MAXE), *tmp = acc + MAXE;
   int32_t list[CAVITY_MAX];
-  for (int64_t j = tid; j < nc; j += (int64_t)gridDim.x * blockDim.x) {
+  for (int64_t w = tid; w < nw; w += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t j = work[w];
     const int8_t kd = kind[j];
-    int n = kd == KIND_NONE ? -1 : cavity_of(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, list, acc, tmp);
-    const unsigned long long pr = priority_of(seed, iteration, (unsigned)cand[j]);
-    if (PASS == 1) {
-      if (n < 0) kind[j] = KIND_NONE;                              // too large (M11) or nothing to insert: waits
-      for (int q = 0; q < n; ++q) atomicMax(claim + list[q], pr);
-    } else {
-      bool mine = n > 0;
-      for (int q = 0; q < n; ++q) mine &= claim[list[q]] == pr;
-      sel[j] = mine ? 1 : 0;
-      seg[j] = (mine && kd == KIND_SEG) ? 1 : 0;
-    }
+    const int n = cavity_of<true>(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, list, acc, tmp);
+    cavity_act<PASS>(j, n, list, kd, priority_of(seed, iteration, (unsigned)cand[j]), kind, claim, sel, seg);
   }
 }
 static __device__ __forceinline__ void swap_side(int32_t *et, int32_t e, int32_t from, int32_t to) {
@@ -568,7 +595,7 @@ insert_kernel(int64_t nc, const int8_t *__restrict__ kind, const double2 *__rest
 }
 // canonical order (reading M12): rotate every triangle to its smallest vertex; sort keys (second, third) and (first)
 __global__ void __launch_bounds__(256)
-canonical_keys_kernel(int64_t nt, int32_t *__restrict__ tv, unsigned long long *__restrict__ key_lo, int32_t *__restrict__ idx) {
+canonical_keys_kernel(int64_t nt, int32_t *__restrict__ tv, int bits, unsigned long long *__restrict__ key_lo, int32_t *__restrict__ idx) {
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= nt) return;
   int32_t *v = tv + 3 * t;
@@ -576,7 +603,7 @@ canonical_keys_kernel(int64_t nt, int32_t *__restrict__ tv, unsigned long long *
   const int r = (a < b && a < c) ? 0 : ((b < a && b < c) ? 1 : 2);
   const int32_t x = r == 0 ? a : (r == 1 ? b : c), y = r == 0 ? b : (r == 1 ? c : a), z = r == 0 ? c : (r == 1 ? a : b);
   v[0] = x; v[1] = y; v[2] = z;
-  key_lo[t] = ((unsigned long long)(unsigned)y << 32) | (unsigned)z;
+  key_lo[t] = ((unsigned long long)(unsigned)y << bits) | (unsigned)z;
   idx[t] = (int32_t)t;
 }
 __global__ void __launch_bounds__(256)
@@ -739,7 +766,7 @@ struct EdgeWork {
   }
 };
 // te, et from tv (arena reserved and locked by the caller); synchronises s
-int build_edges_run(const EdgeWork &w, int64_t n_triangle, const int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_edge, cudaStream_t s) {
+int build_edges_run(const EdgeWork &w, int64_t n_triangle, int bits, const int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_edge, cudaStream_t s) {
   const int64_t n = 3 * n_triangle;
   char *b = g_arena.base;
   unsigned long long *k0 = (unsigned long long *)(b + w.o_k0), *k1 = (unsigned long long *)(b + w.o_k1);
@@ -749,9 +776,9 @@ int build_edges_run(const EdgeWork &w, int64_t n_triangle, const int32_t *tv_dev
   size_t tmp_sort = w.tmp_sort, tmp_scan = w.tmp_scan;
   cudaMemsetAsync(err, 0, sizeof(int), s);
   cudaMemsetAsync(et_dev, 0xFF, sizeof(int32_t) * 2 * (size_t)n, s);   // -1: no second triangle
-  mrdgen::edge_keys_kernel<<<nb, 256, 0, s>>>(n, tv_dev, k0, v0);
-  // (vertex numbers are below 2^31: the keys have 63 significant bits)
-  cub::DeviceRadixSort::SortPairs(b + w.o_tmp, tmp_sort, k0, k1, v0, v1, n, 0, 63, s);
+  mrdgen::edge_keys_kernel<<<nb, 256, 0, s>>>(n, tv_dev, bits, k0, v0);
+  // (only the 2 * bits significant bits are sorted: fewer radix passes when the caller knows how many vertices there are)
+  cub::DeviceRadixSort::SortPairs(b + w.o_tmp, tmp_sort, k0, k1, v0, v1, n, 0, std::min(2 * bits, 64), s);
   mrdgen::edge_heads_kernel<<<nb, 256, 0, s>>>(n, k1, head);
   cub::DeviceScan::InclusiveSum(b + w.o_tmp, tmp_scan, head, incl, n, s);
   mrdgen::edge_fill_kernel<<<nb, 256, 0, s>>>(n, k1, v1, incl, te_dev, et_dev, err);
@@ -838,7 +865,7 @@ int mrd_meshgen_build_edges(int64_t n_triangle, const int32_t *tv_dev, int32_t *
   std::lock_guard<std::mutex> g(g_arena.mu);
   cudaError_t e = g_arena.reserve(c.total);
   if (e != cudaSuccess) return cuda_fail("build_edges", e);
-  return build_edges_run(w, n_triangle, tv_dev, te_dev, et_dev, n_edge, s);
+  return build_edges_run(w, n_triangle, 32, tv_dev, te_dev, et_dev, n_edge, s);
 }
 
 int mrd_meshgen_delaunay_flip(int64_t n_triangle, int64_t n_edge, const double *xy_dev, int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev,
@@ -883,6 +910,7 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   const size_t o_cand = c.add(sizeof(int32_t) * ct), o_kind = c.add(ct), o_pt = c.add(sizeof(double2) * ct);
   const size_t o_tins = c.add(sizeof(int32_t) * ct), o_eins = c.add(sizeof(int32_t) * ct), o_claim = c.add(sizeof(unsigned long long) * ct);
   const size_t o_sel = c.add(sizeof(int32_t) * ct), o_seg = c.add(sizeof(int32_t) * ct), o_rank = c.add(sizeof(int32_t) * ct), o_srank = c.add(sizeof(int32_t) * ct);
+  const size_t o_cwork = c.add(sizeof(int32_t) * ct), o_cwork2 = c.add(sizeof(int32_t) * ct), o_cwn = c.add(2 * sizeof(unsigned long long));
   const size_t o_klo0 = c.add(sizeof(unsigned long long) * ct), o_klo1 = c.add(sizeof(unsigned long long) * ct);
   const size_t o_khi0 = c.add(sizeof(unsigned) * ct), o_khi1 = c.add(sizeof(unsigned) * ct);
   const size_t o_i0 = c.add(sizeof(int32_t) * ct), o_i1 = c.add(sizeof(int32_t) * ct), o_tv2 = c.add(sizeof(int32_t) * 3 * ct);
@@ -908,6 +936,8 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   unsigned long long *klo0 = (unsigned long long *)(b + o_klo0), *klo1 = (unsigned long long *)(b + o_klo1);
   unsigned *khi0 = (unsigned *)(b + o_khi0), *khi1 = (unsigned *)(b + o_khi1);
   int32_t *i0 = (int32_t *)(b + o_i0), *i1 = (int32_t *)(b + o_i1), *tv2 = (int32_t *)(b + o_tv2);
+  int32_t *cwork = (int32_t *)(b + o_cwork), *cwork2 = (int32_t *)(b + o_cwork2);
+  unsigned long long *cwork_n = (unsigned long long *)(b + o_cwn);
   void *tmp = b + o_tmp;
   volatile unsigned long long *hp = g_arena.pinned;
   auto sync = [&](const char *what) -> int {
@@ -934,8 +964,12 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
     // 4.1.1: cavities, claims, selection
     cudaMemsetAsync(claim, 0, sizeof(unsigned long long) * (size_t)nt, s);
     const unsigned itn = (unsigned)(first_iteration + it);
-    mrdgen::cavity_kernel<1><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch);
-    mrdgen::cavity_kernel<2><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch);
+    const unsigned nbc = (unsigned)((nc + 127) / 128);
+    cudaMemsetAsync(cwork_n, 0, 2 * sizeof(unsigned long long), s);
+    mrdgen::cavity_kernel<1><<<nbc, 128, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, cwork, cwork_n);
+    mrdgen::cavity_exact_kernel<1><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cwork_n, cwork, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch);
+    mrdgen::cavity_kernel<2><<<nbc, 128, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, cwork2, cwork_n + 1);
+    mrdgen::cavity_exact_kernel<2><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cwork_n + 1, cwork2, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch);
     tb = tmp_scan;
     cub::DeviceScan::ExclusiveSum(tmp, tb, sel, rank, nc, s);
     tb = tmp_scan;
@@ -961,16 +995,18 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
     if ((rc = flip_run(fw, o_scr, nt, ne, xy, tv_dev, te_dev, et_dev, nullptr, nullptr, nullptr, s)) != MRD_OK) return rc;
     // canonical order (M12) and the edge arrays that go with it
     const unsigned nbt = (unsigned)((nt + 255) / 256);
-    mrdgen::canonical_keys_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, klo0, i0);
+    int bits = 1;
+    while ((1ll << bits) < nv) ++bits;                               // width of a vertex number
+    mrdgen::canonical_keys_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, bits, klo0, i0);
     tb = tmp_s64;
-    cub::DeviceRadixSort::SortPairs(tmp, tb, klo0, klo1, i0, i1, nt, 0, 64, s);
+    cub::DeviceRadixSort::SortPairs(tmp, tb, klo0, klo1, i0, i1, nt, 0, 2 * bits, s);
     mrdgen::gather_first_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, i1, khi0);
     tb = tmp_s32;
-    cub::DeviceRadixSort::SortPairs(tmp, tb, khi0, khi1, i1, i0, nt, 0, 32, s);
+    cub::DeviceRadixSort::SortPairs(tmp, tb, khi0, khi1, i1, i0, nt, 0, bits, s);
     mrdgen::gather_rows_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, i0, tv2);
     cudaMemcpyAsync(tv_dev, tv2, sizeof(int32_t) * 3 * (size_t)nt, cudaMemcpyDeviceToDevice, s);
     int64_t ne_built = 0;
-    if ((rc = build_edges_run(ew, nt, tv_dev, te_dev, et_dev, &ne_built, s)) != MRD_OK) return rc;
+    if ((rc = build_edges_run(ew, nt, bits, tv_dev, te_dev, et_dev, &ne_built, s)) != MRD_OK) return rc;
     if (ne_built != ne) return gen_fail(MRD_EINVAL, "refine: edge count changed under renumbering (internal error)");
     done++;
   }

@@ -12,6 +12,9 @@ counters back, which is inside the time):
 * check_only        the same call on the finished triangulation: one pass of the exact INCIRCLE2D over all edges
 * test_quality      eq. 2 for every triangle
 * find_triangle     the containing triangle of every triangle's circumcentre, walking from that triangle (section 2.4.2)
+* refine            Delaunay refinement (section 2.4, 4.1.1) of a 40 x 40-cell start mesh of the same square down to the
+                    circumradius bound that gives about as many vertices as the mesh above (B = sqrt 2): the paper's own test of
+                    section 4.1.6, "the generation of a uniform unstructured mesh ... with 1.3 million vertices"
 
 Prints one JSON line per item with the algorithmic bytes per unit (stated in DESIGN.md section 9c) and the GB/s they amount
 to.  Needs a GPU and the built extension; there is no CPU fallback."""
@@ -50,7 +53,7 @@ def timed(fn, reps, torch, setup=None):
     return float(np.median(ms[1:])), out
 
 
-def run(cells, reps, out_path):
+def run(cells, reps, out_path, only=None):
     import torch
     if not torch.cuda.is_available():
         raise SystemExit("meshgen_bench: no CUDA device")
@@ -74,6 +77,8 @@ def run(cells, reps, out_path):
         rows.append(row)
         print(json.dumps(row), flush=True)
 
+    if only == "refine":
+        return refine_part(wl, b, torch, nv, reps, rows, out_path)
     ms, (te0, et0) = timed(lambda: b.meshgen_build_edges(tv0), reps, torch)
     ne = et0.shape[0]
     emit("build_edges", ms, nt, "triangles", dict(n_edges=ne))
@@ -103,6 +108,23 @@ def run(cells, reps, out_path):
     moved = int(((t != t0) & (t >= 0)).sum().item())
     emit("find_triangle", ms, nt, "points", dict(found=found, left_the_mesh=nt - found, not_in_start_triangle=moved),
          bytes_total=BYTES["find_triangle"] * nt + BYTES_PER_VISIT * nt)   # at least the start triangle is visited
+    return refine_part(wl, b, torch, nv, reps, rows, out_path)
+
+
+def refine_part(wl, b, torch, nv, reps, rows, out_path):
+    # refinement from a coarse mesh of the same square to about nv vertices: vertices ~ 0.69 area / R^2 at B = sqrt 2 (measured)
+    c = wl.scrambled_triangulation(40, 40, seed=2, Lx=2.0, Ly=2.0)
+    cxy = torch.tensor(c.xy, dtype=torch.float64, device="cuda")
+    ctv = torch.tensor(c.tri, dtype=torch.int32, device="cuda")
+    cte, cet = b.meshgen_build_edges(ctv)
+    b.meshgen_delaunay_flip(cxy, ctv, cte, cet)
+    R = float(np.sqrt(0.69 * 4.0 / nv))
+    ms, g = timed(lambda: b.meshgen_refine(cxy, ctv, cte, cet, R, np.sqrt(2.0), seed=1, cap_vertex=int(1.6 * nv)), min(reps, 3), torch)
+    row = dict(kernel="refine", ms=ms, units=int(g[0].shape[0]) - c.nv, unit="vertices inserted",
+               g_units_per_s=(int(g[0].shape[0]) - c.nv) / ms / 1e6, n_vertices=int(g[0].shape[0]), n_triangles=int(g[1].shape[0]),
+               n_edges=int(g[3].shape[0]), R=R, B=float(np.sqrt(2.0)), start_vertices=c.nv, **g[4])
+    rows.append(row)
+    print(json.dumps(row), flush=True)
     if out_path:
         with open(out_path, "w") as f:
             json.dump(rows, f, indent=1)
@@ -114,8 +136,9 @@ def main():
     ap.add_argument("--cells", type=int, default=1140)
     ap.add_argument("--reps", type=int, default=5)
     ap.add_argument("--out", default=None)
+    ap.add_argument("--only", default=None, choices=["refine"], help="time the refinement alone")
     a = ap.parse_args()
-    run(a.cells, a.reps, a.out)
+    run(a.cells, a.reps, a.out, a.only)
     return 0
 
 

@@ -154,3 +154,43 @@ def test_capacity_and_bad_input_are_reported(mrdb):
     assert g[4]["iterations"] == 2 and g[4]["bad_left"] > 0
     with pytest.raises(mrdb.MrdError):
         mrdb.meshgen_refine(*d, -1.0, 1.0)
+
+
+def test_generated_mesh_runs_in_the_solver(mrdb):
+    """The point of the generator (section 4): the refined mesh goes straight into the solver.  A mesh refined on the GPU
+    (bounded rectangle, boundary vertices frozen) carries 20 RK2 steps of scheme B to the oracle's result, and a uniform
+    flow on it has residuals that are exactly zero."""
+    import torch
+    from types import SimpleNamespace
+    import oracle
+    import paper_1705_02028_b200 as mrd
+    from helpers import field_errors
+    xy, tv, te, et = start(2, (9, 7))
+    gx, gt, gte, get, info = mrdb.meshgen_refine(*to_dev(xy, tv, te, et), 0.02, np.sqrt(2.0), seed=4, cap_vertex=40000)
+    X, T, TE, ET = gx.cpu().numpy(), gt.cpu().numpy(), gte.cpu().numpy(), get.cpu().numpy()
+    assert info["bad_left"] == 0 and 3000 < X.shape[0] < 40000
+    seg = np.nonzero(ET[:, 1] < 0)[0]
+    k = (TE[ET[seg, 0]] == seg[:, None]).argmax(axis=1)
+    flag = np.zeros(X.shape[0], dtype=np.uint8)
+    flag[T[ET[seg, 0], (k + 1) % 3]] = 1
+    flag[T[ET[seg, 0], (k + 2) % 3]] = 1
+    val = np.bincount(T.ravel(), minlength=X.shape[0])
+    assert val.max() >= 8 and val[flag == 0].min() >= 4             # an unstructured mesh: variable valence
+    mesh = SimpleNamespace(xy=X, nv=X.shape[0], lengths=(2.0, 1.5))
+    W = wl.random_smooth_state(mesh, mach=0.7, seed=2)
+    gm = mrd.Mesh(X, T, vertex_flag=flag, scheme=mrd.SCHEME_B, time_order=2)
+    om = oracle.OracleMesh(X, T, vertex_flag=flag, scheme=oracle.SCHEME_B, time_order=2, threads=4)
+    gm.set_state(torch.tensor(W, device="cuda"))
+    om.set_state(W)
+    gm.step(1)
+    om.step(1)
+    assert field_errors(gm.get_state().cpu().numpy(), om.get_state()) <= 1e-12
+    gm.step(19)
+    om.step(19)
+    Wg = gm.get_state().cpu().numpy()
+    assert field_errors(Wg, om.get_state()) <= 1e-9
+    assert np.array_equal(Wg[:, flag == 1], W[:, flag == 1]) and Wg[0].min() > 0
+    U = wl.uniform_state(mesh)
+    gm.set_state(torch.tensor(U, device="cuda"))
+    gm.step(3)
+    assert np.array_equal(gm.get_state().cpu().numpy(), U)          # zero residuals, bit for bit (reading C3)
