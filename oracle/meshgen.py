@@ -345,12 +345,36 @@ def canonical_order(tv):
     return np.array(rows, dtype=np.int32).reshape(-1, 3)
 
 
-def refine_iteration(xy, tv, te, et, R, B, seed, iteration):
+def morton_key(x, y, box):
+    """Morton value of a vertex (section 4.1.4; reading M14): 21 bits per coordinate, i = min(2^21 - 1,
+    floor((x - x0) * (2^21 / (x1 - x0)))) with one IEEE operation at a time, the bits of i_x in the even places."""
+    x0, y0, x1, y1 = (float(v) for v in box)
+    sx, sy = 2097152.0 / (x1 - x0), 2097152.0 / (y1 - y0)
+    ix = min(2097151, max(0, int(np.floor((float(x) - x0) * sx))))
+    iy = min(2097151, max(0, int(np.floor((float(y) - y0) * sy))))
+    key = 0
+    for b in range(21):
+        key |= ((ix >> b) & 1) << (2 * b) | ((iy >> b) & 1) << (2 * b + 1)
+    return key
+
+
+def morton_order(xy, tv, box):
+    """Renumber the vertices in ascending Morton value (ties keep their order) and the triangles' entries with them; the
+    triangle order is then made canonical, which follows the vertices' curve.  Returns (xy, tv, new number of every old vertex)."""
+    keys = [morton_key(x, y, box) for x, y in np.asarray(xy)]
+    order = sorted(range(len(keys)), key=lambda i: (keys[i], i))
+    new = np.empty(len(keys), dtype=np.int32)
+    new[order] = np.arange(len(keys), dtype=np.int32)
+    return np.asarray(xy)[order].copy(), canonical_order(new[np.asarray(tv)]), new
+
+
+def refine_iteration(xy, tv, te, et, R, B, seed, iteration, box=None):
     """One iteration of section 2.4 on a Delaunay triangulation: TestQuality; for every bad triangle, in ascending order, its
     candidate; cavities and the independent set of section 4.1.1 (a triangle claimed by several cavities goes to the highest
     priority; a candidate is selected when it holds every triangle of its cavity); the selected vertices are numbered, and
     their triangles and edges appended, in ascending order of their bad triangle; flips restore the Delaunay property; the
-    triangles are put in canonical order (reading M12).
+    triangles are put in canonical order (reading M12) -- after the vertices have been renumbered along the Morton curve of
+    the rectangle `box` = (x0, y0, x1, y1), when one is given (section 4.1.4, reading M14).
     Returns (xy, tv, te, et, info) as new arrays; info: n_bad, n_selected, kinds of the selected, flips."""
     xy = np.asarray(xy, dtype=np.float64)
     q = test_quality(xy, tv, R, B)
@@ -382,14 +406,17 @@ def refine_iteration(xy, tv, te, et, R, B, seed, iteration):
         dt, de = insert_vertex(tv2, te2, et2, kind, t_ins, e, nv + j, nt, ne)
         nt, ne = nt + dt, ne + de
     flips = flip_to_delaunay(xy2, tv2, te2, et2)
-    tv2 = canonical_order(tv2)
+    if box is not None:                                           # section 4.1.4: Morton order after every insertion step
+        xy2, tv2, _ = morton_order(xy2, tv2, box)
+    else:
+        tv2 = canonical_order(tv2)
     te2, et2 = build_edges(tv2)
     info = dict(n_bad=len(bad), n_candidates=len(cands), n_selected=len(sel), kinds=[cd[1] for cd in sel], flips=flips,
                 selected=[(cd[0], cd[1], cd[2], cd[5]) for cd in sel])
     return xy2, tv2, te2, et2, info
 
 
-def refine(xy, tv, R, B, seed=0, max_iterations=10 ** 6):
+def refine(xy, tv, R, B, seed=0, max_iterations=10 ** 6, box=None):
     """Section 2.4: iterate "until no more vertices need to be inserted".  The input is made Delaunay first.
     Returns (xy, tv, te, et, number of iterations that inserted something)."""
     xy = np.asarray(xy, dtype=np.float64)
@@ -397,7 +424,7 @@ def refine(xy, tv, R, B, seed=0, max_iterations=10 ** 6):
     te, et = build_edges(tv)
     it = 0
     while it < max_iterations:
-        xy, tv, te, et, info = refine_iteration(xy, tv, te, et, R, B, seed, it)
+        xy, tv, te, et, info = refine_iteration(xy, tv, te, et, R, B, seed, it, box)
         if info["n_bad"] == 0:
             break
         it += 1

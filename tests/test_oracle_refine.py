@@ -198,3 +198,31 @@ def test_canonical_order_renumbers_without_changing_the_triangulation():
     assert (np.lexsort((c[:, 2], c[:, 1], c[:, 0])) == np.arange(len(c))).all()
     assert all(mg.orient2d(*xy[t]) == 1 for t in c)               # rotation only: every triangle stays counter-clockwise
     assert np.array_equal(mg.canonical_order(c), c)
+
+
+def test_morton_order_follows_the_z_curve_and_changes_numbers_only():
+    """Section 4.1.4: 'assigning a Morton value to each vertex, and then sorting'.  On a 4 x 4 grid of cell centres the order is
+    the textbook Z curve; on a mesh it is a renumbering (same points, same triangles) with neighbours in number close in space."""
+    c = (np.arange(4) + 0.5) / 4
+    pts = np.array([(x, y) for y in c for x in c])                # row-major
+    keys = [mg.morton_key(x, y, (0.0, 0.0, 1.0, 1.0)) for x, y in pts]
+    z = [0, 1, 4, 5, 2, 3, 6, 7, 8, 9, 12, 13, 10, 11, 14, 15]     # Z order of a 4 x 4 block, row-major index
+    assert [int(np.argsort(keys)[i]) for i in range(16)] == z
+    assert mg.morton_key(0.0, 0.0, (0, 0, 1, 1)) == 0 and mg.morton_key(1.0, 1.0, (0, 0, 1, 1)) == 2 ** 42 - 1   # the far corner is clamped
+    assert mg.morton_key(1.0, 0.0, (0, 0, 1, 1)) == int("01" * 21, 2) and mg.morton_key(0.0, 1.0, (0, 0, 1, 1)) == int("10" * 21, 2)
+    xy, tv, te, et = start_mesh(seed=6, shape=(12, 9))
+    box = (0.0, 0.0, 2.0, 1.5)
+    xy2, tv2, new = mg.morton_order(xy, tv, box)
+    assert sorted(new) == list(range(len(new))) and np.array_equal(xy2[new], xy)
+    assert mg.triangle_set(tv2) == mg.triangle_set(new[tv]) and np.array_equal(tv2, mg.canonical_order(tv2))
+    k2 = [mg.morton_key(x, y, box) for x, y in xy2]
+    assert k2 == sorted(k2)
+    step = np.hypot(*(xy2[1:] - xy2[:-1]).T)
+    step0 = np.hypot(*(xy[1:] - xy[:-1]).T)
+    assert np.median(step) < 1.5 * np.median(step0) and step.max() <= 2.5   # consecutive numbers are neighbours; the curve's jumps stay in the box
+    # refinement with the reordering gives the same kind of mesh (another vertex order changes the insertion order, L144)
+    xa, ta, _, _, ita = mg.refine(xy, tv, 0.08, 1.0, seed=2, box=box)
+    q = mg.test_quality(xa, ta, 0.08, 1.0)
+    assert q["bad"].sum() == 0 and mg.triangle_set(ta) == library_triangulation(xa)
+    ka = [mg.morton_key(x, y, box) for x, y in xa]
+    assert ka == sorted(ka)
