@@ -367,8 +367,12 @@ int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_
  *      one triangle at a segment split in two), numbered -- like their new triangles and edges -- in ascending order of
  *      their bad triangle;
  *   6. flips restore the Delaunay property (2.4.6);
- *   7. the triangles are renumbered canonically (each rotated to its smallest vertex, sorted by vertex triple) and te, et
- *      rebuilt as by mrd_meshgen_build_edges (the paper re-sorts after every insertion step too, 4.1.4).
+ *   7. re-sort (4.1.4): when `box` = (x0, y0, x1, y1) (HOST, the rectangle the domain lies in) is given, the vertices are
+ *      renumbered in ascending Morton value -- 21 bits per coordinate, i = min(2^21 - 1, floor((x - x0) * (2^21 / (x1 - x0)))),
+ *      x in the even bit places, ties keep their order -- and xy, tv follow; with box = NULL the vertices keep their numbers
+ *      (input vertices first, inserted ones in order of insertion).  Then the triangles are renumbered canonically (each
+ *      rotated to its smallest vertex, sorted by vertex triple: along the same curve when the vertices are) and te, et
+ *      rebuilt as by mrd_meshgen_build_edges.
  *   Every step is deterministic and independent of the order in which threads run: the result is, array for array, the one
  *   of oracle/meshgen.py: refine.
  *   In: a Delaunay triangulation (xy, tv, te, et) with *n_vertex, *n_triangle, *n_edge entries in device arrays with room
@@ -380,10 +384,10 @@ int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_
  *   MRD_ENOMEM when the next insertion would exceed a capacity (the arrays then hold a valid Delaunay mesh, partly
  *   refined); MRD_EINVAL for an input that is not a Delaunay triangulation (a walk that does not end).
  * ---------------------------------------------------------------------------------------------- */
-int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteration, int64_t max_iterations, int64_t cap_vertex,
-                       int64_t cap_triangle, int64_t cap_edge, int64_t *n_vertex, int64_t *n_triangle, int64_t *n_edge,
-                       double *xy_dev, int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_iterations,
-                       int64_t *n_bad_left, void *stream);
+int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteration, int64_t max_iterations, const double *box,
+                       int64_t cap_vertex, int64_t cap_triangle, int64_t cap_edge, int64_t *n_vertex, int64_t *n_triangle,
+                       int64_t *n_edge, double *xy_dev, int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev,
+                       int64_t *n_iterations, int64_t *n_bad_left, void *stream);
 
 /* Kernel launch counter: number of the library's own kernel launches since the mesh was created. */
 int mrd_launch_count(const mrd_mesh *m, int64_t *launches);

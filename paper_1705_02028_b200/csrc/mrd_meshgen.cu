@@ -593,6 +593,42 @@ insert_kernel(int64_t nc, const int8_t *__restrict__ kind, const double2 *__rest
   swap_side(et, e_ca, t, n1);
   swap_side(et, e_dc, t2, n2);
 }
+// Morton value of every vertex (section 4.1.4; reading M14): 21 bits per coordinate, x in the even places
+static __device__ __forceinline__ unsigned long long spread21(unsigned v) {
+  unsigned long long x = v & 0x1FFFFFull;
+  x = (x | (x << 16)) & 0x0000FFFF0000FFFFull;
+  x = (x | (x << 8)) & 0x00FF00FF00FF00FFull;
+  x = (x | (x << 4)) & 0x0F0F0F0F0F0F0F0Full;
+  x = (x | (x << 2)) & 0x3333333333333333ull;
+  x = (x | (x << 1)) & 0x5555555555555555ull;
+  return x;
+}
+__global__ void __launch_bounds__(256)
+morton_keys_kernel(int64_t nv, const double2 *__restrict__ xy, double x0, double y0, double sx, double sy,
+                   unsigned long long *__restrict__ key, int32_t *__restrict__ idx) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nv) return;
+  const double2 p = xy[i];
+  const double fx = floor(__dmul_rn(__dsub_rn(p.x, x0), sx)), fy = floor(__dmul_rn(__dsub_rn(p.y, y0), sy));
+  const unsigned ix = (unsigned)fmin(2097151.0, fmax(0.0, fx)), iy = (unsigned)fmin(2097151.0, fmax(0.0, fy));
+  key[i] = spread21(ix) | (spread21(iy) << 1);
+  idx[i] = (int32_t)i;
+}
+// order[i] = old number of the vertex that becomes i
+__global__ void __launch_bounds__(256)
+vertex_permute_kernel(int64_t nv, const int32_t *__restrict__ order, const double2 *__restrict__ xy, double2 *__restrict__ xy_new,
+                      int32_t *__restrict__ number) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nv) return;
+  const int32_t o = order[i];
+  xy_new[i] = xy[o];
+  number[o] = (int32_t)i;
+}
+__global__ void __launch_bounds__(256)
+relabel_kernel(int64_t n, const int32_t *__restrict__ number, int32_t *__restrict__ tv) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) tv[i] = number[tv[i]];
+}
 // canonical order (reading M12): rotate every triangle to its smallest vertex; sort keys (second, third) and (first)
 __global__ void __launch_bounds__(256)
 canonical_keys_kernel(int64_t nt, int32_t *__restrict__ tv, int bits, unsigned long long *__restrict__ key_lo, int32_t *__restrict__ idx) {
@@ -887,11 +923,13 @@ int mrd_meshgen_delaunay_flip(int64_t n_triangle, int64_t n_edge, const double *
   return flip_run(w, w.o_scr, n_triangle, n_edge, (const double2 *)xy_dev, tv_dev, te_dev, et_dev, n_flips, n_iterations, n_exact, s);
 }
 
-int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteration, int64_t max_iterations, int64_t cap_vertex,
-                       int64_t cap_triangle, int64_t cap_edge, int64_t *n_vertex, int64_t *n_triangle, int64_t *n_edge, double *xy_dev,
-                       int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_iterations, int64_t *n_bad_left, void *stream) {
+int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteration, int64_t max_iterations, const double *box,
+                       int64_t cap_vertex, int64_t cap_triangle, int64_t cap_edge, int64_t *n_vertex, int64_t *n_triangle, int64_t *n_edge,
+                       double *xy_dev, int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_iterations, int64_t *n_bad_left,
+                       void *stream) {
   if (!n_vertex || !n_triangle || !n_edge || !xy_dev || !tv_dev || !te_dev || !et_dev) return gen_fail(MRD_EINVAL, "null argument");
   if (!(R > 0.0) || !(B > 0.0)) return gen_fail(MRD_EINVAL, "R and B must be positive");
+  if (box && !(box[2] > box[0] && box[3] > box[1])) return gen_fail(MRD_EINVAL, "refine: box must be (x0, y0, x1, y1) with x1 > x0, y1 > y0");
   int64_t nv = *n_vertex, nt = *n_triangle, ne = *n_edge;
   if (nv < 3 || nt < 1 || ne < 3 || nv > cap_vertex || nt > cap_triangle || ne > cap_edge || first_iteration < 0 || max_iterations < 0)
     return gen_fail(MRD_EINVAL, "refine: sizes out of range");
@@ -911,13 +949,15 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   const size_t o_tins = c.add(sizeof(int32_t) * ct), o_eins = c.add(sizeof(int32_t) * ct), o_claim = c.add(sizeof(unsigned long long) * ct);
   const size_t o_sel = c.add(sizeof(int32_t) * ct), o_seg = c.add(sizeof(int32_t) * ct), o_rank = c.add(sizeof(int32_t) * ct), o_srank = c.add(sizeof(int32_t) * ct);
   const size_t o_cwork = c.add(sizeof(int32_t) * ct), o_cwork2 = c.add(sizeof(int32_t) * ct), o_cwn = c.add(2 * sizeof(unsigned long long));
-  const size_t o_klo0 = c.add(sizeof(unsigned long long) * ct), o_klo1 = c.add(sizeof(unsigned long long) * ct);
+  const size_t cm = std::max(ct, (size_t)cap_vertex);               // the sort buffers serve triangles and vertices
+  const size_t o_klo0 = c.add(sizeof(unsigned long long) * cm), o_klo1 = c.add(sizeof(unsigned long long) * cm);
   const size_t o_khi0 = c.add(sizeof(unsigned) * ct), o_khi1 = c.add(sizeof(unsigned) * ct);
-  const size_t o_i0 = c.add(sizeof(int32_t) * ct), o_i1 = c.add(sizeof(int32_t) * ct), o_tv2 = c.add(sizeof(int32_t) * 3 * ct);
+  const size_t o_i0 = c.add(sizeof(int32_t) * cm), o_i1 = c.add(sizeof(int32_t) * cm), o_tv2 = c.add(sizeof(int32_t) * 3 * ct);
+  const size_t o_xy2 = c.add(sizeof(double2) * (size_t)cap_vertex), o_num = c.add(sizeof(int32_t) * (size_t)cap_vertex);   // (cap_vertex <= cap_triangle is not required)
   size_t tmp_sel = 0, tmp_scan = 0, tmp_s64 = 0, tmp_s32 = 0;
   cub::DeviceSelect::Flagged(nullptr, tmp_sel, thrust::counting_iterator<int32_t>(0), (const uint8_t *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, s);
   cub::DeviceScan::ExclusiveSum(nullptr, tmp_scan, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, s);
-  cub::DeviceRadixSort::SortPairs(nullptr, tmp_s64, (unsigned long long *)nullptr, (unsigned long long *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, 0, 64, s);
+  cub::DeviceRadixSort::SortPairs(nullptr, tmp_s64, (unsigned long long *)nullptr, (unsigned long long *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)cm, 0, 64, s);
   cub::DeviceRadixSort::SortPairs(nullptr, tmp_s32, (unsigned *)nullptr, (unsigned *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, 0, 32, s);
   const size_t o_tmp = c.add(std::max(std::max(tmp_sel, tmp_scan), std::max(tmp_s64, tmp_s32)));
   std::lock_guard<std::mutex> g(g_arena.mu);
@@ -935,7 +975,8 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   int32_t *sel = (int32_t *)(b + o_sel), *seg = (int32_t *)(b + o_seg), *rank = (int32_t *)(b + o_rank), *srank = (int32_t *)(b + o_srank);
   unsigned long long *klo0 = (unsigned long long *)(b + o_klo0), *klo1 = (unsigned long long *)(b + o_klo1);
   unsigned *khi0 = (unsigned *)(b + o_khi0), *khi1 = (unsigned *)(b + o_khi1);
-  int32_t *i0 = (int32_t *)(b + o_i0), *i1 = (int32_t *)(b + o_i1), *tv2 = (int32_t *)(b + o_tv2);
+  int32_t *i0 = (int32_t *)(b + o_i0), *i1 = (int32_t *)(b + o_i1), *tv2 = (int32_t *)(b + o_tv2), *number = (int32_t *)(b + o_num);
+  double2 *xy2 = (double2 *)(b + o_xy2);
   int32_t *cwork = (int32_t *)(b + o_cwork), *cwork2 = (int32_t *)(b + o_cwork2);
   unsigned long long *cwork_n = (unsigned long long *)(b + o_cwn);
   void *tmp = b + o_tmp;
@@ -997,6 +1038,15 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
     const unsigned nbt = (unsigned)((nt + 255) / 256);
     int bits = 1;
     while ((1ll << bits) < nv) ++bits;                               // width of a vertex number
+    if (box) {                                                       // 4.1.4: vertices along the Morton curve of the box (M14)
+      const unsigned nbv = (unsigned)((nv + 255) / 256);
+      mrdgen::morton_keys_kernel<<<nbv, 256, 0, s>>>(nv, xy, box[0], box[1], 2097152.0 / (box[2] - box[0]), 2097152.0 / (box[3] - box[1]), klo0, i0);
+      tb = tmp_s64;
+      cub::DeviceRadixSort::SortPairs(tmp, tb, klo0, klo1, i0, i1, nv, 0, 42, s);   // stable: ties keep their order
+      mrdgen::vertex_permute_kernel<<<nbv, 256, 0, s>>>(nv, i1, xy, xy2, number);
+      cudaMemcpyAsync(xy, xy2, sizeof(double2) * (size_t)nv, cudaMemcpyDeviceToDevice, s);
+      mrdgen::relabel_kernel<<<(unsigned)((3 * nt + 255) / 256), 256, 0, s>>>(3 * nt, number, tv_dev);
+    }
     mrdgen::canonical_keys_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, bits, klo0, i0);
     tb = tmp_s64;
     cub::DeviceRadixSort::SortPairs(tmp, tb, klo0, klo1, i0, i1, nt, 0, 2 * bits, s);

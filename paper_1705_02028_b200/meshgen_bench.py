@@ -119,12 +119,13 @@ def refine_part(wl, b, torch, nv, reps, rows, out_path):
     cte, cet = b.meshgen_build_edges(ctv)
     b.meshgen_delaunay_flip(cxy, ctv, cte, cet)
     R = float(np.sqrt(0.69 * 4.0 / nv))
-    ms, g = timed(lambda: b.meshgen_refine(cxy, ctv, cte, cet, R, np.sqrt(2.0), seed=1, cap_vertex=int(1.6 * nv)), min(reps, 3), torch)
-    row = dict(kernel="refine", ms=ms, units=int(g[0].shape[0]) - c.nv, unit="vertices inserted",
-               g_units_per_s=(int(g[0].shape[0]) - c.nv) / ms / 1e6, n_vertices=int(g[0].shape[0]), n_triangles=int(g[1].shape[0]),
-               n_edges=int(g[3].shape[0]), R=R, B=float(np.sqrt(2.0)), start_vertices=c.nv, **g[4])
-    rows.append(row)
-    print(json.dumps(row), flush=True)
+    for name, box in (("refine", None), ("refine_morton", (0.0, 0.0, 2.0, 2.0))):
+        ms, g = timed(lambda: b.meshgen_refine(cxy, ctv, cte, cet, R, np.sqrt(2.0), seed=1, cap_vertex=int(1.6 * nv), box=box), min(reps, 3), torch)
+        row = dict(kernel=name, ms=ms, units=int(g[0].shape[0]) - c.nv, unit="vertices inserted",
+                   g_units_per_s=(int(g[0].shape[0]) - c.nv) / ms / 1e6, n_vertices=int(g[0].shape[0]), n_triangles=int(g[1].shape[0]),
+                   n_edges=int(g[3].shape[0]), R=R, B=float(np.sqrt(2.0)), start_vertices=c.nv, **g[4])
+        rows.append(row)
+        print(json.dumps(row), flush=True)
     if out_path:
         with open(out_path, "w") as f:
             json.dump(rows, f, indent=1)

@@ -63,6 +63,29 @@ def test_every_iteration_and_the_whole_run_match_the_oracle(mrdb, B, R, seed, sh
     assert g[0].shape[0] > 3 * xy.shape[0]
 
 
+@pytest.mark.parametrize("B,R,seed,shape", [(1.0, 0.07, 4, (6, 5)), (np.sqrt(2.0), 0.045, 5, (8, 6))])
+def test_refinement_with_morton_reordering_matches_the_oracle(mrdb, B, R, seed, shape):
+    """Section 4.1.4: vertices renumbered along the Morton curve after every insertion step -- every iteration and the whole
+    run array for array the oracle's, keys in ascending order at the end."""
+    xy, tv, te, et = start(seed, shape)
+    box = (0.0, 0.0, 2.0, 1.5)
+    state = (xy, tv, te, et)
+    for it in range(100):
+        o = mg.refine_iteration(*state, R, B, seed, it, box)
+        g = mrdb.meshgen_refine(*to_dev(*state), R, B, seed=seed, first_iteration=it, max_iterations=1, box=box)
+        assert same(g[:4], o[:4]), it
+        if o[4]["n_bad"] == 0:
+            break
+        state = o[:4]
+    g = mrdb.meshgen_refine(*to_dev(xy, tv, te, et), R, B, seed=seed, box=box)
+    assert same(g[:4], state) and g[4]["iterations"] == it and it >= 4
+    X = g[0].cpu().numpy()
+    keys = [mg.morton_key(x, y, box) for x, y in X]
+    assert keys == sorted(keys) and len(X) > 3 * len(xy)
+    with pytest.raises(mrdb.MrdError):
+        mrdb.meshgen_refine(*to_dev(xy, tv, te, et), R, B, box=(0.0, 0.0, 0.0, 1.0))
+
+
 def test_edge_insertions_on_a_uniform_mesh(mrdb):
     """Right isosceles triangles: every circumcentre is the midpoint of a hypotenuse -- on an interior edge (KIND_EDGE) or on a
     segment -- and every interior edge has four cocircular vertices (all INCIRCLE2D tests take the exact path)."""
