@@ -483,10 +483,10 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
     if (fused) {
       auto td = tile_dev<R>(m);
       if (!rk2)
-        mrd::slot_gather_update_kernel<R, 1><<<vb, 256, 0, s>>>(md, td, gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
+        mrd::slot_gather_update_kernel<R, 1><<<blocks_for(md.nv, mrd::VtxShape<R>::threads), mrd::VtxShape<R>::threads, 0, s>>>(md, td, gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
                                                              (const V4 *)m->d_W[a], (V4 *)m->d_W[b], sink_for<R>(m, b, true, false), m->d_flag);
       else
-        mrd::slot_gather_update_kernel<R, 0><<<vb, 256, 0, s>>>(md, td, gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
+        mrd::slot_gather_update_kernel<R, 0><<<blocks_for(md.nv, mrd::VtxShape<R>::threads), mrd::VtxShape<R>::threads, 0, s>>>(md, td, gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
                                                              (const V4 *)m->d_W[a], (V4 *)m->d_W[b], sink_for<R>(m, b, false, true), m->d_flag);
     } else {
       if (!rk2)
@@ -518,7 +518,7 @@ template <class R> void enqueue_step(mrd_mesh *m, int scheme, int a, cudaStream_
       PROF_MARK(MRD_PROF_WALL2)
     }
     if (fused)
-      mrd::slot_gather_update_kernel<R, 2><<<vb, 256, 0, s>>>(md, tile_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
+      mrd::slot_gather_update_kernel<R, 2><<<blocks_for(md.nv, mrd::VtxShape<R>::threads), mrd::VtxShape<R>::threads, 0, s>>>(md, tile_dev<R>(m), gamma, m->d_ctl, (const V4 *)m->d_part, (const V4 *)m->d_wall_acc,
                                                            (const V4 *)m->d_W[b], (V4 *)m->d_W[b], sink_for<R>(m, b, true, false), m->d_flag);
     else
       mrd::gather_update_kernel<R><<<vb, 256, 0, s>>>(md, gamma, m->d_ctl, (const V4 *)m->d_phi, (const V4 *)m->d_wall_acc, (V4 *)m->d_W[b],

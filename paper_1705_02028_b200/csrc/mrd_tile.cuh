@@ -462,8 +462,15 @@ slot_dt_kernel(MeshDev<R> m, TileDev<R> td, Ctl *__restrict__ ctl, const R *__re
 //   MODE 0: stage 1 of RK2   W* = W^n - dt/V sum        (Win -> Wout; Z*, dW/dt to the slots)
 //   MODE 1: single stage     W^{n+1} = W^n - dt/V sum   (Win -> Wout; Z, |v|+c to the slots)        eq. 43
 //   MODE 2: stage 2 of RK2   W^{n+1} = W* - dt/V sum    (in place: Win == Wout; Z, |v|+c to the slots) eq. 61
+// Launch shape (measured at 4096^2, profiles/r02_experiments.md section 7): blocks of 128 threads; in fp64 enough of them resident
+// that the three-level gather (vslot_off -> vslot_ent -> part) has more loads in flight -- 40 registers for the stage-1 update
+// (24 bytes spilled), 32 for the final update (40 bytes spilled): 0.614 -> 0.585 ms and 0.509 -> 0.472 ms.  In fp32 the register
+// caps lose (0.336 -> 0.395 ms for the stage-1 update), so there is no minimum (0).
+template <class R> struct VtxShape;
+template <> struct VtxShape<double> { static constexpr int threads = 128, minb_update = 12, minb_final = 16; };
+template <> struct VtxShape<float> { static constexpr int threads = 128, minb_update = 0, minb_final = 0; };
 template <class R, int MODE>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(VtxShape<R>::threads, MODE == 2 ? VtxShape<R>::minb_final : VtxShape<R>::minb_update)
 slot_gather_update_kernel(MeshDev<R> m, TileDev<R> td, R gamma, const Ctl *__restrict__ ctl,
                           const Vec4<R> *__restrict__ part, const Vec4<R> *__restrict__ wall_acc, const Vec4<R> *Win,
                           Vec4<R> *Wout, VertexSink<R> sink, int *status) {
