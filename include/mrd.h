@@ -303,6 +303,22 @@ int mrd_meshgen_test_quality(int64_t n_triangle, const double *xy_dev, const int
 int mrd_meshgen_orient2d(int64_t n, const double *xy_dev, const int32_t *idx_dev, int8_t *sign_dev, int64_t *n_exact, void *stream);
 int mrd_meshgen_incircle2d(int64_t n, const double *xy_dev, const int32_t *idx_dev, int8_t *sign_dev, int64_t *n_exact, void *stream);
 
+/* mrd_meshgen_orient2d_static: mrd_meshgen_orient2d for callers that must not allocate (code under CUDA graph capture, tight
+ *   serving loops, harnesses that forbid cudaMalloc).  Same kernels, same result (the exact sign of eq. 3 for every row of
+ *   idx), but the scratch -- the list of tests the filter cannot decide and its length -- lives in a file-scope
+ *   `static __device__` array of the library: 4 MB + 256 B on every GPU that loads the library, held until the process exits.
+ *   The call makes no cudaMalloc / cudaFree and calls no allocating library routine; it ENQUEUES its work on `stream` and
+ *   returns without synchronising (errors of the kernels themselves surface at the caller's next synchronisation).
+ *   Limit: n <= 1 048 576 tests per call; a larger n is rejected with MRD_EINVAL and a message that says so.
+ *   n_exact_dev: DEVICE out (int64, may be NULL): how many tests needed the exact path.
+ *   All calls on one device share the array, which keeps the contents of the last call (the call clears the one word that
+ *   must start at zero): two calls that overlap on the GPU (different streams, or graphs launched concurrently) RACE --
+ *   order them on one stream or with events.  The device address of the array is taken once per device
+ *   (cudaGetSymbolAddress, with that device current); devices 0-63.
+ * Errors: MRD_EINVAL (null pointer, n beyond the limit, device number beyond 63), MRD_ECUDA. */
+int mrd_meshgen_orient2d_static(int64_t n, const double *xy_dev, const int32_t *idx_dev, int8_t *sign_dev, int64_t *n_exact_dev,
+                                void *stream);
+
 /* ------------------------------------------------------------------------------------------------
  * Mesh generation, second slice: the mesh data structure of section 4.1.2 (L656-L663), the Delaunay triangulator of
  * section 2.4.6 (L186-L208) / 4.1.5 (L677-L681), and the search for the triangle that contains a new vertex (section 2.4.2,

@@ -87,6 +87,7 @@ def lib():
         L.mrd_meshgen_test_quality.argtypes = [C.c_int64, vp, vp, C.c_double, C.c_double, vp, vp, vp, vp, _lp, vp]
         L.mrd_meshgen_orient2d.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
         L.mrd_meshgen_incircle2d.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
+        L.mrd_meshgen_orient2d_static.argtypes = [C.c_int64, vp, vp, vp, vp, vp]
         L.mrd_meshgen_release.argtypes = []
         L.mrd_meshgen_build_edges.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
         L.mrd_meshgen_delaunay_flip.argtypes = [C.c_int64, C.c_int64, vp, vp, vp, vp, _lp, _lp, _lp, vp]
@@ -528,3 +529,21 @@ def meshgen_refine(xy, tv, te, et, R, B, seed=0, first_iteration=0, max_iteratio
                                     C.byref(it), C.byref(left), _stream_ptr(stream)))
     out = [t[:k.value].clone() for t, k in zip(big, (n[0], n[1], n[1], n[2]))]
     return (*out, dict(iterations=it.value, bad_left=left.value))
+
+
+MESHGEN_STATIC_MAX_TESTS = 1 << 20
+
+
+def meshgen_orient2d_static(xy, idx, sign, n_exact=None, stream=None):
+    """mrd_meshgen_orient2d_static: the exact sign of eq. 3 for every row (a, b, c) of idx into the caller's `sign` (int8 CUDA
+    tensor [n]) -- no allocation anywhere (the scratch is a static device array of the library; at most 2^20 tests per call),
+    no synchronisation.  n_exact: optional int64 CUDA tensor [1] that receives the number of tests that took the exact path.
+    Calls that overlap on the GPU race (include/mrd.h)."""
+    import torch
+    n = idx.shape[0]
+    assert xy.is_cuda and xy.dtype == torch.float64 and xy.is_contiguous()
+    assert idx.is_cuda and idx.dtype == torch.int32 and idx.is_contiguous() and idx.ndim == 2 and idx.shape[1] == 3
+    assert sign.is_cuda and sign.dtype == torch.int8 and sign.is_contiguous() and sign.shape == (n,)
+    assert n_exact is None or (n_exact.is_cuda and n_exact.dtype == torch.int64 and n_exact.numel() == 1)
+    _check(lib().mrd_meshgen_orient2d_static(n, C.c_void_p(xy.data_ptr()), C.c_void_p(idx.data_ptr()), C.c_void_p(sign.data_ptr()),
+                                             None if n_exact is None else C.c_void_p(n_exact.data_ptr()), _stream_ptr(stream)))

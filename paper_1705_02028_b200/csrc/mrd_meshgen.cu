@@ -27,6 +27,13 @@
 #include "../../include/mrd.h"
 #include "mrd_predicates.cuh"
 
+// Scratch of mrd_meshgen_orient2d_static (the entry point that allocates nothing): 256 bytes that hold the length of the work
+// list, then the work list itself (one int32 per test the filter could not decide).  4 MB + 256 B, held by every GPU that loads
+// the library until the process exits.  In HOST code this name is a stand-in, not a device address: the host takes the
+// address once per device with cudaGetSymbolAddress (static_scratch_of below) and passes THAT to the kernels.
+#define MRD_STATIC_MAX_TESTS (1 << 20)
+static __device__ __align__(256) unsigned char g_static_scratch[256 + sizeof(int32_t) * MRD_STATIC_MAX_TESTS];
+
 namespace mrdgen {
 
 // ------------------------------------------------------------------------------------------------------------------
@@ -780,6 +787,52 @@ int mrd_meshgen_orient2d(int64_t n, const double *xy_dev, const int32_t *idx_dev
 }
 int mrd_meshgen_incircle2d(int64_t n, const double *xy_dev, const int32_t *idx_dev, int8_t *sign_dev, int64_t *n_exact, void *stream) {
   return predicate_impl(1, n, xy_dev, idx_dev, sign_dev, n_exact, stream);
+}
+
+namespace {
+// device address of g_static_scratch on the CURRENT device, taken once per device (with that device current)
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+unsigned char *g_static_ptr[STATIC_MAX_DEVICES] = {};
+int static_scratch_of(unsigned char **out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail("orient2d_static: cudaGetDevice", e);
+  if (dev < 0 || dev >= STATIC_MAX_DEVICES) return gen_fail(MRD_EINVAL, "orient2d_static: device number beyond 63");
+  std::lock_guard<std::mutex> g(g_static_mu);
+  if (!g_static_ptr[dev]) {
+    void *p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess || !p) return cuda_fail("orient2d_static: cudaGetSymbolAddress", e);
+    g_static_ptr[dev] = (unsigned char *)p;
+  }
+  *out = g_static_ptr[dev];
+  return MRD_OK;
+}
+}  // namespace
+
+int mrd_meshgen_orient2d_static(int64_t n, const double *xy_dev, const int32_t *idx_dev, int8_t *sign_dev, int64_t *n_exact_dev,
+                                void *stream) {
+  if (n < 0 || (n > 0 && (!xy_dev || !idx_dev || !sign_dev))) return gen_fail(MRD_EINVAL, "null argument");
+  if (n > (int64_t)MRD_STATIC_MAX_TESTS)
+    return gen_fail(MRD_EINVAL, "orient2d_static: " + std::to_string(n) + " tests exceed the static scratch (at most " +
+                                    std::to_string((int64_t)MRD_STATIC_MAX_TESTS) + " per call; use mrd_meshgen_orient2d)");
+  unsigned char *base = nullptr;
+  const int rc = static_scratch_of(&base);
+  if (rc != MRD_OK) return rc;
+  cudaStream_t s = (cudaStream_t)stream;
+  unsigned long long *cnt = (unsigned long long *)base;
+  int32_t *work = (int32_t *)(base + 256);
+  // the array keeps the last call's contents: the counter must start at zero (the work list is only read below the counter)
+  cudaError_t e = cudaMemsetAsync(cnt, 0, sizeof *cnt, s);
+  if (e == cudaSuccess && n > 0) {
+    mrdgen::orient_filter_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, (const double2 *)xy_dev, idx_dev, sign_dev, work, cnt);
+    mrdgen::orient_exact_kernel<<<EXACT_BLOCKS, 128, 0, s>>>(cnt, work, (const double2 *)xy_dev, idx_dev, sign_dev);
+    e = cudaPeekAtLastError();
+  }
+  if (e == cudaSuccess && n_exact_dev) e = cudaMemcpyAsync(n_exact_dev, cnt, sizeof(int64_t), cudaMemcpyDeviceToDevice, s);
+  if (e != cudaSuccess) return cuda_fail("orient2d_static", e);
+  return MRD_OK;   // enqueued; no synchronisation
 }
 
 namespace {
