@@ -368,14 +368,9 @@ def morton_order(xy, tv, box):
     return np.asarray(xy)[order].copy(), canonical_order(new[np.asarray(tv)]), new
 
 
-def refine_iteration(xy, tv, te, et, R, B, seed, iteration, box=None):
-    """One iteration of section 2.4 on a Delaunay triangulation: TestQuality; for every bad triangle, in ascending order, its
-    candidate; cavities and the independent set of section 4.1.1 (a triangle claimed by several cavities goes to the highest
-    priority; a candidate is selected when it holds every triangle of its cavity); the selected vertices are numbered, and
-    their triangles and edges appended, in ascending order of their bad triangle; flips restore the Delaunay property; the
-    triangles are put in canonical order (reading M12) -- after the vertices have been renumbered along the Morton curve of
-    the rectangle `box` = (x0, y0, x1, y1), when one is given (section 4.1.4, reading M14).
-    Returns (xy, tv, te, et, info) as new arrays; info: n_bad, n_selected, kinds of the selected, flips."""
+def _insert_and_flip(xy, tv, te, et, R, B, seed, iteration):
+    """Steps 2.4.1-2.4.6 of one iteration (everything but the re-sort): returns the enlarged arrays, Delaunay again, numbered as
+    the insertions and flips left them (which depends on the order of the flips), and the info record."""
     xy = np.asarray(xy, dtype=np.float64)
     q = test_quality(xy, tv, R, B)
     bad = np.nonzero(q["bad"])[0]
@@ -406,26 +401,113 @@ def refine_iteration(xy, tv, te, et, R, B, seed, iteration, box=None):
         dt, de = insert_vertex(tv2, te2, et2, kind, t_ins, e, nv + j, nt, ne)
         nt, ne = nt + dt, ne + de
     flips = flip_to_delaunay(xy2, tv2, te2, et2)
-    if box is not None:                                           # section 4.1.4: Morton order after every insertion step
-        xy2, tv2, _ = morton_order(xy2, tv2, box)
-    else:
-        tv2 = canonical_order(tv2)
-    te2, et2 = build_edges(tv2)
     info = dict(n_bad=len(bad), n_candidates=len(cands), n_selected=len(sel), kinds=[cd[1] for cd in sel], flips=flips,
                 selected=[(cd[0], cd[1], cd[2], cd[5]) for cd in sel])
     return xy2, tv2, te2, et2, info
 
 
+def refine_iteration(xy, tv, te, et, R, B, seed, iteration, box=None):
+    """One iteration of section 2.4 on a Delaunay triangulation: TestQuality; for every bad triangle, in ascending order, its
+    candidate; cavities and the independent set of section 4.1.1 (a triangle claimed by several cavities goes to the highest
+    priority; a candidate is selected when it holds every triangle of its cavity); the selected vertices are numbered, and
+    their triangles and edges appended, in ascending order of their bad triangle; flips restore the Delaunay property; the
+    triangles are put in canonical order (reading M12) -- after the vertices have been renumbered along the Morton curve of
+    the rectangle `box` = (x0, y0, x1, y1), when one is given (section 4.1.4, reading M14).
+    Returns (xy, tv, te, et, info) as new arrays; info: n_bad, n_selected, kinds of the selected, flips."""
+    xy2, tv2, te2, et2, info = _insert_and_flip(xy, tv, te, et, R, B, seed, iteration)
+    if box is not None:                                           # section 4.1.4: Morton order after every insertion step
+        xy2, tv2, _ = morton_order(xy2, tv2, box)
+    else:
+        tv2 = canonical_order(tv2)
+    te2, et2 = build_edges(tv2)
+    return xy2, tv2, te2, et2, info
+
+
+def _canon(row):
+    a, b, c = (int(v) for v in row)
+    m = min(a, b, c)
+    return (a, b, c) if a == m else (b, c, a) if b == m else (c, a, b)
+
+
+def renumber_in_place(tv0, te0, et0, tv2):
+    """Reading M15: the numbering an iteration leaves behind when it is NOT followed by a re-sort.  tv0, te0, et0: the mesh
+    before the iteration; tv2: the triangles after it, in any order and rotation.  A triangle that survives the iteration keeps
+    its number and its rotation; the numbers of the triangles that did not survive, and the new numbers at the end, go to the
+    triangles the iteration created, in ascending order of their vertex triple (each rotated to its smallest vertex).  Edges
+    likewise, by their pair of end points (smaller, larger).  te and et then follow from the triangles (edge k opposite local
+    vertex k; neighbours in ascending order, -1 for the missing one).  Nothing here depends on the order in which the flips
+    happened.  Returns (tv, te, et)."""
+    nt0, nt2 = np.asarray(tv0).shape[0], np.asarray(tv2).shape[0]
+    final = triangle_set(tv2)
+    kept = [s for s in range(nt0) if _canon(tv0[s]) in final]
+    kept_set = set(kept)
+    free = [s for s in range(nt0) if s not in kept_set] + list(range(nt0, nt2))
+    added = sorted(final - {_canon(tv0[s]) for s in kept})
+    assert len(free) == len(added)
+    tv = np.full((nt2, 3), -1, dtype=np.int32)
+    for s in kept:
+        tv[s] = tv0[s]
+    for s, row in zip(free, added):
+        tv[s] = row
+    # edges: end points of the old slots, the edge set of the new triangulation
+    def sides(rows):
+        out = {}
+        for t, (a, b, c) in enumerate(np.asarray(rows).tolist()):
+            for k, (u, w) in enumerate(((b, c), (c, a), (a, b))):
+                out.setdefault((min(u, w), max(u, w)), []).append((t, k))
+        return out
+    ne0 = np.asarray(et0).shape[0]
+    old_ends = {}
+    for (u, w), uses in sides(tv0).items():
+        t, k = uses[0]
+        old_ends[int(te0[t, k])] = (u, w)
+    new_sides = sides(tv)
+    ne2 = len(new_sides)
+    slot = {}
+    for e in range(ne0):
+        if old_ends[e] in new_sides:
+            slot[old_ends[e]] = e
+    free_e = [e for e in range(ne0) if old_ends[e] not in new_sides] + list(range(ne0, ne2))
+    added_e = sorted(k for k in new_sides if k not in slot)
+    assert len(free_e) == len(added_e)
+    for e, key in zip(free_e, added_e):
+        slot[key] = e
+    te = np.full((nt2, 3), -1, dtype=np.int32)
+    et = np.full((ne2, 2), -1, dtype=np.int32)
+    for key, uses in new_sides.items():
+        e = slot[key]
+        for j, (t, k) in enumerate(sorted(uses)):
+            te[t, k] = e
+            et[e, j] = t
+    return tv, te, et
+
+
+def refine_iteration_in_place(xy, tv, te, et, R, B, seed, iteration):
+    """One iteration as refine_iteration, but WITHOUT the re-sort: the mesh keeps its numbering where it did not change
+    (renumber_in_place, reading M15).  This is what the iterations of refine() do when no Morton box is given."""
+    xy2, tv2, te2, et2, info = _insert_and_flip(xy, tv, te, et, R, B, seed, iteration)
+    tv3, te3, et3 = renumber_in_place(tv, te, et, tv2)
+    return xy2, tv3, te3, et3, info
+
+
 def refine(xy, tv, R, B, seed=0, max_iterations=10 ** 6, box=None):
-    """Section 2.4: iterate "until no more vertices need to be inserted".  The input is made Delaunay first.
-    Returns (xy, tv, te, et, number of iterations that inserted something)."""
+    """Section 2.4: iterate "until no more vertices need to be inserted".  The input is made Delaunay and put in canonical
+    order first.  With a Morton `box` every iteration ends with the re-sort of section 4.1.4 (readings M12, M14); without one
+    the iterations renumber in place (reading M15) and ONE canonical re-sort follows the last of them (so a run of a single
+    iteration is refine_iteration either way).  Returns (xy, tv, te, et, number of iterations that inserted something)."""
     xy = np.asarray(xy, dtype=np.float64)
     tv = canonical_order(delaunay_flip(xy, tv)[0])
     te, et = build_edges(tv)
     it = 0
     while it < max_iterations:
-        xy, tv, te, et, info = refine_iteration(xy, tv, te, et, R, B, seed, it, box)
+        if box is not None:
+            xy, tv, te, et, info = refine_iteration(xy, tv, te, et, R, B, seed, it, box)
+        else:
+            xy, tv, te, et, info = refine_iteration_in_place(xy, tv, te, et, R, B, seed, it)
         if info["n_bad"] == 0:
             break
         it += 1
+    if box is None and it > 0:
+        tv = canonical_order(tv)
+        te, et = build_edges(tv)
     return xy, tv, te, et, it

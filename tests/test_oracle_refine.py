@@ -226,3 +226,55 @@ def test_morton_order_follows_the_z_curve_and_changes_numbers_only():
     assert q["bad"].sum() == 0 and mg.triangle_set(ta) == library_triangulation(xa)
     ka = [mg.morton_key(x, y, box) for x, y in xa]
     assert ka == sorted(ka)
+
+
+def test_in_place_renumbering_keeps_survivors_and_does_not_depend_on_the_flip_order():
+    """Reading M15 (renumber_in_place): what an iteration without re-sort leaves behind."""
+    xy, tv, te, et = start_mesh(seed=7, shape=(10, 8))
+    tv = mg.canonical_order(tv)
+    te, et = mg.build_edges(tv)
+    xy2, tvr, ter, etr, info = mg.refine_iteration(xy, tv, te, et, 0.3, 0.9, seed=5, iteration=0)
+    xy3, tvp, tep, etp, _ = mg.refine_iteration_in_place(xy, tv, te, et, 0.3, 0.9, seed=5, iteration=0)
+    assert np.array_equal(xy2, xy3) and 0 < info["n_selected"]
+    assert_structure(xy3, tvp, tep, etp)
+    assert mg.triangle_set(tvp) == mg.triangle_set(tvr)           # the same mesh ...
+    tvs = mg.canonical_order(tvp)
+    assert np.array_equal(tvs, tvr) and all(np.array_equal(a, b) for a, b in zip(mg.build_edges(tvs), (ter, etr)))   # ... and the same after a re-sort
+    nt0, ne0 = tv.shape[0], et.shape[0]
+    final = mg.triangle_set(tvp)
+    survives = np.array([mg._canon(r) in final for r in tv])
+    assert 0.2 < survives.mean() < 1.0
+    assert np.array_equal(tvp[:nt0][survives], tv[survives])      # survivors: same number, same rotation
+    assert np.array_equal(tep[:nt0][survives], te[survives])      # ... and so the same edges
+    free = np.concatenate([np.nonzero(~survives)[0], np.arange(nt0, tvp.shape[0])])
+    rows = tvp[free]
+    assert (rows[:, 0] < rows[:, 1]).all() and (rows[:, 0] < rows[:, 2]).all()
+    assert (np.lexsort((rows[:, 2], rows[:, 1], rows[:, 0])) == np.arange(len(rows))).all()    # created triangles: ascending triples into ascending slots
+    assert ((etp[:, 1] < 0) | (etp[:, 0] < etp[:, 1])).all()
+    old_pairs = {tuple(sorted(mg._edge_ends(tv, te, int(et[e, 0]), e))): e for e in range(ne0)}
+    new_pairs = {tuple(sorted(mg._edge_ends(tvp, tep, int(etp[e, 0]), e))): e for e in range(etp.shape[0])}
+    same = [k for k in old_pairs if k in new_pairs]
+    assert len(same) > 0.2 * ne0 and all(old_pairs[k] == new_pairs[k] for k in same)            # surviving edges keep their numbers
+    created = sorted(k for k in new_pairs if k not in old_pairs)
+    assert [new_pairs[k] for k in created] == sorted(new_pairs[k] for k in created)
+    # any numbering and rotation of the triangles after the flips gives the same result
+    rng = np.random.default_rng(1)
+    sh = tvr[rng.permutation(tvr.shape[0])]
+    rot = rng.integers(0, 3, size=sh.shape[0])
+    sh = np.stack([sh[np.arange(len(rot)), (rot + j) % 3] for j in range(3)], axis=1).astype(np.int32)
+    again = mg.renumber_in_place(tv, te, et, sh)
+    assert all(np.array_equal(a, b) for a, b in zip(again, (tvp, tep, etp)))
+
+
+def test_refine_without_box_is_in_place_iterations_and_one_final_sort():
+    xy0, tv0, te0, et0 = start_mesh(seed=2)
+    xy, tv, te, et, it = mg.refine(xy0, tv0, 0.09, 1.0, seed=6)
+    sx, st = xy0, mg.canonical_order(tv0)
+    ste, set_ = mg.build_edges(st)
+    for k in range(it):
+        sx, st, ste, set_, info = mg.refine_iteration_in_place(sx, st, ste, set_, 0.09, 1.0, 6, k)
+        assert info["n_selected"] > 0
+    assert mg.refine_iteration_in_place(sx, st, ste, set_, 0.09, 1.0, 6, it)[4]["n_bad"] == 0
+    assert np.array_equal(xy, sx) and np.array_equal(tv, mg.canonical_order(st))
+    assert np.array_equal(mg.refine(xy0, tv0, 0.09, 1.0, seed=6, max_iterations=1)[1],
+                          mg.refine_iteration(xy0, mg.canonical_order(tv0), *mg.build_edges(mg.canonical_order(tv0)), 0.09, 1.0, 6, 0)[1])
