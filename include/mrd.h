@@ -383,12 +383,16 @@ int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_
  *      one triangle at a segment split in two), numbered -- like their new triangles and edges -- in ascending order of
  *      their bad triangle;
  *   6. flips restore the Delaunay property (2.4.6);
- *   7. re-sort (4.1.4): when `box` = (x0, y0, x1, y1) (HOST, the rectangle the domain lies in) is given, the vertices are
- *      renumbered in ascending Morton value -- 21 bits per coordinate, i = min(2^21 - 1, floor((x - x0) * (2^21 / (x1 - x0)))),
- *      x in the even bit places, ties keep their order -- and xy, tv follow; with box = NULL the vertices keep their numbers
- *      (input vertices first, inserted ones in order of insertion).  Then the triangles are renumbered canonically (each
- *      rotated to its smallest vertex, sorted by vertex triple: along the same curve when the vertices are) and te, et
- *      rebuilt as by mrd_meshgen_build_edges.
+ *   7. numbering.  With `box` = (x0, y0, x1, y1) (HOST, the rectangle the domain lies in) every iteration ends with the
+ *      re-sort of 4.1.4: the vertices are renumbered in ascending Morton value -- 21 bits per coordinate,
+ *      i = min(2^21 - 1, floor((x - x0) * (2^21 / (x1 - x0)))), x in the even bit places, ties keep their order -- and xy, tv
+ *      follow; then the triangles are renumbered canonically (each rotated to its smallest vertex, sorted by vertex triple:
+ *      along the same curve) and te, et rebuilt as by mrd_meshgen_build_edges.
+ *      With box = NULL the vertices keep their numbers (input vertices first, inserted ones in order of insertion) and the
+ *      iterations renumber IN PLACE: a triangle or edge that survives an iteration keeps its number (and rotation); the
+ *      numbers of those that did not, and the new numbers at the end, go to the triangles / edges the iteration created,
+ *      in ascending order of their vertex triple / pair of end points.  ONE canonical re-sort (as above, without the
+ *      vertices) follows the last iteration of the call, whatever ended it.
  *   Every step is deterministic and independent of the order in which threads run: the result is, array for array, the one
  *   of oracle/meshgen.py: refine.
  *   In: a Delaunay triangulation (xy, tv, te, et) with *n_vertex, *n_triangle, *n_edge entries in device arrays with room

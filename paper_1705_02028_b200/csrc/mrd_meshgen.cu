@@ -153,6 +153,21 @@ edge_fill_kernel(int64_t n, const unsigned long long *__restrict__ key, const in
 // ------------------------------------------------------------------------------------------------------------------
 struct FlipCounters { unsigned long long n_work, n_bad, n_flip, n_next, n_exact; };
 
+// Bookkeeping of the refinement's in-place renumbering (reading M15), all optional (null members: nothing is recorded):
+// T[t] / E[e] = 1 when triangle slot t / edge slot e received a new content (its old triangle / edge does not exist any
+// more, or the slot is new); list / n: the edges whose quadrilateral changed, once each (mark[e] = -1), as the first
+// candidates of the flip loop.
+struct Touch {
+  uint8_t *T, *E;
+  int32_t *mark, *list;
+  unsigned long long *n;
+  __device__ __forceinline__ void tri(int32_t t) const { if (T) T[t] = 1; }
+  __device__ __forceinline__ void edge(int32_t e) const { if (E) E[e] = 1; }
+  __device__ __forceinline__ void check(int32_t e) const {
+    if (list && atomicExch(mark + e, -1) != -1) list[atomicAdd(n, 1ull)] = e;
+  }
+};
+
 struct Quad { int32_t t1, t2; double2 a, b, c, d; };
 static __device__ __forceinline__ bool load_quad(int32_t e, const double2 *xy, const int32_t *tv, const int32_t *te, const int32_t *et, Quad &q) {
   q.t1 = et[2 * (int64_t)e];
@@ -176,9 +191,11 @@ static __device__ __forceinline__ void bid(int32_t e, const Quad &q, unsigned lo
 __global__ void __launch_bounds__(256)
 check_edge_kernel(int64_t n, const int32_t *__restrict__ cand, const double2 *__restrict__ xy, const int32_t *__restrict__ tv,
                   const int32_t *__restrict__ te, const int32_t *__restrict__ et, int8_t *__restrict__ state,
-                  unsigned long long *__restrict__ lock, unsigned long long stamp, int32_t *__restrict__ work, FlipCounters *c) {
+                  unsigned long long *__restrict__ lock, unsigned long long stamp, int32_t *__restrict__ work, FlipCounters *c,
+                  const unsigned long long *__restrict__ n_dev) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   bool bad = false;
+  if (n_dev) n = min(n, (int64_t)*n_dev);                          // (the host knows only an upper bound of the list's length)
   if (i < n) {
     const int32_t e = cand ? cand[i] : (int32_t)i;
     Quad q;
@@ -214,8 +231,10 @@ check_edge_exact_kernel(const int32_t *__restrict__ work, const double2 *__restr
 __global__ void __launch_bounds__(256)
 flip_kernel(int64_t n, const int32_t *__restrict__ cand, int32_t *__restrict__ tv, int32_t *__restrict__ te, int32_t *__restrict__ et,
             int8_t *__restrict__ state, const unsigned long long *__restrict__ lock, unsigned long long stamp, int32_t iter,
-            int32_t *__restrict__ mark, int32_t *__restrict__ next, FlipCounters *c) {
+            int32_t *__restrict__ mark, int32_t *__restrict__ next, FlipCounters *c, const unsigned long long *__restrict__ n_dev,
+            Touch touch) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (n_dev) n = min(n, (int64_t)*n_dev);
   int32_t items[4];                                              // this thread's candidates for the next iteration
   int cnt = 0;
   bool flipped = false;
@@ -242,6 +261,9 @@ flip_kernel(int64_t n, const int32_t *__restrict__ cand, int32_t *__restrict__ t
       f = et + 2 * (int64_t)e_ca;
       f[f[0] == t1 ? 0 : 1] = t2;
       state[e] = 0;                                              // "E' would be locally Delaunay" (L102)
+      touch.tri(t1);
+      touch.tri(t2);
+      touch.edge(e);
       const int32_t outer[4] = {e_ca, e_ab, e_bd, e_dc};         // their quadrilaterals changed: check them next
 #pragma unroll
       for (int j = 0; j < 4; ++j)
@@ -552,7 +574,7 @@ __global__ void __launch_bounds__(128)
 insert_kernel(int64_t nc, const int8_t *__restrict__ kind, const double2 *__restrict__ pt, const int32_t *__restrict__ t_ins,
               const int32_t *__restrict__ e_ins, const int32_t *__restrict__ sel, const int32_t *__restrict__ rank,
               const int32_t *__restrict__ segrank, int32_t nv, int32_t nt, int32_t ne, double2 *__restrict__ xy,
-              int32_t *__restrict__ tv, int32_t *__restrict__ te, int32_t *__restrict__ et) {
+              int32_t *__restrict__ tv, int32_t *__restrict__ te, int32_t *__restrict__ et, Touch touch) {
   const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= nc || !sel[j]) return;
   const int32_t v = nv + rank[j];
@@ -571,6 +593,9 @@ insert_kernel(int64_t nc, const int8_t *__restrict__ kind, const double2 *__rest
     et[2 * (int64_t)f2] = t1; et[2 * (int64_t)f2 + 1] = t2;
     swap_side(et, e0, t, t1);
     swap_side(et, e1, t, t2);
+    touch.tri(t); touch.tri(t1); touch.tri(t2);
+    touch.edge(f0); touch.edge(f1); touch.edge(f2);
+    touch.check(e0); touch.check(e1); touch.check(e2); touch.check(f0); touch.check(f1); touch.check(f2);
     return;
   }
   const int i1 = local_of(E, e);
@@ -583,6 +608,9 @@ insert_kernel(int64_t nc, const int8_t *__restrict__ kind, const double2 *__rest
     et[2 * (int64_t)g0] = n1; et[2 * (int64_t)g0 + 1] = -1;
     et[2 * (int64_t)g1] = t; et[2 * (int64_t)g1 + 1] = n1;
     swap_side(et, e_ca, t, n1);
+    touch.tri(t); touch.tri(n1);
+    touch.edge(e); touch.edge(g0); touch.edge(g1);               // E = (b, c) is (b, v) now
+    touch.check(e); touch.check(g0); touch.check(g1); touch.check(e_ca); touch.check(e_ab);
     return;
   }
   const int32_t t2 = across(et, e, t);
@@ -599,6 +627,10 @@ insert_kernel(int64_t nc, const int8_t *__restrict__ kind, const double2 *__rest
   et[2 * (int64_t)g2] = t2; et[2 * (int64_t)g2 + 1] = n2;
   swap_side(et, e_ca, t, n1);
   swap_side(et, e_dc, t2, n2);
+  touch.tri(t); touch.tri(n1); touch.tri(t2); touch.tri(n2);
+  touch.edge(e); touch.edge(g0); touch.edge(g1); touch.edge(g2);
+  touch.check(e); touch.check(g0); touch.check(g1); touch.check(g2);
+  touch.check(e_ca); touch.check(e_ab); touch.check(e_bd); touch.check(e_dc);
 }
 // Morton value of every vertex (section 4.1.4; reading M14): 21 bits per coordinate, x in the even places
 static __device__ __forceinline__ unsigned long long spread21(unsigned v) {
@@ -636,6 +668,107 @@ relabel_kernel(int64_t n, const int32_t *__restrict__ number, int32_t *__restric
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) tv[i] = number[tv[i]];
 }
+// ---- in-place renumbering (reading M15; oracle/meshgen.py: renumber_in_place) ---------------------------------------------
+// S: the touched triangle slots in ascending order.  Rotate their rows (tv and te together) to the smallest vertex; sort keys.
+__global__ void __launch_bounds__(256)
+touched_keys_kernel(int64_t ns, const int32_t *__restrict__ S, int32_t *__restrict__ tv, int32_t *__restrict__ te, int bits,
+                    unsigned long long *__restrict__ key_lo, int32_t *__restrict__ idx) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= ns) return;
+  int32_t *v = tv + 3 * (int64_t)S[i], *ed = te + 3 * (int64_t)S[i];
+  const int32_t a = v[0], b = v[1], c = v[2], ea = ed[0], eb = ed[1], ec = ed[2];
+  const int r = (a < b && a < c) ? 0 : ((b < a && b < c) ? 1 : 2);
+  const int32_t x = r == 0 ? a : (r == 1 ? b : c), y = r == 0 ? b : (r == 1 ? c : a), z = r == 0 ? c : (r == 1 ? a : b);
+  put3(v, x, y, z);
+  put3(ed, r == 0 ? ea : (r == 1 ? eb : ec), r == 0 ? eb : (r == 1 ? ec : ea), r == 0 ? ec : (r == 1 ? ea : eb));
+  key_lo[i] = ((unsigned long long)(unsigned)y << bits) | (unsigned)z;
+  idx[i] = (int32_t)i;
+}
+__global__ void __launch_bounds__(256)
+touched_first_kernel(int64_t ns, const int32_t *__restrict__ S, const int32_t *__restrict__ tv, const int32_t *__restrict__ idx,
+                     unsigned *__restrict__ key_hi) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < ns) key_hi[i] = (unsigned)tv[3 * (int64_t)S[idx[i]]];
+}
+// order[r]: which entry of S holds the r-th smallest triple.  It moves to slot S[r].
+__global__ void __launch_bounds__(256)
+tri_map_kernel(int64_t ns, const int32_t *__restrict__ S, const int32_t *__restrict__ order, const int32_t *__restrict__ tv,
+               const int32_t *__restrict__ te, int32_t *__restrict__ tri_map, int32_t *__restrict__ tmp_tv, int32_t *__restrict__ tmp_te) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= ns) return;
+  const int32_t told = S[order[r]];
+  tri_map[told] = S[r];
+  const int32_t *v = tv + 3 * (int64_t)told, *ed = te + 3 * (int64_t)told;
+  put3(tmp_tv + 3 * r, v[0], v[1], v[2]);
+  put3(tmp_te + 3 * r, ed[0], ed[1], ed[2]);
+}
+// SE: the touched edge slots in ascending order; key = (smaller end point, larger end point)
+__global__ void __launch_bounds__(256)
+touched_edge_keys_kernel(int64_t nse, const int32_t *__restrict__ SE, const int32_t *__restrict__ tv, const int32_t *__restrict__ te,
+                         const int32_t *__restrict__ et, int bits, unsigned long long *__restrict__ key, int32_t *__restrict__ idx) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nse) return;
+  const int32_t e = SE[i], t = et[2 * (int64_t)e];
+  const int k = local_of(te + 3 * (int64_t)t, e);
+  const unsigned u = (unsigned)tv[3 * (int64_t)t + (k + 1) % 3], w = (unsigned)tv[3 * (int64_t)t + (k + 2) % 3];
+  key[i] = ((unsigned long long)min(u, w) << bits) | max(u, w);
+  idx[i] = (int32_t)i;
+}
+__global__ void __launch_bounds__(256)
+edge_map_kernel(int64_t nse, const int32_t *__restrict__ SE, const int32_t *__restrict__ order, const int32_t *__restrict__ et,
+                int32_t *__restrict__ edge_map, int2 *__restrict__ tmp_et) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= nse) return;
+  const int32_t eold = SE[order[r]];
+  edge_map[eold] = SE[r];
+  tmp_et[r] = make_int2(et[2 * (int64_t)eold], et[2 * (int64_t)eold + 1]);
+}
+// where, in the pair of an UNTOUCHED edge, a touched triangle is named (read before anything is rewritten)
+__global__ void __launch_bounds__(256)
+side_pos_kernel(int64_t ns, const int32_t *__restrict__ S, const int32_t *__restrict__ order, const int32_t *__restrict__ tmp_te,
+                const uint8_t *__restrict__ touch_e, const int32_t *__restrict__ et, int8_t *__restrict__ jpos) {
+  const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= 3 * ns) return;
+  const int64_t r = q / 3;
+  const int32_t eold = tmp_te[q], told = S[order[r]];
+  jpos[q] = touch_e[eold] ? (int8_t)-1 : (int8_t)(et[2 * (int64_t)eold] == told ? 0 : 1);
+}
+// the rows go to their new slots, with the new numbers of the edges and triangles they name
+__global__ void __launch_bounds__(256)
+renumber_scatter_kernel(int64_t ns, int64_t nse, const int32_t *__restrict__ S, const int32_t *__restrict__ SE,
+                        const int32_t *__restrict__ tmp_tv, const int32_t *__restrict__ tmp_te, const int2 *__restrict__ tmp_et,
+                        const int8_t *__restrict__ jpos, const uint8_t *__restrict__ touch_e, const int32_t *__restrict__ tri_map,
+                        const int32_t *__restrict__ edge_map, int32_t *__restrict__ tv, int32_t *__restrict__ te, int32_t *__restrict__ et) {
+  const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r < ns) {
+    const int32_t s = S[r];
+    put3(tv + 3 * (int64_t)s, tmp_tv[3 * r], tmp_tv[3 * r + 1], tmp_tv[3 * r + 2]);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const int32_t eold = tmp_te[3 * r + k];
+      if (touch_e[eold]) te[3 * (int64_t)s + k] = edge_map[eold];
+      else {
+        te[3 * (int64_t)s + k] = eold;
+        et[2 * (int64_t)eold + jpos[3 * r + k]] = s;                // an untouched edge keeps its slot; its neighbour moved
+      }
+    }
+  }
+  if (r < nse) {                                                   // a touched edge lies between touched triangles only
+    const int2 p = tmp_et[r];
+    const int32_t x = tri_map[p.x], y = p.y >= 0 ? tri_map[p.y] : -1;
+    *reinterpret_cast<int2 *>(et + 2 * (int64_t)SE[r]) = (y >= 0 && x > y) ? make_int2(y, x) : make_int2(x, y);
+  }
+}
+// neighbours in ascending order (one 8-byte load and store per pair: two threads that meet at an edge write the same value)
+__global__ void __launch_bounds__(256)
+renumber_order_kernel(int64_t ns, const int32_t *__restrict__ S, const int32_t *__restrict__ te, int32_t *__restrict__ et) {
+  const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= 3 * ns) return;
+  int2 *pair = reinterpret_cast<int2 *>(et + 2 * (int64_t)te[3 * (int64_t)S[q / 3] + q % 3]);
+  const int2 p = *pair;
+  if (p.y >= 0 && p.x > p.y) *pair = make_int2(p.y, p.x);
+}
+
 // canonical order (reading M12): rotate every triangle to its smallest vertex; sort keys (second, third) and (first)
 __global__ void __launch_bounds__(256)
 canonical_keys_kernel(int64_t nt, int32_t *__restrict__ tv, int bits, unsigned long long *__restrict__ key_lo, int32_t *__restrict__ idx) {
@@ -897,8 +1030,15 @@ struct FlipWork {
   }
 };
 // flips (tv, te, et) to the Delaunay triangulation (arena reserved and locked by the caller); synchronises s every iteration
+// `init` (refinement only): the caller has cleared state / lock / mark, put the first candidates into the list at w.o_l0 (their
+// number in device memory, n_upper an upper bound of it) and wants touched slots recorded
+struct FlipInit {
+  const unsigned long long *n_dev;
+  int64_t n_upper;
+  mrdgen::Touch touch;
+};
 int flip_run(const FlipWork &w, size_t o_scratch, int64_t n_triangle, int64_t n_edge, const double2 *xy, int32_t *tv_dev, int32_t *te_dev,
-             int32_t *et_dev, int64_t *flips_out, int64_t *iters_out, int64_t *exact_out, cudaStream_t s) {
+             int32_t *et_dev, int64_t *flips_out, int64_t *iters_out, int64_t *exact_out, cudaStream_t s, const FlipInit *init = nullptr) {
   using mrdgen::FlipCounters;
   const size_t nt = (size_t)std::max<int64_t>(n_triangle, 1), ne = (size_t)n_edge;
   char *b = g_arena.base;
@@ -910,20 +1050,24 @@ int flip_run(const FlipWork &w, size_t o_scratch, int64_t n_triangle, int64_t n_
   static_assert(sizeof(FlipCounters) <= 16 * sizeof(unsigned long long), "pinned block too small");
   const FlipCounters *h = (const FlipCounters *)g_arena.pinned;
   int64_t flips = 0, iters = 0, exact = 0;
-  cudaMemsetAsync(state, 0, ne, s);
-  cudaMemsetAsync(lock, 0, sizeof(unsigned long long) * nt, s);
-  cudaMemsetAsync(mark, 0, sizeof(int32_t) * ne, s);
-  int64_t n = n_edge;
-  const int32_t *cand = nullptr;                                 // first iteration: every edge
+  if (!init) {
+    cudaMemsetAsync(state, 0, ne, s);
+    cudaMemsetAsync(lock, 0, sizeof(unsigned long long) * nt, s);
+    cudaMemsetAsync(mark, 0, sizeof(int32_t) * ne, s);
+  }
+  int64_t n = init ? init->n_upper : n_edge;
+  const int32_t *cand = init ? list[0] : nullptr;                // first iteration: every edge, unless the caller knows better
+  const unsigned long long *n_dev = init ? init->n_dev : nullptr;
+  const mrdgen::Touch touch = init ? init->touch : mrdgen::Touch{nullptr, nullptr, nullptr, nullptr, nullptr};
   for (int32_t iter = 1;; ++iter) {
     if (iter > 100000) return gen_fail(MRD_EINVAL, "delaunay_flip: no convergence (is the input a valid triangulation?)");
     const unsigned long long stamp = (unsigned long long)iter << 32;
     int32_t *next = list[iter & 1];
     const unsigned nb = (unsigned)((n + 255) / 256);
     cudaMemsetAsync(cnt, 0, sizeof(FlipCounters), s);
-    mrdgen::check_edge_kernel<<<nb, 256, 0, s>>>(n, cand, xy, tv_dev, te_dev, et_dev, state, lock, stamp, work, cnt);
+    if (n > 0) mrdgen::check_edge_kernel<<<nb, 256, 0, s>>>(n, cand, xy, tv_dev, te_dev, et_dev, state, lock, stamp, work, cnt, n_dev);
     mrdgen::check_edge_exact_kernel<<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(work, xy, tv_dev, te_dev, et_dev, state, lock, stamp, cnt, scratch);
-    mrdgen::flip_kernel<<<nb, 256, 0, s>>>(n, cand, tv_dev, te_dev, et_dev, state, lock, stamp, iter, mark, next, cnt);
+    if (n > 0) mrdgen::flip_kernel<<<nb, 256, 0, s>>>(n, cand, tv_dev, te_dev, et_dev, state, lock, stamp, iter, mark, next, cnt, n_dev, touch);
     cudaError_t e = cudaMemcpyAsync(g_arena.pinned, cnt, sizeof(FlipCounters), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e == cudaSuccess) e = cudaGetLastError();
@@ -934,6 +1078,7 @@ int flip_run(const FlipWork &w, size_t o_scratch, int64_t n_triangle, int64_t n_
     if (h->n_bad == 0) break;                                    // every edge is locally Delaunay
     cand = next;
     n = (int64_t)h->n_next;
+    n_dev = nullptr;
   }
   if (flips_out) *flips_out = flips;
   if (iters_out) *iters_out = iters;
@@ -1001,6 +1146,9 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   const size_t o_cand = c.add(sizeof(int32_t) * ct), o_kind = c.add(ct), o_pt = c.add(sizeof(double2) * ct);
   const size_t o_tins = c.add(sizeof(int32_t) * ct), o_eins = c.add(sizeof(int32_t) * ct), o_claim = c.add(sizeof(unsigned long long) * ct);
   const size_t o_sel = c.add(sizeof(int32_t) * ct), o_seg = c.add(sizeof(int32_t) * ct), o_rank = c.add(sizeof(int32_t) * ct), o_srank = c.add(sizeof(int32_t) * ct);
+  const size_t o_touch_t = c.add(ct), o_touch_e = c.add(ce), o_slot_t = c.add(sizeof(int32_t) * ct), o_slot_e = c.add(sizeof(int32_t) * ce);
+  const size_t o_tri_map = c.add(sizeof(int32_t) * ct), o_edge_map = c.add(sizeof(int32_t) * ce), o_tmp_te = c.add(sizeof(int32_t) * 3 * ct);
+  const size_t o_tmp_et = c.add(sizeof(int2) * ce), o_jpos = c.add(3 * ct), o_ninit = c.add(sizeof(unsigned long long));
   const size_t o_cwork = c.add(sizeof(int32_t) * ct), o_cwork2 = c.add(sizeof(int32_t) * ct), o_cwn = c.add(2 * sizeof(unsigned long long));
   const size_t cm = std::max(ct, (size_t)cap_vertex);               // the sort buffers serve triangles and vertices
   const size_t o_klo0 = c.add(sizeof(unsigned long long) * cm), o_klo1 = c.add(sizeof(unsigned long long) * cm);
@@ -1008,7 +1156,7 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   const size_t o_i0 = c.add(sizeof(int32_t) * cm), o_i1 = c.add(sizeof(int32_t) * cm), o_tv2 = c.add(sizeof(int32_t) * 3 * ct);
   const size_t o_xy2 = c.add(sizeof(double2) * (size_t)cap_vertex), o_num = c.add(sizeof(int32_t) * (size_t)cap_vertex);   // (cap_vertex <= cap_triangle is not required)
   size_t tmp_sel = 0, tmp_scan = 0, tmp_s64 = 0, tmp_s32 = 0;
-  cub::DeviceSelect::Flagged(nullptr, tmp_sel, thrust::counting_iterator<int32_t>(0), (const uint8_t *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, s);
+  cub::DeviceSelect::Flagged(nullptr, tmp_sel, thrust::counting_iterator<int32_t>(0), (const uint8_t *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ce, s);
   cub::DeviceScan::ExclusiveSum(nullptr, tmp_scan, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, s);
   cub::DeviceRadixSort::SortPairs(nullptr, tmp_s64, (unsigned long long *)nullptr, (unsigned long long *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)cm, 0, 64, s);
   cub::DeviceRadixSort::SortPairs(nullptr, tmp_s32, (unsigned *)nullptr, (unsigned *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, 0, 32, s);
@@ -1030,6 +1178,12 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   unsigned *khi0 = (unsigned *)(b + o_khi0), *khi1 = (unsigned *)(b + o_khi1);
   int32_t *i0 = (int32_t *)(b + o_i0), *i1 = (int32_t *)(b + o_i1), *tv2 = (int32_t *)(b + o_tv2), *number = (int32_t *)(b + o_num);
   double2 *xy2 = (double2 *)(b + o_xy2);
+  uint8_t *touch_t = (uint8_t *)(b + o_touch_t), *touch_e = (uint8_t *)(b + o_touch_e);
+  int32_t *slot_t = (int32_t *)(b + o_slot_t), *slot_e = (int32_t *)(b + o_slot_e), *tri_map = (int32_t *)(b + o_tri_map);
+  int32_t *edge_map = (int32_t *)(b + o_edge_map), *tmp_te = (int32_t *)(b + o_tmp_te);
+  int2 *tmp_et = (int2 *)(b + o_tmp_et);
+  int8_t *jpos = (int8_t *)(b + o_jpos);
+  unsigned long long *n_init = (unsigned long long *)(b + o_ninit);
   int32_t *cwork = (int32_t *)(b + o_cwork), *cwork2 = (int32_t *)(b + o_cwork2);
   unsigned long long *cwork_n = (unsigned long long *)(b + o_cwn);
   void *tmp = b + o_tmp;
@@ -1038,6 +1192,33 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
     cudaError_t e2 = cudaStreamSynchronize(s);
     if (e2 == cudaSuccess) e2 = cudaGetLastError();
     return e2 == cudaSuccess ? MRD_OK : cuda_fail(what, e2);
+  };
+  // 4.1.4 / M12 / M14: (vertices along the Morton curve of the box,) triangles in canonical order, edges rebuilt
+  auto resort = [&](int bits) -> int {
+    size_t tb;
+    const unsigned nbt = (unsigned)((nt + 255) / 256);
+    if (box) {
+      const unsigned nbv = (unsigned)((nv + 255) / 256);
+      mrdgen::morton_keys_kernel<<<nbv, 256, 0, s>>>(nv, xy, box[0], box[1], 2097152.0 / (box[2] - box[0]), 2097152.0 / (box[3] - box[1]), klo0, i0);
+      tb = tmp_s64;
+      cub::DeviceRadixSort::SortPairs(tmp, tb, klo0, klo1, i0, i1, nv, 0, 42, s);   // stable: ties keep their order
+      mrdgen::vertex_permute_kernel<<<nbv, 256, 0, s>>>(nv, i1, xy, xy2, number);
+      cudaMemcpyAsync(xy, xy2, sizeof(double2) * (size_t)nv, cudaMemcpyDeviceToDevice, s);
+      mrdgen::relabel_kernel<<<(unsigned)((3 * nt + 255) / 256), 256, 0, s>>>(3 * nt, number, tv_dev);
+    }
+    mrdgen::canonical_keys_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, bits, klo0, i0);
+    tb = tmp_s64;
+    cub::DeviceRadixSort::SortPairs(tmp, tb, klo0, klo1, i0, i1, nt, 0, 2 * bits, s);
+    mrdgen::gather_first_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, i1, khi0);
+    tb = tmp_s32;
+    cub::DeviceRadixSort::SortPairs(tmp, tb, khi0, khi1, i1, i0, nt, 0, bits, s);
+    mrdgen::gather_rows_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, i0, tv2);
+    cudaMemcpyAsync(tv_dev, tv2, sizeof(int32_t) * 3 * (size_t)nt, cudaMemcpyDeviceToDevice, s);
+    int64_t ne_built = 0;
+    const int r2 = build_edges_run(ew, nt, bits, tv_dev, te_dev, et_dev, &ne_built, s);
+    if (r2 != MRD_OK) return r2;
+    if (ne_built != ne) return gen_fail(MRD_EINVAL, "refine: edge count changed under renumbering (internal error)");
+    return MRD_OK;
   };
   int64_t done = 0, left = 0;
   int rc = MRD_OK;
@@ -1084,34 +1265,62 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
       break;
     }
     // 2.4.4: insert; 2.4.6: flips
-    mrdgen::insert_kernel<<<(unsigned)((nc + 127) / 128), 128, 0, s>>>(nc, kind, pt, tins, eins, sel, rank, srank, (int32_t)nv, (int32_t)nt, (int32_t)ne, xy, tv_dev, te_dev, et_dev);
+    const bool in_place = box == nullptr;                          // reading M15: no re-sort inside the loop
+    mrdgen::Touch touch{nullptr, nullptr, nullptr, nullptr, nullptr};
+    FlipInit init{nullptr, 0, touch};
+    if (in_place) {
+      cudaMemsetAsync(touch_t, 0, (size_t)nt2, s);
+      cudaMemsetAsync(touch_e, 0, (size_t)ne2, s);
+      cudaMemsetAsync(b + fw.o_state, 0, (size_t)ne2, s);
+      cudaMemsetAsync(b + fw.o_lock, 0, sizeof(unsigned long long) * (size_t)nt2, s);
+      cudaMemsetAsync(b + fw.o_mark, 0, sizeof(int32_t) * (size_t)ne2, s);
+      cudaMemsetAsync(n_init, 0, sizeof(unsigned long long), s);
+      touch = mrdgen::Touch{touch_t, touch_e, (int32_t *)(b + fw.o_mark), (int32_t *)(b + fw.o_l0), n_init};
+      init = FlipInit{n_init, 8 * nsel, touch};                    // at most 8 edges per inserted vertex
+    }
+    mrdgen::insert_kernel<<<(unsigned)((nc + 127) / 128), 128, 0, s>>>(nc, kind, pt, tins, eins, sel, rank, srank, (int32_t)nv, (int32_t)nt, (int32_t)ne, xy, tv_dev, te_dev, et_dev, touch);
     nv = nv2; nt = nt2; ne = ne2;
-    if ((rc = flip_run(fw, o_scr, nt, ne, xy, tv_dev, te_dev, et_dev, nullptr, nullptr, nullptr, s)) != MRD_OK) return rc;
-    // canonical order (M12) and the edge arrays that go with it
-    const unsigned nbt = (unsigned)((nt + 255) / 256);
+    if ((rc = flip_run(fw, o_scr, nt, ne, xy, tv_dev, te_dev, et_dev, nullptr, nullptr, nullptr, s, in_place ? &init : nullptr)) != MRD_OK) return rc;
     int bits = 1;
     while ((1ll << bits) < nv) ++bits;                               // width of a vertex number
-    if (box) {                                                       // 4.1.4: vertices along the Morton curve of the box (M14)
-      const unsigned nbv = (unsigned)((nv + 255) / 256);
-      mrdgen::morton_keys_kernel<<<nbv, 256, 0, s>>>(nv, xy, box[0], box[1], 2097152.0 / (box[2] - box[0]), 2097152.0 / (box[3] - box[1]), klo0, i0);
+    if (in_place) {
+      // created triangles and edges into the freed and the new slots, in ascending order (M15)
+      size_t tb = tmp_sel;
+      cub::DeviceSelect::Flagged(tmp, tb, thrust::counting_iterator<int32_t>(0), (const uint8_t *)touch_t, slot_t, d_nsel, nt, s);
+      tb = tmp_sel;
+      cub::DeviceSelect::Flagged(tmp, tb, thrust::counting_iterator<int32_t>(0), (const uint8_t *)touch_e, slot_e, d_nsel + 1, ne, s);
+      int32_t *h32b = (int32_t *)hp;
+      cudaMemcpyAsync(h32b, d_nsel, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+      if ((rc = sync("refine: touched slots")) != MRD_OK) return rc;
+      const int64_t ns = h32b[0], nse = h32b[1];
+      const unsigned nbs = (unsigned)((ns + 255) / 256), nbs3 = (unsigned)((3 * ns + 255) / 256), nbe = (unsigned)((nse + 255) / 256);
+      mrdgen::touched_keys_kernel<<<nbs, 256, 0, s>>>(ns, slot_t, tv_dev, te_dev, bits, klo0, i0);
       tb = tmp_s64;
-      cub::DeviceRadixSort::SortPairs(tmp, tb, klo0, klo1, i0, i1, nv, 0, 42, s);   // stable: ties keep their order
-      mrdgen::vertex_permute_kernel<<<nbv, 256, 0, s>>>(nv, i1, xy, xy2, number);
-      cudaMemcpyAsync(xy, xy2, sizeof(double2) * (size_t)nv, cudaMemcpyDeviceToDevice, s);
-      mrdgen::relabel_kernel<<<(unsigned)((3 * nt + 255) / 256), 256, 0, s>>>(3 * nt, number, tv_dev);
+      cub::DeviceRadixSort::SortPairs(tmp, tb, klo0, klo1, i0, i1, ns, 0, 2 * bits, s);
+      mrdgen::touched_first_kernel<<<nbs, 256, 0, s>>>(ns, slot_t, tv_dev, i1, khi0);
+      tb = tmp_s32;
+      cub::DeviceRadixSort::SortPairs(tmp, tb, khi0, khi1, i1, i0, ns, 0, bits, s);        // i0: order of the touched triangles
+      mrdgen::tri_map_kernel<<<nbs, 256, 0, s>>>(ns, slot_t, i0, tv_dev, te_dev, tri_map, tv2, tmp_te);
+      unsigned long long *ek0 = (unsigned long long *)(b + ew.o_k0), *ek1 = (unsigned long long *)(b + ew.o_k1);
+      int32_t *ev0 = (int32_t *)(b + ew.o_v0), *ev1 = (int32_t *)(b + ew.o_v1);             // (the edge builder's buffers are idle here)
+      mrdgen::touched_edge_keys_kernel<<<nbe, 256, 0, s>>>(nse, slot_e, tv_dev, te_dev, et_dev, bits, ek0, ev0);
+      tb = ew.tmp_sort;
+      cub::DeviceRadixSort::SortPairs(b + ew.o_tmp, tb, ek0, ek1, ev0, ev1, nse, 0, 2 * bits, s);   // ev1: order of the touched edges
+      mrdgen::edge_map_kernel<<<nbe, 256, 0, s>>>(nse, slot_e, ev1, et_dev, edge_map, tmp_et);
+      mrdgen::side_pos_kernel<<<nbs3, 256, 0, s>>>(ns, slot_t, i0, tmp_te, touch_e, et_dev, jpos);
+      mrdgen::renumber_scatter_kernel<<<std::max(nbs, nbe), 256, 0, s>>>(ns, nse, slot_t, slot_e, tv2, tmp_te, tmp_et, jpos, touch_e, tri_map, edge_map,
+                                                                        tv_dev, te_dev, et_dev);
+      mrdgen::renumber_order_kernel<<<nbs3, 256, 0, s>>>(ns, slot_t, te_dev, et_dev);
+    } else {
+      if ((rc = resort(bits)) != MRD_OK) return rc;                // 4.1.4: vertices along the Morton curve, canonical triangles (M12, M14)
     }
-    mrdgen::canonical_keys_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, bits, klo0, i0);
-    tb = tmp_s64;
-    cub::DeviceRadixSort::SortPairs(tmp, tb, klo0, klo1, i0, i1, nt, 0, 2 * bits, s);
-    mrdgen::gather_first_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, i1, khi0);
-    tb = tmp_s32;
-    cub::DeviceRadixSort::SortPairs(tmp, tb, khi0, khi1, i1, i0, nt, 0, bits, s);
-    mrdgen::gather_rows_kernel<<<nbt, 256, 0, s>>>(nt, tv_dev, i0, tv2);
-    cudaMemcpyAsync(tv_dev, tv2, sizeof(int32_t) * 3 * (size_t)nt, cudaMemcpyDeviceToDevice, s);
-    int64_t ne_built = 0;
-    if ((rc = build_edges_run(ew, nt, bits, tv_dev, te_dev, et_dev, &ne_built, s)) != MRD_OK) return rc;
-    if (ne_built != ne) return gen_fail(MRD_EINVAL, "refine: edge count changed under renumbering (internal error)");
     done++;
+  }
+  if (!box && done > 0) {                                          // one canonical re-sort after the last in-place iteration
+    int bits = 1;
+    while ((1ll << bits) < nv) ++bits;
+    const int rc2 = resort(bits);
+    if (rc2 != MRD_OK) return rc2;
   }
   *n_vertex = nv;
   *n_triangle = nt;

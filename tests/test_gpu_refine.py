@@ -1,6 +1,7 @@
 """GPU parity of the Delaunay refinement (section 2.3-2.4, 4.1.1) against oracle/meshgen.py: refine.
 Integer and index work with IEEE-exact coordinates: the refined mesh must be the oracle's ARRAY FOR ARRAY (vertex coordinates
-bit for bit, triangleVertices, triangleEdges, edgeTriangles) -- iteration by iteration and for the whole run -- because every
+bit for bit, triangleVertices, triangleEdges, edgeTriangles) -- iteration by iteration, after k in-place iterations and for the
+whole run -- because every
 decision is exact (ORIENT2D, INCIRCLE2D), prescribed (eq. 2 and eq. 4 one IEEE operation at a time) or an integer rule
 (priorities, numbering, canonical order).  At sizes beyond the oracle: the guarantees of section 2.3 and the library
 triangulation of the final vertex set."""
@@ -58,9 +59,18 @@ def test_every_iteration_and_the_whole_run_match_the_oracle(mrdb, B, R, seed, sh
             break
         state = o[:4]
     assert it >= 4 and kinds[mg.KIND_TRI] > 20 and kinds[mg.KIND_SEG] > 5     # both common kinds of insertion were exercised
-    g = mrdb.meshgen_refine(*to_dev(xy, tv, te, et), R, B, seed=seed)          # free-running
-    assert same(g[:4], state) and g[4] == dict(iterations=it, bad_left=0)
-    assert g[0].shape[0] > 3 * xy.shape[0]
+    # free-running: the iterations renumber in place (reading M15), one re-sort at the end -- after 2, 3, 5 iterations and for
+    # the whole run the oracle's arrays
+    for k in (2, 3, 5):
+        o = mg.refine(xy, tv, R, B, seed=seed, max_iterations=k)
+        g = mrdb.meshgen_refine(*to_dev(xy, tv, te, et), R, B, seed=seed, max_iterations=k)
+        assert same(g[:4], o[:4]) and g[4]["iterations"] == k and g[4]["bad_left"] > 0, k
+    o = mg.refine(xy, tv, R, B, seed=seed)
+    g = mrdb.meshgen_refine(*to_dev(xy, tv, te, et), R, B, seed=seed)
+    assert same(g[:4], o[:4]) and g[4] == dict(iterations=o[4], bad_left=0)
+    assert g[0].shape[0] > 3 * xy.shape[0] and o[4] >= 5
+    q = mg.test_quality(o[0], o[1], R, B)
+    assert q["bad"].sum() == 0
 
 
 @pytest.mark.parametrize("B,R,seed,shape", [(1.0, 0.07, 4, (6, 5)), (np.sqrt(2.0), 0.045, 5, (8, 6))])
