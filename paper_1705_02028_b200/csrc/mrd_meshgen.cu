@@ -163,8 +163,15 @@ struct Touch {
   unsigned long long *n;
   __device__ __forceinline__ void tri(int32_t t) const { if (T) T[t] = 1; }
   __device__ __forceinline__ void edge(int32_t e) const { if (E) E[e] = 1; }
-  __device__ __forceinline__ void check(int32_t e) const {
-    if (list && atomicExch(mark + e, -1) != -1) list[atomicAdd(n, 1ull)] = e;
+  // (one atomicAdd on the list's length per thread, not per edge: up to 3 M increments of one address serialise in L2)
+  struct Pending { int32_t e[8]; int n; };
+  __device__ __forceinline__ void check(int32_t e, Pending &p) const {
+    if (list && atomicExch(mark + e, -1) != -1) p.e[p.n++] = e;
+  }
+  __device__ __forceinline__ void flush(const Pending &p) const {
+    if (p.n == 0) return;
+    const unsigned long long base = atomicAdd(n, (unsigned long long)p.n);
+    for (int q = 0; q < p.n; ++q) list[base + q] = p.e[q];
   }
 };
 
@@ -542,25 +549,43 @@ cavity_kernel(int64_t nc, const int32_t *__restrict__ cand, int8_t *__restrict__
   int32_t list[CAVITY_MAX];
   const int8_t kd = kind[j];
   const int n = kd == KIND_NONE ? -1 : cavity_of<false>(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, list, nullptr, nullptr);
-  if (n == -2) { work[atomicAdd(n_work, 1ull)] = (int32_t)j; return; }
+  if (n == -2) {                                                  // undecided: pass 1 lists it, pass 2 finds it in that list
+    if (PASS == 1) work[atomicAdd(n_work, 1ull)] = (int32_t)j;
+    return;
+  }
   cavity_act<PASS>(j, n, list, kd, priority_of(seed, iteration, (unsigned)cand[j]), kind, claim, sel, seg);
 }
 // the listed candidates again, with the exact INCIRCLE2D where the filter fails.  Grid-stride with few threads: every thread
-// owns a slice of the expansion scratch.
+// owns a slice of the expansion scratch.  One exact evaluation is a serial chain of ~10^4 operations on expansions in global
+// memory (~100 us), so pass 1 keeps the cavities it found (the first CAVITY_STORE work items) and pass 2 reads them back
+// instead of finding them again: both passes walk the work list of pass 1.
+constexpr int CAVITY_STORE = 1 << 15;
 template <int PASS>
 __global__ void __launch_bounds__(32)
 cavity_exact_kernel(const unsigned long long *__restrict__ n_work, const int32_t *__restrict__ work, const int32_t *__restrict__ cand,
                     int8_t *__restrict__ kind, const double2 *__restrict__ pt, const int32_t *__restrict__ t_ins,
                     const int32_t *__restrict__ e_ins, const double2 *__restrict__ xy, const int32_t *__restrict__ tv,
                     const int32_t *__restrict__ te, const int32_t *__restrict__ et, unsigned long long *__restrict__ claim, unsigned seed,
-                    unsigned iteration, int32_t *__restrict__ sel, int32_t *__restrict__ seg, double *__restrict__ scratch) {
+                    unsigned iteration, int32_t *__restrict__ sel, int32_t *__restrict__ seg, double *__restrict__ scratch,
+                    int32_t *__restrict__ store) {
   const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, nw = (int64_t)*n_work;
   double *acc = scratch + tid * (2 * MAXE), *tmp = acc + MAXE;
   int32_t list[CAVITY_MAX];
   for (int64_t w = tid; w < nw; w += (int64_t)gridDim.x * blockDim.x) {
     const int64_t j = work[w];
     const int8_t kd = kind[j];
-    const int n = cavity_of<true>(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, list, acc, tmp);
+    int32_t *st = store + w * (CAVITY_MAX + 1);
+    int n;
+    if (PASS == 2 && w < CAVITY_STORE) {
+      n = st[0];
+      for (int q = 0; q < n; ++q) list[q] = st[1 + q];
+    } else {
+      n = kd == KIND_NONE ? -1 : cavity_of<true>(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, list, acc, tmp);
+      if (PASS == 1 && w < CAVITY_STORE) {
+        st[0] = n;
+        for (int q = 0; q < n; ++q) st[1 + q] = list[q];
+      }
+    }
     cavity_act<PASS>(j, n, list, kd, priority_of(seed, iteration, (unsigned)cand[j]), kind, claim, sel, seg);
   }
 }
@@ -580,6 +605,8 @@ insert_kernel(int64_t nc, const int8_t *__restrict__ kind, const double2 *__rest
   const int32_t v = nv + rank[j];
   const int32_t tn = nt + 2 * rank[j] - segrank[j], en = ne + 3 * rank[j] - segrank[j];   // SEG adds 1 / 2, the others 2 / 3
   xy[v] = pt[j];
+  Touch::Pending pend;
+  pend.n = 0;
   const int32_t t = t_ins[j], e = e_ins[j];
   int32_t *V = tv + 3 * (int64_t)t, *E = te + 3 * (int64_t)t;
   if (kind[j] == KIND_TRI) {
@@ -595,7 +622,8 @@ insert_kernel(int64_t nc, const int8_t *__restrict__ kind, const double2 *__rest
     swap_side(et, e1, t, t2);
     touch.tri(t); touch.tri(t1); touch.tri(t2);
     touch.edge(f0); touch.edge(f1); touch.edge(f2);
-    touch.check(e0); touch.check(e1); touch.check(e2); touch.check(f0); touch.check(f1); touch.check(f2);
+    touch.check(e0, pend); touch.check(e1, pend); touch.check(e2, pend); touch.check(f0, pend); touch.check(f1, pend); touch.check(f2, pend);
+    touch.flush(pend);
     return;
   }
   const int i1 = local_of(E, e);
@@ -610,7 +638,8 @@ insert_kernel(int64_t nc, const int8_t *__restrict__ kind, const double2 *__rest
     swap_side(et, e_ca, t, n1);
     touch.tri(t); touch.tri(n1);
     touch.edge(e); touch.edge(g0); touch.edge(g1);               // E = (b, c) is (b, v) now
-    touch.check(e); touch.check(g0); touch.check(g1); touch.check(e_ca); touch.check(e_ab);
+    touch.check(e, pend); touch.check(g0, pend); touch.check(g1, pend); touch.check(e_ca, pend); touch.check(e_ab, pend);
+    touch.flush(pend);
     return;
   }
   const int32_t t2 = across(et, e, t);
@@ -629,8 +658,9 @@ insert_kernel(int64_t nc, const int8_t *__restrict__ kind, const double2 *__rest
   swap_side(et, e_dc, t2, n2);
   touch.tri(t); touch.tri(n1); touch.tri(t2); touch.tri(n2);
   touch.edge(e); touch.edge(g0); touch.edge(g1); touch.edge(g2);
-  touch.check(e); touch.check(g0); touch.check(g1); touch.check(g2);
-  touch.check(e_ca); touch.check(e_ab); touch.check(e_bd); touch.check(e_dc);
+  touch.check(e, pend); touch.check(g0, pend); touch.check(g1, pend); touch.check(g2, pend);
+  touch.check(e_ca, pend); touch.check(e_ab, pend); touch.check(e_bd, pend); touch.check(e_dc, pend);
+  touch.flush(pend);
 }
 // Morton value of every vertex (section 4.1.4; reading M14): 21 bits per coordinate, x in the even places
 static __device__ __forceinline__ unsigned long long spread21(unsigned v) {
@@ -1149,6 +1179,7 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   const size_t o_touch_t = c.add(ct), o_touch_e = c.add(ce), o_slot_t = c.add(sizeof(int32_t) * ct), o_slot_e = c.add(sizeof(int32_t) * ce);
   const size_t o_tri_map = c.add(sizeof(int32_t) * ct), o_edge_map = c.add(sizeof(int32_t) * ce), o_tmp_te = c.add(sizeof(int32_t) * 3 * ct);
   const size_t o_tmp_et = c.add(sizeof(int2) * ce), o_jpos = c.add(3 * ct), o_ninit = c.add(sizeof(unsigned long long));
+  const size_t o_cav_store = c.add(sizeof(int32_t) * (size_t)mrdgen::CAVITY_STORE * (mrdgen::CAVITY_MAX + 1));
   const size_t o_cwork = c.add(sizeof(int32_t) * ct), o_cwork2 = c.add(sizeof(int32_t) * ct), o_cwn = c.add(2 * sizeof(unsigned long long));
   const size_t cm = std::max(ct, (size_t)cap_vertex);               // the sort buffers serve triangles and vertices
   const size_t o_klo0 = c.add(sizeof(unsigned long long) * cm), o_klo1 = c.add(sizeof(unsigned long long) * cm);
@@ -1184,6 +1215,7 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   int2 *tmp_et = (int2 *)(b + o_tmp_et);
   int8_t *jpos = (int8_t *)(b + o_jpos);
   unsigned long long *n_init = (unsigned long long *)(b + o_ninit);
+  int32_t *cav_store = (int32_t *)(b + o_cav_store);
   int32_t *cwork = (int32_t *)(b + o_cwork), *cwork2 = (int32_t *)(b + o_cwork2);
   unsigned long long *cwork_n = (unsigned long long *)(b + o_cwn);
   void *tmp = b + o_tmp;
@@ -1242,9 +1274,9 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
     const unsigned nbc = (unsigned)((nc + 127) / 128);
     cudaMemsetAsync(cwork_n, 0, 2 * sizeof(unsigned long long), s);
     mrdgen::cavity_kernel<1><<<nbc, 128, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, cwork, cwork_n);
-    mrdgen::cavity_exact_kernel<1><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cwork_n, cwork, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch);
+    mrdgen::cavity_exact_kernel<1><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cwork_n, cwork, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch, cav_store);
     mrdgen::cavity_kernel<2><<<nbc, 128, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, cwork2, cwork_n + 1);
-    mrdgen::cavity_exact_kernel<2><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cwork_n + 1, cwork2, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch);
+    mrdgen::cavity_exact_kernel<2><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cwork_n, cwork, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch, cav_store);
     tb = tmp_scan;
     cub::DeviceScan::ExclusiveSum(tmp, tb, sel, rank, nc, s);
     tb = tmp_scan;
