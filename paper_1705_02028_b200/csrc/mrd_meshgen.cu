@@ -203,19 +203,25 @@ check_edge_kernel(int64_t n, const int32_t *__restrict__ cand, const double2 *__
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   bool bad = false;
   if (n_dev) n = min(n, (int64_t)*n_dev);                          // (the host knows only an upper bound of the list's length)
+  bool exact = false;
   if (i < n) {
     const int32_t e = cand ? cand[i] : (int32_t)i;
     Quad q;
     if (!load_quad(e, xy, tv, te, et, q)) state[e] = 0;
     else {
-      const int sg = incircle2d_filter(q.a, q.b, q.c, q.d);
+      int sg = incircle2d_filter(q.a, q.b, q.c, q.d);
+      if (sg == 2) {                                               // exact, in place when the translations are exact
+        sg = incircle2d_exact_short(q.a, q.b, q.c, q.d);
+        exact = sg != 2;
+      }
       if (sg == 2) work[atomicAdd(&c->n_work, 1ull)] = e;          // rare
       else if (sg == 1) { bid(e, q, stamp, state, lock); bad = true; }
       else state[e] = 0;
     }
   }
-  const unsigned m = __ballot_sync(0xFFFFFFFFu, bad);
+  const unsigned m = __ballot_sync(0xFFFFFFFFu, bad), mx = __ballot_sync(0xFFFFFFFFu, exact);
   if ((threadIdx.x & 31) == 0 && m) atomicAdd(&c->n_bad, (unsigned long long)__popc(m));
+  if ((threadIdx.x & 31) == 0 && mx) atomicAdd(&c->n_exact, (unsigned long long)__popc(mx));
 }
 __global__ void __launch_bounds__(32)
 check_edge_exact_kernel(const int32_t *__restrict__ work, const double2 *__restrict__ xy, const int32_t *__restrict__ tv,
@@ -510,6 +516,7 @@ static __device__ int cavity_of(double2 p, int8_t kd, int32_t ti, int32_t ei, co
       const int32_t *v = tv + 3 * (int64_t)nb;
       const double2 A = xy[v[0]], B = xy[v[1]], C = xy[v[2]];
       int sg = incircle2d_filter(A, B, C, p);
+      if (sg == 2) sg = incircle2d_exact_short(A, B, C, p);       // exact translations (neighbouring points): short expansions
       if (sg == 2) {
         if (!EXACT) return -2;
         sg = incircle2d_exact(A, B, C, p, acc, tmp);

@@ -125,6 +125,43 @@ static __device__ int incircle2d_exact(double2 a, double2 b, double2 c, double2 
   return sign_of(acc, na);
 }
 
+// The same determinant when the six translations a - d, b - d, c - d are EXACT (no rounding: the usual case for neighbouring
+// points, whose coordinates are within a factor 2 of each other): every factor is then a single double and the expansions stay
+// short -- lift <= 4 components, minor <= 4, their product <= 32, the sum of the three <= 96 -- so they fit thread-local arrays
+// and any thread can do it.  Returns the exact sign, or 2 when a translation is inexact (the caller falls back to
+// incircle2d_exact with its 1152-component scratch).
+static __device__ int incircle2d_exact_short(double2 a, double2 b, double2 c, double2 d) {
+  const double px[3] = {a.x, b.x, c.x}, py[3] = {a.y, b.y, c.y};
+  double X[3], Y[3];
+  for (int k = 0; k < 3; ++k) {
+    double lo;
+    two_diff(px[k], d.x, X[k], lo);
+    if (lo != 0.0) return 2;
+    two_diff(py[k], d.y, Y[k], lo);
+    if (lo != 0.0) return 2;
+  }
+  double acc[100], tmp[36];
+  acc[0] = 0.0;
+  int na = 1;
+  for (int k = 0; k < 3; ++k) {
+    const int i = (k + 1) % 3, j = (k + 2) % 3;
+    double lift[8], minor[8];
+    lift[0] = 0.0;
+    int nl = 1;
+    nl = add_product(lift, nl, &X[k], 1, &X[k], 1, 1.0);
+    nl = add_product(lift, nl, &Y[k], 1, &Y[k], 1, 1.0);
+    minor[0] = 0.0;
+    int nm = 1;
+    nm = add_product(minor, nm, &X[i], 1, &Y[j], 1, 1.0);
+    nm = add_product(minor, nm, &Y[i], 1, &X[j], 1, -1.0);
+    tmp[0] = 0.0;
+    int nt = 1;
+    nt = add_product(tmp, nt, lift, nl, minor, nm, 1.0);
+    na = expansion_add(acc, na, tmp, nt);
+  }
+  return sign_of(acc, na);
+}
+
 constexpr double EPS = 1.1102230246251565e-16;   // 2^-53
 
 // Filters: the determinant in plain fp64 and a bound on its rounding error.  Return +1 / -1 when the sign is certain, 2 when the
