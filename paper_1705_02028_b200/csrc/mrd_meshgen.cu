@@ -17,6 +17,7 @@
 
 #include <algorithm>
 #include <cstdint>
+#include <cub/device/device_merge_sort.cuh>
 #include <cub/device/device_radix_sort.cuh>
 #include <cub/device/device_scan.cuh>
 #include <cub/device/device_select.cuh>
@@ -721,6 +722,30 @@ touched_keys_kernel(int64_t ns, const int32_t *__restrict__ S, int32_t *__restri
   key_lo[i] = ((unsigned long long)(unsigned)y << bits) | (unsigned)z;
   idx[i] = (int32_t)i;
 }
+// small touched sets: the whole triple as ONE key for a merge sort (a handful of launches instead of two radix sorts)
+struct TriKey { int32_t a, b, c; };
+struct TriKeyLess {
+  __device__ __forceinline__ bool operator()(const TriKey &x, const TriKey &y) const {
+    return x.a != y.a ? x.a < y.a : (x.b != y.b ? x.b < y.b : x.c < y.c);
+  }
+};
+struct U64Less {
+  __device__ __forceinline__ bool operator()(unsigned long long x, unsigned long long y) const { return x < y; }
+};
+__global__ void __launch_bounds__(256)
+touched_triples_kernel(int64_t ns, const int32_t *__restrict__ S, int32_t *__restrict__ tv, int32_t *__restrict__ te,
+                       TriKey *__restrict__ key, int32_t *__restrict__ idx) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= ns) return;
+  int32_t *v = tv + 3 * (int64_t)S[i], *ed = te + 3 * (int64_t)S[i];
+  const int32_t a = v[0], b = v[1], c = v[2], ea = ed[0], eb = ed[1], ec = ed[2];
+  const int r = (a < b && a < c) ? 0 : ((b < a && b < c) ? 1 : 2);
+  const int32_t x = r == 0 ? a : (r == 1 ? b : c), y = r == 0 ? b : (r == 1 ? c : a), z = r == 0 ? c : (r == 1 ? a : b);
+  put3(v, x, y, z);
+  put3(ed, r == 0 ? ea : (r == 1 ? eb : ec), r == 0 ? eb : (r == 1 ? ec : ea), r == 0 ? ec : (r == 1 ? ea : eb));
+  key[i] = TriKey{x, y, z};
+  idx[i] = (int32_t)i;
+}
 __global__ void __launch_bounds__(256)
 touched_first_kernel(int64_t ns, const int32_t *__restrict__ S, const int32_t *__restrict__ tv, const int32_t *__restrict__ idx,
                      unsigned *__restrict__ key_hi) {
@@ -1198,7 +1223,12 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   cub::DeviceScan::ExclusiveSum(nullptr, tmp_scan, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, s);
   cub::DeviceRadixSort::SortPairs(nullptr, tmp_s64, (unsigned long long *)nullptr, (unsigned long long *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)cm, 0, 64, s);
   cub::DeviceRadixSort::SortPairs(nullptr, tmp_s32, (unsigned *)nullptr, (unsigned *)nullptr, (int32_t *)nullptr, (int32_t *)nullptr, (int64_t)ct, 0, 32, s);
-  const size_t o_tmp = c.add(std::max(std::max(tmp_sel, tmp_scan), std::max(tmp_s64, tmp_s32)));
+  constexpr int64_t MERGE_MAX = 1 << 16;                              // touched sets up to this size go through a merge sort
+  size_t tmp_m3 = 0, tmp_m1 = 0;
+  cub::DeviceMergeSort::SortPairs(nullptr, tmp_m3, (mrdgen::TriKey *)nullptr, (int32_t *)nullptr, MERGE_MAX, mrdgen::TriKeyLess(), s);
+  cub::DeviceMergeSort::SortPairs(nullptr, tmp_m1, (unsigned long long *)nullptr, (int32_t *)nullptr, MERGE_MAX, mrdgen::U64Less(), s);
+  const size_t tmp_all = std::max(std::max(std::max(tmp_sel, tmp_scan), std::max(tmp_s64, tmp_s32)), std::max(tmp_m3, tmp_m1));
+  const size_t o_tmp = c.add(tmp_all);
   std::lock_guard<std::mutex> g(g_arena.mu);
   cudaError_t e = g_arena.reserve(c.total);
   if (e != cudaSuccess) return cuda_fail("refine", e);
@@ -1333,19 +1363,33 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
       if ((rc = sync("refine: touched slots")) != MRD_OK) return rc;
       const int64_t ns = h32b[0], nse = h32b[1];
       const unsigned nbs = (unsigned)((ns + 255) / 256), nbs3 = (unsigned)((3 * ns + 255) / 256), nbe = (unsigned)((nse + 255) / 256);
-      mrdgen::touched_keys_kernel<<<nbs, 256, 0, s>>>(ns, slot_t, tv_dev, te_dev, bits, klo0, i0);
-      tb = tmp_s64;
-      cub::DeviceRadixSort::SortPairs(tmp, tb, klo0, klo1, i0, i1, ns, 0, 2 * bits, s);
-      mrdgen::touched_first_kernel<<<nbs, 256, 0, s>>>(ns, slot_t, tv_dev, i1, khi0);
-      tb = tmp_s32;
-      cub::DeviceRadixSort::SortPairs(tmp, tb, khi0, khi1, i1, i0, ns, 0, bits, s);        // i0: order of the touched triangles
+      if (ns <= MERGE_MAX) {
+        mrdgen::TriKey *tk = (mrdgen::TriKey *)klo0;               // (12 bytes per key: klo0 and klo1 are adjacent and 16 bytes per item together)
+        mrdgen::touched_triples_kernel<<<nbs, 256, 0, s>>>(ns, slot_t, tv_dev, te_dev, tk, i0);
+        tb = tmp_all;
+        cub::DeviceMergeSort::SortPairs(tmp, tb, tk, i0, ns, mrdgen::TriKeyLess(), s);     // i0: order of the touched triangles
+      } else {
+        mrdgen::touched_keys_kernel<<<nbs, 256, 0, s>>>(ns, slot_t, tv_dev, te_dev, bits, klo0, i0);
+        tb = tmp_s64;
+        cub::DeviceRadixSort::SortPairs(tmp, tb, klo0, klo1, i0, i1, ns, 0, 2 * bits, s);
+        mrdgen::touched_first_kernel<<<nbs, 256, 0, s>>>(ns, slot_t, tv_dev, i1, khi0);
+        tb = tmp_s32;
+        cub::DeviceRadixSort::SortPairs(tmp, tb, khi0, khi1, i1, i0, ns, 0, bits, s);      // i0: order of the touched triangles
+      }
       mrdgen::tri_map_kernel<<<nbs, 256, 0, s>>>(ns, slot_t, i0, tv_dev, te_dev, tri_map, tv2, tmp_te);
       unsigned long long *ek0 = (unsigned long long *)(b + ew.o_k0), *ek1 = (unsigned long long *)(b + ew.o_k1);
       int32_t *ev0 = (int32_t *)(b + ew.o_v0), *ev1 = (int32_t *)(b + ew.o_v1);             // (the edge builder's buffers are idle here)
       mrdgen::touched_edge_keys_kernel<<<nbe, 256, 0, s>>>(nse, slot_e, tv_dev, te_dev, et_dev, bits, ek0, ev0);
-      tb = ew.tmp_sort;
-      cub::DeviceRadixSort::SortPairs(b + ew.o_tmp, tb, ek0, ek1, ev0, ev1, nse, 0, 2 * bits, s);   // ev1: order of the touched edges
-      mrdgen::edge_map_kernel<<<nbe, 256, 0, s>>>(nse, slot_e, ev1, et_dev, edge_map, tmp_et);
+      const int32_t *eorder = ev1;                                 // order of the touched edges
+      if (nse <= MERGE_MAX) {
+        tb = tmp_all;
+        cub::DeviceMergeSort::SortPairs(tmp, tb, ek0, ev0, nse, mrdgen::U64Less(), s);
+        eorder = ev0;
+      } else {
+        tb = ew.tmp_sort;
+        cub::DeviceRadixSort::SortPairs(b + ew.o_tmp, tb, ek0, ek1, ev0, ev1, nse, 0, 2 * bits, s);
+      }
+      mrdgen::edge_map_kernel<<<nbe, 256, 0, s>>>(nse, slot_e, eorder, et_dev, edge_map, tmp_et);
       mrdgen::side_pos_kernel<<<nbs3, 256, 0, s>>>(ns, slot_t, i0, tmp_te, touch_e, et_dev, jpos);
       mrdgen::renumber_scatter_kernel<<<std::max(nbs, nbe), 256, 0, s>>>(ns, nse, slot_t, slot_e, tv2, tmp_te, tmp_et, jpos, touch_e, tri_map, edge_map,
                                                                         tv_dev, te_dev, et_dev);
