@@ -160,6 +160,35 @@ def build_workload(n: int, numbering: str, kind: str = "uniform"):
         cfg.vertex_flag = cfg.mesh.boundary
         cfg.W0 = wl.vortex_state(cfg.mesh)
         return cfg
+    if kind == "refined":
+        # the paper's own pipeline (section 4): the mesh is GENERATED on the GPU by the library's Delaunay refinement (about n^2
+        # vertices in [0, 10]^2, B = sqrt 2, vertices along the Morton curve), its boundary vertices frozen, then solved on
+        import torch
+        from paper_1705_02028_b200 import binding as b
+        from workloads.meshes import UniformMesh
+        cfg = wl.make_config("sweep", n=32, numbering="natural")
+        c = wl.scrambled_triangulation(40, 40, seed=2, Lx=10.0, Ly=10.0)
+        xy = torch.tensor(c.xy, dtype=torch.float64, device="cuda")
+        tv = torch.tensor(c.tri, dtype=torch.int32, device="cuda")
+        te, et = b.meshgen_build_edges(tv)
+        b.meshgen_delaunay_flip(xy, tv, te, et)
+        t0 = time.perf_counter()
+        xy, tv, te, et, info = b.meshgen_refine(xy, tv, te, et, float(np.sqrt(0.69 * 100.0 / (n * n))), float(np.sqrt(2.0)), seed=1,
+                                                cap_vertex=int(1.6 * n * n) + 4096, box=(0.0, 0.0, 10.0, 10.0))
+        torch.cuda.synchronize()
+        gen_s = time.perf_counter() - t0
+        assert info["bad_left"] == 0
+        X, T, TE, ET = xy.cpu().numpy(), tv.cpu().numpy(), te.cpu().numpy(), et.cpu().numpy()
+        seg = np.nonzero(ET[:, 1] < 0)[0]
+        k = (TE[ET[seg, 0]] == seg[:, None]).argmax(axis=1)
+        flag = np.zeros(X.shape[0], dtype=np.uint8)
+        flag[T[ET[seg, 0], (k + 1) % 3]] = 1
+        flag[T[ET[seg, 0], (k + 2) % 3]] = 1
+        cfg.mesh = UniformMesh(X, T, (0.0, 0.0), None, None, None, (10.0, 10.0))
+        cfg.vertex_flag = flag
+        cfg.W0 = wl.vortex_state(cfg.mesh)
+        cfg.generated = dict(seconds=gen_s, iterations=info["iterations"], n_vertices=int(X.shape[0]))
+        return cfg
     cfg = wl.make_config("sweep", n=n, numbering=numbering)
     if kind in ("jitter", "flip"):
         cfg.mesh = wl.jitter_mesh(cfg.mesh, 0.2, seed=7)
@@ -176,6 +205,10 @@ def workload_text(args, nt: int) -> str:
     if args.mesh == "delaunay":
         return (f"isentropic vortex on a seeded graded Delaunay triangulation ({args.n}^2 points, cell size 100:1, frozen boundary ring; the "
                 f"shape of the paper's unstructured mesh, PAPER.md L685), Morton-ordered by the layout stage, {tail}")
+    if args.mesh == "refined":
+        return (f"isentropic vortex on a mesh GENERATED on the GPU by the library's Delaunay refinement (section 2.4 / 4.1 of the paper: about "
+                f"{args.n}^2 vertices in [0, 10]^2, B = sqrt 2, Morton-ordered, frozen boundary; the paper's test mesh has 1.3 M vertices, "
+                f"L685), {tail}")
     head = f"BASELINE.json config 5: isentropic vortex, periodic uniform triangulation {args.n}^2 vertices"
     if args.mesh == "jitter":
         head += ", every vertex moved by up to 0.2 cell widths (seed 7: no two triangles alike)"
@@ -448,7 +481,8 @@ def run_mrd(args):
                        "parallelism": parallelism,
                        "layout_s": layout_s, "device_gb": gm.device_bytes() / 1e9, "t_sim": t_sim,
                        "host_rss_gb": __import__("resource").getrusage(__import__("resource").RUSAGE_SELF).ru_maxrss / 1e6,
-                       "part_setup_s": None if setup is None else setup["setup_s"]},
+                       "part_setup_s": None if setup is None else setup["setup_s"],
+                       "mesh_generation": getattr(cfg, "generated", None) if not halo else None},
             "vertex_updates_per_s": nv_job * args.steps / (ms_total * 1e-3),
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
@@ -471,9 +505,10 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--traffic", type=float, default=None, help="dram bytes per launch of the dominant kernel (ncu)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--mesh", default="uniform", choices=["uniform", "jitter", "flip", "delaunay"],
+    ap.add_argument("--mesh", default="uniform", choices=["uniform", "jitter", "flip", "delaunay", "refined"],
                     help="uniform triangulation (config 5), jittered vertices, jittered + flipped edges (variable valence), or a seeded "
-                         "graded Delaunay triangulation of --size^2 points with a frozen boundary ring (--size 1140: the paper's 1.3 M vertices)")
+                         "graded Delaunay triangulation of --size^2 points with a frozen boundary ring (--size 1140: the paper's 1.3 M vertices), or "
+                         "(refined) a mesh of about --size^2 vertices generated on the GPU by mrd_meshgen_refine")
     ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
                     help="N > 1: torch.distributed backend (gloo stages the halo rows through host memory; functional tests only)")
     ap.add_argument("--decomposition", default="halo", choices=["halo", "replicas"],

@@ -141,3 +141,16 @@ def test_bench_line_carries_every_key_of_the_contract():
         assert key in d["clocks"], key
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["unit"] == d["unit"] and c["sample"]
+
+
+def test_bench_on_a_mesh_generated_by_the_library():
+    """python bench.py --mesh refined: the paper's pipeline (generate the mesh on the GPU, then solve on it) at a small size."""
+    import json
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--mesh", "refined", "--size", "160", "--steps", "4", "--warmup", "3",
+                        "--no-cpu-baseline"], capture_output=True, text=True, timeout=900, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-3000:]
+    d = json.loads([l for l in r.stdout.splitlines() if l.startswith("{")][-1])
+    gen = d["config"]["mesh_generation"]
+    assert gen["iterations"] >= 5 and 0.7 * 160 * 160 < gen["n_vertices"] == d["config"]["n_vertices"] < 1.4 * 160 * 160
+    assert 1.9 < d["config"]["n_triangles"] / d["config"]["n_vertices"] < 2.0 and d["value"] > 0
+    assert "GENERATED on the GPU" in d["config"]["workload"] and d["roofline"]["traffic"] is None
