@@ -111,6 +111,11 @@ def test_edge_insertions_on_a_uniform_mesh(mrdb):
         seen += np.bincount(o[4]["kinds"], minlength=4)
         state = o[:4]
     assert seen[mg.KIND_EDGE] > 5
+    # ... and free-running (in-place renumbering between the iterations) on the same degenerate mesh
+    for k in (2, 4):
+        o = mg.refine(m.xy, m.tri, 0.12, 0.6, seed=5, max_iterations=k)
+        g = mrdb.meshgen_refine(*to_dev(m.xy, tv, te, et), 0.12, 0.6, seed=5, max_iterations=k)
+        assert same(g[:4], o[:4]) and g[4]["iterations"] == k, k
 
 
 def test_refinement_at_size_keeps_the_guarantees_of_section_2_3(mrdb):
