@@ -447,13 +447,42 @@ slot_dt_kernel(MeshDev<R> m, TileDev<R> td, Ctl *__restrict__ ctl, const R *__re
   MRD_CTL_GUARD(ctl)
   // grid-stride: a few blocks per SM, so that only ~10^3 atomicMin hit the one address (65 536 one-per-block atomics
   // serialise in L2 and took longer than the gather itself)
+  // Four vertices per thread and pass, their loads issued together (the gather is a chain vslot_off -> vslot_ent -> partS of
+  // dependent loads; every resident thread slot is taken already, so more loads in flight have to come from each thread).
+  // The sum of a vertex still runs over its slots in ascending order.
   double d = __longlong_as_double(0x7FF0000000000000ll);
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m.nv; i += (int64_t)gridDim.x * blockDim.x) {
-    if (m.frozen && m.frozen[i] == 2) continue;  // halo vertex of a partition: its fan is incomplete here
-    R S = 0;
-    const int32_t q0 = __ldg(td.vslot_off + i), q1 = __ldg(td.vslot_off + i + 1);
-    for (int32_t q = q0; q < q1; ++q) S += __ldg(partS + __ldg(td.vslot_ent + q));
-    d = fmin(d, 2.0 * (double)__ldg(m.vol + i) / (double)S);
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  constexpr int U = 4;
+  for (int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i0 < m.nv; i0 += U * stride) {
+    int32_t q0[U], q1[U], ent[U][4];
+    R ps[U][4], vol[U];
+    bool on[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int64_t i = i0 + u * stride;
+      on[u] = i < m.nv && !(m.frozen && m.frozen[i] == 2);   // (2: halo vertex of a partition, its fan is incomplete here)
+      q0[u] = on[u] ? __ldg(td.vslot_off + i) : 0;
+      q1[u] = on[u] ? __ldg(td.vslot_off + i + 1) : 0;
+      vol[u] = on[u] ? __ldg(m.vol + i) : R(1);
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+#pragma unroll
+      for (int k = 0; k < 4; ++k) ent[u][k] = q0[u] + k < q1[u] ? __ldg(td.vslot_ent + q0[u] + k) : -1;
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+#pragma unroll
+      for (int k = 0; k < 4; ++k) ps[u][k] = ent[u][k] >= 0 ? __ldg(partS + ent[u][k]) : R(0);
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (!on[u]) continue;
+      R S = 0;
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (q0[u] + k < q1[u]) S += ps[u][k];
+      for (int32_t q = q0[u] + 4; q < q1[u]; ++q) S += __ldg(partS + __ldg(td.vslot_ent + q));
+      d = fmin(d, 2.0 * (double)vol[u] / (double)S);
+    }
   }
   block_min_to_global(d, &ctl->dmin_bits);
 }
