@@ -302,6 +302,20 @@ flip_kernel(int64_t n, const int32_t *__restrict__ cand, int32_t *__restrict__ t
   if (lane == 0 && fm) atomicAdd(&c->n_flip, (unsigned long long)__popc(fm));
 }
 
+// input check of the triangulator and the refinement: every triangle counter-clockwise (exact ORIENT2D > 0), vertex numbers in range
+__global__ void __launch_bounds__(256)
+validate_kernel(int64_t nt, int64_t nv, const double2 *__restrict__ xy, const int32_t *__restrict__ tv, unsigned long long *__restrict__ n_bad) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool bad = false;
+  if (t < nt) {
+    const int32_t a = tv[3 * t], b = tv[3 * t + 1], c = tv[3 * t + 2];
+    bad = a < 0 || b < 0 || c < 0 || a >= nv || b >= nv || c >= nv || a == b || b == c || a == c;
+    if (!bad) bad = orient2d_sign(xy[a], xy[b], xy[c]) <= 0;
+  }
+  const unsigned m = __ballot_sync(0xFFFFFFFFu, bad);
+  if ((threadIdx.x & 31) == 0 && m) atomicAdd(n_bad, (unsigned long long)__popc(m));
+}
+
 // ------------------------------------------------------------------------------------------------------------------
 // Point location (section 2.4.2)
 // ------------------------------------------------------------------------------------------------------------------
@@ -1180,6 +1194,17 @@ int mrd_meshgen_delaunay_flip(int64_t n_triangle, int64_t n_edge, const double *
   std::lock_guard<std::mutex> g(g_arena.mu);
   cudaError_t e = g_arena.reserve(c.total);
   if (e != cudaSuccess) return cuda_fail("delaunay_flip", e);
+  // a triangulation with a clockwise triangle is not valid, and flips on it need not terminate: refuse it
+  unsigned long long *bad = (unsigned long long *)(g_arena.base + w.o_cnt);
+  cudaMemsetAsync(bad, 0, sizeof *bad, s);
+  if (n_triangle > 0)
+    mrdgen::validate_kernel<<<(unsigned)((n_triangle + 255) / 256), 256, 0, s>>>(n_triangle, 0x7FFFFFFF, (const double2 *)xy_dev, tv_dev, bad);
+  e = cudaMemcpyAsync(g_arena.pinned, bad, sizeof *bad, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("delaunay_flip", e);
+  if (g_arena.pinned[0] != 0)
+    return gen_fail(MRD_EINVAL, "delaunay_flip: " + std::to_string(g_arena.pinned[0]) + " triangles of the input are clockwise or degenerate");
   return flip_run(w, w.o_scr, n_triangle, n_edge, (const double2 *)xy_dev, tv_dev, te_dev, et_dev, n_flips, n_iterations, n_exact, s);
 }
 
@@ -1291,6 +1316,12 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   };
   int64_t done = 0, left = 0;
   int rc = MRD_OK;
+  cudaMemsetAsync(cnt, 0, sizeof *cnt, s);
+  mrdgen::validate_kernel<<<(unsigned)((nt + 255) / 256), 256, 0, s>>>(nt, nv, xy, tv_dev, cnt);
+  cudaMemcpyAsync((void *)hp, cnt, sizeof *cnt, cudaMemcpyDeviceToHost, s);
+  if ((rc = sync("refine: input check")) != MRD_OK) return rc;
+  if (hp[0] != 0)
+    return gen_fail(MRD_EINVAL, "refine: " + std::to_string((unsigned long long)hp[0]) + " triangles of the input are clockwise, degenerate or name vertices out of range");
   for (int64_t it = 0;; ++it) {
     // 2.4.1: bad triangles and their circumcentres
     cudaMemsetAsync(cnt, 0, sizeof *cnt, s);

@@ -192,6 +192,15 @@ def test_capacity_and_bad_input_are_reported(mrdb):
     assert g[4]["iterations"] == 2 and g[4]["bad_left"] > 0
     with pytest.raises(mrdb.MrdError):
         mrdb.meshgen_refine(*d, -1.0, 1.0)
+    # an input that is not a valid triangulation (one triangle turned over) is refused by the refinement and by the triangulator
+    import torch
+    bad_tv = tv.copy()
+    bad_tv[5] = bad_tv[5][[0, 2, 1]]
+    db = to_dev(xy, bad_tv, te, et)
+    for call in (lambda: mrdb.meshgen_refine(*db, 0.05, 1.0), lambda: mrdb.meshgen_delaunay_flip(*db)):
+        with pytest.raises(mrdb.MrdError) as ex:
+            call()
+        assert ex.value.code == mrdb.MRD_EINVAL and "clockwise" in str(ex.value)
 
 
 def test_generated_mesh_runs_in_the_solver(mrdb):

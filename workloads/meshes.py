@@ -196,6 +196,8 @@ def scrambled_triangulation(ncx: int, ncy: int, seed: int = 1, amplitude: float 
     general position inside a rectangle -- a jittered ncx x ncy-cell grid (boundary vertices slide along the boundary, so the
     hull stays the rectangle and the Delaunay triangulation of the points is the triangulation of the domain), then `rounds`
     rounds of seeded flips of strictly convex quadrilaterals (every second edge a candidate)."""
+    if not 0.0 <= amplitude <= 0.3:
+        raise ValueError("scrambled_triangulation: amplitude beyond 0.3 cell widths can turn triangles over (not a valid triangulation)")
     m = jitter_mesh(uniform_mesh(ncx, ncy, Lx, Ly, periodic=False), amplitude, seed=seed)
     return flip_edges(m, fraction=0.5, seed=seed + 1, rounds=rounds)
 
