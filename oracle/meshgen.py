@@ -13,10 +13,32 @@ from fractions import Fraction
 import numpy as np
 
 
-def test_quality(xy, tri, R, B):
+def size_factor(p, grid, box):
+    """Section 2.3.1 (L126): "the maximum size can be a function of space, allowing for non-uniform meshes".  Reading M16: the
+    function is given on a grid -- grid[j][i] > 0 at the points (x0 + i (x1 - x0) / (nx - 1), y0 + j (y1 - y0) / (ny - 1)) of the
+    rectangle box = (x0, y0, x1, y1) -- and interpolated bilinearly (points outside the rectangle take the value of the nearest
+    point of its rim); a triangle is too big when r > R * size_factor(circumcentre).  One IEEE operation at a time, in this order."""
+    grid = np.asarray(grid, dtype=np.float64)
+    p = np.asarray(p, dtype=np.float64).reshape(-1, 2)
+    ny, nx = grid.shape
+    x0, y0, x1, y1 = (float(v) for v in box)
+    sx, sy = (nx - 1.0) / (x1 - x0), (ny - 1.0) / (y1 - y0)
+    fx = np.minimum(np.maximum((p[:, 0] - x0) * sx, 0.0), nx - 1.0)
+    fy = np.minimum(np.maximum((p[:, 1] - y0) * sy, 0.0), ny - 1.0)
+    fi, fj = np.minimum(np.floor(fx), nx - 2.0), np.minimum(np.floor(fy), ny - 2.0)
+    i, j = fi.astype(np.int64), fj.astype(np.int64)
+    tx, ty = fx - fi, fy - fj
+    ux, uy = 1.0 - tx, 1.0 - ty
+    g0 = grid[j, i] * ux + grid[j, i + 1] * tx
+    g1 = grid[j + 1, i] * ux + grid[j + 1, i + 1] * tx
+    return g0 * uy + g1 * ty
+
+
+def test_quality(xy, tri, R, B, size=None):
     """eq. 2 (L146): r = l_a l_b l_c / (2 det), det = |a_x - c_x, a_y - c_y; b_x - c_x, b_y - c_y| (eq. 3; footnote 5);
     beta = r / shortest edge (L120); bad = r > R or beta > B (L150), or det <= 0 (the mesh is counter-clockwise);
-    cc = circumcentre, where the new vertex goes (L150): c + (|A|^2 (B_y, -B_x) - |B|^2 (A_y, -A_x)) / (2 det), A = a - c, B = b - c."""
+    cc = circumcentre, where the new vertex goes (L150): c + (|A|^2 (B_y, -B_x) - |B|^2 (A_y, -A_x)) / (2 det), A = a - c, B = b - c.
+    size = (grid, box): the size bound is R * size_factor(cc, grid, box) instead of R (reading M16)."""
     xy = np.asarray(xy, dtype=np.float64)
     a, b, c = xy[tri[:, 0]], xy[tri[:, 1]], xy[tri[:, 2]]
     Ax, Ay, Bx, By = a[:, 0] - c[:, 0], a[:, 1] - c[:, 1], b[:, 0] - c[:, 0], b[:, 1] - c[:, 1]
@@ -31,7 +53,8 @@ def test_quality(xy, tri, R, B):
         ux = (lb2 * By - la2 * Ay) / d2
         uy = (la2 * Ax - lb2 * Bx) / d2
     cc = np.stack([c[:, 0] + ux, c[:, 1] + uy], axis=1)
-    bad = ((r > R) | (beta > B) | ~(det > 0.0)).astype(np.uint8)
+    Rloc = R if size is None else R * size_factor(cc, size[0], size[1])
+    bad = ((r > Rloc) | (beta > B) | ~(det > 0.0)).astype(np.uint8)
     return dict(r=r, beta=beta, cc=cc, bad=bad)
 
 
@@ -368,11 +391,11 @@ def morton_order(xy, tv, box):
     return np.asarray(xy)[order].copy(), canonical_order(new[np.asarray(tv)]), new
 
 
-def _insert_and_flip(xy, tv, te, et, R, B, seed, iteration):
+def _insert_and_flip(xy, tv, te, et, R, B, seed, iteration, size=None):
     """Steps 2.4.1-2.4.6 of one iteration (everything but the re-sort): returns the enlarged arrays, Delaunay again, numbered as
     the insertions and flips left them (which depends on the order of the flips), and the info record."""
     xy = np.asarray(xy, dtype=np.float64)
-    q = test_quality(xy, tv, R, B)
+    q = test_quality(xy, tv, R, B, size)
     bad = np.nonzero(q["bad"])[0]
     cands = []
     for t in bad:
@@ -406,7 +429,7 @@ def _insert_and_flip(xy, tv, te, et, R, B, seed, iteration):
     return xy2, tv2, te2, et2, info
 
 
-def refine_iteration(xy, tv, te, et, R, B, seed, iteration, box=None):
+def refine_iteration(xy, tv, te, et, R, B, seed, iteration, box=None, size=None):
     """One iteration of section 2.4 on a Delaunay triangulation: TestQuality; for every bad triangle, in ascending order, its
     candidate; cavities and the independent set of section 4.1.1 (a triangle claimed by several cavities goes to the highest
     priority; a candidate is selected when it holds every triangle of its cavity); the selected vertices are numbered, and
@@ -414,7 +437,7 @@ def refine_iteration(xy, tv, te, et, R, B, seed, iteration, box=None):
     triangles are put in canonical order (reading M12) -- after the vertices have been renumbered along the Morton curve of
     the rectangle `box` = (x0, y0, x1, y1), when one is given (section 4.1.4, reading M14).
     Returns (xy, tv, te, et, info) as new arrays; info: n_bad, n_selected, kinds of the selected, flips."""
-    xy2, tv2, te2, et2, info = _insert_and_flip(xy, tv, te, et, R, B, seed, iteration)
+    xy2, tv2, te2, et2, info = _insert_and_flip(xy, tv, te, et, R, B, seed, iteration, size)
     if box is not None:                                           # section 4.1.4: Morton order after every insertion step
         xy2, tv2, _ = morton_order(xy2, tv2, box)
     else:
@@ -482,28 +505,28 @@ def renumber_in_place(tv0, te0, et0, tv2):
     return tv, te, et
 
 
-def refine_iteration_in_place(xy, tv, te, et, R, B, seed, iteration):
+def refine_iteration_in_place(xy, tv, te, et, R, B, seed, iteration, size=None):
     """One iteration as refine_iteration, but WITHOUT the re-sort: the mesh keeps its numbering where it did not change
     (renumber_in_place, reading M15).  This is what the iterations of refine() do when no Morton box is given."""
-    xy2, tv2, te2, et2, info = _insert_and_flip(xy, tv, te, et, R, B, seed, iteration)
+    xy2, tv2, te2, et2, info = _insert_and_flip(xy, tv, te, et, R, B, seed, iteration, size)
     tv3, te3, et3 = renumber_in_place(tv, te, et, tv2)
     return xy2, tv3, te3, et3, info
 
 
-def refine(xy, tv, R, B, seed=0, max_iterations=10 ** 6, box=None):
+def refine(xy, tv, R, B, seed=0, max_iterations=10 ** 6, box=None, size=None):
     """Section 2.4: iterate "until no more vertices need to be inserted".  The input is made Delaunay and put in canonical
     order first.  With a Morton `box` every iteration ends with the re-sort of section 4.1.4 (readings M12, M14); without one
     the iterations renumber in place (reading M15) and ONE canonical re-sort follows the last of them (so a run of a single
-    iteration is refine_iteration either way).  Returns (xy, tv, te, et, number of iterations that inserted something)."""
+    iteration is refine_iteration either way).  size = (grid, box of the grid): a size bound that varies in space (reading M16).  Returns (xy, tv, te, et, number of iterations that inserted something)."""
     xy = np.asarray(xy, dtype=np.float64)
     tv = canonical_order(delaunay_flip(xy, tv)[0])
     te, et = build_edges(tv)
     it = 0
     while it < max_iterations:
         if box is not None:
-            xy, tv, te, et, info = refine_iteration(xy, tv, te, et, R, B, seed, it, box)
+            xy, tv, te, et, info = refine_iteration(xy, tv, te, et, R, B, seed, it, box, size)
         else:
-            xy, tv, te, et, info = refine_iteration_in_place(xy, tv, te, et, R, B, seed, it)
+            xy, tv, te, et, info = refine_iteration_in_place(xy, tv, te, et, R, B, seed, it, size)
         if info["n_bad"] == 0:
             break
         it += 1

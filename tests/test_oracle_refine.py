@@ -278,3 +278,34 @@ def test_refine_without_box_is_in_place_iterations_and_one_final_sort():
     assert np.array_equal(xy, sx) and np.array_equal(tv, mg.canonical_order(st))
     assert np.array_equal(mg.refine(xy0, tv0, 0.09, 1.0, seed=6, max_iterations=1)[1],
                           mg.refine_iteration(xy0, mg.canonical_order(tv0), *mg.build_edges(mg.canonical_order(tv0)), 0.09, 1.0, 6, 0)[1])
+
+
+def test_size_function_is_bilinear_and_grades_the_mesh():
+    """Reading M16 (section 2.3.1: the size bound as a function of space)."""
+    grid = np.array([[1.0, 2.0, 4.0], [3.0, 5.0, 9.0]])             # ny = 2, nx = 3 on the rectangle [0, 2] x [10, 11]
+    box = (0.0, 10.0, 2.0, 11.0)
+    f = lambda x, y: float(mg.size_factor([[x, y]], grid, box)[0])
+    assert [f(0, 10), f(1, 10), f(2, 10), f(0, 11), f(1, 11), f(2, 11)] == [1.0, 2.0, 4.0, 3.0, 5.0, 9.0]   # the grid points themselves
+    assert f(0.5, 10) == 1.5 and f(1.5, 11) == 7.0 and f(0, 10.5) == 2.0 and f(1.5, 10.5) == 5.0            # midpoints of edges and of a cell
+    assert f(0.25, 10.25) == (1.0 * 0.75 + 2.0 * 0.25) * 0.75 + (3.0 * 0.75 + 5.0 * 0.25) * 0.25
+    assert f(-3, 9) == 1.0 and f(5, 12) == 9.0 and f(1, 99) == 5.0                                           # outside: the nearest point of the rim
+    rng = np.random.default_rng(0)
+    a, b, c = 0.7, -0.3, 1.9                                        # bilinear interpolation reproduces a + b x + c y + d x y
+    gx, gy = np.meshgrid(np.linspace(0, 2, 5), np.linspace(10, 11, 4))
+    lin = a + b * gx + c * gy + 0.5 * gx * gy
+    pts = rng.random((50, 2)) * np.array([2.0, 1.0]) + np.array([0.0, 10.0])
+    assert np.allclose(mg.size_factor(pts, lin, box), a + b * pts[:, 0] + c * pts[:, 1] + 0.5 * pts[:, 0] * pts[:, 1], rtol=1e-13)
+    # a constant function changes nothing; a graded one grades the mesh and keeps the guarantees
+    xy0, tv0, te0, et0 = start_mesh(seed=4)
+    dom = (0.0, 0.0, 2.0, 1.5)
+    plain = mg.refine(xy0, tv0, 0.1, 1.0, seed=1)
+    const = mg.refine(xy0, tv0, 0.05, 1.0, seed=1, size=(np.full((3, 4), 2.0), dom))
+    assert np.array_equal(plain[0], const[0]) and np.array_equal(plain[1], const[1])
+    g = np.array([[0.25, 1.0, 1.0], [0.25, 1.0, 1.0]])              # a quarter of the size at the left side
+    xy, tv, te, et, it = mg.refine(xy0, tv0, 0.2, 1.0, seed=1, size=(g, dom))
+    q = mg.test_quality(xy, tv, 0.2, 1.0, size=(g, dom))
+    assert q["bad"].sum() == 0 and (q["r"] <= 0.2 * mg.size_factor(q["cc"], g, dom)).all() and q["beta"].max() <= 1.0
+    assert mg.triangle_set(tv) == library_triangulation(xy)
+    left, right = (xy[:, 0] < 0.3).sum() / 0.3, (xy[:, 0] > 1.2).sum() / 0.8
+    assert left > 4 * right                                         # ~16 times the vertex density where the bound is a quarter
+    assert mg.test_quality(xy, tv, 0.2, 1.0)["bad"].sum() == 0 and mg.test_quality(xy, tv, 0.05, 1.0)["bad"].sum() > 0
