@@ -368,7 +368,12 @@ int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_
  *
  * mrd_meshgen_refine: repeats, at most max_iterations times and until no triangle is bad,
  *   1. TestQuality (eq. 2): every triangle with circumradius r > R or r / shortest edge > B is bad; its circumcentre is a
- *      candidate vertex (2.4.1);
+ *      candidate vertex (2.4.1).  The size bound may vary in space (section 2.3.1): with size_dev (DEVICE, double
+ *      [size_ny][size_nx], row-major, all > 0: factors at the points of a regular grid over the rectangle size_box =
+ *      (x0, y0, x1, y1), HOST) the bound is R * f(circumcentre), f the bilinear interpolant of the grid (the nearest rim value
+ *      outside the rectangle), evaluated one IEEE operation at a time: fx = min(max((x - x0) * ((nx - 1) / (x1 - x0)), 0),
+ *      nx - 1), i = min(floor(fx), nx - 2), tx = fx - i (likewise y); f = (g[j][i] (1 - tx) + g[j][i+1] tx) (1 - ty) +
+ *      (g[j+1][i] (1 - tx) + g[j+1][i+1] tx) ty.  size_dev = NULL: f = 1.  Termination needs f >= some M > 0 (L126);
  *   2. the triangle containing the candidate, by the walk of mrd_meshgen_find_triangle from the bad triangle (2.4.2).  A
  *      candidate outside the triangulation becomes the midpoint of the segment the walk left through; one on a segment the
  *      midpoint of that segment; one that coincides with a vertex is dropped;
@@ -407,9 +412,10 @@ int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_
  *   or one that is not a Delaunay triangulation (a walk that does not end).
  * ---------------------------------------------------------------------------------------------- */
 int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteration, int64_t max_iterations, const double *box,
-                       int64_t cap_vertex, int64_t cap_triangle, int64_t cap_edge, int64_t *n_vertex, int64_t *n_triangle,
-                       int64_t *n_edge, double *xy_dev, int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev,
-                       int64_t *n_iterations, int64_t *n_bad_left, void *stream);
+                       const double *size_dev, const double *size_box, int64_t size_nx, int64_t size_ny, int64_t cap_vertex,
+                       int64_t cap_triangle, int64_t cap_edge, int64_t *n_vertex, int64_t *n_triangle, int64_t *n_edge,
+                       double *xy_dev, int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_iterations,
+                       int64_t *n_bad_left, void *stream);
 
 /* Kernel launch counter: number of the library's own kernel launches since the mesh was created. */
 int mrd_launch_count(const mrd_mesh *m, int64_t *launches);

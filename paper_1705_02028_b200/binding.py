@@ -91,7 +91,8 @@ def lib():
         L.mrd_meshgen_release.argtypes = []
         L.mrd_meshgen_build_edges.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
         L.mrd_meshgen_delaunay_flip.argtypes = [C.c_int64, C.c_int64, vp, vp, vp, vp, _lp, _lp, _lp, vp]
-        L.mrd_meshgen_refine.argtypes = [C.c_double, C.c_double, C.c_uint32, C.c_int64, C.c_int64, _dp, C.c_int64, C.c_int64, C.c_int64,
+        L.mrd_meshgen_refine.argtypes = [C.c_double, C.c_double, C.c_uint32, C.c_int64, C.c_int64, _dp, vp, _dp, C.c_int64, C.c_int64,
+                                         C.c_int64, C.c_int64, C.c_int64,
                                          _lp, _lp, _lp, vp, vp, vp, vp, _lp, _lp, vp]
         L.mrd_meshgen_find_triangle.argtypes = [C.c_int64, vp, vp, C.c_int64, vp, vp, vp, vp, vp, vp, vp]
         L.mrd_last_error.restype = C.c_char_p
@@ -507,11 +508,13 @@ def meshgen_release():
     _check(lib().mrd_meshgen_release())
 
 
-def meshgen_refine(xy, tv, te, et, R, B, seed=0, first_iteration=0, max_iterations=10 ** 6, cap_vertex=None, box=None, stream=None):
+def meshgen_refine(xy, tv, te, et, R, B, seed=0, first_iteration=0, max_iterations=10 ** 6, cap_vertex=None, box=None, size=None,
+                   stream=None):
     """Delaunay refinement (include/mrd.h: mrd_meshgen_refine) of the Delaunay triangulation (xy, tv, te, et) (CUDA tensors).
     Returns (xy, tv, te, et, info) as new tensors trimmed to the refined mesh; info: iterations, bad_left.  cap_vertex bounds
     the refined mesh (default 8 x the input + 1024); MrdError(MRD_ENOMEM) when it does not suffice.  box = (x0, y0, x1, y1):
-    renumber the vertices along the Morton curve of that rectangle after every insertion step."""
+    renumber the vertices along the Morton curve of that rectangle after every insertion step.  size = (grid, rectangle): the
+    size bound is R times the bilinear interpolant of grid (float64 CUDA tensor [ny][nx], > 0) over rectangle = (x0, y0, x1, y1)."""
     import torch
     nv, nt, ne = xy.shape[0], tv.shape[0], et.shape[0]
     cv = int(cap_vertex) if cap_vertex else 8 * nv + 1024
@@ -524,7 +527,13 @@ def meshgen_refine(xy, tv, te, et, R, B, seed=0, first_iteration=0, max_iteratio
     n = [C.c_int64(nv), C.c_int64(nt), C.c_int64(ne)]
     it, left = C.c_int64(0), C.c_int64(0)
     hbox = None if box is None else (C.c_double * 4)(*[float(v) for v in box])
-    _check(lib().mrd_meshgen_refine(float(R), float(B), int(seed) & 0xFFFFFFFF, int(first_iteration), int(max_iterations), hbox, cv, ct, ce,
+    sgrid, sbox, snx, sny = None, None, 0, 0
+    if size is not None:
+        g = size[0]
+        assert g.is_cuda and g.dtype == torch.float64 and g.is_contiguous() and g.ndim == 2
+        sgrid, sbox, sny, snx = C.c_void_p(g.data_ptr()), (C.c_double * 4)(*[float(v) for v in size[1]]), g.shape[0], g.shape[1]
+    _check(lib().mrd_meshgen_refine(float(R), float(B), int(seed) & 0xFFFFFFFF, int(first_iteration), int(max_iterations), hbox,
+                                    sgrid, sbox, snx, sny, cv, ct, ce,
                                     C.byref(n[0]), C.byref(n[1]), C.byref(n[2]), *[C.c_void_p(t.data_ptr()) for t in big],
                                     C.byref(it), C.byref(left), _stream_ptr(stream)))
     out = [t[:k.value].clone() for t, k in zip(big, (n[0], n[1], n[1], n[2]))]

@@ -40,10 +40,28 @@ namespace mrdgen {
 // ------------------------------------------------------------------------------------------------------------------
 // TestQuality (eq. 2): one thread per triangle
 // ------------------------------------------------------------------------------------------------------------------
+// Size bound as a function of space (section 2.3.1; reading M16): factors on a grid over a rectangle, interpolated
+// bilinearly at the circumcentre, one IEEE operation at a time in the oracle's order.  g == nullptr: the factor is 1.
+struct SizeGrid {
+  const double *g;        // [ny][nx], row-major
+  int nx, ny;
+  double x0, y0, sx, sy;  // sx = (nx - 1) / (x1 - x0)
+  __device__ __forceinline__ double at(double2 p) const {
+    const double fx = fmin(fmax(__dmul_rn(__dsub_rn(p.x, x0), sx), 0.0), (double)(nx - 1));
+    const double fy = fmin(fmax(__dmul_rn(__dsub_rn(p.y, y0), sy), 0.0), (double)(ny - 1));
+    const double fi = fmin(floor(fx), (double)(nx - 2)), fj = fmin(floor(fy), (double)(ny - 2));
+    const int i = (int)fi, j = (int)fj;
+    const double tx = __dsub_rn(fx, fi), ty = __dsub_rn(fy, fj), ux = __dsub_rn(1.0, tx), uy = __dsub_rn(1.0, ty);
+    const double *row = g + (int64_t)j * nx + i;
+    const double g0 = __dadd_rn(__dmul_rn(row[0], ux), __dmul_rn(row[1], tx));
+    const double g1 = __dadd_rn(__dmul_rn(row[nx], ux), __dmul_rn(row[nx + 1], tx));
+    return __dadd_rn(__dmul_rn(g0, uy), __dmul_rn(g1, ty));
+  }
+};
 __global__ void __launch_bounds__(256)
 test_quality_kernel(int64_t nt, const double2 *__restrict__ xy, const int32_t *__restrict__ tri, double R, double B,
                     double *__restrict__ r_out, double *__restrict__ beta_out, double2 *__restrict__ cc_out,
-                    uint8_t *__restrict__ bad_out, unsigned long long *__restrict__ n_bad) {
+                    uint8_t *__restrict__ bad_out, unsigned long long *__restrict__ n_bad, SizeGrid size) {
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   int bad = 0;
   if (t < nt) {
@@ -66,7 +84,9 @@ test_quality_kernel(int64_t nt, const double2 *__restrict__ xy, const int32_t *_
     const double uy = __ddiv_rn(__dsub_rn(__dmul_rn(la2, Ax), __dmul_rn(lb2, Bx)), d2);
     r_out[t] = r;
     beta_out[t] = beta;
-    cc_out[t] = make_double2(__dadd_rn(c.x, ux), __dadd_rn(c.y, uy));
+    const double2 cc = make_double2(__dadd_rn(c.x, ux), __dadd_rn(c.y, uy));
+    cc_out[t] = cc;
+    if (size.g && det > 0.0) R = __dmul_rn(R, size.at(cc));
     bad = (r > R || beta > B) ? 1 : 0;   // L150 (a triangle with det <= 0 has r <= 0 or inf: flagged by beta or not at all; the
     if (!(det > 0.0)) bad = 1;           //       mesh is counter-clockwise, so det <= 0 is itself a defect: flag it)
     bad_out[t] = (uint8_t)bad;
@@ -950,7 +970,7 @@ int mrd_meshgen_test_quality(int64_t n_triangle, const double *xy_dev, const int
   cudaMemsetAsync(cnt, 0, sizeof *cnt, s);
   if (n_triangle > 0)
     mrdgen::test_quality_kernel<<<(unsigned)((n_triangle + 255) / 256), 256, 0, s>>>(n_triangle, (const double2 *)xy_dev, tri_dev, R, B, r_dev, beta_dev,
-                                                                                     (double2 *)cc_dev, bad_dev, cnt);
+                                                                                     (double2 *)cc_dev, bad_dev, cnt, mrdgen::SizeGrid{nullptr, 0, 0, 0, 0, 0, 0});
   e = cudaMemcpyAsync(g_arena.pinned, cnt, sizeof *cnt, cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e == cudaSuccess) e = cudaGetLastError();
@@ -1209,12 +1229,19 @@ int mrd_meshgen_delaunay_flip(int64_t n_triangle, int64_t n_edge, const double *
 }
 
 int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteration, int64_t max_iterations, const double *box,
-                       int64_t cap_vertex, int64_t cap_triangle, int64_t cap_edge, int64_t *n_vertex, int64_t *n_triangle, int64_t *n_edge,
-                       double *xy_dev, int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_iterations, int64_t *n_bad_left,
-                       void *stream) {
+                       const double *size_dev, const double *size_box, int64_t size_nx, int64_t size_ny, int64_t cap_vertex,
+                       int64_t cap_triangle, int64_t cap_edge, int64_t *n_vertex, int64_t *n_triangle, int64_t *n_edge, double *xy_dev,
+                       int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_iterations, int64_t *n_bad_left, void *stream) {
   if (!n_vertex || !n_triangle || !n_edge || !xy_dev || !tv_dev || !te_dev || !et_dev) return gen_fail(MRD_EINVAL, "null argument");
   if (!(R > 0.0) || !(B > 0.0)) return gen_fail(MRD_EINVAL, "R and B must be positive");
   if (box && !(box[2] > box[0] && box[3] > box[1])) return gen_fail(MRD_EINVAL, "refine: box must be (x0, y0, x1, y1) with x1 > x0, y1 > y0");
+  mrdgen::SizeGrid size_grid{nullptr, 0, 0, 0, 0, 0, 0};
+  if (size_dev) {
+    if (!size_box || !(size_box[2] > size_box[0] && size_box[3] > size_box[1]) || size_nx < 2 || size_ny < 2 || size_nx > 1 << 20 || size_ny > 1 << 20)
+      return gen_fail(MRD_EINVAL, "refine: the size grid needs its rectangle (x0, y0, x1, y1) and at least 2 x 2 points");
+    size_grid = mrdgen::SizeGrid{size_dev, (int)size_nx, (int)size_ny, size_box[0], size_box[1], ((double)size_nx - 1.0) / (size_box[2] - size_box[0]),
+                                 ((double)size_ny - 1.0) / (size_box[3] - size_box[1])};
+  }
   int64_t nv = *n_vertex, nt = *n_triangle, ne = *n_edge;
   if (nv < 3 || nt < 1 || ne < 3 || nv > cap_vertex || nt > cap_triangle || ne > cap_edge || first_iteration < 0 || max_iterations < 0)
     return gen_fail(MRD_EINVAL, "refine: sizes out of range");
@@ -1325,7 +1352,7 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   for (int64_t it = 0;; ++it) {
     // 2.4.1: bad triangles and their circumcentres
     cudaMemsetAsync(cnt, 0, sizeof *cnt, s);
-    mrdgen::test_quality_kernel<<<(unsigned)((nt + 255) / 256), 256, 0, s>>>(nt, xy, tv_dev, R, B, r, beta, cc, bad, cnt);
+    mrdgen::test_quality_kernel<<<(unsigned)((nt + 255) / 256), 256, 0, s>>>(nt, xy, tv_dev, R, B, r, beta, cc, bad, cnt, size_grid);
     cudaMemcpyAsync((void *)hp, cnt, sizeof *cnt, cudaMemcpyDeviceToHost, s);
     if ((rc = sync("refine: test_quality")) != MRD_OK) return rc;
     const int64_t nc = (int64_t)hp[0];

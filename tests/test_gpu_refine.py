@@ -96,6 +96,36 @@ def test_refinement_with_morton_reordering_matches_the_oracle(mrdb, B, R, seed, 
         mrdb.meshgen_refine(*to_dev(xy, tv, te, et), R, B, box=(0.0, 0.0, 0.0, 1.0))
 
 
+def test_graded_refinement_matches_the_oracle(mrdb):
+    """Section 2.3.1: the size bound as a function of space (reading M16) -- iteration by iteration and whole runs the oracle's
+    arrays, in both numbering modes; the refined mesh is finer where the factor is small."""
+    import torch
+    xy, tv, te, et = start(6, (7, 5))
+    dom = (0.0, 0.0, 2.0, 1.5)
+    grid = np.array([[0.2, 0.5, 1.0, 1.0], [0.3, 0.6, 1.0, 1.3], [0.2, 0.5, 1.0, 1.0]])
+    dgrid = dev(grid, torch.float64)
+    R, B, seed = 0.25, 1.1, 6
+    state = (xy, tv, te, et)
+    for it in range(100):
+        o = mg.refine_iteration(*state, R, B, seed, it, size=(grid, dom))
+        g = mrdb.meshgen_refine(*to_dev(*state), R, B, seed=seed, first_iteration=it, max_iterations=1, size=(dgrid, dom))
+        assert same(g[:4], o[:4]), it
+        if o[4]["n_bad"] == 0:
+            break
+        state = o[:4]
+    assert it >= 5
+    for box in (None, dom):
+        o = mg.refine(xy, tv, R, B, seed=seed, box=box, size=(grid, dom))
+        g = mrdb.meshgen_refine(*to_dev(xy, tv, te, et), R, B, seed=seed, box=box, size=(dgrid, dom))
+        assert same(g[:4], o[:4]) and g[4] == dict(iterations=o[4], bad_left=0)
+    X = g[0].cpu().numpy()
+    assert (X[:, 0] < 0.4).sum() / 0.4 > 4 * (X[:, 0] > 1.4).sum() / 0.6
+    q = mg.test_quality(o[0], o[1], R, B, size=(grid, dom))
+    assert q["bad"].sum() == 0
+    with pytest.raises(mrdb.MrdError):
+        mrdb.meshgen_refine(*to_dev(xy, tv, te, et), R, B, size=(dev(np.ones((1, 4)), torch.float64), dom))
+
+
 def test_edge_insertions_on_a_uniform_mesh(mrdb):
     """Right isosceles triangles: every circumcentre is the midpoint of a hypotenuse -- on an interior edge (KIND_EDGE) or on a
     segment -- and every interior edge has four cocircular vertices (all INCIRCLE2D tests take the exact path)."""
