@@ -211,12 +211,15 @@ def find_triangle(xy, tv, te, et, p, t0, max_steps=10 ** 7):
 # ----------------------------------------------------------------------------------------------------------------------
 CAVITY_MAX = 64     # reading M11: a candidate whose cavity has more triangles than this waits for a later iteration
 KIND_NONE, KIND_TRI, KIND_EDGE, KIND_SEG = 0, 1, 2, 3
+PRIORITY_REGULAR = 0xFFFFFFFF   # this value of `seed` selects the regular assignment i(v) = number of the bad triangle (Fig. 8)
 
 
 def priority(seed: int, iteration: int, t: int) -> int:
     """The "unique random integer" i(v) of L648 for the candidate of bad triangle t (reading M10): a 32-bit mix of (seed,
     iteration, t) in the upper half, t itself in the lower half (which makes it unique).  Integer arithmetic modulo 2^32."""
     m = 0xFFFFFFFF
+    if seed == PRIORITY_REGULAR:                                  # "regular integer assignment (i.e. i(v_n) = n)", L654 / Fig. 8
+        return (t << 32) | t
     x = (t * 2654435761 + iteration * 40503 + seed) & m
     x ^= x >> 15
     x = (x * 2246822519) & m

@@ -309,3 +309,25 @@ def test_size_function_is_bilinear_and_grades_the_mesh():
     left, right = (xy[:, 0] < 0.3).sum() / 0.3, (xy[:, 0] > 1.2).sum() / 0.8
     assert left > 4 * right                                         # ~16 times the vertex density where the bound is a quarter
     assert mg.test_quality(xy, tv, 0.2, 1.0)["bad"].sum() == 0 and mg.test_quality(xy, tv, 0.05, 1.0)["bad"].sum() > 0
+
+
+def test_regular_priorities_need_more_iterations_than_random_ones_on_a_morton_ordered_mesh():
+    """L654 / Fig. 8: "because of Morton ordering, vertices with large values of i are located very close to each other, making
+    the parallel selection method very inefficient.  However, for random integer assignment, the number of iterations necessary
+    follows the theoretical limit rather nicely."  Same guarantees either way."""
+    assert mg.priority(mg.PRIORITY_REGULAR, 3, 41) == (41 << 32) | 41 and mg.priority(mg.PRIORITY_REGULAR, 0, 7) < mg.priority(mg.PRIORITY_REGULAR, 9, 8)
+    xy0, tv0, te0, et0 = start_mesh(seed=3)
+    box = (0.0, 0.0, 2.0, 1.5)
+    xr, tr, _, _, it_random = mg.refine(xy0, tv0, 0.09, np.sqrt(2.0), seed=7, box=box)
+    xg, tg, _, _, it_regular = mg.refine(xy0, tv0, 0.09, np.sqrt(2.0), seed=mg.PRIORITY_REGULAR, box=box)
+    assert it_regular > 1.3 * it_random
+    for x, t in ((xr, tr), (xg, tg)):
+        assert mg.test_quality(x, t, 0.09, np.sqrt(2.0))["bad"].sum() == 0 and mg.triangle_set(t) == library_triangulation(x)
+    # in one iteration the regular assignment selects fewer vertices from the same candidates
+    tvc = mg.canonical_order(tv0)
+    tec, etc = mg.build_edges(tvc)
+    xm, tm, _ = mg.morton_order(xy0, tvc, box)
+    tem, etm = mg.build_edges(tm)
+    a = mg.refine_iteration(xm, tm, tem, etm, 0.05, np.sqrt(2.0), 7, 0, box)[4]
+    b = mg.refine_iteration(xm, tm, tem, etm, 0.05, np.sqrt(2.0), mg.PRIORITY_REGULAR, 0, box)[4]
+    assert a["n_candidates"] == b["n_candidates"] and b["n_selected"] < a["n_selected"]
