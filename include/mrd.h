@@ -384,7 +384,9 @@ int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_
  *      insertion triangle(s) through shared edges -- claims its triangles with the candidate's priority i(v) (atomicMax, L648);
  *      a candidate is selected when it holds all of them (4.1.1).  i(v) = mix32(seed, iteration, bad triangle) * 2^32 + bad
  *      triangle; mix32(x): x ^= x >> 15, x *= 2246822519, x ^= x >> 13, x *= 3266489917, x ^= x >> 16 on
- *      x = t * 2654435761 + iteration * 40503 + seed (mod 2^32).  A cavity of more than 64 triangles waits;
+ *      x = t * 2654435761 + iteration * 40503 + seed (mod 2^32).  seed = MRD_MESHGEN_PRIORITY_REGULAR selects the paper's
+ *      "regular integer assignment" i(v) = bad triangle instead (L654, Fig. 8: many more iterations on a Morton-ordered mesh;
+ *      for comparison only).  A cavity of more than 64 triangles waits;
  *   5. the selected vertices are inserted (2.4.4: a triangle split in three, the two triangles at an edge split in two each, the
  *      one triangle at a segment split in two), numbered -- like their new triangles and edges -- in ascending order of
  *      their bad triangle;
@@ -411,6 +413,7 @@ int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_
  *   refined); MRD_EINVAL for an input with a clockwise or degenerate triangle or a vertex number out of range (checked first),
  *   or one that is not a Delaunay triangulation (a walk that does not end).
  * ---------------------------------------------------------------------------------------------- */
+#define MRD_MESHGEN_PRIORITY_REGULAR 0xFFFFFFFFu
 int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteration, int64_t max_iterations, const double *box,
                        const double *size_dev, const double *size_box, int64_t size_nx, int64_t size_ny, int64_t cap_vertex,
                        int64_t cap_triangle, int64_t cap_edge, int64_t *n_vertex, int64_t *n_triangle, int64_t *n_edge,

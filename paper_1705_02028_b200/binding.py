@@ -541,6 +541,7 @@ def meshgen_refine(xy, tv, te, et, R, B, seed=0, first_iteration=0, max_iteratio
 
 
 MESHGEN_STATIC_MAX_TESTS = 1 << 20
+MESHGEN_PRIORITY_REGULAR = 0xFFFFFFFF    # seed value of meshgen_refine: regular instead of random priorities (Fig. 8 of the paper)
 
 
 def meshgen_orient2d_static(xy, idx, sign, n_exact=None, stream=None):

@@ -393,6 +393,7 @@ enum { KIND_NONE = 0, KIND_TRI = 1, KIND_EDGE = 2, KIND_SEG = 3 };
 
 // i(v) of L648 (reading M10): 32-bit mix of (seed, iteration, bad triangle) above the bad triangle's number
 static __device__ __forceinline__ unsigned long long priority_of(unsigned seed, unsigned iteration, unsigned t) {
+  if (seed == 0xFFFFFFFFu) return ((unsigned long long)t << 32) | t;   // MRD_MESHGEN_PRIORITY_REGULAR: i(v_n) = n (L654, Fig. 8)
   unsigned x = t * 2654435761u + iteration * 40503u + seed;
   x ^= x >> 15;
   x *= 2246822519u;

@@ -15,6 +15,7 @@ counters back, which is inside the time):
 * refine            Delaunay refinement (section 2.4, 4.1.1) of a 40 x 40-cell start mesh of the same square down to the
                     circumradius bound that gives about as many vertices as the mesh above (B = sqrt 2): the paper's own test of
                     section 4.1.6, "the generation of a uniform unstructured mesh ... with 1.3 million vertices"
+* --only fig8       the experiment of Fig. 8: insertion iterations against L / s for random and regular priorities
 
 Prints one JSON line per item with the algorithmic bytes per unit (stated in DESIGN.md section 9c) and the GB/s they amount
 to.  Needs a GPU and the built extension; there is no CPU fallback."""
@@ -79,6 +80,8 @@ def run(cells, reps, out_path, only=None):
 
     if only == "refine":
         return refine_part(wl, b, torch, nv, reps, rows, out_path)
+    if only == "fig8":
+        return fig8_part(wl, b, torch, out_path)
     ms, (te0, et0) = timed(lambda: b.meshgen_build_edges(tv0), reps, torch)
     ne = et0.shape[0]
     emit("build_edges", ms, nt, "triangles", dict(n_edges=ne))
@@ -111,6 +114,29 @@ def run(cells, reps, out_path, only=None):
     return refine_part(wl, b, torch, nv, reps, rows, out_path)
 
 
+def fig8_part(wl, b, torch, out_path):
+    """Fig. 8 of the paper (L654): the number of insertion iterations against the mesh size L / s (s: the circumradius bound), for
+    random priorities and for the regular assignment i(v_n) = n, on a mesh that is Morton-ordered after every insertion step;
+    beside the O(log^2(L / s)) of Spielman et al.  Unit square, B = sqrt 2, from a 21 x 21-vertex start mesh."""
+    m = wl.scrambled_triangulation(20, 20, seed=1, Lx=1.0, Ly=1.0)
+    xy = torch.tensor(m.xy, dtype=torch.float64, device="cuda")
+    tv = torch.tensor(m.tri, dtype=torch.int32, device="cuda")
+    te, et = b.meshgen_build_edges(tv)
+    b.meshgen_delaunay_flip(xy, tv, te, et)
+    rows = []
+    for R in (0.02, 0.01, 0.005, 0.0025, 0.00125, 0.000625):
+        row = dict(R=R, L_over_s=1.0 / R, log2_squared=float(np.log2(1.0 / R) ** 2))
+        for name, seed, box in (("random", 7, (0, 0, 1, 1)), ("regular", b.MESHGEN_PRIORITY_REGULAR, (0, 0, 1, 1)), ("random_in_place", 7, None)):
+            g = b.meshgen_refine(xy, tv, te, et, R, float(np.sqrt(2.0)), seed=seed, box=box, cap_vertex=4000000, max_iterations=3000)
+            row["iterations_" + name], row["vertices_" + name], row["bad_left_" + name] = g[4]["iterations"], int(g[0].shape[0]), g[4]["bad_left"]
+        rows.append(row)
+        print(json.dumps(row), flush=True)
+    if out_path:
+        with open(out_path, "w") as f:
+            json.dump(rows, f, indent=1)
+    return rows
+
+
 def refine_part(wl, b, torch, nv, reps, rows, out_path):
     # refinement from a coarse mesh of the same square to about nv vertices: vertices ~ 0.69 area / R^2 at B = sqrt 2 (measured)
     c = wl.scrambled_triangulation(40, 40, seed=2, Lx=2.0, Ly=2.0)
@@ -137,7 +163,8 @@ def main():
     ap.add_argument("--cells", type=int, default=1140)
     ap.add_argument("--reps", type=int, default=5)
     ap.add_argument("--out", default=None)
-    ap.add_argument("--only", default=None, choices=["refine"], help="time the refinement alone")
+    ap.add_argument("--only", default=None, choices=["refine", "fig8"],
+                    help="refine: time the refinement alone; fig8: iterations against mesh size for random and regular priorities")
     a = ap.parse_args()
     run(a.cells, a.reps, a.out, a.only)
     return 0

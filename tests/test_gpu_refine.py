@@ -126,6 +126,26 @@ def test_graded_refinement_matches_the_oracle(mrdb):
         mrdb.meshgen_refine(*to_dev(xy, tv, te, et), R, B, size=(dev(np.ones((1, 4)), torch.float64), dom))
 
 
+def test_regular_priorities_match_the_oracle_and_need_more_iterations(mrdb):
+    """L654 / Fig. 8: regular integer assignment i(v_n) = n against random integers, on a Morton-ordered mesh."""
+    xy, tv, te, et = start(3, (6, 5))
+    box = (0.0, 0.0, 2.0, 1.5)
+    o = mg.refine(xy, tv, 0.09, np.sqrt(2.0), seed=mg.PRIORITY_REGULAR, box=box)
+    g = mrdb.meshgen_refine(*to_dev(xy, tv, te, et), 0.09, np.sqrt(2.0), seed=mrdb.MESHGEN_PRIORITY_REGULAR, box=box)
+    assert same(g[:4], o[:4]) and g[4] == dict(iterations=o[4], bad_left=0)
+    r = mrdb.meshgen_refine(*to_dev(xy, tv, te, et), 0.09, np.sqrt(2.0), seed=7, box=box)
+    assert g[4]["iterations"] > 1.3 * r[4]["iterations"]
+    # at a size beyond the oracle the gap widens
+    m = wl.scrambled_triangulation(30, 30, seed=1, Lx=2.0, Ly=2.0)
+    import torch
+    dxy, dtv = dev(m.xy, torch.float64), dev(m.tri, torch.int32)
+    dte, det = mrdb.meshgen_build_edges(dtv)
+    mrdb.meshgen_delaunay_flip(dxy, dtv, dte, det)
+    its = [mrdb.meshgen_refine(dxy, dtv, dte, det, 0.01, np.sqrt(2.0), seed=sd, box=(0, 0, 2, 2), cap_vertex=200000)[4]["iterations"]
+           for sd in (7, mrdb.MESHGEN_PRIORITY_REGULAR)]
+    assert its[1] > 2 * its[0]
+
+
 def test_edge_insertions_on_a_uniform_mesh(mrdb):
     """Right isosceles triangles: every circumcentre is the midpoint of a hypotenuse -- on an interior edge (KIND_EDGE) or on a
     segment -- and every interior edge has four cocircular vertices (all INCIRCLE2D tests take the exact path)."""
