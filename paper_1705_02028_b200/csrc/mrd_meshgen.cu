@@ -579,23 +579,61 @@ static __device__ __forceinline__ void cavity_act(int64_t j, int n, const int32_
     seg[j] = (mine && kd == KIND_SEG) ? 1 : 0;
   }
 }
-// one thread per candidate, filter only; the candidates with an undecided test are listed for cavity_exact_kernel
+// one thread per candidate, filter and short exact evaluation only; the candidates with a test that needs the long expansions
+// are listed for cavity_exact_kernel.  Pass 1 keeps the cavities it finds in a pool (one atomic per warp reserves the room;
+// off[j] = -1 when the pool is full), pass 2 reads them back instead of walking the mesh again.
 template <int PASS>
 __global__ void __launch_bounds__(128)
 cavity_kernel(int64_t nc, const int32_t *__restrict__ cand, int8_t *__restrict__ kind, const double2 *__restrict__ pt,
               const int32_t *__restrict__ t_ins, const int32_t *__restrict__ e_ins, const double2 *__restrict__ xy,
               const int32_t *__restrict__ tv, const int32_t *__restrict__ te, const int32_t *__restrict__ et,
               unsigned long long *__restrict__ claim, unsigned seed, unsigned iteration, int32_t *__restrict__ sel,
-              int32_t *__restrict__ seg, int32_t *__restrict__ work, unsigned long long *__restrict__ n_work) {
+              int32_t *__restrict__ seg, int32_t *__restrict__ work, unsigned long long *__restrict__ n_work,
+              int32_t *__restrict__ pool, unsigned long long *__restrict__ pool_n, int64_t pool_cap, int32_t *__restrict__ off) {
   const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= nc) return;
+  const bool live = j < nc;
   int32_t list[CAVITY_MAX];
-  const int8_t kd = kind[j];
-  const int n = kd == KIND_NONE ? -1 : cavity_of<false>(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, list, nullptr, nullptr);
+  const int8_t kd = live ? kind[j] : (int8_t)KIND_NONE;
+  int n = -1;
+  bool stored = false;
+  if (PASS == 2 && live && off[j] >= 0) {                         // found in pass 1
+    const int32_t *src = pool + off[j];
+    n = src[0];
+    for (int q = 0; q < n; ++q) list[q] = src[1 + q];
+    stored = true;
+  } else if (live && kd != KIND_NONE) {
+    n = cavity_of<false>(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, list, nullptr, nullptr);
+  }
+  if (PASS == 1) {
+    // room in the pool: 1 + n entries for every cavity found here, reserved once per warp
+    const int want = (live && n > 0) ? n + 1 : 0;
+    const int lane = threadIdx.x & 31;
+    int incl = want;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+      if (lane >= d) incl += v;
+    }
+    const int total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    unsigned long long base = 0;
+    if (lane == 31 && total) base = atomicAdd(pool_n, (unsigned long long)total);
+    base = __shfl_sync(0xFFFFFFFFu, base, 31);
+    if (live) {
+      int32_t o = -1;
+      if (want && (int64_t)(base + incl) <= pool_cap) {
+        o = (int32_t)(base + incl - want);
+        pool[o] = n;
+        for (int q = 0; q < n; ++q) pool[o + 1 + q] = list[q];
+      }
+      off[j] = o;
+    }
+  }
+  if (!live) return;
   if (n == -2) {                                                  // undecided: pass 1 lists it, pass 2 finds it in that list
     if (PASS == 1) work[atomicAdd(n_work, 1ull)] = (int32_t)j;
     return;
   }
+  (void)stored;
   cavity_act<PASS>(j, n, list, kd, priority_of(seed, iteration, (unsigned)cand[j]), kind, claim, sel, seg);
 }
 // the listed candidates again, with the exact INCIRCLE2D where the filter fails.  Grid-stride with few threads: every thread
@@ -1264,6 +1302,8 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   const size_t o_touch_t = c.add(ct), o_touch_e = c.add(ce), o_slot_t = c.add(sizeof(int32_t) * ct), o_slot_e = c.add(sizeof(int32_t) * ce);
   const size_t o_tri_map = c.add(sizeof(int32_t) * ct), o_edge_map = c.add(sizeof(int32_t) * ce), o_tmp_te = c.add(sizeof(int32_t) * 3 * ct);
   const size_t o_tmp_et = c.add(sizeof(int2) * ce), o_jpos = c.add(3 * ct), o_ninit = c.add(sizeof(unsigned long long));
+  const int64_t pool_cap = (int64_t)std::min<size_t>(4 * ct, (size_t)1 << 28);   // ints; a cavity takes 1 + its size
+  const size_t o_cav_pool = c.add(sizeof(int32_t) * (size_t)pool_cap), o_cav_off = c.add(sizeof(int32_t) * ct), o_pool_n = c.add(sizeof(unsigned long long));
   const size_t o_cav_store = c.add(sizeof(int32_t) * (size_t)mrdgen::CAVITY_STORE * (mrdgen::CAVITY_MAX + 1));
   const size_t o_cwork = c.add(sizeof(int32_t) * ct), o_cwork2 = c.add(sizeof(int32_t) * ct), o_cwn = c.add(2 * sizeof(unsigned long long));
   const size_t cm = std::max(ct, (size_t)cap_vertex);               // the sort buffers serve triangles and vertices
@@ -1305,7 +1345,8 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   int2 *tmp_et = (int2 *)(b + o_tmp_et);
   int8_t *jpos = (int8_t *)(b + o_jpos);
   unsigned long long *n_init = (unsigned long long *)(b + o_ninit);
-  int32_t *cav_store = (int32_t *)(b + o_cav_store);
+  int32_t *cav_store = (int32_t *)(b + o_cav_store), *cav_pool = (int32_t *)(b + o_cav_pool), *cav_off = (int32_t *)(b + o_cav_off);
+  unsigned long long *pool_n = (unsigned long long *)(b + o_pool_n);
   int32_t *cwork = (int32_t *)(b + o_cwork), *cwork2 = (int32_t *)(b + o_cwork2);
   unsigned long long *cwork_n = (unsigned long long *)(b + o_cwn);
   void *tmp = b + o_tmp;
@@ -1369,9 +1410,12 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
     const unsigned itn = (unsigned)(first_iteration + it);
     const unsigned nbc = (unsigned)((nc + 127) / 128);
     cudaMemsetAsync(cwork_n, 0, 2 * sizeof(unsigned long long), s);
-    mrdgen::cavity_kernel<1><<<nbc, 128, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, cwork, cwork_n);
+    cudaMemsetAsync(pool_n, 0, sizeof(unsigned long long), s);
+    mrdgen::cavity_kernel<1><<<nbc, 128, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, cwork, cwork_n,
+                                                 cav_pool, pool_n, pool_cap, cav_off);
     mrdgen::cavity_exact_kernel<1><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cwork_n, cwork, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch, cav_store);
-    mrdgen::cavity_kernel<2><<<nbc, 128, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, cwork2, cwork_n + 1);
+    mrdgen::cavity_kernel<2><<<nbc, 128, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, cwork2, cwork_n + 1,
+                                                 cav_pool, pool_n, pool_cap, cav_off);
     mrdgen::cavity_exact_kernel<2><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cwork_n, cwork, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch, cav_store);
     tb = tmp_scan;
     cub::DeviceScan::ExclusiveSum(tmp, tb, sel, rank, nc, s);
