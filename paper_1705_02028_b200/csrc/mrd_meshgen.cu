@@ -445,12 +445,22 @@ static __device__ void around_vertex(int32_t x, int32_t t, double2 p, const doub
 static __device__ __forceinline__ double2 midpoint(double2 u, double2 w) {
   return make_double2(__dmul_rn(0.5, __dadd_rn(u.x, w.x)), __dmul_rn(0.5, __dadd_rn(u.y, w.y)));
 }
+// near[v] = 1 when a triangle that has v as a vertex has a segment for an edge: only around such vertices can the rotation of
+// around_vertex meet a segment, so the encroachment test of all other vertices is skipped (same result, most candidates are
+// far from every segment)
+__global__ void __launch_bounds__(256)
+near_segment_kernel(int64_t ne, const int32_t *__restrict__ et, const int32_t *__restrict__ tv, uint8_t *__restrict__ near) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= ne || et[2 * e + 1] >= 0) return;
+  const int32_t *v = tv + 3 * (int64_t)et[2 * e];
+  near[v[0]] = 1; near[v[1]] = 1; near[v[2]] = 1;
+}
 // sections 2.4.2-2.4.3 for the circumcentre of every bad triangle (oracle/meshgen.py: candidate)
 __global__ void __launch_bounds__(128)
 candidate_kernel(int64_t nc, const int32_t *__restrict__ cand, const double2 *__restrict__ cc, int64_t max_steps,
                  const double2 *__restrict__ xy, const int32_t *__restrict__ tv, const int32_t *__restrict__ te,
                  const int32_t *__restrict__ et, int8_t *__restrict__ kind, double2 *__restrict__ pt, int32_t *__restrict__ t_ins,
-                 int32_t *__restrict__ e_ins, int *__restrict__ err) {
+                 int32_t *__restrict__ e_ins, int *__restrict__ err, const uint8_t *__restrict__ near) {
   const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= nc) return;
   const int32_t tb = cand[j];
@@ -512,10 +522,11 @@ candidate_kernel(int64_t nc, const int32_t *__restrict__ cand, const double2 *__
     if (kd != KIND_SEG) {                                          // eq. 4 around every vertex of the insertion triangle(s)
       int32_t best_e = -1, best_t = -1;
       const int32_t *v = tv + 3 * (int64_t)ti;
-      for (int k = 0; k < 3; ++k) around_vertex(v[k], ti, P, xy, tv, te, et, best_e, best_t);
+      for (int k = 0; k < 3; ++k)
+        if (near[v[k]]) around_vertex(v[k], ti, P, xy, tv, te, et, best_e, best_t);
       if (t2 >= 0) {
-        const int32_t *w = tv + 3 * (int64_t)t2;
-        around_vertex(w[local_of(te + 3 * (int64_t)t2, ei)], t2, P, xy, tv, te, et, best_e, best_t);   // the fourth vertex
+        const int32_t x4 = tv[3 * (int64_t)t2 + local_of(te + 3 * (int64_t)t2, ei)];                    // the fourth vertex
+        if (near[x4]) around_vertex(x4, t2, P, xy, tv, te, et, best_e, best_t);
       }
       if (best_e >= 0) {
         const int k = local_of(te + 3 * (int64_t)best_t, best_e);
@@ -1304,6 +1315,7 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   const size_t o_tmp_et = c.add(sizeof(int2) * ce), o_jpos = c.add(3 * ct), o_ninit = c.add(sizeof(unsigned long long));
   const int64_t pool_cap = (int64_t)std::min<size_t>(4 * ct, (size_t)1 << 28);   // ints; a cavity takes 1 + its size
   const size_t o_cav_pool = c.add(sizeof(int32_t) * (size_t)pool_cap), o_cav_off = c.add(sizeof(int32_t) * ct), o_pool_n = c.add(sizeof(unsigned long long));
+  const size_t o_near = c.add((size_t)cap_vertex);
   const size_t o_cav_store = c.add(sizeof(int32_t) * (size_t)mrdgen::CAVITY_STORE * (mrdgen::CAVITY_MAX + 1));
   const size_t o_cwork = c.add(sizeof(int32_t) * ct), o_cwork2 = c.add(sizeof(int32_t) * ct), o_cwn = c.add(2 * sizeof(unsigned long long));
   const size_t cm = std::max(ct, (size_t)cap_vertex);               // the sort buffers serve triangles and vertices
@@ -1347,6 +1359,7 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   unsigned long long *n_init = (unsigned long long *)(b + o_ninit);
   int32_t *cav_store = (int32_t *)(b + o_cav_store), *cav_pool = (int32_t *)(b + o_cav_pool), *cav_off = (int32_t *)(b + o_cav_off);
   unsigned long long *pool_n = (unsigned long long *)(b + o_pool_n);
+  uint8_t *near_seg = (uint8_t *)(b + o_near);
   int32_t *cwork = (int32_t *)(b + o_cwork), *cwork2 = (int32_t *)(b + o_cwork2);
   unsigned long long *cwork_n = (unsigned long long *)(b + o_cwn);
   void *tmp = b + o_tmp;
@@ -1404,7 +1417,9 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
     size_t tb = tmp_sel;
     cub::DeviceSelect::Flagged(tmp, tb, thrust::counting_iterator<int32_t>(0), (const uint8_t *)bad, cand, d_nsel, nt, s);
     cudaMemsetAsync(err, 0, sizeof(int), s);
-    mrdgen::candidate_kernel<<<(unsigned)((nc + 127) / 128), 128, 0, s>>>(nc, cand, cc, nt + 16, xy, tv_dev, te_dev, et_dev, kind, pt, tins, eins, err);
+    cudaMemsetAsync(near_seg, 0, (size_t)nv, s);
+    mrdgen::near_segment_kernel<<<(unsigned)((ne + 255) / 256), 256, 0, s>>>(ne, et_dev, tv_dev, near_seg);
+    mrdgen::candidate_kernel<<<(unsigned)((nc + 127) / 128), 128, 0, s>>>(nc, cand, cc, nt + 16, xy, tv_dev, te_dev, et_dev, kind, pt, tins, eins, err, near_seg);
     // 4.1.1: cavities, claims, selection
     cudaMemsetAsync(claim, 0, sizeof(unsigned long long) * (size_t)nt, s);
     const unsigned itn = (unsigned)(first_iteration + it);
