@@ -348,9 +348,11 @@ int mrd_meshgen_orient2d_static(int64_t n, const double *xy_dev, const int32_t *
  *   eq. 3).  t[i] >= 0: found, with code[i] = 0 strictly inside, 1 + k on edge k of t, 4 + k on local vertex k (L168);
  *   t[i] = -1 - t_last: the walk left the triangulation through a boundary edge of t_last.  The walk terminates on Delaunay
  *   triangulations; MRD_EINVAL if a walk exceeds n_triangle + 16 steps (not a Delaunay triangulation).
- * Work space: the mrd_meshgen_* calls keep one device block (grown on demand; ~200 MB for the scratch of the exact
- *   predicates plus ~40 B per edge) and a small pinned host block between calls, because allocating them costs more than the
- *   kernels; calls are serialised by a lock.  mrd_meshgen_release frees both (they come back on the next call).
+ * Work space: the mrd_meshgen_* calls keep one device block (grown on demand) and a small pinned host block between calls,
+ *   because allocating them costs more than the kernels; calls are serialised by a lock.  Size: 182 MB for the scratch of the
+ *   exact predicates, plus about 40 bytes per edge for build_edges / delaunay_flip, plus -- for mrd_meshgen_refine -- about 0.9 KB
+ *   per vertex of CAPACITY (sort buffers, candidate records, cavity pool, renumbering maps: 1.8 GB for cap_vertex = 2.1 M).
+ *   mrd_meshgen_release frees both blocks (they come back on the next call).
  * Errors: MRD_EINVAL (null pointer, inconsistent structure), MRD_ENOMEM, MRD_ECUDA.
  * ---------------------------------------------------------------------------------------------- */
 int mrd_meshgen_release(void);
