@@ -356,6 +356,12 @@ int mrd_meshgen_orient2d_static(int64_t n, const double *xy_dev, const int32_t *
  * Errors: MRD_EINVAL (null pointer, inconsistent structure), MRD_ENOMEM, MRD_ECUDA.
  * ---------------------------------------------------------------------------------------------- */
 int mrd_meshgen_release(void);
+/* Diagnostics of the flip loops (mrd_meshgen_delaunay_flip and the flips inside mrd_meshgen_refine) of this process since the last
+ * reset.  Candidate sets of at most 65 536 edges run check -> flip -> check ... in ONE cooperative launch with grid-wide
+ * barriers; that launch can evaluate INCIRCLE2D exactly only when the six translations of the test are exact, and hands an
+ * iteration that meets another test back to the kernels with the long expansions.  stats (HOST out, may be NULL):
+ * [0] cooperative launches, [1] iterations run inside them, [2] iterations handed back, [3] iterations run launch by launch. */
+int mrd_meshgen_flip_stats(int64_t stats[4], int reset);
 int mrd_meshgen_build_edges(int64_t n_triangle, const int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_edge,
                             void *stream);
 int mrd_meshgen_delaunay_flip(int64_t n_triangle, int64_t n_edge, const double *xy_dev, int32_t *tv_dev, int32_t *te_dev,

@@ -89,6 +89,7 @@ def lib():
         L.mrd_meshgen_incircle2d.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
         L.mrd_meshgen_orient2d_static.argtypes = [C.c_int64, vp, vp, vp, vp, vp]
         L.mrd_meshgen_release.argtypes = []
+        L.mrd_meshgen_flip_stats.argtypes = [_lp, C.c_int]
         L.mrd_meshgen_build_edges.argtypes = [C.c_int64, vp, vp, vp, _lp, vp]
         L.mrd_meshgen_delaunay_flip.argtypes = [C.c_int64, C.c_int64, vp, vp, vp, vp, _lp, _lp, _lp, vp]
         L.mrd_meshgen_refine.argtypes = [C.c_double, C.c_double, C.c_uint32, C.c_int64, C.c_int64, _dp, vp, _dp, C.c_int64, C.c_int64,
@@ -557,3 +558,10 @@ def meshgen_orient2d_static(xy, idx, sign, n_exact=None, stream=None):
     assert n_exact is None or (n_exact.is_cuda and n_exact.dtype == torch.int64 and n_exact.numel() == 1)
     _check(lib().mrd_meshgen_orient2d_static(n, C.c_void_p(xy.data_ptr()), C.c_void_p(idx.data_ptr()), C.c_void_p(sign.data_ptr()),
                                              None if n_exact is None else C.c_void_p(n_exact.data_ptr()), _stream_ptr(stream)))
+
+
+def meshgen_flip_stats(reset=False):
+    """dict(cooperative_launches, cooperative_iterations, handed_back, launched_iterations) of the flip loops since the last reset."""
+    out = (C.c_int64 * 4)()
+    _check(lib().mrd_meshgen_flip_stats(out, 1 if reset else 0))
+    return dict(zip(("cooperative_launches", "cooperative_iterations", "handed_back", "launched_iterations"), [int(v) for v in out]))

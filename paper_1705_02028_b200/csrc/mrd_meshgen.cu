@@ -14,6 +14,7 @@
 // expansion arithmetic (error-free transformations TwoSum / TwoProduct with FMA; sums of non-overlapping components with
 // zero elimination).  The sign of an expansion is the sign of its largest component.
 #include <cuda_runtime.h>
+#include <cooperative_groups.h>
 
 #include <algorithm>
 #include <cstdint>
@@ -320,6 +321,120 @@ flip_kernel(int64_t n, const int32_t *__restrict__ cand, int32_t *__restrict__ t
   for (int j = 0; j < cnt; ++j) next[base + incl - cnt + j] = items[j];
   const unsigned fm = __ballot_sync(0xFFFFFFFFu, flipped);
   if (lane == 0 && fm) atomicAdd(&c->n_flip, (unsigned long long)__popc(fm));
+}
+
+// Small candidate sets (the late iterations of a flip loop, the late iterations of a refinement): the whole loop check -> flip ->
+// check -> ... in ONE cooperative launch with grid-wide barriers between the phases, instead of three launches and a counter
+// read-back per iteration.  Same decisions as check_edge_kernel / flip_kernel (the independent set does not depend on which
+// thread looks at which edge).  A test that needs the long expansions cannot be done here (no scratch): the loop stops BEFORE
+// that iteration changes anything and the host path takes over from it.
+struct FlipLoopState {
+  unsigned long long n_bad[2], n_next[2];   // indexed by the parity of the iteration
+  unsigned long long n_flip, n_exact;       // accumulated
+  unsigned long long n_cur;                 // out: candidates of the iteration the loop stopped at
+  int done_iters, converged, abort;         // out
+};
+__global__ void __launch_bounds__(256)
+flip_loop_kernel(int64_t n0, const unsigned long long *__restrict__ n0_dev, int32_t iter0, int max_iters, int32_t *list0, int32_t *list1,
+                 const double2 *__restrict__ xy, int32_t *tv, int32_t *te, int32_t *et, int8_t *state, unsigned long long *lock,
+                 int32_t *mark, FlipLoopState *st, Touch touch) {
+  cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+  const int64_t total = (int64_t)gridDim.x * blockDim.x, gtid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  int64_t n = n0_dev ? min(n0, (int64_t)*n0_dev) : n0;
+  int it = 0;
+  bool converged = false;
+  for (; it < max_iters; ++it) {
+    const int32_t iter = iter0 + it;
+    const int p = iter & 1;
+    const unsigned long long stamp = (unsigned long long)iter << 32;
+    const int32_t *cur = p ? list0 : list1;                       // (the host loop: next = list[iter & 1])
+    int32_t *nxt = p ? list1 : list0;
+    // ---- check
+    for (int64_t base = 0; base < n; base += total) {
+      const int64_t i = base + gtid;
+      bool bad = false, exact = false;
+      if (i < n) {
+        const int32_t e = cur[i];
+        Quad q;
+        if (!load_quad(e, xy, tv, te, et, q)) state[e] = 0;
+        else {
+          int sg = incircle2d_filter(q.a, q.b, q.c, q.d);
+          if (sg == 2) {
+            sg = incircle2d_exact_short(q.a, q.b, q.c, q.d);
+            exact = sg != 2;
+          }
+          if (sg == 2) st->abort = 1;
+          else if (sg == 1) { bid(e, q, stamp, state, lock); bad = true; }
+          else state[e] = 0;
+        }
+      }
+      const unsigned m = __ballot_sync(0xFFFFFFFFu, bad), mx = __ballot_sync(0xFFFFFFFFu, exact);
+      if (lane == 0 && m) atomicAdd(&st->n_bad[p], (unsigned long long)__popc(m));
+      if (lane == 0 && mx) atomicAdd(&st->n_exact, (unsigned long long)__popc(mx));
+    }
+    grid.sync();
+    if (*(volatile int *)&st->abort) break;                        // (uniform: read after the barrier, written only before it)
+    if (*(volatile unsigned long long *)&st->n_bad[p] == 0) { converged = true; ++it; break; }   // (this iteration counts: it found every edge locally Delaunay)
+    if (gtid == 0) { st->n_bad[p ^ 1] = 0; st->n_next[p ^ 1] = 0; }   // for the next iteration; nobody reads them before the next barrier
+    // ---- flip
+    for (int64_t base = 0; base < n; base += total) {
+      const int64_t i = base + gtid;
+      int32_t items[4];
+      int cnt = 0;
+      bool flipped = false;
+      const int32_t e = i < n ? cur[i] : -1;
+      if (e >= 0 && state[e] == 1) {
+        const int32_t t1 = et[2 * (int64_t)e], t2 = et[2 * (int64_t)e + 1];
+        const unsigned long long mine = stamp | (unsigned)e;
+        if (lock[t1] != mine || lock[t2] != mine) {
+          if (atomicExch(mark + e, iter) != iter) items[cnt++] = e;
+        } else {
+          int32_t *v1 = tv + 3 * (int64_t)t1, *v2 = tv + 3 * (int64_t)t2, *e1 = te + 3 * (int64_t)t1, *e2 = te + 3 * (int64_t)t2;
+          const int i1 = e1[0] == e ? 0 : (e1[1] == e ? 1 : 2), i2 = e2[0] == e ? 0 : (e2[1] == e ? 1 : 2);
+          const int32_t a = v1[i1], b = v1[(i1 + 1) % 3], cc = v1[(i1 + 2) % 3], d = v2[i2];
+          const int32_t e_ca = e1[(i1 + 1) % 3], e_ab = e1[(i1 + 2) % 3], e_bd = e2[(i2 + 1) % 3], e_dc = e2[(i2 + 2) % 3];
+          v1[0] = a; v1[1] = b; v1[2] = d;
+          e1[0] = e_bd; e1[1] = e; e1[2] = e_ab;
+          v2[0] = a; v2[1] = d; v2[2] = cc;
+          e2[0] = e_dc; e2[1] = e_ca; e2[2] = e;
+          int32_t *f = et + 2 * (int64_t)e_bd;
+          f[f[0] == t2 ? 0 : 1] = t1;
+          f = et + 2 * (int64_t)e_ca;
+          f[f[0] == t1 ? 0 : 1] = t2;
+          state[e] = 0;
+          touch.tri(t1);
+          touch.tri(t2);
+          touch.edge(e);
+          const int32_t outer[4] = {e_ca, e_ab, e_bd, e_dc};
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            if (atomicExch(mark + outer[j], iter) != iter) items[cnt++] = outer[j];
+          flipped = true;
+        }
+      }
+      int incl = cnt;
+#pragma unroll
+      for (int dlt = 1; dlt < 32; dlt <<= 1) {
+        const int v = __shfl_up_sync(0xFFFFFFFFu, incl, dlt);
+        if (lane >= dlt) incl += v;
+      }
+      const int tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+      unsigned long long bs = 0;
+      if (lane == 31 && tot) bs = atomicAdd(&st->n_next[p], (unsigned long long)tot);
+      bs = __shfl_sync(0xFFFFFFFFu, bs, 31);
+      for (int j = 0; j < cnt; ++j) nxt[bs + incl - cnt + j] = items[j];
+      const unsigned fm = __ballot_sync(0xFFFFFFFFu, flipped);
+      if (lane == 0 && fm) atomicAdd(&st->n_flip, (unsigned long long)__popc(fm));
+    }
+    grid.sync();
+    n = (int64_t)*(volatile unsigned long long *)&st->n_next[p];
+  }
+  if (gtid == 0) {
+    st->done_iters = it;
+    st->converged = converged ? 1 : 0;
+    st->n_cur = (unsigned long long)n;
+  }
 }
 
 // input check of the triangulator and the refinement: every triangle counter-clockwise (exact ORIENT2D > 0), vertex numbers in range
@@ -1163,9 +1278,10 @@ int build_edges_run(const EdgeWork &w, int64_t n_triangle, int bits, const int32
 
 // work space of the flip loop for up to nt triangles and ne edges
 struct FlipWork {
-  size_t o_cnt, o_state, o_lock, o_mark, o_l0, o_l1, o_work, o_scr;
+  size_t o_cnt, o_state, o_lock, o_mark, o_l0, o_l1, o_work, o_scr, o_loop;
   void plan(Carve &c, size_t nt, size_t ne, bool with_scratch) {
     o_cnt = c.add(sizeof(mrdgen::FlipCounters));
+    o_loop = c.add(sizeof(mrdgen::FlipLoopState));
     o_state = c.add(ne);
     o_lock = c.add(sizeof(unsigned long long) * nt);
     o_mark = c.add(sizeof(int32_t) * ne);
@@ -1176,6 +1292,23 @@ struct FlipWork {
   }
 };
 // flips (tv, te, et) to the Delaunay triangulation (arena reserved and locked by the caller); synchronises s every iteration
+// diagnostics of the flip loops since the last mrd_meshgen_flip_stats(reset): cooperative launches, iterations run inside them,
+// iterations handed back to the host path because a test needed the long expansions, iterations run by the host path
+int64_t g_flip_stats[4] = {0, 0, 0, 0};
+constexpr int64_t FLIP_LOOP_MAX = 1 << 16;                           // candidate sets up to this size go through the cooperative loop
+int flip_loop_blocks() {                                          // resident blocks of flip_loop_kernel on the current device (0: not available)
+  static int cached[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 0;
+  if (cached[dev] == 0) {
+    int coop = 0, per_sm = 0, sms = 0;
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (!coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mrdgen::flip_loop_kernel, 256, 0) != cudaSuccess || per_sm < 1) cached[dev] = -1;
+    else cached[dev] = per_sm * sms;
+  }
+  return cached[dev] > 0 ? cached[dev] : 0;
+}
 // `init` (refinement only): the caller has cleared state / lock / mark, put the first candidates into the list at w.o_l0 (their
 // number in device memory, n_upper an upper bound of it) and wants touched slots recorded
 struct FlipInit {
@@ -1205,8 +1338,45 @@ int flip_run(const FlipWork &w, size_t o_scratch, int64_t n_triangle, int64_t n_
   const int32_t *cand = init ? list[0] : nullptr;                // first iteration: every edge, unless the caller knows better
   const unsigned long long *n_dev = init ? init->n_dev : nullptr;
   const mrdgen::Touch touch = init ? init->touch : mrdgen::Touch{nullptr, nullptr, nullptr, nullptr, nullptr};
+  mrdgen::FlipLoopState *loop_dev = (mrdgen::FlipLoopState *)(b + w.o_loop);
+  static_assert(sizeof(mrdgen::FlipLoopState) <= 16 * sizeof(unsigned long long), "pinned block too small");
+  bool host_once = false;                                         // the cooperative loop handed one iteration back
   for (int32_t iter = 1;; ++iter) {
     if (iter > 100000) return gen_fail(MRD_EINVAL, "delaunay_flip: no convergence (is the input a valid triangulation?)");
+    if (cand && n > 0 && n <= FLIP_LOOP_MAX && !host_once) {
+      // small candidate set: the rest of the loop in one cooperative launch (flip_loop_kernel)
+      const int blocks = std::min<int64_t>((n + 255) / 256, flip_loop_blocks());
+      if (blocks > 0) {
+        cudaMemsetAsync(loop_dev, 0, sizeof(mrdgen::FlipLoopState), s);
+        int64_t n0 = n;
+        int32_t iter0 = iter;
+        int max_iters = 64;
+        int32_t *l0 = list[0], *l1 = list[1];
+        void *args[] = {&n0, (void *)&n_dev, &iter0, &max_iters, &l0, &l1, (void *)&xy, &tv_dev, &te_dev, &et_dev, &state, &lock, &mark, &loop_dev, (void *)&touch};
+        cudaError_t e = cudaLaunchCooperativeKernel((const void *)mrdgen::flip_loop_kernel, dim3(blocks), dim3(256), args, 0, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(g_arena.pinned, loop_dev, sizeof(mrdgen::FlipLoopState), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail("delaunay_flip (cooperative loop)", e);
+        const mrdgen::FlipLoopState *hl = (const mrdgen::FlipLoopState *)g_arena.pinned;
+        g_flip_stats[0] += 1;
+        g_flip_stats[1] += hl->done_iters;
+        g_flip_stats[2] += hl->abort ? 1 : 0;
+        iters += hl->done_iters;
+        flips += (int64_t)hl->n_flip;
+        exact += (int64_t)hl->n_exact;
+        if (hl->converged) break;
+        iter += hl->done_iters;                                   // resume at the iteration the loop stopped at
+        cand = list[(iter & 1) ^ 1];
+        n = (int64_t)hl->n_cur;
+        n_dev = nullptr;
+        host_once = hl->abort != 0;                               // that iteration needs the long expansions: host path once
+        --iter;                                                   // (the for statement adds it back)
+        continue;
+      }
+    }
+    host_once = false;
+    g_flip_stats[3] += 1;
     const unsigned long long stamp = (unsigned long long)iter << 32;
     int32_t *next = list[iter & 1];
     const unsigned nb = (unsigned)((n + 255) / 256);
@@ -1232,6 +1402,15 @@ int flip_run(const FlipWork &w, size_t o_scratch, int64_t n_triangle, int64_t n_
   return MRD_OK;
 }
 }  // namespace
+
+int mrd_meshgen_flip_stats(int64_t stats[4], int reset) {
+  std::lock_guard<std::mutex> g(g_arena.mu);
+  if (stats)
+    for (int k = 0; k < 4; ++k) stats[k] = g_flip_stats[k];
+  if (reset)
+    for (int k = 0; k < 4; ++k) g_flip_stats[k] = 0;
+  return MRD_OK;
+}
 
 int mrd_meshgen_build_edges(int64_t n_triangle, const int32_t *tv_dev, int32_t *te_dev, int32_t *et_dev, int64_t *n_edge, void *stream) {
   if (n_triangle < 0 || !n_edge || (n_triangle > 0 && (!tv_dev || !te_dev || !et_dev))) return gen_fail(MRD_EINVAL, "null argument");

@@ -185,3 +185,38 @@ def test_find_triangle_matches_the_oracle(mrdb):
     # strictly inside: the start triangle does not matter
     t_b, _ = mrdb.meshgen_find_triangle(xy, tv, te, et, dev(inside, torch.float64), dev(np.zeros(3000), torch.int32))
     assert np.array_equal(t_b.cpu().numpy(), t[:3000])
+
+
+def test_flip_loop_hands_tests_that_need_long_expansions_back_to_the_host_path(mrdb):
+    """The late iterations of a flip loop run in one cooperative launch that can evaluate INCIRCLE2D exactly only when the six
+    translations are exact.  Here: the fan triangulation of 40 points on the unit circle (as doubles: cocircular to within
+    rounding, so every INCIRCLE2D test is beyond the filter and decided by the last bits; coordinates of every magnitude, so
+    translations are rarely exact).  Neighbouring diagonals share triangles, so many edges lose their triangle and come back
+    in the next iteration with the same test: those iterations go back to the kernels with the long expansions.
+    Result: the oracle's triangles (exact rational arithmetic), every edge locally Delaunay."""
+    import torch
+    from fractions import Fraction
+    n = 40
+    ang = 2.0 * np.pi * np.arange(n) / n + 0.1
+    xy = np.stack([np.cos(ang), np.sin(ang)], axis=1)
+    tri = np.array([[0, i, i + 1] for i in range(1, n - 1)], dtype=np.int32)
+    te0, et0 = mg.build_edges(tri)                                  # how many INCIRCLE2D tests of the input have an inexact translation?
+    inexact = 0
+    for e in np.nonzero(et0[:, 1] >= 0)[0]:
+        t1, t2 = et0[e]
+        d = xy[tri[t2, list(te0[t2]).index(e)]]
+        inexact += any(Fraction(float(p[k])) - Fraction(float(d[k])) != Fraction(float(p[k] - d[k])) for p in xy[tri[t1]] for k in (0, 1))
+    assert inexact > 10
+    dxy, tv = dev(xy, torch.float64), dev(tri, torch.int32)
+    te, et = mrdb.meshgen_build_edges(tv)
+    mrdb.meshgen_flip_stats(reset=True)
+    info = mrdb.meshgen_delaunay_flip(dxy, tv, te, et)
+    stats = mrdb.meshgen_flip_stats()
+    otv, ote, oet, oflips = mg.delaunay_flip(xy, tri)
+    gtv, gte, get = tv.cpu().numpy(), te.cpu().numpy(), et.cpu().numpy()
+    assert oflips > 5 and info["flips"] > 5 and info["iterations"] >= 3 and info["exact"] > 20
+    assert stats["cooperative_launches"] >= 1 and stats["handed_back"] >= 1, stats
+    assert stats["cooperative_iterations"] + stats["launched_iterations"] == info["iterations"]
+    assert mg.triangle_set(gtv) == mg.triangle_set(otv) and structure_ok(gtv, gte, get)
+    for e in range(get.shape[0]):
+        assert not mg.check_edge(xy, gtv, gte, get, e)
