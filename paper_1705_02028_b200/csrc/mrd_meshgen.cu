@@ -1296,8 +1296,9 @@ struct FlipWork {
 // iterations handed back to the host path because a test needed the long expansions, iterations run by the host path
 int64_t g_flip_stats[4] = {0, 0, 0, 0};
 constexpr int64_t FLIP_LOOP_MAX = 1 << 16;                           // candidate sets up to this size go through the cooperative loop
+int g_flip_loop_cached[64] = {};
 int flip_loop_blocks() {                                          // resident blocks of flip_loop_kernel on the current device (0: not available)
-  static int cached[64] = {};
+  int *cached = g_flip_loop_cached;
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 0;
   if (cached[dev] == 0) {
@@ -1354,7 +1355,17 @@ int flip_run(const FlipWork &w, size_t o_scratch, int64_t n_triangle, int64_t n_
         int32_t *l0 = list[0], *l1 = list[1];
         void *args[] = {&n0, (void *)&n_dev, &iter0, &max_iters, &l0, &l1, (void *)&xy, &tv_dev, &te_dev, &et_dev, &state, &lock, &mark, &loop_dev, (void *)&touch};
         cudaError_t e = cudaLaunchCooperativeKernel((const void *)mrdgen::flip_loop_kernel, dim3(blocks), dim3(256), args, 0, s);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(g_arena.pinned, loop_dev, sizeof(mrdgen::FlipLoopState), cudaMemcpyDeviceToHost, s);
+        if (e != cudaSuccess) {
+          // the device cannot hold the grid right now (another context shares it, MPS limits, ...): nothing has run, so the
+          // launch-by-launch path does this and every later iteration of the process
+          cudaGetLastError();
+          int dev = 0;
+          if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64) g_flip_loop_cached[dev] = -1;
+          host_once = true;
+          --iter;
+          continue;
+        }
+        e = cudaMemcpyAsync(g_arena.pinned, loop_dev, sizeof(mrdgen::FlipLoopState), cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
         if (e == cudaSuccess) e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail("delaunay_flip (cooperative loop)", e);
