@@ -1,18 +1,25 @@
-// mrd_meshgen.cu -- first slice of the mesh-generation layer (section 2.4 and 4.1): the two kernels every
-// iteration of the parallel Delaunay refinement starts with, and the two geometric predicates everything else rests on.
+// mrd_meshgen.cu -- the mesh-generation layer (section 2.3-2.4 and 4.1): parallel Delaunay refinement
+// of bounded domains on the GPU, entry points mrd_meshgen_* of include/mrd.h.
 //
-//   test_quality   for every triangle the circumradius r of eq. 2 (L146), the circumradius-to-shortest-edge ratio beta
-//                  (L118-L126), the flag "r > R or beta > B" (L150) and the circumcentre, where the new vertex goes (L150);
-//   orient2d       the sign of the determinant of eq. 3 (L160), EXACT;
-//   incircle2d     the sign of the determinant of eq. 5 (L198), EXACT.
+//   test_quality    for every triangle the circumradius r of eq. 2 (L146), the circumradius-to-shortest-edge ratio beta
+//                   (L118-L126), the flag "r > R or beta > B" (L150) and the circumcentre, where the new vertex goes (L150);
+//   orient2d        the sign of the determinant of eq. 3 (L160), EXACT (also without any allocation: orient2d_static);
+//   incircle2d      the sign of the determinant of eq. 5 (L198), EXACT;
+//   build_edges     triangleEdges and edgeTriangles from triangleVertices (section 4.1.2);
+//   delaunay_flip   flips of independent sets of edges until every edge is locally Delaunay (section 2.4.6, 4.1.5);
+//   find_triangle   the triangle containing a point, by walking (section 2.4.2);
+//   refine          the six steps of section 2.4 with the parallel insertion set of section 4.1.1 and the re-sort of 4.1.4.
 //
 // test_quality is written operation by operation with round-to-nearest intrinsics (no FMA contraction), so that it agrees
 // bit for bit with the CPU oracle (oracle/meshgen.py), which evaluates the same formulas in the same order.
 // The predicates must be exact (L162-L166, L665-L667: "mutually contradictory results inevitably lead to ... invalid
-// triangulations").  The paper uses adaptive exact predicates; here: a floating-point FILTER with a rigorous error bound
-// decides almost every test, and the rest go to a second kernel that evaluates the determinant exactly in floating-point
-// expansion arithmetic (error-free transformations TwoSum / TwoProduct with FMA; sums of non-overlapping components with
-// zero elimination).  The sign of an expansion is the sign of its largest component.
+// triangulations").  The paper uses adaptive exact predicates; here (mrd_predicates.cuh): a floating-point FILTER with a
+// rigorous error bound decides almost every test; the rest are evaluated exactly in floating-point expansion arithmetic
+// (error-free transformations TwoSum / TwoProduct with FMA; sums of non-overlapping components with zero elimination) -- in
+// place, in short thread-local expansions, when the translations of the test are exact, else by threads that own 19 KB of
+// scratch each.  The sign of an expansion is the sign of its largest component.
+// Every integer decision of the refinement (candidate order, priorities, numbering) is a function of the input alone, so the
+// result is, array for array, the oracle's; DESIGN.md section 9c lists the readings M1-M16 behind that.
 #include <cuda_runtime.h>
 #include <cooperative_groups.h>
 
@@ -721,12 +728,10 @@ cavity_kernel(int64_t nc, const int32_t *__restrict__ cand, int8_t *__restrict__
   int32_t list[CAVITY_MAX];
   const int8_t kd = live ? kind[j] : (int8_t)KIND_NONE;
   int n = -1;
-  bool stored = false;
   if (PASS == 2 && live && off[j] >= 0) {                         // found in pass 1
     const int32_t *src = pool + off[j];
     n = src[0];
     for (int q = 0; q < n; ++q) list[q] = src[1 + q];
-    stored = true;
   } else if (live && kd != KIND_NONE) {
     n = cavity_of<false>(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, list, nullptr, nullptr);
   }
@@ -759,7 +764,6 @@ cavity_kernel(int64_t nc, const int32_t *__restrict__ cand, int8_t *__restrict__
     if (PASS == 1) work[atomicAdd(n_work, 1ull)] = (int32_t)j;
     return;
   }
-  (void)stored;
   cavity_act<PASS>(j, n, list, kd, priority_of(seed, iteration, (unsigned)cand[j]), kind, claim, sel, seg);
 }
 // the listed candidates again, with the exact INCIRCLE2D where the filter fails.  Grid-stride with few threads: every thread
