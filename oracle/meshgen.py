@@ -1,10 +1,21 @@
-"""CPU ORACLE of the mesh-generation slice -- test infrastructure, NOT the product.
+"""CPU ORACLE of the mesh-generation layer -- test infrastructure, NOT the product.
 
-Written from PAPER.md section 2.4 (L142-L208): TestQuality (eq. 2) in numpy fp64, one IEEE operation at a time in the order
-the formulas are written (numpy never contracts to FMA), and the two geometric predicates ORIENT2D (eq. 3) and INCIRCLE2D
-(eq. 5) EXACTLY, in rational arithmetic (`fractions.Fraction` represents every double exactly): the sign of the determinant
-as the paper demands it (L162-L166, L206), with no floating-point rounding anywhere.  Pure-Python loops: small cases only.
-Shares nothing with paper_1705_02028_b200/.
+Only tests/ may import it.  Written from PAPER.md sections 2.2-2.4 (L84-L208) and 4.1 (L624-L681), step by step in the paper's
+order; shares nothing with paper_1705_02028_b200/.  Plain Python and numpy fp64; pure-Python loops: small cases only.
+
+* TestQuality (eq. 2), eq. 4 and the size function: one IEEE operation at a time in the order the formulas are written (numpy
+  never contracts to FMA), so that the kernels can be compared bit for bit;
+* ORIENT2D (eq. 3) and INCIRCLE2D (eq. 5): EXACTLY, in rational arithmetic (`fractions.Fraction` represents every double
+  exactly), the sign of the determinant as the paper demands it (L162-L166, L206);
+* the mesh data structure (section 4.1.2), the Delaunay triangulator by sequential edge flips (2.4.6), the walk to the containing
+  triangle (2.4.2), candidates with encroachment (2.4.3), cavities and the independent insertion set (4.1.1), the three vertex
+  insertions (2.4.4), the re-sorts (4.1.4) and the refinement loop (2.4).
+
+Readings where the paper is silent (M1-M16) are listed in DESIGN.md section 9c.  Pins (tests/test_oracle_meshgen.py,
+test_oracle_triangulator.py, test_oracle_refine.py): textbook triangles, the library Delaunay triangulation of the same points,
+brute-force empty circumcircles and cavities, Lawson's angle criterion, exhaustive containment search, the diametric circle of
+eq. 4, disjoint selected cavities, the guarantees of section 2.3 on finished meshes, the Z curve of a 4 x 4 grid, bilinear
+functions, Fig. 8's ordering of random against regular priorities.  No function here is "parity unpinned".
 """
 from __future__ import annotations
 
