@@ -154,3 +154,20 @@ def test_bench_on_a_mesh_generated_by_the_library():
     assert gen["iterations"] >= 5 and 0.7 * 160 * 160 < gen["n_vertices"] == d["config"]["n_vertices"] < 1.4 * 160 * 160
     assert 1.9 < d["config"]["n_triangles"] / d["config"]["n_vertices"] < 2.0 and d["value"] > 0
     assert "GENERATED on the GPU" in d["config"]["workload"] and d["roofline"]["traffic"] is None
+
+
+def test_measurement_modules_run_at_a_small_size():
+    """python -m paper_1705_02028_b200.sweep and .meshgen_bench (the commands behind BASELINE.md section 6 and profiles/r02_meshgen.md)."""
+    import json
+    r = subprocess.run([sys.executable, "-m", "paper_1705_02028_b200.sweep", "--sizes", "64", "--steps", "5", "--reps", "2"],
+                       capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    rows = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(rows) == 6 and all(row["ms_per_step"] > 0 and row["triangles"] == 2 * 64 * 64 for row in rows)
+    r = subprocess.run([sys.executable, "-m", "paper_1705_02028_b200.meshgen_bench", "--cells", "60", "--reps", "1"],
+                       capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    rows = {row["kernel"]: row for row in (json.loads(l) for l in r.stdout.splitlines() if l.startswith("{"))}
+    assert set(rows) == {"build_edges", "delaunay_flip", "check_only", "test_quality", "find_triangle", "refine", "refine_morton"}
+    assert rows["delaunay_flip"]["flips"] > 1000 and rows["refine"]["bad_left"] == 0 and rows["refine_morton"]["bad_left"] == 0
+    assert rows["find_triangle"]["found"] == rows["find_triangle"]["units"]
