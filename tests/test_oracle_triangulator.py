@@ -39,6 +39,20 @@ def assert_structure(xy, tv, te, et):
     assert (et[:, 0] >= 0).all()
 
 
+@pytest.mark.parametrize("shape,Lx,Ly,seed", [((36, 48), 100.0, 64.0, 778), ((3, 59), 1.0, 64.0, 5), ((200, 200), 2.0, 2.0, 3)])
+def test_the_workload_is_a_valid_triangulation_at_the_largest_allowed_jitter(shape, Lx, Ly, seed):
+    # the input recipe of DESIGN.md 9c: every triangle counter-clockwise (exact test), the areas add up to the rectangle; the first
+    # case is one that a jitter of 0.3 cell widths turns over, which is why the generator stops at 0.25
+    m = wl.scrambled_triangulation(*shape, seed=seed, amplitude=0.25, Lx=Lx, Ly=Ly)
+    p = m.xy[m.tri]
+    area = 0.5 * ((p[:, 1, 0] - p[:, 0, 0]) * (p[:, 2, 1] - p[:, 0, 1]) - (p[:, 1, 1] - p[:, 0, 1]) * (p[:, 2, 0] - p[:, 0, 0]))
+    assert (area > 0).all() and abs(area.sum() - Lx * Ly) < 1e-9 * Lx * Ly
+    worst = np.argsort(area)[:50]
+    assert all(mg.orient2d(*m.xy[m.tri[t]]) == 1 for t in worst)
+    with pytest.raises(ValueError, match="0.25"):
+        wl.scrambled_triangulation(*shape, seed=seed, amplitude=0.3, Lx=Lx, Ly=Ly)
+
+
 def test_build_edges_follows_the_stated_conventions():
     m = wl.uniform_mesh(7, 5, 1.0, 1.0, periodic=False)
     tv = m.tri.astype(np.int32)

@@ -117,7 +117,9 @@ def morton_order_mesh(mesh: UniformMesh):
 
 def jitter_mesh(mesh: UniformMesh, amplitude: float = 0.25, seed: int = 7) -> UniformMesh:
     """Move every vertex by a seeded uniform offset of at most `amplitude` cell widths in x and y
-    (amplitude < 0.5 keeps all triangles positively oriented for the SW-NE split when < ~0.3).
+    (amplitude <= 0.25 keeps every triangle of the SW-NE split positively oriented: a corner and the opposite side
+    can each move 0.25 sqrt 2 cell widths towards each other, together the 0.707 between them; 0.3 already turns about one
+    triangle in 10^4 over).
     Gives non-uniform triangle shapes/areas for pins and parity on "genuinely unstructured" geometry.
     Boundary vertices of bounded meshes are only moved along their boundary."""
     rng = np.random.default_rng(seed)
@@ -196,8 +198,8 @@ def scrambled_triangulation(ncx: int, ncy: int, seed: int = 1, amplitude: float 
     general position inside a rectangle -- a jittered ncx x ncy-cell grid (boundary vertices slide along the boundary, so the
     hull stays the rectangle and the Delaunay triangulation of the points is the triangulation of the domain), then `rounds`
     rounds of seeded flips of strictly convex quadrilaterals (every second edge a candidate)."""
-    if not 0.0 <= amplitude <= 0.3:
-        raise ValueError("scrambled_triangulation: amplitude beyond 0.3 cell widths can turn triangles over (not a valid triangulation)")
+    if not 0.0 <= amplitude <= 0.25:
+        raise ValueError("scrambled_triangulation: amplitude beyond 0.25 cell widths can turn triangles over (not a valid triangulation)")
     m = jitter_mesh(uniform_mesh(ncx, ncy, Lx, Ly, periodic=False), amplitude, seed=seed)
     return flip_edges(m, fraction=0.5, seed=seed + 1, rounds=rounds)
 
