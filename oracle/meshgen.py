@@ -220,7 +220,6 @@ def find_triangle(xy, tv, te, et, p, t0, max_steps=10 ** 7):
 # ----------------------------------------------------------------------------------------------------------------------
 # Delaunay refinement (section 2.4) with the parallel insertion set of section 4.1.1 (L634-L654), bounded domains
 # ----------------------------------------------------------------------------------------------------------------------
-CAVITY_MAX = 64     # reading M11: a candidate whose cavity has more triangles than this waits for a later iteration
 KIND_NONE, KIND_TRI, KIND_EDGE, KIND_SEG = 0, 1, 2, 3
 PRIORITY_REGULAR = 0xFFFFFFFF   # this value of `seed` selects the regular assignment i(v) = number of the bad triangle (Fig. 8)
 
@@ -417,9 +416,7 @@ def _insert_and_flip(xy, tv, te, et, R, B, seed, iteration, size=None):
         if kind == KIND_NONE:
             continue
         start = [int(et[e, 0]), int(et[e, 1])] if kind == KIND_EDGE else [t_ins]
-        cav = cavity(xy, tv, te, et, p, start)
-        if len(cav) > CAVITY_MAX:
-            continue
+        cav = cavity(xy, tv, te, et, p, start)        # the whole set of L638, however large (reading M11)
         cands.append((int(t), kind, p, t_ins, e, cav))
     lock = {}
     for t, kind, p, t_ins, e, cav in cands:

@@ -84,6 +84,54 @@ def test_cavity_is_every_triangle_whose_circumcircle_contains_the_point():
         assert cav == brute and t in cav and len(cav) >= 1        # connected: the walk from t finds them all (L644)
 
 
+def sliver_mesh(cells=34, height=8.0, seed=4):
+    """A Delaunay start mesh made of slivers: two rows of `cells` + 1 boundary vertices, `height` apart, seeded spacing along the rows
+    (a coarse outline, as a user would give it): the circumcircles are as large as the strip, so the first cavities hold most
+    of the mesh."""
+    m = wl.jitter_mesh(wl.uniform_mesh(cells, 1, 1.0, height, periodic=False), 0.25, seed=seed)
+    tv, te, et, _ = mg.delaunay_flip(m.xy, m.tri)
+    return m.xy, tv, te, et
+
+
+def test_a_cavity_has_no_vertex_inside_so_its_triangles_form_a_tree():
+    # what lets a walk without a list of visited triangles find a cavity (L640-L646; reading M11): a vertex with every one of its
+    # triangles in the cavity would vanish from the new triangulation, so there is none, and a triangulated polygon without inner
+    # vertices has one shared edge less than it has triangles
+    for xy, tv, te, et in (start_mesh(seed=5, shape=(9, 7)), sliver_mesh()):
+        rng = np.random.default_rng(3)
+        lo, hi = xy.min(axis=0), xy.max(axis=0)
+        sizes = []
+        for p in lo + rng.random((40, 2)) * (hi - lo):
+            t, code = mg.find_triangle(xy, tv, te, et, p, 0)
+            if code != 0:
+                continue
+            cav = set(mg.cavity(xy, tv, te, et, p, [t]))
+            inner = [e for e in range(et.shape[0]) if int(et[e, 0]) in cav and int(et[e, 1]) in cav]
+            assert len(inner) == len(cav) - 1
+            rim = {int(v) for e in np.nonzero(et[:, 1] < 0)[0] for v in mg._edge_ends(tv, te, int(et[e, 0]), int(e))}
+            used = {int(v) for c in cav for v in tv[c]} - rim      # vertices inside the domain
+            assert not any(all(k in cav for k in np.nonzero((tv == v).any(axis=1))[0]) for v in used)
+            sizes.append(len(cav))
+        assert len(sizes) > 20
+    assert max(sizes) > 40                                        # the sliver mesh: most of its 68 triangles in one cavity
+
+
+def test_refinement_from_a_mesh_of_slivers_with_cavities_of_most_of_the_mesh():
+    # L638 defines the cavity as the whole set: no bound on its size (reading M11)
+    xy0, tv0, te0, et0 = sliver_mesh()
+    q0 = mg.test_quality(xy0, tv0, 1.0, np.sqrt(2.0))
+    first = [len(mg.cavity(xy0, tv0, te0, et0, q0["cc"][t], [mg.find_triangle(xy0, tv0, te0, et0, q0["cc"][t], int(t))[0]]))
+             for t in np.nonzero(q0["bad"])[0] if mg.find_triangle(xy0, tv0, te0, et0, q0["cc"][t], int(t))[1] == 0]
+    assert max(first) > 64
+    xy, tv, te, et, it = mg.refine(xy0, tv0, 1.0, np.sqrt(2.0), seed=2)
+    assert mg.test_quality(xy, tv, 1.0, np.sqrt(2.0))["bad"].sum() == 0 and xy.shape[0] > 2 * xy0.shape[0]
+    assert_structure(xy, tv, te, et)
+    assert all(not mg.check_edge(xy, tv, te, et, e) for e in range(et.shape[0]))
+    # the library's triangulation of the same points, up to the diagonals of cocircular quadrilaterals (midpoints of a strip's sides)
+    assert len(mg.triangle_set(tv) ^ library_triangulation(xy)) <= 0.05 * tv.shape[0]
+    assert abs(area(xy, tv).sum() - 8.0) < 1e-12 and np.array_equal(xy[:xy0.shape[0]], xy0)
+
+
 def test_eq_4_is_the_diametric_circle():
     rng = np.random.default_rng(2)
     xy = rng.random((2, 2))
