@@ -394,7 +394,9 @@ int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_
  *      triangle; mix32(x): x ^= x >> 15, x *= 2246822519, x ^= x >> 13, x *= 3266489917, x ^= x >> 16 on
  *      x = t * 2654435761 + iteration * 40503 + seed (mod 2^32).  seed = MRD_MESHGEN_PRIORITY_REGULAR selects the paper's
  *      "regular integer assignment" i(v) = bad triangle instead (L654, Fig. 8: many more iterations on a Morton-ordered mesh;
- *      for comparison only).  A cavity of more than 64 triangles waits;
+ *      for comparison only).  A cavity may be of any size (a start mesh of slivers has cavities of most of its triangles): up to
+ *      64 triangles are kept in a per-thread list, a larger cavity is walked along its outline without a list, which relies on
+ *      the input being a Delaunay triangulation (its cavities are trees; a walk that does not close makes the candidate wait);
  *   5. the selected vertices are inserted (2.4.4: a triangle split in three, the two triangles at an edge split in two each, the
  *      one triangle at a segment split in two), numbered -- like their new triangles and edges -- in ascending order of
  *      their bad triangle;

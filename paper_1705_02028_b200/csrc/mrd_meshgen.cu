@@ -698,16 +698,82 @@ static __device__ int cavity_of(double2 p, int8_t kd, int32_t ti, int32_t ei, co
   }
   return n;
 }
-// pass 1: claim the cavity's triangles; pass 2: selected when every one of them still carries this candidate's priority
-template <int PASS>
+// Reading M11: a cavity that does not fit the per-thread list is walked without a list.  The cavity of a point in a Delaunay
+// triangulation has no vertex inside it (the fan from the new vertex over its rim IS the new triangulation), so under "shares an
+// edge" its triangles form a tree, and the walk follows the outline of that tree (L640-L646: "by always checking the neighbours
+// in anti-clockwise order"): arrived in t through its local edge k it tries k+1 and k+2 and then leaves through k again; the
+// root tries its edges 0, 1, 2 once.  A triangle is tested again when the walk comes back to it from a child -- the actions are
+// idempotent.  PASS 1 claims every triangle on arrival, PASS 2 compares every one.  Returns 1 (PASS 2: 0 when a triangle
+// carries another priority), -2 when EXACT is false and the filter cannot decide a test, -1 when the walk does not close within
+// 4 nt + 16 moves (the input was not a Delaunay triangulation): the candidate waits.
+template <int PASS, bool EXACT>
+static __device__ int cavity_walk(double2 p, int8_t kd, int32_t ti, int32_t ei, const double2 *xy, const int32_t *tv, const int32_t *te,
+                                  const int32_t *et, int64_t nt, unsigned long long pr, unsigned long long *claim, double *acc,
+                                  double *tmp) {
+  const int32_t root = kd == KIND_EDGE ? et[2 * (int64_t)ei] : ti;
+  const int32_t root2 = kd == KIND_EDGE ? et[2 * (int64_t)ei + 1] : -1;
+  if (PASS == 1) atomicMax(claim + root, pr);
+  else if (claim[root] != pr) return 0;
+  int32_t t = root;
+  int k = -1;                                                     // root: the last of its edges that was tried
+  for (int64_t moves = 0; moves < 4 * nt + 16; ++moves) {
+    int go = -1;
+    const bool at_root = t == root;
+    for (int d = 1; d <= (at_root ? 2 - k : 2) && go < 0; ++d) {
+      const int q = at_root ? k + d : (k + d) % 3;
+      const int32_t nb = across(et, te[3 * (int64_t)t + q], t);
+      if (nb < 0) continue;
+      int sg = 1;
+      if (nb != root && nb != root2) {
+        const int32_t *v = tv + 3 * (int64_t)nb;
+        const double2 A = xy[v[0]], B = xy[v[1]], C = xy[v[2]];
+        sg = incircle2d_filter(A, B, C, p);
+        if (sg == 2) sg = incircle2d_exact_short(A, B, C, p);
+        if (sg == 2) {
+          if (!EXACT) return -2;
+          sg = incircle2d_exact(A, B, C, p, acc, tmp);
+        }
+      }
+      if (sg > 0) go = q;
+    }
+    if (go < 0) {
+      if (at_root) return 1;                                      // the outline is closed
+      go = k;                                                     // back to where this triangle was entered from
+    }
+    const int32_t e = te[3 * (int64_t)t + go];
+    const int32_t nb = across(et, e, t);
+    if (PASS == 1) atomicMax(claim + nb, pr);
+    else if (claim[nb] != pr) return 0;
+    k = local_of(te + 3 * (int64_t)nb, e);
+    t = nb;
+  }
+  return -1;
+}
+// pass 1: claim the cavity's triangles; pass 2: selected when every one of them still carries this candidate's priority.
+// n > 0: the cavity is in `list`; n == -1: it did not fit (cavity_walk); n == -3: nothing to insert
+template <int PASS, bool EXACT>
 static __device__ __forceinline__ void cavity_act(int64_t j, int n, const int32_t *list, int8_t kd, unsigned long long pr, int8_t *kind,
-                                                  unsigned long long *claim, int32_t *sel, int32_t *seg) {
+                                                  unsigned long long *claim, int32_t *sel, int32_t *seg, const double2 *pt,
+                                                  const int32_t *t_ins, const int32_t *e_ins, const double2 *xy, const int32_t *tv,
+                                                  const int32_t *te, const int32_t *et, int64_t nt, double *acc, double *tmp,
+                                                  int32_t *work, unsigned long long *n_work) {
   if (PASS == 1) {
-    if (n < 0) kind[j] = KIND_NONE;                                // too large (M11) or nothing to insert: waits
+    if (n == -1) {
+      const int r = cavity_walk<1, EXACT>(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, nt, pr, claim, acc, tmp);
+      if (r == -2) work[atomicAdd(n_work, 1ull)] = (int32_t)j;     // only when EXACT is false: the exact kernel walks it again
+      else if (r < 0) kind[j] = KIND_NONE;
+      return;
+    }
+    if (n < 0) kind[j] = KIND_NONE;                                // nothing to insert: waits
     for (int q = 0; q < n; ++q) atomicMax(claim + list[q], pr);
   } else {
     bool mine = n > 0;
     for (int q = 0; q < n; ++q) mine &= claim[list[q]] == pr;
+    if (n == -1) {
+      const int r = cavity_walk<2, EXACT>(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, nt, pr, claim, acc, tmp);
+      if (r == -2) return;                                         // in the work list of pass 1: the exact kernel decides
+      mine = r == 1;
+    }
     sel[j] = mine ? 1 : 0;
     seg[j] = (mine && kd == KIND_SEG) ? 1 : 0;
   }
@@ -722,12 +788,13 @@ cavity_kernel(int64_t nc, const int32_t *__restrict__ cand, int8_t *__restrict__
               const int32_t *__restrict__ tv, const int32_t *__restrict__ te, const int32_t *__restrict__ et,
               unsigned long long *__restrict__ claim, unsigned seed, unsigned iteration, int32_t *__restrict__ sel,
               int32_t *__restrict__ seg, int32_t *__restrict__ work, unsigned long long *__restrict__ n_work,
-              int32_t *__restrict__ pool, unsigned long long *__restrict__ pool_n, int64_t pool_cap, int32_t *__restrict__ off) {
+              int32_t *__restrict__ pool, unsigned long long *__restrict__ pool_n, int64_t pool_cap, int32_t *__restrict__ off,
+              int64_t nt) {
   const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool live = j < nc;
   int32_t list[CAVITY_MAX];
   const int8_t kd = live ? kind[j] : (int8_t)KIND_NONE;
-  int n = -1;
+  int n = -3;
   if (PASS == 2 && live && off[j] >= 0) {                         // found in pass 1
     const int32_t *src = pool + off[j];
     n = src[0];
@@ -764,7 +831,8 @@ cavity_kernel(int64_t nc, const int32_t *__restrict__ cand, int8_t *__restrict__
     if (PASS == 1) work[atomicAdd(n_work, 1ull)] = (int32_t)j;
     return;
   }
-  cavity_act<PASS>(j, n, list, kd, priority_of(seed, iteration, (unsigned)cand[j]), kind, claim, sel, seg);
+  cavity_act<PASS, false>(j, n, list, kd, priority_of(seed, iteration, (unsigned)cand[j]), kind, claim, sel, seg, pt, t_ins, e_ins, xy,
+                          tv, te, et, nt, nullptr, nullptr, work, n_work);
 }
 // the listed candidates again, with the exact INCIRCLE2D where the filter fails.  Grid-stride with few threads: every thread
 // owns a slice of the expansion scratch.  One exact evaluation is a serial chain of ~10^4 operations on expansions in global
@@ -778,7 +846,7 @@ cavity_exact_kernel(const unsigned long long *__restrict__ n_work, const int32_t
                     const int32_t *__restrict__ e_ins, const double2 *__restrict__ xy, const int32_t *__restrict__ tv,
                     const int32_t *__restrict__ te, const int32_t *__restrict__ et, unsigned long long *__restrict__ claim, unsigned seed,
                     unsigned iteration, int32_t *__restrict__ sel, int32_t *__restrict__ seg, double *__restrict__ scratch,
-                    int32_t *__restrict__ store) {
+                    int32_t *__restrict__ store, int64_t nt) {
   const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, nw = (int64_t)*n_work;
   double *acc = scratch + tid * (2 * MAXE), *tmp = acc + MAXE;
   int32_t list[CAVITY_MAX];
@@ -791,13 +859,14 @@ cavity_exact_kernel(const unsigned long long *__restrict__ n_work, const int32_t
       n = st[0];
       for (int q = 0; q < n; ++q) list[q] = st[1 + q];
     } else {
-      n = kd == KIND_NONE ? -1 : cavity_of<true>(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, list, acc, tmp);
+      n = kd == KIND_NONE ? -3 : cavity_of<true>(pt[j], kd, t_ins[j], e_ins[j], xy, tv, te, et, list, acc, tmp);
       if (PASS == 1 && w < CAVITY_STORE) {
         st[0] = n;
         for (int q = 0; q < n; ++q) st[1 + q] = list[q];
       }
     }
-    cavity_act<PASS>(j, n, list, kd, priority_of(seed, iteration, (unsigned)cand[j]), kind, claim, sel, seg);
+    cavity_act<PASS, true>(j, n, list, kd, priority_of(seed, iteration, (unsigned)cand[j]), kind, claim, sel, seg, pt, t_ins, e_ins, xy, tv,
+                           te, et, nt, acc, tmp, nullptr, nullptr);
   }
 }
 static __device__ __forceinline__ void swap_side(int32_t *et, int32_t e, int32_t from, int32_t to) {
@@ -1621,11 +1690,11 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
     cudaMemsetAsync(cwork_n, 0, 2 * sizeof(unsigned long long), s);
     cudaMemsetAsync(pool_n, 0, sizeof(unsigned long long), s);
     mrdgen::cavity_kernel<1><<<nbc, 128, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, cwork, cwork_n,
-                                                 cav_pool, pool_n, pool_cap, cav_off);
-    mrdgen::cavity_exact_kernel<1><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cwork_n, cwork, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch, cav_store);
+                                                 cav_pool, pool_n, pool_cap, cav_off, nt);
+    mrdgen::cavity_exact_kernel<1><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cwork_n, cwork, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch, cav_store, nt);
     mrdgen::cavity_kernel<2><<<nbc, 128, 0, s>>>(nc, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, cwork2, cwork_n + 1,
-                                                 cav_pool, pool_n, pool_cap, cav_off);
-    mrdgen::cavity_exact_kernel<2><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cwork_n, cwork, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch, cav_store);
+                                                 cav_pool, pool_n, pool_cap, cav_off, nt);
+    mrdgen::cavity_exact_kernel<2><<<EXACT_BLOCKS, EXACT_THREADS, 0, s>>>(cwork_n, cwork, cand, kind, pt, tins, eins, xy, tv_dev, te_dev, et_dev, claim, seed, itn, sel, seg, scratch, cav_store, nt);
     tb = tmp_scan;
     cub::DeviceScan::ExclusiveSum(tmp, tb, sel, rank, nc, s);
     tb = tmp_scan;
@@ -1639,7 +1708,7 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
     if ((rc = sync("refine: candidates")) != MRD_OK) return rc;
     if (h32[0]) return gen_fail(MRD_EINVAL, "refine: a point-location walk did not end (the input is not a Delaunay triangulation)");
     const int64_t nsel = (int64_t)h32[1] + h32[2], nseg = (int64_t)h32[3] + h32[4];
-    if (nsel == 0) return gen_fail(MRD_EINVAL, "refine: bad triangles remain but no vertex can be inserted (cavities beyond 64 triangles or circumcentres on vertices)");
+    if (nsel == 0) return gen_fail(MRD_EINVAL, "refine: bad triangles remain but no vertex can be inserted (every circumcentre falls on a vertex, or the input was not a Delaunay triangulation)");
     const int64_t nv2 = nv + nsel, nt2 = nt + 2 * nsel - nseg, ne2 = ne + 3 * nsel - nseg;
     if (nv2 > cap_vertex || nt2 > cap_triangle || ne2 > cap_edge) {
       rc = gen_fail(MRD_ENOMEM, "refine: capacity of the mesh arrays reached (the mesh is valid and Delaunay; call again with larger arrays)");

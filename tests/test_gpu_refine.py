@@ -73,6 +73,42 @@ def test_every_iteration_and_the_whole_run_match_the_oracle(mrdb, B, R, seed, sh
     assert q["bad"].sum() == 0
 
 
+@pytest.mark.parametrize("jitter,cells,height,R,whole", [(0.25, 34, 8.0, 1.0, True), (0.0, 40, 6.0, 0.8, True), (0.2, 90, 20.0, 3.0, False)])
+def test_cavities_beyond_the_per_thread_list_match_the_oracle(mrdb, jitter, cells, height, R, whole):
+    """Reading M11 / L638: a cavity is the whole set, however large.  A start mesh of slivers (two rows of boundary vertices: a coarse
+    outline) has first cavities of most of its triangles -- more than the 64 a thread keeps in its list, so the kernels walk the
+    outline of the cavity instead (cavity_walk).  Every iteration from the oracle's state and the whole run, array for array;
+    jitter 0 makes every cell's four vertices cocircular (INCIRCLE2D exactly zero: the exact path)."""
+    m = wl.uniform_mesh(cells, 1, 1.0, height, periodic=False)
+    if jitter:
+        m = wl.jitter_mesh(m, jitter, seed=4)
+    tv = mg.canonical_order(mg.delaunay_flip(m.xy, m.tri)[0])
+    te, et = mg.build_edges(tv)
+    xy, B, seed = m.xy, float(np.sqrt(2.0)), 2
+    q0 = mg.test_quality(xy, tv, R, B)
+    sizes = [len(mg.cavity(xy, tv, te, et, q0["cc"][t], [loc[0]])) for t in np.nonzero(q0["bad"])[0]
+             for loc in [mg.find_triangle(xy, tv, te, et, q0["cc"][t], int(t))] if loc[1] == 0]
+    assert max(sizes) > (64 if whole else 150)
+    state = (xy, tv, te, et)
+    for it in range(100 if whole else 6):                          # the third case: the first iterations only (the oracle's time)
+        o = mg.refine_iteration(*state, R, B, seed, it)
+        g = mrdb.meshgen_refine(*to_dev(*state), R, B, seed=seed, first_iteration=it, max_iterations=1)
+        assert same(g[:4], o[:4]), it
+        if o[4]["n_bad"] == 0:
+            break
+        state = o[:4]
+    assert it >= 3
+    if not whole:
+        return
+    o = mg.refine(xy, tv, R, B, seed=seed)
+    g = mrdb.meshgen_refine(*to_dev(xy, tv, te, et), R, B, seed=seed)
+    assert same(g[:4], o[:4]) and g[4] == dict(iterations=o[4], bad_left=0)
+    box = (0.0, 0.0, 1.0, height)
+    o = mg.refine(xy, tv, R, B, seed=seed, box=box)
+    g = mrdb.meshgen_refine(*to_dev(xy, tv, te, et), R, B, seed=seed, box=box)
+    assert same(g[:4], o[:4]) and g[4]["bad_left"] == 0
+
+
 @pytest.mark.parametrize("B,R,seed,shape", [(1.0, 0.07, 4, (6, 5)), (np.sqrt(2.0), 0.045, 5, (8, 6))])
 def test_refinement_with_morton_reordering_matches_the_oracle(mrdb, B, R, seed, shape):
     """Section 4.1.4: vertices renumbered along the Morton curve after every insertion step -- every iteration and the whole
