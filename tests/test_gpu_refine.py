@@ -266,6 +266,51 @@ def test_refinement_at_size_keeps_the_guarantees_of_section_2_3(mrdb):
     assert all(torch.equal(a, b) for a, b in zip((gx, gt, gte, get), g2[:4]))
 
 
+@pytest.mark.parametrize("n,ax,ay,B,target", [(400, 3.0, 2.0, np.sqrt(2.0), 20000), (2000, 1.0, 1.0, 1.0, 200000), (30, 3.0, 1.0, 1.2, 2000)])
+def test_refinement_of_an_outline_keeps_the_guarantees(mrdb, n, ax, ay, B, target):
+    """The way a user starts (section 2.4: "starting from the boundary"): the domain given by its boundary vertices only -- a convex
+    polygon inscribed in an ellipse, triangulated as a fan, made Delaunay by flips (slivers: the first cavities hold most of
+    the mesh, reading M11), then refined.  No bad triangle left, every edge locally Delaunay by the exact test, the polygon
+    covered exactly once, boundary vertices only on the polygon's sides, the same result on a second call."""
+    import torch
+    rng = np.random.default_rng(n)
+    ang = np.unique(np.sort(rng.random(n)) * 2 * np.pi)
+    n = len(ang)
+    X0 = np.stack([ax * np.cos(ang), ay * np.sin(ang)], axis=1)
+    T0 = np.stack([np.zeros(n - 2, dtype=np.int32), np.arange(1, n - 1, dtype=np.int32), np.arange(2, n, dtype=np.int32)], axis=1)
+    area0 = 0.5 * np.abs(np.sum(X0[:, 0] * np.roll(X0[:, 1], -1) - np.roll(X0[:, 0], -1) * X0[:, 1]))
+    R = float(np.sqrt(0.69 * area0 / target))
+    xy, tv = dev(X0, torch.float64), dev(T0, torch.int32)
+    te, et = mrdb.meshgen_build_edges(tv)
+    mrdb.meshgen_delaunay_flip(xy, tv, te, et)
+    gx, gt, gte, get, info = mrdb.meshgen_refine(xy, tv, te, et, R, B, seed=3, cap_vertex=20 * target)
+    assert info["bad_left"] == 0 and info["iterations"] >= 5
+    X, T, TE, ET = gx.cpu().numpy(), gt.cpu().numpy(), gte.cpu().numpy(), get.cpu().numpy()
+    assert X.shape[0] > 0.3 * target and np.array_equal(X[:n], X0)
+    assert mg.test_quality(X, T, R, B)["bad"].sum() == 0
+    p = X[T]
+    area = 0.5 * ((p[:, 1, 0] - p[:, 0, 0]) * (p[:, 2, 1] - p[:, 0, 1]) - (p[:, 1, 1] - p[:, 0, 1]) * (p[:, 2, 0] - p[:, 0, 0]))
+    assert (area > 0).all() and abs(area.sum() - area0) < 1e-10 * area0
+    inner = np.nonzero(ET[:, 1] >= 0)[0]
+    t1, t2 = ET[inner, 0], ET[inner, 1]
+    k2 = (TE[t2] == inner[:, None]).argmax(axis=1)
+    quads = np.concatenate([T[t1], T[t2, k2][:, None]], axis=1).astype(np.int32)
+    sgn, _ = mrdb.meshgen_incircle2d(gx, dev(quads, torch.int32))
+    assert (sgn <= 0).all().item()
+    for qd in quads[np.random.default_rng(1).choice(len(quads), 100, replace=False)]:
+        assert mg.incircle2d(*X[qd]) <= 0
+    # the boundary vertices of the result lie on the sides of the polygon (midpoints of midpoints ... of its sides, up to rounding)
+    seg = np.nonzero(ET[:, 1] < 0)[0]
+    k = (TE[ET[seg, 0]] == seg[:, None]).argmax(axis=1)
+    on = np.unique(np.concatenate([T[ET[seg, 0], (k + 1) % 3], T[ET[seg, 0], (k + 2) % 3]]))
+    side = np.clip(np.searchsorted(ang, np.arctan2(X[on, 1] / ay, X[on, 0] / ax) % (2 * np.pi), side="right") - 1, -1, n - 1)
+    a, c = X0[side], X0[(side + 1) % n]
+    dist = np.abs((c[:, 0] - a[:, 0]) * (X[on, 1] - a[:, 1]) - (c[:, 1] - a[:, 1]) * (X[on, 0] - a[:, 0])) / np.hypot(*(c - a).T)
+    assert dist.max() < 1e-12 * max(ax, ay)
+    g2 = mrdb.meshgen_refine(xy, tv, te, et, R, B, seed=3, cap_vertex=20 * target)
+    assert all(torch.equal(u, w) for u, w in zip((gx, gt, gte, get), g2[:4]))
+
+
 def test_capacity_and_bad_input_are_reported(mrdb):
     xy, tv, te, et = start(1, (6, 5))
     d = to_dev(xy, tv, te, et)
