@@ -266,6 +266,36 @@ def test_refinement_at_size_keeps_the_guarantees_of_section_2_3(mrdb):
     assert all(torch.equal(a, b) for a, b in zip((gx, gt, gte, get), g2[:4]))
 
 
+def refined_and_checked(mrdb, X0, T0, R, B, seed, cap, area0):
+    """Start mesh (X0, T0) made Delaunay and refined on the device; asserts what section 2.3 guarantees and what must hold of any
+    refinement -- no bad triangle left, every triangle counter-clockwise, the domain covered exactly once, the input vertices kept,
+    every interior edge locally Delaunay by the exact test (the kernel's, a sample again by the oracle's rational arithmetic), the
+    same arrays on a second call -- and returns the refined mesh on the host."""
+    import torch
+    xy, tv = dev(X0, torch.float64), dev(T0, torch.int32)
+    te, et = mrdb.meshgen_build_edges(tv)
+    mrdb.meshgen_delaunay_flip(xy, tv, te, et)
+    gx, gt, gte, get, info = mrdb.meshgen_refine(xy, tv, te, et, R, B, seed=seed, cap_vertex=cap)
+    assert info["bad_left"] == 0 and info["iterations"] >= 3
+    X, T, TE, ET = gx.cpu().numpy(), gt.cpu().numpy(), gte.cpu().numpy(), get.cpu().numpy()
+    assert np.array_equal(X[:len(X0)], X0)
+    assert mg.test_quality(X, T, R, B)["bad"].sum() == 0
+    p = X[T]
+    area = 0.5 * ((p[:, 1, 0] - p[:, 0, 0]) * (p[:, 2, 1] - p[:, 0, 1]) - (p[:, 1, 1] - p[:, 0, 1]) * (p[:, 2, 0] - p[:, 0, 0]))
+    assert (area > 0).all() and abs(area.sum() - area0) < 1e-10 * area0
+    inner = np.nonzero(ET[:, 1] >= 0)[0]
+    t1, t2 = ET[inner, 0], ET[inner, 1]
+    k2 = (TE[t2] == inner[:, None]).argmax(axis=1)
+    quads = np.concatenate([T[t1], T[t2, k2][:, None]], axis=1).astype(np.int32)
+    sgn, _ = mrdb.meshgen_incircle2d(gx, dev(quads, torch.int32))
+    assert (sgn <= 0).all().item()
+    for qd in quads[np.random.default_rng(1).choice(len(quads), min(100, len(quads)), replace=False)]:
+        assert mg.incircle2d(*X[qd]) <= 0
+    g2 = mrdb.meshgen_refine(xy, tv, te, et, R, B, seed=seed, cap_vertex=cap)
+    assert all(torch.equal(u, w) for u, w in zip((gx, gt, gte, get), g2[:4]))
+    return X, T, TE, ET
+
+
 @pytest.mark.parametrize("n,ax,ay,B,target", [(400, 3.0, 2.0, np.sqrt(2.0), 20000), (2000, 1.0, 1.0, 1.0, 200000), (30, 3.0, 1.0, 1.2, 2000)])
 def test_refinement_of_an_outline_keeps_the_guarantees(mrdb, n, ax, ay, B, target):
     """The way a user starts (section 2.4: "starting from the boundary"): the domain given by its boundary vertices only -- a convex
@@ -280,25 +310,8 @@ def test_refinement_of_an_outline_keeps_the_guarantees(mrdb, n, ax, ay, B, targe
     T0 = np.stack([np.zeros(n - 2, dtype=np.int32), np.arange(1, n - 1, dtype=np.int32), np.arange(2, n, dtype=np.int32)], axis=1)
     area0 = 0.5 * np.abs(np.sum(X0[:, 0] * np.roll(X0[:, 1], -1) - np.roll(X0[:, 0], -1) * X0[:, 1]))
     R = float(np.sqrt(0.69 * area0 / target))
-    xy, tv = dev(X0, torch.float64), dev(T0, torch.int32)
-    te, et = mrdb.meshgen_build_edges(tv)
-    mrdb.meshgen_delaunay_flip(xy, tv, te, et)
-    gx, gt, gte, get, info = mrdb.meshgen_refine(xy, tv, te, et, R, B, seed=3, cap_vertex=20 * target)
-    assert info["bad_left"] == 0 and info["iterations"] >= 5
-    X, T, TE, ET = gx.cpu().numpy(), gt.cpu().numpy(), gte.cpu().numpy(), get.cpu().numpy()
-    assert X.shape[0] > 0.3 * target and np.array_equal(X[:n], X0)
-    assert mg.test_quality(X, T, R, B)["bad"].sum() == 0
-    p = X[T]
-    area = 0.5 * ((p[:, 1, 0] - p[:, 0, 0]) * (p[:, 2, 1] - p[:, 0, 1]) - (p[:, 1, 1] - p[:, 0, 1]) * (p[:, 2, 0] - p[:, 0, 0]))
-    assert (area > 0).all() and abs(area.sum() - area0) < 1e-10 * area0
-    inner = np.nonzero(ET[:, 1] >= 0)[0]
-    t1, t2 = ET[inner, 0], ET[inner, 1]
-    k2 = (TE[t2] == inner[:, None]).argmax(axis=1)
-    quads = np.concatenate([T[t1], T[t2, k2][:, None]], axis=1).astype(np.int32)
-    sgn, _ = mrdb.meshgen_incircle2d(gx, dev(quads, torch.int32))
-    assert (sgn <= 0).all().item()
-    for qd in quads[np.random.default_rng(1).choice(len(quads), 100, replace=False)]:
-        assert mg.incircle2d(*X[qd]) <= 0
+    X, T, TE, ET = refined_and_checked(mrdb, X0, T0, R, B, 3, 20 * target, area0)
+    assert X.shape[0] > 0.3 * target
     # the boundary vertices of the result lie on the sides of the polygon (midpoints of midpoints ... of its sides, up to rounding)
     seg = np.nonzero(ET[:, 1] < 0)[0]
     k = (TE[ET[seg, 0]] == seg[:, None]).argmax(axis=1)
@@ -307,8 +320,34 @@ def test_refinement_of_an_outline_keeps_the_guarantees(mrdb, n, ax, ay, B, targe
     a, c = X0[side], X0[(side + 1) % n]
     dist = np.abs((c[:, 0] - a[:, 0]) * (X[on, 1] - a[:, 1]) - (c[:, 1] - a[:, 1]) * (X[on, 0] - a[:, 0])) / np.hypot(*(c - a).T)
     assert dist.max() < 1e-12 * max(ax, ay)
-    g2 = mrdb.meshgen_refine(xy, tv, te, et, R, B, seed=3, cap_vertex=20 * target)
-    assert all(torch.equal(u, w) for u, w in zip((gx, gt, gte, get), g2[:4]))
+
+
+@pytest.mark.parametrize("domain,shape,Lx,Ly,B,target", [("L", (8, 6), 2.0, 1.5, 1.2, 300), ("hole", (7, 7), 1.0, 1.0, np.sqrt(2.0), 300),
+                                                          ("notch", (9, 6), 2.0, 1.0, 1.0, 300), ("hole", (40, 3), 30.0, 1.0, 1.2, 20000),
+                                                          ("L", (33, 47), 2.0, 20.0, np.sqrt(2.0), 200000), ("notch", (5, 44), 30.0, 1.5, 2.0, 20000)])
+def test_domains_with_reentrant_corners_notches_and_holes(mrdb, domain, shape, Lx, Ly, B, target):
+    """Bounded domains that are not convex: a grid with its upper right quarter ("L"), a block of cells in the middle ("hole") or
+    most of one column of cells ("notch") taken out.  A circumcentre beyond a reentrant corner or across a notch is outside the
+    triangulation as far as the walk of section 2.4.2 can tell: the segment the walk left through is split (reading M8).  The
+    small cases whole runs against the oracle, array for array; all cases the guarantees."""
+    m = wl.uniform_mesh(*shape, Lx, Ly, periodic=False)
+    c = m.xy[m.tri].mean(axis=1)
+    ci, cj = np.floor(c[:, 0] / Lx * shape[0]).astype(int), np.floor(c[:, 1] / Ly * shape[1]).astype(int)
+    drop = {"L": (ci >= shape[0] // 2) & (cj >= shape[1] // 2),
+            "hole": (ci >= shape[0] // 2) & (ci < shape[0] // 2 + 2) & (cj == shape[1] // 2),
+            "notch": (ci == shape[0] // 2) & (cj >= shape[1] // 3)}[domain]
+    tri = m.tri[~drop]
+    used = np.unique(tri)
+    new = -np.ones(m.nv, dtype=np.int64)
+    new[used] = np.arange(len(used))
+    X0, T0 = m.xy[used], mg.canonical_order(new[tri].astype(np.int32))      # a grid: Delaunay as it stands (cocircular cells)
+    area0 = Lx * Ly * (1.0 - drop.sum() / len(drop))
+    R = float(np.sqrt(0.69 * area0 / target))
+    X, T, TE, ET = refined_and_checked(mrdb, X0, T0, R, B, 5, 3000000, area0)
+    assert X.shape[0] > 0.3 * target
+    if target <= 300:
+        o = mg.refine(X0, T0, R, B, seed=5)
+        assert np.array_equal(o[0], X) and np.array_equal(o[1], T) and np.array_equal(o[2], TE) and np.array_equal(o[3], ET)
 
 
 def test_capacity_and_bad_input_are_reported(mrdb):
