@@ -158,7 +158,7 @@ class Layout:
 
     def __del__(self):
         h, self._h = getattr(self, "_h", None), None
-        if h:
+        if h and lib is not None:                                  # module globals are gone when the interpreter shuts down
             lib().mrd_layout_destroy(h)
 
     def get(self):
@@ -268,7 +268,7 @@ class Mesh:
 
     def __del__(self):
         h, self._h = getattr(self, "_h", None), None
-        if h:
+        if h and lib is not None:                                  # module globals are gone when the interpreter shuts down
             lib().mrd_mesh_destroy(h)
 
     close = __del__
