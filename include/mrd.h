@@ -342,7 +342,10 @@ int mrd_meshgen_orient2d_static(int64_t n, const double *xy_dev, const int32_t *
  *   (four cocircular vertices) are left alone.  The result is unique as a set of triangles when no four vertices are
  *   cocircular (L96), and deterministic (bitwise the same arrays on every run) in any case.
  *   HOST outs (may be NULL): n_flips, n_iterations, n_exact (INCIRCLE2D tests that needed the exact path).
- *   MRD_EINVAL when a triangle of the input is clockwise or degenerate (exact ORIENT2D <= 0): not a valid triangulation.
+ *   MRD_EINVAL when a triangle of the input is clockwise or degenerate (exact ORIENT2D <= 0), when te and et disagree, or when
+ *   the two triangles of an edge run along it in the same direction (they lie on the same side: an overlap): not a valid
+ *   triangulation, and flips on it need not end or keep the structure.  (What is not checked: overlaps of triangles that share
+ *   no edge.)
  * mrd_meshgen_find_triangle: for every point p[i] (double[n][2]) the triangle that contains it, by walking from t0[i] across
  *   the first edge -- tried in the order (a, b), (b, c), (c, a) -- that has p strictly on its outer side (exact ORIENT2D,
  *   eq. 3).  t[i] >= 0: found, with code[i] = 0 strictly inside, 1 + k on edge k of t, 4 + k on local vertex k (L168);
@@ -420,8 +423,9 @@ int mrd_meshgen_find_triangle(int64_t n_point, const double *p_dev, const int32_
  *   Guarantees on completion (section 2.3): no triangle with r > R or beta > B, hence no angle below arcsin(1 / 2B); Delaunay;
  *   no encroached segment.  Termination is guaranteed for B >= sqrt(2) and domains without small angles (L126).
  *   MRD_ENOMEM when the next insertion would exceed a capacity (the arrays then hold a valid Delaunay mesh, partly
- *   refined); MRD_EINVAL for an input with a clockwise or degenerate triangle or a vertex number out of range (checked first),
- *   or one that is not a Delaunay triangulation (a walk that does not end).
+ *   refined); MRD_EINVAL for an input with a clockwise or degenerate triangle or a vertex number out of range, or edge tables
+ *   that do not describe a triangulation (as for mrd_meshgen_delaunay_flip; all checked first), or one that is not a Delaunay
+ *   triangulation (a walk that does not end).
  * ---------------------------------------------------------------------------------------------- */
 #define MRD_MESHGEN_PRIORITY_REGULAR 0xFFFFFFFFu
 int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteration, int64_t max_iterations, const double *box,

@@ -458,6 +458,45 @@ validate_kernel(int64_t nt, int64_t nv, const double2 *__restrict__ xy, const in
   if ((threadIdx.x & 31) == 0 && m) atomicAdd(n_bad, (unsigned long long)__popc(m));
 }
 
+// the edge tables describe a triangulation: every edge is listed by the triangle(s) edgeTriangles names for it, at the local
+// place opposite the vertex that is not on it, and its two triangles run along it in opposite directions (two counter-clockwise
+// triangles that run along a shared edge in the same direction lie on the same side of it: they overlap)
+__global__ void __launch_bounds__(256)
+validate_edges_kernel(int64_t ne, int64_t nt, const int32_t *__restrict__ tv, const int32_t *__restrict__ te, const int32_t *__restrict__ et,
+                      unsigned long long *__restrict__ n_bad) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool bad = false;
+  if (e < ne) {
+    const int32_t t1 = et[2 * e], t2 = et[2 * e + 1];
+    bad = t1 < 0 || t1 >= nt || t2 >= nt || t1 == t2;
+    if (!bad) {
+      const int32_t *E1 = te + 3 * (int64_t)t1, *V1 = tv + 3 * (int64_t)t1;
+      const int k1 = E1[0] == e ? 0 : E1[1] == e ? 1 : E1[2] == e ? 2 : -1;
+      bad = k1 < 0;
+      if (!bad && t2 >= 0) {
+        const int32_t *E2 = te + 3 * (int64_t)t2, *V2 = tv + 3 * (int64_t)t2;
+        const int k2 = E2[0] == e ? 0 : E2[1] == e ? 1 : E2[2] == e ? 2 : -1;
+        bad = k2 < 0 || V1[(k1 + 1) % 3] != V2[(k2 + 2) % 3] || V1[(k1 + 2) % 3] != V2[(k2 + 1) % 3];
+      }
+    }
+  }
+  const unsigned m = __ballot_sync(0xFFFFFFFFu, bad);
+  if ((threadIdx.x & 31) == 0 && m) atomicAdd(n_bad, (unsigned long long)__popc(m));
+}
+// every triangle's three edges exist and name the triangle
+__global__ void __launch_bounds__(256)
+validate_sides_kernel(int64_t nt, int64_t ne, const int32_t *__restrict__ te, const int32_t *__restrict__ et, unsigned long long *__restrict__ n_bad) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool bad = false;
+  if (t < nt)
+    for (int k = 0; k < 3; ++k) {
+      const int32_t e = te[3 * t + k];
+      bad |= e < 0 || e >= ne || (et[2 * (int64_t)e] != t && et[2 * (int64_t)e + 1] != t);
+    }
+  const unsigned m = __ballot_sync(0xFFFFFFFFu, bad);
+  if ((threadIdx.x & 31) == 0 && m) atomicAdd(n_bad, (unsigned long long)__popc(m));
+}
+
 // ------------------------------------------------------------------------------------------------------------------
 // Point location (section 2.4.2)
 // ------------------------------------------------------------------------------------------------------------------
@@ -1538,6 +1577,16 @@ int mrd_meshgen_delaunay_flip(int64_t n_triangle, int64_t n_edge, const double *
   if (e != cudaSuccess) return cuda_fail("delaunay_flip", e);
   if (g_arena.pinned[0] != 0)
     return gen_fail(MRD_EINVAL, "delaunay_flip: " + std::to_string(g_arena.pinned[0]) + " triangles of the input are clockwise or degenerate");
+  cudaMemsetAsync(bad, 0, sizeof *bad, s);
+  if (n_triangle > 0) mrdgen::validate_sides_kernel<<<(unsigned)((n_triangle + 255) / 256), 256, 0, s>>>(n_triangle, n_edge, te_dev, et_dev, bad);
+  if (n_edge > 0) mrdgen::validate_edges_kernel<<<(unsigned)((n_edge + 255) / 256), 256, 0, s>>>(n_edge, n_triangle, tv_dev, te_dev, et_dev, bad);
+  e = cudaMemcpyAsync(g_arena.pinned, bad, sizeof *bad, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("delaunay_flip", e);
+  if (g_arena.pinned[0] != 0)
+    return gen_fail(MRD_EINVAL, "delaunay_flip: the edge tables do not describe a triangulation (" + std::to_string(g_arena.pinned[0]) +
+                    " entries: triangleEdges and edgeTriangles disagree, or the two triangles of an edge lie on the same side of it)");
   return flip_run(w, w.o_scr, n_triangle, n_edge, (const double2 *)xy_dev, tv_dev, te_dev, et_dev, n_flips, n_iterations, n_exact, s);
 }
 
@@ -1667,6 +1716,14 @@ int mrd_meshgen_refine(double R, double B, uint32_t seed, int64_t first_iteratio
   if ((rc = sync("refine: input check")) != MRD_OK) return rc;
   if (hp[0] != 0)
     return gen_fail(MRD_EINVAL, "refine: " + std::to_string((unsigned long long)hp[0]) + " triangles of the input are clockwise, degenerate or name vertices out of range");
+  cudaMemsetAsync(cnt, 0, sizeof *cnt, s);
+  mrdgen::validate_sides_kernel<<<(unsigned)((nt + 255) / 256), 256, 0, s>>>(nt, ne, te_dev, et_dev, cnt);
+  mrdgen::validate_edges_kernel<<<(unsigned)((ne + 255) / 256), 256, 0, s>>>(ne, nt, tv_dev, te_dev, et_dev, cnt);
+  cudaMemcpyAsync((void *)hp, cnt, sizeof *cnt, cudaMemcpyDeviceToHost, s);
+  if ((rc = sync("refine: input check")) != MRD_OK) return rc;
+  if (hp[0] != 0)
+    return gen_fail(MRD_EINVAL, "refine: the edge tables do not describe a triangulation (" + std::to_string((unsigned long long)hp[0]) +
+                    " entries: triangleEdges and edgeTriangles disagree, or the two triangles of an edge lie on the same side of it)");
   for (int64_t it = 0;; ++it) {
     // 2.4.1: bad triangles and their circumcentres
     cudaMemsetAsync(cnt, 0, sizeof *cnt, s);

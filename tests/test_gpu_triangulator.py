@@ -162,6 +162,38 @@ def test_delaunay_flip_leaves_cocircular_points_alone_and_handles_degenerate_siz
     assert mrdb.meshgen_delaunay_flip(xy, tv, te, et)["flips"] == 0
 
 
+def test_overlapping_triangles_and_inconsistent_edge_tables_are_refused(mrdb):
+    """Input validation of the triangulator and the refinement: two counter-clockwise triangles on the SAME side of their shared
+    edge pass every local check (orientation, at most two triangles per edge) and still overlap -- flips on such an input
+    produce edges with three triangles (found by a soak run on library triangulations of clustered points, which drop
+    near-duplicate points); edge tables that belong to another numbering are refused as well."""
+    import torch
+    xy = dev(np.array([[0.0, 0.0], [1.0, 0.0], [0.5, 1.0], [0.5, 0.4]]), torch.float64)
+    tv = dev(np.array([[0, 1, 2], [0, 1, 3]]), torch.int32)
+    te, et = mrdb.meshgen_build_edges(tv)
+    with pytest.raises(mrdb.MrdError, match="same side"):
+        mrdb.meshgen_delaunay_flip(xy, tv, te, et)
+    with pytest.raises(mrdb.MrdError, match="same side"):
+        mrdb.meshgen_refine(xy, tv, te, et, 0.1, 1.5)
+    m = wl.scrambled_triangulation(6, 5, seed=3)
+    xy, tv = dev(m.xy, torch.float64), dev(m.tri, torch.int32)
+    te, et = mrdb.meshgen_build_edges(tv)
+    for k in range(3):
+        te2, et2 = te.clone(), et.clone()
+        if k == 0:
+            et2[[4, 9]] = et2[[9, 4]]                              # edgeTriangles of two edges exchanged
+        elif k == 1:
+            te2[7] = te2[7].roll(1)                                # a triangle's edges in the wrong local places
+        else:
+            inner = int((et[:, 1] >= 0).nonzero()[0])
+            et2[inner, 1] = et2[inner, 0]                          # an edge with the same triangle twice
+        with pytest.raises(mrdb.MrdError, match="do not describe a triangulation"):
+            mrdb.meshgen_delaunay_flip(xy, tv.clone(), te2, et2)
+        with pytest.raises(mrdb.MrdError, match="do not describe a triangulation"):
+            mrdb.meshgen_refine(xy, tv, te2, et2, 0.1, 1.5)
+    assert mrdb.meshgen_delaunay_flip(xy, tv, te, et)["flips"] > 0     # the unchanged tables are accepted
+
+
 def test_find_triangle_matches_the_oracle(mrdb):
     import torch
     m = wl.scrambled_triangulation(40, 31, seed=7)
