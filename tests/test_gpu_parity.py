@@ -484,3 +484,31 @@ def test_fp32_on_the_variable_valence_mesh(mrd, scheme):
     gm.step(10)
     om.step(10)
     assert field_errors(gm.get_state().cpu().numpy().astype(np.float64), om.get_state()) <= TOL_F32
+
+
+@pytest.mark.parametrize("n,free_rim", [(3, False), (5, True), (300, False), (2000, True), (20000, False)])
+@pytest.mark.parametrize("tile", [64, 256])
+def test_extreme_valence_a_fan_and_a_wheel(mrd, n, free_rim, tile):
+    """One vertex in every triangle of the mesh: a fan over a convex polygon (vertex 0, valence n - 2) and a wheel (a hub of
+    valence n) -- incidence lists far longer than a tile, tiles whose triangles all share a vertex, and meshes of one to three
+    triangles.  Five RK2 steps of scheme B against the oracle, rim frozen or free."""
+    import torch
+    from types import SimpleNamespace
+    rng = np.random.default_rng(n)
+    ang = np.sort(rng.random(n)) * 2 * np.pi if n > 5 else (np.arange(n) + 0.3) * 2 * np.pi / n
+    rim = np.stack([2.0 * np.cos(ang), np.sin(ang)], axis=1)
+    i = np.arange(n, dtype=np.int32)
+    fan = (rim, np.stack([np.zeros(n - 2, dtype=np.int32), i[1:-1], i[2:]], axis=1), np.ones(n, dtype=np.uint8))
+    wheel = (np.concatenate([rim, [[0.1, 0.05]]]), np.stack([np.full(n, n, dtype=np.int32), i, (i + 1) % n], axis=1),
+             np.concatenate([np.zeros(n, dtype=np.uint8) if free_rim else np.ones(n, dtype=np.uint8), [0]]))
+    for X, T, flag in (fan, wheel):
+        W = wl.random_smooth_state(SimpleNamespace(xy=X, nv=X.shape[0], lengths=(4.0, 2.0)), mach=0.5, seed=2)
+        gm = mrd.Mesh(X, T, vertex_flag=flag, scheme=mrd.SCHEME_B, time_order=2, tile=tile)
+        gm.set_state(torch.tensor(W, device="cuda"))
+        om = oracle.OracleMesh(X, T, vertex_flag=flag, scheme=oracle.SCHEME_B, time_order=2, threads=4)
+        om.set_state(W)
+        gm.step(5)
+        om.step(5)
+        Wg = gm.get_state().cpu().numpy()
+        assert field_errors(Wg, om.get_state()) <= 1e-10
+        assert np.array_equal(Wg[:, flag == 1], W[:, flag == 1])
