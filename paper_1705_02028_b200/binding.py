@@ -513,7 +513,9 @@ def meshgen_refine(xy, tv, te, et, R, B, seed=0, first_iteration=0, max_iteratio
                    stream=None):
     """Delaunay refinement (include/mrd.h: mrd_meshgen_refine) of the Delaunay triangulation (xy, tv, te, et) (CUDA tensors).
     Returns (xy, tv, te, et, info) as new tensors trimmed to the refined mesh; info: iterations, bad_left.  cap_vertex bounds
-    the refined mesh (default 8 x the input + 1024); MrdError(MRD_ENOMEM) when it does not suffice.  box = (x0, y0, x1, y1):
+    the refined mesh (default 8 x the input + 1024); MrdError(MRD_ENOMEM) when it does not suffice -- its attribute `partial` is
+    the valid, partly refined mesh (same tuple as the return value), to go on from with a larger cap_vertex (and, with box,
+    first_iteration = first_iteration + partial[4]["iterations"] for the same mesh as an uninterrupted run).  box = (x0, y0, x1, y1):
     renumber the vertices along the Morton curve of that rectangle after every insertion step.  size = (grid, rectangle): the
     size bound is R times the bilinear interpolant of grid (float64 CUDA tensor [ny][nx], > 0) over rectangle = (x0, y0, x1, y1)."""
     import torch
@@ -533,10 +535,16 @@ def meshgen_refine(xy, tv, te, et, R, B, seed=0, first_iteration=0, max_iteratio
         g = size[0]
         assert g.is_cuda and g.dtype == torch.float64 and g.is_contiguous() and g.ndim == 2
         sgrid, sbox, sny, snx = C.c_void_p(g.data_ptr()), (C.c_double * 4)(*[float(v) for v in size[1]]), g.shape[0], g.shape[1]
-    _check(lib().mrd_meshgen_refine(float(R), float(B), int(seed) & 0xFFFFFFFF, int(first_iteration), int(max_iterations), hbox,
-                                    sgrid, sbox, snx, sny, cv, ct, ce,
-                                    C.byref(n[0]), C.byref(n[1]), C.byref(n[2]), *[C.c_void_p(t.data_ptr()) for t in big],
-                                    C.byref(it), C.byref(left), _stream_ptr(stream)))
+    rc = lib().mrd_meshgen_refine(float(R), float(B), int(seed) & 0xFFFFFFFF, int(first_iteration), int(max_iterations), hbox,
+                                  sgrid, sbox, snx, sny, cv, ct, ce,
+                                  C.byref(n[0]), C.byref(n[1]), C.byref(n[2]), *[C.c_void_p(t.data_ptr()) for t in big],
+                                  C.byref(it), C.byref(left), _stream_ptr(stream))
+    if rc == MRD_ENOMEM:                              # the arrays hold a valid, partly refined Delaunay mesh: hand it to the caller
+        err = MrdError(rc, lib().mrd_last_error().decode())
+        out = [t[:k.value].clone() for t, k in zip(big, (n[0], n[1], n[1], n[2]))]
+        err.partial = (*out, dict(iterations=it.value, bad_left=left.value))
+        raise err
+    _check(rc)
     out = [t[:k.value].clone() for t, k in zip(big, (n[0], n[1], n[1], n[2]))]
     return (*out, dict(iterations=it.value, bad_left=left.value))
 

@@ -351,11 +351,28 @@ def test_domains_with_reentrant_corners_notches_and_holes(mrdb, domain, shape, L
 
 
 def test_capacity_and_bad_input_are_reported(mrdb):
+    import torch
     xy, tv, te, et = start(1, (6, 5))
     d = to_dev(xy, tv, te, et)
     with pytest.raises(mrdb.MrdError) as ex:
         mrdb.meshgen_refine(*d, 0.02, 1.0, cap_vertex=xy.shape[0] + 20)
     assert ex.value.code == mrdb.MRD_ENOMEM
+    # "the arrays then hold a valid Delaunay mesh, partly refined" (include/mrd.h): with a Morton box, going on from it with more room
+    # and the iteration count carried over gives the arrays of an uninterrupted run
+    box = (0.0, 0.0, 2.0, 1.5)
+    whole = mrdb.meshgen_refine(*d, 0.03, 1.2, seed=3, box=box, cap_vertex=20000)
+    with pytest.raises(mrdb.MrdError) as ex:
+        mrdb.meshgen_refine(*d, 0.03, 1.2, seed=3, box=box, cap_vertex=whole[0].shape[0] // 3)
+    part = ex.value.partial
+    assert ex.value.code == mrdb.MRD_ENOMEM and 0 < part[4]["iterations"] < whole[4]["iterations"] and part[4]["bad_left"] > 0
+    assert xy.shape[0] < part[0].shape[0] <= whole[0].shape[0] // 3
+    P, PT = part[0].cpu().numpy(), part[1].cpu().numpy()
+    pe, pet = mg.build_edges(PT)
+    assert np.array_equal(pe, part[2].cpu().numpy()) and np.array_equal(pet, part[3].cpu().numpy())
+    assert all(not mg.check_edge(P, PT, pe, pet, e) for e in range(pet.shape[0]))             # Delaunay
+    rest = mrdb.meshgen_refine(*part[:4], 0.03, 1.2, seed=3, box=box, first_iteration=part[4]["iterations"], cap_vertex=20000)
+    assert all(torch.equal(a, b) for a, b in zip(rest[:4], whole[:4]))
+    assert rest[4]["iterations"] + part[4]["iterations"] == whole[4]["iterations"] and rest[4]["bad_left"] == 0
     g = mrdb.meshgen_refine(*d, 0.5, 10.0)                         # nothing is bad: nothing happens
     assert g[4] == dict(iterations=0, bad_left=0) and same(g[:4], (xy, tv, te, et))
     g = mrdb.meshgen_refine(*d, 0.05, 1.0, max_iterations=2)       # stopped early: still a valid mesh, and says what is left
