@@ -144,6 +144,53 @@ def test_delaunay_flip_at_size_against_the_library_triangulation(mrdb):
         assert mg.incircle2d(*m.xy[q]) <= 0
 
 
+@pytest.mark.parametrize("dist,n", [("uniform", 20000), ("ring", 20000), ("aniso", 20000), ("cluster", 3000)])
+def test_delaunay_flip_on_scrambled_triangulations_of_random_point_sets(mrdb, dist, n):
+    """Point sets that are nothing like a grid: uniform, a thin ring (every point near one circle), anisotropic (10^5 : 1) and
+    clustered (distances from 1e-9 to 0.5).  A library triangulation of the points, scrambled by seeded flips of convex
+    quadrilaterals, goes back to a triangulation in which every interior edge passes the exact INCIRCLE2D with no zero -- the
+    unique Delaunay triangulation, whatever the library made of the same points (it is off by a few triangles on the last two)."""
+    import torch
+    from scipy.spatial import Delaunay
+    rng = np.random.default_rng(17)
+    P = rng.random((n, 2))
+    if dist == "ring":
+        a, r = rng.random(n) * 2 * np.pi, 1 + 1e-3 * rng.random(n)
+        P = np.stack([r * np.cos(a), r * np.sin(a)], axis=1)
+    elif dist == "aniso":
+        P = P * np.array([1000.0, 0.01])
+    elif dist == "cluster":
+        P = 0.5 + 0.2 * rng.standard_normal((n, 2)) * rng.random((n, 1)) ** 3
+    lib = Delaunay(P).simplices.astype(np.int64)
+    used = np.unique(lib)                                          # the library drops points it takes for duplicates
+    new = -np.ones(n, dtype=np.int64)
+    new[used] = np.arange(len(used))
+    P, lib = P[used], new[lib]
+    pl = P[lib]
+    cw = (pl[:, 1, 0] - pl[:, 0, 0]) * (pl[:, 2, 1] - pl[:, 0, 1]) - (pl[:, 1, 1] - pl[:, 0, 1]) * (pl[:, 2, 0] - pl[:, 0, 0]) < 0
+    lib[cw] = lib[cw][:, [0, 2, 1]]
+    m = wl.flip_edges(wl.UniformMesh(P, lib.astype(np.int32), (0.0, 0.0), None, None, None, (1.0, 1.0)), fraction=0.7, seed=3, rounds=3)
+    xy, tv = dev(P, torch.float64), dev(m.tri, torch.int32)
+    te, et = mrdb.meshgen_build_edges(tv)
+    try:
+        info = mrdb.meshgen_delaunay_flip(xy, tv, te, et)
+    except mrdb.MrdError as ex:                                    # a library result that is not a triangulation is refused, not flipped
+        assert dist == "cluster" and "do not describe a triangulation" in str(ex)
+        return
+    assert info["flips"] > 50                                      # (the scrambler only flips quadrilaterals that stay well-shaped: few on the ring)
+    gtv, gte, get = tv.cpu().numpy(), te.cpu().numpy(), et.cpu().numpy()
+    te2, et2 = mrdb.meshgen_build_edges(tv)                        # still a triangulation: the tables can be rebuilt, same edges
+    assert len(gtv) == len(lib) and et2.shape == et.shape and ccw_all(mrdb, P, gtv)
+    inner = np.nonzero(get[:, 1] >= 0)[0]
+    t1, t2 = get[inner, 0], get[inner, 1]
+    k2 = (gte[t2] == inner[:, None]).argmax(axis=1)
+    quads = np.concatenate([gtv[t1], gtv[t2, k2][:, None]], axis=1).astype(np.int32)
+    s, _ = mrdb.meshgen_incircle2d(xy, dev(quads, torch.int32))
+    assert (s < 0).all().item()
+    for q in quads[np.random.default_rng(0).choice(len(quads), 200, replace=False)]:
+        assert mg.incircle2d(*P[q]) < 0
+
+
 def test_delaunay_flip_leaves_cocircular_points_alone_and_handles_degenerate_sizes(mrdb):
     import torch
     m = wl.uniform_mesh(40, 30, 1.0, 1.0, periodic=False)          # INCIRCLE2D = 0 on every interior edge: all take the exact path
